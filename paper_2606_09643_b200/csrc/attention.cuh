@@ -1,0 +1,202 @@
+// Fused variable-length attention (S3d): softmax(q k^T / sqrt(d_h) + mask) v per request and head,
+// online softmax in fp32, GQA (query head g reads KV head g / (H_q/H_kv)), optional causal mask.
+// Reads q, k, v from the fused bf16 qkv buffer [N, (H_q + 2 H_kv) d_h] (task-sorted packed rows,
+// request p owns rows cu_tok[p] .. cu_tok[p+1]); writes bf16 [N, H_q d_h].
+//
+// Round-1 implementation: flash-style tiles (64 queries x 64 keys per step) on warp-level
+// mma.sync.m16n8k16 with cp.async double-buffered K/V.  Attention is 1-4 % of the forward's
+// FLOPs; the tcgen05 version is listed in DESIGN.md "next".
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "ptx.cuh"
+
+namespace fmx {
+
+struct AttnArgs {
+  const __nv_bfloat16 *qkv;
+  __nv_bfloat16 *out;
+  const int *cu_tok;
+  int ld_qkv, ld_out;
+  int n_q_heads, n_kv_heads;
+  int causal;
+  float scale_log2;      // log2(e) / sqrt(d_h)
+};
+
+__device__ __forceinline__ void cp_async_16(void *smem, const void *gmem, int src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(smem_u32(smem)), "l"(gmem), "r"(src_bytes)
+               : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
+__device__ __forceinline__ void ldmatrix_x4(uint32_t (&r)[4], const void *p) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];\n"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(smem_u32(p)));
+}
+__device__ __forceinline__ void ldmatrix_x2(uint32_t (&r)[2], const void *p) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x2.shared.b16 {%0,%1}, [%2];\n" : "=r"(r[0]), "=r"(r[1]) : "r"(smem_u32(p)));
+}
+__device__ __forceinline__ void ldmatrix_x2_trans(uint32_t (&r)[2], const void *p) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x2.trans.shared.b16 {%0,%1}, [%2];\n"
+               : "=r"(r[0]), "=r"(r[1]) : "r"(smem_u32(p)));
+}
+__device__ __forceinline__ void mma_bf16_16816(float (&c)[4], const uint32_t (&a)[4], const uint32_t (&b)[2]) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
+               : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+               : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
+}
+
+constexpr int kAttnBQ = 64, kAttnBKV = 64, kAttnThreads = 128;
+
+template <int DH>
+constexpr int attn_smem_bytes() { return (kAttnBQ + 4 * kAttnBKV) * (DH + 8) * 2; }
+
+// Copies rows [row0, row0+64) x DH bf16 of a strided global matrix into smem (stride DH+8); rows >= n_valid zero.
+template <int DH>
+__device__ __forceinline__ void load_tile_async(__nv_bfloat16 *s, const __nv_bfloat16 *g, int ld, int row0, int n_valid) {
+  constexpr int kChunks = DH / 8;                       // 16-byte chunks per row
+  for (int idx = threadIdx.x; idx < 64 * kChunks; idx += kAttnThreads) {
+    const int r = idx / kChunks, c = idx - r * kChunks;
+    const int row = row0 + r;
+    const bool ok = row < n_valid;
+    cp_async_16(s + r * (DH + 8) + c * 8, g + (size_t)(ok ? row : 0) * ld + c * 8, ok ? 16 : 0);
+  }
+}
+
+template <int DH>
+__global__ void __launch_bounds__(kAttnThreads) attention_kernel(const AttnArgs a) {
+  constexpr int LD = DH + 8;
+  extern __shared__ __align__(16) uint8_t attn_smem[];
+  __nv_bfloat16 *sQ = reinterpret_cast<__nv_bfloat16 *>(attn_smem);
+  __nv_bfloat16 *sK = sQ + kAttnBQ * LD;                // 2 stages
+  __nv_bfloat16 *sV = sK + 2 * kAttnBKV * LD;           // 2 stages
+
+  const int p = blockIdx.z, head = blockIdx.y, q0 = blockIdx.x * kAttnBQ;
+  const int r0 = a.cu_tok[p], n = a.cu_tok[p + 1] - r0;
+  if (q0 >= n) return;
+  const int kvh = head / (a.n_q_heads / a.n_kv_heads);
+  const __nv_bfloat16 *gq = a.qkv + (size_t)r0 * a.ld_qkv + head * DH;
+  const __nv_bfloat16 *gk = a.qkv + (size_t)r0 * a.ld_qkv + (a.n_q_heads + kvh) * DH;
+  const __nv_bfloat16 *gv = a.qkv + (size_t)r0 * a.ld_qkv + (a.n_q_heads + a.n_kv_heads + kvh) * DH;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+
+  const int kv_end = a.causal ? min(n, q0 + kAttnBQ) : n;   // keys beyond are masked for every query of the tile
+  const int n_kv_tiles = (kv_end + kAttnBKV - 1) / kAttnBKV;
+
+  load_tile_async<DH>(sQ, gq, a.ld_qkv, q0, n);
+  load_tile_async<DH>(sK, gk, a.ld_qkv, 0, n);
+  load_tile_async<DH>(sV, gv, a.ld_qkv, 0, n);
+  cp_async_commit();
+
+  uint32_t qf[DH / 16][4];
+  float o[DH / 8][4];
+#pragma unroll
+  for (int i = 0; i < DH / 8; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.0f;
+  float m_run[2] = {-1e30f, -1e30f}, l_run[2] = {0.0f, 0.0f};
+  const int qrow_a = q0 + warp * 16 + g, qrow_b = qrow_a + 8;   // position of this thread's two rows in the request
+
+  for (int j = 0; j < n_kv_tiles; ++j) {
+    const int st = j & 1;
+    if (j + 1 < n_kv_tiles) {
+      load_tile_async<DH>(sK + (st ^ 1) * kAttnBKV * LD, gk, a.ld_qkv, (j + 1) * kAttnBKV, n);
+      load_tile_async<DH>(sV + (st ^ 1) * kAttnBKV * LD, gv, a.ld_qkv, (j + 1) * kAttnBKV, n);
+      cp_async_commit();
+      cp_async_wait<1>();
+    } else {
+      cp_async_wait<0>();
+    }
+    __syncthreads();
+    if (j == 0) {
+#pragma unroll
+      for (int ks = 0; ks < DH / 16; ++ks)
+        ldmatrix_x4(qf[ks], sQ + (warp * 16 + (lane & 15)) * LD + ks * 16 + (lane >> 4) * 8);
+    }
+    const __nv_bfloat16 *k_s = sK + st * kAttnBKV * LD, *v_s = sV + st * kAttnBKV * LD;
+    // ---- S = Q K^T (16 x 64 per warp) ----
+    float s[8][4];
+#pragma unroll
+    for (int nt = 0; nt < 8; ++nt) {
+      s[nt][0] = s[nt][1] = s[nt][2] = s[nt][3] = 0.0f;
+#pragma unroll
+      for (int ks = 0; ks < DH / 16; ++ks) {
+        uint32_t b[2];
+        ldmatrix_x2(b, k_s + (nt * 8 + (lane & 7)) * LD + ks * 16 + ((lane >> 3) & 1) * 8);
+        mma_bf16_16816(s[nt], qf[ks], b);
+      }
+    }
+    // ---- scale, mask, online softmax ----
+    const int key0 = j * kAttnBKV;
+    float mx[2] = {-1e30f, -1e30f};
+#pragma unroll
+    for (int nt = 0; nt < 8; ++nt) {
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        const int key = key0 + nt * 8 + t * 2 + (e & 1);
+        const int qrow = (e < 2) ? qrow_a : qrow_b;
+        const bool masked = key >= n || (a.causal && key > qrow);
+        const float v = masked ? -1e30f : s[nt][e] * a.scale_log2;
+        s[nt][e] = v;
+        mx[e >> 1] = fmaxf(mx[e >> 1], v);
+      }
+    }
+    float corr[2];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      mx[h] = fmaxf(mx[h], __shfl_xor_sync(0xffffffffu, mx[h], 1));
+      mx[h] = fmaxf(mx[h], __shfl_xor_sync(0xffffffffu, mx[h], 2));
+      const float m_new = fmaxf(m_run[h], mx[h]);
+      corr[h] = exp2f(m_run[h] - m_new);
+      m_run[h] = m_new;
+    }
+    float rs[2] = {0.0f, 0.0f};
+#pragma unroll
+    for (int nt = 0; nt < 8; ++nt) {
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        const float pv = exp2f(s[nt][e] - m_run[e >> 1]);
+        s[nt][e] = pv;
+        rs[e >> 1] += pv;
+      }
+    }
+#pragma unroll
+    for (int h = 0; h < 2; ++h) l_run[h] = l_run[h] * corr[h] + rs[h];
+#pragma unroll
+    for (int i = 0; i < DH / 8; ++i) { o[i][0] *= corr[0]; o[i][1] *= corr[0]; o[i][2] *= corr[1]; o[i][3] *= corr[1]; }
+    // ---- O += P V ----
+#pragma unroll
+    for (int kk = 0; kk < 4; ++kk) {
+      uint32_t pa[4];
+      pa[0] = pack_bf16(s[2 * kk][0], s[2 * kk][1]);
+      pa[1] = pack_bf16(s[2 * kk][2], s[2 * kk][3]);
+      pa[2] = pack_bf16(s[2 * kk + 1][0], s[2 * kk + 1][1]);
+      pa[3] = pack_bf16(s[2 * kk + 1][2], s[2 * kk + 1][3]);
+#pragma unroll
+      for (int dt = 0; dt < DH / 8; ++dt) {
+        uint32_t b[2];
+        ldmatrix_x2_trans(b, v_s + (kk * 16 + (lane & 15)) * LD + dt * 8);
+        mma_bf16_16816(o[dt], pa, b);
+      }
+    }
+    __syncthreads();      // all warps done with stage st before it is refilled
+  }
+  // ---- normalise and store ----
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    l_run[h] += __shfl_xor_sync(0xffffffffu, l_run[h], 1);
+    l_run[h] += __shfl_xor_sync(0xffffffffu, l_run[h], 2);
+  }
+  const float inv_a = 1.0f / l_run[0], inv_b = 1.0f / l_run[1];
+  __nv_bfloat16 *out = a.out + (size_t)r0 * a.ld_out + head * DH;
+#pragma unroll
+  for (int dt = 0; dt < DH / 8; ++dt) {
+    const int col = dt * 8 + t * 2;
+    if (qrow_a < n) *reinterpret_cast<uint32_t *>(out + (size_t)qrow_a * a.ld_out + col) = pack_bf16(o[dt][0] * inv_a, o[dt][1] * inv_a);
+    if (qrow_b < n) *reinterpret_cast<uint32_t *>(out + (size_t)qrow_b * a.ld_out + col) = pack_bf16(o[dt][2] * inv_b, o[dt][3] * inv_b);
+  }
+}
+
+}  // namespace fmx

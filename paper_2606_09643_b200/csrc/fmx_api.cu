@@ -1,0 +1,970 @@
+// libfmx host runtime: context, backbone/task registry, LoRA slab arena, workspace carving and
+// the launch sequence of fmx_forward_mixed.  All compute runs in the kernels of
+// gemm.cuh / attention.cuh / kernels.cuh; there is no CPU fallback.
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <memory>
+#include <mutex>
+#include <vector>
+
+#include "attention.cuh"
+#include "common.h"
+#include "fmx.h"
+#include "gemm.cuh"
+#include "kernels.cuh"
+
+using namespace fmx;
+typedef __nv_bfloat16 bf16;
+
+#define CU_OK(expr)                                                                                   \
+  do {                                                                                                \
+    cudaError_t _e = (expr);                                                                          \
+    if (_e != cudaSuccess)                                                                            \
+      return fmx_fail(FMX_E_CUDA, "%s failed: %s (%d) at %s:%d", #expr, cudaGetErrorString(_e), (int)_e, __FILE__, __LINE__); \
+  } while (0)
+
+namespace {
+
+enum Family { F_SORT = 0, F_EMBED, F_NORM, F_SHRINK, F_GEMM_QKV, F_ATTN, F_GEMM_O, F_GEMM_FFN_IN, F_GEMM_FFN_OUT,
+              F_ROPE, F_POOL, F_HEAD };
+const char *kFamilyNames[FMX_N_FAMILIES] = {"task_sort", "embed", "norm", "lora_shrink", "gemm_qkv", "attention",
+                                            "gemm_o", "gemm_ffn_in", "gemm_ffn_out", "rope", "final_pool", "head"};
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct TaskRec {
+  bool live = false;
+  int bb = -1;
+  int coff = 0, rpad = 0;                 // slab columns [coff, coff + rpad)
+  unsigned char trpad[7] = {0};
+  float scale[7] = {0};
+  int head_kind = 0, head_out = 0;
+  bf16 *head_W = nullptr, *head_b = nullptr;   // library-owned copies
+};
+
+struct Backbone {
+  fmx_backbone_desc d;
+  // deep copies of the caller's per-layer pointer arrays
+  std::vector<const void *> norm1_g, norm1_b, Wq, Wk, Wv, Wo, bq, bk, bv, bo, norm2_g, norm2_b, Wup, Wgate, Wdown, bup, bgate, bdown;
+  int d_q = 0, d_kv = 0, d_qkv = 0;
+  int Kp = 0;                              // padded patch_dim
+  bf16 *embed_Wpad = nullptr;              // [d, Kp]
+  float *posb = nullptr;                   // [n_pos, d]
+  float2 *rope_cs = nullptr;               // [max_seq, dh/2]
+  std::vector<CUtensorMap> mWq, mWk, mWv, mWo, mWup, mWgate, mWdown;
+  CUtensorMap mEmbedW;
+  // LoRA slabs
+  int Rcap = 0;
+  std::vector<unsigned char> col_used;     // units of 16 columns
+  bf16 *slabA[7] = {nullptr};              // per target: [L][Rcap, d_in]
+  bf16 *slabB[7] = {nullptr};              // per target: [L][d_out, Rcap]
+  std::vector<CUtensorMap> mA[7], mB[7];   // per target, per layer
+  int n_adapters[7] = {0};                 // live adapters per target
+  int din[7], dout[7];
+};
+
+struct ProfEvent { int family; cudaEvent_t e0, e1; };
+
+}  // namespace
+
+struct fmx_ctx {
+  int device = 0, sm_count = 0;
+  EncodeTiledFn encode = nullptr;
+  std::vector<std::unique_ptr<Backbone>> bbs;
+  std::vector<TaskRec> tasks;              // slot = task id
+  int n_slots = 0;
+  // device task tables (FMX_MAX_TASKS entries)
+  int *d_task_coff = nullptr, *d_task_head_kind = nullptr, *d_task_head_out = nullptr;
+  unsigned char *d_task_trpad = nullptr;
+  float *d_task_scale = nullptr;
+  const bf16 **d_task_head_W = nullptr, **d_task_head_b = nullptr;
+  // pinned staging for ids / lengths
+  int *h_stage = nullptr;
+  // host-buffer forward staging
+  void *d_in_stage = nullptr; size_t in_stage_bytes = 0;
+  float *d_out_stage = nullptr; size_t out_stage_bytes = 0;
+  // last forward (debug)
+  SegTables last_t{};
+  int last_B = 0, last_T = 0, last_n_tiles = 0, last_launches = 0;
+  cudaStream_t last_stream = nullptr;
+  void *last_buf[7] = {nullptr}; size_t last_buf_bytes[7] = {0};
+  // profiling
+  bool prof_on = false;
+  std::vector<ProfEvent> prof;
+  std::mutex mu;
+};
+
+namespace {
+
+int encode_2d(fmx_ctx *c, CUtensorMap *m, const void *base, uint64_t rows, uint64_t cols, uint64_t ld_elems,
+              uint32_t box_rows) {
+  cuuint64_t dims[2] = {cols, rows};
+  cuuint64_t strides[1] = {ld_elems * 2};
+  cuuint32_t box[2] = {64, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  if ((reinterpret_cast<uintptr_t>(base) & 15) || (strides[0] & 15))
+    return fmx_fail(FMX_E_INVALID_ARG, "tensor map: base %p / row stride %llu B not 16-byte aligned", base,
+                    (unsigned long long)strides[0]);
+  CUresult r = c->encode(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), dims, strides, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fmx_fail(FMX_E_CUDA, "cuTensorMapEncodeTiled failed (%d) rows=%llu cols=%llu ld=%llu", (int)r,
+                                         (unsigned long long)rows, (unsigned long long)cols, (unsigned long long)ld_elems);
+  return FMX_OK;
+}
+
+void target_dims(const fmx_backbone_desc &d, int tg, int &din, int &dout) {
+  const int dq = d.n_q_heads * d.head_dim, dkv = d.n_kv_heads * d.head_dim;
+  switch (tg) {
+    case FMX_TGT_Q: din = d.d_model; dout = dq; break;
+    case FMX_TGT_K: case FMX_TGT_V: din = d.d_model; dout = dkv; break;
+    case FMX_TGT_O: din = dq; dout = d.d_model; break;
+    case FMX_TGT_GATE: case FMX_TGT_UP: din = d.d_model; dout = d.d_ffn; break;
+    default: din = d.d_ffn; dout = d.d_model; break;
+  }
+}
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// ---------------------------------------------------------------- workspace layout
+struct Workspace {
+  SegTables t{};
+  float *X = nullptr, *feat = nullptr;
+  bf16 *Xn = nullptr, *QKV = nullptr, *AttnO = nullptr, *Hid = nullptr, *U = nullptr;
+  int n_tiles = 0, n_blk_cap = 0;
+  size_t bytes = 0;
+};
+
+Workspace carve(const Backbone &bb, void *base, int B, long long N, int T) {
+  Workspace w;
+  uint8_t *p = static_cast<uint8_t *>(base);
+  size_t off = 0;
+  auto take = [&](size_t bytes) { void *r = p ? p + off : nullptr; off = align_up(off + bytes, 1024); return r; };
+  w.n_tiles = (int)((N + 127) / 128);
+  w.n_blk_cap = w.n_tiles + std::min(T, B);
+  const fmx_backbone_desc &d = bb.d;
+  w.t.task_ids = (int *)take(sizeof(int) * B);
+  w.t.lengths = (int *)take(sizeof(int) * B);
+  w.t.perm = (int *)take(sizeof(int) * B);
+  w.t.inv_perm = (int *)take(sizeof(int) * B);
+  w.t.task_sorted = (int *)take(sizeof(int) * B);
+  w.t.task_req_off = (int *)take(sizeof(int) * (T + 1));
+  w.t.task_tok_off = (int *)take(sizeof(int) * (T + 1));
+  w.t.cu_tok = (int *)take(sizeof(int) * (B + 1));
+  w.t.in_off = (long long *)take(sizeof(long long) * (B + 1));
+  w.t.out_off = (long long *)take(sizeof(long long) * (B + 1));
+  w.t.tile_blk_off = (int *)take(sizeof(int) * (w.n_tiles + 1));
+  w.t.blk_tile = (int *)take(sizeof(int) * w.n_blk_cap);
+  w.t.blk_task = (int *)take(sizeof(int) * w.n_blk_cap);
+  w.t.blk_lo = (int *)take(sizeof(int) * w.n_blk_cap);
+  w.t.blk_hi = (int *)take(sizeof(int) * w.n_blk_cap);
+  w.t.n_blk = (int *)take(sizeof(int));
+  w.t.row_req = (int *)take(sizeof(int) * N);
+  w.t.row_pos = (int *)take(sizeof(int) * N);
+  w.X = (float *)take(sizeof(float) * N * d.d_model);
+  w.Xn = (bf16 *)take(sizeof(bf16) * N * d.d_model);
+  w.QKV = (bf16 *)take(sizeof(bf16) * N * bb.d_qkv);
+  w.AttnO = (bf16 *)take(sizeof(bf16) * N * bb.d_q);
+  w.Hid = (bf16 *)take(sizeof(bf16) * N * std::max(d.d_ffn, bb.Kp));     // also the patch-pack buffer
+  w.U = (bf16 *)take(sizeof(bf16) * (size_t)w.n_blk_cap * 128 * 192);
+  w.feat = (float *)take(sizeof(float) * (size_t)B * d.d_model);
+  w.bytes = off;
+  return w;
+}
+
+// ---------------------------------------------------------------- launch bookkeeping
+struct Launcher {
+  fmx_ctx *c;
+  cudaStream_t s;
+  int count = 0;
+  cudaEvent_t pending = nullptr;
+  int begin(int family) {
+    ++count;
+    if (c->prof_on) {
+      ProfEvent pe{family, nullptr, nullptr};
+      CU_OK(cudaEventCreate(&pe.e0));
+      CU_OK(cudaEventCreate(&pe.e1));
+      CU_OK(cudaEventRecord(pe.e0, s));
+      c->prof.push_back(pe);
+    }
+    return FMX_OK;
+  }
+  int end() {
+    CU_OK(cudaGetLastError());
+    if (c->prof_on) CU_OK(cudaEventRecord(c->prof.back().e1, s));
+    return FMX_OK;
+  }
+};
+#define LAUNCH(L, family, ...)                    \
+  do {                                            \
+    if (int _e = (L).begin(family)) return _e;    \
+    __VA_ARGS__;                                  \
+    if (int _e = (L).end()) return _e;            \
+  } while (0)
+
+template <int kVec>
+void launch_norm(cudaStream_t s, const float *X, bf16 *Y, const bf16 *g, const bf16 *b, int N, float eps, int rms) {
+  norm_kernel<kVec><<<(N + 7) / 8, 256, 0, s>>>(X, Y, g, b, N, eps, rms);
+}
+bool dispatch_norm(cudaStream_t s, int d, const float *X, bf16 *Y, const bf16 *g, const bf16 *b, int N, float eps, int rms) {
+  switch (d / 128) {
+    case 1: launch_norm<1>(s, X, Y, g, b, N, eps, rms); return true;
+    case 2: launch_norm<2>(s, X, Y, g, b, N, eps, rms); return true;
+    case 4: launch_norm<4>(s, X, Y, g, b, N, eps, rms); return true;
+    case 6: launch_norm<6>(s, X, Y, g, b, N, eps, rms); return true;
+    case 8: launch_norm<8>(s, X, Y, g, b, N, eps, rms); return true;
+    case 12: launch_norm<12>(s, X, Y, g, b, N, eps, rms); return true;
+    case 16: launch_norm<16>(s, X, Y, g, b, N, eps, rms); return true;
+  }
+  return false;
+}
+bool dispatch_pool(cudaStream_t s, int d, int B, const PoolArgs &a) {
+  switch (d / 128) {
+    case 1: final_pool_kernel<1><<<B, 128, 0, s>>>(a); return true;
+    case 2: final_pool_kernel<2><<<B, 128, 0, s>>>(a); return true;
+    case 4: final_pool_kernel<4><<<B, 128, 0, s>>>(a); return true;
+    case 6: final_pool_kernel<6><<<B, 128, 0, s>>>(a); return true;
+    case 8: final_pool_kernel<8><<<B, 128, 0, s>>>(a); return true;
+    case 12: final_pool_kernel<12><<<B, 128, 0, s>>>(a); return true;
+    case 16: final_pool_kernel<16><<<B, 128, 0, s>>>(a); return true;
+  }
+  return false;
+}
+bool norm_dim_supported(int d) {
+  const int v = d / 128;
+  return d % 128 == 0 && (v == 1 || v == 2 || v == 4 || v == 6 || v == 8 || v == 12 || v == 16);
+}
+
+void launch_gemm(fmx_ctx *c, cudaStream_t s, const GemmParams &p) {
+  if (p.mode == GM_SHRINK) {
+    const int grid = c->sm_count;
+    gemm_kernel<128, gemm_stages<128, true>(), true><<<grid, kGemmThreads, gemm_smem_bytes<128, true>(), s>>>(p);
+  } else if (p.n_chunks % 2 == 0) {
+    const int tiles = p.n_mtiles * (p.n_chunks / 2);
+    gemm_kernel<256, gemm_stages<256, false>(), false><<<std::min(tiles, c->sm_count), kGemmThreads, gemm_smem_bytes<256, false>(), s>>>(p);
+  } else {
+    const int tiles = p.n_mtiles * p.n_chunks;
+    gemm_kernel<128, gemm_stages<128, false>(), false><<<std::min(tiles, c->sm_count), kGemmThreads, gemm_smem_bytes<128, false>(), s>>>(p);
+  }
+}
+
+void launch_attention(cudaStream_t s, int dh, dim3 grid, const AttnArgs &a) {
+  if (dh == 32) attention_kernel<32><<<grid, kAttnThreads, attn_smem_bytes<32>(), s>>>(a);
+  else if (dh == 64) attention_kernel<64><<<grid, kAttnThreads, attn_smem_bytes<64>(), s>>>(a);
+  else attention_kernel<128><<<grid, kAttnThreads, attn_smem_bytes<128>(), s>>>(a);
+}
+
+int set_kernel_attrs() {
+  CU_OK(cudaFuncSetAttribute(gemm_kernel<256, gemm_stages<256, false>(), false>, cudaFuncAttributeMaxDynamicSharedMemorySize, gemm_smem_bytes<256, false>()));
+  CU_OK(cudaFuncSetAttribute(gemm_kernel<128, gemm_stages<128, false>(), false>, cudaFuncAttributeMaxDynamicSharedMemorySize, gemm_smem_bytes<128, false>()));
+  CU_OK(cudaFuncSetAttribute(gemm_kernel<128, gemm_stages<128, true>(), true>, cudaFuncAttributeMaxDynamicSharedMemorySize, gemm_smem_bytes<128, true>()));
+  CU_OK(cudaFuncSetAttribute(attention_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_smem_bytes<32>()));
+  CU_OK(cudaFuncSetAttribute(attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_smem_bytes<64>()));
+  CU_OK(cudaFuncSetAttribute(attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_smem_bytes<128>()));
+  return FMX_OK;
+}
+
+std::vector<const void *> copy_ptrs(const void *const *arr, int n) {
+  std::vector<const void *> v(n, nullptr);
+  if (arr) for (int i = 0; i < n; ++i) v[i] = arr[i];
+  return v;
+}
+
+// ---------------------------------------------------------------- LoRA slab arena
+int rebuild_slab_maps(fmx_ctx *c, Backbone &bb, int tg) {
+  const int L = bb.d.n_layers;
+  bb.mA[tg].resize(L);
+  bb.mB[tg].resize(L);
+  for (int l = 0; l < L; ++l) {
+    bf16 *A = bb.slabA[tg] + (size_t)l * bb.Rcap * bb.din[tg];
+    bf16 *B = bb.slabB[tg] + (size_t)l * bb.dout[tg] * bb.Rcap;
+    if (int e = encode_2d(c, &bb.mA[tg][l], A, bb.Rcap, bb.din[tg], bb.din[tg], 64)) return e;
+    if (int e = encode_2d(c, &bb.mB[tg][l], B, bb.dout[tg], bb.Rcap, bb.Rcap, 128)) return e;
+  }
+  return FMX_OK;
+}
+
+int alloc_slab(fmx_ctx *c, Backbone &bb, int tg) {
+  const size_t L = bb.d.n_layers;
+  const size_t na = L * bb.Rcap * bb.din[tg], nb = L * bb.dout[tg] * bb.Rcap;
+  CU_OK(cudaMalloc(&bb.slabA[tg], na * sizeof(bf16)));
+  CU_OK(cudaMalloc(&bb.slabB[tg], nb * sizeof(bf16)));
+  CU_OK(cudaMemset(bb.slabA[tg], 0, na * sizeof(bf16)));
+  CU_OK(cudaMemset(bb.slabB[tg], 0, nb * sizeof(bf16)));
+  return rebuild_slab_maps(c, bb, tg);
+}
+
+int grow_slabs(fmx_ctx *c, Backbone &bb, int new_cap) {
+  const size_t L = bb.d.n_layers;
+  const int old = bb.Rcap;
+  for (int tg = 0; tg < 7; ++tg) {
+    if (!bb.slabA[tg]) continue;
+    bf16 *nA = nullptr, *nB = nullptr;
+    const size_t na = L * new_cap * bb.din[tg], nb = L * bb.dout[tg] * (size_t)new_cap;
+    CU_OK(cudaMalloc(&nA, na * sizeof(bf16)));
+    CU_OK(cudaMalloc(&nB, nb * sizeof(bf16)));
+    CU_OK(cudaMemset(nA, 0, na * sizeof(bf16)));
+    CU_OK(cudaMemset(nB, 0, nb * sizeof(bf16)));
+    for (size_t l = 0; l < L; ++l)
+      CU_OK(cudaMemcpy(nA + l * new_cap * bb.din[tg], bb.slabA[tg] + l * old * bb.din[tg], (size_t)old * bb.din[tg] * sizeof(bf16),
+                       cudaMemcpyDeviceToDevice));
+    CU_OK(cudaMemcpy2D(nB, (size_t)new_cap * sizeof(bf16), bb.slabB[tg], (size_t)old * sizeof(bf16), (size_t)old * sizeof(bf16),
+                       L * bb.dout[tg], cudaMemcpyDeviceToDevice));
+    cudaFree(bb.slabA[tg]);
+    cudaFree(bb.slabB[tg]);
+    bb.slabA[tg] = nA;
+    bb.slabB[tg] = nB;
+  }
+  bb.Rcap = new_cap;
+  bb.col_used.resize(new_cap / 16, 0);
+  for (int tg = 0; tg < 7; ++tg)
+    if (bb.slabA[tg]) if (int e = rebuild_slab_maps(c, bb, tg)) return e;
+  return FMX_OK;
+}
+
+int find_columns(const Backbone &bb, int units) {        // first fit, units of 16 columns
+  const int n = (int)bb.col_used.size();
+  for (int i = 0; i + units <= n; ++i) {
+    int j = 0;
+    while (j < units && !bb.col_used[i + j]) ++j;
+    if (j == units) return i;
+    i += j;
+  }
+  return -1;
+}
+
+int upload_task_tables(fmx_ctx *c, int t) {
+  const TaskRec &r = c->tasks[t];
+  CU_OK(cudaMemcpy(c->d_task_coff + t, &r.coff, sizeof(int), cudaMemcpyHostToDevice));
+  CU_OK(cudaMemcpy(c->d_task_trpad + t * 7, r.trpad, 7, cudaMemcpyHostToDevice));
+  CU_OK(cudaMemcpy(c->d_task_scale + t * 7, r.scale, 7 * sizeof(float), cudaMemcpyHostToDevice));
+  CU_OK(cudaMemcpy(c->d_task_head_kind + t, &r.head_kind, sizeof(int), cudaMemcpyHostToDevice));
+  CU_OK(cudaMemcpy(c->d_task_head_out + t, &r.head_out, sizeof(int), cudaMemcpyHostToDevice));
+  const bf16 *w = r.head_W, *b = r.head_b;
+  CU_OK(cudaMemcpy(c->d_task_head_W + t, &w, sizeof(void *), cudaMemcpyHostToDevice));
+  CU_OK(cudaMemcpy(c->d_task_head_b + t, &b, sizeof(void *), cudaMemcpyHostToDevice));
+  return FMX_OK;
+}
+
+Backbone *get_bb(fmx_ctx *c, fmx_backbone_t h) {
+  if (h < 0 || h >= (int)c->bbs.size() || !c->bbs[h]) return nullptr;
+  return c->bbs[h].get();
+}
+
+}  // namespace
+
+// =====================================================================================
+extern "C" {
+
+int fmx_create(fmx_ctx **out, int device_ordinal) {
+  if (!out) return fmx_fail(FMX_E_INVALID_ARG, "fmx_create: out is NULL");
+  *out = nullptr;
+  int n_dev = 0;
+  cudaError_t e = cudaGetDeviceCount(&n_dev);
+  if (e != cudaSuccess || n_dev == 0)
+    return fmx_fail(FMX_E_CUDA, "fmx_create: no CUDA device (%s); libfmx has no CPU fallback", cudaGetErrorString(e));
+  if (device_ordinal < 0 || device_ordinal >= n_dev) return fmx_fail(FMX_E_INVALID_ARG, "fmx_create: device %d of %d", device_ordinal, n_dev);
+  CU_OK(cudaSetDevice(device_ordinal));
+  cudaDeviceProp prop;
+  CU_OK(cudaGetDeviceProperties(&prop, device_ordinal));
+  if (prop.major != 10) return fmx_fail(FMX_E_CUDA, "fmx_create: device is sm_%d%d; libfmx is built for sm_100a only", prop.major, prop.minor);
+  std::unique_ptr<fmx_ctx> c(new fmx_ctx());
+  c->device = device_ordinal;
+  c->sm_count = prop.multiProcessorCount;
+  void *fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  CU_OK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+  if (!fn || qres != cudaDriverEntryPointSuccess) return fmx_fail(FMX_E_CUDA, "fmx_create: cuTensorMapEncodeTiled not available");
+  c->encode = reinterpret_cast<EncodeTiledFn>(fn);
+  if (int err = set_kernel_attrs()) return err;
+  c->tasks.resize(FMX_MAX_TASKS);
+  CU_OK(cudaMalloc(&c->d_task_coff, sizeof(int) * FMX_MAX_TASKS));
+  CU_OK(cudaMalloc(&c->d_task_head_kind, sizeof(int) * FMX_MAX_TASKS));
+  CU_OK(cudaMalloc(&c->d_task_head_out, sizeof(int) * FMX_MAX_TASKS));
+  CU_OK(cudaMalloc(&c->d_task_trpad, 7 * FMX_MAX_TASKS));
+  CU_OK(cudaMalloc(&c->d_task_scale, sizeof(float) * 7 * FMX_MAX_TASKS));
+  CU_OK(cudaMalloc(&c->d_task_head_W, sizeof(void *) * FMX_MAX_TASKS));
+  CU_OK(cudaMalloc(&c->d_task_head_b, sizeof(void *) * FMX_MAX_TASKS));
+  CU_OK(cudaMemset(c->d_task_coff, 0, sizeof(int) * FMX_MAX_TASKS));
+  CU_OK(cudaMemset(c->d_task_head_kind, 0, sizeof(int) * FMX_MAX_TASKS));
+  CU_OK(cudaMemset(c->d_task_head_out, 0, sizeof(int) * FMX_MAX_TASKS));
+  CU_OK(cudaMemset(c->d_task_trpad, 0, 7 * FMX_MAX_TASKS));
+  CU_OK(cudaMemset(c->d_task_scale, 0, sizeof(float) * 7 * FMX_MAX_TASKS));
+  CU_OK(cudaMemset(c->d_task_head_W, 0, sizeof(void *) * FMX_MAX_TASKS));
+  CU_OK(cudaMemset(c->d_task_head_b, 0, sizeof(void *) * FMX_MAX_TASKS));
+  CU_OK(cudaMallocHost(&c->h_stage, sizeof(int) * 2 * FMX_MAX_REQUESTS));
+  *out = c.release();
+  fmx_clear_error();
+  return FMX_OK;
+}
+
+int fmx_destroy(fmx_ctx *c) {
+  if (!c) return FMX_OK;
+  cudaSetDevice(c->device);
+  cudaDeviceSynchronize();
+  for (auto &pe : c->prof) { cudaEventDestroy(pe.e0); cudaEventDestroy(pe.e1); }
+  for (auto &bp : c->bbs) {
+    if (!bp) continue;
+    cudaFree(bp->embed_Wpad); cudaFree(bp->posb); cudaFree(bp->rope_cs);
+    for (int tg = 0; tg < 7; ++tg) { cudaFree(bp->slabA[tg]); cudaFree(bp->slabB[tg]); }
+  }
+  for (auto &t : c->tasks) { cudaFree(t.head_W); cudaFree(t.head_b); }
+  cudaFree(c->d_task_coff); cudaFree(c->d_task_head_kind); cudaFree(c->d_task_head_out); cudaFree(c->d_task_trpad);
+  cudaFree(c->d_task_scale); cudaFree(c->d_task_head_W); cudaFree(c->d_task_head_b);
+  cudaFree(c->d_in_stage); cudaFree(c->d_out_stage);
+  cudaFreeHost(c->h_stage);
+  delete c;
+  return FMX_OK;
+}
+
+int fmx_task_slots(fmx_ctx *c) { return c ? c->n_slots : 0; }
+
+int fmx_register_backbone(fmx_ctx *c, const fmx_backbone_desc *desc, fmx_backbone_t *out) {
+  if (!c || !desc || !out) return fmx_fail(FMX_E_INVALID_ARG, "register_backbone: NULL argument");
+  std::lock_guard<std::mutex> lk(c->mu);
+  CU_OK(cudaSetDevice(c->device));
+  const fmx_backbone_desc &d = *desc;
+  if (d.n_layers < 1 || d.d_model < 128 || d.n_q_heads < 1 || d.n_kv_heads < 1 || d.d_ffn < 128 || d.max_seq < 1)
+    return fmx_fail(FMX_E_INVALID_ARG, "register_backbone: non-positive dimension");
+  const int dq = d.n_q_heads * d.head_dim, dkv = d.n_kv_heads * d.head_dim;
+  if (!norm_dim_supported(d.d_model) || dq % 128 || dkv % 128 || d.d_ffn % 128 || d.n_q_heads % d.n_kv_heads ||
+      !(d.head_dim == 32 || d.head_dim == 64 || d.head_dim == 128))
+    return fmx_fail(FMX_E_SHAPE, "register_backbone: unsupported dims (d_model=%d d_q=%d d_kv=%d d_ffn=%d head_dim=%d)", d.d_model, dq, dkv, d.d_ffn, d.head_dim);
+  if (d.act < 0 || d.act > 2 || d.norm < 0 || d.norm > 1 || d.input_kind < 0 || d.input_kind > 2)
+    return fmx_fail(FMX_E_INVALID_ARG, "register_backbone: bad enum");
+  if (d.tokens_per_request < 0 || d.tokens_per_request > d.max_seq) return fmx_fail(FMX_E_INVALID_ARG, "register_backbone: tokens_per_request > max_seq");
+  if (!d.norm1_g || !d.norm2_g || !d.Wq || !d.Wk || !d.Wv || !d.Wo || !d.Wup || !d.Wdown || !d.final_g ||
+      (d.act == FMX_ACT_SWIGLU && !d.Wgate))
+    return fmx_fail(FMX_E_INVALID_ARG, "register_backbone: missing weight array");
+  if (d.norm == FMX_NORM_LAYERNORM && (!d.norm1_b || !d.norm2_b || !d.final_b)) return fmx_fail(FMX_E_INVALID_ARG, "register_backbone: LayerNorm needs *_b");
+  if (d.input_kind == FMX_INPUT_PATCH_LINEAR) {
+    if (!d.embed_W || d.patch_dim < 1 || d.tokens_per_request < 1) return fmx_fail(FMX_E_INVALID_ARG, "register_backbone: PATCH_LINEAR needs embed_W, patch_dim, tokens_per_request");
+    if (d.has_cls && !d.embed_cls) return fmx_fail(FMX_E_INVALID_ARG, "register_backbone: has_cls needs embed_cls");
+    if (d.img_c) {
+      const int g = d.patch_hw > 0 ? d.img_hw / d.patch_hw : 0;
+      if (d.patch_hw < 1 || d.img_hw % d.patch_hw || d.img_c * d.patch_hw * d.patch_hw != d.patch_dim ||
+          g * g != d.tokens_per_request - (d.has_cls ? 1 : 0))
+        return fmx_fail(FMX_E_SHAPE, "register_backbone: image geometry inconsistent with patch_dim / tokens_per_request");
+    }
+  }
+  if (d.input_kind == FMX_INPUT_TOKEN_IDS && (!d.embed_table || d.vocab < 1)) return fmx_fail(FMX_E_INVALID_ARG, "register_backbone: TOKEN_IDS needs embed_table, vocab");
+  if (d.rope_theta > 0 && d.head_dim % 2) return fmx_fail(FMX_E_SHAPE, "register_backbone: RoPE needs even head_dim");
+
+  std::unique_ptr<Backbone> b(new Backbone());
+  b->d = d;
+  const int L = d.n_layers;
+  b->norm1_g = copy_ptrs(d.norm1_g, L); b->norm1_b = copy_ptrs(d.norm1_b, L);
+  b->norm2_g = copy_ptrs(d.norm2_g, L); b->norm2_b = copy_ptrs(d.norm2_b, L);
+  b->Wq = copy_ptrs(d.Wq, L); b->Wk = copy_ptrs(d.Wk, L); b->Wv = copy_ptrs(d.Wv, L); b->Wo = copy_ptrs(d.Wo, L);
+  b->bq = copy_ptrs(d.bq, L); b->bk = copy_ptrs(d.bk, L); b->bv = copy_ptrs(d.bv, L); b->bo = copy_ptrs(d.bo, L);
+  b->Wup = copy_ptrs(d.Wup, L); b->Wgate = copy_ptrs(d.Wgate, L); b->Wdown = copy_ptrs(d.Wdown, L);
+  b->bup = copy_ptrs(d.bup, L); b->bgate = copy_ptrs(d.bgate, L); b->bdown = copy_ptrs(d.bdown, L);
+  b->d_q = dq; b->d_kv = dkv; b->d_qkv = dq + 2 * dkv;
+  for (int tg = 0; tg < 7; ++tg) target_dims(d, tg, b->din[tg], b->dout[tg]);
+  for (int l = 0; l < L; ++l) {
+    if (!b->norm1_g[l] || !b->norm2_g[l] || !b->Wq[l] || !b->Wk[l] || !b->Wv[l] || !b->Wo[l] || !b->Wup[l] || !b->Wdown[l] ||
+        (d.act == FMX_ACT_SWIGLU && !b->Wgate[l]))
+      return fmx_fail(FMX_E_INVALID_ARG, "register_backbone: NULL weight pointer in layer %d", l);
+  }
+  b->mWq.resize(L); b->mWk.resize(L); b->mWv.resize(L); b->mWo.resize(L); b->mWup.resize(L); b->mWgate.resize(L); b->mWdown.resize(L);
+  for (int l = 0; l < L; ++l) {
+    int e;
+    if ((e = encode_2d(c, &b->mWq[l], b->Wq[l], dq, d.d_model, d.d_model, 128))) return e;
+    if ((e = encode_2d(c, &b->mWk[l], b->Wk[l], dkv, d.d_model, d.d_model, 128))) return e;
+    if ((e = encode_2d(c, &b->mWv[l], b->Wv[l], dkv, d.d_model, d.d_model, 128))) return e;
+    if ((e = encode_2d(c, &b->mWo[l], b->Wo[l], d.d_model, dq, dq, 128))) return e;
+    if ((e = encode_2d(c, &b->mWup[l], b->Wup[l], d.d_ffn, d.d_model, d.d_model, 128))) return e;
+    if (d.act == FMX_ACT_SWIGLU && (e = encode_2d(c, &b->mWgate[l], b->Wgate[l], d.d_ffn, d.d_model, d.d_model, 128))) return e;
+    if ((e = encode_2d(c, &b->mWdown[l], b->Wdown[l], d.d_model, d.d_ffn, d.d_ffn, 128))) return e;
+  }
+  if (d.input_kind == FMX_INPUT_PATCH_LINEAR) {
+    b->Kp = (d.patch_dim + 7) / 8 * 8;
+    CU_OK(cudaMalloc(&b->embed_Wpad, sizeof(bf16) * d.d_model * b->Kp));
+    const int n = d.d_model * b->Kp;
+    pad_rows_kernel<<<(n + 255) / 256, 256>>>((const bf16 *)d.embed_W, b->embed_Wpad, d.d_model, d.patch_dim, b->Kp);
+    const int n_pos = d.tokens_per_request;
+    CU_OK(cudaMalloc(&b->posb, sizeof(float) * n_pos * d.d_model));
+    build_posb_kernel<<<(n_pos * d.d_model + 255) / 256, 256>>>(b->posb, (const bf16 *)d.embed_b, (const bf16 *)d.embed_cls,
+                                                                   (const bf16 *)d.embed_pos, n_pos, d.d_model, d.has_cls);
+    CU_OK(cudaGetLastError());
+    if (int e = encode_2d(c, &b->mEmbedW, b->embed_Wpad, d.d_model, b->Kp, b->Kp, 128)) return e;
+  }
+  if (d.rope_theta > 0) {
+    const int n = d.max_seq * (d.head_dim / 2);
+    CU_OK(cudaMalloc(&b->rope_cs, sizeof(float2) * n));
+    build_rope_table_kernel<<<(n + 255) / 256, 256>>>(b->rope_cs, d.max_seq, d.head_dim, (double)d.rope_theta);
+    CU_OK(cudaGetLastError());
+  }
+  CU_OK(cudaDeviceSynchronize());
+  b->Rcap = 256;
+  b->col_used.assign(b->Rcap / 16, 0);
+  c->bbs.push_back(std::move(b));
+  *out = (int)c->bbs.size() - 1;
+  return FMX_OK;
+}
+
+int fmx_register_task(fmx_ctx *c, fmx_backbone_t h, const fmx_task_desc *desc, fmx_task_t *out) {
+  if (!c || !desc || !out) return fmx_fail(FMX_E_INVALID_ARG, "register_task: NULL argument");
+  std::lock_guard<std::mutex> lk(c->mu);
+  CU_OK(cudaSetDevice(c->device));
+  Backbone *bb = get_bb(c, h);
+  if (!bb) return fmx_fail(FMX_E_UNKNOWN_BACKBONE, "register_task: unknown backbone %d", h);
+  const fmx_backbone_desc &d = bb->d;
+  const int L = d.n_layers;
+  // ---- validate everything before touching state ----
+  if (desc->n_adapters < 0 || desc->n_adapters > 7 || (desc->n_adapters && !desc->adapters)) return fmx_fail(FMX_E_INVALID_ARG, "register_task: bad n_adapters");
+  if (desc->head_kind < 0 || desc->head_kind > 3 || desc->head_out < 1 || !desc->head_W) return fmx_fail(FMX_E_INVALID_ARG, "register_task: bad head");
+  if (desc->head_kind == FMX_HEAD_FLATTEN && d.tokens_per_request < 1) return fmx_fail(FMX_E_SHAPE, "register_task: FLATTEN head needs a fixed-length backbone");
+  bool seen[7] = {false};
+  int rpad = 0;
+  for (int i = 0; i < desc->n_adapters; ++i) {
+    const fmx_adapter_desc &a = desc->adapters[i];
+    if (a.target < 0 || a.target > 6) return fmx_fail(FMX_E_INVALID_ARG, "register_task: adapter %d: bad target", i);
+    if (seen[a.target]) return fmx_fail(FMX_E_INVALID_ARG, "register_task: two adapters on target %d", a.target);
+    seen[a.target] = true;
+    if (a.rank < 1 || a.rank > FMX_MAX_RANK) return fmx_fail(FMX_E_SHAPE, "register_task: adapter %d: rank %d not in [1,%d]", i, a.rank, FMX_MAX_RANK);
+    if ((a.target == FMX_TGT_GATE) && d.act != FMX_ACT_SWIGLU) return fmx_fail(FMX_E_SHAPE, "register_task: gate adapter on a backbone without a gate projection");
+    if (!a.A || !a.B) return fmx_fail(FMX_E_INVALID_ARG, "register_task: adapter %d: NULL A/B array", i);
+    for (int l = 0; l < L; ++l) if (!a.A[l] || !a.B[l]) return fmx_fail(FMX_E_INVALID_ARG, "register_task: adapter %d: NULL A/B in layer %d", i, l);
+    rpad = std::max(rpad, (a.rank + 15) / 16 * 16);
+  }
+  int slot = -1;
+  for (int t = 0; t < FMX_MAX_TASKS; ++t) if (!c->tasks[t].live) { slot = t; break; }
+  if (slot < 0) return fmx_fail(FMX_E_CAPACITY, "register_task: all %d task slots in use", FMX_MAX_TASKS);
+
+  TaskRec r;
+  r.live = true; r.bb = h; r.head_kind = desc->head_kind; r.head_out = desc->head_out; r.rpad = rpad;
+  // ---- slab columns ----
+  if (rpad) {
+    int units = rpad / 16, pos = find_columns(*bb, units);
+    if (pos < 0) {
+      int new_cap = bb->Rcap;
+      while (pos < 0) {
+        new_cap *= 2;
+        if (new_cap > 16 * 65536) return fmx_fail(FMX_E_CAPACITY, "register_task: LoRA slab capacity exceeded");
+        if (int e = grow_slabs(c, *bb, new_cap)) return e;
+        pos = find_columns(*bb, units);
+      }
+    }
+    r.coff = pos * 16;
+    for (int i = 0; i < desc->n_adapters; ++i) {
+      const fmx_adapter_desc &a = desc->adapters[i];
+      const int tg = a.target;
+      if (!bb->slabA[tg]) if (int e = alloc_slab(c, *bb, tg)) return e;
+      const int din = bb->din[tg], dout = bb->dout[tg];
+      for (int l = 0; l < L; ++l) {
+        bf16 *A = bb->slabA[tg] + ((size_t)l * bb->Rcap + r.coff) * din;
+        bf16 *B = bb->slabB[tg] + (size_t)l * dout * bb->Rcap + r.coff;
+        CU_OK(cudaMemcpyAsync(A, a.A[l], (size_t)a.rank * din * sizeof(bf16), cudaMemcpyDeviceToDevice, 0));
+        CU_OK(cudaMemcpy2DAsync(B, (size_t)bb->Rcap * sizeof(bf16), a.B[l], (size_t)a.rank * sizeof(bf16), (size_t)a.rank * sizeof(bf16),
+                                dout, cudaMemcpyDeviceToDevice, 0));
+      }
+      r.trpad[tg] = (unsigned char)((a.rank + 15) / 16 * 16);
+      r.scale[tg] = a.scaling;
+      bb->n_adapters[tg]++;
+    }
+    for (int u = 0; u < units; ++u) bb->col_used[pos + u] = 1;
+  }
+  // ---- head ----
+  const size_t d_feat = desc->head_kind == FMX_HEAD_FLATTEN ? (size_t)d.tokens_per_request * d.d_model : (size_t)d.d_model;
+  CU_OK(cudaMalloc(&r.head_W, sizeof(bf16) * d_feat * desc->head_out));
+  CU_OK(cudaMemcpyAsync(r.head_W, desc->head_W, sizeof(bf16) * d_feat * desc->head_out, cudaMemcpyDeviceToDevice, 0));
+  if (desc->head_b) {
+    CU_OK(cudaMalloc(&r.head_b, sizeof(bf16) * desc->head_out));
+    CU_OK(cudaMemcpyAsync(r.head_b, desc->head_b, sizeof(bf16) * desc->head_out, cudaMemcpyDeviceToDevice, 0));
+  }
+  c->tasks[slot] = r;
+  c->n_slots = std::max(c->n_slots, slot + 1);
+  if (int e = upload_task_tables(c, slot)) return e;
+  CU_OK(cudaDeviceSynchronize());
+  *out = slot;
+  return FMX_OK;
+}
+
+int fmx_unregister_task(fmx_ctx *c, fmx_task_t t) {
+  if (!c) return fmx_fail(FMX_E_INVALID_ARG, "unregister_task: NULL ctx");
+  std::lock_guard<std::mutex> lk(c->mu);
+  if (t < 0 || t >= FMX_MAX_TASKS || !c->tasks[t].live) return fmx_fail(FMX_E_UNKNOWN_TASK, "unregister_task: task %d is not registered", t);
+  CU_OK(cudaSetDevice(c->device));
+  CU_OK(cudaDeviceSynchronize());
+  TaskRec &r = c->tasks[t];
+  Backbone *bb = get_bb(c, r.bb);
+  const int L = bb->d.n_layers;
+  for (int tg = 0; tg < 7; ++tg) {
+    if (!r.trpad[tg]) continue;
+    for (int l = 0; l < L; ++l) {      // leave unowned columns zero
+      bf16 *A = bb->slabA[tg] + ((size_t)l * bb->Rcap + r.coff) * bb->din[tg];
+      bf16 *B = bb->slabB[tg] + (size_t)l * bb->dout[tg] * bb->Rcap + r.coff;
+      CU_OK(cudaMemsetAsync(A, 0, (size_t)r.trpad[tg] * bb->din[tg] * sizeof(bf16), 0));
+      CU_OK(cudaMemset2DAsync(B, (size_t)bb->Rcap * sizeof(bf16), 0, (size_t)r.trpad[tg] * sizeof(bf16), bb->dout[tg], 0));
+    }
+    bb->n_adapters[tg]--;
+  }
+  for (int u = 0; u < r.rpad / 16; ++u) bb->col_used[r.coff / 16 + u] = 0;
+  cudaFree(r.head_W);
+  cudaFree(r.head_b);
+  r = TaskRec();
+  if (int e = upload_task_tables(c, t)) return e;
+  CU_OK(cudaDeviceSynchronize());
+  return FMX_OK;
+}
+
+int fmx_output_layout(fmx_ctx *c, const int32_t *task_ids, int32_t n_req, int64_t *out_off) {
+  if (!c || !out_off || (n_req > 0 && !task_ids) || n_req < 0) return fmx_fail(FMX_E_INVALID_ARG, "output_layout: bad argument");
+  int64_t run = 0;
+  for (int i = 0; i < n_req; ++i) {
+    const int t = task_ids[i];
+    if (t < 0 || t >= FMX_MAX_TASKS || !c->tasks[t].live) return fmx_fail(FMX_E_UNKNOWN_TASK, "output_layout: request %d: task %d is not registered", i, t);
+    out_off[i] = run;
+    run += c->tasks[t].head_out;
+  }
+  out_off[n_req] = run;
+  return FMX_OK;
+}
+
+int fmx_workspace_bytes(fmx_ctx *c, fmx_backbone_t h, int32_t max_req, int64_t max_tokens, size_t *bytes) {
+  if (!c || !bytes) return fmx_fail(FMX_E_INVALID_ARG, "workspace_bytes: NULL argument");
+  Backbone *bb = get_bb(c, h);
+  if (!bb) return fmx_fail(FMX_E_UNKNOWN_BACKBONE, "workspace_bytes: unknown backbone %d", h);
+  if (max_req < 1 || max_req > FMX_MAX_REQUESTS || max_tokens < 1 || max_tokens > (1ll << 24))
+    return fmx_fail(FMX_E_CAPACITY, "workspace_bytes: max_req in [1,%d], max_tokens in [1,2^24]", FMX_MAX_REQUESTS);
+  *bytes = carve(*bb, nullptr, max_req, max_tokens, FMX_MAX_TASKS).bytes;
+  return FMX_OK;
+}
+
+// ---------------------------------------------------------------- the forward
+static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int32_t *task_ids, const int32_t *lengths,
+                        int32_t B, float *outputs, void *workspace, size_t workspace_bytes, cudaStream_t s) {
+  const fmx_backbone_desc &d = bb.d;
+  // ---- host validation (nothing is enqueued on failure) ----
+  long long N = 0;
+  int max_len = 0, max_out = 0;
+  int bb_index = -1;
+  for (size_t i = 0; i < c->bbs.size(); ++i) if (c->bbs[i].get() == &bb) bb_index = (int)i;
+  for (int i = 0; i < B; ++i) {
+    const int t = task_ids[i];
+    if (t < 0 || t >= FMX_MAX_TASKS || !c->tasks[t].live || c->tasks[t].bb != bb_index)
+      return fmx_fail(FMX_E_UNKNOWN_TASK, "forward_mixed: request %d: task %d is not registered on this backbone", i, t);
+    const int n = lengths[i];
+    if (n < 1 || n > d.max_seq || (d.tokens_per_request && n != d.tokens_per_request))
+      return fmx_fail(FMX_E_BAD_LENGTH, "forward_mixed: request %d: length %d (max_seq %d, fixed %d)", i, n, d.max_seq, d.tokens_per_request);
+    N += n;
+    max_len = std::max(max_len, n);
+    max_out = std::max(max_out, c->tasks[t].head_out);
+  }
+  if (N > (1ll << 24)) return fmx_fail(FMX_E_CAPACITY, "forward_mixed: %lld tokens > 2^24", N);
+  const int T = c->n_slots;
+  if (reinterpret_cast<uintptr_t>(workspace) & 1023) return fmx_fail(FMX_E_WORKSPACE, "forward_mixed: workspace must be 1024-byte aligned");
+  Workspace w = carve(bb, workspace, B, N, T);
+  if (w.bytes > workspace_bytes) return fmx_fail(FMX_E_WORKSPACE, "forward_mixed: workspace %zu B < required %zu B", workspace_bytes, w.bytes);
+
+  const int Ni = (int)N;
+  Launcher Lh{c, s};
+  // ---- S1: ids/lengths to the device, counting sort, tables ----
+  memcpy(c->h_stage, task_ids, sizeof(int) * B);
+  memcpy(c->h_stage + FMX_MAX_REQUESTS, lengths, sizeof(int) * B);
+  CU_OK(cudaMemcpyAsync(w.t.task_ids, c->h_stage, sizeof(int) * B, cudaMemcpyHostToDevice, s));
+  CU_OK(cudaMemcpyAsync(w.t.lengths, c->h_stage + FMX_MAX_REQUESTS, sizeof(int) * B, cudaMemcpyHostToDevice, s));
+  SortArgs sa{};
+  sa.t = w.t; sa.B = B; sa.T = T; sa.n_tiles = w.n_tiles; sa.task_head_out = c->d_task_head_out;
+  if (d.input_kind == FMX_INPUT_EMBEDDED) { sa.in_per_tok = d.d_model; sa.in_per_req = 0; }
+  else if (d.input_kind == FMX_INPUT_TOKEN_IDS) { sa.in_per_tok = 1; sa.in_per_req = 0; }
+  else if (d.img_c) { sa.in_per_tok = 0; sa.in_per_req = (long long)d.img_c * d.img_hw * d.img_hw; }
+  else { sa.in_per_tok = 0; sa.in_per_req = (long long)(d.tokens_per_request - (d.has_cls ? 1 : 0)) * d.patch_dim; }
+  LAUNCH(Lh, F_SORT, (task_sort_kernel<<<1, kSortThreads, 0, s>>>(sa)));
+  LAUNCH(Lh, F_SORT, (row_tables_kernel<<<(Ni + 255) / 256, 256, 0, s>>>(w.t.cu_tok, B, Ni, w.t.row_req, w.t.row_pos)));
+
+  // ---- common GEMM parameter pieces ----
+  GemmParams base{};
+  base.M = Ni; base.n_mtiles = w.n_tiles;
+  base.tile_blk_off = w.t.tile_blk_off; base.blk_task = w.t.blk_task; base.blk_lo = w.t.blk_lo; base.blk_hi = w.t.blk_hi;
+  base.blk_tile = w.t.blk_tile; base.n_blk = w.t.n_blk;
+  base.task_coff = c->d_task_coff; base.task_trpad = c->d_task_trpad; base.task_scale = c->d_task_scale;
+  base.row_pos = w.t.row_pos;
+  for (int i = 0; i < 3; ++i) { base.lora_tgt[i] = -1; base.src_end[i] = 1 << 30; }
+  CUtensorMap mXn, mAttnO, mHid, mU, mPk;
+  int e;
+  if ((e = encode_2d(c, &mXn, w.Xn, Ni, d.d_model, d.d_model, 128))) return e;
+  if ((e = encode_2d(c, &mAttnO, w.AttnO, Ni, bb.d_q, bb.d_q, 128))) return e;
+  if ((e = encode_2d(c, &mHid, w.Hid, Ni, d.d_ffn, d.d_ffn, 128))) return e;
+  if ((e = encode_2d(c, &mU, w.U, (uint64_t)w.n_blk_cap * 128, 192, 192, 128))) return e;
+  base.umap = mU;
+
+  // shrink over an input group: targets tgs[0..n) that currently have adapters; fills uslot_of[tg]
+  int uslot_of[7] = {-1, -1, -1, -1, -1, -1, -1};
+  auto shrink = [&](const CUtensorMap &amap, int K, const int *tgs, int n, int layer) -> int {
+    GemmParams p = base;
+    p.mode = GM_SHRINK; p.amap = amap; p.K = K; p.out = w.U; p.ld_out = 192; p.n_tg = 0;
+    for (int i = 0; i < n; ++i) {
+      const int tg = tgs[i];
+      uslot_of[tg] = -1;
+      if (bb.n_adapters[tg] <= 0) continue;
+      p.wmap[p.n_tg] = bb.mA[tg][layer];
+      p.tg_ids[p.n_tg] = tg;
+      uslot_of[tg] = p.n_tg++;
+    }
+    if (p.n_tg == 0) return FMX_OK;
+    LAUNCH(Lh, F_SHRINK, launch_gemm(c, s, p));
+    return FMX_OK;
+  };
+  auto set_lora = [&](GemmParams &p, int src, int tg, int layer) {
+    if (bb.n_adapters[tg] > 0 && uslot_of[tg] >= 0) {
+      p.lora_tgt[src] = tg; p.uslot[src] = uslot_of[tg]; p.lmap[src] = bb.mB[tg][layer]; p.has_lora = 1;
+    }
+  };
+
+  // ---- S2: embed ----
+  if (d.input_kind == FMX_INPUT_PATCH_LINEAR) {
+    PackArgs pa{};
+    pa.inputs = (const bf16 *)inputs; pa.perm = w.t.perm; pa.row_req = w.t.row_req; pa.row_pos = w.t.row_pos; pa.in_off = w.t.in_off;
+    pa.N = Ni; pa.patch_dim = d.patch_dim; pa.Kp = bb.Kp; pa.has_cls = d.has_cls; pa.img_c = d.img_c; pa.img_hw = d.img_hw; pa.patch_hw = d.patch_hw;
+    pa.A = w.Hid;
+    LAUNCH(Lh, F_EMBED, (pack_patches_kernel<<<Ni, 128, 0, s>>>(pa)));
+    if ((e = encode_2d(c, &mPk, w.Hid, Ni, bb.Kp, bb.Kp, 128))) return e;
+    GemmParams p = base;
+    p.mode = GM_EMBED_F32; p.amap = mPk; p.wmap[0] = bb.mEmbedW; p.K = bb.Kp; p.n_chunks = d.d_model / 128;
+    p.out = w.X; p.ld_out = d.d_model; p.posb = bb.posb;
+    LAUNCH(Lh, F_EMBED, launch_gemm(c, s, p));
+  } else {
+    EmbedArgs ea{};
+    ea.inputs = inputs; ea.perm = w.t.perm; ea.row_req = w.t.row_req; ea.row_pos = w.t.row_pos; ea.in_off = w.t.in_off;
+    ea.N = Ni; ea.d = d.d_model; ea.X = w.X; ea.table = (const bf16 *)d.embed_table; ea.pos = (const bf16 *)d.embed_pos;
+    LAUNCH(Lh, F_EMBED, (embed_rows_kernel<<<(Ni + 7) / 8, 256, 0, s>>>(ea, d.input_kind == FMX_INPUT_TOKEN_IDS)));
+  }
+
+  // ---- layers ----
+  const int rms = d.norm == FMX_NORM_RMSNORM;
+  const float scale_log2 = 1.4426950408889634f / sqrtf((float)d.head_dim);
+  for (int l = 0; l < d.n_layers; ++l) {
+    LAUNCH(Lh, F_NORM, dispatch_norm(s, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm1_g[l], (const bf16 *)bb.norm1_b[l], Ni, d.norm_eps, rms));
+    {
+      const int tgs[3] = {FMX_TGT_Q, FMX_TGT_K, FMX_TGT_V};
+      if ((e = shrink(mXn, d.d_model, tgs, 3, l))) return e;
+      GemmParams p = base;
+      p.mode = GM_OUT_BF16; p.amap = mXn; p.K = d.d_model; p.n_chunks = bb.d_qkv / 128;
+      p.wmap[0] = bb.mWq[l]; p.wmap[1] = bb.mWk[l]; p.wmap[2] = bb.mWv[l];
+      p.src_end[0] = bb.d_q / 128; p.src_end[1] = (bb.d_q + bb.d_kv) / 128; p.src_end[2] = 1 << 30;
+      p.bias[0] = (const bf16 *)bb.bq[l]; p.bias[1] = (const bf16 *)bb.bk[l]; p.bias[2] = (const bf16 *)bb.bv[l];
+      set_lora(p, 0, FMX_TGT_Q, l); set_lora(p, 1, FMX_TGT_K, l); set_lora(p, 2, FMX_TGT_V, l);
+      p.out = w.QKV; p.ld_out = bb.d_qkv;
+      LAUNCH(Lh, F_GEMM_QKV, launch_gemm(c, s, p));
+    }
+    if (d.rope_theta > 0) {
+      const int nh = d.n_q_heads + d.n_kv_heads;
+      const long long total = (long long)Ni * nh * (d.head_dim / 2);
+      LAUNCH(Lh, F_ROPE, (rope_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(w.QKV, bb.d_qkv, w.t.row_pos, bb.rope_cs, Ni, nh, d.head_dim)));
+    }
+    {
+      AttnArgs aa{};
+      aa.qkv = w.QKV; aa.out = w.AttnO; aa.cu_tok = w.t.cu_tok; aa.ld_qkv = bb.d_qkv; aa.ld_out = bb.d_q;
+      aa.n_q_heads = d.n_q_heads; aa.n_kv_heads = d.n_kv_heads; aa.causal = d.causal; aa.scale_log2 = scale_log2;
+      dim3 grid((max_len + kAttnBQ - 1) / kAttnBQ, d.n_q_heads, B);
+      LAUNCH(Lh, F_ATTN, launch_attention(s, d.head_dim, grid, aa));
+    }
+    {
+      const int tgs[1] = {FMX_TGT_O};
+      if ((e = shrink(mAttnO, bb.d_q, tgs, 1, l))) return e;
+      GemmParams p = base;
+      p.mode = GM_RESID_F32; p.amap = mAttnO; p.K = bb.d_q; p.n_chunks = d.d_model / 128;
+      p.wmap[0] = bb.mWo[l]; p.bias[0] = (const bf16 *)bb.bo[l];
+      set_lora(p, 0, FMX_TGT_O, l);
+      p.out = w.X; p.ld_out = d.d_model;
+      LAUNCH(Lh, F_GEMM_O, launch_gemm(c, s, p));
+    }
+    LAUNCH(Lh, F_NORM, dispatch_norm(s, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm2_g[l], (const bf16 *)bb.norm2_b[l], Ni, d.norm_eps, rms));
+    if (d.act == FMX_ACT_SWIGLU) {
+      const int tgs[2] = {FMX_TGT_GATE, FMX_TGT_UP};
+      if ((e = shrink(mXn, d.d_model, tgs, 2, l))) return e;
+      GemmParams p = base;
+      p.mode = GM_OUT_BF16_SWIGLU; p.amap = mXn; p.K = d.d_model; p.n_chunks = 2 * d.d_ffn / 128; p.interleave2 = 1;
+      p.wmap[0] = bb.mWgate[l]; p.wmap[1] = bb.mWup[l];
+      p.bias[0] = (const bf16 *)bb.bgate[l]; p.bias[1] = (const bf16 *)bb.bup[l];
+      set_lora(p, 0, FMX_TGT_GATE, l); set_lora(p, 1, FMX_TGT_UP, l);
+      p.out = w.Hid; p.ld_out = d.d_ffn;
+      LAUNCH(Lh, F_GEMM_FFN_IN, launch_gemm(c, s, p));
+    } else {
+      const int tgs[1] = {FMX_TGT_UP};
+      if ((e = shrink(mXn, d.d_model, tgs, 1, l))) return e;
+      GemmParams p = base;
+      p.mode = d.act == FMX_ACT_GELU_ERF ? GM_OUT_BF16_GELU : GM_OUT_BF16_RELU; p.amap = mXn; p.K = d.d_model; p.n_chunks = d.d_ffn / 128;
+      p.wmap[0] = bb.mWup[l]; p.bias[0] = (const bf16 *)bb.bup[l];
+      set_lora(p, 0, FMX_TGT_UP, l);
+      p.out = w.Hid; p.ld_out = d.d_ffn;
+      LAUNCH(Lh, F_GEMM_FFN_IN, launch_gemm(c, s, p));
+    }
+    {
+      const int tgs[1] = {FMX_TGT_DOWN};
+      if ((e = shrink(mHid, d.d_ffn, tgs, 1, l))) return e;
+      GemmParams p = base;
+      p.mode = GM_RESID_F32; p.amap = mHid; p.K = d.d_ffn; p.n_chunks = d.d_model / 128;
+      p.wmap[0] = bb.mWdown[l]; p.bias[0] = (const bf16 *)bb.bdown[l];
+      set_lora(p, 0, FMX_TGT_DOWN, l);
+      p.out = w.X; p.ld_out = d.d_model;
+      LAUNCH(Lh, F_GEMM_FFN_OUT, launch_gemm(c, s, p));
+    }
+  }
+  // ---- S4-S6 ----
+  PoolArgs pa{};
+  pa.X = w.X; pa.g = (const bf16 *)d.final_g; pa.b = (const bf16 *)d.final_b; pa.cu_tok = w.t.cu_tok; pa.task_sorted = w.t.task_sorted;
+  pa.task_head_kind = c->d_task_head_kind; pa.feat = w.feat; pa.Fn = w.Xn; pa.d = d.d_model; pa.eps = d.norm_eps; pa.rms = rms;
+  LAUNCH(Lh, F_POOL, dispatch_pool(s, d.d_model, B, pa));
+  HeadArgs ha{};
+  ha.feat = w.feat; ha.Fn = w.Xn; ha.cu_tok = w.t.cu_tok; ha.task_sorted = w.t.task_sorted; ha.perm = w.t.perm; ha.out_off = w.t.out_off;
+  ha.task_head_kind = c->d_task_head_kind; ha.task_head_out = c->d_task_head_out;
+  ha.task_head_W = (const bf16 *const *)c->d_task_head_W; ha.task_head_b = (const bf16 *const *)c->d_task_head_b;
+  ha.out = outputs; ha.d = d.d_model;
+  LAUNCH(Lh, F_HEAD, (head_kernel<<<dim3(B, (max_out + 7) / 8), 256, 0, s>>>(ha)));
+
+  {
+    void *bufs[7] = {w.X, w.Xn, w.QKV, w.AttnO, w.Hid, w.U, w.feat};
+    size_t sz[7] = {sizeof(float) * N * d.d_model, sizeof(bf16) * N * d.d_model, sizeof(bf16) * N * bb.d_qkv, sizeof(bf16) * N * bb.d_q,
+                    sizeof(bf16) * N * d.d_ffn, sizeof(bf16) * (size_t)w.n_blk_cap * 128 * 192, sizeof(float) * (size_t)B * d.d_model};
+    for (int i = 0; i < 7; ++i) { c->last_buf[i] = bufs[i]; c->last_buf_bytes[i] = sz[i]; }
+  }
+  c->last_t = w.t; c->last_B = B; c->last_T = T; c->last_n_tiles = w.n_tiles; c->last_stream = s; c->last_launches = Lh.count;
+  return FMX_OK;
+}
+
+int fmx_forward_mixed(fmx_ctx *c, fmx_backbone_t h, const void *inputs, const int32_t *task_ids, const int32_t *lengths,
+                      int32_t n_req, float *outputs, void *workspace, size_t workspace_bytes, void *cuda_stream) {
+  if (!c) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed: NULL ctx");
+  if (n_req < 0) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed: n_req < 0");
+  Backbone *bb = get_bb(c, h);
+  if (!bb) return fmx_fail(FMX_E_UNKNOWN_BACKBONE, "forward_mixed: unknown backbone %d", h);
+  if (n_req == 0) return FMX_OK;
+  if (n_req > FMX_MAX_REQUESTS) return fmx_fail(FMX_E_CAPACITY, "forward_mixed: %d requests > %d", n_req, FMX_MAX_REQUESTS);
+  if (!inputs || !task_ids || !lengths || !outputs || !workspace) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed: NULL pointer");
+  std::lock_guard<std::mutex> lk(c->mu);
+  CU_OK(cudaSetDevice(c->device));
+  return forward_impl(c, *bb, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, (cudaStream_t)cuda_stream);
+}
+
+int fmx_forward_mixed_host(fmx_ctx *c, fmx_backbone_t h, const void *inputs_host, size_t inputs_bytes, const int32_t *task_ids,
+                           const int32_t *lengths, int32_t n_req, float *outputs_host, void *workspace, size_t workspace_bytes,
+                           void *cuda_stream) {
+  if (!c) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed_host: NULL ctx");
+  if (n_req < 0) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed_host: n_req < 0");
+  Backbone *bb = get_bb(c, h);
+  if (!bb) return fmx_fail(FMX_E_UNKNOWN_BACKBONE, "forward_mixed_host: unknown backbone %d", h);
+  if (n_req == 0) return FMX_OK;
+  if (!inputs_host || !task_ids || !lengths || !outputs_host || !workspace) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed_host: NULL pointer");
+  std::vector<int64_t> off(n_req + 1);
+  if (int e = fmx_output_layout(c, task_ids, n_req, off.data())) return e;
+  std::lock_guard<std::mutex> lk(c->mu);
+  CU_OK(cudaSetDevice(c->device));
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const size_t out_bytes = (size_t)off[n_req] * sizeof(float);
+  if (inputs_bytes > c->in_stage_bytes) {
+    CU_OK(cudaStreamSynchronize(s));
+    cudaFree(c->d_in_stage);
+    c->d_in_stage = nullptr; c->in_stage_bytes = 0;
+    CU_OK(cudaMalloc(&c->d_in_stage, align_up(inputs_bytes, 1 << 20)));
+    c->in_stage_bytes = align_up(inputs_bytes, 1 << 20);
+  }
+  if (out_bytes > c->out_stage_bytes) {
+    CU_OK(cudaStreamSynchronize(s));
+    cudaFree(c->d_out_stage);
+    c->d_out_stage = nullptr; c->out_stage_bytes = 0;
+    CU_OK(cudaMalloc(&c->d_out_stage, align_up(out_bytes, 1 << 16)));
+    c->out_stage_bytes = align_up(out_bytes, 1 << 16);
+  }
+  CU_OK(cudaMemcpyAsync(c->d_in_stage, inputs_host, inputs_bytes, cudaMemcpyHostToDevice, s));
+  if (int e = forward_impl(c, *bb, c->d_in_stage, task_ids, lengths, n_req, c->d_out_stage, workspace, workspace_bytes, s)) return e;
+  CU_OK(cudaMemcpyAsync(outputs_host, c->d_out_stage, out_bytes, cudaMemcpyDeviceToHost, s));
+  CU_OK(cudaStreamSynchronize(s));
+  return FMX_OK;
+}
+
+int fmx_debug_get_segments(fmx_ctx *c, int32_t *perm, int32_t *inv_perm, int32_t *task_req_off, int32_t *cu_tok, int32_t *task_tok_off) {
+  if (!c || c->last_B == 0) return fmx_fail(FMX_E_INVALID_ARG, "debug_get_segments: no forward has run");
+  CU_OK(cudaStreamSynchronize(c->last_stream));
+  const SegTables &t = c->last_t;
+  const int B = c->last_B, T = c->last_T;
+  if (perm) CU_OK(cudaMemcpy(perm, t.perm, sizeof(int) * B, cudaMemcpyDeviceToHost));
+  if (inv_perm) CU_OK(cudaMemcpy(inv_perm, t.inv_perm, sizeof(int) * B, cudaMemcpyDeviceToHost));
+  if (task_req_off) CU_OK(cudaMemcpy(task_req_off, t.task_req_off, sizeof(int) * (T + 1), cudaMemcpyDeviceToHost));
+  if (cu_tok) CU_OK(cudaMemcpy(cu_tok, t.cu_tok, sizeof(int) * (B + 1), cudaMemcpyDeviceToHost));
+  if (task_tok_off) CU_OK(cudaMemcpy(task_tok_off, t.task_tok_off, sizeof(int) * (T + 1), cudaMemcpyDeviceToHost));
+  return FMX_OK;
+}
+
+int fmx_debug_get_tiles(fmx_ctx *c, int32_t *n_tiles, int32_t *n_blocks, int32_t *blocks, int32_t cap) {
+  if (!c || c->last_B == 0) return fmx_fail(FMX_E_INVALID_ARG, "debug_get_tiles: no forward has run");
+  CU_OK(cudaStreamSynchronize(c->last_stream));
+  const SegTables &t = c->last_t;
+  int nb = 0;
+  CU_OK(cudaMemcpy(&nb, t.n_blk, sizeof(int), cudaMemcpyDeviceToHost));
+  if (n_tiles) *n_tiles = c->last_n_tiles;
+  if (n_blocks) *n_blocks = nb;
+  if (blocks) {
+    const int n = std::min(nb, cap);
+    std::vector<int> a(n), b(n), lo(n), hi(n);
+    CU_OK(cudaMemcpy(a.data(), t.blk_tile, sizeof(int) * n, cudaMemcpyDeviceToHost));
+    CU_OK(cudaMemcpy(b.data(), t.blk_task, sizeof(int) * n, cudaMemcpyDeviceToHost));
+    CU_OK(cudaMemcpy(lo.data(), t.blk_lo, sizeof(int) * n, cudaMemcpyDeviceToHost));
+    CU_OK(cudaMemcpy(hi.data(), t.blk_hi, sizeof(int) * n, cudaMemcpyDeviceToHost));
+    for (int i = 0; i < n; ++i) { blocks[4 * i] = a[i]; blocks[4 * i + 1] = b[i]; blocks[4 * i + 2] = lo[i]; blocks[4 * i + 3] = hi[i]; }
+  }
+  return FMX_OK;
+}
+
+int fmx_debug_read(fmx_ctx *c, int which, void *host, size_t bytes) {
+  if (!c || c->last_B == 0 || which < 0 || which > 6 || !host) return fmx_fail(FMX_E_INVALID_ARG, "debug_read: bad argument or no forward has run");
+  if (bytes > c->last_buf_bytes[which]) return fmx_fail(FMX_E_INVALID_ARG, "debug_read: %zu > %zu bytes", bytes, c->last_buf_bytes[which]);
+  CU_OK(cudaStreamSynchronize(c->last_stream));
+  CU_OK(cudaMemcpy(host, c->last_buf[which], bytes, cudaMemcpyDeviceToHost));
+  return FMX_OK;
+}
+
+int fmx_profile_enable(fmx_ctx *c, int on) {
+  if (!c) return fmx_fail(FMX_E_INVALID_ARG, "profile_enable: NULL ctx");
+  std::lock_guard<std::mutex> lk(c->mu);
+  CU_OK(cudaDeviceSynchronize());
+  for (auto &pe : c->prof) { cudaEventDestroy(pe.e0); cudaEventDestroy(pe.e1); }
+  c->prof.clear();
+  c->prof_on = on != 0;
+  return FMX_OK;
+}
+
+int fmx_profile_read(fmx_ctx *c, int32_t *launches, double *total_ms) {
+  if (!c || !launches || !total_ms) return fmx_fail(FMX_E_INVALID_ARG, "profile_read: NULL argument");
+  std::lock_guard<std::mutex> lk(c->mu);
+  CU_OK(cudaDeviceSynchronize());
+  for (int f = 0; f < FMX_N_FAMILIES; ++f) { launches[f] = 0; total_ms[f] = 0.0; }
+  for (auto &pe : c->prof) {
+    float ms = 0.0f;
+    CU_OK(cudaEventElapsedTime(&ms, pe.e0, pe.e1));
+    launches[pe.family]++;
+    total_ms[pe.family] += ms;
+  }
+  return FMX_OK;
+}
+
+const char *fmx_profile_family_name(int f) { return (f >= 0 && f < FMX_N_FAMILIES) ? kFamilyNames[f] : ""; }
+int fmx_last_launch_count(fmx_ctx *c) { return c ? c->last_launches : 0; }
+
+int fmx_debug_gemm(fmx_ctx *c, const void *A, const void *W, float *C, int32_t M, int32_t N, int32_t K, void *cuda_stream) {
+  if (!c || !A || !W || !C) return fmx_fail(FMX_E_INVALID_ARG, "debug_gemm: NULL argument");
+  if (M < 1 || N < 128 || N % 128 || K < 8 || K % 8) return fmx_fail(FMX_E_SHAPE, "debug_gemm: need N %% 128 == 0, K %% 8 == 0");
+  std::lock_guard<std::mutex> lk(c->mu);
+  CU_OK(cudaSetDevice(c->device));
+  GemmParams p{};
+  int e;
+  if ((e = encode_2d(c, &p.amap, A, M, K, K, 128))) return e;
+  if ((e = encode_2d(c, &p.wmap[0], W, N, K, K, 128))) return e;
+  p.M = M; p.K = K; p.n_chunks = N / 128; p.n_mtiles = (M + 127) / 128; p.mode = GM_OUT_F32;
+  for (int i = 0; i < 3; ++i) { p.lora_tgt[i] = -1; p.src_end[i] = 1 << 30; }
+  p.out = C; p.ld_out = N;
+  launch_gemm(c, (cudaStream_t)cuda_stream, p);
+  CU_OK(cudaGetLastError());
+  return FMX_OK;
+}
+
+}  // extern "C"

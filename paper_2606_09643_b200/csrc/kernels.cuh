@@ -1,0 +1,478 @@
+// Memory-bound and integer kernels of the mixed-task forward: task counting sort + segment
+// tables (S1), row tables, embed/pack (S2), LayerNorm/RMSNorm (S3a), RoPE, final norm + pool
+// (S4), per-task heads + output un-permute (S5/S6).
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "ptx.cuh"
+
+namespace fmx {
+
+// ============================================================================= S1
+// Device pointers of the segment tables (all int32 unless noted), carved from the workspace.
+struct SegTables {
+  int *task_ids, *lengths;         // [B] copies of the caller's host arrays (original order)
+  int *perm, *inv_perm;            // [B]
+  int *task_req_off, *task_tok_off;  // [T+1]
+  int *cu_tok;                     // [B+1]
+  int *task_sorted;                // [B] task id at sorted position p
+  long long *in_off;               // [B+1] element offset of request i in the packed input (original order)
+  long long *out_off;              // [B+1] fp32 offset of request i in the output (original order)
+  int *tile_blk_off;               // [n_tiles+1]
+  int *blk_tile, *blk_task, *blk_lo, *blk_hi;   // [n_blk_cap]
+  int *n_blk;                      // scalar
+  int *row_req, *row_pos;          // [N] sorted request index / position within request, per token row
+};
+
+struct SortArgs {
+  SegTables t;
+  int B, T;                        // requests, task slots
+  int n_tiles;                     // ceil(N / 128)
+  long long in_per_tok, in_per_req;  // packed-input elements per token / per request
+  const int *task_head_out;        // [T]
+};
+
+constexpr int kSortThreads = 1024;
+
+// Block-wide exclusive scan of n ints (global or shared), in place; returns the total.
+// Every thread of the block must call it.  scratch: kSortThreads + 1 ints of shared memory.
+__device__ inline long long block_exclusive_scan_ll(long long *a, int n, long long *scratch) {
+  const int tid = threadIdx.x, nt = blockDim.x;
+  const int per = (n + nt - 1) / nt;
+  const int lo = min(tid * per, n), hi = min(lo + per, n);
+  long long s = 0;
+  for (int i = lo; i < hi; ++i) s += a[i];
+  scratch[tid] = s;
+  __syncthreads();
+  if (tid == 0) {
+    long long run = 0;
+    for (int i = 0; i < nt; ++i) { long long v = scratch[i]; scratch[i] = run; run += v; }
+    scratch[nt] = run;
+  }
+  __syncthreads();
+  long long run = scratch[tid];
+  for (int i = lo; i < hi; ++i) { long long v = a[i]; a[i] = run; run += v; }
+  const long long total = scratch[nt];
+  __syncthreads();
+  return total;
+}
+
+__device__ inline int block_exclusive_scan_i(int *a, int n, int *scratch) {
+  const int tid = threadIdx.x, nt = blockDim.x;
+  const int per = (n + nt - 1) / nt;
+  const int lo = min(tid * per, n), hi = min(lo + per, n);
+  int s = 0;
+  for (int i = lo; i < hi; ++i) s += a[i];
+  scratch[tid] = s;
+  __syncthreads();
+  if (tid < 32) {                                  // warp 0 scans the 1024 partials, 32 per lane
+    const int seg = nt / 32;
+    int part = 0;
+    for (int i = 0; i < seg; ++i) part += scratch[tid * seg + i];
+    int incl = part;
+    for (int d = 1; d < 32; d <<= 1) { int v = __shfl_up_sync(0xffffffffu, incl, d); if (tid >= d) incl += v; }
+    int run = incl - part;
+    for (int i = 0; i < seg; ++i) { int v = scratch[tid * seg + i]; scratch[tid * seg + i] = run; run += v; }
+    if (tid == 31) scratch[nt] = incl;
+  }
+  __syncthreads();
+  int run = scratch[tid];
+  for (int i = lo; i < hi; ++i) { int v = a[i]; a[i] = run; run += v; }
+  const int total = scratch[nt];
+  __syncthreads();
+  return total;
+}
+
+// One CTA.  Stable counting sort of request indices by task id, then the prefix tables and the
+// (row-tile, task) block table the segmented GEMMs walk.  Integer only; deterministic.
+__global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortArgs a) {
+  __shared__ int s_cnt[1024 + 1];          // per-task count, then task_req_off
+  __shared__ int s_tok[1024 + 1];          // task_tok_off
+  __shared__ int s_scratch[kSortThreads + 1];
+  __shared__ long long s_scratch_ll[kSortThreads + 1];
+  __shared__ int s_rank[4096];             // rank of request i within its task
+  const int tid = threadIdx.x, B = a.B, T = a.T;
+  const SegTables &t = a.t;
+
+  for (int i = tid; i <= T; i += blockDim.x) s_cnt[i] = 0;
+  __syncthreads();
+  // (1) stable rank within task: warp 0 walks the requests 32 at a time, in order.
+  if (tid < 32) {
+    for (int base = 0; base < B; base += 32) {
+      const int i = base + tid;
+      const bool ok = i < B;
+      const int key = ok ? t.task_ids[i] : -1 - tid;           // inactive lanes get unique keys
+      const unsigned m = __match_any_sync(0xffffffffu, key);
+      const int leader = __ffs(m) - 1;
+      const int rank_in_chunk = __popc(m & ((1u << tid) - 1u));
+      int start = 0;
+      if (ok && tid == leader) { start = s_cnt[key]; s_cnt[key] = start + __popc(m); }
+      start = __shfl_sync(0xffffffffu, start, leader);
+      if (ok) s_rank[i] = start + rank_in_chunk;
+      __syncwarp();
+    }
+  }
+  __syncthreads();
+  // (2) task_req_off = exclusive scan of the counts
+  if (tid == 0) s_cnt[T] = 0;
+  __syncthreads();
+  block_exclusive_scan_i(s_cnt, T + 1, s_scratch);
+  for (int i = tid; i <= T; i += blockDim.x) t.task_req_off[i] = s_cnt[i];
+  // (3) perm / inv_perm / sorted lengths
+  for (int i = tid; i < B; i += blockDim.x) {
+    const int tk = t.task_ids[i];
+    const int pos = s_cnt[tk] + s_rank[i];
+    t.perm[pos] = i;
+    t.inv_perm[i] = pos;
+    t.task_sorted[pos] = tk;
+    t.cu_tok[pos] = t.lengths[i];
+  }
+  if (tid == 0) t.cu_tok[B] = 0;
+  __syncthreads();
+  // (4) cu_tok = exclusive scan of the sorted lengths; task_tok_off
+  block_exclusive_scan_i(t.cu_tok, B + 1, s_scratch);
+  for (int i = tid; i <= T; i += blockDim.x) { const int v = t.cu_tok[s_cnt[i]]; s_tok[i] = v; t.task_tok_off[i] = v; }
+  // (5) input / output offsets in ORIGINAL request order
+  for (int i = tid; i < B; i += blockDim.x) {
+    t.in_off[i] = (long long)t.lengths[i] * a.in_per_tok + a.in_per_req;
+    t.out_off[i] = a.task_head_out[t.task_ids[i]];
+  }
+  if (tid == 0) { t.in_off[B] = 0; t.out_off[B] = 0; }
+  __syncthreads();
+  block_exclusive_scan_ll(t.in_off, B + 1, s_scratch_ll);
+  block_exclusive_scan_ll(t.out_off, B + 1, s_scratch_ll);
+  // (6) block table: for each 128-row tile, the non-empty task segments that intersect it.
+  const int n_tok = s_tok[T];
+  auto first_task_after = [&](int row) {     // smallest task with tok_off[task+1] > row
+    int lo = 0, hi = T;                      // invariant: answer in [lo, hi)
+    while (lo < hi) { int mid = (lo + hi) >> 1; if (s_tok[mid + 1] > row) hi = mid; else lo = mid + 1; }
+    return lo;
+  };
+  for (int m = tid; m < a.n_tiles; m += blockDim.x) {
+    const int r0 = m * 128, r1 = min(r0 + 128, n_tok);
+    int cnt = 0;
+    for (int k = first_task_after(r0); k < T && s_tok[k] < r1; ++k) cnt += (s_tok[k + 1] > s_tok[k]);
+    t.tile_blk_off[m] = cnt;
+  }
+  if (tid == 0) t.tile_blk_off[a.n_tiles] = 0;
+  __syncthreads();
+  const int n_blk = block_exclusive_scan_i(t.tile_blk_off, a.n_tiles + 1, s_scratch);
+  if (tid == 0) *t.n_blk = n_blk;
+  for (int m = tid; m < a.n_tiles; m += blockDim.x) {
+    const int r0 = m * 128, r1 = min(r0 + 128, n_tok);
+    int b = t.tile_blk_off[m];
+    for (int k = first_task_after(r0); k < T && s_tok[k] < r1; ++k) {
+      if (s_tok[k + 1] <= s_tok[k]) continue;
+      t.blk_tile[b] = m;
+      t.blk_task[b] = k;
+      t.blk_lo[b] = max(s_tok[k], r0) - r0;
+      t.blk_hi[b] = min(s_tok[k + 1], r1) - r0;
+      ++b;
+    }
+  }
+}
+
+// row -> (sorted request index, position within the request)
+__global__ void row_tables_kernel(const int *__restrict__ cu_tok, int B, int N, int *__restrict__ row_req,
+                                  int *__restrict__ row_pos) {
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= N) return;
+  int lo = 0, hi = B;                          // largest p with cu_tok[p] <= r
+  while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (cu_tok[mid] <= r) lo = mid; else hi = mid; }
+  row_req[r] = lo;
+  row_pos[r] = r - cu_tok[lo];
+}
+
+// ============================================================================= S2
+struct EmbedArgs {
+  const void *inputs;              // packed, original request order
+  const int *perm, *row_req, *row_pos;
+  const long long *in_off;
+  int N, d;
+  float *X;                        // fp32 residual [N, d], task-sorted rows
+  const __nv_bfloat16 *table;      // TOKEN_IDS
+  const __nv_bfloat16 *pos;        // optional positional table [max_seq, d] (EMBEDDED/TOKEN_IDS)
+};
+
+// EMBEDDED: X[r] = x_i[pos] (+ Pos[pos]);   one warp per row, 8 bf16 per lane per step
+__global__ void embed_rows_kernel(const EmbedArgs a, int token_ids) {
+  const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (warp >= a.N) return;
+  const int r = warp, pos = a.row_pos[r], i = a.perm[a.row_req[r]];
+  const __nv_bfloat16 *src;
+  if (token_ids) {
+    const int id = reinterpret_cast<const int *>(a.inputs)[a.in_off[i] + pos];
+    src = a.table + (size_t)id * a.d;
+  } else {
+    src = reinterpret_cast<const __nv_bfloat16 *>(a.inputs) + a.in_off[i] + (size_t)pos * a.d;
+  }
+  float *dst = a.X + (size_t)r * a.d;
+  for (int c = lane * 8; c < a.d; c += 256) {
+    const uint4 v = *reinterpret_cast<const uint4 *>(src + c);
+    float f[8] = {bf16_lo(v.x), bf16_hi(v.x), bf16_lo(v.y), bf16_hi(v.y), bf16_lo(v.z), bf16_hi(v.z), bf16_lo(v.w), bf16_hi(v.w)};
+    if (a.pos) {
+      const uint4 q = *reinterpret_cast<const uint4 *>(a.pos + (size_t)pos * a.d + c);
+      f[0] += bf16_lo(q.x); f[1] += bf16_hi(q.x); f[2] += bf16_lo(q.y); f[3] += bf16_hi(q.y);
+      f[4] += bf16_lo(q.z); f[5] += bf16_hi(q.z); f[6] += bf16_lo(q.w); f[7] += bf16_hi(q.w);
+    }
+    *reinterpret_cast<float4 *>(dst + c) = make_float4(f[0], f[1], f[2], f[3]);
+    *reinterpret_cast<float4 *>(dst + c + 4) = make_float4(f[4], f[5], f[6], f[7]);
+  }
+}
+
+struct PackArgs {
+  const __nv_bfloat16 *inputs;
+  const int *perm, *row_req, *row_pos;
+  const long long *in_off;
+  int N, patch_dim, Kp, has_cls;
+  int img_c, img_hw, patch_hw;     // img_c = 0: input already [n_patches, patch_dim]
+  __nv_bfloat16 *A;                // [N, Kp] task-sorted patch rows (CLS rows and the K pad are zero)
+};
+
+// PATCH_LINEAR: gather (and patchify) into the A operand of the embed GEMM.  One block per row.
+__global__ void pack_patches_kernel(const PackArgs a) {
+  const int r = blockIdx.x;
+  const int pos = a.row_pos[r], i = a.perm[a.row_req[r]];
+  const __nv_bfloat16 *src = a.inputs + a.in_off[i];
+  __nv_bfloat16 *dst = a.A + (size_t)r * a.Kp;
+  const int pi = pos - a.has_cls;
+  const int P = a.patch_hw, g = a.img_c ? a.img_hw / P : 1;
+  const int gy = pi / g, gx = pi - gy * g;
+  for (int e = threadIdx.x; e < a.Kp; e += blockDim.x) {
+    __nv_bfloat16 v = __float2bfloat16(0.0f);
+    if (pi >= 0 && e < a.patch_dim) {
+      if (a.img_c) {
+        const int c = e / (P * P), rem = e - c * P * P, py = rem / P, px = rem - py * P;
+        v = src[((size_t)c * a.img_hw + gy * P + py) * a.img_hw + gx * P + px];
+      } else {
+        v = src[(size_t)pi * a.patch_dim + e];
+      }
+    }
+    dst[e] = v;
+  }
+}
+
+// posb[p, :] = (p == 0 && has_cls ? cls : embed_b) + Pos[p]     (fp32; built once at registration)
+__global__ void build_posb_kernel(float *posb, const __nv_bfloat16 *b, const __nv_bfloat16 *cls,
+                                  const __nv_bfloat16 *pos, int n_pos, int d, int has_cls) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n_pos * d) return;
+  const int p = idx / d, c = idx - p * d;
+  float v = 0.0f;
+  if (has_cls && p == 0) v = __bfloat162float(cls[c]);
+  else if (b) v = __bfloat162float(b[c]);
+  if (pos) v += __bfloat162float(pos[idx]);
+  posb[idx] = v;
+}
+
+// W_e [d, patch_dim] -> [d, Kp] zero padded (row stride must be a multiple of 16 B for TMA)
+__global__ void pad_rows_kernel(const __nv_bfloat16 *src, __nv_bfloat16 *dst, int rows, int k, int kp) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= rows * kp) return;
+  const int r = idx / kp, c = idx - r * kp;
+  dst[idx] = c < k ? src[(size_t)r * k + c] : __float2bfloat16(0.0f);
+}
+
+// ============================================================================= S3a
+// One warp per row: fp32 X [N, d] -> bf16 Y [N, d].  LayerNorm (g, b) or RMSNorm (g); fp32 statistics.
+template <int kVec>   // float4s per lane: d = 128 * kVec
+__global__ void __launch_bounds__(256) norm_kernel(const float *__restrict__ X, __nv_bfloat16 *__restrict__ Y,
+                                                   const __nv_bfloat16 *__restrict__ g,
+                                                   const __nv_bfloat16 *__restrict__ b, int N, float eps, int rms) {
+  const int row = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (row >= N) return;
+  constexpr int d = 128 * kVec;
+  const float4 *x = reinterpret_cast<const float4 *>(X + (size_t)row * d);
+  float4 v[kVec];
+  float s = 0.0f;
+#pragma unroll
+  for (int j = 0; j < kVec; ++j) { v[j] = x[j * 32 + lane]; s += v[j].x + v[j].y + v[j].z + v[j].w; }
+  float mean = 0.0f;
+  if (!rms) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    mean = s * (1.0f / d);
+  }
+  float q = 0.0f;
+#pragma unroll
+  for (int j = 0; j < kVec; ++j) {
+    const float a0 = v[j].x - mean, a1 = v[j].y - mean, a2 = v[j].z - mean, a3 = v[j].w - mean;
+    q += a0 * a0 + a1 * a1 + a2 * a2 + a3 * a3;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) q += __shfl_xor_sync(0xffffffffu, q, o);
+  const float inv = rsqrtf(q * (1.0f / d) + eps);
+  uint2 *y = reinterpret_cast<uint2 *>(Y + (size_t)row * d);
+#pragma unroll
+  for (int j = 0; j < kVec; ++j) {
+    const int c4 = j * 32 + lane;
+    const uint2 gg = reinterpret_cast<const uint2 *>(g)[c4];
+    float o0 = (v[j].x - mean) * inv * bf16_lo(gg.x), o1 = (v[j].y - mean) * inv * bf16_hi(gg.x);
+    float o2 = (v[j].z - mean) * inv * bf16_lo(gg.y), o3 = (v[j].w - mean) * inv * bf16_hi(gg.y);
+    if (b) {
+      const uint2 bb = reinterpret_cast<const uint2 *>(b)[c4];
+      o0 += bf16_lo(bb.x); o1 += bf16_hi(bb.x); o2 += bf16_lo(bb.y); o3 += bf16_hi(bb.y);
+    }
+    y[c4] = make_uint2(pack_bf16(o0, o1), pack_bf16(o2, o3));
+  }
+}
+
+// ============================================================================= RoPE (in place on the fused qkv buffer)
+// rotate-half pairing (j, j + dh/2); position = row_pos[row]; cs = [max_seq, dh/2] float2 (cos, sin)
+__global__ void rope_kernel(__nv_bfloat16 *qkv, int ld, const int *__restrict__ row_pos, const float2 *__restrict__ cs,
+                            int N, int n_heads_qk, int dh) {
+  const int half = dh >> 1;
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;     // (row, head, j)
+  const long long total = (long long)N * n_heads_qk * half;
+  if (idx >= total) return;
+  const int j = (int)(idx % half);
+  const int h = (int)((idx / half) % n_heads_qk);
+  const int row = (int)(idx / ((long long)half * n_heads_qk));
+  const float2 c = cs[(size_t)row_pos[row] * half + j];
+  __nv_bfloat16 *p = qkv + (size_t)row * ld + h * dh + j;
+  const float x1 = __bfloat162float(p[0]), x2 = __bfloat162float(p[half]);
+  p[0] = __float2bfloat16(x1 * c.x - x2 * c.y);
+  p[half] = __float2bfloat16(x2 * c.x + x1 * c.y);
+}
+
+__global__ void build_rope_table_kernel(float2 *cs, int max_seq, int dh, double theta) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int half = dh >> 1;
+  if (idx >= max_seq * half) return;
+  const int p = idx / half, j = idx - p * half;
+  const double ang = (double)p * pow(theta, -2.0 * (double)j / (double)dh);
+  cs[idx] = make_float2((float)cos(ang), (float)sin(ang));
+}
+
+// ============================================================================= S4: final norm + pool
+struct PoolArgs {
+  const float *X;                  // [N, d]
+  const __nv_bfloat16 *g, *b;
+  const int *cu_tok, *task_sorted;
+  const int *task_head_kind;       // [T]
+  float *feat;                     // [B, d] fp32 pooled feature per SORTED request (mean / cls / last)
+  __nv_bfloat16 *Fn;               // [N, d] bf16 normed rows (written for FLATTEN requests only)
+  int d;
+  float eps;
+  int rms;
+};
+
+// One block (128 threads = 4 warps) per sorted request.  Each warp normalises rows; mean-pool is
+// accumulated per warp in registers (fixed row->warp assignment and fixed combine order: deterministic).
+template <int kVec>
+__global__ void __launch_bounds__(128) final_pool_kernel(const PoolArgs a) {
+  constexpr int d = 128 * kVec;
+  __shared__ float s_part[4][d];
+  const int p = blockIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int r0 = a.cu_tok[p], n = a.cu_tok[p + 1] - r0;
+  const int kind = a.task_head_kind[a.task_sorted[p]];
+  float4 accv[kVec];
+#pragma unroll
+  for (int j = 0; j < kVec; ++j) accv[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+  int first = 0, last = n;
+  if (kind == 1) { first = 0; last = 1; }            // CLS
+  else if (kind == 2) { first = n - 1; last = n; }   // LAST
+  for (int i = first + warp; i < last; i += 4) {
+    const float4 *x = reinterpret_cast<const float4 *>(a.X + (size_t)(r0 + i) * d);
+    float4 v[kVec];
+    float s = 0.0f;
+#pragma unroll
+    for (int j = 0; j < kVec; ++j) { v[j] = x[j * 32 + lane]; s += v[j].x + v[j].y + v[j].z + v[j].w; }
+    float mean = 0.0f;
+    if (!a.rms) {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+      mean = s * (1.0f / d);
+    }
+    float q = 0.0f;
+#pragma unroll
+    for (int j = 0; j < kVec; ++j) {
+      const float a0 = v[j].x - mean, a1 = v[j].y - mean, a2 = v[j].z - mean, a3 = v[j].w - mean;
+      q += a0 * a0 + a1 * a1 + a2 * a2 + a3 * a3;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) q += __shfl_xor_sync(0xffffffffu, q, o);
+    const float inv = rsqrtf(q * (1.0f / d) + a.eps);
+#pragma unroll
+    for (int j = 0; j < kVec; ++j) {
+      const int c4 = j * 32 + lane;
+      const uint2 gg = reinterpret_cast<const uint2 *>(a.g)[c4];
+      float o0 = (v[j].x - mean) * inv * bf16_lo(gg.x), o1 = (v[j].y - mean) * inv * bf16_hi(gg.x);
+      float o2 = (v[j].z - mean) * inv * bf16_lo(gg.y), o3 = (v[j].w - mean) * inv * bf16_hi(gg.y);
+      if (a.b) {
+        const uint2 bb = reinterpret_cast<const uint2 *>(a.b)[c4];
+        o0 += bf16_lo(bb.x); o1 += bf16_hi(bb.x); o2 += bf16_lo(bb.y); o3 += bf16_hi(bb.y);
+      }
+      if (kind == 3) {
+        reinterpret_cast<uint2 *>(a.Fn + (size_t)(r0 + i) * d)[c4] = make_uint2(pack_bf16(o0, o1), pack_bf16(o2, o3));
+      } else {
+        accv[j].x += o0; accv[j].y += o1; accv[j].z += o2; accv[j].w += o3;
+      }
+    }
+  }
+  if (kind == 3) return;
+#pragma unroll
+  for (int j = 0; j < kVec; ++j) reinterpret_cast<float4 *>(s_part[warp])[j * 32 + lane] = accv[j];
+  __syncthreads();
+  const float scale = kind == 0 ? 1.0f / (float)n : 1.0f;
+  for (int c = threadIdx.x; c < d; c += 128) {
+    float s = 0.0f;
+#pragma unroll
+    for (int w = 0; w < 4; ++w) s += s_part[w][c];
+    a.feat[(size_t)p * d + c] = s * scale;
+  }
+}
+
+// ============================================================================= S5 + S6: per-task heads
+struct HeadArgs {
+  const float *feat;               // [B, d] (pooled kinds)
+  const __nv_bfloat16 *Fn;         // [N, d] (FLATTEN)
+  const int *cu_tok, *task_sorted, *perm;
+  const long long *out_off;
+  const int *task_head_kind, *task_head_out;
+  const __nv_bfloat16 *const *task_head_W, *const *task_head_b;
+  float *out;
+  int d;
+};
+
+// grid (sorted request p, output tile of 8): each warp computes one output o as a dot product over
+// d_feat with 16-byte loads; result written straight to the caller's buffer in ORIGINAL order.
+__global__ void __launch_bounds__(256) head_kernel(const HeadArgs a) {
+  const int p = blockIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int t = a.task_sorted[p];
+  const int o = blockIdx.y * 8 + warp;
+  const int n_out = a.task_head_out[t];
+  if (o >= n_out) return;
+  const int kind = a.task_head_kind[t];
+  const int r0 = a.cu_tok[p], n = a.cu_tok[p + 1] - r0;
+  const long long K = kind == 3 ? (long long)n * a.d : a.d;
+  const __nv_bfloat16 *w = a.task_head_W[t] + (size_t)o * K;
+  float acc = 0.0f;
+  if (kind == 3) {
+    const __nv_bfloat16 *f = a.Fn + (size_t)r0 * a.d;
+    for (long long c = lane * 8; c < K; c += 256) {
+      const uint4 wv = *reinterpret_cast<const uint4 *>(w + c), fv = *reinterpret_cast<const uint4 *>(f + c);
+      acc += bf16_lo(wv.x) * bf16_lo(fv.x) + bf16_hi(wv.x) * bf16_hi(fv.x) + bf16_lo(wv.y) * bf16_lo(fv.y) +
+             bf16_hi(wv.y) * bf16_hi(fv.y) + bf16_lo(wv.z) * bf16_lo(fv.z) + bf16_hi(wv.z) * bf16_hi(fv.z) +
+             bf16_lo(wv.w) * bf16_lo(fv.w) + bf16_hi(wv.w) * bf16_hi(fv.w);
+    }
+  } else {
+    const float *f = a.feat + (size_t)p * a.d;
+    for (int c = lane * 8; c < a.d; c += 256) {
+      const uint4 wv = *reinterpret_cast<const uint4 *>(w + c);
+      const float4 f0 = *reinterpret_cast<const float4 *>(f + c), f1 = *reinterpret_cast<const float4 *>(f + c + 4);
+      acc += bf16_lo(wv.x) * f0.x + bf16_hi(wv.x) * f0.y + bf16_lo(wv.y) * f0.z + bf16_hi(wv.y) * f0.w +
+             bf16_lo(wv.z) * f1.x + bf16_hi(wv.z) * f1.y + bf16_lo(wv.w) * f1.z + bf16_hi(wv.w) * f1.w;
+    }
+  }
+#pragma unroll
+  for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
+  if (lane == 0) {
+    const __nv_bfloat16 *b = a.task_head_b[t];
+    a.out[a.out_off[a.perm[p]] + o] = acc + (b ? __bfloat162float(b[o]) : 0.0f);
+  }
+}
+
+}  // namespace fmx

@@ -1,0 +1,114 @@
+"""Session: upload a seeded `fmx_workloads.Workload` to the GPU and run it through libfmx.
+
+Marshalling only — torch provides device memory and streams; every compute step is in libfmx.
+"""
+import numpy as np
+import torch
+
+from fmx_workloads import Workload, target_dims
+from .binding import ACT, HEAD_KIND, INPUT_KIND, NORM, TARGET, Fmx
+
+
+def _dev_bf16(bits, device):
+    """uint16 bf16 bit patterns -> torch.bfloat16 tensor on the device (same bits)."""
+    t = torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).to(device)
+    return t.view(torch.bfloat16)
+
+
+class Session:
+    def __init__(self, wl: Workload, device=0, fmx: Fmx = None, max_req=None, max_tokens=None):
+        self.wl = wl
+        self.dev = torch.device("cuda", device)
+        torch.cuda.set_device(self.dev)
+        self.fmx = fmx or Fmx(device)
+        self._weights = {}
+        self.bb = self._register_backbone()
+        self.task_ids_of = [self._register_task(t) for t in range(len(wl.tasks))]
+        B = max_req or wl.n_req
+        N = max_tokens or max(wl.n_tokens, 1)
+        self.ws_bytes = self.fmx.workspace_bytes(self.bb, B, N)
+        self.workspace = torch.empty(self.ws_bytes + 1024, dtype=torch.uint8, device=self.dev)
+        self.ws_ptr = (self.workspace.data_ptr() + 1023) // 1024 * 1024
+        self.inputs_dev = None
+        self.out_dev = None
+
+    # ------------------------------------------------------------------ registration
+    def _w(self, name):
+        if name not in self._weights:
+            self._weights[name] = _dev_bf16(self.wl.tensor(name), self.dev)
+        return self._weights[name].data_ptr()
+
+    def _register_backbone(self):
+        wl, bb = self.wl, self.wl.bb
+        L = bb.n_layers
+        fields = dict(n_layers=L, d_model=bb.d_model, n_q_heads=bb.n_q_heads, n_kv_heads=bb.n_kv_heads,
+                      head_dim=bb.head_dim, d_ffn=bb.d_ffn, act=ACT[bb.act], norm=NORM[bb.norm], norm_eps=bb.norm_eps,
+                      causal=int(bb.causal), rope_theta=bb.rope_theta, input_kind=INPUT_KIND[bb.input_kind],
+                      patch_dim=bb.patch_dim, tokens_per_request=bb.tokens_per_request, has_cls=int(bb.has_cls),
+                      vocab=bb.vocab, max_seq=bb.max_seq, img_c=bb.img_c, img_hw=bb.img_hw, patch_hw=bb.patch_hw)
+        lay = lambda n: [self._w(f"L{l:02d}.{n}") for l in range(L)]
+        per_layer = dict(norm1_g=lay("norm1.g"), norm2_g=lay("norm2.g"), Wq=lay("Wq"), Wk=lay("Wk"), Wv=lay("Wv"),
+                         Wo=lay("Wo"), Wup=lay("Wup"), Wdown=lay("Wdown"),
+                         Wgate=lay("Wgate") if bb.act == "swiglu" else None,
+                         norm1_b=lay("norm1.b") if bb.norm == "ln" else None,
+                         norm2_b=lay("norm2.b") if bb.norm == "ln" else None)
+        for b in ("bq", "bk", "bv", "bo", "bup", "bdown"):
+            per_layer[b] = lay(b) if bb.has_bias else None
+        per_layer["bgate"] = lay("bgate") if (bb.has_bias and bb.act == "swiglu") else None
+        singles = dict(final_g=self._w("final.g"), final_b=self._w("final.b") if bb.norm == "ln" else None,
+                       embed_W=self._w("embed.W") if bb.input_kind == "patch" else None,
+                       embed_b=self._w("embed.b") if bb.input_kind == "patch" else None,
+                       embed_cls=self._w("embed.cls") if bb.has_cls else None,
+                       embed_pos=self._w("embed.pos") if bb.pos_kind != "none" else None,
+                       embed_table=self._w("embed.table") if bb.input_kind == "tokens" else None)
+        return self.fmx.register_backbone(fields, per_layer, singles)
+
+    def _register_task(self, t):
+        wl, bb = self.wl, self.wl.bb
+        ts = wl.tasks[t]
+        tmp = []
+        def up(name):
+            x = _dev_bf16(wl.tensor(name), self.dev)
+            tmp.append(x)
+            return x.data_ptr()
+        adapters = []
+        for ad in ts.adapters:
+            A = [up(f"task{t:03d}.L{l:02d}.{ad.target}.A") for l in range(bb.n_layers)]
+            Bm = [up(f"task{t:03d}.L{l:02d}.{ad.target}.B") for l in range(bb.n_layers)]
+            adapters.append((TARGET[ad.target], ad.rank, float(ad.scaling), A, Bm))
+        tid = self.fmx.register_task(self.bb, adapters, HEAD_KIND[ts.head_kind], ts.head_out,
+                                     up(f"task{t:03d}.head.W"), up(f"task{t:03d}.head.b"))
+        del tmp      # the library copied everything into its arena
+        return tid
+
+    # ------------------------------------------------------------------ running
+    def upload_inputs(self, packed=None):
+        packed = self.wl.packed_inputs() if packed is None else packed
+        raw = np.ascontiguousarray(packed)
+        self.inputs_host = torch.from_numpy(raw.view(np.int16) if raw.dtype == np.uint16 else raw).pin_memory()
+        self.inputs_dev = self.inputs_host.to(self.dev)
+        return self.inputs_dev
+
+    def forward(self, task_ids=None, lengths=None, stream=None):
+        """Enqueue one mixed forward on the current (or given) stream; returns the device output tensor."""
+        wl = self.wl
+        ids = wl.task_ids if task_ids is None else task_ids
+        ids = np.asarray([self.task_ids_of[int(t)] for t in ids], dtype=np.int32)
+        lens = wl.lengths if lengths is None else lengths
+        if self.inputs_dev is None:
+            self.upload_inputs()
+        off = self.fmx.output_layout(ids)
+        if self.out_dev is None or self.out_dev.numel() < int(off[-1]):
+            self.out_dev = torch.empty(max(int(off[-1]), 1), dtype=torch.float32, device=self.dev)
+        s = stream if stream is not None else torch.cuda.current_stream(self.dev)
+        self.fmx.forward_mixed(self.bb, self.inputs_dev.data_ptr(), ids, lens, self.out_dev.data_ptr(), self.ws_ptr,
+                               self.ws_bytes, s.cuda_stream)
+        self.last_off = off
+        return self.out_dev
+
+    def forward_numpy(self, task_ids=None, lengths=None):
+        """Run and return a list of per-request fp32 output vectors (original request order)."""
+        out = self.forward(task_ids, lengths)
+        torch.cuda.synchronize(self.dev)
+        flat = out.cpu().numpy()
+        return [flat[self.last_off[i]:self.last_off[i + 1]].copy() for i in range(len(self.last_off) - 1)]
