@@ -1,0 +1,280 @@
+"""GPU parity tests (run on the B200 box): the CUDA path, called through the C ABI (ctypes
+binding), against the fp64 oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star): max-abs error <= 2e-2 and per-row cosine >= 0.999 for the
+outputs (bf16 storage, fp32 accumulate); segment tables bit-exact.  Because cfg1's outputs are
+~0.04 in magnitude, every parity check additionally bounds the error RELATIVE to the output
+scale (max-abs / rms <= 0.05), which is the binding bar on the small configs.
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from fmx_workloads import bf16_bits_to_f64, f32_to_bf16_bits, make_workload  # noqa: E402
+from oracle import from_workload as G  # noqa: E402
+from oracle.segments import segment_tables  # noqa: E402
+
+MAX_ABS, MIN_COS, MAX_REL = 2e-2, 0.999, 0.05
+
+
+@pytest.fixture(scope="module")
+def fmx_mod():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test needs a CUDA device; the product has no CPU fallback")
+    import paper_2606_09643_b200 as pkg
+    return pkg
+
+
+def _session(fmx_mod, wl, **kw):
+    from paper_2606_09643_b200.session import Session
+    return Session(wl, **kw)
+
+
+def check_parity(y, ref, label=""):
+    """y, ref: lists of per-request vectors."""
+    assert len(y) == len(ref)
+    flat_ref = np.concatenate(ref)
+    rms = float(np.sqrt(np.mean(flat_ref ** 2)))
+    mx = max(float(np.abs(a - b).max()) for a, b in zip(y, ref))
+    assert all(np.isfinite(a).all() for a in y), f"{label}: non-finite output"
+    assert mx <= MAX_ABS, f"{label}: max-abs {mx:.3e} > {MAX_ABS}"
+    assert mx <= MAX_REL * rms, f"{label}: max-abs {mx:.3e} > {MAX_REL} * rms {rms:.3e}"
+    for i, (a, b) in enumerate(zip(y, ref)):
+        if len(b) > 1:                      # rows with o_t = 1 are checked by max-abs only (reading 22)
+            cos = float(a @ b / (np.linalg.norm(a) * np.linalg.norm(b) + 1e-300))
+            assert cos >= MIN_COS, f"{label}: request {i} cosine {cos:.6f} < {MIN_COS}"
+    return mx, rms
+
+
+def check_segments(s, wl):
+    seg = s.fmx.debug_get_segments(wl.n_req)
+    ids = np.array([s.task_ids_of[int(t)] for t in wl.task_ids])
+    ref = segment_tables(ids, wl.lengths, s.fmx.task_slots())
+    for k, v in ref.items():
+        assert seg[k].dtype == np.int32 and np.array_equal(seg[k], v), f"segment table {k} differs"
+    # the private (row-tile, task) block table: valid cover of every tile by same-task row ranges
+    n_tiles, n_blk, blocks = s.fmx.debug_get_tiles()
+    N = wl.n_tokens
+    assert n_tiles == (N + 127) // 128
+    covered = np.zeros(n_tiles * 128, dtype=np.int32)
+    row_task = np.repeat(ids[ref["perm"]], wl.lengths[ref["perm"]])
+    prev = (-1, -1)
+    for tile, task, lo, hi in blocks:
+        assert (tile, task) > prev and 0 <= lo < hi <= 128
+        prev = (tile, task)
+        rows = np.arange(tile * 128 + lo, tile * 128 + hi)
+        assert rows[-1] < N and np.all(row_task[rows] == task)
+        covered[rows] += 1
+    assert np.all(covered[:N] == 1) and np.all(covered[N:] == 0)
+    return seg
+
+
+# ---------------------------------------------------------------- the tcgen05 GEMM alone
+@pytest.mark.parametrize("M,N,K", [(128, 128, 64), (300, 384, 192), (1000, 512, 1024), (257, 256, 592), (4096, 1024, 1024),
+                                   (1, 128, 8), (129, 640, 72)])
+def test_tcgen05_gemm_matches_fp64(fmx_mod, M, N, K):
+    fmx = fmx_mod.Fmx(0)
+    rng = np.random.default_rng(M * 7 + N * 3 + K)
+    a = f32_to_bf16_bits(rng.standard_normal((M, K)).astype(np.float32))
+    w = f32_to_bf16_bits(rng.standard_normal((N, K)).astype(np.float32))
+    A = torch.from_numpy(a.view(np.int16)).cuda()
+    W = torch.from_numpy(w.view(np.int16)).cuda()
+    Cout = torch.full((M, N), float("nan"), dtype=torch.float32, device="cuda")
+    fmx.debug_gemm(A.data_ptr(), W.data_ptr(), Cout.data_ptr(), M, N, K)
+    torch.cuda.synchronize()
+    ref = bf16_bits_to_f64(a) @ bf16_bits_to_f64(w).T
+    got = Cout.cpu().numpy().astype(np.float64)
+    # fp32 accumulation of K products of O(1) terms: error << 1e-3 * sqrt(K)
+    assert np.isfinite(got).all() and np.abs(got - ref).max() <= 2e-5 * K ** 0.5 * 4
+
+
+# ---------------------------------------------------------------- config 1 in full
+def test_cfg1_full_parity_and_segments(fmx_mod):
+    wl = make_workload("cfg1")
+    s = _session(fmx_mod, wl)
+    y = s.forward_numpy()
+    check_segments(s, wl)
+    mx, rms = check_parity(y, G.oracle_outputs(wl), "cfg1")
+    assert mx < 1e-3          # far inside the bar: bf16 rounding on 0.04-scale outputs
+    assert s.fmx.last_launch_count() > 0
+
+
+@pytest.mark.parametrize("cfg,kw", [
+    ("cfg1", dict(lora_std=0.25)),                                  # stress: adapters dominate
+    ("cfg2", dict(n_layers=2, batch=20)),                           # 20*64 = 1280 rows: 10 tiles, flatten + mean heads
+    ("cfg2", dict(n_layers=2, batch=7, lora_std=0.1)),              # ragged last tile (448 rows), stress adapters
+    ("cfg3", dict(n_layers=2, batch=6)),                            # 1542 rows: ragged tail, CLS, image patchify, LN + bias
+    ("cfg4", dict(n_layers=2, batch=8, max_len=200)),               # varlen causal GQA RoPE SwiGLU, 7 targets, ranks to 64
+    ("cfg5", dict(n_layers=2, batch=24, n_tasks=16, dist="zipf1.5")),
+])
+def test_reduced_configs_parity(fmx_mod, cfg, kw):
+    wl = make_workload(cfg, **kw)
+    s = _session(fmx_mod, wl)
+    y = s.forward_numpy()
+    check_segments(s, wl)
+    check_parity(y, G.oracle_outputs(wl), f"{cfg} {kw}")
+
+
+# ---------------------------------------------------------------- full sizes, sampled outputs
+@pytest.mark.parametrize("cfg,kw,n_sample", [
+    ("cfg2", {}, 6),
+    ("cfg3", {}, 3),
+    ("cfg5", dict(n_tasks=92, dist="zipf0.8"), 4),
+    ("cfg5", dict(n_tasks=1), 2),
+])
+def test_full_size_sampled_parity(fmx_mod, cfg, kw, n_sample):
+    """BASELINE.json's full sizes in the launch configuration bench.py times; the oracle computes
+    a seeded sample of requests one by one (requests are independent by definition)."""
+    wl = make_workload(cfg, **kw)
+    s = _session(fmx_mod, wl)
+    y = s.forward_numpy()
+    check_segments(s, wl)
+    rng = np.random.default_rng(1)
+    idx = sorted(rng.choice(wl.n_req, size=n_sample, replace=False).tolist())
+    ref = G.oracle_outputs(wl, idx)
+    check_parity([y[i] for i in idx], ref, f"{cfg} full {kw}")
+    assert all(np.isfinite(v).all() for v in y)
+
+
+def test_cfg4_full_size_sampled_parity(fmx_mod):
+    """cfg4 at full depth/width with all 92 tasks registered; batch of 64 variable-length prompts;
+    the oracle checks the two shortest requests and one mid-length one."""
+    wl = make_workload("cfg4")
+    s = _session(fmx_mod, wl)
+    y = s.forward_numpy()
+    check_segments(s, wl)
+    order = np.argsort(wl.lengths)
+    idx = sorted([int(order[0]), int(order[1]), int(order[len(order) // 3])])
+    ref = G.oracle_outputs(wl, idx)
+    check_parity([y[i] for i in idx], ref, "cfg4 full")
+
+
+# ---------------------------------------------------------------- invariants on the GPU
+def test_mixed_equals_separate_and_order_invariance(fmx_mod):
+    wl = make_workload("cfg2", n_layers=2, batch=24, lora_std=0.1)
+    s = _session(fmx_mod, wl)
+    mixed = s.forward_numpy()
+    per_req = wl.bb.n_patches * wl.bb.patch_dim
+    packed = wl.packed_inputs().reshape(wl.n_req, per_req)
+    # (a) each task alone on its own requests: bit-identical to its rows of the mixed batch
+    for t in sorted(set(wl.task_ids.tolist())):
+        sel = np.nonzero(wl.task_ids == t)[0]
+        s.upload_inputs(packed[sel].reshape(-1))
+        alone = s.forward_numpy(task_ids=wl.task_ids[sel], lengths=wl.lengths[sel])
+        for j, i in enumerate(sel):
+            assert np.array_equal(alone[j], mixed[i]), f"task {t} request {i}: mixed != separate"
+    # (b) permuted request order, outputs un-permuted: bit-identical
+    perm = np.random.default_rng(5).permutation(wl.n_req)
+    s.upload_inputs(packed[perm].reshape(-1))
+    shuffled = s.forward_numpy(task_ids=wl.task_ids[perm], lengths=wl.lengths[perm])
+    for p, i in enumerate(perm):
+        assert np.array_equal(shuffled[p], mixed[i])
+
+
+def test_zero_adapter_reproduces_backbone_only(fmx_mod):
+    wl_on = make_workload("cfg1", lora_std=0.25)
+    wl_off = make_workload("cfg1", adapters=False, lora_std=0.25)
+    y_on = _session(fmx_mod, wl_on).forward_numpy()
+    y_off = _session(fmx_mod, wl_off).forward_numpy()
+    check_parity(y_off, G.oracle_outputs(wl_off), "cfg1 adapter-free")
+    assert max(np.abs(a - b).max() for a, b in zip(y_on, y_off)) > 1e-3     # the adapters do matter here
+    # registering zero-B adapters must give the adapter-free result exactly
+    class ZeroB(type(wl_on)):
+        def tensor(self, name):
+            x = super().tensor(name)
+            return np.zeros_like(x) if name.endswith(".B") else x
+    wl_zero = ZeroB(**wl_on.__dict__)
+    y_zero = _session(fmx_mod, wl_zero).forward_numpy()
+    for a, b in zip(y_zero, y_off):
+        assert np.array_equal(a, b)
+
+
+def test_task_lifecycle_isolation(fmx_mod):
+    """Registering an extra task / unregistering an unrelated one leaves other tasks' outputs
+    bit-identical (PAPER.md L92 lifecycle decoupling, L150 remove_adapter)."""
+    wl = make_workload("cfg2", n_layers=2, batch=12)
+    s = _session(fmx_mod, wl)
+    before = s.forward_numpy()
+    extra = s._register_task(0)                        # a duplicate of task 0 under a new id
+    assert extra == len(wl.tasks)
+    mid = s.forward_numpy()
+    s.fmx.unregister_task(extra)
+    victim = max(set(range(len(wl.tasks))) - set(wl.task_ids.tolist()), default=None)
+    if victim is not None:
+        s.fmx.unregister_task(s.task_ids_of[victim])
+    after = s.forward_numpy()
+    for a, b, c in zip(before, mid, after):
+        assert np.array_equal(a, b) and np.array_equal(a, c)
+    # the freed slot is reused lowest-first and works
+    again = s._register_task(0)
+    assert again == (s.task_ids_of[victim] if victim is not None and s.task_ids_of[victim] < extra else extra)
+
+
+# ---------------------------------------------------------------- edge cases and errors
+def test_edge_cases(fmx_mod):
+    wl = make_workload("cfg4", n_layers=1, batch=5, max_len=130, n_tasks=6)
+    s = _session(fmx_mod, wl, max_req=16, max_tokens=4096)
+    # single request, length 1 (causal attention of one token returns v)
+    toks = np.array([17], dtype=np.int32)
+    s.upload_inputs(toks)
+    y = s.forward_numpy(task_ids=np.array([2]), lengths=np.array([1]))
+    bb, get, tasks = G.bb_dict(wl), G.make_get(wl), G.task_dicts(wl)
+    from oracle.vfm_forward import forward_request
+    check_parity(y, [forward_request(bb, get, tasks[2], toks)], "len-1 request")
+    # all requests of one task; maximum length; registered-but-absent tasks give empty segments
+    L = wl.bb.max_seq
+    rng = np.random.default_rng(3)
+    toks = rng.integers(0, wl.bb.vocab, size=L + 64, dtype=np.int32)
+    s2 = _session(fmx_mod, wl, max_req=4, max_tokens=L + 64)
+    s2.upload_inputs(toks)
+    y = s2.forward_numpy(task_ids=np.array([5, 5]), lengths=np.array([L, 64]))
+    seg = s2.fmx.debug_get_segments(2)
+    assert seg["task_req_off"].tolist() == [0, 0, 0, 0, 0, 0, 2]
+    ref = [forward_request(bb, get, tasks[5], toks[:L]), forward_request(bb, get, tasks[5], toks[L:])]
+    check_parity(y, ref, "max-length + short request")
+
+
+def test_error_paths_enqueue_nothing(fmx_mod):
+    wl = make_workload("cfg1")
+    s = _session(fmx_mod, wl)
+    good = s.forward_numpy()
+    E = fmx_mod.FmxError
+    ids, lens = wl.task_ids.copy(), wl.lengths.copy()
+    with pytest.raises(E) as e:
+        bad = lens.copy(); bad[3] = 63
+        s.forward(lengths=bad)
+    assert e.value.code == -5
+    with pytest.raises(E) as e:
+        s.fmx.forward_mixed(s.bb, s.inputs_dev.data_ptr(), np.array([0, 99]), np.array([64, 64]), s.out_dev.data_ptr(), s.ws_ptr, s.ws_bytes)
+    assert e.value.code == -3
+    with pytest.raises(E) as e:
+        s.fmx.forward_mixed(s.bb, s.inputs_dev.data_ptr(), ids, lens, s.out_dev.data_ptr(), s.ws_ptr, 4096)
+    assert e.value.code == -6
+    with pytest.raises(E) as e:
+        s.fmx.forward_mixed(7, s.inputs_dev.data_ptr(), ids, lens, s.out_dev.data_ptr(), s.ws_ptr, s.ws_bytes)
+    assert e.value.code == -2
+    s.fmx.forward_mixed(s.bb, s.inputs_dev.data_ptr(), ids[:0], lens[:0], s.out_dev.data_ptr(), s.ws_ptr, s.ws_bytes)   # n_req = 0: OK, no launch
+    with pytest.raises(E) as e:                                       # rank 65 is refused, nothing registered
+        s.fmx.register_task(s.bb, [(0, 65, 1.0, [1] * wl.bb.n_layers, [1] * wl.bb.n_layers)], 0, 3, 1, None)
+    assert e.value.code == -4
+    again = s.forward_numpy()
+    for a, b in zip(good, again):
+        assert np.array_equal(a, b)
+
+
+def test_host_buffer_forward_matches_device_forward(fmx_mod):
+    wl = make_workload("cfg2", n_layers=1, batch=9)
+    s = _session(fmx_mod, wl)
+    dev = s.forward_numpy()
+    packed = wl.packed_inputs()
+    host_in = torch.from_numpy(packed.view(np.int16)).pin_memory()
+    ids = np.array([s.task_ids_of[int(t)] for t in wl.task_ids], dtype=np.int32)
+    off = s.fmx.output_layout(ids)
+    host_out = torch.empty(int(off[-1]), dtype=torch.float32).pin_memory()
+    s.fmx.forward_mixed_host(s.bb, host_in.data_ptr(), packed.nbytes, ids, wl.lengths, host_out.data_ptr(), s.ws_ptr, s.ws_bytes,
+                             torch.cuda.current_stream().cuda_stream)
+    got = host_out.numpy()
+    for i in range(wl.n_req):
+        assert np.array_equal(got[off[i]:off[i + 1]], dev[i])
