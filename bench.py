@@ -1,0 +1,382 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the mixed-task vFM forward (fmx_forward_mixed) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2|cfg3|cfg4|cfg5|sweep5]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+    python bench.py --impl reference ...        # the fp64 CPU oracle on the host cores
+
+A step is one pass of the whole hot path (S1 task sort .. S6 output scatter) over
+one synthetic mixed batch.  The default workload is BASELINE.json configs[1] ("cfg2": T5-large-
+encoder-shaped time-series backbone, batch 256, 10 tasks, Zipf(1.1) task ids); configs[0] is the
+tiny parity case and the other configs are selectable with --workload.  Rank 0 prints ONE JSON line.
+
+  value      whole-job samples/s, inputs resident in HBM, CUDA events around every step on the
+             launching stream, L2 flushed (256 MB memset) between steps outside the events.
+  e2e        the same metric through fmx_forward_mixed_host: pinned HOST inputs -> device, forward,
+             outputs -> HOST, inside the timed region (wall clock around the synchronous calls).
+  roofline   the tcgen05 GEMM kernel (all four projection families): algorithmic FLOPs per launch
+             / average launch duration from CUDA events recorded around those launches INSIDE the
+             timed region, against MEASURED_PEAKS.json (sustained bf16 figure: the kernel is timed
+             inside a long step; the burst fraction is given too).
+  cpu_baseline  the oracle (numpy fp64, as it stands) on a bounded sample of the same workload.
+
+Multi-GPU is replicas only: every rank runs the same batch shape on its own GPU, no
+data-path collective; value = units of all ranks / max-over-ranks time; scaling "weak".
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "mixed-task samples/s per B200 and % of bf16 tensor peak vs #co-batched tasks"
+GEMM_FAMILIES = ("gemm_qkv", "gemm_o", "gemm_ffn_in", "gemm_ffn_out")
+WORKLOAD_NAMES = {
+    "cfg2": "configs[1]: T5-large-encoder-shaped time-series backbone (24L d1024 FFN4096 ReLU RMSNorm), batch 256 x 64 tokens, "
+            "10 tasks, rank-8 LoRA on q/k/v/o, forecast (flatten->96) or mean-pool heads, task ids Zipf(1.1)",
+    "cfg3": "configs[2]: ViT-L/14-shaped vision backbone, batch 128 x 257 tokens, 32 tasks, rank 8/16 LoRA on q/k/v/o, CLS heads",
+    "cfg4": "configs[3]: decoder-only LM prefill (28L d1536 GQA 12/2 SwiGLU 8960 RoPE causal), batch 64, lengths U[64,1024], "
+            "92 tasks, LoRA rank {4..64} on 7 targets, last-token heads, task ids Zipf(1.0)",
+    "cfg5": "configs[4]: task-count/skew sweep point on the cfg2 backbone, batch 512",
+}
+
+
+def peaks():
+    """Measured roofline denominators (driver-written), else the profiling guide's fallback."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(source="measured", hbm_gbs=float(d["hbm_gbs"]), bf16_tflops=float(d["bf16_tflops"]),
+                    bf16_tflops_sustained=float(d.get("bf16_tflops_sustained", d["bf16_tflops"])))
+    return dict(source="fallback", hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (profiling recipe)."""
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "20"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+        self.t0 = self.t1 = None
+
+    def start(self):
+        self.t0 = time.time()
+
+    def stop(self):
+        self.t1 = time.time()
+
+    def result(self):
+        import datetime
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.05)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.strip().split(", ") for r in open(self.f.name) if r.strip()]
+        os.unlink(self.f.name)
+        inside, allr = [], []
+        for r in rows:
+            if len(r) < 8:
+                continue
+            try:
+                ts = datetime.datetime.strptime(r[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                rec = (ts, float(r[1]), float(r[2]), float(r[3]), r[4:8])
+            except ValueError:
+                continue
+            allr.append(rec)
+            if self.t0 - 0.01 <= ts <= self.t1 + 0.01:
+                inside.append(rec)
+        use = inside or allr
+        if not use:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm = sorted(x[1] for x in use)
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        reasons = [n for k, n in enumerate(names) if any(x[4][k].strip().lower().startswith("active") for x in use)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": use[0][2], "power_w_max": max(x[3] for x in use), "samples": len(use),
+                "samples_in_timed_region": len(inside), "reasons": reasons}
+
+
+def build_workload(args):
+    from fmx_workloads import make_workload
+    if args.workload == "cfg5":
+        return make_workload("cfg5", n_tasks=args.tasks, dist=args.dist, adapters=not args.no_adapters)
+    return make_workload(args.workload)
+
+
+# ------------------------------------------------------------------------------------- the oracle legs
+def oracle_time(wl, idx, get=None, warm=True):
+    """Seconds the oracle (as it stands) takes for requests idx; weights widened to fp64 beforehand."""
+    from oracle import from_workload as G
+    from oracle.vfm_forward import forward_requests
+    get = get or G.make_get(wl, max_cached_bytes=12 << 30)
+    if warm:
+        for name in wl.backbone_tensor_names():
+            get(name)
+        for t in sorted({int(wl.task_ids[i]) for i in idx}):
+            for name in wl.task_tensor_names(t):
+                get(name)
+    inputs = G.request_inputs(wl, idx)
+    bb, tasks = G.bb_dict(wl), G.task_dicts(wl)
+    t0 = time.perf_counter()
+    out = forward_requests(bb, get, tasks, [int(wl.task_ids[i]) for i in idx], inputs)
+    return time.perf_counter() - t0, out
+
+
+def blas_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [p.get("num_threads", 0) for p in threadpool_info() if p.get("user_api") == "blas"]
+        if n:
+            return max(n)
+    except Exception:
+        pass
+    return os.cpu_count()
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores; each step = a bounded sample of the workload."""
+    from paper_2606_09643_b200 import replicas
+    rank, _, world = replicas.env_world()
+    if rank != 0:
+        return 0
+    wl = build_workload(args)
+    n = min(args.ref_sample, wl.n_req)
+    times = []
+    from oracle import from_workload as G
+    get = G.make_get(wl, max_cached_bytes=12 << 30)
+    for s in range(args.warmup + args.steps):
+        idx = [(s * n + j) % wl.n_req for j in range(n)]
+        dt, _ = oracle_time(wl, idx, get=get, warm=True)
+        if s >= args.warmup:
+            times.append(dt)
+    total = sum(times)
+    v = n * len(times) / total
+    line = {"metric": METRIC, "value": v, "unit": "samples/s", "impl": "reference", "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD_NAMES.get(args.workload, args.workload), "sample": f"{n} requests per step"},
+            "cpu_baseline": {"value": v, "unit": "samples/s", "cores": blas_threads(), "kind": "oracle",
+                             "sample": f"{n} of {wl.n_req} requests per step, {len(times)} timed steps, weights widened to fp64 outside the clock"},
+            "e2e": {"value": v, "unit": "samples/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------- the CUDA arm
+def timed_steps(sess, torch, steps, flush):
+    """K steps, each bracketed by its own CUDA events on the launching stream; L2 flushed between
+    steps outside the events.  Returns total ms."""
+    e0 = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+    e1 = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+    for i in range(steps):
+        if flush is not None:
+            flush.zero_()
+        e0[i].record()
+        sess.forward()
+        e1[i].record()
+    torch.cuda.synchronize()
+    return sum(a.elapsed_time(b) for a, b in zip(e0, e1))
+
+
+def measure(args, wl, rank, local_rank, world, with_cpu_baseline=True):
+    import numpy as np
+    import torch
+    from paper_2606_09643_b200 import accounting, replicas
+    from paper_2606_09643_b200.session import Session
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libfmx has no CPU fallback (use --impl reference for the oracle)")
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    pk = peaks()
+    sess = Session(wl, device=local_rank)
+    sess.upload_inputs()
+    fl = accounting.flops(wl)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if not args.no_flush else None
+    B = wl.n_req
+
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    for _ in range(max(args.warmup, 3)):
+        sess.forward()
+    torch.cuda.synchronize()
+    launches_per_step = sess.fmx.last_launch_count()
+
+    # ---- timed region: K steps; events around the GEMM launches only (the roofline's kernel) ----
+    if not args.no_kernel_events:
+        sess.fmx.profile_select(GEMM_FAMILIES)
+        sess.fmx.profile_enable(True)
+    replicas.barrier()
+    torch.cuda.synchronize()
+    if sampler:
+        sampler.start()
+    ms_total = timed_steps(sess, torch, args.steps, flush)
+    torch.cuda.synchronize()
+    replicas.barrier()
+    if sampler:
+        sampler.stop()
+    gemm_prof = sess.fmx.profile_read() if not args.no_kernel_events else {}
+    sess.fmx.profile_enable(False)
+    ms_max = replicas.max_over_ranks(ms_total, dev if world > 1 else None)
+    value = replicas.whole_job_throughput(B, args.steps, ms_max, world)
+    clocks = sampler.result() if sampler else None
+
+    # ---- per-family breakdown (extra profiled steps, outside the timed region) ----
+    sess.fmx.profile_select(None)
+    sess.fmx.profile_enable(True)
+    n_prof = 3
+    for _ in range(n_prof):
+        if flush is not None:
+            flush.zero_()
+        sess.forward()
+    fam = sess.fmx.profile_read()
+    sess.fmx.profile_enable(False)
+    breakdown = {k: {"launches_per_step": n // n_prof, "ms_per_step": round(ms / n_prof, 4)} for k, (n, ms) in fam.items() if n}
+
+    # ---- e2e through the host-buffer entry point ----
+    packed = wl.packed_inputs()
+    host_in = torch.from_numpy(packed.view(np.int16) if packed.dtype == np.uint16 else packed).pin_memory()
+    ids = np.array([sess.task_ids_of[int(t)] for t in wl.task_ids], dtype=np.int32)
+    off = sess.fmx.output_layout(ids)
+    host_out = torch.empty(int(off[-1]), dtype=torch.float32).pin_memory()
+    stream = torch.cuda.current_stream().cuda_stream
+    e2e_steps = max(3, min(args.steps, 20))
+    for _ in range(2):
+        sess.fmx.forward_mixed_host(sess.bb, host_in.data_ptr(), packed.nbytes, ids, wl.lengths, host_out.data_ptr(), sess.ws_ptr,
+                                    sess.ws_bytes, stream)
+    replicas.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        if flush is not None:
+            flush.zero_()
+        sess.fmx.forward_mixed_host(sess.bb, host_in.data_ptr(), packed.nbytes, ids, wl.lengths, host_out.data_ptr(), sess.ws_ptr,
+                                    sess.ws_bytes, stream)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    e2e_ms_max = replicas.max_over_ranks(e2e_s * 1e3, dev if world > 1 else None)
+    e2e = {"value": replicas.whole_job_throughput(B, e2e_steps, e2e_ms_max, world), "unit": "samples/s",
+           "h2d_bytes_per_step": int(packed.nbytes + 8 * B), "d2h_bytes_per_step": int(off[-1]) * 4, "steps": e2e_steps,
+           "includes": "L2 flush memset between steps"}
+
+    # ---- roofline of the dominant kernel (tcgen05 GEMM, all four projection families) ----
+    roof = None
+    if gemm_prof:
+        n_l = sum(gemm_prof[f][0] for f in GEMM_FAMILIES)
+        ms_g = sum(gemm_prof[f][1] for f in GEMM_FAMILIES)
+        fl_g = sum(fl["families"][f] for f in GEMM_FAMILIES)            # per forward
+        avg_ms = ms_g / max(n_l, 1)
+        flops_per_launch = fl_g / accounting.gemm_launches_per_forward(wl)
+        achieved = flops_per_launch / (avg_ms * 1e-3) / 1e12
+        roof = {"kernel": "fmx::gemm_kernel (tcgen05/TMEM/TMA, fused LoRA expand)", "bound": "tensor", "achieved": round(achieved, 2),
+                "peak": pk["bf16_tflops_sustained"], "unit": "TFLOP/s", "frac": round(achieved / pk["bf16_tflops_sustained"], 4),
+                "peak_kind": f"{pk['source']} sustained bf16 (kernel timed inside a long step)",
+                "frac_of_burst_peak": round(achieved / pk["bf16_tflops"], 4), "traffic": None,
+                "flops_per_launch": flops_per_launch, "avg_launch_ms": round(avg_ms, 5), "launches_timed": n_l,
+                "share_of_step": round(ms_g / ms_total, 4),
+                "per_family_tflops": {f: round(fl["families"][f] * args.steps / (gemm_prof[f][1] * 1e-3) / 1e12, 1)
+                                      for f in GEMM_FAMILIES if gemm_prof[f][1] > 0}}
+    line = {"metric": METRIC, "value": round(value, 2), "unit": "samples/s", "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": round(ms_max / args.steps, 4), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": WORKLOAD_NAMES.get(args.workload, args.workload), "requests": B, "tokens": wl.n_tokens,
+                       "tasks": len(wl.tasks), "tasks_in_batch": int(len(set(wl.task_ids.tolist()))), "dist": wl.notes.get("dist"),
+                       "l2": "flushed (256 MB memset) between steps, outside the per-step events" if flush is not None else "no flush",
+                       "accumulate": "fp32 (TMEM), fp32 residual stream", "replicas": world},
+            "pct_bf16_tensor_peak": {"of_burst": round(100 * fl["total"] * world * args.steps / (ms_max * 1e-3) / 1e12 / pk["bf16_tflops"], 2),
+                                     "of_sustained": round(100 * fl["total"] * world * args.steps / (ms_max * 1e-3) / 1e12 / pk["bf16_tflops_sustained"], 2),
+                                     "algorithmic_tflop_per_step": round(fl["total"] / 1e12, 4), "peaks": pk["source"]},
+            "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "launches_per_step": launches_per_step,
+            "clocks": clocks, "roofline": roof, "breakdown": breakdown}
+    if with_cpu_baseline and rank == 0 and world == 1 and not args.no_cpu_baseline:
+        n = min(args.cpu_sample, B)
+        idx = list(range(n))
+        dt, ref = oracle_time(wl, idx)
+        # the same requests through the CUDA path: parity of the timed sample, reported not asserted
+        y = sess.forward_numpy()
+        mx = max(float(np.abs(y[i] - r).max()) for i, r in zip(idx, ref))
+        line["cpu_baseline"] = {"value": round(n / dt, 4), "unit": "samples/s", "cores": blas_threads(), "kind": "oracle",
+                                "sample": f"first {n} of {B} requests, one by one in numpy fp64 ({dt:.1f} s; weights widened before the clock)",
+                                "max_abs_vs_cuda": mx}
+    sess.fmx.destroy()
+    return line
+
+
+def run_sweep5(args, rank, local_rank, world):
+    """BASELINE.json configs[4]: T x distribution -> samples/s, ratio to the single-task batch."""
+    from fmx_workloads import make_workload
+    rows = []
+    ref = {}
+    for T, dist, ad in [(1, "uniform", True), (1, "uniform", False)] + [(T, d, True) for T in (4, 16, 48, 92)
+                                                                         for d in ("uniform", "zipf0.8", "zipf1.5")]:
+        wl = make_workload("cfg5", n_tasks=T, dist=dist, adapters=ad)
+        a = argparse.Namespace(**vars(args))
+        a.workload, a.tasks, a.dist, a.no_adapters = "cfg5", T, dist, not ad
+        line = measure(a, wl, rank, local_rank, world, with_cpu_baseline=False)
+        key = "single_task" if (T == 1 and ad) else ("adapter_free" if T == 1 else None)
+        if key:
+            ref[key] = line["value"]
+        rows.append({"tasks": T, "dist": dist, "adapters": ad, "samples_per_s": line["value"], "ms_per_step": line["ms_per_step"],
+                     "pct_peak_sustained": line["pct_bf16_tensor_peak"]["of_sustained"],
+                     "vs_single_task": round(line["value"] / ref["single_task"], 4) if "single_task" in ref else None,
+                     "vs_adapter_free": round(line["value"] / ref["adapter_free"], 4) if "adapter_free" in ref else None,
+                     "gemm_frac": line["roofline"]["frac"] if line["roofline"] else None})
+        last = line
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    if rank == 0:
+        json.dump(rows, open(os.path.join(ROOT, "gpurun_out", "sweep5.json"), "w"), indent=1)
+    last["config"]["workload"] = "configs[4] sweep; this line = T=92, Zipf(1.5); full table in gpurun_out/sweep5.json"
+    last["sweep"] = rows
+    return last
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="fmx", choices=["fmx", "reference"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5", "sweep5"])
+    ap.add_argument("--tasks", type=int, default=92, help="cfg5: number of co-batched tasks")
+    ap.add_argument("--dist", default="zipf0.8", choices=["uniform", "zipf0.8", "zipf1.5"])
+    ap.add_argument("--no-adapters", action="store_true", help="cfg5: head-only tasks (adapter-free reference)")
+    ap.add_argument("--no-flush", action="store_true")
+    ap.add_argument("--no-kernel-events", action="store_true", help="no per-GEMM events inside the timed region (no roofline)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-sample", type=int, default=24, help="requests the oracle is timed on (cpu_baseline)")
+    ap.add_argument("--ref-sample", type=int, default=4, help="--impl reference: requests per step")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    from paper_2606_09643_b200 import replicas
+    rank, local_rank, world = replicas.init()
+    if world != args.gpus and rank == 0:
+        sys.stderr.write(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; launch N>1 with torch.distributed.run\n")
+    if args.workload == "sweep5":
+        line = run_sweep5(args, rank, local_rank, world)
+    else:
+        line = measure(args, build_workload(args), rank, local_rank, world)
+    if rank == 0:
+        print(json.dumps(line))
+    replicas.finalize()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

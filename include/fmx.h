@@ -187,6 +187,9 @@ int fmx_task_slots(fmx_ctx *ctx);                 /* number of task slots (highe
  * and returns, per family, launches and total milliseconds since the last fmx_profile_enable(1). */
 enum { FMX_N_FAMILIES = 12 };
 int fmx_profile_enable(fmx_ctx *ctx, int on);
+/* Restricts the events to the families whose bit is set (bit f = family f; default all), so a timed
+ * region can carry events around its dominant kernels only. */
+int fmx_profile_select(fmx_ctx *ctx, uint32_t family_mask);
 int fmx_profile_read(fmx_ctx *ctx, int32_t *launches /*[FMX_N_FAMILIES]*/, double *total_ms /*[FMX_N_FAMILIES]*/);
 const char *fmx_profile_family_name(int family);
 /* Kernels launched by the last forward (the count bench.py reports as gpu_launches). */

@@ -62,7 +62,7 @@ _lib = None
 
 EXPORTS = ["fmx_create", "fmx_destroy", "fmx_last_error", "fmx_version", "fmx_register_backbone", "fmx_register_task",
            "fmx_unregister_task", "fmx_output_layout", "fmx_workspace_bytes", "fmx_forward_mixed", "fmx_forward_mixed_host",
-           "fmx_debug_get_segments", "fmx_debug_get_tiles", "fmx_debug_read", "fmx_task_slots", "fmx_profile_enable", "fmx_profile_read",
+           "fmx_debug_get_segments", "fmx_debug_get_tiles", "fmx_debug_read", "fmx_task_slots", "fmx_profile_enable", "fmx_profile_select", "fmx_profile_read",
            "fmx_profile_family_name", "fmx_last_launch_count", "fmx_debug_gemm", "fmx_bfq_create", "fmx_bfq_destroy",
            "fmx_bfq_set_task", "fmx_bfq_enqueue", "fmx_bfq_next_batch", "fmx_bfq_complete", "fmx_bfq_stats", "fmx_bfq_peek"]
 
@@ -95,6 +95,7 @@ def load():
     lib.fmx_task_slots.argtypes = [_vp]
     lib.fmx_debug_read.argtypes = [_vp, C.c_int, _vp, C.c_size_t]
     lib.fmx_profile_enable.argtypes = [_vp, C.c_int]
+    lib.fmx_profile_select.argtypes = [_vp, C.c_uint32]
     lib.fmx_profile_read.argtypes = [_vp, i32p, f64p]
     lib.fmx_last_launch_count.argtypes = [_vp]
     lib.fmx_debug_gemm.argtypes = [_vp, _vp, _vp, _vp, C.c_int32, C.c_int32, C.c_int32, _vp]
@@ -235,6 +236,12 @@ class Fmx:
 
     def profile_enable(self, on=True):
         _check(self.lib.fmx_profile_enable(self.h, 1 if on else 0))
+
+    def profile_select(self, families=None):
+        """families: iterable of family names (None = all) that get events while profiling is on."""
+        names = [self.lib.fmx_profile_family_name(i).decode() for i in range(N_FAMILIES)]
+        mask = 0xFFFFFFFF if families is None else sum(1 << names.index(f) for f in families)
+        _check(self.lib.fmx_profile_select(self.h, mask))
 
     def profile_read(self):
         n = np.zeros(N_FAMILIES, np.int32)

@@ -97,7 +97,9 @@ struct fmx_ctx {
   void *last_buf[7] = {nullptr}; size_t last_buf_bytes[7] = {0};
   // profiling
   bool prof_on = false;
+  uint32_t prof_mask = 0xFFFFFFFFu;        // families that get events while prof_on
   std::vector<ProfEvent> prof;
+  std::vector<cudaEvent_t> ev_pool;        // recycled events
   std::mutex mu;
 };
 
@@ -184,13 +186,19 @@ struct Launcher {
   fmx_ctx *c;
   cudaStream_t s;
   int count = 0;
-  cudaEvent_t pending = nullptr;
+  bool rec = false;
+  int get_event(cudaEvent_t *e) {
+    if (!c->ev_pool.empty()) { *e = c->ev_pool.back(); c->ev_pool.pop_back(); return FMX_OK; }
+    CU_OK(cudaEventCreate(e));
+    return FMX_OK;
+  }
   int begin(int family) {
     ++count;
-    if (c->prof_on) {
+    rec = c->prof_on && ((c->prof_mask >> family) & 1u);
+    if (rec) {
       ProfEvent pe{family, nullptr, nullptr};
-      CU_OK(cudaEventCreate(&pe.e0));
-      CU_OK(cudaEventCreate(&pe.e1));
+      if (int e = get_event(&pe.e0)) return e;
+      if (int e = get_event(&pe.e1)) return e;
       CU_OK(cudaEventRecord(pe.e0, s));
       c->prof.push_back(pe);
     }
@@ -198,7 +206,7 @@ struct Launcher {
   }
   int end() {
     CU_OK(cudaGetLastError());
-    if (c->prof_on) CU_OK(cudaEventRecord(c->prof.back().e1, s));
+    if (rec) CU_OK(cudaEventRecord(c->prof.back().e1, s));
     return FMX_OK;
   }
 };
@@ -410,6 +418,7 @@ int fmx_destroy(fmx_ctx *c) {
   cudaSetDevice(c->device);
   cudaDeviceSynchronize();
   for (auto &pe : c->prof) { cudaEventDestroy(pe.e0); cudaEventDestroy(pe.e1); }
+  for (auto e : c->ev_pool) cudaEventDestroy(e);
   for (auto &bp : c->bbs) {
     if (!bp) continue;
     cudaFree(bp->embed_Wpad); cudaFree(bp->posb); cudaFree(bp->rope_cs);
@@ -927,9 +936,16 @@ int fmx_profile_enable(fmx_ctx *c, int on) {
   if (!c) return fmx_fail(FMX_E_INVALID_ARG, "profile_enable: NULL ctx");
   std::lock_guard<std::mutex> lk(c->mu);
   CU_OK(cudaDeviceSynchronize());
-  for (auto &pe : c->prof) { cudaEventDestroy(pe.e0); cudaEventDestroy(pe.e1); }
+  for (auto &pe : c->prof) { c->ev_pool.push_back(pe.e0); c->ev_pool.push_back(pe.e1); }
   c->prof.clear();
   c->prof_on = on != 0;
+  return FMX_OK;
+}
+
+int fmx_profile_select(fmx_ctx *c, uint32_t family_mask) {
+  if (!c) return fmx_fail(FMX_E_INVALID_ARG, "profile_select: NULL ctx");
+  std::lock_guard<std::mutex> lk(c->mu);
+  c->prof_mask = family_mask;
   return FMX_OK;
 }
 
