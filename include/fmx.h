@@ -173,12 +173,12 @@ int fmx_forward_mixed_host(fmx_ctx *ctx, fmx_backbone_t bb, const void *inputs_h
  * n_slots = fmx_task_slots().  Any pointer may be NULL. */
 int fmx_debug_get_segments(fmx_ctx *ctx, int32_t *perm, int32_t *inv_perm, int32_t *task_req_off,
                            int32_t *cu_tok, int32_t *task_tok_off);
-/* Debug/test: the private row-tile table of the last forward: n_tiles, n_blocks, and per
- * block (tile, task, row_lo, row_hi) into blocks[4*n_blocks] (cap entries available). */
+/* Debug/test: the private row-tile table of the last forward (256-row CTA-pair tiles): n_tiles,
+ * n_blocks, and per block (tile, task, row_lo, row_hi) into blocks[4*n_blocks] (cap entries available). */
 int fmx_debug_get_tiles(fmx_ctx *ctx, int32_t *n_tiles, int32_t *n_blocks, int32_t *blocks, int32_t cap);
 /* Debug/test: copies an activation buffer of the LAST forward to HOST (synchronises).  which:
  * 0 X fp32 [N,d] (residual, task-sorted rows)  1 Xn bf16 [N,d]  2 QKV bf16 [N,d_qkv]  3 attention out
- * bf16 [N,d_q]  4 FFN hidden bf16 [N,d_ffn]  5 U bf16 [n_blk_cap*128,192]  6 pooled feature fp32 [B,d]. */
+ * bf16 [N,d_q]  4 FFN hidden bf16 [N,d_ffn]  5 U bf16 [n_blk_cap*256,192]  6 pooled feature fp32 [B,d]. */
 int fmx_debug_read(fmx_ctx *ctx, int which, void *host, size_t bytes);
 int fmx_task_slots(fmx_ctx *ctx);                 /* number of task slots (highest id ever live + 1) */
 

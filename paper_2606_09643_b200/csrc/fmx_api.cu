@@ -17,6 +17,7 @@
 #include "fmx.h"
 #include "gemm.cuh"
 #include "kernels.cuh"
+#include "pair_gemm.cuh"
 
 using namespace fmx;
 typedef __nv_bfloat16 bf16;
@@ -58,8 +59,9 @@ struct Backbone {
   bf16 *embed_Wpad = nullptr;              // [d, Kp]
   float *posb = nullptr;                   // [n_pos, d]
   float2 *rope_cs = nullptr;               // [max_seq, dh/2]
-  std::vector<CUtensorMap> mWq, mWk, mWv, mWo, mWup, mWgate, mWdown;
-  CUtensorMap mEmbedW;
+  // weight maps, [0] = box {64,128} (pair tile 256x256: one CTA loads a whole chunk), [1] = box {64,64} (256x128 tiles)
+  std::vector<CUtensorMap> mWq[2], mWk[2], mWv[2], mWo[2], mWup[2], mWgate[2], mWdown[2];
+  CUtensorMap mEmbedW[2];
   // LoRA slabs
   int Rcap = 0;
   std::vector<unsigned char> col_used;     // units of 16 columns
@@ -106,15 +108,16 @@ struct fmx_ctx {
 namespace {
 
 int encode_2d(fmx_ctx *c, CUtensorMap *m, const void *base, uint64_t rows, uint64_t cols, uint64_t ld_elems,
-              uint32_t box_rows) {
+              uint32_t box_rows, bool f32 = false) {
+  const uint64_t esz = f32 ? 4 : 2;
   cuuint64_t dims[2] = {cols, rows};
-  cuuint64_t strides[1] = {ld_elems * 2};
-  cuuint32_t box[2] = {64, box_rows};
+  cuuint64_t strides[1] = {ld_elems * esz};
+  cuuint32_t box[2] = {f32 ? 32u : 64u, box_rows};          // 128-byte inner box = one swizzle row
   cuuint32_t estr[2] = {1, 1};
   if ((reinterpret_cast<uintptr_t>(base) & 15) || (strides[0] & 15))
     return fmx_fail(FMX_E_INVALID_ARG, "tensor map: base %p / row stride %llu B not 16-byte aligned", base,
                     (unsigned long long)strides[0]);
-  CUresult r = c->encode(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), dims, strides, box, estr,
+  CUresult r = c->encode(m, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), dims, strides, box, estr,
                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fmx_fail(FMX_E_CUDA, "cuTensorMapEncodeTiled failed (%d) rows=%llu cols=%llu ld=%llu", (int)r,
@@ -149,7 +152,7 @@ Workspace carve(const Backbone &bb, void *base, int B, long long N, int T) {
   uint8_t *p = static_cast<uint8_t *>(base);
   size_t off = 0;
   auto take = [&](size_t bytes) { void *r = p ? p + off : nullptr; off = align_up(off + bytes, 1024); return r; };
-  w.n_tiles = (int)((N + 127) / 128);
+  w.n_tiles = (int)((N + kPairRows - 1) / kPairRows);        // 256-row pair tiles
   w.n_blk_cap = w.n_tiles + std::min(T, B);
   const fmx_backbone_desc &d = bb.d;
   w.t.task_ids = (int *)take(sizeof(int) * B);
@@ -175,7 +178,7 @@ Workspace carve(const Backbone &bb, void *base, int B, long long N, int T) {
   w.QKV = (bf16 *)take(sizeof(bf16) * N * bb.d_qkv);
   w.AttnO = (bf16 *)take(sizeof(bf16) * N * bb.d_q);
   w.Hid = (bf16 *)take(sizeof(bf16) * N * std::max(d.d_ffn, bb.Kp));     // also the patch-pack buffer
-  w.U = (bf16 *)take(sizeof(bf16) * (size_t)w.n_blk_cap * 128 * 192);
+  w.U = (bf16 *)take(sizeof(bf16) * (size_t)w.n_blk_cap * kPairRows * 192);
   w.feat = (float *)take(sizeof(float) * (size_t)B * d.d_model);
   w.bytes = off;
   return w;
@@ -250,16 +253,20 @@ bool norm_dim_supported(int d) {
   return d % 128 == 0 && (v == 1 || v == 2 || v == 4 || v == 6 || v == 8 || v == 12 || v == 16);
 }
 
-void launch_gemm(fmx_ctx *c, cudaStream_t s, const GemmParams &p) {
-  if (p.mode == GM_SHRINK) {
-    const int grid = c->sm_count;
-    gemm_kernel<128, gemm_stages<128, true>(), true><<<grid, kGemmThreads, gemm_smem_bytes<128, true>(), s>>>(p);
-  } else if (p.n_chunks % 2 == 0) {
-    const int tiles = p.n_mtiles * (p.n_chunks / 2);
-    gemm_kernel<256, gemm_stages<256, false>(), false><<<std::min(tiles, c->sm_count), kGemmThreads, gemm_smem_bytes<256, false>(), s>>>(p);
+void launch_shrink(fmx_ctx *c, cudaStream_t s, const GemmParams &p) {
+  shrink_kernel<kShrinkStages><<<c->sm_count, kGemmThreads, shrink_smem_bytes(), s>>>(p);
+}
+
+// Pair tiles 256 x 256 when the chunk count is even, else 256 x 128; one cluster of 2 CTAs per SM pair.
+bool pair_wide(const PairGemmParams &p) { return p.n_chunks % 2 == 0; }
+void launch_pair_gemm(fmx_ctx *c, cudaStream_t s, const PairGemmParams &p) {
+  const int pairs = c->sm_count / 2;
+  if (pair_wide(p)) {
+    const int tiles = p.n_ptiles * (p.n_chunks / 2);
+    pair_gemm_kernel<256><<<2 * std::min(tiles, pairs), kGemmThreads, pair_smem_bytes<256>(), s>>>(p);
   } else {
-    const int tiles = p.n_mtiles * p.n_chunks;
-    gemm_kernel<128, gemm_stages<128, false>(), false><<<std::min(tiles, c->sm_count), kGemmThreads, gemm_smem_bytes<128, false>(), s>>>(p);
+    const int tiles = p.n_ptiles * p.n_chunks;
+    pair_gemm_kernel<128><<<2 * std::min(tiles, pairs), kGemmThreads, pair_smem_bytes<128>(), s>>>(p);
   }
 }
 
@@ -270,9 +277,9 @@ void launch_attention(cudaStream_t s, int dh, dim3 grid, const AttnArgs &a) {
 }
 
 int set_kernel_attrs() {
-  CU_OK(cudaFuncSetAttribute(gemm_kernel<256, gemm_stages<256, false>(), false>, cudaFuncAttributeMaxDynamicSharedMemorySize, gemm_smem_bytes<256, false>()));
-  CU_OK(cudaFuncSetAttribute(gemm_kernel<128, gemm_stages<128, false>(), false>, cudaFuncAttributeMaxDynamicSharedMemorySize, gemm_smem_bytes<128, false>()));
-  CU_OK(cudaFuncSetAttribute(gemm_kernel<128, gemm_stages<128, true>(), true>, cudaFuncAttributeMaxDynamicSharedMemorySize, gemm_smem_bytes<128, true>()));
+  CU_OK(cudaFuncSetAttribute(pair_gemm_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<256>()));
+  CU_OK(cudaFuncSetAttribute(pair_gemm_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<128>()));
+  CU_OK(cudaFuncSetAttribute(shrink_kernel<kShrinkStages>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes()));
   CU_OK(cudaFuncSetAttribute(attention_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_smem_bytes<32>()));
   CU_OK(cudaFuncSetAttribute(attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_smem_bytes<64>()));
   CU_OK(cudaFuncSetAttribute(attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_smem_bytes<128>()));
@@ -294,7 +301,7 @@ int rebuild_slab_maps(fmx_ctx *c, Backbone &bb, int tg) {
     bf16 *A = bb.slabA[tg] + (size_t)l * bb.Rcap * bb.din[tg];
     bf16 *B = bb.slabB[tg] + (size_t)l * bb.dout[tg] * bb.Rcap;
     if (int e = encode_2d(c, &bb.mA[tg][l], A, bb.Rcap, bb.din[tg], bb.din[tg], 64)) return e;
-    if (int e = encode_2d(c, &bb.mB[tg][l], B, bb.dout[tg], bb.Rcap, bb.Rcap, 128)) return e;
+    if (int e = encode_2d(c, &bb.mB[tg][l], B, bb.dout[tg], bb.Rcap, bb.Rcap, 64)) return e;
   }
   return FMX_OK;
 }
@@ -482,16 +489,19 @@ int fmx_register_backbone(fmx_ctx *c, const fmx_backbone_desc *desc, fmx_backbon
         (d.act == FMX_ACT_SWIGLU && !b->Wgate[l]))
       return fmx_fail(FMX_E_INVALID_ARG, "register_backbone: NULL weight pointer in layer %d", l);
   }
-  b->mWq.resize(L); b->mWk.resize(L); b->mWv.resize(L); b->mWo.resize(L); b->mWup.resize(L); b->mWgate.resize(L); b->mWdown.resize(L);
-  for (int l = 0; l < L; ++l) {
-    int e;
-    if ((e = encode_2d(c, &b->mWq[l], b->Wq[l], dq, d.d_model, d.d_model, 128))) return e;
-    if ((e = encode_2d(c, &b->mWk[l], b->Wk[l], dkv, d.d_model, d.d_model, 128))) return e;
-    if ((e = encode_2d(c, &b->mWv[l], b->Wv[l], dkv, d.d_model, d.d_model, 128))) return e;
-    if ((e = encode_2d(c, &b->mWo[l], b->Wo[l], d.d_model, dq, dq, 128))) return e;
-    if ((e = encode_2d(c, &b->mWup[l], b->Wup[l], d.d_ffn, d.d_model, d.d_model, 128))) return e;
-    if (d.act == FMX_ACT_SWIGLU && (e = encode_2d(c, &b->mWgate[l], b->Wgate[l], d.d_ffn, d.d_model, d.d_model, 128))) return e;
-    if ((e = encode_2d(c, &b->mWdown[l], b->Wdown[l], d.d_model, d.d_ffn, d.d_ffn, 128))) return e;
+  for (int v = 0; v < 2; ++v) {
+    const uint32_t br = v == 0 ? 128 : 64;
+    b->mWq[v].resize(L); b->mWk[v].resize(L); b->mWv[v].resize(L); b->mWo[v].resize(L); b->mWup[v].resize(L); b->mWgate[v].resize(L); b->mWdown[v].resize(L);
+    for (int l = 0; l < L; ++l) {
+      int e;
+      if ((e = encode_2d(c, &b->mWq[v][l], b->Wq[l], dq, d.d_model, d.d_model, br))) return e;
+      if ((e = encode_2d(c, &b->mWk[v][l], b->Wk[l], dkv, d.d_model, d.d_model, br))) return e;
+      if ((e = encode_2d(c, &b->mWv[v][l], b->Wv[l], dkv, d.d_model, d.d_model, br))) return e;
+      if ((e = encode_2d(c, &b->mWo[v][l], b->Wo[l], d.d_model, dq, dq, br))) return e;
+      if ((e = encode_2d(c, &b->mWup[v][l], b->Wup[l], d.d_ffn, d.d_model, d.d_model, br))) return e;
+      if (d.act == FMX_ACT_SWIGLU && (e = encode_2d(c, &b->mWgate[v][l], b->Wgate[l], d.d_ffn, d.d_model, d.d_model, br))) return e;
+      if ((e = encode_2d(c, &b->mWdown[v][l], b->Wdown[l], d.d_model, d.d_ffn, d.d_ffn, br))) return e;
+    }
   }
   if (d.input_kind == FMX_INPUT_PATCH_LINEAR) {
     b->Kp = (d.patch_dim + 7) / 8 * 8;
@@ -503,7 +513,8 @@ int fmx_register_backbone(fmx_ctx *c, const fmx_backbone_desc *desc, fmx_backbon
     build_posb_kernel<<<(n_pos * d.d_model + 255) / 256, 256>>>(b->posb, (const bf16 *)d.embed_b, (const bf16 *)d.embed_cls,
                                                                    (const bf16 *)d.embed_pos, n_pos, d.d_model, d.has_cls);
     CU_OK(cudaGetLastError());
-    if (int e = encode_2d(c, &b->mEmbedW, b->embed_Wpad, d.d_model, b->Kp, b->Kp, 128)) return e;
+    if (int e = encode_2d(c, &b->mEmbedW[0], b->embed_Wpad, d.d_model, b->Kp, b->Kp, 128)) return e;
+    if (int e = encode_2d(c, &b->mEmbedW[1], b->embed_Wpad, d.d_model, b->Kp, b->Kp, 64)) return e;
   }
   if (d.rope_theta > 0) {
     const int n = d.max_seq * (d.head_dim / 2);
@@ -682,7 +693,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   CU_OK(cudaMemcpyAsync(w.t.task_ids, c->h_stage, sizeof(int) * B, cudaMemcpyHostToDevice, s));
   CU_OK(cudaMemcpyAsync(w.t.lengths, c->h_stage + FMX_MAX_REQUESTS, sizeof(int) * B, cudaMemcpyHostToDevice, s));
   SortArgs sa{};
-  sa.t = w.t; sa.B = B; sa.T = T; sa.n_tiles = w.n_tiles; sa.task_head_out = c->d_task_head_out;
+  sa.t = w.t; sa.B = B; sa.T = T; sa.n_tiles = w.n_tiles; sa.tile_rows = kPairRows; sa.task_head_out = c->d_task_head_out;
   if (d.input_kind == FMX_INPUT_EMBEDDED) { sa.in_per_tok = d.d_model; sa.in_per_req = 0; }
   else if (d.input_kind == FMX_INPUT_TOKEN_IDS) { sa.in_per_tok = 1; sa.in_per_req = 0; }
   else if (d.img_c) { sa.in_per_tok = 0; sa.in_per_req = (long long)d.img_c * d.img_hw * d.img_hw; }
@@ -691,25 +702,33 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   LAUNCH(Lh, F_SORT, (row_tables_kernel<<<(Ni + 255) / 256, 256, 0, s>>>(w.t.cu_tok, B, Ni, w.t.row_req, w.t.row_pos)));
 
   // ---- common GEMM parameter pieces ----
-  GemmParams base{};
-  base.M = Ni; base.n_mtiles = w.n_tiles;
-  base.tile_blk_off = w.t.tile_blk_off; base.blk_task = w.t.blk_task; base.blk_lo = w.t.blk_lo; base.blk_hi = w.t.blk_hi;
-  base.blk_tile = w.t.blk_tile; base.n_blk = w.t.n_blk;
-  base.task_coff = c->d_task_coff; base.task_trpad = c->d_task_trpad; base.task_scale = c->d_task_scale;
+  GemmParams sbase{};                       // segmented shrink
+  sbase.M = Ni; sbase.n_mtiles = w.n_tiles;
+  sbase.tile_blk_off = w.t.tile_blk_off; sbase.blk_task = w.t.blk_task; sbase.blk_lo = w.t.blk_lo; sbase.blk_hi = w.t.blk_hi;
+  sbase.blk_tile = w.t.blk_tile; sbase.n_blk = w.t.n_blk;
+  sbase.task_coff = c->d_task_coff; sbase.task_trpad = c->d_task_trpad; sbase.task_scale = c->d_task_scale;
+  PairGemmParams base{};                    // projections
+  base.M = Ni; base.n_ptiles = w.n_tiles;
+  base.tile_blk_off = w.t.tile_blk_off; base.blk_task = w.t.blk_task;
+  base.task_coff = c->d_task_coff; base.task_trpad = c->d_task_trpad;
   base.row_pos = w.t.row_pos;
   for (int i = 0; i < 3; ++i) { base.lora_tgt[i] = -1; base.src_end[i] = 1 << 30; }
-  CUtensorMap mXn, mAttnO, mHid, mU, mPk;
+  CUtensorMap mXn, mAttnO, mHid, mU, mPk, oQKV, oHid, oX;
   int e;
   if ((e = encode_2d(c, &mXn, w.Xn, Ni, d.d_model, d.d_model, 128))) return e;
   if ((e = encode_2d(c, &mAttnO, w.AttnO, Ni, bb.d_q, bb.d_q, 128))) return e;
   if ((e = encode_2d(c, &mHid, w.Hid, Ni, d.d_ffn, d.d_ffn, 128))) return e;
-  if ((e = encode_2d(c, &mU, w.U, (uint64_t)w.n_blk_cap * 128, 192, 192, 128))) return e;
+  if ((e = encode_2d(c, &mU, w.U, (uint64_t)w.n_blk_cap * kPairRows, 192, 192, 128))) return e;
+  if ((e = encode_2d(c, &oQKV, w.QKV, Ni, bb.d_qkv, bb.d_qkv, 128))) return e;
+  oHid = mHid;                              // same bf16 {64,128} box serves loads and stores
+  if ((e = encode_2d(c, &oX, w.X, Ni, d.d_model, d.d_model, 128, true))) return e;
   base.umap = mU;
+  auto wv = [](const PairGemmParams &p) { return p.n_chunks % 2 == 0 ? 0 : 1; };   // weight-map variant (box rows 128 / 64)
 
   // shrink over an input group: targets tgs[0..n) that currently have adapters; fills uslot_of[tg]
   int uslot_of[7] = {-1, -1, -1, -1, -1, -1, -1};
   auto shrink = [&](const CUtensorMap &amap, int K, const int *tgs, int n, int layer) -> int {
-    GemmParams p = base;
+    GemmParams p = sbase;
     p.mode = GM_SHRINK; p.amap = amap; p.K = K; p.out = w.U; p.ld_out = 192; p.n_tg = 0;
     for (int i = 0; i < n; ++i) {
       const int tg = tgs[i];
@@ -720,10 +739,10 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       uslot_of[tg] = p.n_tg++;
     }
     if (p.n_tg == 0) return FMX_OK;
-    LAUNCH(Lh, F_SHRINK, launch_gemm(c, s, p));
+    LAUNCH(Lh, F_SHRINK, launch_shrink(c, s, p));
     return FMX_OK;
   };
-  auto set_lora = [&](GemmParams &p, int src, int tg, int layer) {
+  auto set_lora = [&](PairGemmParams &p, int src, int tg, int layer) {
     if (bb.n_adapters[tg] > 0 && uslot_of[tg] >= 0) {
       p.lora_tgt[src] = tg; p.uslot[src] = uslot_of[tg]; p.lmap[src] = bb.mB[tg][layer]; p.has_lora = 1;
     }
@@ -737,10 +756,10 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     pa.A = w.Hid;
     LAUNCH(Lh, F_EMBED, (pack_patches_kernel<<<Ni, 128, 0, s>>>(pa)));
     if ((e = encode_2d(c, &mPk, w.Hid, Ni, bb.Kp, bb.Kp, 128))) return e;
-    GemmParams p = base;
-    p.mode = GM_EMBED_F32; p.amap = mPk; p.wmap[0] = bb.mEmbedW; p.K = bb.Kp; p.n_chunks = d.d_model / 128;
-    p.out = w.X; p.ld_out = d.d_model; p.posb = bb.posb;
-    LAUNCH(Lh, F_EMBED, launch_gemm(c, s, p));
+    PairGemmParams p = base;
+    p.mode = GM_EMBED_F32; p.amap = mPk; p.K = bb.Kp; p.n_chunks = d.d_model / 128;
+    p.wmap[0] = bb.mEmbedW[wv(p)]; p.omap = oX; p.posb = bb.posb; p.ld_pos = d.d_model;
+    LAUNCH(Lh, F_EMBED, launch_pair_gemm(c, s, p));
   } else {
     EmbedArgs ea{};
     ea.inputs = inputs; ea.perm = w.t.perm; ea.row_req = w.t.row_req; ea.row_pos = w.t.row_pos; ea.in_off = w.t.in_off;
@@ -756,14 +775,15 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     {
       const int tgs[3] = {FMX_TGT_Q, FMX_TGT_K, FMX_TGT_V};
       if ((e = shrink(mXn, d.d_model, tgs, 3, l))) return e;
-      GemmParams p = base;
+      PairGemmParams p = base;
       p.mode = GM_OUT_BF16; p.amap = mXn; p.K = d.d_model; p.n_chunks = bb.d_qkv / 128;
-      p.wmap[0] = bb.mWq[l]; p.wmap[1] = bb.mWk[l]; p.wmap[2] = bb.mWv[l];
+      const int v = wv(p);
+      p.wmap[0] = bb.mWq[v][l]; p.wmap[1] = bb.mWk[v][l]; p.wmap[2] = bb.mWv[v][l];
       p.src_end[0] = bb.d_q / 128; p.src_end[1] = (bb.d_q + bb.d_kv) / 128; p.src_end[2] = 1 << 30;
       p.bias[0] = (const bf16 *)bb.bq[l]; p.bias[1] = (const bf16 *)bb.bk[l]; p.bias[2] = (const bf16 *)bb.bv[l];
       set_lora(p, 0, FMX_TGT_Q, l); set_lora(p, 1, FMX_TGT_K, l); set_lora(p, 2, FMX_TGT_V, l);
-      p.out = w.QKV; p.ld_out = bb.d_qkv;
-      LAUNCH(Lh, F_GEMM_QKV, launch_gemm(c, s, p));
+      p.omap = oQKV;
+      LAUNCH(Lh, F_GEMM_QKV, launch_pair_gemm(c, s, p));
     }
     if (d.rope_theta > 0) {
       const int nh = d.n_q_heads + d.n_kv_heads;
@@ -780,43 +800,43 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     {
       const int tgs[1] = {FMX_TGT_O};
       if ((e = shrink(mAttnO, bb.d_q, tgs, 1, l))) return e;
-      GemmParams p = base;
+      PairGemmParams p = base;
       p.mode = GM_RESID_F32; p.amap = mAttnO; p.K = bb.d_q; p.n_chunks = d.d_model / 128;
-      p.wmap[0] = bb.mWo[l]; p.bias[0] = (const bf16 *)bb.bo[l];
+      p.wmap[0] = bb.mWo[wv(p)][l]; p.bias[0] = (const bf16 *)bb.bo[l];
       set_lora(p, 0, FMX_TGT_O, l);
-      p.out = w.X; p.ld_out = d.d_model;
-      LAUNCH(Lh, F_GEMM_O, launch_gemm(c, s, p));
+      p.omap = oX;
+      LAUNCH(Lh, F_GEMM_O, launch_pair_gemm(c, s, p));
     }
     LAUNCH(Lh, F_NORM, dispatch_norm(s, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm2_g[l], (const bf16 *)bb.norm2_b[l], Ni, d.norm_eps, rms));
     if (d.act == FMX_ACT_SWIGLU) {
       const int tgs[2] = {FMX_TGT_GATE, FMX_TGT_UP};
       if ((e = shrink(mXn, d.d_model, tgs, 2, l))) return e;
-      GemmParams p = base;
+      PairGemmParams p = base;
       p.mode = GM_OUT_BF16_SWIGLU; p.amap = mXn; p.K = d.d_model; p.n_chunks = 2 * d.d_ffn / 128; p.interleave2 = 1;
-      p.wmap[0] = bb.mWgate[l]; p.wmap[1] = bb.mWup[l];
+      p.wmap[0] = bb.mWgate[0][l]; p.wmap[1] = bb.mWup[0][l];
       p.bias[0] = (const bf16 *)bb.bgate[l]; p.bias[1] = (const bf16 *)bb.bup[l];
       set_lora(p, 0, FMX_TGT_GATE, l); set_lora(p, 1, FMX_TGT_UP, l);
-      p.out = w.Hid; p.ld_out = d.d_ffn;
-      LAUNCH(Lh, F_GEMM_FFN_IN, launch_gemm(c, s, p));
+      p.omap = oHid;
+      LAUNCH(Lh, F_GEMM_FFN_IN, launch_pair_gemm(c, s, p));
     } else {
       const int tgs[1] = {FMX_TGT_UP};
       if ((e = shrink(mXn, d.d_model, tgs, 1, l))) return e;
-      GemmParams p = base;
+      PairGemmParams p = base;
       p.mode = d.act == FMX_ACT_GELU_ERF ? GM_OUT_BF16_GELU : GM_OUT_BF16_RELU; p.amap = mXn; p.K = d.d_model; p.n_chunks = d.d_ffn / 128;
-      p.wmap[0] = bb.mWup[l]; p.bias[0] = (const bf16 *)bb.bup[l];
+      p.wmap[0] = bb.mWup[wv(p)][l]; p.bias[0] = (const bf16 *)bb.bup[l];
       set_lora(p, 0, FMX_TGT_UP, l);
-      p.out = w.Hid; p.ld_out = d.d_ffn;
-      LAUNCH(Lh, F_GEMM_FFN_IN, launch_gemm(c, s, p));
+      p.omap = oHid;
+      LAUNCH(Lh, F_GEMM_FFN_IN, launch_pair_gemm(c, s, p));
     }
     {
       const int tgs[1] = {FMX_TGT_DOWN};
       if ((e = shrink(mHid, d.d_ffn, tgs, 1, l))) return e;
-      GemmParams p = base;
+      PairGemmParams p = base;
       p.mode = GM_RESID_F32; p.amap = mHid; p.K = d.d_ffn; p.n_chunks = d.d_model / 128;
-      p.wmap[0] = bb.mWdown[l]; p.bias[0] = (const bf16 *)bb.bdown[l];
+      p.wmap[0] = bb.mWdown[wv(p)][l]; p.bias[0] = (const bf16 *)bb.bdown[l];
       set_lora(p, 0, FMX_TGT_DOWN, l);
-      p.out = w.X; p.ld_out = d.d_model;
-      LAUNCH(Lh, F_GEMM_FFN_OUT, launch_gemm(c, s, p));
+      p.omap = oX;
+      LAUNCH(Lh, F_GEMM_FFN_OUT, launch_pair_gemm(c, s, p));
     }
   }
   // ---- S4-S6 ----
@@ -834,7 +854,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   {
     void *bufs[7] = {w.X, w.Xn, w.QKV, w.AttnO, w.Hid, w.U, w.feat};
     size_t sz[7] = {sizeof(float) * N * d.d_model, sizeof(bf16) * N * d.d_model, sizeof(bf16) * N * bb.d_qkv, sizeof(bf16) * N * bb.d_q,
-                    sizeof(bf16) * N * d.d_ffn, sizeof(bf16) * (size_t)w.n_blk_cap * 128 * 192, sizeof(float) * (size_t)B * d.d_model};
+                    sizeof(bf16) * N * d.d_ffn, sizeof(bf16) * (size_t)w.n_blk_cap * kPairRows * 192, sizeof(float) * (size_t)B * d.d_model};
     for (int i = 0; i < 7; ++i) { c->last_buf[i] = bufs[i]; c->last_buf_bytes[i] = sz[i]; }
   }
   c->last_t = w.t; c->last_B = B; c->last_T = T; c->last_n_tiles = w.n_tiles; c->last_stream = s; c->last_launches = Lh.count;
@@ -971,14 +991,14 @@ int fmx_debug_gemm(fmx_ctx *c, const void *A, const void *W, float *C, int32_t M
   if (M < 1 || N < 128 || N % 128 || K < 8 || K % 8) return fmx_fail(FMX_E_SHAPE, "debug_gemm: need N %% 128 == 0, K %% 8 == 0");
   std::lock_guard<std::mutex> lk(c->mu);
   CU_OK(cudaSetDevice(c->device));
-  GemmParams p{};
+  PairGemmParams p{};
   int e;
+  p.M = M; p.K = K; p.n_chunks = N / 128; p.n_ptiles = (M + kPairRows - 1) / kPairRows; p.mode = GM_OUT_F32;
   if ((e = encode_2d(c, &p.amap, A, M, K, K, 128))) return e;
-  if ((e = encode_2d(c, &p.wmap[0], W, N, K, K, 128))) return e;
-  p.M = M; p.K = K; p.n_chunks = N / 128; p.n_mtiles = (M + 127) / 128; p.mode = GM_OUT_F32;
+  if ((e = encode_2d(c, &p.wmap[0], W, N, K, K, pair_wide(p) ? 128 : 64))) return e;
+  if ((e = encode_2d(c, &p.omap, C, M, N, N, 128, true))) return e;
   for (int i = 0; i < 3; ++i) { p.lora_tgt[i] = -1; p.src_end[i] = 1 << 30; }
-  p.out = C; p.ld_out = N;
-  launch_gemm(c, (cudaStream_t)cuda_stream, p);
+  launch_pair_gemm(c, (cudaStream_t)cuda_stream, p);
   CU_OK(cudaGetLastError());
   return FMX_OK;
 }

@@ -29,7 +29,8 @@ struct SegTables {
 struct SortArgs {
   SegTables t;
   int B, T;                        // requests, task slots
-  int n_tiles;                     // ceil(N / 128)
+  int n_tiles;                     // ceil(N / tile_rows)
+  int tile_rows;                   // rows of a GEMM row tile (256: one CTA-pair tile)
   long long in_per_tok, in_per_req;  // packed-input elements per token / per request
   const int *task_head_out;        // [T]
 };
@@ -143,7 +144,7 @@ __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortAr
   __syncthreads();
   block_exclusive_scan_ll(t.in_off, B + 1, s_scratch_ll);
   block_exclusive_scan_ll(t.out_off, B + 1, s_scratch_ll);
-  // (6) block table: for each 128-row tile, the non-empty task segments that intersect it.
+  // (6) block table: for each row tile, the non-empty task segments that intersect it.
   const int n_tok = s_tok[T];
   auto first_task_after = [&](int row) {     // smallest task with tok_off[task+1] > row
     int lo = 0, hi = T;                      // invariant: answer in [lo, hi)
@@ -151,7 +152,7 @@ __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortAr
     return lo;
   };
   for (int m = tid; m < a.n_tiles; m += blockDim.x) {
-    const int r0 = m * 128, r1 = min(r0 + 128, n_tok);
+    const int r0 = m * a.tile_rows, r1 = min(r0 + a.tile_rows, n_tok);
     int cnt = 0;
     for (int k = first_task_after(r0); k < T && s_tok[k] < r1; ++k) cnt += (s_tok[k + 1] > s_tok[k]);
     t.tile_blk_off[m] = cnt;
@@ -161,7 +162,7 @@ __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortAr
   const int n_blk = block_exclusive_scan_i(t.tile_blk_off, a.n_tiles + 1, s_scratch);
   if (tid == 0) *t.n_blk = n_blk;
   for (int m = tid; m < a.n_tiles; m += blockDim.x) {
-    const int r0 = m * 128, r1 = min(r0 + 128, n_tok);
+    const int r0 = m * a.tile_rows, r1 = min(r0 + a.tile_rows, n_tok);
     int b = t.tile_blk_off[m];
     for (int k = first_task_after(r0); k < T && s_tok[k] < r1; ++k) {
       if (s_tok[k + 1] <= s_tok[k]) continue;

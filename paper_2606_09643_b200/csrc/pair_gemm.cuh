@@ -1,0 +1,408 @@
+// CTA-pair (cta_group::2) tcgen05 / TMEM / TMA GEMM for the backbone projections, with the per-task
+// LoRA expand fused in as extra K-steps and a shared-memory staged epilogue that leaves through TMA.
+//
+//   C[M, N] = A[M, K] · W[N, K]^T  (+ Σ_blocks  U_blk[256, r_pad] · B_task[N, r_pad]^T)      fp32 in TMEM
+//
+// Why a pair: one SM's 128x256 tile pulls (128+256)·64·2 B = 48 KB of operands from L2 per 512 tensor
+// cycles; at 148 SMs that saturates the L2->SM fabric at ~65 % tensor utilisation (profiles/r1_01).
+// Two SMs of a cluster share one 256 x kBN tile: each loads its own 128 rows of A and HALF of the W
+// rows (32 KB per SM per k-block for kBN = 256), and one tcgen05.mma.cta_group::2 issued by the
+// leader CTA multiplies [A0; A1] by [W0; W1]^T into both CTAs' TMEM.
+//
+// Rows are task-sorted token rows (S1).  The N axis is cut into 128-column CHUNKS; a chunk names its
+// weight source (q | k | v, gate | up, or the single matrix), so fused QKV and SwiGLU gate/up need no
+// repacked weights.  kBN = 256: the pair tile holds two chunks (CTA r loads chunk r's 128 W rows);
+// kBN = 128: one chunk (CTA r loads 64 of its W rows).
+//
+// LoRA expand (BASELINE.json north_star item 4): after the main K loop, for every (256-row tile, task)
+// BLOCK of the tile and every chunk whose source has an adapter for that task, r_pad/16 more K-steps
+// (M = 256, N = 128) with A = the block's masked shrink output U (rows of other tasks are zero) and
+// B = that task's B-slab columns go into the SAME TMEM accumulator, before the epilogue.  No segment
+// padding: a tile may span any number of tasks.
+//
+// Warp roles (384 threads per CTA, persistent over tiles, 1 CTA/SM, cluster of 2):
+//   warp 0   TMA producer (lane 0, both CTAs): own A rows + own W half; bytes complete on the LEADER's
+//            full barrier (count 2: one arrive.expect_tx per CTA)
+//   warp 1   tcgen05.mma issuer (lane 0, leader CTA only); tcgen05.commit multicast frees the smem
+//            stage in both CTAs and publishes the accumulator to both CTAs' epilogues
+//   warp 2   TMEM alloc / dealloc (cta_group::2, both CTAs)
+//   warps 4-11  epilogue: two warpgroups x 128 threads; thread = accumulator row (TMEM lane);
+//            tcgen05.ld -> bias / activation / SwiGLU -> 128B-swizzled staging tile in smem ->
+//            TMA store (bf16 / fp32) or TMA reduce-add (fp32 residual stream, one add per element)
+#pragma once
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "gemm.cuh"
+#include "ptx.cuh"
+
+namespace fmx {
+
+constexpr int kPairRows = 256;                    // rows of a pair tile (2 x 128)
+constexpr int kStagingBytes = 2 * 2 * 16384;      // 2 warpgroups x 2 buffers x 16 KB
+
+struct PairGemmParams {
+  CUtensorMap amap;        // A [M, K] bf16, box {64, 128}
+  CUtensorMap wmap[3];     // weight sources [rows_s, K] bf16, box {64, kBN/2}
+  CUtensorMap umap;        // U [n_blk_cap*256, 192] bf16, box {64, 128}
+  CUtensorMap lmap[3];     // B-slabs [d_out_s, Rcap] bf16, box {64, 64}
+  CUtensorMap omap;        // output [M, ld]: bf16 box {64, 128}, or fp32 box {32, 128}
+  int M, K;
+  int n_chunks;            // N / 128
+  int n_ptiles;            // ceil(M / 256)
+  int mode;                // GemmMode (not GM_SHRINK)
+  int interleave2;         // chunk c -> source c&1, row (c>>1)*128  (SwiGLU)
+  int has_lora;
+  int src_end[3];          // cumulative chunk count per source (non-interleaved)
+  int lora_tgt[3];         // target id of source s, or -1
+  int uslot[3];            // U column block (x64) of source s
+  const __nv_bfloat16 *bias[3];
+  const int *tile_blk_off, *blk_task;   // S1 block table over 256-row tiles
+  const int *task_coff;
+  const unsigned char *task_trpad;
+  const float *posb;       // [max_seq, ld_pos] fp32 (embed)
+  const int *row_pos;
+  int ld_pos;
+};
+
+__device__ __forceinline__ void pair_chunk_source(const PairGemmParams &p, int c, int &s, int &r0) {
+  if (p.interleave2) {
+    s = c & 1;
+    r0 = (c >> 1) * kChunk;
+  } else {
+    s = 0;
+    int begin = 0;
+    if (c >= p.src_end[0]) { s = 1; begin = p.src_end[0]; }
+    if (c >= p.src_end[1]) { s = 2; begin = p.src_end[1]; }
+    r0 = (c - begin) * kChunk;
+  }
+}
+
+template <int kBN>
+__host__ __device__ constexpr int pair_stage_bytes() { return kATileBytes + (kBN / 2) * kBK * 2; }
+template <int kBN>
+__host__ __device__ constexpr int pair_stages() { return kBN == 256 ? 5 : 6; }
+template <int kBN>
+constexpr int pair_smem_bytes() { return pair_stages<kBN>() * pair_stage_bytes<kBN>() + kStagingBytes + 1024; }
+
+// 32 fp32 accumulator columns (+ bias, activation) -> 4 swizzled 16-byte chunks of bf16 in the staging row.
+__device__ __forceinline__ void stage_bf16_32(const uint32_t (&v)[32], const __nv_bfloat16 *bias, int mode, uint8_t *row_base,
+                                              int chunk0, int rsw) {
+  float f[32];
+#pragma unroll
+  for (int j = 0; j < 32; ++j) f[j] = __uint_as_float(v[j]);
+  if (bias) {
+    const uint4 *bp = reinterpret_cast<const uint4 *>(bias);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const uint4 b = bp[j];
+      f[8 * j + 0] += bf16_lo(b.x); f[8 * j + 1] += bf16_hi(b.x);
+      f[8 * j + 2] += bf16_lo(b.y); f[8 * j + 3] += bf16_hi(b.y);
+      f[8 * j + 4] += bf16_lo(b.z); f[8 * j + 5] += bf16_hi(b.z);
+      f[8 * j + 6] += bf16_lo(b.w); f[8 * j + 7] += bf16_hi(b.w);
+    }
+  }
+  if (mode == GM_OUT_BF16_GELU) {
+#pragma unroll
+    for (int j = 0; j < 32; ++j) f[j] = gelu_erf_f(f[j]);
+  } else if (mode == GM_OUT_BF16_RELU) {
+#pragma unroll
+    for (int j = 0; j < 32; ++j) f[j] = fmaxf(f[j], 0.0f);
+  }
+#pragma unroll
+  for (int j = 0; j < 4; ++j)
+    *reinterpret_cast<uint4 *>(row_base + (((chunk0 + j) ^ rsw) << 4)) =
+        make_uint4(pack_bf16(f[8 * j], f[8 * j + 1]), pack_bf16(f[8 * j + 2], f[8 * j + 3]), pack_bf16(f[8 * j + 4], f[8 * j + 5]),
+                   pack_bf16(f[8 * j + 6], f[8 * j + 7]));
+}
+
+template <int kBN>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pair_gemm_kernel(const __grid_constant__ PairGemmParams p) {
+  constexpr int kCH = kBN / kChunk;
+  constexpr int kStages = pair_stages<kBN>();
+  constexpr int kStageBytes = pair_stage_bytes<kBN>();
+  constexpr int kBHalf = kBN / 2;                          // W rows per CTA per stage
+  constexpr int kExpandBytes = kATileBytes + 64 * kBK * 2; // U half tile + 64 slab rows
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t *staging = smem + kStages * kStageBytes;
+  __shared__ __align__(8) uint64_t full_bar[kStages], empty_bar[kStages], tfull_bar[2], tempty_bar[2];
+  __shared__ uint32_t tmem_base_slot;
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const int nK = (p.K + kBK - 1) / kBK;
+  const int n_ntiles = p.n_chunks / kCH;
+  const int total_tiles = p.n_ptiles * n_ntiles;
+  const int tile0 = (int)cluster_id_x(), tile_step = (int)cluster_nctaid_x();
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < kStages; ++s) { mbar_init(&full_bar[s], 2); mbar_init(&empty_bar[s], 1); }
+    for (int a = 0; a < 2; ++a) { mbar_init(&tfull_bar[a], 1); mbar_init(&tempty_bar[a], 16); }
+    fence_barrier_init();
+  }
+  if (warp == 2) {
+    tmem_alloc_2sm(&tmem_base_slot, 512);
+    tmem_relinquish_2sm();
+  }
+  tc_fence_before();
+  cluster_sync_all();
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_base_slot;
+
+  if (warp == 0) {
+    // ================================ TMA producer (both CTAs) ================================
+    if (lane == 0) {
+      tma_prefetch_desc(&p.amap);
+      tma_prefetch_desc(&p.wmap[0]);
+      int stage = 0; uint32_t phase = 0;
+      for (int tile = tile0; tile < total_tiles; tile += tile_step) {
+        const int m_pt = tile / n_ntiles, n_tile = tile - m_pt * n_ntiles;
+        const int m0 = m_pt * kPairRows + (int)rank * kBM;
+        int bsrc, brow;
+        if constexpr (kBN == 256) {
+          pair_chunk_source(p, n_tile * 2 + (int)rank, bsrc, brow);
+        } else {
+          pair_chunk_source(p, n_tile, bsrc, brow);
+          brow += (int)rank * kBHalf;
+        }
+        for (int kb = 0; kb < nK; ++kb) {
+          mbar_wait(&empty_bar[stage], phase ^ 1);
+          uint8_t *sa = smem + stage * kStageBytes, *sb = sa + kATileBytes;
+          const uint32_t fb = mapa_shared(smem_u32(&full_bar[stage]), 0);
+          mbar_arrive_expect_tx_cluster(fb, kStageBytes);
+          tma_load_2d_2sm(sa, &p.amap, fb, kb * kBK, m0);
+          tma_load_2d_2sm(sb, &p.wmap[bsrc], fb, kb * kBK, brow);
+          if (++stage == kStages) { stage = 0; phase ^= 1; }
+        }
+        if (p.has_lora) {
+          const int b0 = p.tile_blk_off[m_pt], b1 = p.tile_blk_off[m_pt + 1];
+#pragma unroll
+          for (int c = 0; c < kCH; ++c) {
+            int s, r0;
+            pair_chunk_source(p, n_tile * kCH + c, s, r0);
+            const int tg = p.lora_tgt[s];
+            if (tg < 0) continue;
+            for (int b = b0; b < b1; ++b) {
+              const int t = p.blk_task[b];
+              if (p.task_trpad[t * 7 + tg] == 0) continue;
+              mbar_wait(&empty_bar[stage], phase ^ 1);
+              uint8_t *sa = smem + stage * kStageBytes, *sb = sa + kATileBytes;
+              const uint32_t fb = mapa_shared(smem_u32(&full_bar[stage]), 0);
+              mbar_arrive_expect_tx_cluster(fb, kExpandBytes);
+              tma_load_2d_2sm(sa, &p.umap, fb, p.uslot[s] * 64, b * kPairRows + (int)rank * kBM);
+              tma_load_2d_2sm(sb, &p.lmap[s], fb, p.task_coff[t], r0 + (int)rank * 64);
+              if (++stage == kStages) { stage = 0; phase ^= 1; }
+            }
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ================================ MMA issuer (leader CTA only) ================================
+    if (rank == 0 && lane == 0) {
+      int stage = 0; uint32_t phase = 0; int acc = 0; uint32_t accphase = 0;
+      constexpr uint32_t idesc_main = make_idesc_bf16(kPairRows, kBN);
+      constexpr uint32_t idesc_lora = make_idesc_bf16(kPairRows, kChunk);
+      for (int tile = tile0; tile < total_tiles; tile += tile_step) {
+        const int m_pt = tile / n_ntiles, n_tile = tile - m_pt * n_ntiles;
+        mbar_wait_cluster(&tempty_bar[acc], accphase ^ 1);
+        tc_fence_after();
+        const uint32_t d_tmem = tmem_base + acc * kAccStride;
+        for (int kb = 0; kb < nK; ++kb) {
+          mbar_wait_cluster(&full_bar[stage], phase);
+          tc_fence_after();
+          const uint32_t sa = smem_u32(smem + stage * kStageBytes);
+          const uint64_t adesc = make_smem_desc_sw128(sa), bdesc = make_smem_desc_sw128(sa + kATileBytes);
+#pragma unroll
+          for (int k = 0; k < kBK / 16; ++k)
+            umma_bf16_2sm(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc_main, (kb | k) != 0);
+          umma_commit_2sm(&empty_bar[stage], 3);
+          if (++stage == kStages) { stage = 0; phase ^= 1; }
+        }
+        if (p.has_lora) {
+          const int b0 = p.tile_blk_off[m_pt], b1 = p.tile_blk_off[m_pt + 1];
+#pragma unroll
+          for (int c = 0; c < kCH; ++c) {
+            int s, r0;
+            pair_chunk_source(p, n_tile * kCH + c, s, r0);
+            const int tg = p.lora_tgt[s];
+            if (tg < 0) continue;
+            for (int b = b0; b < b1; ++b) {
+              const int ksteps = p.task_trpad[p.blk_task[b] * 7 + tg] >> 4;
+              if (ksteps == 0) continue;
+              mbar_wait_cluster(&full_bar[stage], phase);
+              tc_fence_after();
+              const uint32_t sa = smem_u32(smem + stage * kStageBytes);
+              const uint64_t adesc = make_smem_desc_sw128(sa), bdesc = make_smem_desc_sw128(sa + kATileBytes);
+              for (int k = 0; k < ksteps; ++k)
+                umma_bf16_2sm(d_tmem + c * kChunk, adesc + 2 * k, bdesc + 2 * k, idesc_lora, 1);
+              umma_commit_2sm(&empty_bar[stage], 3);
+              if (++stage == kStages) { stage = 0; phase ^= 1; }
+            }
+          }
+        }
+        umma_commit_2sm(&tfull_bar[acc], 3);
+        if (++acc == 2) { acc = 0; accphase ^= 1; }
+      }
+    }
+  } else if (warp >= 4) {
+    // ================================ epilogue (both CTAs) ================================
+    const int wg = (warp - 4) >> 2, quad = warp & 3;
+    const int r_in_tile = quad * 32 + lane;
+    const int rsw = r_in_tile & 7;
+    const bool issuer = (threadIdx.x == 128 + wg * 128);
+    const uint32_t bar_id = 1 + wg;
+    uint8_t *stg = staging + wg * 32768;
+    int box_seq = 0;
+    int acc = 0; uint32_t accphase = 0;
+    const int mode = p.mode;
+    for (int tile = tile0; tile < total_tiles; tile += tile_step) {
+      const int m_pt = tile / n_ntiles, n_tile = tile - m_pt * n_ntiles;
+      const int row0_cta = m_pt * kPairRows + (int)rank * kBM;
+      const int row = row0_cta + r_in_tile;
+      mbar_wait(&tfull_bar[acc], accphase);
+      tc_fence_after();
+      const uint32_t t_row = tmem_base + (uint32_t(quad * 32) << 16) + acc * kAccStride;
+      const uint32_t tempty_remote = mapa_shared(smem_u32(&tempty_bar[acc]), 0);
+      uint32_t v[32], u[32];
+
+      if (mode == GM_OUT_BF16_SWIGLU) {
+        // tile = [gate chunk | up chunk] of the same 128 output features; this warpgroup: 64 of them
+        const int r0 = n_tile * kChunk;                         // feature offset of the tile
+        const int fcol = wg * 64;
+        uint8_t *buf = stg + (box_seq & 1) * 16384;
+        if (issuer) bulk_wait_read<1>();
+        named_bar_sync(bar_id, 128);
+        uint8_t *row_base = buf + r_in_tile * 128;
+#pragma unroll 1
+        for (int h = 0; h < 2; ++h) {
+          tmem_ld_32x32(t_row + fcol + h * 32, v);
+          tmem_ld_32x32(t_row + kChunk + fcol + h * 32, u);
+          tmem_ld_wait();
+          if (h == 1) {
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(tempty_remote);
+          }
+          const __nv_bfloat16 *bg = p.bias[0], *bu = p.bias[1];
+          const int nb = r0 + fcol + h * 32;
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            float r[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+              float gt = __uint_as_float(v[8 * j + e]), up = __uint_as_float(u[8 * j + e]);
+              if (bg) gt += __bfloat162float(bg[nb + 8 * j + e]);
+              if (bu) up += __bfloat162float(bu[nb + 8 * j + e]);
+              r[e] = silu_f(gt) * up;
+            }
+            *reinterpret_cast<uint4 *>(row_base + (((h * 4 + j) ^ rsw) << 4)) =
+                make_uint4(pack_bf16(r[0], r[1]), pack_bf16(r[2], r[3]), pack_bf16(r[4], r[5]), pack_bf16(r[6], r[7]));
+          }
+        }
+        fence_proxy_async();
+        named_bar_sync(bar_id, 128);
+        if (issuer) { tma_store_2d(&p.omap, buf, r0 + fcol, row0_cta); bulk_commit(); }
+        ++box_seq;
+      } else if (mode == GM_OUT_BF16 || mode == GM_OUT_BF16_GELU || mode == GM_OUT_BF16_RELU) {
+        constexpr int kBoxes = kBN / 128;                       // 64-column boxes per warpgroup
+#pragma unroll 1
+        for (int j = 0; j < kBoxes; ++j) {
+          const int col = wg * (kBN / 2) + j * 64;              // column within the tile
+          int s, r0;
+          pair_chunk_source(p, n_tile * kCH + col / kChunk, s, r0);
+          const int n_src = r0 + (col % kChunk);
+          const int n_out = n_tile * kBN + col;
+          uint8_t *buf = stg + (box_seq & 1) * 16384;
+          if (issuer) bulk_wait_read<1>();
+          named_bar_sync(bar_id, 128);
+          tmem_ld_32x32(t_row + col, v);
+          tmem_ld_32x32(t_row + col + 32, u);
+          tmem_ld_wait();
+          if (j == kBoxes - 1) {
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(tempty_remote);
+          }
+          uint8_t *row_base = buf + r_in_tile * 128;
+          const __nv_bfloat16 *bias = p.bias[s];
+          stage_bf16_32(v, bias ? bias + n_src : nullptr, mode, row_base, 0, rsw);
+          stage_bf16_32(u, bias ? bias + n_src + 32 : nullptr, mode, row_base, 4, rsw);
+          fence_proxy_async();
+          named_bar_sync(bar_id, 128);
+          if (issuer) { tma_store_2d(&p.omap, buf, n_out, row0_cta); bulk_commit(); }
+          ++box_seq;
+        }
+      } else {
+        // fp32 outputs: residual reduce-add, embed (+ positional table), plain store
+        constexpr int kBoxes = kBN / 64;                        // 32-column boxes per warpgroup
+        const float *posrow = nullptr;
+        if (mode == GM_EMBED_F32 && row < p.M) posrow = p.posb + (size_t)p.row_pos[row] * p.ld_pos;
+#pragma unroll 1
+        for (int j = 0; j < kBoxes; ++j) {
+          const int col = wg * (kBN / 2) + j * 32;
+          int s, r0;
+          pair_chunk_source(p, n_tile * kCH + col / kChunk, s, r0);
+          const int n_src = r0 + (col % kChunk);
+          const int n_out = n_tile * kBN + col;
+          uint8_t *buf = stg + (box_seq & 1) * 16384;
+          if (issuer) bulk_wait_read<1>();
+          named_bar_sync(bar_id, 128);
+          tmem_ld_32x32(t_row + col, v);
+          tmem_ld_wait();
+          if (j == kBoxes - 1) {
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(tempty_remote);
+          }
+          float f[32];
+#pragma unroll
+          for (int e = 0; e < 32; ++e) f[e] = __uint_as_float(v[e]);
+          const __nv_bfloat16 *bias = p.bias[s];
+          if (bias) {
+            const uint4 *bp = reinterpret_cast<const uint4 *>(bias + n_src);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              const uint4 b = bp[q];
+              f[8 * q + 0] += bf16_lo(b.x); f[8 * q + 1] += bf16_hi(b.x);
+              f[8 * q + 2] += bf16_lo(b.y); f[8 * q + 3] += bf16_hi(b.y);
+              f[8 * q + 4] += bf16_lo(b.z); f[8 * q + 5] += bf16_hi(b.z);
+              f[8 * q + 6] += bf16_lo(b.w); f[8 * q + 7] += bf16_hi(b.w);
+            }
+          }
+          if (posrow) {
+            const float4 *P = reinterpret_cast<const float4 *>(posrow + n_out);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+              const float4 w = P[q];
+              f[4 * q] += w.x; f[4 * q + 1] += w.y; f[4 * q + 2] += w.z; f[4 * q + 3] += w.w;
+            }
+          }
+          uint8_t *row_base = buf + r_in_tile * 128;
+#pragma unroll
+          for (int q = 0; q < 8; ++q)
+            *reinterpret_cast<float4 *>(row_base + ((q ^ rsw) << 4)) = make_float4(f[4 * q], f[4 * q + 1], f[4 * q + 2], f[4 * q + 3]);
+          fence_proxy_async();
+          named_bar_sync(bar_id, 128);
+          if (issuer) {
+            if (mode == GM_RESID_F32) tma_reduce_add_2d(&p.omap, buf, n_out, row0_cta);
+            else tma_store_2d(&p.omap, buf, n_out, row0_cta);
+            bulk_commit();
+          }
+          ++box_seq;
+        }
+      }
+      if (++acc == 2) { acc = 0; accphase ^= 1; }
+    }
+    if (issuer) bulk_wait<0>();
+  }
+
+  tc_fence_before();
+  cluster_sync_all();
+  if (warp == 2) tmem_dealloc_2sm(tmem_base, 512);
+}
+
+}  // namespace fmx

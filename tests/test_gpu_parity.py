@@ -57,14 +57,15 @@ def check_segments(s, wl):
     # the private (row-tile, task) block table: valid cover of every tile by same-task row ranges
     n_tiles, n_blk, blocks = s.fmx.debug_get_tiles()
     N = wl.n_tokens
-    assert n_tiles == (N + 127) // 128
-    covered = np.zeros(n_tiles * 128, dtype=np.int32)
+    R = 256                                    # rows of a CTA-pair GEMM tile
+    assert n_tiles == (N + R - 1) // R
+    covered = np.zeros(n_tiles * R, dtype=np.int32)
     row_task = np.repeat(ids[ref["perm"]], wl.lengths[ref["perm"]])
     prev = (-1, -1)
     for tile, task, lo, hi in blocks:
-        assert (tile, task) > prev and 0 <= lo < hi <= 128
+        assert (tile, task) > prev and 0 <= lo < hi <= R
         prev = (tile, task)
-        rows = np.arange(tile * 128 + lo, tile * 128 + hi)
+        rows = np.arange(tile * R + lo, tile * R + hi)
         assert rows[-1] < N and np.all(row_task[rows] == task)
         covered[rows] += 1
     assert np.all(covered[:N] == 1) and np.all(covered[N:] == 0)
