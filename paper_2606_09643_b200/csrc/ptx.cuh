@@ -145,24 +145,17 @@ __device__ __forceinline__ uint32_t mapa_shared(uint32_t cta_addr, uint32_t rank
   return r;
 }
 __device__ __forceinline__ void mbar_arrive_expect_tx_cluster(uint32_t cluster_addr, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.release.cluster.shared::cluster.b64 _, [%0], %1;\n" ::"r"(cluster_addr), "r"(bytes)
+  asm volatile("mbarrier.arrive.expect_tx.shared::cluster.b64 _, [%0], %1;\n" ::"r"(cluster_addr), "r"(bytes)
                : "memory");
 }
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
-  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];\n" ::"r"(cluster_addr) : "memory");
+  asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];\n" ::"r"(cluster_addr) : "memory");
 }
-__device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, uint32_t parity) {     // acquire at cluster scope
-  uint32_t ok;
-  do {
-    asm volatile(
-        "{\n\t.reg .pred P;\n\t"
-        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 P, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, P;\n\t}\n"
-        : "=r"(ok)
-        : "r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-  } while (!ok);
-}
+// Waits on a barrier that CTAs of the cluster arrive on remotely.  Default (.acquire.cta) semantics on purpose: an
+// explicit cluster-scope acquire/release makes ptxas emit MEMBAR.ALL.GPU + CCTL.IVALL around every arrive / wait, which
+// serialised the TMA producer (profiles/r1_02); TMA bytes and tcgen05 results are ordered by complete_tx / tcgen05.commit
+// and the tcgen05 fences, not by these barriers' memory semantics.
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, uint32_t parity) { mbar_wait(bar, parity); }
 // 2-D tiled load issued by either CTA of a pair; completion bytes land on the mbarrier at cluster address `bar`
 // (the leader CTA's barrier).
 __device__ __forceinline__ void tma_load_2d_2sm(void *smem_dst, const CUtensorMap *m, uint32_t bar_cluster_addr, int32_t c0,
