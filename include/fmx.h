@@ -200,6 +200,23 @@ int fmx_last_launch_count(fmx_ctx *ctx);
 int fmx_debug_gemm(fmx_ctx *ctx, const void *A, const void *W, float *C, int32_t M, int32_t N, int32_t K,
                    void *cuda_stream);
 
+/* Debug/test: the fused variable-length attention step (S3d) alone.  qkv DEVICE bf16
+ * [n_tokens, (n_q_heads + 2 n_kv_heads) * head_dim] (q | k | v per row, requests packed back to back),
+ * cu_tok HOST int32 [n_req + 1] (prefix sums of the request lengths), out DEVICE bf16
+ * [n_tokens, n_q_heads * head_dim].  impl: an FMX_ATTN_* value.  Scale 1/sqrt(head_dim). */
+int fmx_debug_attention(fmx_ctx *ctx, const void *qkv, void *out, const int32_t *cu_tok, int32_t n_req,
+                        int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim, int32_t causal, int32_t impl,
+                        void *cuda_stream);
+
+/* Tuning knobs (process-local experiments; defaults are what bench.py measures). */
+enum {
+  FMX_OPT_ATTENTION_IMPL = 0,    /* FMX_ATTN_AUTO | FMX_ATTN_MMA_SYNC | FMX_ATTN_TCGEN05 */
+  FMX_OPT_ATTENTION_VARIANT = 1  /* tcgen05 attention: 0 = one 128-query tile per CTA, two CTAs per SM;
+                                    1 = two q-tiles per CTA sharing K/V, one CTA per SM */
+};
+enum { FMX_ATTN_AUTO = 0, FMX_ATTN_MMA_SYNC = 1, FMX_ATTN_TCGEN05 = 2 };
+int fmx_set_option(fmx_ctx *ctx, int32_t option, int32_t value);
+
 /* ---- BFQ: host-side batch-aware fair-queue batch builder (§4.2, Eq. 1-3) ------------
  * Pure host code (no CUDA).  It emits the task ids / lengths fmx_forward_mixed consumes. */
 typedef struct fmx_bfq fmx_bfq;

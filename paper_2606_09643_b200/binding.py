@@ -52,6 +52,9 @@ class BfqParams(C.Structure):
     _fields_ = [("n_tasks", C.c_int32), ("b_max", C.c_int32), ("lat_ms", C.POINTER(C.c_double)), ("l_tok_ms", C.c_double)]
 
 
+OPTIONS = {"attention_impl": 0, "attention_variant": 1}
+
+
 class FmxError(RuntimeError):
     def __init__(self, code, msg):
         super().__init__(f"{STATUS.get(code, code)}: {msg}")
@@ -63,7 +66,7 @@ _lib = None
 EXPORTS = ["fmx_create", "fmx_destroy", "fmx_last_error", "fmx_version", "fmx_register_backbone", "fmx_register_task",
            "fmx_unregister_task", "fmx_output_layout", "fmx_workspace_bytes", "fmx_forward_mixed", "fmx_forward_mixed_host",
            "fmx_debug_get_segments", "fmx_debug_get_tiles", "fmx_debug_read", "fmx_task_slots", "fmx_profile_enable", "fmx_profile_select", "fmx_profile_read",
-           "fmx_profile_family_name", "fmx_last_launch_count", "fmx_debug_gemm", "fmx_bfq_create", "fmx_bfq_destroy",
+           "fmx_profile_family_name", "fmx_last_launch_count", "fmx_debug_gemm", "fmx_debug_attention", "fmx_set_option", "fmx_bfq_create", "fmx_bfq_destroy",
            "fmx_bfq_set_task", "fmx_bfq_enqueue", "fmx_bfq_next_batch", "fmx_bfq_complete", "fmx_bfq_stats", "fmx_bfq_peek"]
 
 
@@ -99,6 +102,8 @@ def load():
     lib.fmx_profile_read.argtypes = [_vp, i32p, f64p]
     lib.fmx_last_launch_count.argtypes = [_vp]
     lib.fmx_debug_gemm.argtypes = [_vp, _vp, _vp, _vp, C.c_int32, C.c_int32, C.c_int32, _vp]
+    lib.fmx_debug_attention.argtypes = [_vp, _vp, _vp, i32p, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, _vp]
+    lib.fmx_set_option.argtypes = [_vp, C.c_int32, C.c_int32]
     lib.fmx_bfq_create.argtypes = [C.POINTER(BfqParams), C.POINTER(_vp)]
     lib.fmx_bfq_destroy.argtypes = [_vp]
     lib.fmx_bfq_set_task.argtypes = [_vp, C.c_int32, C.c_double, C.c_double]
@@ -254,6 +259,15 @@ class Fmx:
 
     def debug_gemm(self, A, W, Cout, M, N, K, stream=0):
         _check(self.lib.fmx_debug_gemm(self.h, A, W, Cout, M, N, K, stream or None))
+
+    def debug_attention(self, qkv, out, cu_tok, n_q_heads, n_kv_heads, head_dim, causal, impl=0, stream=0):
+        cu = np.ascontiguousarray(cu_tok, dtype=np.int32)
+        _check(self.lib.fmx_debug_attention(self.h, qkv, out, cu.ctypes.data_as(C.POINTER(C.c_int32)), len(cu) - 1, n_q_heads,
+                                            n_kv_heads, head_dim, int(causal), impl, stream or None))
+
+    def set_option(self, option, value):
+        """option: 'attention_impl' (0 auto, 1 mma.sync, 2 tcgen05)."""
+        _check(self.lib.fmx_set_option(self.h, OPTIONS[option], int(value)))
 
 
 class Bfq:

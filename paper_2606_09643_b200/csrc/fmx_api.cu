@@ -7,12 +7,14 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <memory>
 #include <mutex>
 #include <vector>
 
 #include "attention.cuh"
+#include "attention_tc.cuh"
 #include "common.h"
 #include "fmx.h"
 #include "gemm.cuh"
@@ -102,6 +104,8 @@ struct fmx_ctx {
   uint32_t prof_mask = 0xFFFFFFFFu;        // families that get events while prof_on
   std::vector<ProfEvent> prof;
   std::vector<cudaEvent_t> ev_pool;        // recycled events
+  int opt_attn_impl = FMX_ATTN_AUTO, opt_attn_variant = 0;
+  int *d_dbg_cu = nullptr; int dbg_cu_cap = 0;   // fmx_debug_attention's device copy of cu_tok
   std::mutex mu;
 };
 
@@ -276,7 +280,53 @@ void launch_attention(cudaStream_t s, int dh, dim3 grid, const AttnArgs &a) {
   else attention_kernel<128><<<grid, kAttnThreads, attn_smem_bytes<128>(), s>>>(a);
 }
 
+// The tcgen05 kernel serves head_dim 64 / 128 (a TMA box is 64 columns wide); head_dim 32 stays on mma.sync.
+// Variant v: 0 = one q-tile (128 queries) per CTA, two CTAs per SM; 1 = two q-tiles per CTA sharing K/V, one CTA per SM.
+// AUTO: short sequences (one KV tile per request, cfg2/cfg5's 64 tokens) are bound by per-CTA latency, where the
+// lighter mma.sync kernel measured faster (47 vs 65 us per layer on cfg2); everything longer goes to tcgen05.
+bool attn_use_tc(int impl, int dh, int max_len) {
+  if (dh != 64 && dh != 128) return false;
+  if (impl == FMX_ATTN_AUTO) return max_len > 64;
+  return impl != FMX_ATTN_MMA_SYNC;
+}
+template <int DH, int kQT, int kSt, int kMinB>
+void launch_attention_tc_v(cudaStream_t s, int max_len, int n_heads, int B, const AttnTcArgs &a) {
+  dim3 grid((max_len + kAtBQ * kQT - 1) / (kAtBQ * kQT), n_heads, B);
+  attention_tc_kernel<DH, kQT, kSt, kMinB><<<grid, attn_tc_threads<kQT>(), attn_tc_smem_bytes<DH, kQT, kSt>(), s>>>(a);
+}
+void launch_attention_tc(cudaStream_t s, int dh, int variant, int max_len, int n_heads, int B, const AttnTcArgs &a) {
+  if (dh == 64) {
+    if (variant == 0) launch_attention_tc_v<64, 1, 3, 2>(s, max_len, n_heads, B, a);
+    else launch_attention_tc_v<64, 2, 3, 1>(s, max_len, n_heads, B, a);
+  } else {
+    if (variant == 0) launch_attention_tc_v<128, 1, 2, 2>(s, max_len, n_heads, B, a);
+    else launch_attention_tc_v<128, 2, 3, 1>(s, max_len, n_heads, B, a);
+  }
+}
+template <int DH, int kQT, int kSt, int kMinB>
+cudaError_t set_attn_tc_attr() {
+  cudaError_t e = cudaFuncSetAttribute(attention_tc_kernel<DH, kQT, kSt, kMinB>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_tc_smem_bytes<DH, kQT, kSt>());
+  // without this the driver sizes the L1/shared split for ONE block and a second CTA never becomes resident
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(attention_tc_kernel<DH, kQT, kSt, kMinB>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  if (e == cudaSuccess && getenv("FMX_DEBUG")) {
+    int nb = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, attention_tc_kernel<DH, kQT, kSt, kMinB>, attn_tc_threads<kQT>(), attn_tc_smem_bytes<DH, kQT, kSt>());
+    cudaFuncAttributes fa{};
+    cudaFuncGetAttributes(&fa, attention_tc_kernel<DH, kQT, kSt, kMinB>);
+    cudaDeviceProp pr{};
+    cudaGetDeviceProperties(&pr, 0);
+    fprintf(stderr, "fmx: attention_tc<%d,%d,%d,%d>: %d B smem, %d CTA/SM; regs %d static %zu maxdyn %d carveout %d; SM smem %zu regs %d reserved %zu\n",
+            DH, kQT, kSt, kMinB, attn_tc_smem_bytes<DH, kQT, kSt>(), nb, fa.numRegs, fa.sharedSizeBytes, fa.maxDynamicSharedSizeBytes,
+            fa.preferredShmemCarveout, pr.sharedMemPerMultiprocessor, pr.regsPerMultiprocessor, pr.reservedSharedMemPerBlock);
+  }
+  return e;
+}
+
 int set_kernel_attrs() {
+  CU_OK((set_attn_tc_attr<64, 1, 3, 2>()));
+  CU_OK((set_attn_tc_attr<64, 2, 3, 1>()));
+  CU_OK((set_attn_tc_attr<128, 1, 2, 2>()));
+  CU_OK((set_attn_tc_attr<128, 2, 3, 1>()));
   CU_OK(cudaFuncSetAttribute(pair_gemm_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<256>()));
   CU_OK(cudaFuncSetAttribute(pair_gemm_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<128>()));
   CU_OK(cudaFuncSetAttribute(shrink_kernel<kShrinkStages>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes()));
@@ -434,7 +484,7 @@ int fmx_destroy(fmx_ctx *c) {
   for (auto &t : c->tasks) { cudaFree(t.head_W); cudaFree(t.head_b); }
   cudaFree(c->d_task_coff); cudaFree(c->d_task_head_kind); cudaFree(c->d_task_head_out); cudaFree(c->d_task_trpad);
   cudaFree(c->d_task_scale); cudaFree(c->d_task_head_W); cudaFree(c->d_task_head_b);
-  cudaFree(c->d_in_stage); cudaFree(c->d_out_stage);
+  cudaFree(c->d_in_stage); cudaFree(c->d_out_stage); cudaFree(c->d_dbg_cu);
   cudaFreeHost(c->h_stage);
   delete c;
   return FMX_OK;
@@ -713,13 +763,14 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   base.task_coff = c->d_task_coff; base.task_trpad = c->d_task_trpad;
   base.row_pos = w.t.row_pos;
   for (int i = 0; i < 3; ++i) { base.lora_tgt[i] = -1; base.src_end[i] = 1 << 30; }
-  CUtensorMap mXn, mAttnO, mHid, mU, mPk, oQKV, oHid, oX;
+  CUtensorMap mXn, mAttnO, mHid, mU, mPk, oQKV, oHid, oX, mQKV64;
   int e;
   if ((e = encode_2d(c, &mXn, w.Xn, Ni, d.d_model, d.d_model, 128))) return e;
   if ((e = encode_2d(c, &mAttnO, w.AttnO, Ni, bb.d_q, bb.d_q, 128))) return e;
   if ((e = encode_2d(c, &mHid, w.Hid, Ni, d.d_ffn, d.d_ffn, 128))) return e;
   if ((e = encode_2d(c, &mU, w.U, (uint64_t)w.n_blk_cap * kPairRows, 192, 192, 128))) return e;
   if ((e = encode_2d(c, &oQKV, w.QKV, Ni, bb.d_qkv, bb.d_qkv, 128))) return e;
+  if ((e = encode_2d(c, &mQKV64, w.QKV, Ni, bb.d_qkv, bb.d_qkv, 64))) return e;     // attention: box {64, 64}
   oHid = mHid;                              // same bf16 {64,128} box serves loads and stores
   if ((e = encode_2d(c, &oX, w.X, Ni, d.d_model, d.d_model, 128, true))) return e;
   base.umap = mU;
@@ -787,10 +838,15 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     }
     if (d.rope_theta > 0) {
       const int nh = d.n_q_heads + d.n_kv_heads;
-      const long long total = (long long)Ni * nh * (d.head_dim / 2);
+      const long long total = (long long)Ni * nh * (d.head_dim / 16);
       LAUNCH(Lh, F_ROPE, (rope_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(w.QKV, bb.d_qkv, w.t.row_pos, bb.rope_cs, Ni, nh, d.head_dim)));
     }
-    {
+    if (attn_use_tc(c->opt_attn_impl, d.head_dim, max_len)) {
+      AttnTcArgs ta{};
+      ta.qkv_map = mQKV64; ta.out = w.AttnO; ta.cu_tok = w.t.cu_tok; ta.ld_out = bb.d_q;
+      ta.n_q_heads = d.n_q_heads; ta.n_kv_heads = d.n_kv_heads; ta.causal = d.causal; ta.scale_log2 = scale_log2;
+      LAUNCH(Lh, F_ATTN, launch_attention_tc(s, d.head_dim, c->opt_attn_variant, max_len, d.n_q_heads, B, ta));
+    } else {
       AttnArgs aa{};
       aa.qkv = w.QKV; aa.out = w.AttnO; aa.cu_tok = w.t.cu_tok; aa.ld_qkv = bb.d_qkv; aa.ld_out = bb.d_q;
       aa.n_q_heads = d.n_q_heads; aa.n_kv_heads = d.n_kv_heads; aa.causal = d.causal; aa.scale_log2 = scale_log2;
@@ -1001,6 +1057,62 @@ int fmx_debug_gemm(fmx_ctx *c, const void *A, const void *W, float *C, int32_t M
   launch_pair_gemm(c, (cudaStream_t)cuda_stream, p);
   CU_OK(cudaGetLastError());
   return FMX_OK;
+}
+
+int fmx_debug_attention(fmx_ctx *c, const void *qkv, void *out, const int32_t *cu_tok, int32_t n_req, int32_t n_q_heads,
+                        int32_t n_kv_heads, int32_t head_dim, int32_t causal, int32_t impl, void *cuda_stream) {
+  if (!c || !qkv || !out || !cu_tok) return fmx_fail(FMX_E_INVALID_ARG, "debug_attention: NULL argument");
+  if (n_req < 1 || n_q_heads < 1 || n_kv_heads < 1 || n_q_heads % n_kv_heads || !(head_dim == 32 || head_dim == 64 || head_dim == 128))
+    return fmx_fail(FMX_E_SHAPE, "debug_attention: bad head configuration");
+  std::lock_guard<std::mutex> lk(c->mu);
+  CU_OK(cudaSetDevice(c->device));
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  int max_len = 0;
+  for (int i = 0; i < n_req; ++i) {
+    if (cu_tok[i + 1] <= cu_tok[i]) return fmx_fail(FMX_E_BAD_LENGTH, "debug_attention: request %d has no tokens", i);
+    max_len = std::max(max_len, cu_tok[i + 1] - cu_tok[i]);
+  }
+  if (n_req + 1 > c->dbg_cu_cap) {
+    CU_OK(cudaStreamSynchronize(s));
+    cudaFree(c->d_dbg_cu);
+    c->d_dbg_cu = nullptr; c->dbg_cu_cap = 0;
+    CU_OK(cudaMalloc(&c->d_dbg_cu, sizeof(int) * (n_req + 1)));
+    c->dbg_cu_cap = n_req + 1;
+  }
+  CU_OK(cudaMemcpyAsync(c->d_dbg_cu, cu_tok, sizeof(int) * (n_req + 1), cudaMemcpyHostToDevice, s));
+  const int N = cu_tok[n_req], d_q = n_q_heads * head_dim, d_qkv = (n_q_heads + 2 * n_kv_heads) * head_dim;
+  const float scale_log2 = 1.4426950408889634f / sqrtf((float)head_dim);
+  if (attn_use_tc(impl, head_dim, max_len)) {
+    AttnTcArgs ta{};
+    if (int e = encode_2d(c, &ta.qkv_map, qkv, N, d_qkv, d_qkv, 64)) return e;
+    ta.out = (bf16 *)out; ta.cu_tok = c->d_dbg_cu; ta.ld_out = d_q; ta.n_q_heads = n_q_heads; ta.n_kv_heads = n_kv_heads;
+    ta.causal = causal; ta.scale_log2 = scale_log2;
+    launch_attention_tc(s, head_dim, c->opt_attn_variant, max_len, n_q_heads, n_req, ta);
+  } else {
+    AttnArgs aa{};
+    aa.qkv = (const bf16 *)qkv; aa.out = (bf16 *)out; aa.cu_tok = c->d_dbg_cu; aa.ld_qkv = d_qkv; aa.ld_out = d_q;
+    aa.n_q_heads = n_q_heads; aa.n_kv_heads = n_kv_heads; aa.causal = causal; aa.scale_log2 = scale_log2;
+    launch_attention(s, head_dim, dim3((max_len + kAttnBQ - 1) / kAttnBQ, n_q_heads, n_req), aa);
+  }
+  CU_OK(cudaGetLastError());
+  CU_OK(cudaStreamSynchronize(s));      // cu_tok is a host array of the caller
+  return FMX_OK;
+}
+
+int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
+  if (!c) return fmx_fail(FMX_E_INVALID_ARG, "set_option: NULL ctx");
+  std::lock_guard<std::mutex> lk(c->mu);
+  switch (option) {
+    case FMX_OPT_ATTENTION_IMPL:
+      if (value < FMX_ATTN_AUTO || value > FMX_ATTN_TCGEN05) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attention impl %d", value);
+      c->opt_attn_impl = value;
+      return FMX_OK;
+    case FMX_OPT_ATTENTION_VARIANT:
+      if (value < 0 || value > 1) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attention variant %d", value);
+      c->opt_attn_variant = value;
+      return FMX_OK;
+  }
+  return fmx_fail(FMX_E_INVALID_ARG, "set_option: unknown option %d", option);
 }
 
 }  // extern "C"

@@ -321,21 +321,32 @@ __global__ void __launch_bounds__(256) norm_kernel(const float *__restrict__ X, 
 }
 
 // ============================================================================= RoPE (in place on the fused qkv buffer)
-// rotate-half pairing (j, j + dh/2); position = row_pos[row]; cs = [max_seq, dh/2] float2 (cos, sin)
-__global__ void rope_kernel(__nv_bfloat16 *qkv, int ld, const int *__restrict__ row_pos, const float2 *__restrict__ cs,
-                            int N, int n_heads_qk, int dh) {
-  const int half = dh >> 1;
-  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;     // (row, head, j)
-  const long long total = (long long)N * n_heads_qk * half;
+// rotate-half pairing (j, j + dh/2); position = row_pos[row]; cs = [max_seq, dh/2] float2 (cos, sin).
+// One thread rotates 8 pairs: two 16-byte loads/stores of the row (first and second half of the head) and
+// 64 bytes of the table, so a warp touches whole 128-byte lines (dh/2 must be a multiple of 8).
+__global__ void __launch_bounds__(256) rope_kernel(__nv_bfloat16 *qkv, int ld, const int *__restrict__ row_pos,
+                                                   const float2 *__restrict__ cs, int N, int n_heads_qk, int dh) {
+  const int half = dh >> 1, vec_per_head = half >> 3;
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;     // (row, head, vector of 8 pairs)
+  const long long total = (long long)N * n_heads_qk * vec_per_head;
   if (idx >= total) return;
-  const int j = (int)(idx % half);
-  const int h = (int)((idx / half) % n_heads_qk);
-  const int row = (int)(idx / ((long long)half * n_heads_qk));
-  const float2 c = cs[(size_t)row_pos[row] * half + j];
-  __nv_bfloat16 *p = qkv + (size_t)row * ld + h * dh + j;
-  const float x1 = __bfloat162float(p[0]), x2 = __bfloat162float(p[half]);
-  p[0] = __float2bfloat16(x1 * c.x - x2 * c.y);
-  p[half] = __float2bfloat16(x2 * c.x + x1 * c.y);
+  const int jv = (int)(idx % vec_per_head);
+  const int h = (int)((idx / vec_per_head) % n_heads_qk);
+  const int row = (int)(idx / ((long long)vec_per_head * n_heads_qk));
+  const float4 *c4 = reinterpret_cast<const float4 *>(cs + (size_t)row_pos[row] * half + jv * 8);
+  __nv_bfloat16 *p = qkv + (size_t)row * ld + h * dh + jv * 8;
+  const uint4 a = *reinterpret_cast<const uint4 *>(p), b = *reinterpret_cast<const uint4 *>(p + half);
+  const uint32_t av[4] = {a.x, a.y, a.z, a.w}, bv[4] = {b.x, b.y, b.z, b.w};
+  uint32_t ao[4], bo[4];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    const float4 c = c4[q];                       // (cos, sin) of pairs 2q, 2q+1
+    const float x1l = bf16_lo(av[q]), x1h = bf16_hi(av[q]), x2l = bf16_lo(bv[q]), x2h = bf16_hi(bv[q]);
+    ao[q] = pack_bf16(x1l * c.x - x2l * c.y, x1h * c.z - x2h * c.w);
+    bo[q] = pack_bf16(x2l * c.x + x1l * c.y, x2h * c.z + x1h * c.w);
+  }
+  *reinterpret_cast<uint4 *>(p) = make_uint4(ao[0], ao[1], ao[2], ao[3]);
+  *reinterpret_cast<uint4 *>(p + half) = make_uint4(bo[0], bo[1], bo[2], bo[3]);
 }
 
 __global__ void build_rope_table_kernel(float2 *cs, int max_seq, int dh, double theta) {

@@ -1,0 +1,107 @@
+"""GPU parity of the fused variable-length attention step (S3d) alone, through the C ABI
+(`fmx_debug_attention`), against the oracle's `attention` (fp64, per request, per head) on the
+same bf16 inputs.  Both implementations are covered: the tcgen05/TMEM/TMA kernel (head_dim 64,
+128) and the warp-level mma.sync kernel (head_dim 32 and the fallback switch).
+
+Tolerance: the output is bf16 (rel. 2^-9) of a convex combination of v rows with P rounded to
+bf16 before the PV product: |err| <= ~2^-8 * max|v| per element; the bar used is
+max-abs <= 1.5e-2 * max|v| and per-row cosine >= 0.9995.
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from fmx_workloads import bf16_bits_to_f64, f32_to_bf16_bits  # noqa: E402
+from oracle.vfm_forward import attention  # noqa: E402
+
+MMA_SYNC, TCGEN05 = 1, 2
+
+
+@pytest.fixture(scope="module")
+def fmx():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test needs a CUDA device; the product has no CPU fallback")
+    import paper_2606_09643_b200 as pkg
+    return pkg.Fmx(0)
+
+
+def run_case(fmx, lengths, hq, hkv, dh, causal, impl, seed, q_scale=1.0, ramp=0.0):
+    rng = np.random.default_rng(seed)
+    N = int(np.sum(lengths))
+    dq, dkv = hq * dh, hkv * dh
+    x = rng.standard_normal((N, dq + 2 * dkv)).astype(np.float32)
+    x[:, :dq] *= q_scale
+    if ramp:
+        # key norms grow along each request, so the row maximum keeps rising: forces the O rescale path
+        off = 0
+        for n in lengths:
+            x[off:off + n, dq:dq + dkv] *= (1.0 + ramp * np.arange(n, dtype=np.float32) / n)[:, None]
+            off += n
+    bits = f32_to_bf16_bits(x)
+    qkv = torch.from_numpy(bits.view(np.int16)).cuda()
+    out = torch.full((N, dq), float("nan"), dtype=torch.bfloat16, device="cuda")
+    cu = np.concatenate([[0], np.cumsum(lengths)]).astype(np.int32)
+    fmx.debug_attention(qkv.data_ptr(), out.data_ptr(), cu, hq, hkv, dh, causal, impl)
+    torch.cuda.synchronize()
+    got = out.float().cpu().numpy().astype(np.float64)
+    xf = bf16_bits_to_f64(bits)
+    worst_abs, worst_cos = 0.0, 1.0
+    for i in range(len(lengths)):
+        r = xf[cu[i]:cu[i + 1]]
+        ref = attention(r[:, :dq], r[:, dq:dq + dkv], r[:, dq + dkv:], hq, hkv, dh, causal)
+        g = got[cu[i]:cu[i + 1]]
+        assert np.isfinite(g).all(), f"request {i}: non-finite attention output"
+        worst_abs = max(worst_abs, float(np.abs(g - ref).max()))
+        cos = np.sum(g * ref, axis=1) / (np.linalg.norm(g, axis=1) * np.linalg.norm(ref, axis=1) + 1e-300)
+        worst_cos = min(worst_cos, float(cos.min()))
+    vmax = float(np.abs(xf[:, dq + dkv:]).max())
+    assert worst_abs <= 1.5e-2 * vmax, f"max-abs {worst_abs:.3e} > 1.5e-2 * max|v| {vmax:.2f}"
+    assert worst_cos >= 0.9995, f"min row cosine {worst_cos:.6f}"
+
+
+CASES = [
+    # lengths,                        hq, hkv, dh, causal
+    ([64, 64, 64],                    4, 4, 64, 0),      # cfg2-like: one KV tile, half-empty q-tile
+    ([257, 257],                      3, 3, 64, 0),      # cfg3-like: 3 q-tiles, ragged last KV tile (1 key)
+    ([1, 2, 63, 65, 127, 129, 300],   2, 2, 64, 0),      # ragged everything
+    ([1, 64, 200, 1024],              12, 2, 128, 1),    # cfg4-like: GQA 6:1, causal, max length
+    ([130, 511, 77],                  4, 1, 128, 1),
+    ([256, 128, 384],                 2, 2, 128, 0),     # exact multiples of the tiles
+    ([640],                           2, 1, 64, 1),
+]
+
+
+@pytest.mark.parametrize("variant", [0, 1])       # 0: one q-tile per CTA, two CTAs per SM; 1: two q-tiles per CTA
+@pytest.mark.parametrize("lengths,hq,hkv,dh,causal", CASES)
+def test_tcgen05_attention_matches_oracle(fmx, lengths, hq, hkv, dh, causal, variant):
+    fmx.set_option("attention_variant", variant)
+    try:
+        run_case(fmx, lengths, hq, hkv, dh, causal, TCGEN05, seed=len(lengths) * 131 + dh)
+    finally:
+        fmx.set_option("attention_variant", 0)
+
+
+@pytest.mark.parametrize("lengths,hq,hkv,dh,causal", [
+    ([300, 700], 2, 2, 64, 0),
+    ([1024, 90], 6, 1, 128, 1),
+])
+@pytest.mark.parametrize("variant", [0, 1])
+def test_tcgen05_attention_large_scores_rescale_path(fmx, lengths, hq, hkv, dh, causal, variant):
+    """Scores of magnitude ~10^2 in the log2 domain with the largest ones late in the sequence: the
+    lazily updated reference maximum must move (more than once) and O in TMEM must be rescaled."""
+    fmx.set_option("attention_variant", variant)
+    try:
+        run_case(fmx, lengths, hq, hkv, dh, causal, TCGEN05, seed=7, q_scale=6.0, ramp=3.0)
+    finally:
+        fmx.set_option("attention_variant", 0)
+
+
+@pytest.mark.parametrize("lengths,hq,hkv,dh,causal", [
+    ([64, 64, 64], 4, 4, 32, 0),                          # cfg1's head_dim
+    ([1, 64, 200, 333], 12, 2, 128, 1),
+    ([257, 100], 3, 3, 64, 0),
+])
+def test_mma_sync_attention_matches_oracle(fmx, lengths, hq, hkv, dh, causal):
+    run_case(fmx, lengths, hq, hkv, dh, causal, MMA_SYNC, seed=5)
