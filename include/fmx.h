@@ -210,11 +210,14 @@ int fmx_debug_attention(fmx_ctx *ctx, const void *qkv, void *out, const int32_t 
 
 /* Tuning knobs (process-local experiments; defaults are what bench.py measures). */
 enum {
-  FMX_OPT_ATTENTION_IMPL = 0,    /* FMX_ATTN_AUTO | FMX_ATTN_MMA_SYNC | FMX_ATTN_TCGEN05 */
-  FMX_OPT_ATTENTION_VARIANT = 1  /* tcgen05 attention: 0 = one 128-query tile per CTA, two CTAs per SM;
-                                    1 = two q-tiles per CTA sharing K/V, one CTA per SM */
+  FMX_OPT_ATTENTION_IMPL = 0,    /* FMX_ATTN_AUTO | FMX_ATTN_MMA_SYNC | FMX_ATTN_TCGEN05 | FMX_ATTN_LANES */
+  FMX_OPT_ATTENTION_VARIANT = 1, /* tcgen05 attention: 0 = one 128-query tile per CTA; 1 = two q-tiles per CTA
+                                    sharing K/V.  FMX_ATTN_LANES: 0 / 1 / 2 = 4 / 2 / 3 lanes per CTA (head_dim 64) */
+  FMX_OPT_SHRINK_STAGES = 3,     /* shared-memory pipeline depth of the LoRA shrink kernel: 4 or 5 (default) */
+  FMX_OPT_PDL = 2                /* programmatic dependent launch of the forward's kernels (process-wide):
+                                    0 = off, 1 = always, 2 (default) = only for batches of <= 4096 token rows */
 };
-enum { FMX_ATTN_AUTO = 0, FMX_ATTN_MMA_SYNC = 1, FMX_ATTN_TCGEN05 = 2 };
+enum { FMX_ATTN_AUTO = 0, FMX_ATTN_MMA_SYNC = 1, FMX_ATTN_TCGEN05 = 2, FMX_ATTN_LANES = 3 };
 int fmx_set_option(fmx_ctx *ctx, int32_t option, int32_t value);
 
 /* ---- BFQ: host-side batch-aware fair-queue batch builder (§4.2, Eq. 1-3) ------------

@@ -52,7 +52,7 @@ class BfqParams(C.Structure):
     _fields_ = [("n_tasks", C.c_int32), ("b_max", C.c_int32), ("lat_ms", C.POINTER(C.c_double)), ("l_tok_ms", C.c_double)]
 
 
-OPTIONS = {"attention_impl": 0, "attention_variant": 1}
+OPTIONS = {"attention_impl": 0, "attention_variant": 1, "pdl": 2, "shrink_stages": 3}
 
 
 class FmxError(RuntimeError):
@@ -266,7 +266,7 @@ class Fmx:
                                             n_kv_heads, head_dim, int(causal), impl, stream or None))
 
     def set_option(self, option, value):
-        """option: 'attention_impl' (0 auto, 1 mma.sync, 2 tcgen05)."""
+        """option: 'attention_impl' (0 auto, 1 mma.sync, 2 tcgen05, 3 lanes), 'attention_variant', 'pdl' (0/1)."""
         _check(self.lib.fmx_set_option(self.h, OPTIONS[option], int(value)))
 
 

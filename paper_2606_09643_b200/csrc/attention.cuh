@@ -76,6 +76,8 @@ __global__ void __launch_bounds__(kAttnThreads) attention_kernel(const AttnArgs 
   __nv_bfloat16 *sV = sK + 2 * kAttnBKV * LD;           // 2 stages
 
   const int p = blockIdx.z, head = blockIdx.y, q0 = blockIdx.x * kAttnBQ;
+  griddep_launch();
+  griddep_wait();
   const int r0 = a.cu_tok[p], n = a.cu_tok[p + 1] - r0;
   if (q0 >= n) return;
   const int kvh = head / (a.n_q_heads / a.n_kv_heads);

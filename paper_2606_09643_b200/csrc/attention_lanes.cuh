@@ -58,15 +58,6 @@ __device__ __forceinline__ void umma_bf16_ts(uint32_t d_tmem, uint32_t a_tmem, u
       "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
       : "memory");
 }
-__device__ __forceinline__ void tmem_ld_32x16(uint32_t taddr, uint32_t (&v)[16]) {
-  asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
-      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];\n"
-      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
-        "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-      : "r"(taddr)
-      : "memory");
-}
 __device__ __forceinline__ void tmem_st_32x8(uint32_t taddr, const uint32_t (&v)[8]) {
   asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};\n" ::"r"(taddr), "r"(v[0]),
                "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7])
@@ -159,6 +150,8 @@ __global__ void __launch_bounds__(256 + 128 * kLanes, 1) attention_lanes_kernel(
   const int warp = threadIdx.x >> 5, lane_id = threadIdx.x & 31;
   const int wg = warp >> 2;                                                            // 0 producers, 1 MMA issuers, 2.. softmax
   const bool cu_in_smem = a.n_req < kLaneCuCap;
+  griddep_launch();
+  griddep_wait();
   if (cu_in_smem)
     for (int i = threadIdx.x; i <= a.n_req; i += blockDim.x) s_cu[i] = a.cu_tok[i];
   const int *cu = cu_in_smem ? s_cu : a.cu_tok;

@@ -87,6 +87,8 @@ __global__ void __launch_bounds__(128 + 128 * kQT, kMinBlocks) attention_tc_kern
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int p = blockIdx.z, head = blockIdx.y;
+  griddep_launch();
+  griddep_wait();
   const int r0 = a.cu_tok[p], n = a.cu_tok[p + 1] - r0;
   const int q0 = ((int)gridDim.x - 1 - (int)blockIdx.x) * (kAtBQ * kQT);      // heavy (late) causal tiles first
   if (q0 >= n) return;

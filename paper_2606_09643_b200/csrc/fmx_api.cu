@@ -14,6 +14,7 @@
 #include <vector>
 
 #include "attention.cuh"
+#include "attention_lanes.cuh"
 #include "attention_tc.cuh"
 #include "common.h"
 #include "fmx.h"
@@ -224,9 +225,29 @@ struct Launcher {
     if (int _e = (L).end()) return _e;            \
   } while (0)
 
+
+// Every forward-path kernel is launched with the programmatic-stream-serialization attribute (PDL, see ptx.cuh):
+// the next kernel's CTAs become resident and run their prologue while this one drains; each kernel blocks in
+// griddepcontrol.wait before it touches global memory.  FMX_OPT_PDL: 0 = plain stream order, 1 = always, 2 (default) =
+// only for small batches (<= kPdlAutoRows token rows), where the step is bound by launch latency: measured on B200 it
+// takes cfg1 from 0.208 to 0.163 ms per forward and is neutral to slightly negative (< 1 %) on the large configs.
+int g_pdl = 2, g_pdl_eff = 0;
+int g_shrink_stages = 5;
+constexpr int kPdlAutoRows = 4096;
+template <typename... KArgs, typename... Args>
+void launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args &&...args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = g_pdl_eff;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 template <int kVec>
 void launch_norm(cudaStream_t s, const float *X, bf16 *Y, const bf16 *g, const bf16 *b, int N, float eps, int rms) {
-  norm_kernel<kVec><<<(N + 7) / 8, 256, 0, s>>>(X, Y, g, b, N, eps, rms);
+  launch_k(norm_kernel<kVec>, (N + 7) / 8, 256, 0, s, X, Y, g, b, N, eps, rms);
 }
 bool dispatch_norm(cudaStream_t s, int d, const float *X, bf16 *Y, const bf16 *g, const bf16 *b, int N, float eps, int rms) {
   switch (d / 128) {
@@ -242,13 +263,13 @@ bool dispatch_norm(cudaStream_t s, int d, const float *X, bf16 *Y, const bf16 *g
 }
 bool dispatch_pool(cudaStream_t s, int d, int B, const PoolArgs &a) {
   switch (d / 128) {
-    case 1: final_pool_kernel<1><<<B, 128, 0, s>>>(a); return true;
-    case 2: final_pool_kernel<2><<<B, 128, 0, s>>>(a); return true;
-    case 4: final_pool_kernel<4><<<B, 128, 0, s>>>(a); return true;
-    case 6: final_pool_kernel<6><<<B, 128, 0, s>>>(a); return true;
-    case 8: final_pool_kernel<8><<<B, 128, 0, s>>>(a); return true;
-    case 12: final_pool_kernel<12><<<B, 128, 0, s>>>(a); return true;
-    case 16: final_pool_kernel<16><<<B, 128, 0, s>>>(a); return true;
+    case 1: launch_k(final_pool_kernel<1>, B, 128, 0, s, a); return true;
+    case 2: launch_k(final_pool_kernel<2>, B, 128, 0, s, a); return true;
+    case 4: launch_k(final_pool_kernel<4>, B, 128, 0, s, a); return true;
+    case 6: launch_k(final_pool_kernel<6>, B, 128, 0, s, a); return true;
+    case 8: launch_k(final_pool_kernel<8>, B, 128, 0, s, a); return true;
+    case 12: launch_k(final_pool_kernel<12>, B, 128, 0, s, a); return true;
+    case 16: launch_k(final_pool_kernel<16>, B, 128, 0, s, a); return true;
   }
   return false;
 }
@@ -258,7 +279,8 @@ bool norm_dim_supported(int d) {
 }
 
 void launch_shrink(fmx_ctx *c, cudaStream_t s, const GemmParams &p) {
-  shrink_kernel<kShrinkStages><<<c->sm_count, kGemmThreads, shrink_smem_bytes(), s>>>(p);
+  if (g_shrink_stages == 5) launch_k(shrink_kernel<5>, c->sm_count, kGemmThreads, shrink_smem_bytes<5>(), s, p);
+  else launch_k(shrink_kernel<4>, c->sm_count, kGemmThreads, shrink_smem_bytes<4>(), s, p);
 }
 
 // Pair tiles 256 x 256 when the chunk count is even, else 256 x 128; one cluster of 2 CTAs per SM pair.
@@ -267,17 +289,17 @@ void launch_pair_gemm(fmx_ctx *c, cudaStream_t s, const PairGemmParams &p) {
   const int pairs = c->sm_count / 2;
   if (pair_wide(p)) {
     const int tiles = p.n_ptiles * (p.n_chunks / 2);
-    pair_gemm_kernel<256><<<2 * std::min(tiles, pairs), kGemmThreads, pair_smem_bytes<256>(), s>>>(p);
+    launch_k(pair_gemm_kernel<256>, 2 * std::min(tiles, pairs), kGemmThreads, pair_smem_bytes<256>(), s, p);
   } else {
     const int tiles = p.n_ptiles * p.n_chunks;
-    pair_gemm_kernel<128><<<2 * std::min(tiles, pairs), kGemmThreads, pair_smem_bytes<128>(), s>>>(p);
+    launch_k(pair_gemm_kernel<128>, 2 * std::min(tiles, pairs), kGemmThreads, pair_smem_bytes<128>(), s, p);
   }
 }
 
 void launch_attention(cudaStream_t s, int dh, dim3 grid, const AttnArgs &a) {
-  if (dh == 32) attention_kernel<32><<<grid, kAttnThreads, attn_smem_bytes<32>(), s>>>(a);
-  else if (dh == 64) attention_kernel<64><<<grid, kAttnThreads, attn_smem_bytes<64>(), s>>>(a);
-  else attention_kernel<128><<<grid, kAttnThreads, attn_smem_bytes<128>(), s>>>(a);
+  if (dh == 32) launch_k(attention_kernel<32>, grid, kAttnThreads, attn_smem_bytes<32>(), s, a);
+  else if (dh == 64) launch_k(attention_kernel<64>, grid, kAttnThreads, attn_smem_bytes<64>(), s, a);
+  else launch_k(attention_kernel<128>, grid, kAttnThreads, attn_smem_bytes<128>(), s, a);
 }
 
 // The tcgen05 kernel serves head_dim 64 / 128 (a TMA box is 64 columns wide); head_dim 32 stays on mma.sync.
@@ -289,10 +311,31 @@ bool attn_use_tc(int impl, int dh, int max_len) {
   if (impl == FMX_ATTN_AUTO) return max_len > 64;
   return impl != FMX_ATTN_MMA_SYNC;
 }
+bool attn_use_lanes(int impl, int dh, int max_len) {
+  if (dh != 64 && dh != 128) return false;
+  return impl == FMX_ATTN_LANES;
+}
+template <int DH, int kLanes>
+void launch_attention_lanes_v(cudaStream_t s, int sm_count, int max_len, const AttnLaneArgs &a0) {
+  AttnLaneArgs a = a0;
+  a.n_qt_max = (max_len + kAtBQ - 1) / kAtBQ;
+  const long long items = (long long)a.n_qt_max * a.n_req * a.n_q_heads;
+  const int grid = (int)std::min<long long>(sm_count, (items + kLanes - 1) / kLanes);
+  launch_k((attention_lanes_kernel<DH, kLanes>), grid, attn_lanes_threads<kLanes>(), attn_lanes_smem_bytes<DH, kLanes>(), s, a);
+}
+void launch_attention_lanes(cudaStream_t s, int sm_count, int dh, int variant, int max_len, const AttnLaneArgs &a) {
+  if (dh == 64) {
+    if (variant == 0) launch_attention_lanes_v<64, 4>(s, sm_count, max_len, a);
+    else if (variant == 1) launch_attention_lanes_v<64, 2>(s, sm_count, max_len, a);
+    else launch_attention_lanes_v<64, 3>(s, sm_count, max_len, a);
+  } else {
+    launch_attention_lanes_v<128, 2>(s, sm_count, max_len, a);
+  }
+}
 template <int DH, int kQT, int kSt, int kMinB>
 void launch_attention_tc_v(cudaStream_t s, int max_len, int n_heads, int B, const AttnTcArgs &a) {
   dim3 grid((max_len + kAtBQ * kQT - 1) / (kAtBQ * kQT), n_heads, B);
-  attention_tc_kernel<DH, kQT, kSt, kMinB><<<grid, attn_tc_threads<kQT>(), attn_tc_smem_bytes<DH, kQT, kSt>(), s>>>(a);
+  launch_k((attention_tc_kernel<DH, kQT, kSt, kMinB>), grid, attn_tc_threads<kQT>(), attn_tc_smem_bytes<DH, kQT, kSt>(), s, a);
 }
 void launch_attention_tc(cudaStream_t s, int dh, int variant, int max_len, int n_heads, int B, const AttnTcArgs &a) {
   if (dh == 64) {
@@ -327,9 +370,14 @@ int set_kernel_attrs() {
   CU_OK((set_attn_tc_attr<64, 2, 3, 1>()));
   CU_OK((set_attn_tc_attr<128, 1, 2, 2>()));
   CU_OK((set_attn_tc_attr<128, 2, 3, 1>()));
+  CU_OK((cudaFuncSetAttribute(attention_lanes_kernel<64, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_lanes_smem_bytes<64, 4>())));
+  CU_OK((cudaFuncSetAttribute(attention_lanes_kernel<64, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_lanes_smem_bytes<64, 2>())));
+  CU_OK((cudaFuncSetAttribute(attention_lanes_kernel<64, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_lanes_smem_bytes<64, 3>())));
+  CU_OK((cudaFuncSetAttribute(attention_lanes_kernel<128, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_lanes_smem_bytes<128, 2>())));
   CU_OK(cudaFuncSetAttribute(pair_gemm_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<256>()));
   CU_OK(cudaFuncSetAttribute(pair_gemm_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<128>()));
-  CU_OK(cudaFuncSetAttribute(shrink_kernel<kShrinkStages>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes()));
+  CU_OK(cudaFuncSetAttribute(shrink_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<4>()));
+  CU_OK(cudaFuncSetAttribute(shrink_kernel<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<5>()));
   CU_OK(cudaFuncSetAttribute(attention_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_smem_bytes<32>()));
   CU_OK(cudaFuncSetAttribute(attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_smem_bytes<64>()));
   CU_OK(cudaFuncSetAttribute(attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_smem_bytes<128>()));
@@ -736,6 +784,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   if (w.bytes > workspace_bytes) return fmx_fail(FMX_E_WORKSPACE, "forward_mixed: workspace %zu B < required %zu B", workspace_bytes, w.bytes);
 
   const int Ni = (int)N;
+  g_pdl_eff = g_pdl == 1 || (g_pdl == 2 && Ni <= kPdlAutoRows);
   Launcher Lh{c, s};
   // ---- S1: ids/lengths to the device, counting sort, tables ----
   memcpy(c->h_stage, task_ids, sizeof(int) * B);
@@ -748,8 +797,8 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   else if (d.input_kind == FMX_INPUT_TOKEN_IDS) { sa.in_per_tok = 1; sa.in_per_req = 0; }
   else if (d.img_c) { sa.in_per_tok = 0; sa.in_per_req = (long long)d.img_c * d.img_hw * d.img_hw; }
   else { sa.in_per_tok = 0; sa.in_per_req = (long long)(d.tokens_per_request - (d.has_cls ? 1 : 0)) * d.patch_dim; }
-  LAUNCH(Lh, F_SORT, (task_sort_kernel<<<1, kSortThreads, 0, s>>>(sa)));
-  LAUNCH(Lh, F_SORT, (row_tables_kernel<<<(Ni + 255) / 256, 256, 0, s>>>(w.t.cu_tok, B, Ni, w.t.row_req, w.t.row_pos)));
+  LAUNCH(Lh, F_SORT, (launch_k(task_sort_kernel, 1, kSortThreads, 0, s, sa)));
+  LAUNCH(Lh, F_SORT, (launch_k(row_tables_kernel, (Ni + 255) / 256, 256, 0, s, w.t.cu_tok, B, Ni, w.t.row_req, w.t.row_pos)));
 
   // ---- common GEMM parameter pieces ----
   GemmParams sbase{};                       // segmented shrink
@@ -805,7 +854,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     pa.inputs = (const bf16 *)inputs; pa.perm = w.t.perm; pa.row_req = w.t.row_req; pa.row_pos = w.t.row_pos; pa.in_off = w.t.in_off;
     pa.N = Ni; pa.patch_dim = d.patch_dim; pa.Kp = bb.Kp; pa.has_cls = d.has_cls; pa.img_c = d.img_c; pa.img_hw = d.img_hw; pa.patch_hw = d.patch_hw;
     pa.A = w.Hid;
-    LAUNCH(Lh, F_EMBED, (pack_patches_kernel<<<Ni, 128, 0, s>>>(pa)));
+    LAUNCH(Lh, F_EMBED, (launch_k(pack_patches_kernel, Ni, 128, 0, s, pa)));
     if ((e = encode_2d(c, &mPk, w.Hid, Ni, bb.Kp, bb.Kp, 128))) return e;
     PairGemmParams p = base;
     p.mode = GM_EMBED_F32; p.amap = mPk; p.K = bb.Kp; p.n_chunks = d.d_model / 128;
@@ -815,7 +864,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     EmbedArgs ea{};
     ea.inputs = inputs; ea.perm = w.t.perm; ea.row_req = w.t.row_req; ea.row_pos = w.t.row_pos; ea.in_off = w.t.in_off;
     ea.N = Ni; ea.d = d.d_model; ea.X = w.X; ea.table = (const bf16 *)d.embed_table; ea.pos = (const bf16 *)d.embed_pos;
-    LAUNCH(Lh, F_EMBED, (embed_rows_kernel<<<(Ni + 7) / 8, 256, 0, s>>>(ea, d.input_kind == FMX_INPUT_TOKEN_IDS)));
+    LAUNCH(Lh, F_EMBED, (launch_k(embed_rows_kernel, (Ni + 7) / 8, 256, 0, s, ea, d.input_kind == FMX_INPUT_TOKEN_IDS)));
   }
 
   // ---- layers ----
@@ -839,9 +888,14 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     if (d.rope_theta > 0) {
       const int nh = d.n_q_heads + d.n_kv_heads;
       const long long total = (long long)Ni * nh * (d.head_dim / 16);
-      LAUNCH(Lh, F_ROPE, (rope_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(w.QKV, bb.d_qkv, w.t.row_pos, bb.rope_cs, Ni, nh, d.head_dim)));
+      LAUNCH(Lh, F_ROPE, (launch_k(rope_kernel, (unsigned)((total + 255) / 256), 256, 0, s, w.QKV, bb.d_qkv, w.t.row_pos, bb.rope_cs, Ni, nh, d.head_dim)));
     }
-    if (attn_use_tc(c->opt_attn_impl, d.head_dim, max_len)) {
+    if (attn_use_lanes(c->opt_attn_impl, d.head_dim, max_len)) {
+      AttnLaneArgs la{};
+      la.qkv_map = mQKV64; la.out = w.AttnO; la.cu_tok = w.t.cu_tok; la.ld_out = bb.d_q; la.n_req = B;
+      la.n_q_heads = d.n_q_heads; la.n_kv_heads = d.n_kv_heads; la.causal = d.causal; la.scale_log2 = scale_log2;
+      LAUNCH(Lh, F_ATTN, launch_attention_lanes(s, c->sm_count, d.head_dim, c->opt_attn_variant, max_len, la));
+    } else if (attn_use_tc(c->opt_attn_impl, d.head_dim, max_len)) {
       AttnTcArgs ta{};
       ta.qkv_map = mQKV64; ta.out = w.AttnO; ta.cu_tok = w.t.cu_tok; ta.ld_out = bb.d_q;
       ta.n_q_heads = d.n_q_heads; ta.n_kv_heads = d.n_kv_heads; ta.causal = d.causal; ta.scale_log2 = scale_log2;
@@ -905,7 +959,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   ha.task_head_kind = c->d_task_head_kind; ha.task_head_out = c->d_task_head_out;
   ha.task_head_W = (const bf16 *const *)c->d_task_head_W; ha.task_head_b = (const bf16 *const *)c->d_task_head_b;
   ha.out = outputs; ha.d = d.d_model;
-  LAUNCH(Lh, F_HEAD, (head_kernel<<<dim3(B, (max_out + 7) / 8), 256, 0, s>>>(ha)));
+  LAUNCH(Lh, F_HEAD, (launch_k(head_kernel, dim3(B, (max_out + 7) / 8), 256, 0, s, ha)));
 
   {
     void *bufs[7] = {w.X, w.Xn, w.QKV, w.AttnO, w.Hid, w.U, w.feat};
@@ -1082,7 +1136,13 @@ int fmx_debug_attention(fmx_ctx *c, const void *qkv, void *out, const int32_t *c
   CU_OK(cudaMemcpyAsync(c->d_dbg_cu, cu_tok, sizeof(int) * (n_req + 1), cudaMemcpyHostToDevice, s));
   const int N = cu_tok[n_req], d_q = n_q_heads * head_dim, d_qkv = (n_q_heads + 2 * n_kv_heads) * head_dim;
   const float scale_log2 = 1.4426950408889634f / sqrtf((float)head_dim);
-  if (attn_use_tc(impl, head_dim, max_len)) {
+  if (attn_use_lanes(impl, head_dim, max_len)) {
+    AttnLaneArgs la{};
+    if (int e = encode_2d(c, &la.qkv_map, qkv, N, d_qkv, d_qkv, 64)) return e;
+    la.out = (bf16 *)out; la.cu_tok = c->d_dbg_cu; la.ld_out = d_q; la.n_req = n_req; la.n_q_heads = n_q_heads; la.n_kv_heads = n_kv_heads;
+    la.causal = causal; la.scale_log2 = scale_log2;
+    launch_attention_lanes(s, c->sm_count, head_dim, c->opt_attn_variant, max_len, la);
+  } else if (attn_use_tc(impl, head_dim, max_len)) {
     AttnTcArgs ta{};
     if (int e = encode_2d(c, &ta.qkv_map, qkv, N, d_qkv, d_qkv, 64)) return e;
     ta.out = (bf16 *)out; ta.cu_tok = c->d_dbg_cu; ta.ld_out = d_q; ta.n_q_heads = n_q_heads; ta.n_kv_heads = n_kv_heads;
@@ -1104,11 +1164,19 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
   std::lock_guard<std::mutex> lk(c->mu);
   switch (option) {
     case FMX_OPT_ATTENTION_IMPL:
-      if (value < FMX_ATTN_AUTO || value > FMX_ATTN_TCGEN05) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attention impl %d", value);
+      if (value < FMX_ATTN_AUTO || value > FMX_ATTN_LANES) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attention impl %d", value);
       c->opt_attn_impl = value;
       return FMX_OK;
+    case FMX_OPT_SHRINK_STAGES:
+      if (value != 4 && value != 5) return fmx_fail(FMX_E_INVALID_ARG, "set_option: shrink stages %d", value);
+      g_shrink_stages = value;
+      return FMX_OK;
+    case FMX_OPT_PDL:
+      if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: pdl %d", value);
+      g_pdl = value;
+      return FMX_OK;
     case FMX_OPT_ATTENTION_VARIANT:
-      if (value < 0 || value > 1) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attention variant %d", value);
+      if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attention variant %d", value);
       c->opt_attn_variant = value;
       return FMX_OK;
   }

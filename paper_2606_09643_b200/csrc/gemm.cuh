@@ -72,21 +72,22 @@ __device__ __forceinline__ void chunk_source(const GemmParams &p, int c, int &s,
   }
 }
 
-// GeLU(x) = x * Phi(x), Phi(x) = 0.5 erfc(-x / sqrt 2).  erfc by Abramowitz & Stegun 7.1.26 (|error| <= 1.5e-7 in erf,
-// far below the bf16 rounding of the output): erfc(z) = (a1 t + ... + a5 t^5) exp(-z^2), t = 1 / (1 + p z), z >= 0.
-// Phi is formed without cancellation on either side: x < 0: 0.5 P E;  x >= 0: 1 - 0.5 P E.  Two MUFU ops (rcp, ex2) and
-// ~10 FMAs per element instead of erff's branchy ~30 instructions: the GeLU epilogue of the FFN-in GEMM was issue-bound.
+// GeLU(x) = x * Phi(x), Phi(x) = 0.5 erfc(-x / sqrt 2), with erfc(z) = 2^(-z Q(z)) for z >= 0, Q a quartic fitted (minimax
+// on |erf error|, fp32 evaluation) to -log2(erfc z) / z on [0, 4.2]: |error| <= 6.7e-7 in erf, |error| <= 1.4e-6 in GeLU over
+// [-12, 12], far below the bf16 rounding of the output; beyond the fit range the quartic keeps growing, so erfc -> 0.  The
+// 1/sqrt(2) is folded into the coefficients (in |x|).  Phi is formed without cancellation on either side: x < 0: 0.5 E;
+// x >= 0: 1 - 0.5 E.  One MUFU op (ex2) and 4 FMAs per element: the GeLU epilogue of the FFN-in GEMM was issue-bound with
+// erff (~30 instructions) and still the slower side with the Abramowitz-Stegun 7.1.26 form (rcp + ex2 + 10 FMA-pipe ops).
 __device__ __forceinline__ float gelu_erf_f(float x) {
-  const float z = fabsf(x) * 0.70710678118654752440f;
-  float t, e;
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t) : "f"(fmaf(0.3275911f, z, 1.0f)));
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(z * z * -1.4426950408889634f));
-  float pl = fmaf(1.061405429f, t, -1.453152027f);
-  pl = fmaf(pl, t, 1.421413741f);
-  pl = fmaf(pl, t, -0.284496736f);
-  pl = fmaf(pl, t, 0.254829592f);
-  const float half_pe = 0.5f * pl * t * e;
-  return x * (x < 0.0f ? half_pe : 1.0f - half_pe);
+  const float ax = fabsf(x);
+  float p = fmaf(-0.00052327975f, ax, 0.0074127913f);
+  p = fmaf(p, ax, -0.0525887412f);
+  p = fmaf(p, ax, -0.459236082f);
+  p = fmaf(p, ax, -1.15109488f);
+  float e;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(p * ax));
+  const float h = 0.5f * e;
+  return x * (x < 0.0f ? h : 1.0f - h);
 }
 __device__ __forceinline__ float silu_f(float x) { return x / (1.0f + __expf(-x)); }
 
@@ -108,7 +109,6 @@ __global__ void __launch_bounds__(kGemmThreads, 1) shrink_kernel(const __grid_co
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int nK = (p.K + kBK - 1) / kBK;
-  const int total_units = 2 * (*p.n_blk);
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < kStages; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
@@ -123,6 +123,9 @@ __global__ void __launch_bounds__(kGemmThreads, 1) shrink_kernel(const __grid_co
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = tmem_base_slot;
+  griddep_launch();
+  griddep_wait();
+  const int total_units = 2 * (*p.n_blk);
   // unit -> (block, half); live = the half holds at least one row of the block's task
   auto unit_live = [&](int unit, int &blk, int &half) {
     blk = unit >> 1; half = unit & 1;
@@ -139,6 +142,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) shrink_kernel(const __grid_co
         if (!unit_live(unit, blk, half)) continue;
         const int m0 = p.blk_tile[blk] * 256 + half * kBM;
         const int coff = p.task_coff[p.blk_task[blk]];
+        // All 64 slab rows of each target are fetched whatever the task's rank: fetching only the padded rank with a
+        // 16-row box measured SLOWER on B200 (cfg4: 11.6 vs 10.2 ms per step) although it moves fewer bytes.
         for (int kb = 0; kb < nK; ++kb) {
           mbar_wait(&empty_bar[stage], phase ^ 1);
           uint8_t *sa = smem + stage * kStageBytes, *sb = sa + kATileBytes;
@@ -226,7 +231,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) shrink_kernel(const __grid_co
   if (warp == 2) tmem_dealloc(tmem_base, 512);
 }
 
-constexpr int kShrinkStages = 4;
-constexpr int shrink_smem_bytes() { return kShrinkStages * (kATileBytes + 3 * 64 * kBK * 2) + 1024; }
+template <int kStages>
+constexpr int shrink_smem_bytes() { return kStages * (kATileBytes + 3 * 64 * kBK * 2) + 1024; }
 
 }  // namespace fmx

@@ -96,6 +96,8 @@ __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortAr
   __shared__ int s_rank[4096];             // rank of request i within its task
   const int tid = threadIdx.x, B = a.B, T = a.T;
   const SegTables &t = a.t;
+  griddep_launch();
+  griddep_wait();
 
   for (int i = tid; i <= T; i += blockDim.x) s_cnt[i] = 0;
   __syncthreads();
@@ -178,6 +180,8 @@ __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortAr
 // row -> (sorted request index, position within the request)
 __global__ void row_tables_kernel(const int *__restrict__ cu_tok, int B, int N, int *__restrict__ row_req,
                                   int *__restrict__ row_pos) {
+  griddep_launch();
+  griddep_wait();
   const int r = blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= N) return;
   int lo = 0, hi = B;                          // largest p with cu_tok[p] <= r
@@ -199,6 +203,8 @@ struct EmbedArgs {
 
 // EMBEDDED: X[r] = x_i[pos] (+ Pos[pos]);   one warp per row, 8 bf16 per lane per step
 __global__ void embed_rows_kernel(const EmbedArgs a, int token_ids) {
+  griddep_launch();
+  griddep_wait();
   const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (warp >= a.N) return;
   const int r = warp, pos = a.row_pos[r], i = a.perm[a.row_req[r]];
@@ -234,6 +240,8 @@ struct PackArgs {
 
 // PATCH_LINEAR: gather (and patchify) into the A operand of the embed GEMM.  One block per row.
 __global__ void pack_patches_kernel(const PackArgs a) {
+  griddep_launch();
+  griddep_wait();
   const int r = blockIdx.x;
   const int pos = a.row_pos[r], i = a.perm[a.row_req[r]];
   const __nv_bfloat16 *src = a.inputs + a.in_off[i];
@@ -282,6 +290,8 @@ template <int kVec>   // float4s per lane: d = 128 * kVec
 __global__ void __launch_bounds__(256) norm_kernel(const float *__restrict__ X, __nv_bfloat16 *__restrict__ Y,
                                                    const __nv_bfloat16 *__restrict__ g,
                                                    const __nv_bfloat16 *__restrict__ b, int N, float eps, int rms) {
+  griddep_launch();
+  griddep_wait();
   const int row = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (row >= N) return;
   constexpr int d = 128 * kVec;
@@ -326,6 +336,8 @@ __global__ void __launch_bounds__(256) norm_kernel(const float *__restrict__ X, 
 // 64 bytes of the table, so a warp touches whole 128-byte lines (dh/2 must be a multiple of 8).
 __global__ void __launch_bounds__(256) rope_kernel(__nv_bfloat16 *qkv, int ld, const int *__restrict__ row_pos,
                                                    const float2 *__restrict__ cs, int N, int n_heads_qk, int dh) {
+  griddep_launch();
+  griddep_wait();
   const int half = dh >> 1, vec_per_head = half >> 3;
   const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;     // (row, head, vector of 8 pairs)
   const long long total = (long long)N * n_heads_qk * vec_per_head;
@@ -375,6 +387,8 @@ struct PoolArgs {
 // accumulated per warp in registers (fixed row->warp assignment and fixed combine order: deterministic).
 template <int kVec>
 __global__ void __launch_bounds__(128) final_pool_kernel(const PoolArgs a) {
+  griddep_launch();
+  griddep_wait();
   constexpr int d = 128 * kVec;
   __shared__ float s_part[4][d];
   const int p = blockIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -452,6 +466,8 @@ struct HeadArgs {
 // grid (sorted request p, output tile of 8): each warp computes one output o as a dot product over
 // d_feat with 16-byte loads; result written straight to the caller's buffer in ORIGINAL order.
 __global__ void __launch_bounds__(256) head_kernel(const HeadArgs a) {
+  griddep_launch();
+  griddep_wait();
   const int p = blockIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int t = a.task_sorted[p];
   const int o = blockIdx.y * 8 + warp;

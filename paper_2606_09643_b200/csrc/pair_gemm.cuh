@@ -151,6 +151,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
   cluster_sync_all();
   tc_fence_after();
   const uint32_t tmem_base = tmem_base_slot;
+  griddep_launch();
+  griddep_wait();
 
   if (warp == 0) {
     // ================================ TMA producer (both CTAs) ================================

@@ -16,7 +16,7 @@ pytestmark = pytest.mark.gpu
 from fmx_workloads import bf16_bits_to_f64, f32_to_bf16_bits  # noqa: E402
 from oracle.vfm_forward import attention  # noqa: E402
 
-MMA_SYNC, TCGEN05 = 1, 2
+MMA_SYNC, TCGEN05, LANES = 1, 2, 3
 
 
 @pytest.fixture(scope="module")
@@ -96,6 +96,28 @@ def test_tcgen05_attention_large_scores_rescale_path(fmx, lengths, hq, hkv, dh, 
         run_case(fmx, lengths, hq, hkv, dh, causal, TCGEN05, seed=7, q_scale=6.0, ramp=3.0)
     finally:
         fmx.set_option("attention_variant", 0)
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2])    # 4, 2, 3 lanes per CTA (head_dim 128: always 2)
+@pytest.mark.parametrize("lengths,hq,hkv,dh,causal", CASES + [([17] * 40 + [257] * 9, 16, 16, 64, 0)])
+def test_lanes_attention_matches_oracle(fmx, lengths, hq, hkv, dh, causal, variant):
+    """Persistent multi-lane tcgen05 kernel (P kept in TMEM, 16-key tail tile): more work items than lanes, so every
+    lane walks several items and the Q / K / V rings wrap."""
+    if dh == 128 and variant > 0:
+        pytest.skip("head_dim 128 has one lane count")
+    fmx.set_option("attention_variant", variant)
+    try:
+        run_case(fmx, lengths, hq, hkv, dh, causal, LANES, seed=len(lengths) * 17 + dh)
+    finally:
+        fmx.set_option("attention_variant", 0)
+
+
+@pytest.mark.parametrize("lengths,hq,hkv,dh,causal", [
+    ([300, 700], 2, 2, 64, 0),
+    ([1024, 90], 6, 1, 128, 1),
+])
+def test_lanes_attention_large_scores_rescale_path(fmx, lengths, hq, hkv, dh, causal):
+    run_case(fmx, lengths, hq, hkv, dh, causal, LANES, seed=7, q_scale=6.0, ramp=3.0)
 
 
 @pytest.mark.parametrize("lengths,hq,hkv,dh,causal", [
