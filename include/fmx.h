@@ -214,6 +214,7 @@ enum {
   FMX_OPT_ATTENTION_VARIANT = 1, /* tcgen05 attention: 0 = one 128-query tile per CTA; 1 = two q-tiles per CTA
                                     sharing K/V.  FMX_ATTN_LANES: 0 / 1 / 2 = 4 / 2 / 3 lanes per CTA (head_dim 64) */
   FMX_OPT_SHRINK_STAGES = 3,     /* shared-memory pipeline depth of the LoRA shrink kernel: 4 or 5 (default) */
+  FMX_OPT_HALF_TILES = 4,        /* 1 (default): a short last GEMM wave is cut into 256 x 128 half tiles */
   FMX_OPT_PDL = 2                /* programmatic dependent launch of the forward's kernels (process-wide):
                                     0 = off, 1 = always, 2 (default) = only for batches of <= 4096 token rows */
 };

@@ -233,6 +233,7 @@ struct Launcher {
 // takes cfg1 from 0.208 to 0.163 ms per forward and is neutral to slightly negative (< 1 %) on the large configs.
 int g_pdl = 2, g_pdl_eff = 0;
 int g_shrink_stages = 5;
+int g_half_tiles = 1;
 constexpr int kPdlAutoRows = 4096;
 template <typename... KArgs, typename... Args>
 void launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args &&...args) {
@@ -289,7 +290,13 @@ void launch_pair_gemm(fmx_ctx *c, cudaStream_t s, const PairGemmParams &p) {
   const int pairs = c->sm_count / 2;
   if (pair_wide(p)) {
     const int tiles = p.n_ptiles * (p.n_chunks / 2);
-    launch_k(pair_gemm_kernel<256>, 2 * std::min(tiles, pairs), kGemmThreads, pair_smem_bytes<256>(), s, p);
+    // Wave quantisation: when the last wave would hold at most half as many tiles as there are pairs, its tiles are cut
+    // into 256 x 128 halves so that it lasts half a tile time (cfg2 O / FFN-out: 256 tiles on 74 pairs, 4 -> 3.5 waves).
+    PairGemmParams q = p;
+    const int rem = tiles % pairs;
+    q.n_full = (g_half_tiles && p.mode != GM_OUT_BF16_SWIGLU && tiles > pairs && rem > 0 && 2 * rem <= pairs) ? tiles - rem : -1;
+    const int items = q.n_full >= 0 ? q.n_full + 2 * rem : tiles;
+    launch_k(pair_gemm_kernel<256>, 2 * std::min(items, pairs), kGemmThreads, pair_smem_bytes<256>(), s, q);
   } else {
     const int tiles = p.n_ptiles * p.n_chunks;
     launch_k(pair_gemm_kernel<128>, 2 * std::min(tiles, pairs), kGemmThreads, pair_smem_bytes<128>(), s, p);
@@ -858,7 +865,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     if ((e = encode_2d(c, &mPk, w.Hid, Ni, bb.Kp, bb.Kp, 128))) return e;
     PairGemmParams p = base;
     p.mode = GM_EMBED_F32; p.amap = mPk; p.K = bb.Kp; p.n_chunks = d.d_model / 128;
-    p.wmap[0] = bb.mEmbedW[wv(p)]; p.omap = oX; p.posb = bb.posb; p.ld_pos = d.d_model;
+    p.wmap[0] = bb.mEmbedW[wv(p)]; p.wmap_h[0] = bb.mEmbedW[1]; p.omap = oX; p.posb = bb.posb; p.ld_pos = d.d_model;
     LAUNCH(Lh, F_EMBED, launch_pair_gemm(c, s, p));
   } else {
     EmbedArgs ea{};
@@ -879,6 +886,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       p.mode = GM_OUT_BF16; p.amap = mXn; p.K = d.d_model; p.n_chunks = bb.d_qkv / 128;
       const int v = wv(p);
       p.wmap[0] = bb.mWq[v][l]; p.wmap[1] = bb.mWk[v][l]; p.wmap[2] = bb.mWv[v][l];
+      p.wmap_h[0] = bb.mWq[1][l]; p.wmap_h[1] = bb.mWk[1][l]; p.wmap_h[2] = bb.mWv[1][l];
       p.src_end[0] = bb.d_q / 128; p.src_end[1] = (bb.d_q + bb.d_kv) / 128; p.src_end[2] = 1 << 30;
       p.bias[0] = (const bf16 *)bb.bq[l]; p.bias[1] = (const bf16 *)bb.bk[l]; p.bias[2] = (const bf16 *)bb.bv[l];
       set_lora(p, 0, FMX_TGT_Q, l); set_lora(p, 1, FMX_TGT_K, l); set_lora(p, 2, FMX_TGT_V, l);
@@ -912,7 +920,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       if ((e = shrink(mAttnO, bb.d_q, tgs, 1, l))) return e;
       PairGemmParams p = base;
       p.mode = GM_RESID_F32; p.amap = mAttnO; p.K = bb.d_q; p.n_chunks = d.d_model / 128;
-      p.wmap[0] = bb.mWo[wv(p)][l]; p.bias[0] = (const bf16 *)bb.bo[l];
+      p.wmap[0] = bb.mWo[wv(p)][l]; p.wmap_h[0] = bb.mWo[1][l]; p.bias[0] = (const bf16 *)bb.bo[l];
       set_lora(p, 0, FMX_TGT_O, l);
       p.omap = oX;
       LAUNCH(Lh, F_GEMM_O, launch_pair_gemm(c, s, p));
@@ -933,7 +941,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       if ((e = shrink(mXn, d.d_model, tgs, 1, l))) return e;
       PairGemmParams p = base;
       p.mode = d.act == FMX_ACT_GELU_ERF ? GM_OUT_BF16_GELU : GM_OUT_BF16_RELU; p.amap = mXn; p.K = d.d_model; p.n_chunks = d.d_ffn / 128;
-      p.wmap[0] = bb.mWup[wv(p)][l]; p.bias[0] = (const bf16 *)bb.bup[l];
+      p.wmap[0] = bb.mWup[wv(p)][l]; p.wmap_h[0] = bb.mWup[1][l]; p.bias[0] = (const bf16 *)bb.bup[l];
       set_lora(p, 0, FMX_TGT_UP, l);
       p.omap = oHid;
       LAUNCH(Lh, F_GEMM_FFN_IN, launch_pair_gemm(c, s, p));
@@ -943,7 +951,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       if ((e = shrink(mHid, d.d_ffn, tgs, 1, l))) return e;
       PairGemmParams p = base;
       p.mode = GM_RESID_F32; p.amap = mHid; p.K = d.d_ffn; p.n_chunks = d.d_model / 128;
-      p.wmap[0] = bb.mWdown[wv(p)][l]; p.bias[0] = (const bf16 *)bb.bdown[l];
+      p.wmap[0] = bb.mWdown[wv(p)][l]; p.wmap_h[0] = bb.mWdown[1][l]; p.bias[0] = (const bf16 *)bb.bdown[l];
       set_lora(p, 0, FMX_TGT_DOWN, l);
       p.omap = oX;
       LAUNCH(Lh, F_GEMM_FFN_OUT, launch_pair_gemm(c, s, p));
@@ -1106,6 +1114,7 @@ int fmx_debug_gemm(fmx_ctx *c, const void *A, const void *W, float *C, int32_t M
   p.M = M; p.K = K; p.n_chunks = N / 128; p.n_ptiles = (M + kPairRows - 1) / kPairRows; p.mode = GM_OUT_F32;
   if ((e = encode_2d(c, &p.amap, A, M, K, K, 128))) return e;
   if ((e = encode_2d(c, &p.wmap[0], W, N, K, K, pair_wide(p) ? 128 : 64))) return e;
+  if ((e = encode_2d(c, &p.wmap_h[0], W, N, K, K, 64))) return e;
   if ((e = encode_2d(c, &p.omap, C, M, N, N, 128, true))) return e;
   for (int i = 0; i < 3; ++i) { p.lora_tgt[i] = -1; p.src_end[i] = 1 << 30; }
   launch_pair_gemm(c, (cudaStream_t)cuda_stream, p);
@@ -1170,6 +1179,9 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
     case FMX_OPT_SHRINK_STAGES:
       if (value != 4 && value != 5) return fmx_fail(FMX_E_INVALID_ARG, "set_option: shrink stages %d", value);
       g_shrink_stages = value;
+      return FMX_OK;
+    case FMX_OPT_HALF_TILES:
+      g_half_tiles = value ? 1 : 0;
       return FMX_OK;
     case FMX_OPT_PDL:
       if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: pdl %d", value);

@@ -46,12 +46,15 @@ constexpr int kStagingBytes = 2 * 2 * 16384;      // 2 warpgroups x 2 buffers x 
 struct PairGemmParams {
   CUtensorMap amap;        // A [M, K] bf16, box {64, 128}
   CUtensorMap wmap[3];     // weight sources [rows_s, K] bf16, box {64, kBN/2}
+  CUtensorMap wmap_h[3];   // the same sources with box {64, 64}: W rows of a HALF tile (kBN = 256 only)
   CUtensorMap umap;        // U [n_blk_cap*256, 192] bf16, box {64, 128}
   CUtensorMap lmap[3];     // B-slabs [d_out_s, Rcap] bf16, box {64, 64}
   CUtensorMap omap;        // output [M, ld]: bf16 box {64, 128}, or fp32 box {32, 128}
   int M, K;
   int n_chunks;            // N / 128
   int n_ptiles;            // ceil(M / 256)
+  int n_full;              // kBN = 256: tiles [0, n_full) are 256 x 256; each later tile is cut into two 256 x 128 halves
+                           // taken by different pairs, so a short last wave costs half a tile time (-1 = no half tiles)
   int mode;                // GemmMode (not GM_SHRINK)
   int interleave2;         // chunk c -> source c&1, row (c>>1)*128  (SwiGLU)
   int has_lora;
@@ -118,6 +121,23 @@ __device__ __forceinline__ void stage_bf16_32(const uint32_t (&v)[32], const __n
                    pack_bf16(f[8 * j + 6], f[8 * j + 7]));
 }
 
+// Work item `item` of the persistent loop -> (row tile, first chunk, chunk count).  Items [0, n_full) are whole tiles of
+// kCH chunks; item n_full + 2 i + h is half h (one chunk) of whole tile n_full + i.
+template <int kCH>
+__device__ __forceinline__ void pair_decode(const PairGemmParams &p, int item, int n_ntiles, int n_full, int &m_pt, int &c0, int &nch) {
+  int tile = item;
+  int h = -1;
+  if (kCH == 2 && item >= n_full) {
+    const int t2 = item - n_full;
+    tile = n_full + (t2 >> 1);
+    h = t2 & 1;
+  }
+  m_pt = tile / n_ntiles;
+  const int n_tile = tile - m_pt * n_ntiles;
+  c0 = n_tile * kCH + (h > 0 ? 1 : 0);
+  nch = h >= 0 ? 1 : kCH;
+}
+
 template <int kBN>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pair_gemm_kernel(const __grid_constant__ PairGemmParams p) {
   constexpr int kCH = kBN / kChunk;
@@ -135,7 +155,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
   const uint32_t rank = cluster_ctarank();
   const int nK = (p.K + kBK - 1) / kBK;
   const int n_ntiles = p.n_chunks / kCH;
-  const int total_tiles = p.n_ptiles * n_ntiles;
+  const int whole_tiles = p.n_ptiles * n_ntiles;
+  const int n_full = (kCH == 2 && p.n_full >= 0) ? p.n_full : whole_tiles;
+  const int total_tiles = n_full + 2 * (whole_tiles - n_full);
   const int tile0 = (int)cluster_id_x(), tile_step = (int)cluster_nctaid_x();
 
   if (threadIdx.x == 0) {
@@ -161,30 +183,35 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
       tma_prefetch_desc(&p.wmap[0]);
       int stage = 0; uint32_t phase = 0;
       for (int tile = tile0; tile < total_tiles; tile += tile_step) {
-        const int m_pt = tile / n_ntiles, n_tile = tile - m_pt * n_ntiles;
+        int m_pt, c0, nch;
+        pair_decode<kCH>(p, tile, n_ntiles, n_full, m_pt, c0, nch);
         const int m0 = m_pt * kPairRows + (int)rank * kBM;
         int bsrc, brow;
-        if constexpr (kBN == 256) {
-          pair_chunk_source(p, n_tile * 2 + (int)rank, bsrc, brow);
-        } else {
-          pair_chunk_source(p, n_tile, bsrc, brow);
-          brow += (int)rank * kBHalf;
+        const CUtensorMap *wm;
+        uint32_t stage_tx = kStageBytes;
+        if (kBN == 256 && nch == 2) {                 // whole tile: CTA r loads chunk r's 128 W rows
+          pair_chunk_source(p, c0 + (int)rank, bsrc, brow);
+          wm = &p.wmap[bsrc];
+        } else {                                      // one chunk: CTA r loads 64 of its W rows
+          pair_chunk_source(p, c0, bsrc, brow);
+          brow += (int)rank * 64;
+          wm = kBN == 256 ? &p.wmap_h[bsrc] : &p.wmap[bsrc];
+          stage_tx = kATileBytes + 64 * kBK * 2;
         }
         for (int kb = 0; kb < nK; ++kb) {
           mbar_wait(&empty_bar[stage], phase ^ 1);
           uint8_t *sa = smem + stage * kStageBytes, *sb = sa + kATileBytes;
           const uint32_t fb = mapa_shared(smem_u32(&full_bar[stage]), 0);
-          mbar_arrive_expect_tx_cluster(fb, kStageBytes);
+          mbar_arrive_expect_tx_cluster(fb, stage_tx);
           tma_load_2d_2sm(sa, &p.amap, fb, kb * kBK, m0);
-          tma_load_2d_2sm(sb, &p.wmap[bsrc], fb, kb * kBK, brow);
+          tma_load_2d_2sm(sb, wm, fb, kb * kBK, brow);
           if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
         if (p.has_lora) {
           const int b0 = p.tile_blk_off[m_pt], b1 = p.tile_blk_off[m_pt + 1];
-#pragma unroll
-          for (int c = 0; c < kCH; ++c) {
+          for (int c = 0; c < nch; ++c) {
             int s, r0;
-            pair_chunk_source(p, n_tile * kCH + c, s, r0);
+            pair_chunk_source(p, c0 + c, s, r0);
             const int tg = p.lora_tgt[s];
             if (tg < 0) continue;
             for (int b = b0; b < b1; ++b) {
@@ -206,10 +233,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
     // ================================ MMA issuer (leader CTA only) ================================
     if (rank == 0 && lane == 0) {
       int stage = 0; uint32_t phase = 0; int acc = 0; uint32_t accphase = 0;
-      constexpr uint32_t idesc_main = make_idesc_bf16(kPairRows, kBN);
+      constexpr uint32_t idesc_whole = make_idesc_bf16(kPairRows, kBN);
       constexpr uint32_t idesc_lora = make_idesc_bf16(kPairRows, kChunk);
       for (int tile = tile0; tile < total_tiles; tile += tile_step) {
-        const int m_pt = tile / n_ntiles, n_tile = tile - m_pt * n_ntiles;
+        int m_pt, c0, nch;
+        pair_decode<kCH>(p, tile, n_ntiles, n_full, m_pt, c0, nch);
+        const uint32_t idesc_main = nch == kCH ? idesc_whole : idesc_lora;
         mbar_wait_cluster(&tempty_bar[acc], accphase ^ 1);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + acc * kAccStride;
@@ -226,10 +255,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
         }
         if (p.has_lora) {
           const int b0 = p.tile_blk_off[m_pt], b1 = p.tile_blk_off[m_pt + 1];
-#pragma unroll
-          for (int c = 0; c < kCH; ++c) {
+          for (int c = 0; c < nch; ++c) {
             int s, r0;
-            pair_chunk_source(p, n_tile * kCH + c, s, r0);
+            pair_chunk_source(p, c0 + c, s, r0);
             const int tg = p.lora_tgt[s];
             if (tg < 0) continue;
             for (int b = b0; b < b1; ++b) {
@@ -262,7 +290,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
     int acc = 0; uint32_t accphase = 0;
     const int mode = p.mode;
     for (int tile = tile0; tile < total_tiles; tile += tile_step) {
-      const int m_pt = tile / n_ntiles, n_tile = tile - m_pt * n_ntiles;
+      int m_pt, c0, nch;
+      pair_decode<kCH>(p, tile, n_ntiles, n_full, m_pt, c0, nch);
+      const int bn = nch * kChunk;                              // columns of this work item (a half tile has 128)
       const int row0_cta = m_pt * kPairRows + (int)rank * kBM;
       const int row = row0_cta + r_in_tile;
       mbar_wait(&tfull_bar[acc], accphase);
@@ -273,7 +303,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
 
       if (mode == GM_OUT_BF16_SWIGLU) {
         // tile = [gate chunk | up chunk] of the same 128 output features; this warpgroup: 64 of them
-        const int r0 = n_tile * kChunk;                         // feature offset of the tile
+        const int r0 = (c0 >> 1) * kChunk;                      // feature offset of the tile (never a half tile)
         const int fcol = wg * 64;
         uint8_t *buf = stg + (box_seq & 1) * 16384;
         if (issuer) bulk_wait_read<1>();
@@ -310,14 +340,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
         if (issuer) { tma_store_2d(&p.omap, buf, r0 + fcol, row0_cta); bulk_commit(); }
         ++box_seq;
       } else if (mode == GM_OUT_BF16 || mode == GM_OUT_BF16_GELU || mode == GM_OUT_BF16_RELU) {
-        constexpr int kBoxes = kBN / 128;                       // 64-column boxes per warpgroup
+        const int kBoxes = bn / 128;                            // 64-column boxes per warpgroup
 #pragma unroll 1
         for (int j = 0; j < kBoxes; ++j) {
-          const int col = wg * (kBN / 2) + j * 64;              // column within the tile
+          const int col = wg * (bn / 2) + j * 64;               // column within the tile
           int s, r0;
-          pair_chunk_source(p, n_tile * kCH + col / kChunk, s, r0);
+          pair_chunk_source(p, c0 + col / kChunk, s, r0);
           const int n_src = r0 + (col % kChunk);
-          const int n_out = n_tile * kBN + col;
+          const int n_out = c0 * kChunk + col;
           uint8_t *buf = stg + (box_seq & 1) * 16384;
           if (issuer) bulk_wait_read<1>();
           named_bar_sync(bar_id, 128);
@@ -340,16 +370,16 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
         }
       } else {
         // fp32 outputs: residual reduce-add, embed (+ positional table), plain store
-        constexpr int kBoxes = kBN / 64;                        // 32-column boxes per warpgroup
+        const int kBoxes = bn / 64;                             // 32-column boxes per warpgroup
         const float *posrow = nullptr;
         if (mode == GM_EMBED_F32 && row < p.M) posrow = p.posb + (size_t)p.row_pos[row] * p.ld_pos;
 #pragma unroll 1
         for (int j = 0; j < kBoxes; ++j) {
-          const int col = wg * (kBN / 2) + j * 32;
+          const int col = wg * (bn / 2) + j * 32;
           int s, r0;
-          pair_chunk_source(p, n_tile * kCH + col / kChunk, s, r0);
+          pair_chunk_source(p, c0 + col / kChunk, s, r0);
           const int n_src = r0 + (col % kChunk);
-          const int n_out = n_tile * kBN + col;
+          const int n_out = c0 * kChunk + col;
           uint8_t *buf = stg + (box_seq & 1) * 16384;
           if (issuer) bulk_wait_read<1>();
           named_bar_sync(bar_id, 128);

@@ -74,7 +74,9 @@ def check_segments(s, wl):
 
 # ---------------------------------------------------------------- the tcgen05 GEMM alone
 @pytest.mark.parametrize("M,N,K", [(128, 128, 64), (300, 384, 192), (1000, 512, 1024), (257, 256, 592), (4096, 1024, 1024),
-                                   (1, 128, 8), (129, 640, 72)])
+                                   (1, 128, 8), (129, 640, 72),
+                                   # more tiles than CTA pairs with a short last wave: its tiles run as 256 x 128 halves
+                                   (5000, 1024, 200), (9984, 512, 64), (19200, 256, 128)])
 def test_tcgen05_gemm_matches_fp64(fmx_mod, M, N, K):
     fmx = fmx_mod.Fmx(0)
     rng = np.random.default_rng(M * 7 + N * 3 + K)
