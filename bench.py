@@ -47,6 +47,19 @@ WORKLOAD_NAMES = {
 }
 
 
+def gemm_traffic(workload):
+    """DRAM bytes per launch of the pair GEMM (dram__bytes_read.sum + dram__bytes_write.sum averaged over the GEMM launches of
+    one layer, from the committed `ncu --set full` capture summary profiles/gemm_traffic.csv), or None for a workload without one."""
+    p = os.path.join(ROOT, "profiles", "gemm_traffic.csv")
+    if not os.path.exists(p):
+        return None
+    for line in open(p):
+        f = line.strip().split(",")
+        if len(f) >= 3 and f[0] == workload:
+            return float(f[2])
+    return None
+
+
 def peaks():
     """Measured roofline denominators (driver-written), else the profiling guide's fallback."""
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
@@ -284,10 +297,11 @@ def measure(args, wl, rank, local_rank, world, with_cpu_baseline=True):
         avg_ms = ms_g / max(n_l, 1)
         flops_per_launch = fl_g / accounting.gemm_launches_per_forward(wl)
         achieved = flops_per_launch / (avg_ms * 1e-3) / 1e12
-        roof = {"kernel": "fmx::gemm_kernel (tcgen05/TMEM/TMA, fused LoRA expand)", "bound": "tensor", "achieved": round(achieved, 2),
+        roof = {"kernel": "fmx::pair_gemm_kernel<256> (tcgen05 cta_group::2 / TMEM / TMA, fused LoRA expand)", "bound": "tensor", "achieved": round(achieved, 2),
                 "peak": pk["bf16_tflops_sustained"], "unit": "TFLOP/s", "frac": round(achieved / pk["bf16_tflops_sustained"], 4),
                 "peak_kind": f"{pk['source']} sustained bf16 (kernel timed inside a long step)",
-                "frac_of_burst_peak": round(achieved / pk["bf16_tflops"], 4), "traffic": None,
+                "frac_of_burst_peak": round(achieved / pk["bf16_tflops"], 4), "traffic": gemm_traffic(args.workload),
+                "traffic_unit": "DRAM bytes per launch (ncu --set full, cold cache; profiles/gemm_traffic.csv)",
                 "flops_per_launch": flops_per_launch, "avg_launch_ms": round(avg_ms, 5), "launches_timed": n_l,
                 "share_of_step": round(ms_g / ms_total, 4),
                 "per_family_tflops": {f: round(fl["families"][f] * args.steps / (gemm_prof[f][1] * 1e-3) / 1e12, 1)

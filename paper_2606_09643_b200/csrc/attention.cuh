@@ -201,4 +201,142 @@ __global__ void __launch_bounds__(kAttnThreads) attention_kernel(const AttnArgs 
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// Short sequences (every request <= 64 tokens: cfg1 / cfg2 / cfg5): one (request, head) item is a single 64 x 64 tile, so
+// the flash loop above degenerates into load -> compute -> store with nothing to overlap, and the step is bound by
+// per-CTA latency (ncu, cfg2: 42 us per layer for 113 MB of traffic).  Here a CTA walks a strided list of items with a
+// two-stage cp.async pipeline (Q, K, V of item i+1 are in flight while item i is computed), and the output tile leaves
+// through shared memory as whole 128-byte row segments.
+template <int DH>
+constexpr int attn_short_smem_bytes() { return 2 * 3 * 64 * (DH + 8) * 2; }
+
+template <int DH>
+__global__ void __launch_bounds__(kAttnThreads) attention_short_kernel(const AttnArgs a, int n_req) {
+  constexpr int LD = DH + 8;
+  constexpr int kTile = 64 * LD;                        // elements of one 64-row tile
+  extern __shared__ __align__(16) uint8_t attn_smem[];
+  __nv_bfloat16 *sbase = reinterpret_cast<__nv_bfloat16 *>(attn_smem);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  const int n_items = n_req * a.n_q_heads;
+  const int group = a.n_q_heads / a.n_kv_heads;
+  griddep_launch();
+  griddep_wait();
+
+  auto issue = [&](int item, int st) {
+    const int p = item / a.n_q_heads, head = item - p * a.n_q_heads;
+    const int r0 = a.cu_tok[p], n = a.cu_tok[p + 1] - r0;
+    const int kvh = head / group;
+    const __nv_bfloat16 *base = a.qkv + (size_t)r0 * a.ld_qkv;
+    __nv_bfloat16 *s = sbase + st * 3 * kTile;
+    load_tile_async<DH>(s, base + head * DH, a.ld_qkv, 0, n);
+    load_tile_async<DH>(s + kTile, base + (a.n_q_heads + kvh) * DH, a.ld_qkv, 0, n);
+    load_tile_async<DH>(s + 2 * kTile, base + (a.n_q_heads + a.n_kv_heads + kvh) * DH, a.ld_qkv, 0, n);
+  };
+
+  int item = blockIdx.x;
+  if (item < n_items) issue(item, 0);
+  cp_async_commit();
+  for (int it = 0; item < n_items; item += gridDim.x, ++it) {
+    const int st = it & 1;
+    const int next = item + gridDim.x;
+    if (next < n_items) issue(next, st ^ 1);
+    cp_async_commit();
+    cp_async_wait<1>();
+    __syncthreads();
+    const int p = item / a.n_q_heads, head = item - p * a.n_q_heads;
+    const int r0 = a.cu_tok[p], n = a.cu_tok[p + 1] - r0;
+    __nv_bfloat16 *sQ = sbase + st * 3 * kTile, *k_s = sQ + kTile, *v_s = sQ + 2 * kTile;
+    const int qrow_a = warp * 16 + g, qrow_b = qrow_a + 8;
+    if (warp * 16 < n) {                                  // warps whose 16 queries do not exist skip the math
+      uint32_t qf[DH / 16][4];
+#pragma unroll
+      for (int ks = 0; ks < DH / 16; ++ks) ldmatrix_x4(qf[ks], sQ + (warp * 16 + (lane & 15)) * LD + ks * 16 + (lane >> 4) * 8);
+      float s[8][4];
+#pragma unroll
+      for (int nt = 0; nt < 8; ++nt) {
+        s[nt][0] = s[nt][1] = s[nt][2] = s[nt][3] = 0.0f;
+#pragma unroll
+        for (int ks = 0; ks < DH / 16; ++ks) {
+          uint32_t b[2];
+          ldmatrix_x2(b, k_s + (nt * 8 + (lane & 7)) * LD + ks * 16 + ((lane >> 3) & 1) * 8);
+          mma_bf16_16816(s[nt], qf[ks], b);
+        }
+      }
+      // raw scores; the 1/sqrt(d_h) log2(e) scale is folded into the exponent: p = 2^(s c - max(s) c), c > 0
+      if (n < 64 || a.causal) {                           // CTA-uniform: a full non-causal tile needs no mask
+#pragma unroll
+        for (int nt = 0; nt < 8; ++nt) {
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const int key = nt * 8 + t * 2 + (e & 1);
+            const int qrow = (e < 2) ? qrow_a : qrow_b;
+            if (key >= n || (a.causal && key > qrow)) s[nt][e] = -INFINITY;
+          }
+        }
+      }
+      float mx[2] = {-INFINITY, -INFINITY};
+#pragma unroll
+      for (int nt = 0; nt < 8; ++nt) {
+        mx[0] = fmaxf(mx[0], fmaxf(s[nt][0], s[nt][1]));
+        mx[1] = fmaxf(mx[1], fmaxf(s[nt][2], s[nt][3]));
+      }
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        mx[h] = fmaxf(mx[h], __shfl_xor_sync(0xffffffffu, mx[h], 1));
+        mx[h] = fmaxf(mx[h], __shfl_xor_sync(0xffffffffu, mx[h], 2));
+        mx[h] *= -a.scale_log2;                           // key 0 is visible to every query: the maximum is finite
+      }
+      float rs[2] = {0.0f, 0.0f};
+#pragma unroll
+      for (int nt = 0; nt < 8; ++nt) {
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const float pv = fast_exp2(fmaf(s[nt][e], a.scale_log2, mx[e >> 1]));
+          s[nt][e] = pv;
+          rs[e >> 1] += pv;
+        }
+      }
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        rs[h] += __shfl_xor_sync(0xffffffffu, rs[h], 1);
+        rs[h] += __shfl_xor_sync(0xffffffffu, rs[h], 2);
+      }
+      float o[DH / 8][4];
+#pragma unroll
+      for (int i = 0; i < DH / 8; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.0f;
+#pragma unroll
+      for (int kk = 0; kk < 4; ++kk) {
+        uint32_t pa[4];
+        pa[0] = pack_bf16(s[2 * kk][0], s[2 * kk][1]);
+        pa[1] = pack_bf16(s[2 * kk][2], s[2 * kk][3]);
+        pa[2] = pack_bf16(s[2 * kk + 1][0], s[2 * kk + 1][1]);
+        pa[3] = pack_bf16(s[2 * kk + 1][2], s[2 * kk + 1][3]);
+#pragma unroll
+        for (int dt = 0; dt < DH / 8; ++dt) {
+          uint32_t b[2];
+          ldmatrix_x2_trans(b, v_s + (kk * 16 + (lane & 15)) * LD + dt * 8);
+          mma_bf16_16816(o[dt], pa, b);
+        }
+      }
+      // O / l -> bf16 into this warp's own 16 rows of the Q tile (only this warp read them), then whole rows to global
+      const float inv_a = 1.0f / rs[0], inv_b = 1.0f / rs[1];
+      __syncwarp();
+#pragma unroll
+      for (int dt = 0; dt < DH / 8; ++dt) {
+        const int col = dt * 8 + t * 2;
+        *reinterpret_cast<uint32_t *>(sQ + qrow_a * LD + col) = pack_bf16(o[dt][0] * inv_a, o[dt][1] * inv_a);
+        *reinterpret_cast<uint32_t *>(sQ + qrow_b * LD + col) = pack_bf16(o[dt][2] * inv_b, o[dt][3] * inv_b);
+      }
+      __syncwarp();
+      constexpr int kChunks = DH / 8;                     // 16-byte chunks per row
+      __nv_bfloat16 *out = a.out + (size_t)r0 * a.ld_out + head * DH;
+      for (int idx = lane; idx < 16 * kChunks; idx += 32) {
+        const int r = warp * 16 + idx / kChunks, c = idx % kChunks;
+        if (r < n) *reinterpret_cast<uint4 *>(out + (size_t)r * a.ld_out + c * 8) = *reinterpret_cast<const uint4 *>(sQ + r * LD + c * 8);
+      }
+    }
+    __syncthreads();      // stage st is refilled by the next iteration's prefetch
+  }
+}
+
 }  // namespace fmx

@@ -303,6 +303,15 @@ void launch_pair_gemm(fmx_ctx *c, cudaStream_t s, const PairGemmParams &p) {
   }
 }
 
+// Every request <= 64 tokens: the pipelined single-tile kernel (4 CTAs per SM, each walking a strided item list).
+int g_attn_short = 1;
+void launch_attention_short(cudaStream_t s, int sm_count, int dh, int n_req, const AttnArgs &a) {
+  const int items = n_req * a.n_q_heads;
+  const int grid = std::min(items, sm_count * 4);
+  if (dh == 32) launch_k(attention_short_kernel<32>, grid, kAttnThreads, attn_short_smem_bytes<32>(), s, a, n_req);
+  else if (dh == 64) launch_k(attention_short_kernel<64>, grid, kAttnThreads, attn_short_smem_bytes<64>(), s, a, n_req);
+  else launch_k(attention_short_kernel<128>, std::min(items, sm_count * 2), kAttnThreads, attn_short_smem_bytes<128>(), s, a, n_req);
+}
 void launch_attention(cudaStream_t s, int dh, dim3 grid, const AttnArgs &a) {
   if (dh == 32) launch_k(attention_kernel<32>, grid, kAttnThreads, attn_smem_bytes<32>(), s, a);
   else if (dh == 64) launch_k(attention_kernel<64>, grid, kAttnThreads, attn_smem_bytes<64>(), s, a);
@@ -385,6 +394,9 @@ int set_kernel_attrs() {
   CU_OK(cudaFuncSetAttribute(pair_gemm_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<128>()));
   CU_OK(cudaFuncSetAttribute(shrink_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<4>()));
   CU_OK(cudaFuncSetAttribute(shrink_kernel<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<5>()));
+  CU_OK(cudaFuncSetAttribute(attention_short_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_short_smem_bytes<32>()));
+  CU_OK(cudaFuncSetAttribute(attention_short_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_short_smem_bytes<64>()));
+  CU_OK(cudaFuncSetAttribute(attention_short_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_short_smem_bytes<128>()));
   CU_OK(cudaFuncSetAttribute(attention_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_smem_bytes<32>()));
   CU_OK(cudaFuncSetAttribute(attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_smem_bytes<64>()));
   CU_OK(cudaFuncSetAttribute(attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_smem_bytes<128>()));
@@ -913,7 +925,8 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       aa.qkv = w.QKV; aa.out = w.AttnO; aa.cu_tok = w.t.cu_tok; aa.ld_qkv = bb.d_qkv; aa.ld_out = bb.d_q;
       aa.n_q_heads = d.n_q_heads; aa.n_kv_heads = d.n_kv_heads; aa.causal = d.causal; aa.scale_log2 = scale_log2;
       dim3 grid((max_len + kAttnBQ - 1) / kAttnBQ, d.n_q_heads, B);
-      LAUNCH(Lh, F_ATTN, launch_attention(s, d.head_dim, grid, aa));
+      if (max_len <= 64 && g_attn_short) LAUNCH(Lh, F_ATTN, launch_attention_short(s, c->sm_count, d.head_dim, B, aa));
+      else LAUNCH(Lh, F_ATTN, launch_attention(s, d.head_dim, grid, aa));
     }
     {
       const int tgs[1] = {FMX_TGT_O};
@@ -1161,7 +1174,8 @@ int fmx_debug_attention(fmx_ctx *c, const void *qkv, void *out, const int32_t *c
     AttnArgs aa{};
     aa.qkv = (const bf16 *)qkv; aa.out = (bf16 *)out; aa.cu_tok = c->d_dbg_cu; aa.ld_qkv = d_qkv; aa.ld_out = d_q;
     aa.n_q_heads = n_q_heads; aa.n_kv_heads = n_kv_heads; aa.causal = causal; aa.scale_log2 = scale_log2;
-    launch_attention(s, head_dim, dim3((max_len + kAttnBQ - 1) / kAttnBQ, n_q_heads, n_req), aa);
+    if (max_len <= 64 && g_attn_short) launch_attention_short(s, c->sm_count, head_dim, n_req, aa);
+    else launch_attention(s, head_dim, dim3((max_len + kAttnBQ - 1) / kAttnBQ, n_q_heads, n_req), aa);
   }
   CU_OK(cudaGetLastError());
   CU_OK(cudaStreamSynchronize(s));      // cu_tok is a host array of the caller
@@ -1179,6 +1193,9 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
     case FMX_OPT_SHRINK_STAGES:
       if (value != 4 && value != 5) return fmx_fail(FMX_E_INVALID_ARG, "set_option: shrink stages %d", value);
       g_shrink_stages = value;
+      return FMX_OK;
+    case FMX_OPT_ATTN_SHORT:
+      g_attn_short = value ? 1 : 0;
       return FMX_OK;
     case FMX_OPT_HALF_TILES:
       g_half_tiles = value ? 1 : 0;

@@ -127,3 +127,20 @@ def test_lanes_attention_large_scores_rescale_path(fmx, lengths, hq, hkv, dh, ca
 ])
 def test_mma_sync_attention_matches_oracle(fmx, lengths, hq, hkv, dh, causal):
     run_case(fmx, lengths, hq, hkv, dh, causal, MMA_SYNC, seed=5)
+
+
+@pytest.mark.parametrize("lengths,hq,hkv,dh,causal", [
+    ([64] * 40, 16, 16, 64, 0),                           # cfg2 / cfg5 shape; more items than resident CTAs' first round
+    ([1, 7, 16, 17, 33, 48, 63, 64, 5], 4, 4, 64, 0),     # ragged, warps with no query, single-token request
+    ([64, 20, 64, 1], 4, 2, 32, 1),                       # GQA + causal, head_dim 32
+    ([50, 64, 3], 6, 1, 128, 1),                          # head_dim 128
+])
+def test_short_sequence_attention_matches_oracle(fmx, lengths, hq, hkv, dh, causal):
+    """Batches whose requests all have <= 64 tokens take the pipelined single-tile kernel (items walked by a strided
+    loop with a two-stage cp.async prefetch); the same cases with the option off take the generic kernel."""
+    for on in (1, 0):
+        fmx.set_option("attn_short", on)
+        try:
+            run_case(fmx, lengths, hq, hkv, dh, causal, MMA_SYNC, seed=11 + dh)
+        finally:
+            fmx.set_option("attn_short", 1)
