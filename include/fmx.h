@@ -215,8 +215,12 @@ enum {
                                     sharing K/V.  FMX_ATTN_LANES: 0 / 1 / 2 = 4 / 2 / 3 lanes per CTA (head_dim 64) */
   FMX_OPT_SHRINK_STAGES = 3,     /* shared-memory pipeline depth of the LoRA shrink kernel: 4 or 5 (default) */
   FMX_OPT_HALF_TILES = 4,        /* 1 (default): a short last GEMM wave is cut into 256 x 128 half tiles */
-  FMX_OPT_ATTN_SHORT = 5,        /* 1 (default): batches whose requests all have <= 64 tokens use the pipelined
-                                    single-tile mma.sync attention kernel */
+  FMX_OPT_ATTN_SHORT = 5,        /* batches whose requests all have <= 64 tokens: 0 = generic kernels, 1 = pipelined
+                                    single-tile mma.sync kernel, 2 (default) = tcgen05 head-pair kernel when head_dim is
+                                    64 and the head count even (FMX_ATTN_AUTO only), else as 1 */
+  FMX_OPT_ROPE_FUSED = 6,        /* 1 (default): head_dim 128 backbones rotate q / k in the QKV GEMM epilogue;
+                                    0: separate RoPE kernel over the bf16 QKV buffer */
+  FMX_OPT_HEAD_TILED = 7,        /* 1 (default): FLATTEN heads run in the 4-request x 4-output register-tiled kernel */
   FMX_OPT_PDL = 2                /* programmatic dependent launch of the forward's kernels (process-wide):
                                     0 = off, 1 = always, 2 (default) = only for batches of <= 4096 token rows */
 };

@@ -15,6 +15,7 @@
 
 #include "attention.cuh"
 #include "attention_lanes.cuh"
+#include "attention_pair64.cuh"
 #include "attention_tc.cuh"
 #include "common.h"
 #include "fmx.h"
@@ -234,6 +235,8 @@ struct Launcher {
 int g_pdl = 2, g_pdl_eff = 0;
 int g_shrink_stages = 5;
 int g_half_tiles = 1;
+int g_rope_fused = 1;
+int g_head_tiled = 1;
 constexpr int kPdlAutoRows = 4096;
 template <typename... KArgs, typename... Args>
 void launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args &&...args) {
@@ -294,7 +297,7 @@ void launch_pair_gemm(fmx_ctx *c, cudaStream_t s, const PairGemmParams &p) {
     // into 256 x 128 halves so that it lasts half a tile time (cfg2 O / FFN-out: 256 tiles on 74 pairs, 4 -> 3.5 waves).
     PairGemmParams q = p;
     const int rem = tiles % pairs;
-    q.n_full = (g_half_tiles && p.mode != GM_OUT_BF16_SWIGLU && tiles > pairs && rem > 0 && 2 * rem <= pairs) ? tiles - rem : -1;
+    q.n_full = (g_half_tiles && p.mode != GM_OUT_BF16_SWIGLU && !p.rope_cs && tiles > pairs && rem > 0 && 2 * rem <= pairs) ? tiles - rem : -1;
     const int items = q.n_full >= 0 ? q.n_full + 2 * rem : tiles;
     launch_k(pair_gemm_kernel<256>, 2 * std::min(items, pairs), kGemmThreads, pair_smem_bytes<256>(), s, q);
   } else {
@@ -304,7 +307,13 @@ void launch_pair_gemm(fmx_ctx *c, cudaStream_t s, const PairGemmParams &p) {
 }
 
 // Every request <= 64 tokens: the pipelined single-tile kernel (4 CTAs per SM, each walking a strided item list).
-int g_attn_short = 1;
+int g_attn_short = 2;    // 0: generic kernel, 1: pipelined mma.sync kernel, 2: tcgen05 head-pair kernel where it applies (d_h 64, even H_q)
+bool attn_pair64_ok(int dh, int n_q_heads, int max_len) { return g_attn_short == 2 && dh == 64 && n_q_heads % 2 == 0 && max_len <= 64; }
+void launch_attention_pair64(cudaStream_t s, int sm_count, const AttnPairArgs &a) {
+  const int items = a.n_req * (a.n_q_heads / 2);
+  const int grid = std::min(sm_count, (items + kP64Lanes - 1) / kP64Lanes);
+  launch_k(attention_pair64_kernel, grid, kP64Threads, attn_pair64_smem_bytes(), s, a);
+}
 void launch_attention_short(cudaStream_t s, int sm_count, int dh, int n_req, const AttnArgs &a) {
   const int items = n_req * a.n_q_heads;
   const int grid = std::min(items, sm_count * 4);
@@ -394,6 +403,7 @@ int set_kernel_attrs() {
   CU_OK(cudaFuncSetAttribute(pair_gemm_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<128>()));
   CU_OK(cudaFuncSetAttribute(shrink_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<4>()));
   CU_OK(cudaFuncSetAttribute(shrink_kernel<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<5>()));
+  CU_OK(cudaFuncSetAttribute(attention_pair64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_pair64_smem_bytes()));
   CU_OK(cudaFuncSetAttribute(attention_short_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_short_smem_bytes<32>()));
   CU_OK(cudaFuncSetAttribute(attention_short_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_short_smem_bytes<64>()));
   CU_OK(cudaFuncSetAttribute(attention_short_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_short_smem_bytes<128>()));
@@ -889,6 +899,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   // ---- layers ----
   const int rms = d.norm == FMX_NORM_RMSNORM;
   const float scale_log2 = 1.4426950408889634f / sqrtf((float)d.head_dim);
+  bool rope_fused = false;
   for (int l = 0; l < d.n_layers; ++l) {
     LAUNCH(Lh, F_NORM, dispatch_norm(s, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm1_g[l], (const bf16 *)bb.norm1_b[l], Ni, d.norm_eps, rms));
     {
@@ -903,14 +914,22 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       p.bias[0] = (const bf16 *)bb.bq[l]; p.bias[1] = (const bf16 *)bb.bk[l]; p.bias[2] = (const bf16 *)bb.bv[l];
       set_lora(p, 0, FMX_TGT_Q, l); set_lora(p, 1, FMX_TGT_K, l); set_lora(p, 2, FMX_TGT_V, l);
       p.omap = oQKV;
+      // head_dim 128: a 128-column chunk is one head, so RoPE is applied in the GEMM epilogue (fp32, one rounding)
+      rope_fused = g_rope_fused && d.rope_theta > 0 && d.head_dim == 128 && pair_wide(p);
+      if (rope_fused) { p.rope_cs = bb.rope_cs; p.rope_src_mask = 3; }
       LAUNCH(Lh, F_GEMM_QKV, launch_pair_gemm(c, s, p));
     }
-    if (d.rope_theta > 0) {
+    if (d.rope_theta > 0 && !rope_fused) {
       const int nh = d.n_q_heads + d.n_kv_heads;
       const long long total = (long long)Ni * nh * (d.head_dim / 16);
       LAUNCH(Lh, F_ROPE, (launch_k(rope_kernel, (unsigned)((total + 255) / 256), 256, 0, s, w.QKV, bb.d_qkv, w.t.row_pos, bb.rope_cs, Ni, nh, d.head_dim)));
     }
-    if (attn_use_lanes(c->opt_attn_impl, d.head_dim, max_len)) {
+    if (c->opt_attn_impl == FMX_ATTN_AUTO && attn_pair64_ok(d.head_dim, d.n_q_heads, max_len)) {
+      AttnPairArgs pa2{};
+      pa2.qkv_map = mQKV64; pa2.out = w.AttnO; pa2.cu_tok = w.t.cu_tok; pa2.ld_out = bb.d_q; pa2.n_req = B;
+      pa2.n_q_heads = d.n_q_heads; pa2.n_kv_heads = d.n_kv_heads; pa2.causal = d.causal; pa2.scale_log2 = scale_log2;
+      LAUNCH(Lh, F_ATTN, launch_attention_pair64(s, c->sm_count, pa2));
+    } else if (attn_use_lanes(c->opt_attn_impl, d.head_dim, max_len)) {
       AttnLaneArgs la{};
       la.qkv_map = mQKV64; la.out = w.AttnO; la.cu_tok = w.t.cu_tok; la.ld_out = bb.d_q; la.n_req = B;
       la.n_q_heads = d.n_q_heads; la.n_kv_heads = d.n_kv_heads; la.causal = d.causal; la.scale_log2 = scale_log2;
@@ -980,7 +999,14 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   ha.task_head_kind = c->d_task_head_kind; ha.task_head_out = c->d_task_head_out;
   ha.task_head_W = (const bf16 *const *)c->d_task_head_W; ha.task_head_b = (const bf16 *const *)c->d_task_head_b;
   ha.out = outputs; ha.d = d.d_model;
-  LAUNCH(Lh, F_HEAD, (launch_k(head_kernel, dim3(B, (max_out + 7) / 8), 256, 0, s, ha)));
+  bool any_flat = false, any_pooled = false;
+  for (int i = 0; i < B; ++i) {
+    if (c->tasks[task_ids[i]].head_kind == FMX_HEAD_FLATTEN) any_flat = true;
+    else any_pooled = true;
+  }
+  ha.skip_flatten = (any_flat && g_head_tiled) ? 1 : 0;
+  if (any_pooled || !ha.skip_flatten) LAUNCH(Lh, F_HEAD, (launch_k(head_kernel, dim3(B, (max_out + 7) / 8), 256, 0, s, ha)));
+  if (ha.skip_flatten) LAUNCH(Lh, F_HEAD, (launch_k(head_flatten_kernel, dim3((B + 3) / 4, (max_out + 31) / 32), 256, 0, s, ha, B)));
 
   {
     void *bufs[7] = {w.X, w.Xn, w.QKV, w.AttnO, w.Hid, w.U, w.feat};
@@ -1158,7 +1184,13 @@ int fmx_debug_attention(fmx_ctx *c, const void *qkv, void *out, const int32_t *c
   CU_OK(cudaMemcpyAsync(c->d_dbg_cu, cu_tok, sizeof(int) * (n_req + 1), cudaMemcpyHostToDevice, s));
   const int N = cu_tok[n_req], d_q = n_q_heads * head_dim, d_qkv = (n_q_heads + 2 * n_kv_heads) * head_dim;
   const float scale_log2 = 1.4426950408889634f / sqrtf((float)head_dim);
-  if (attn_use_lanes(impl, head_dim, max_len)) {
+  if (impl == FMX_ATTN_AUTO && attn_pair64_ok(head_dim, n_q_heads, max_len)) {
+    AttnPairArgs pa2{};
+    if (int e = encode_2d(c, &pa2.qkv_map, qkv, N, d_qkv, d_qkv, 64)) return e;
+    pa2.out = (bf16 *)out; pa2.cu_tok = c->d_dbg_cu; pa2.ld_out = d_q; pa2.n_req = n_req; pa2.n_q_heads = n_q_heads; pa2.n_kv_heads = n_kv_heads;
+    pa2.causal = causal; pa2.scale_log2 = scale_log2;
+    launch_attention_pair64(s, c->sm_count, pa2);
+  } else if (attn_use_lanes(impl, head_dim, max_len)) {
     AttnLaneArgs la{};
     if (int e = encode_2d(c, &la.qkv_map, qkv, N, d_qkv, d_qkv, 64)) return e;
     la.out = (bf16 *)out; la.cu_tok = c->d_dbg_cu; la.ld_out = d_q; la.n_req = n_req; la.n_q_heads = n_q_heads; la.n_kv_heads = n_kv_heads;
@@ -1195,7 +1227,14 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
       g_shrink_stages = value;
       return FMX_OK;
     case FMX_OPT_ATTN_SHORT:
-      g_attn_short = value ? 1 : 0;
+      if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attn_short %d", value);
+      g_attn_short = value;
+      return FMX_OK;
+    case FMX_OPT_HEAD_TILED:
+      g_head_tiled = value ? 1 : 0;
+      return FMX_OK;
+    case FMX_OPT_ROPE_FUSED:
+      g_rope_fused = value ? 1 : 0;
       return FMX_OK;
     case FMX_OPT_HALF_TILES:
       g_half_tiles = value ? 1 : 0;

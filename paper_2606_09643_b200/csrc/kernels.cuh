@@ -461,6 +461,7 @@ struct HeadArgs {
   const __nv_bfloat16 *const *task_head_W, *const *task_head_b;
   float *out;
   int d;
+  int skip_flatten;                // 1: FLATTEN heads are computed by head_flatten_kernel
 };
 
 // grid (sorted request p, output tile of 8): each warp computes one output o as a dot product over
@@ -474,6 +475,7 @@ __global__ void __launch_bounds__(256) head_kernel(const HeadArgs a) {
   const int n_out = a.task_head_out[t];
   if (o >= n_out) return;
   const int kind = a.task_head_kind[t];
+  if (kind == 3 && a.skip_flatten) return;
   const int r0 = a.cu_tok[p], n = a.cu_tok[p + 1] - r0;
   const long long K = kind == 3 ? (long long)n * a.d : a.d;
   const __nv_bfloat16 *w = a.task_head_W[t] + (size_t)o * K;
@@ -500,6 +502,77 @@ __global__ void __launch_bounds__(256) head_kernel(const HeadArgs a) {
   if (lane == 0) {
     const __nv_bfloat16 *b = a.task_head_b[t];
     a.out[a.out_off[a.perm[p]] + o] = acc + (b ? __bfloat162float(b[o]) : 0.0f);
+  }
+}
+
+// FLATTEN heads (cfg2 forecasting: d_feat = 64 x 1024, 96 outputs, 12.6 MB of weights per task).  head_kernel spends ~30
+// instructions per (request, output) per 8 features, almost all of them loads and bf16 unpacking, and is issue-bound.
+// Here a warp owns a 4-request x 4-output register tile: every unpacked weight serves 4 requests and every unpacked
+// feature 4 outputs.  grid (ceil(B / 4) groups of consecutive SORTED requests, ceil(max_out / 32)); requests of a group
+// that belong to another task than its first FLATTEN request are handled in further passes (task boundaries only).
+__global__ void __launch_bounds__(256) head_flatten_kernel(const HeadArgs a, int B) {
+  griddep_launch();
+  griddep_wait();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int p0 = blockIdx.x * 4;
+  const int o0 = (blockIdx.y * 8 + warp) * 4;
+  int task[4];
+  unsigned todo = 0;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    task[i] = p0 + i < B ? a.task_sorted[p0 + i] : -1;
+    if (task[i] >= 0 && a.task_head_kind[task[i]] == 3 && o0 < a.task_head_out[task[i]]) todo |= 1u << i;
+  }
+  while (todo) {
+    const int lead = __ffs(todo) - 1;
+    const int t = task[lead];
+    unsigned grp = 0;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) if (((todo >> i) & 1u) && task[i] == t) grp |= 1u << i;
+    todo &= ~grp;
+    const int n_out = a.task_head_out[t];
+    const int r_lead = a.cu_tok[p0 + lead];
+    const long long K = (long long)(a.cu_tok[p0 + lead + 1] - r_lead) * a.d;
+    const __nv_bfloat16 *f[4], *w[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) f[i] = a.Fn + (size_t)a.cu_tok[p0 + (((grp >> i) & 1u) ? i : lead)] * a.d;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) w[j] = a.task_head_W[t] + (size_t)min(o0 + j, n_out - 1) * K;
+    float acc[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int j = 0; j < 4; ++j) acc[i][j] = 0.0f;
+    for (long long c = lane * 8; c < K; c += 256) {
+      float fv[4][8], wv[8];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const uint4 u = *reinterpret_cast<const uint4 *>(f[i] + c);
+        fv[i][0] = bf16_lo(u.x); fv[i][1] = bf16_hi(u.x); fv[i][2] = bf16_lo(u.y); fv[i][3] = bf16_hi(u.y);
+        fv[i][4] = bf16_lo(u.z); fv[i][5] = bf16_hi(u.z); fv[i][6] = bf16_lo(u.w); fv[i][7] = bf16_hi(u.w);
+      }
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const uint4 u = *reinterpret_cast<const uint4 *>(w[j] + c);
+        wv[0] = bf16_lo(u.x); wv[1] = bf16_hi(u.x); wv[2] = bf16_lo(u.y); wv[3] = bf16_hi(u.y);
+        wv[4] = bf16_lo(u.z); wv[5] = bf16_hi(u.z); wv[6] = bf16_lo(u.w); wv[7] = bf16_hi(u.w);
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int e = 0; e < 8; ++e) acc[i][j] = fmaf(fv[i][e], wv[e], acc[i][j]);
+      }
+    }
+    const __nv_bfloat16 *b = a.task_head_b[t];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        float v = acc[i][j];
+#pragma unroll
+        for (int s = 16; s > 0; s >>= 1) v += __shfl_xor_sync(0xffffffffu, v, s);
+        if (lane == 0 && ((grp >> i) & 1u) && o0 + j < n_out)
+          a.out[a.out_off[a.perm[p0 + i]] + o0 + j] = v + (b ? __bfloat162float(b[o0 + j]) : 0.0f);
+      }
   }
 }
 

@@ -68,6 +68,8 @@ struct PairGemmParams {
   const float *posb;       // [max_seq, ld_pos] fp32 (embed)
   const int *row_pos;
   int ld_pos;
+  const float2 *rope_cs;   // [max_seq, 64] (cos, sin): fused rotate-half RoPE for head_dim 128 (chunk = head), or NULL
+  int rope_src_mask;       // bit s: source s (q | k | v) is rotated
 };
 
 __device__ __forceinline__ void pair_chunk_source(const PairGemmParams &p, int c, int &s, int &r0) {
@@ -341,6 +343,59 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
         ++box_seq;
       } else if (mode == GM_OUT_BF16 || mode == GM_OUT_BF16_GELU || mode == GM_OUT_BF16_RELU) {
         const int kBoxes = bn / 128;                            // 64-column boxes per warpgroup
+        int s_wg, r0_wg;
+        pair_chunk_source(p, c0 + (bn == 256 ? wg : 0), s_wg, r0_wg);
+        if (p.rope_cs && bn == 256 && ((p.rope_src_mask >> s_wg) & 1)) {
+          // Fused RoPE (rotate-half): this warpgroup's 128 columns are one head; dims j and j + 64 of the thread's row
+          // are rotated in fp32 straight from the accumulator (one rounding) and leave as two 64-column boxes.
+          const int n_out = (c0 + wg) * kChunk;
+          uint8_t *rowA = stg + r_in_tile * 128, *rowB = rowA + 16384;
+          if (issuer) bulk_wait_read<0>();
+          named_bar_sync(bar_id, 128);
+          const float2 *cs = p.rope_cs + (size_t)(row < p.M ? p.row_pos[row] : 0) * 64;
+          const __nv_bfloat16 *bias = p.bias[s_wg];
+#pragma unroll 1
+          for (int h = 0; h < 2; ++h) {
+            tmem_ld_32x32(t_row + wg * kChunk + h * 32, v);
+            tmem_ld_32x32(t_row + wg * kChunk + 64 + h * 32, u);
+            tmem_ld_wait();
+            if (h == 1) {
+              tc_fence_before();
+              __syncwarp();
+              if (lane == 0) mbar_arrive_cluster(tempty_remote);
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              float x1[8], x2[8];
+#pragma unroll
+              for (int e = 0; e < 8; ++e) {
+                x1[e] = __uint_as_float(v[8 * q + e]);
+                x2[e] = __uint_as_float(u[8 * q + e]);
+                if (bias) {
+                  x1[e] += __bfloat162float(bias[r0_wg + h * 32 + 8 * q + e]);
+                  x2[e] += __bfloat162float(bias[r0_wg + 64 + h * 32 + 8 * q + e]);
+                }
+              }
+              const float4 *c4 = reinterpret_cast<const float4 *>(cs + h * 32 + q * 8);
+              uint32_t oa[4], ob[4];
+#pragma unroll
+              for (int e = 0; e < 4; ++e) {
+                const float4 c = c4[e];                     // (cos, sin) of dims 2e, 2e+1 of this group
+                oa[e] = pack_bf16(x1[2 * e] * c.x - x2[2 * e] * c.y, x1[2 * e + 1] * c.z - x2[2 * e + 1] * c.w);
+                ob[e] = pack_bf16(x2[2 * e] * c.x + x1[2 * e] * c.y, x2[2 * e + 1] * c.z + x1[2 * e + 1] * c.w);
+              }
+              *reinterpret_cast<uint4 *>(rowA + (((h * 4 + q) ^ rsw) << 4)) = make_uint4(oa[0], oa[1], oa[2], oa[3]);
+              *reinterpret_cast<uint4 *>(rowB + (((h * 4 + q) ^ rsw) << 4)) = make_uint4(ob[0], ob[1], ob[2], ob[3]);
+            }
+          }
+          fence_proxy_async();
+          named_bar_sync(bar_id, 128);
+          if (issuer) {
+            tma_store_2d(&p.omap, stg, n_out, row0_cta); bulk_commit();
+            tma_store_2d(&p.omap, stg + 16384, n_out + 64, row0_cta); bulk_commit();
+          }
+          box_seq = 0;                                          // the next box reuses the first buffer, after group 1
+        } else
 #pragma unroll 1
         for (int j = 0; j < kBoxes; ++j) {
           const int col = wg * (bn / 2) + j * 64;               // column within the tile

@@ -130,17 +130,21 @@ def test_mma_sync_attention_matches_oracle(fmx, lengths, hq, hkv, dh, causal):
 
 
 @pytest.mark.parametrize("lengths,hq,hkv,dh,causal", [
-    ([64] * 40, 16, 16, 64, 0),                           # cfg2 / cfg5 shape; more items than resident CTAs' first round
+    ([64] * 40, 16, 16, 64, 0),                           # cfg2 / cfg5 shape; more items than lanes: the rings wrap
     ([1, 7, 16, 17, 33, 48, 63, 64, 5], 4, 4, 64, 0),     # ragged, warps with no query, single-token request
-    ([64, 20, 64, 1], 4, 2, 32, 1),                       # GQA + causal, head_dim 32
-    ([50, 64, 3], 6, 1, 128, 1),                          # head_dim 128
+    ([64, 31, 64, 2, 40] * 30, 12, 2, 64, 1),             # GQA 6:1 (a head pair shares / splits KV heads), causal
+    ([64, 20, 64, 1], 4, 2, 32, 1),                       # head_dim 32: mma.sync path only
+    ([50, 64, 3], 6, 1, 128, 1),                          # head_dim 128: mma.sync path only
+    ([64, 64, 9], 3, 3, 64, 0),                           # odd head count: no head pairs
 ])
 def test_short_sequence_attention_matches_oracle(fmx, lengths, hq, hkv, dh, causal):
-    """Batches whose requests all have <= 64 tokens take the pipelined single-tile kernel (items walked by a strided
-    loop with a two-stage cp.async prefetch); the same cases with the option off take the generic kernel."""
-    for on in (1, 0):
-        fmx.set_option("attn_short", on)
+    """Batches whose requests all have <= 64 tokens: (a) the tcgen05 head-pair kernel (two heads of a request as one
+    block-diagonal 128-row MMA; default under AUTO when head_dim is 64 and the head count even), (b) the pipelined
+    single-tile mma.sync kernel, (c) the generic kernel."""
+    AUTO = 0
+    for impl, short in ((AUTO, 2), (MMA_SYNC, 1), (MMA_SYNC, 0)):
+        fmx.set_option("attn_short", short)
         try:
-            run_case(fmx, lengths, hq, hkv, dh, causal, MMA_SYNC, seed=11 + dh)
+            run_case(fmx, lengths, hq, hkv, dh, causal, impl, seed=11 + dh)
         finally:
-            fmx.set_option("attn_short", 1)
+            fmx.set_option("attn_short", 2)
