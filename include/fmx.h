@@ -221,6 +221,9 @@ enum {
   FMX_OPT_ROPE_FUSED = 6,        /* 1 (default): head_dim 128 backbones rotate q / k in the QKV GEMM epilogue;
                                     0: separate RoPE kernel over the bf16 QKV buffer */
   FMX_OPT_HEAD_TILED = 7,        /* 1 (default): FLATTEN heads run in the 4-request x 4-output register-tiled kernel */
+  FMX_OPT_SHRINK_FUSED = 8,      /* the LoRA shrink runs as the first work items of the GEMM that consumes it: 0 = never
+                                    (separate shrink kernel), 1 (default) = when the batch has at most one (tile, task)
+                                    block per CTA pair, 2 = always */
   FMX_OPT_PDL = 2                /* programmatic dependent launch of the forward's kernels (process-wide):
                                     0 = off, 1 = always, 2 (default) = only for batches of <= 4096 token rows */
 };

@@ -82,6 +82,7 @@ struct ProfEvent { int family; cudaEvent_t e0, e1; };
 
 struct fmx_ctx {
   int device = 0, sm_count = 0;
+  bool pairs_resident = false;             // sm_count / 2 clusters of the pair GEMM fit the device at once (fused shrink needs it)
   EncodeTiledFn encode = nullptr;
   std::vector<std::unique_ptr<Backbone>> bbs;
   std::vector<TaskRec> tasks;              // slot = task id
@@ -149,6 +150,7 @@ struct Workspace {
   SegTables t{};
   float *X = nullptr, *feat = nullptr;
   bf16 *Xn = nullptr, *QKV = nullptr, *AttnO = nullptr, *Hid = nullptr, *U = nullptr;
+  unsigned *u_flag = nullptr;            // completion counter of the fused-shrink items
   int n_tiles = 0, n_blk_cap = 0;
   size_t bytes = 0;
 };
@@ -186,6 +188,7 @@ Workspace carve(const Backbone &bb, void *base, int B, long long N, int T) {
   w.Hid = (bf16 *)take(sizeof(bf16) * N * std::max(d.d_ffn, bb.Kp));     // also the patch-pack buffer
   w.U = (bf16 *)take(sizeof(bf16) * (size_t)w.n_blk_cap * kPairRows * 192);
   w.feat = (float *)take(sizeof(float) * (size_t)B * d.d_model);
+  w.u_flag = (unsigned *)take(sizeof(unsigned));
   w.bytes = off;
   return w;
 }
@@ -237,6 +240,7 @@ int g_shrink_stages = 5;
 int g_half_tiles = 1;
 int g_rope_fused = 1;
 int g_head_tiled = 1;
+int g_shrink_fused = 1;   // the LoRA shrink runs as the first work items of the GEMM that consumes it (see pair_gemm.cuh)
 constexpr int kPdlAutoRows = 4096;
 template <typename... KArgs, typename... Args>
 void launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args &&...args) {
@@ -299,10 +303,10 @@ void launch_pair_gemm(fmx_ctx *c, cudaStream_t s, const PairGemmParams &p) {
     const int rem = tiles % pairs;
     q.n_full = (g_half_tiles && p.mode != GM_OUT_BF16_SWIGLU && !p.rope_cs && tiles > pairs && rem > 0 && 2 * rem <= pairs) ? tiles - rem : -1;
     const int items = q.n_full >= 0 ? q.n_full + 2 * rem : tiles;
-    launch_k(pair_gemm_kernel<256>, 2 * std::min(items, pairs), kGemmThreads, pair_smem_bytes<256>(), s, q);
+    launch_k(pair_gemm_kernel<256>, 2 * (p.n_sh > 0 ? pairs : std::min(items, pairs)), kGemmThreads, pair_smem_bytes<256>(), s, q);
   } else {
     const int tiles = p.n_ptiles * p.n_chunks;
-    launch_k(pair_gemm_kernel<128>, 2 * std::min(tiles, pairs), kGemmThreads, pair_smem_bytes<128>(), s, p);
+    launch_k(pair_gemm_kernel<128>, 2 * (p.n_sh > 0 ? pairs : std::min(tiles, pairs)), kGemmThreads, pair_smem_bytes<128>(), s, p);
   }
 }
 
@@ -526,6 +530,24 @@ int fmx_create(fmx_ctx **out, int device_ordinal) {
   if (!fn || qres != cudaDriverEntryPointSuccess) return fmx_fail(FMX_E_CUDA, "fmx_create: cuTensorMapEncodeTiled not available");
   c->encode = reinterpret_cast<EncodeTiledFn>(fn);
   if (int err = set_kernel_attrs()) return err;
+  {
+    // The fused LoRA shrink makes one CTA pair wait for another pair's work item: every cluster of the persistent grid
+    // must be resident at the same time.
+    auto max_clusters = [&](auto kern, int smem) {
+      cudaLaunchConfig_t cfg{};
+      cfg.gridDim = dim3(c->sm_count, 1, 1); cfg.blockDim = dim3(kGemmThreads, 1, 1); cfg.dynamicSmemBytes = smem;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      cfg.attrs = at; cfg.numAttrs = 1;
+      int n = 0;
+      if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess) { cudaGetLastError(); n = 0; }
+      return n;
+    };
+    const int n256 = max_clusters(pair_gemm_kernel<256>, pair_smem_bytes<256>()), n128 = max_clusters(pair_gemm_kernel<128>, pair_smem_bytes<128>());
+    c->pairs_resident = n256 >= c->sm_count / 2 && n128 >= c->sm_count / 2;
+    if (getenv("FMX_DEBUG")) fprintf(stderr, "fmx: max active pair-GEMM clusters %d / %d (need %d): fused shrink %s\n", n256, n128, c->sm_count / 2, c->pairs_resident ? "on" : "off");
+  }
   c->tasks.resize(FMX_MAX_TASKS);
   CU_OK(cudaMalloc(&c->d_task_coff, sizeof(int) * FMX_MAX_TASKS));
   CU_OK(cudaMalloc(&c->d_task_head_kind, sizeof(int) * FMX_MAX_TASKS));
@@ -871,6 +893,46 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     LAUNCH(Lh, F_SHRINK, launch_shrink(c, s, p));
     return FMX_OK;
   };
+  // fused form: no launch; the GEMM that reads the same input computes U in its first work items
+  unsigned u_epoch = 0;
+  auto shrink_fused = [&](PairGemmParams &p, const int *tgs, int n, int layer) {
+    p.n_sh = 0;
+    for (int i = 0; i < n; ++i) {
+      const int tg = tgs[i];
+      uslot_of[tg] = -1;
+      if (bb.n_adapters[tg] <= 0) continue;
+      p.smap[p.n_sh] = bb.mA[tg][layer];
+      p.sh_tg[p.n_sh] = tg;
+      uslot_of[tg] = p.n_sh++;
+    }
+    if (p.n_sh == 0) return;
+    p.blk_tile = w.t.blk_tile; p.blk_lo = w.t.blk_lo; p.blk_hi = w.t.blk_hi; p.n_blk = w.t.n_blk;
+    p.task_scale = c->d_task_scale; p.U = w.U; p.u_flag = w.u_flag; p.u_epoch = ++u_epoch;
+  };
+  // (tile, task) blocks of the sorted batch, counted on the host from the caller's ids / lengths (the device computes the
+  // same number in S1).  Measured on B200: fusing pays when the shrink items fit ONE wave of the persistent grid (cfg2:
+  // 73 blocks on 74 pairs, -0.4 ms per step); with more blocks the items' low arithmetic intensity costs as much as the
+  // separate shrink launches (cfg3 / cfg4 / cfg5 at 92 tasks: +-0), so those keep the dedicated kernel.
+  int n_blk_host = 0;
+  {
+    std::vector<long long> tok(T + 1, 0);
+    for (int i = 0; i < B; ++i) tok[task_ids[i]] += lengths[i];
+    long long lo = 0;
+    for (int t = 0; t < T; ++t) {
+      if (tok[t] == 0) continue;
+      const long long hi = lo + tok[t];
+      n_blk_host += (int)((hi - 1) / kPairRows - lo / kPairRows + 1);
+      lo = hi;
+    }
+  }
+  const bool fuse_ok = g_shrink_fused && c->pairs_resident && (g_shrink_fused == 2 || n_blk_host <= c->sm_count / 2);
+  if (fuse_ok) CU_OK(cudaMemsetAsync(w.u_flag, 0, sizeof(unsigned), s));
+  // fusable: all CTA pairs of the persistent grid are co-resident (the expand steps spin on another pair's result) and
+  // a 3-target group needs the 256-wide kernel
+  auto can_fuse = [&](const PairGemmParams &p, int n_targets) {
+    return fuse_ok && (n_targets < 3 || pair_wide(p));
+  };
+
   auto set_lora = [&](PairGemmParams &p, int src, int tg, int layer) {
     if (bb.n_adapters[tg] > 0 && uslot_of[tg] >= 0) {
       p.lora_tgt[src] = tg; p.uslot[src] = uslot_of[tg]; p.lmap[src] = bb.mB[tg][layer]; p.has_lora = 1;
@@ -904,9 +966,10 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     LAUNCH(Lh, F_NORM, dispatch_norm(s, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm1_g[l], (const bf16 *)bb.norm1_b[l], Ni, d.norm_eps, rms));
     {
       const int tgs[3] = {FMX_TGT_Q, FMX_TGT_K, FMX_TGT_V};
-      if ((e = shrink(mXn, d.d_model, tgs, 3, l))) return e;
       PairGemmParams p = base;
       p.mode = GM_OUT_BF16; p.amap = mXn; p.K = d.d_model; p.n_chunks = bb.d_qkv / 128;
+      if (can_fuse(p, 3)) shrink_fused(p, tgs, 3, l);
+      else if ((e = shrink(mXn, d.d_model, tgs, 3, l))) return e;
       const int v = wv(p);
       p.wmap[0] = bb.mWq[v][l]; p.wmap[1] = bb.mWk[v][l]; p.wmap[2] = bb.mWv[v][l];
       p.wmap_h[0] = bb.mWq[1][l]; p.wmap_h[1] = bb.mWk[1][l]; p.wmap_h[2] = bb.mWv[1][l];
@@ -949,9 +1012,10 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     }
     {
       const int tgs[1] = {FMX_TGT_O};
-      if ((e = shrink(mAttnO, bb.d_q, tgs, 1, l))) return e;
       PairGemmParams p = base;
       p.mode = GM_RESID_F32; p.amap = mAttnO; p.K = bb.d_q; p.n_chunks = d.d_model / 128;
+      if (can_fuse(p, 1)) shrink_fused(p, tgs, 1, l);
+      else if ((e = shrink(mAttnO, bb.d_q, tgs, 1, l))) return e;
       p.wmap[0] = bb.mWo[wv(p)][l]; p.wmap_h[0] = bb.mWo[1][l]; p.bias[0] = (const bf16 *)bb.bo[l];
       set_lora(p, 0, FMX_TGT_O, l);
       p.omap = oX;
@@ -960,9 +1024,10 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     LAUNCH(Lh, F_NORM, dispatch_norm(s, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm2_g[l], (const bf16 *)bb.norm2_b[l], Ni, d.norm_eps, rms));
     if (d.act == FMX_ACT_SWIGLU) {
       const int tgs[2] = {FMX_TGT_GATE, FMX_TGT_UP};
-      if ((e = shrink(mXn, d.d_model, tgs, 2, l))) return e;
       PairGemmParams p = base;
       p.mode = GM_OUT_BF16_SWIGLU; p.amap = mXn; p.K = d.d_model; p.n_chunks = 2 * d.d_ffn / 128; p.interleave2 = 1;
+      if (can_fuse(p, 2)) shrink_fused(p, tgs, 2, l);
+      else if ((e = shrink(mXn, d.d_model, tgs, 2, l))) return e;
       p.wmap[0] = bb.mWgate[0][l]; p.wmap[1] = bb.mWup[0][l];
       p.bias[0] = (const bf16 *)bb.bgate[l]; p.bias[1] = (const bf16 *)bb.bup[l];
       set_lora(p, 0, FMX_TGT_GATE, l); set_lora(p, 1, FMX_TGT_UP, l);
@@ -970,9 +1035,10 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       LAUNCH(Lh, F_GEMM_FFN_IN, launch_pair_gemm(c, s, p));
     } else {
       const int tgs[1] = {FMX_TGT_UP};
-      if ((e = shrink(mXn, d.d_model, tgs, 1, l))) return e;
       PairGemmParams p = base;
       p.mode = d.act == FMX_ACT_GELU_ERF ? GM_OUT_BF16_GELU : GM_OUT_BF16_RELU; p.amap = mXn; p.K = d.d_model; p.n_chunks = d.d_ffn / 128;
+      if (can_fuse(p, 1)) shrink_fused(p, tgs, 1, l);
+      else if ((e = shrink(mXn, d.d_model, tgs, 1, l))) return e;
       p.wmap[0] = bb.mWup[wv(p)][l]; p.wmap_h[0] = bb.mWup[1][l]; p.bias[0] = (const bf16 *)bb.bup[l];
       set_lora(p, 0, FMX_TGT_UP, l);
       p.omap = oHid;
@@ -980,9 +1046,10 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     }
     {
       const int tgs[1] = {FMX_TGT_DOWN};
-      if ((e = shrink(mHid, d.d_ffn, tgs, 1, l))) return e;
       PairGemmParams p = base;
       p.mode = GM_RESID_F32; p.amap = mHid; p.K = d.d_ffn; p.n_chunks = d.d_model / 128;
+      if (can_fuse(p, 1)) shrink_fused(p, tgs, 1, l);
+      else if ((e = shrink(mHid, d.d_ffn, tgs, 1, l))) return e;
       p.wmap[0] = bb.mWdown[wv(p)][l]; p.wmap_h[0] = bb.mWdown[1][l]; p.bias[0] = (const bf16 *)bb.bdown[l];
       set_lora(p, 0, FMX_TGT_DOWN, l);
       p.omap = oX;
@@ -1006,7 +1073,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   }
   ha.skip_flatten = (any_flat && g_head_tiled) ? 1 : 0;
   if (any_pooled || !ha.skip_flatten) LAUNCH(Lh, F_HEAD, (launch_k(head_kernel, dim3(B, (max_out + 7) / 8), 256, 0, s, ha)));
-  if (ha.skip_flatten) LAUNCH(Lh, F_HEAD, (launch_k(head_flatten_kernel, dim3((B + 3) / 4, (max_out + 31) / 32), 256, 0, s, ha, B)));
+  if (ha.skip_flatten) LAUNCH(Lh, F_HEAD, (launch_k(head_flatten_kernel, dim3((B + 3) / 4, (max_out + 3) / 4), 256, 0, s, ha, B)));
 
   {
     void *bufs[7] = {w.X, w.Xn, w.QKV, w.AttnO, w.Hid, w.U, w.feat};
@@ -1229,6 +1296,10 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
     case FMX_OPT_ATTN_SHORT:
       if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attn_short %d", value);
       g_attn_short = value;
+      return FMX_OK;
+    case FMX_OPT_SHRINK_FUSED:
+      if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: shrink_fused %d", value);
+      g_shrink_fused = value;
       return FMX_OK;
     case FMX_OPT_HEAD_TILED:
       g_head_tiled = value ? 1 : 0;

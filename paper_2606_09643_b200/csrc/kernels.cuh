@@ -507,15 +507,17 @@ __global__ void __launch_bounds__(256) head_kernel(const HeadArgs a) {
 
 // FLATTEN heads (cfg2 forecasting: d_feat = 64 x 1024, 96 outputs, 12.6 MB of weights per task).  head_kernel spends ~30
 // instructions per (request, output) per 8 features, almost all of them loads and bf16 unpacking, and is issue-bound.
-// Here a warp owns a 4-request x 4-output register tile: every unpacked weight serves 4 requests and every unpacked
-// feature 4 outputs.  grid (ceil(B / 4) groups of consecutive SORTED requests, ceil(max_out / 32)); requests of a group
-// that belong to another task than its first FLATTEN request are handled in further passes (task boundaries only).
+// Here a CTA owns a 4-request x 4-output tile: every unpacked weight serves 4 requests and every unpacked feature 4
+// outputs; its 8 warps split the feature axis and their partial sums are added in warp order (deterministic).
+// grid (ceil(B / 4) groups of consecutive SORTED requests, ceil(max_out / 4)); requests of a group that belong to another
+// task than its first FLATTEN request are handled in further passes (task boundaries only).
 __global__ void __launch_bounds__(256) head_flatten_kernel(const HeadArgs a, int B) {
+  __shared__ float s_part[8][16];
   griddep_launch();
   griddep_wait();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int p0 = blockIdx.x * 4;
-  const int o0 = (blockIdx.y * 8 + warp) * 4;
+  const int o0 = blockIdx.y * 4;
   int task[4];
   unsigned todo = 0;
 #pragma unroll
@@ -523,7 +525,7 @@ __global__ void __launch_bounds__(256) head_flatten_kernel(const HeadArgs a, int
     task[i] = p0 + i < B ? a.task_sorted[p0 + i] : -1;
     if (task[i] >= 0 && a.task_head_kind[task[i]] == 3 && o0 < a.task_head_out[task[i]]) todo |= 1u << i;
   }
-  while (todo) {
+  while (todo) {                                           // CTA-uniform
     const int lead = __ffs(todo) - 1;
     const int t = task[lead];
     unsigned grp = 0;
@@ -543,7 +545,7 @@ __global__ void __launch_bounds__(256) head_flatten_kernel(const HeadArgs a, int
     for (int i = 0; i < 4; ++i)
 #pragma unroll
       for (int j = 0; j < 4; ++j) acc[i][j] = 0.0f;
-    for (long long c = lane * 8; c < K; c += 256) {
+    for (long long c = (long long)(warp * 32 + lane) * 8; c < K; c += 8 * 256) {
       float fv[4][8], wv[8];
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
@@ -562,7 +564,6 @@ __global__ void __launch_bounds__(256) head_flatten_kernel(const HeadArgs a, int
           for (int e = 0; e < 8; ++e) acc[i][j] = fmaf(fv[i][e], wv[e], acc[i][j]);
       }
     }
-    const __nv_bfloat16 *b = a.task_head_b[t];
 #pragma unroll
     for (int i = 0; i < 4; ++i)
 #pragma unroll
@@ -570,9 +571,18 @@ __global__ void __launch_bounds__(256) head_flatten_kernel(const HeadArgs a, int
         float v = acc[i][j];
 #pragma unroll
         for (int s = 16; s > 0; s >>= 1) v += __shfl_xor_sync(0xffffffffu, v, s);
-        if (lane == 0 && ((grp >> i) & 1u) && o0 + j < n_out)
-          a.out[a.out_off[a.perm[p0 + i]] + o0 + j] = v + (b ? __bfloat162float(b[o0 + j]) : 0.0f);
+        if (lane == 0) s_part[warp][i * 4 + j] = v;
       }
+    __syncthreads();
+    if (threadIdx.x < 16) {
+      const int i = threadIdx.x >> 2, j = threadIdx.x & 3;
+      float v = 0.0f;
+#pragma unroll
+      for (int wq = 0; wq < 8; ++wq) v += s_part[wq][threadIdx.x];
+      const __nv_bfloat16 *b = a.task_head_b[t];
+      if (((grp >> i) & 1u) && o0 + j < n_out) a.out[a.out_off[a.perm[p0 + i]] + o0 + j] = v + (b ? __bfloat162float(b[o0 + j]) : 0.0f);
+    }
+    __syncthreads();
   }
 }
 

@@ -68,6 +68,17 @@ struct PairGemmParams {
   const float *posb;       // [max_seq, ld_pos] fp32 (embed)
   const int *row_pos;
   int ld_pos;
+  // ---- fused LoRA shrink (n_sh > 0): the first *n_blk work items compute U_blk = s_t · x A_t^T for the targets that read
+  // this GEMM's own input, one item per (256-row tile, task) block; the expand steps of the regular tiles wait for them
+  CUtensorMap smap[3];     // A-slabs [Rcap, K] of the shrink targets, box {64, 64}
+  int n_sh;                // number of shrink targets (0 = none; 3 needs kBN = 256)
+  int sh_tg[3];            // their target ids
+  const int *blk_tile, *blk_lo, *blk_hi, *n_blk;
+  const float *task_scale; // [T*7] alpha / r
+  __nv_bfloat16 *U;        // [n_blk_cap*256, 192]
+  unsigned *u_flag;        // one counter: arrivals of the epilogue warps that wrote a U block (monotonic over a forward)
+  unsigned u_epoch;        // 1, 2, ... over the fused launches of a forward: this launch's U is complete when the counter
+                           // reaches 16 (epilogue warps of a pair) * n_blk * u_epoch
   const float2 *rope_cs;   // [max_seq, 64] (cos, sin): fused rotate-half RoPE for head_dim 128 (chunk = head), or NULL
   int rope_src_mask;       // bit s: source s (q | k | v) is rotated
 };
@@ -159,7 +170,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
   const int n_ntiles = p.n_chunks / kCH;
   const int whole_tiles = p.n_ptiles * n_ntiles;
   const int n_full = (kCH == 2 && p.n_full >= 0) ? p.n_full : whole_tiles;
-  const int total_tiles = n_full + 2 * (whole_tiles - n_full);
+  const int u_n = p.n_sh == 3 ? 256 : 128;                   // accumulator columns of a shrink item (64 per target)
   const int tile0 = (int)cluster_id_x(), tile_step = (int)cluster_nctaid_x();
 
   if (threadIdx.x == 0) {
@@ -177,6 +188,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
   const uint32_t tmem_base = tmem_base_slot;
   griddep_launch();
   griddep_wait();
+  const int n_u = p.n_sh > 0 ? *p.n_blk : 0;                // fused-shrink items come first in the work list
+  const int total_tiles = n_u + n_full + 2 * (whole_tiles - n_full);
 
   if (warp == 0) {
     // ================================ TMA producer (both CTAs) ================================
@@ -184,9 +197,29 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
       tma_prefetch_desc(&p.amap);
       tma_prefetch_desc(&p.wmap[0]);
       int stage = 0; uint32_t phase = 0;
+      bool u_ready = p.n_sh == 0;
       for (int tile = tile0; tile < total_tiles; tile += tile_step) {
+        if (tile < n_u) {
+          // ---- fused-shrink item: block `tile` of the S1 table; B = the task's A-slab rows of each shrink target.
+          // u_n = 256: CTA 0 loads targets 0, 1 and CTA 1 target 2; u_n = 128: CTA r loads target r.
+          const int m0 = p.blk_tile[tile] * kPairRows + (int)rank * kBM;
+          const int coff = p.task_coff[p.blk_task[tile]];
+          const int tg_lo = u_n == 256 ? (int)rank * 2 : (int)rank;
+          const int tg_hi = min(p.n_sh, u_n == 256 ? tg_lo + 2 : tg_lo + 1);
+          const uint32_t tx = kATileBytes + (uint32_t)max(tg_hi - tg_lo, 0) * 64 * kBK * 2;
+          for (int kb = 0; kb < nK; ++kb) {
+            mbar_wait(&empty_bar[stage], phase ^ 1);
+            uint8_t *sa = smem + stage * kStageBytes, *sb = sa + kATileBytes;
+            const uint32_t fb = mapa_shared(smem_u32(&full_bar[stage]), 0);
+            mbar_arrive_expect_tx_cluster(fb, tx);
+            tma_load_2d_2sm(sa, &p.amap, fb, kb * kBK, m0);
+            for (int g = tg_lo; g < tg_hi; ++g) tma_load_2d_2sm(sb + (g - tg_lo) * 64 * kBK * 2, &p.smap[g], fb, kb * kBK, coff);
+            if (++stage == kStages) { stage = 0; phase ^= 1; }
+          }
+          continue;
+        }
         int m_pt, c0, nch;
-        pair_decode<kCH>(p, tile, n_ntiles, n_full, m_pt, c0, nch);
+        pair_decode<kCH>(p, tile - n_u, n_ntiles, n_full, m_pt, c0, nch);
         const int m0 = m_pt * kPairRows + (int)rank * kBM;
         int bsrc, brow;
         const CUtensorMap *wm;
@@ -219,6 +252,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
             for (int b = b0; b < b1; ++b) {
               const int t = p.blk_task[b];
               if (p.task_trpad[t * 7 + tg] == 0) continue;
+              if (!u_ready) {                               // U is written by the fused-shrink items of all pairs: wait once
+                const unsigned target = 16u * (unsigned)n_u * p.u_epoch;
+                while (ld_acquire_gpu(p.u_flag) < target) {
+                }
+                fence_proxy_async_global();
+                u_ready = true;
+              }
               mbar_wait(&empty_bar[stage], phase ^ 1);
               uint8_t *sa = smem + stage * kStageBytes, *sb = sa + kATileBytes;
               const uint32_t fb = mapa_shared(smem_u32(&full_bar[stage]), 0);
@@ -238,9 +278,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
       constexpr uint32_t idesc_whole = make_idesc_bf16(kPairRows, kBN);
       constexpr uint32_t idesc_lora = make_idesc_bf16(kPairRows, kChunk);
       for (int tile = tile0; tile < total_tiles; tile += tile_step) {
-        int m_pt, c0, nch;
-        pair_decode<kCH>(p, tile, n_ntiles, n_full, m_pt, c0, nch);
-        const uint32_t idesc_main = nch == kCH ? idesc_whole : idesc_lora;
+        int m_pt = 0, c0 = 0, nch = 0;
+        const bool u_item = tile < n_u;
+        if (!u_item) pair_decode<kCH>(p, tile - n_u, n_ntiles, n_full, m_pt, c0, nch);
+        const uint32_t idesc_main = u_item ? (u_n == 256 ? make_idesc_bf16(kPairRows, 256) : idesc_lora) : (nch == kCH ? idesc_whole : idesc_lora);
         mbar_wait_cluster(&tempty_bar[acc], accphase ^ 1);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + acc * kAccStride;
@@ -255,7 +296,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
           umma_commit_2sm(&empty_bar[stage], 3);
           if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
-        if (p.has_lora) {
+        if (p.has_lora && !u_item) {
           const int b0 = p.tile_blk_off[m_pt], b1 = p.tile_blk_off[m_pt + 1];
           for (int c = 0; c < nch; ++c) {
             int s, r0;
@@ -292,8 +333,41 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
     int acc = 0; uint32_t accphase = 0;
     const int mode = p.mode;
     for (int tile = tile0; tile < total_tiles; tile += tile_step) {
+      if (tile < n_u) {
+        // ---- fused-shrink item: U_blk[row, slot*64 + j] = bf16(s_t · acc), rows outside the block's task zeroed ----
+        const int b = tile, t = p.blk_task[b];
+        const int rp = (int)rank * kBM + r_in_tile;             // row within the 256-row tile
+        const bool in_seg = rp >= p.blk_lo[b] && rp < p.blk_hi[b];
+        __nv_bfloat16 *Urow = p.U + (size_t)(b * kPairRows + rp) * 192;
+        mbar_wait(&tfull_bar[acc], accphase);
+        tc_fence_after();
+        const uint32_t t_row = tmem_base + (uint32_t(quad * 32) << 16) + acc * kAccStride;
+        uint32_t v[32];
+        const int n_grp = p.n_sh * 2;                           // 32-column groups, split over the two warpgroups
+        for (int g = wg; g < n_grp; g += 2) {
+          __syncwarp();
+          tmem_ld_32x32(t_row + g * 32, v);
+          tmem_ld_wait();
+          const float sc = in_seg ? p.task_scale[t * 7 + p.sh_tg[g >> 1]] : 0.0f;
+          uint4 *dst = reinterpret_cast<uint4 *>(Urow + g * 32);
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+            dst[j] = make_uint4(pack_bf16(sc * __uint_as_float(v[8 * j + 0]), sc * __uint_as_float(v[8 * j + 1])),
+                                pack_bf16(sc * __uint_as_float(v[8 * j + 2]), sc * __uint_as_float(v[8 * j + 3])),
+                                pack_bf16(sc * __uint_as_float(v[8 * j + 4]), sc * __uint_as_float(v[8 * j + 5])),
+                                pack_bf16(sc * __uint_as_float(v[8 * j + 6]), sc * __uint_as_float(v[8 * j + 7])));
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) {
+          mbar_arrive_cluster(mapa_shared(smem_u32(&tempty_bar[acc]), 0));
+          red_release_gpu_add(p.u_flag, 1u);                    // 16 arrivals (8 epilogue warps x 2 CTAs) per block
+        }
+        if (++acc == 2) { acc = 0; accphase ^= 1; }
+        continue;
+      }
       int m_pt, c0, nch;
-      pair_decode<kCH>(p, tile, n_ntiles, n_full, m_pt, c0, nch);
+      pair_decode<kCH>(p, tile - n_u, n_ntiles, n_full, m_pt, c0, nch);
       const int bn = nch * kChunk;                              // columns of this work item (a half tile has 128)
       const int row0_cta = m_pt * kPairRows + (int)rank * kBM;
       const int row = row0_cta + r_in_tile;

@@ -120,6 +120,40 @@ def test_reduced_configs_parity(fmx_mod, cfg, kw):
     check_parity(y, G.oracle_outputs(wl), f"{cfg} {kw}")
 
 
+@pytest.mark.parametrize("cfg,kw", [
+    ("cfg1", {}),                                                   # q, v adapters only (k has none): 2 of 3 QKV targets
+    ("cfg2", dict(n_layers=2, batch=20)),                           # single-task tiles and tiles that straddle tasks
+    ("cfg3", dict(n_layers=2, batch=6)),                            # ranks 8 / 16, 3 targets -> 256-wide shrink items
+    ("cfg4", dict(n_layers=2, batch=8, max_len=200)),               # 7 targets, ranks to 64, K = 8960 on `down`
+    ("cfg5", dict(n_layers=2, batch=40, n_tasks=16, dist="uniform")),  # more blocks than row tiles
+])
+def test_every_kernel_option_gives_the_oracle_result(fmx_mod, cfg, kw):
+    """The alternative code paths behind fmx_set_option stay parity-green: LoRA shrink as the first work items of the
+    consuming GEMM (forced on: 2) or as separate launches (0) must agree bit for bit (same MMA order, same rounding);
+    whole-tile-only GEMM waves, the separate RoPE kernel, the one-warp-per-output FLATTEN head and programmatic dependent
+    launch forced on each match the oracle within the bar."""
+    wl = make_workload(cfg, **kw)
+    s = _session(fmx_mod, wl)
+    ref = G.oracle_outputs(wl)
+    outs = {}
+    try:
+        for fused in (0, 2):
+            s.fmx.set_option("shrink_fused", fused)
+            outs[fused] = s.forward_numpy()
+            check_parity(outs[fused], ref, f"{cfg} shrink_fused={fused}")
+        for a, b in zip(outs[0], outs[2]):
+            assert np.array_equal(a, b), "fused and separate LoRA shrink must be bit-identical"
+        s.fmx.set_option("shrink_fused", 1)
+        for opt, val, restore in (("half_tiles", 0, 1), ("rope_fused", 0, 1), ("head_tiled", 0, 1), ("pdl", 1, 2), ("pdl", 0, 2)):
+            s.fmx.set_option(opt, val)
+            try:
+                check_parity(s.forward_numpy(), ref, f"{cfg} {opt}={val}")
+            finally:
+                s.fmx.set_option(opt, restore)
+    finally:
+        s.fmx.set_option("shrink_fused", 1)
+
+
 # ---------------------------------------------------------------- full sizes, sampled outputs
 @pytest.mark.parametrize("cfg,kw,n_sample", [
     ("cfg2", {}, 6),
