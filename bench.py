@@ -11,13 +11,19 @@ encoder-shaped time-series backbone, batch 256, 10 tasks, Zipf(1.1) task ids); c
 tiny parity case and the other configs are selectable with --workload.  Rank 0 prints ONE JSON line.
 
   value      whole-job samples/s, inputs resident in HBM, CUDA events around every step on the
-             launching stream, L2 flushed (256 MB memset) between steps outside the events.
+             launching stream, L2 flushed (256 MB memset) between steps outside the events.  The
+             step is the C-ABI call fmx_forward_mixed on a non-default stream; the call is identical
+             every step, so the library replays its cached CUDA graph (FMX_OPT_GRAPH; --no-graph
+             times plain launches).
   e2e        the same metric through fmx_forward_mixed_host: pinned HOST inputs -> device, forward,
              outputs -> HOST, inside the timed region (wall clock around the synchronous calls).
-  roofline   the tcgen05 GEMM kernel (all four projection families): algorithmic FLOPs per launch
-             / average launch duration from CUDA events recorded around those launches INSIDE the
-             timed region, against MEASURED_PEAKS.json (sustained bf16 figure: the kernel is timed
-             inside a long step; the burst fraction is given too).
+  roofline   the tcgen05 pair GEMM kernel (all four projection families): algorithmic FLOPs per
+             launch / average launch duration from CUDA events recorded around those launches in K
+             more steps of the same loop right after the timed ones (per-launch events need plain
+             launches, so they cannot share steps with the graph), against MEASURED_PEAKS.json
+             (sustained bf16 figure: the kernel is timed inside a long step; the burst fraction is
+             given too).  When the LoRA shrink runs fused inside those launches its algorithmic FLOPs
+             are counted with them.
   cpu_baseline  the oracle (numpy fp64, as it stands) on a bounded sample of the same workload.
 
 Multi-GPU is replicas only: every rank runs the same batch shape on its own GPU, no
@@ -209,6 +215,16 @@ def timed_steps(sess, torch, steps, flush):
 
 
 def measure(args, wl, rank, local_rank, world, with_cpu_baseline=True):
+    """Everything runs on one non-default stream: fmx_forward_mixed replays its cached CUDA graph there (FMX_OPT_GRAPH)."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libfmx has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    with torch.cuda.stream(torch.cuda.Stream(torch.device("cuda", local_rank))):
+        return _measure(args, wl, rank, local_rank, world, with_cpu_baseline)
+
+
+def _measure(args, wl, rank, local_rank, world, with_cpu_baseline=True):
     import numpy as np
     import torch
     from paper_2606_09643_b200 import accounting, replicas
@@ -231,21 +247,32 @@ def measure(args, wl, rank, local_rank, world, with_cpu_baseline=True):
     torch.cuda.synchronize()
     launches_per_step = sess.fmx.last_launch_count()
 
-    # ---- timed region: K steps; events around the GEMM launches only (the roofline's kernel) ----
-    if not args.no_kernel_events:
-        sess.fmx.profile_select(GEMM_FAMILIES)
-        sess.fmx.profile_enable(True)
+    # ---- timed region: exactly K steps through fmx_forward_mixed (which replays its cached CUDA graph: the call is
+    # identical every step), then K more steps of the same loop with CUDA events around the GEMM launches (the roofline's
+    # kernel; per-launch events need plain launches, so they cannot share steps with the graph).  The clock sampler
+    # covers both.
+    sess.fmx.set_option("graph", 0 if args.no_graph else 1)
+    for _ in range(2):
+        sess.forward()
     replicas.barrier()
     torch.cuda.synchronize()
     if sampler:
         sampler.start()
+    replays0 = sess.fmx.graph_replays()
     ms_total = timed_steps(sess, torch, args.steps, flush)
     torch.cuda.synchronize()
     replicas.barrier()
+    graph_steps = sess.fmx.graph_replays() - replays0
+    gemm_prof, ms_prof_steps = {}, 0.0
+    if not args.no_kernel_events:
+        sess.fmx.profile_select(GEMM_FAMILIES)
+        sess.fmx.profile_enable(True)
+        ms_prof_steps = timed_steps(sess, torch, args.steps, flush)
+        torch.cuda.synchronize()
+        gemm_prof = sess.fmx.profile_read()
+        sess.fmx.profile_enable(False)
     if sampler:
         sampler.stop()
-    gemm_prof = sess.fmx.profile_read() if not args.no_kernel_events else {}
-    sess.fmx.profile_enable(False)
     ms_max = replicas.max_over_ranks(ms_total, dev if world > 1 else None)
     value = replicas.whole_job_throughput(B, args.steps, ms_max, world)
     clocks = sampler.result() if sampler else None
@@ -293,7 +320,9 @@ def measure(args, wl, rank, local_rank, world, with_cpu_baseline=True):
     if gemm_prof:
         n_l = sum(gemm_prof[f][0] for f in GEMM_FAMILIES)
         ms_g = sum(gemm_prof[f][1] for f in GEMM_FAMILIES)
-        fl_g = sum(fl["families"][f] for f in GEMM_FAMILIES)            # per forward
+        fused = "lora_shrink" not in breakdown      # the LoRA shrink ran as work items of the GEMM launches (no shrink family)
+        fam_fl = {f: fl["families"][f] + (fl["shrink_families"][f] if fused else 0.0) for f in GEMM_FAMILIES}
+        fl_g = sum(fam_fl.values())                                     # per forward
         avg_ms = ms_g / max(n_l, 1)
         flops_per_launch = fl_g / accounting.gemm_launches_per_forward(wl)
         achieved = flops_per_launch / (avg_ms * 1e-3) / 1e12
@@ -303,8 +332,10 @@ def measure(args, wl, rank, local_rank, world, with_cpu_baseline=True):
                 "frac_of_burst_peak": round(achieved / pk["bf16_tflops"], 4), "traffic": gemm_traffic(args.workload),
                 "traffic_unit": "DRAM bytes per launch (ncu --set full, cold cache; profiles/gemm_traffic.csv)",
                 "flops_per_launch": flops_per_launch, "avg_launch_ms": round(avg_ms, 5), "launches_timed": n_l,
-                "share_of_step": round(ms_g / ms_total, 4),
-                "per_family_tflops": {f: round(fl["families"][f] * args.steps / (gemm_prof[f][1] * 1e-3) / 1e12, 1)
+                "share_of_step": round(ms_g / ms_prof_steps, 4),
+                "timed_in": f"{args.steps} steps of the same loop right after the timed region (per-launch events need plain launches; {round(ms_prof_steps / args.steps, 4)} ms/step there)",
+                "fused_lora_shrink": fused,
+                "per_family_tflops": {f: round(fam_fl[f] * args.steps / (gemm_prof[f][1] * 1e-3) / 1e12, 1)
                                       for f in GEMM_FAMILIES if gemm_prof[f][1] > 0}}
     line = {"metric": METRIC, "value": round(value, 2), "unit": "samples/s", "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": round(ms_max / args.steps, 4), "higher_is_better": True, "scaling": "weak",
@@ -312,7 +343,8 @@ def measure(args, wl, rank, local_rank, world, with_cpu_baseline=True):
             "config": {"workload": WORKLOAD_NAMES.get(args.workload, args.workload), "requests": B, "tokens": wl.n_tokens,
                        "tasks": len(wl.tasks), "tasks_in_batch": int(len(set(wl.task_ids.tolist()))), "dist": wl.notes.get("dist"),
                        "l2": "flushed (256 MB memset) between steps, outside the per-step events" if flush is not None else "no flush",
-                       "accumulate": "fp32 (TMEM), fp32 residual stream", "replicas": world},
+                       "accumulate": "fp32 (TMEM), fp32 residual stream", "replicas": world,
+                       "launch": f"CUDA graph replay inside fmx_forward_mixed on {graph_steps} of {args.steps} timed steps" if graph_steps else "plain kernel launches"},
             "pct_bf16_tensor_peak": {"of_burst": round(100 * fl["total"] * world * args.steps / (ms_max * 1e-3) / 1e12 / pk["bf16_tflops"], 2),
                                      "of_sustained": round(100 * fl["total"] * world * args.steps / (ms_max * 1e-3) / 1e12 / pk["bf16_tflops_sustained"], 2),
                                      "algorithmic_tflop_per_step": round(fl["total"] / 1e12, 4), "peaks": pk["source"]},
@@ -371,6 +403,7 @@ def main():
     ap.add_argument("--dist", default="zipf0.8", choices=["uniform", "zipf0.8", "zipf1.5"])
     ap.add_argument("--no-adapters", action="store_true", help="cfg5: head-only tasks (adapter-free reference)")
     ap.add_argument("--no-flush", action="store_true")
+    ap.add_argument("--no-graph", action="store_true", help="plain kernel launches in the timed region (FMX_OPT_GRAPH off)")
     ap.add_argument("--no-kernel-events", action="store_true", help="no per-GEMM events inside the timed region (no roofline)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample", type=int, default=24, help="requests the oracle is timed on (cpu_baseline)")

@@ -194,6 +194,8 @@ int fmx_profile_read(fmx_ctx *ctx, int32_t *launches /*[FMX_N_FAMILIES]*/, doubl
 const char *fmx_profile_family_name(int family);
 /* Kernels launched by the last forward (the count bench.py reports as gpu_launches). */
 int fmx_last_launch_count(fmx_ctx *ctx);
+/* Forwards served by replaying the context's cached CUDA graph so far (FMX_OPT_GRAPH; debug / tests). */
+long long fmx_graph_replays(fmx_ctx *ctx);
 
 /* Debug/test: one GEMM through the tcgen05 kernel, C[M,N] (fp32) = A[M,K] (bf16) · W[N,K]^T (bf16);
  * N a multiple of 128, K a multiple of 8.  All DEVICE pointers. */
@@ -224,6 +226,9 @@ enum {
   FMX_OPT_SHRINK_FUSED = 8,      /* the LoRA shrink runs as the first work items of the GEMM that consumes it: 0 = never
                                     (separate shrink kernel), 1 (default) = when the batch has at most one (tile, task)
                                     block per CTA pair, 2 = always */
+  FMX_OPT_GRAPH = 9,             /* 1 (default): fmx_forward_mixed captures a CUDA graph on the 2nd identical call (same
+                                    buffers, stream, ids, lengths, registrations, options) and replays it afterwards;
+                                    needs a non-default stream; 0: always plain launches */
   FMX_OPT_PDL = 2                /* programmatic dependent launch of the forward's kernels (process-wide):
                                     0 = off, 1 = always, 2 (default) = only for batches of <= 4096 token rows */
 };

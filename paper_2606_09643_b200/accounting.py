@@ -24,10 +24,13 @@ def flops(wl: Workload) -> dict:
     fam_of = {"q": "gemm_qkv", "k": "gemm_qkv", "v": "gemm_qkv", "o": "gemm_o", "gate": "gemm_ffn_in",
               "up": "gemm_ffn_in", "down": "gemm_ffn_out"}
     shrink = expand = 0.0
+    shrink_fam = {k: 0.0 for k in fam}          # shrink FLOPs by the GEMM family that consumes (and, when fused, computes) them
     for t, n in zip(wl.task_ids, wl.lengths):
         for ad in wl.tasks[int(t)].adapters:
             din, dout = target_dims(bb, ad.target)
-            shrink += 2.0 * int(n) * ad.rank * din * L
+            sh = 2.0 * int(n) * ad.rank * din * L
+            shrink += sh
+            shrink_fam[fam_of[ad.target]] += sh
             e = 2.0 * int(n) * ad.rank * dout * L
             expand += e
             fam[fam_of[ad.target]] += e
@@ -39,7 +42,7 @@ def flops(wl: Workload) -> dict:
     embed = 2.0 * bb.patch_dim * d * bb.n_patches * wl.n_req if bb.input_kind == "patch" else 0.0
     total = base + shrink + expand + attn + head + embed
     return dict(base_gemm=base, lora_shrink=shrink, lora_expand=expand, attention=attn, head=head, embed=embed,
-                total=total, families=fam)
+                total=total, families=fam, shrink_families=shrink_fam)
 
 
 def gemm_launches_per_forward(wl: Workload) -> int:

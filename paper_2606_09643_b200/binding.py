@@ -52,7 +52,7 @@ class BfqParams(C.Structure):
     _fields_ = [("n_tasks", C.c_int32), ("b_max", C.c_int32), ("lat_ms", C.POINTER(C.c_double)), ("l_tok_ms", C.c_double)]
 
 
-OPTIONS = {"attention_impl": 0, "attention_variant": 1, "pdl": 2, "shrink_stages": 3, "half_tiles": 4, "attn_short": 5, "rope_fused": 6, "head_tiled": 7, "shrink_fused": 8}
+OPTIONS = {"attention_impl": 0, "attention_variant": 1, "pdl": 2, "shrink_stages": 3, "half_tiles": 4, "attn_short": 5, "rope_fused": 6, "head_tiled": 7, "shrink_fused": 8, "graph": 9}
 
 
 class FmxError(RuntimeError):
@@ -66,7 +66,7 @@ _lib = None
 EXPORTS = ["fmx_create", "fmx_destroy", "fmx_last_error", "fmx_version", "fmx_register_backbone", "fmx_register_task",
            "fmx_unregister_task", "fmx_output_layout", "fmx_workspace_bytes", "fmx_forward_mixed", "fmx_forward_mixed_host",
            "fmx_debug_get_segments", "fmx_debug_get_tiles", "fmx_debug_read", "fmx_task_slots", "fmx_profile_enable", "fmx_profile_select", "fmx_profile_read",
-           "fmx_profile_family_name", "fmx_last_launch_count", "fmx_debug_gemm", "fmx_debug_attention", "fmx_set_option", "fmx_bfq_create", "fmx_bfq_destroy",
+           "fmx_profile_family_name", "fmx_last_launch_count", "fmx_graph_replays", "fmx_debug_gemm", "fmx_debug_attention", "fmx_set_option", "fmx_bfq_create", "fmx_bfq_destroy",
            "fmx_bfq_set_task", "fmx_bfq_enqueue", "fmx_bfq_next_batch", "fmx_bfq_complete", "fmx_bfq_stats", "fmx_bfq_peek"]
 
 
@@ -101,6 +101,8 @@ def load():
     lib.fmx_profile_select.argtypes = [_vp, C.c_uint32]
     lib.fmx_profile_read.argtypes = [_vp, i32p, f64p]
     lib.fmx_last_launch_count.argtypes = [_vp]
+    lib.fmx_graph_replays.argtypes = [_vp]
+    lib.fmx_graph_replays.restype = C.c_longlong
     lib.fmx_debug_gemm.argtypes = [_vp, _vp, _vp, _vp, C.c_int32, C.c_int32, C.c_int32, _vp]
     lib.fmx_debug_attention.argtypes = [_vp, _vp, _vp, i32p, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, _vp]
     lib.fmx_set_option.argtypes = [_vp, C.c_int32, C.c_int32]
@@ -256,6 +258,9 @@ class Fmx:
 
     def last_launch_count(self):
         return self.lib.fmx_last_launch_count(self.h)
+
+    def graph_replays(self):
+        return int(self.lib.fmx_graph_replays(self.h))
 
     def debug_gemm(self, A, W, Cout, M, N, K, stream=0):
         _check(self.lib.fmx_debug_gemm(self.h, A, W, Cout, M, N, K, stream or None))

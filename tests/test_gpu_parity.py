@@ -315,3 +315,42 @@ def test_host_buffer_forward_matches_device_forward(fmx_mod):
     got = host_out.numpy()
     for i in range(wl.n_req):
         assert np.array_equal(got[off[i]:off[i + 1]], dev[i])
+
+
+def test_cuda_graph_cache_replays_only_identical_calls(fmx_mod):
+    """FMX_OPT_GRAPH: on a non-default stream the 2nd identical call is captured and later ones replay the graph.  The
+    replayed result equals the plain one bit for bit; different task ids, a registration change or the default stream
+    never replay a stale graph."""
+    wl = make_workload("cfg2", n_layers=2, batch=20)
+    s = _session(fmx_mod, wl)
+    plain = s.forward_numpy()                                    # torch's default stream: never graphed
+    assert s.fmx.graph_replays() == 0
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        outs = []
+        for _ in range(4):
+            s.forward(stream=st)
+            st.synchronize()
+            flat = s.out_dev.cpu().numpy()
+            outs.append([flat[s.last_off[i]:s.last_off[i + 1]].copy() for i in range(wl.n_req)])
+        assert s.fmx.graph_replays() == 2                        # call 1 plain, call 2 capture + launch, calls 3-4 replay
+        for o in outs:
+            for a, b in zip(o, plain):
+                assert np.array_equal(a, b)
+        # other task ids, same shapes: must run the new batch, not the cached graph
+        ids2 = np.roll(wl.task_ids, 1)
+        s.forward(task_ids=ids2, stream=st)
+        st.synchronize()
+        assert s.fmx.graph_replays() == 2
+        flat = s.out_dev.cpu().numpy()
+        got = [flat[s.last_off[i]:s.last_off[i + 1]].copy() for i in range(wl.n_req)]
+    ref = s.forward_numpy(task_ids=ids2)
+    for a, b in zip(got, ref):
+        assert np.array_equal(a, b)
+    # option change invalidates the cached graph
+    with torch.cuda.stream(st):
+        s.fmx.set_option("half_tiles", 1)
+        n0 = s.fmx.graph_replays()
+        s.forward(stream=st); s.forward(stream=st); s.forward(stream=st)
+        st.synchronize()
+        assert s.fmx.graph_replays() == n0 + 1
