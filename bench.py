@@ -199,6 +199,34 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------- the CUDA arm
+def bfq_host_cost(wl):
+    """S0: the host-side BFQ batch builder on a backlog shaped like the workload (its task-id mix and lengths, weights 1..3):
+    enqueue (Eq. 1-2 tags), next_batch (order by S, extend to B_max) and complete (Eq. 3 retag), timed through the C ABI
+    from Python, so the figure includes ~1 us of ctypes per enqueue.  Paper: 0.35 ms per request on its host."""
+    import numpy as np
+    from paper_2606_09643_b200.binding import Bfq
+    B, T = wl.n_req, len(wl.tasks)
+    rounds = 8
+    q = Bfq(T, B, [1.0 + 0.04 * b for b in range(B)])
+    for t in range(T):
+        q.set_task(t, 1.0 + (t % 3))
+    ids = np.tile(np.asarray(wl.task_ids, dtype=np.int64), rounds)
+    lens = np.tile(np.asarray(wl.lengths, dtype=np.int64), rounds)
+    t0 = time.perf_counter()
+    for i in range(len(ids)):
+        q.enqueue(int(ids[i]), i, int(lens[i]), 0.001 * i)
+    t1 = time.perf_counter()
+    served = 0
+    for r in range(rounds):
+        b_ids, _, _ = q.next_batch(10.0 + r, B)
+        q.complete(1.0 + 0.04 * len(b_ids))
+        served += len(b_ids)
+    t2 = time.perf_counter()
+    return {"us_per_request": round((t2 - t0) * 1e6 / max(served, 1), 3), "enqueue_us_per_request": round((t1 - t0) * 1e6 / len(ids), 3),
+            "batch_build_us_per_batch": round((t2 - t1) * 1e6 / rounds, 1), "requests": int(served), "batch": B, "tasks": T,
+            "how": "fmx_bfq_enqueue / next_batch / complete through ctypes on the host; paper: 350 us per request (P:L418, its host)"}
+
+
 def timed_steps(sess, torch, steps, flush):
     """K steps, each bracketed by its own CUDA events on the launching stream; L2 flushed between
     steps outside the events.  Returns total ms."""
@@ -350,6 +378,8 @@ def _measure(args, wl, rank, local_rank, world, with_cpu_baseline=True):
                                      "algorithmic_tflop_per_step": round(fl["total"] / 1e12, 4), "peaks": pk["source"]},
             "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "launches_per_step": launches_per_step,
             "clocks": clocks, "roofline": roof, "breakdown": breakdown}
+    if rank == 0:
+        line["bfq"] = bfq_host_cost(wl)
     if with_cpu_baseline and rank == 0 and world == 1 and not args.no_cpu_baseline:
         n = min(args.cpu_sample, B)
         idx = list(range(n))
