@@ -354,3 +354,31 @@ def test_cuda_graph_cache_replays_only_identical_calls(fmx_mod):
         s.forward(stream=st); s.forward(stream=st); s.forward(stream=st)
         st.synchronize()
         assert s.fmx.graph_replays() == n0 + 1
+
+
+def test_maximum_sizes_4096_requests_1024_tasks(fmx_mod):
+    """The ABI's limits (FMX_MAX_REQUESTS = 4096, FMX_MAX_TASKS = 1024) on the tiny encoder: 1024 registered tasks, one batch
+    of 4096 requests (262 144 token rows, 1024 row tiles, ~2000 (tile, task) blocks) with skewed task ids, some tasks absent.
+    Sort / segment tables bit-exact against the oracle; sampled requests against the fp64 forward."""
+    from oracle.vfm_forward import forward_request
+    T, B = 1024, 4096
+    wl = make_workload("cfg1", batch=12, n_tasks=T)
+    s = _session(fmx_mod, wl, max_req=B, max_tokens=B * 64)
+    assert s.fmx.task_slots() == T
+    rng = np.random.default_rng(20261104)
+    ids = np.minimum((rng.pareto(0.7, size=B) * 8).astype(np.int64), T - 1).astype(np.int32)   # heavy head, long tail
+    ids[:8] = T - 1                                                                           # the last slot is used too
+    lens = np.full(B, 64, dtype=np.int32)
+    x = f32_to_bf16_bits(rng.standard_normal((B, 64, 128)).astype(np.float32))
+    s.upload_inputs(x.reshape(-1))
+    y = s.forward_numpy(task_ids=ids, lengths=lens)
+    assert len(y) == B and all(np.isfinite(v).all() for v in y)
+    seg = s.fmx.debug_get_segments(B)
+    slot = np.array([s.task_ids_of[int(t)] for t in ids])
+    ref = segment_tables(slot, lens, T)
+    for k, v in ref.items():
+        assert np.array_equal(seg[k], v), f"segment table {k} differs at maximum size"
+    bb, get, tasks = G.bb_dict(wl), G.make_get(wl), G.task_dicts(wl)
+    xf = bf16_bits_to_f64(x)
+    pick = [0, 7, 8, int(np.argmax(ids == ids.max())), B - 1, int(rng.integers(0, B))]
+    check_parity([y[i] for i in pick], [forward_request(bb, get, tasks[int(ids[i])], xf[i]) for i in pick], "4096 x 1024")
