@@ -1127,20 +1127,11 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   return FMX_OK;
 }
 
-int fmx_forward_mixed(fmx_ctx *c, fmx_backbone_t h, const void *inputs, const int32_t *task_ids, const int32_t *lengths,
-                      int32_t n_req, float *outputs, void *workspace, size_t workspace_bytes, void *cuda_stream) {
-  if (!c) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed: NULL ctx");
-  if (n_req < 0) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed: n_req < 0");
-  Backbone *bb = get_bb(c, h);
-  if (!bb) return fmx_fail(FMX_E_UNKNOWN_BACKBONE, "forward_mixed: unknown backbone %d", h);
-  if (n_req == 0) return FMX_OK;
-  if (n_req > FMX_MAX_REQUESTS) return fmx_fail(FMX_E_CAPACITY, "forward_mixed: %d requests > %d", n_req, FMX_MAX_REQUESTS);
-  if (!inputs || !task_ids || !lengths || !outputs || !workspace) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed: NULL pointer");
-  std::lock_guard<std::mutex> lk(c->mu);
-  CU_OK(cudaSetDevice(c->device));
-  cudaStream_t s = (cudaStream_t)cuda_stream;
-  // ---- CUDA-graph cache: the 2nd identical call (same buffers, stream, ids, lengths, registrations, options) is captured,
-  // later ones replay it; a step of ~200 short kernels loses ~4 % to launch gaps otherwise (cfg2: 11.55 -> 11.09 ms).
+// The forward with the context's one-entry CUDA-graph cache in front of it (c->mu held by the caller).  The 2nd identical call
+// (same buffers, stream, ids, lengths, registrations, options) is captured, later ones replay it; a step of ~200 short
+// kernels loses ~4 % to launch gaps otherwise (cfg2: 11.55 -> 11.09 ms).
+static int forward_cached(fmx_ctx *c, Backbone *bb, fmx_backbone_t h, const void *inputs, const int32_t *task_ids, const int32_t *lengths,
+                          int32_t n_req, float *outputs, void *workspace, size_t workspace_bytes, cudaStream_t s) {
   const bool graphable = c->opt_graph && !c->prof_on && s != nullptr && s != cudaStreamLegacy && s != cudaStreamPerThread;
   if (graphable) {
     cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
@@ -1187,6 +1178,20 @@ int fmx_forward_mixed(fmx_ctx *c, fmx_backbone_t h, const void *inputs, const in
   return forward_impl(c, *bb, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, s);
 }
 
+int fmx_forward_mixed(fmx_ctx *c, fmx_backbone_t h, const void *inputs, const int32_t *task_ids, const int32_t *lengths,
+                      int32_t n_req, float *outputs, void *workspace, size_t workspace_bytes, void *cuda_stream) {
+  if (!c) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed: NULL ctx");
+  if (n_req < 0) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed: n_req < 0");
+  Backbone *bb = get_bb(c, h);
+  if (!bb) return fmx_fail(FMX_E_UNKNOWN_BACKBONE, "forward_mixed: unknown backbone %d", h);
+  if (n_req == 0) return FMX_OK;
+  if (n_req > FMX_MAX_REQUESTS) return fmx_fail(FMX_E_CAPACITY, "forward_mixed: %d requests > %d", n_req, FMX_MAX_REQUESTS);
+  if (!inputs || !task_ids || !lengths || !outputs || !workspace) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed: NULL pointer");
+  std::lock_guard<std::mutex> lk(c->mu);
+  CU_OK(cudaSetDevice(c->device));
+  return forward_cached(c, bb, h, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, (cudaStream_t)cuda_stream);
+}
+
 int fmx_forward_mixed_host(fmx_ctx *c, fmx_backbone_t h, const void *inputs_host, size_t inputs_bytes, const int32_t *task_ids,
                            const int32_t *lengths, int32_t n_req, float *outputs_host, void *workspace, size_t workspace_bytes,
                            void *cuda_stream) {
@@ -1217,7 +1222,7 @@ int fmx_forward_mixed_host(fmx_ctx *c, fmx_backbone_t h, const void *inputs_host
     c->out_stage_bytes = align_up(out_bytes, 1 << 16);
   }
   CU_OK(cudaMemcpyAsync(c->d_in_stage, inputs_host, inputs_bytes, cudaMemcpyHostToDevice, s));
-  if (int e = forward_impl(c, *bb, c->d_in_stage, task_ids, lengths, n_req, c->d_out_stage, workspace, workspace_bytes, s)) return e;
+  if (int e = forward_cached(c, bb, h, c->d_in_stage, task_ids, lengths, n_req, c->d_out_stage, workspace, workspace_bytes, s)) return e;
   CU_OK(cudaMemcpyAsync(outputs_host, c->d_out_stage, out_bytes, cudaMemcpyDeviceToHost, s));
   CU_OK(cudaStreamSynchronize(s));
   return FMX_OK;
