@@ -229,6 +229,8 @@ enum {
   FMX_OPT_GRAPH = 9,             /* 1 (default): fmx_forward_mixed captures a CUDA graph on the 2nd identical call (same
                                     buffers, stream, ids, lengths, registrations, options) and replays it afterwards;
                                     needs a non-default stream; 0: always plain launches */
+  FMX_OPT_REVERSE = 10,          /* 1 (default): consecutive kernels of a layer walk the token rows in alternating
+                                    directions, so each starts on the rows its producer wrote last (still in L2) */
   FMX_OPT_PDL = 2                /* programmatic dependent launch of the forward's kernels (process-wide):
                                     0 = off, 1 = always, 2 (default) = only for batches of <= 4096 token rows */
 };

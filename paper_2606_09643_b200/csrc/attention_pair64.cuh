@@ -31,6 +31,7 @@ struct AttnPairArgs {
   int n_req, n_q_heads, n_kv_heads;
   int causal;
   float scale_log2;              // log2(e) / sqrt(d_h)
+  int reverse;                   // 1: items are walked from the last request to the first
 };
 
 constexpr int kP64Lanes = 2;
@@ -88,7 +89,7 @@ __global__ void __launch_bounds__(kP64Threads, 1) attention_pair64_kernel(const 
       tma_prefetch_desc(&a.qkv_map);
       int stage = 0; uint32_t phase = 0;
       for (int idx = item0; idx < total_items; idx += item_step) {
-        const int p = idx / n_hp, h0 = (idx - p * n_hp) * 2;
+        const int p = a.reverse ? a.n_req - 1 - idx / n_hp : idx / n_hp, h0 = (idx % n_hp) * 2;
         const int r0 = a.cu_tok[p];
         const int kv0 = h0 / group, kv1 = (h0 + 1) / group;
         uint8_t *sQ = sIt + stage * kP64StageBytes, *sK = sQ + 16384, *sV = sK + 16384;
@@ -150,7 +151,7 @@ __global__ void __launch_bounds__(kP64Threads, 1) attention_pair64_kernel(const 
     const uint32_t t_s = t_row + hb * 64, t_p = t_row + 128, t_o = t_row + 192;
     uint32_t it = 0;
     for (int idx = item0; idx < total_items; idx += item_step, ++it) {
-      const int p = idx / n_hp, h0 = (idx - p * n_hp) * 2;
+      const int p = a.reverse ? a.n_req - 1 - idx / n_hp : idx / n_hp, h0 = (idx % n_hp) * 2;
       const int r0 = a.cu_tok[p], n = a.cu_tok[p + 1] - r0;
       const bool warp_valid = warp_pos_lo < n;                // else no query of this warp exists: barriers only
       uint32_t v[64];

@@ -38,6 +38,7 @@ struct AttnTcArgs {
   int n_q_heads, n_kv_heads;
   int causal;
   float scale_log2;              // log2(e) / sqrt(d_h)
+  int reverse;                   // 1: requests are walked from the last to the first (blockIdx.z reversed)
 };
 
 // Dynamic shared memory: the operand tiles (1024-byte aligned for the 128B swizzle) plus 1 KB that holds the alignment
@@ -86,7 +87,7 @@ __global__ void __launch_bounds__(128 + 128 * kQT, kMinBlocks) attention_tc_kern
   static_assert((1 + 4 * kAtStages + 4 * kQT + 1) * 8 <= 256, "barrier block");
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int p = blockIdx.z, head = blockIdx.y;
+  const int p = a.reverse ? (int)gridDim.z - 1 - (int)blockIdx.z : (int)blockIdx.z, head = blockIdx.y;
   griddep_launch();
   griddep_wait();
   const int r0 = a.cu_tok[p], n = a.cu_tok[p + 1] - r0;

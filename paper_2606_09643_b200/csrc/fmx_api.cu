@@ -274,18 +274,18 @@ void launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaSt
 }
 
 template <int kVec>
-void launch_norm(cudaStream_t s, const float *X, bf16 *Y, const bf16 *g, const bf16 *b, int N, float eps, int rms) {
-  launch_k(norm_kernel<kVec>, (N + 7) / 8, 256, 0, s, X, Y, g, b, N, eps, rms);
+void launch_norm(cudaStream_t s, const float *X, bf16 *Y, const bf16 *g, const bf16 *b, int N, float eps, int rms, int rev) {
+  launch_k(norm_kernel<kVec>, (N + 7) / 8, 256, 0, s, X, Y, g, b, N, eps, rms, rev);
 }
-bool dispatch_norm(cudaStream_t s, int d, const float *X, bf16 *Y, const bf16 *g, const bf16 *b, int N, float eps, int rms) {
+bool dispatch_norm(cudaStream_t s, int d, const float *X, bf16 *Y, const bf16 *g, const bf16 *b, int N, float eps, int rms, int rev) {
   switch (d / 128) {
-    case 1: launch_norm<1>(s, X, Y, g, b, N, eps, rms); return true;
-    case 2: launch_norm<2>(s, X, Y, g, b, N, eps, rms); return true;
-    case 4: launch_norm<4>(s, X, Y, g, b, N, eps, rms); return true;
-    case 6: launch_norm<6>(s, X, Y, g, b, N, eps, rms); return true;
-    case 8: launch_norm<8>(s, X, Y, g, b, N, eps, rms); return true;
-    case 12: launch_norm<12>(s, X, Y, g, b, N, eps, rms); return true;
-    case 16: launch_norm<16>(s, X, Y, g, b, N, eps, rms); return true;
+    case 1: launch_norm<1>(s, X, Y, g, b, N, eps, rms, rev); return true;
+    case 2: launch_norm<2>(s, X, Y, g, b, N, eps, rms, rev); return true;
+    case 4: launch_norm<4>(s, X, Y, g, b, N, eps, rms, rev); return true;
+    case 6: launch_norm<6>(s, X, Y, g, b, N, eps, rms, rev); return true;
+    case 8: launch_norm<8>(s, X, Y, g, b, N, eps, rms, rev); return true;
+    case 12: launch_norm<12>(s, X, Y, g, b, N, eps, rms, rev); return true;
+    case 16: launch_norm<16>(s, X, Y, g, b, N, eps, rms, rev); return true;
   }
   return false;
 }
@@ -331,6 +331,7 @@ void launch_pair_gemm(fmx_ctx *c, cudaStream_t s, const PairGemmParams &p) {
 }
 
 // Every request <= 64 tokens: the pipelined single-tile kernel (4 CTAs per SM, each walking a strided item list).
+int g_reverse = 1;       // consecutive kernels of a layer walk the rows in alternating directions (L2 reuse)
 int g_attn_short = 2;    // 0: generic kernel, 1: pipelined mma.sync kernel, 2: tcgen05 head-pair kernel where it applies (d_h 64, even H_q)
 bool attn_pair64_ok(int dh, int n_q_heads, int max_len) { return g_attn_short == 2 && dh == 64 && n_q_heads % 2 == 0 && max_len <= 64; }
 void launch_attention_pair64(cudaStream_t s, int sm_count, const AttnPairArgs &a) {
@@ -865,6 +866,10 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   const int Ni = (int)N;
   g_pdl_eff = g_pdl == 1 || (g_pdl == 2 && Ni <= kPdlAutoRows);
   Launcher Lh{c, s};
+  // Every kernel of the layer chain streams over all N rows and the next one reads what it wrote.  Walking the rows in
+  // alternating directions lets each kernel start on the rows its producer wrote last, which are the ones still in L2.
+  int dir = 0;
+  auto rev = [&]() { const int r = g_reverse ? dir : 0; dir ^= 1; return r; };
   // ---- S1: ids/lengths to the device, counting sort, tables ----
   cudaStreamCaptureStatus cap_status = cudaStreamCaptureStatusNone;
   if (!graph_capture) CU_OK(cudaStreamIsCapturing(s, &cap_status));
@@ -932,6 +937,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       uslot_of[tg] = p.n_tg++;
     }
     if (p.n_tg == 0) return FMX_OK;
+    p.reverse = rev();
     LAUNCH(Lh, F_SHRINK, launch_shrink(c, s, p));
     return FMX_OK;
   };
@@ -1005,7 +1011,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   const float scale_log2 = 1.4426950408889634f / sqrtf((float)d.head_dim);
   bool rope_fused = false;
   for (int l = 0; l < d.n_layers; ++l) {
-    LAUNCH(Lh, F_NORM, dispatch_norm(s, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm1_g[l], (const bf16 *)bb.norm1_b[l], Ni, d.norm_eps, rms));
+    LAUNCH(Lh, F_NORM, dispatch_norm(s, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm1_g[l], (const bf16 *)bb.norm1_b[l], Ni, d.norm_eps, rms, rev()));
     {
       const int tgs[3] = {FMX_TGT_Q, FMX_TGT_K, FMX_TGT_V};
       PairGemmParams p = base;
@@ -1022,6 +1028,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       // head_dim 128: a 128-column chunk is one head, so RoPE is applied in the GEMM epilogue (fp32, one rounding)
       rope_fused = g_rope_fused && d.rope_theta > 0 && d.head_dim == 128 && pair_wide(p);
       if (rope_fused) { p.rope_cs = bb.rope_cs; p.rope_src_mask = 3; }
+      p.reverse = rev();
       LAUNCH(Lh, F_GEMM_QKV, launch_pair_gemm(c, s, p));
     }
     if (d.rope_theta > 0 && !rope_fused) {
@@ -1033,6 +1040,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       AttnPairArgs pa2{};
       pa2.qkv_map = mQKV64; pa2.out = w.AttnO; pa2.cu_tok = w.t.cu_tok; pa2.ld_out = bb.d_q; pa2.n_req = B;
       pa2.n_q_heads = d.n_q_heads; pa2.n_kv_heads = d.n_kv_heads; pa2.causal = d.causal; pa2.scale_log2 = scale_log2;
+      pa2.reverse = rev();
       LAUNCH(Lh, F_ATTN, launch_attention_pair64(s, c->sm_count, pa2));
     } else if (attn_use_lanes(c->opt_attn_impl, d.head_dim, max_len)) {
       AttnLaneArgs la{};
@@ -1043,6 +1051,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       AttnTcArgs ta{};
       ta.qkv_map = mQKV64; ta.out = w.AttnO; ta.cu_tok = w.t.cu_tok; ta.ld_out = bb.d_q;
       ta.n_q_heads = d.n_q_heads; ta.n_kv_heads = d.n_kv_heads; ta.causal = d.causal; ta.scale_log2 = scale_log2;
+      ta.reverse = rev();
       LAUNCH(Lh, F_ATTN, launch_attention_tc(s, d.head_dim, c->opt_attn_variant, max_len, d.n_q_heads, B, ta));
     } else {
       AttnArgs aa{};
@@ -1061,9 +1070,10 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       p.wmap[0] = bb.mWo[wv(p)][l]; p.wmap_h[0] = bb.mWo[1][l]; p.bias[0] = (const bf16 *)bb.bo[l];
       set_lora(p, 0, FMX_TGT_O, l);
       p.omap = oX;
+      p.reverse = rev();
       LAUNCH(Lh, F_GEMM_O, launch_pair_gemm(c, s, p));
     }
-    LAUNCH(Lh, F_NORM, dispatch_norm(s, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm2_g[l], (const bf16 *)bb.norm2_b[l], Ni, d.norm_eps, rms));
+    LAUNCH(Lh, F_NORM, dispatch_norm(s, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm2_g[l], (const bf16 *)bb.norm2_b[l], Ni, d.norm_eps, rms, rev()));
     if (d.act == FMX_ACT_SWIGLU) {
       const int tgs[2] = {FMX_TGT_GATE, FMX_TGT_UP};
       PairGemmParams p = base;
@@ -1074,6 +1084,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       p.bias[0] = (const bf16 *)bb.bgate[l]; p.bias[1] = (const bf16 *)bb.bup[l];
       set_lora(p, 0, FMX_TGT_GATE, l); set_lora(p, 1, FMX_TGT_UP, l);
       p.omap = oHid;
+      p.reverse = rev();
       LAUNCH(Lh, F_GEMM_FFN_IN, launch_pair_gemm(c, s, p));
     } else {
       const int tgs[1] = {FMX_TGT_UP};
@@ -1084,6 +1095,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       p.wmap[0] = bb.mWup[wv(p)][l]; p.wmap_h[0] = bb.mWup[1][l]; p.bias[0] = (const bf16 *)bb.bup[l];
       set_lora(p, 0, FMX_TGT_UP, l);
       p.omap = oHid;
+      p.reverse = rev();
       LAUNCH(Lh, F_GEMM_FFN_IN, launch_pair_gemm(c, s, p));
     }
     {
@@ -1095,6 +1107,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       p.wmap[0] = bb.mWdown[wv(p)][l]; p.wmap_h[0] = bb.mWdown[1][l]; p.bias[0] = (const bf16 *)bb.bdown[l];
       set_lora(p, 0, FMX_TGT_DOWN, l);
       p.omap = oX;
+      p.reverse = rev();
       LAUNCH(Lh, F_GEMM_FFN_OUT, launch_pair_gemm(c, s, p));
     }
   }
@@ -1391,6 +1404,9 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
     case FMX_OPT_ATTN_SHORT:
       if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attn_short %d", value);
       g_attn_short = value;
+      return FMX_OK;
+    case FMX_OPT_REVERSE:
+      g_reverse = value ? 1 : 0;
       return FMX_OK;
     case FMX_OPT_GRAPH:
       c->opt_graph = value ? 1 : 0;

@@ -57,6 +57,7 @@ struct GemmParams {
   // shrink
   int n_tg;                        // targets in the input group (1..3)
   int tg_ids[3];
+  int reverse;                     // 1: units are walked from the last block to the first
 };
 
 __device__ __forceinline__ void chunk_source(const GemmParams &p, int c, int &s, int &r0) {
@@ -136,6 +137,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) shrink_kernel(const __grid_co
   const int total_units = 2 * (*p.n_blk);
   // unit -> (block, half); live = the half holds at least one row of the block's task
   auto unit_live = [&](int unit, int &blk, int &half) {
+    if (p.reverse) unit = total_units - 1 - unit;
     blk = unit >> 1; half = unit & 1;
     return max(p.blk_lo[blk], half * kBM) < min(p.blk_hi[blk], half * kBM + kBM);
   };

@@ -289,11 +289,13 @@ __global__ void pad_rows_kernel(const __nv_bfloat16 *src, __nv_bfloat16 *dst, in
 template <int kVec>   // float4s per lane: d = 128 * kVec
 __global__ void __launch_bounds__(256) norm_kernel(const float *__restrict__ X, __nv_bfloat16 *__restrict__ Y,
                                                    const __nv_bfloat16 *__restrict__ g,
-                                                   const __nv_bfloat16 *__restrict__ b, int N, float eps, int rms) {
+                                                   const __nv_bfloat16 *__restrict__ b, int N, float eps, int rms, int reverse) {
   griddep_launch();
   griddep_wait();
-  const int row = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  int row = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
   if (row >= N) return;
+  if (reverse) row = N - 1 - row;          // early CTAs take the rows the producing GEMM wrote last (still in L2)
   constexpr int d = 128 * kVec;
   const float4 *x = reinterpret_cast<const float4 *>(X + (size_t)row * d);
   float4 v[kVec];

@@ -53,6 +53,8 @@ struct PairGemmParams {
   int M, K;
   int n_chunks;            // N / 128
   int n_ptiles;            // ceil(M / 256)
+  int reverse;             // 1: row tiles are walked from the last to the first (the producer of this GEMM's input wrote
+                           // ascending: its most recent rows are the ones still in L2)
   int n_full;              // kBN = 256: tiles [0, n_full) are 256 x 256; each later tile is cut into two 256 x 128 halves
                            // taken by different pairs, so a short last wave costs half a tile time (-1 = no half tiles)
   int mode;                // GemmMode (not GM_SHRINK)
@@ -147,6 +149,7 @@ __device__ __forceinline__ void pair_decode(const PairGemmParams &p, int item, i
   }
   m_pt = tile / n_ntiles;
   const int n_tile = tile - m_pt * n_ntiles;
+  if (p.reverse) m_pt = p.n_ptiles - 1 - m_pt;
   c0 = n_tile * kCH + (h > 0 ? 1 : 0);
   nch = h >= 0 ? 1 : kCH;
 }
