@@ -222,7 +222,8 @@ enum {
                                     64 and the head count even (FMX_ATTN_AUTO only), else as 1 */
   FMX_OPT_ROPE_FUSED = 6,        /* 1 (default): head_dim 128 backbones rotate q / k in the QKV GEMM epilogue;
                                     0: separate RoPE kernel over the bf16 QKV buffer */
-  FMX_OPT_HEAD_TILED = 7,        /* 1 (default): FLATTEN heads run in the 4-request x 4-output register-tiled kernel */
+  FMX_OPT_HEAD_TILED = 7,        /* FLATTEN heads: 0 = one warp per (request, output), 1 = CUDA-core 4 x 4 register tiles,
+                                    2 (default) = mma.sync 16-request x 32-output tiles over K chunks */
   FMX_OPT_SHRINK_FUSED = 8,      /* the LoRA shrink runs as the first work items of the GEMM that consumes it: 0 = never
                                     (separate shrink kernel), 1 (default) = when the batch has at most one (tile, task)
                                     block per CTA pair, 2 = always */

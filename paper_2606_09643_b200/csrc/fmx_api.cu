@@ -117,6 +117,7 @@ struct fmx_ctx {
   // host-buffer forward staging
   void *d_in_stage = nullptr; size_t in_stage_bytes = 0;
   float *d_out_stage = nullptr; size_t out_stage_bytes = 0;
+  float *d_head_part = nullptr; size_t head_part_bytes = 0;     // K-chunk partials of the tensor-core FLATTEN head
   // last forward (debug)
   SegTables last_t{};
   int last_B = 0, last_T = 0, last_n_tiles = 0, last_launches = 0;
@@ -259,7 +260,7 @@ int g_pdl = 2, g_pdl_eff = 0;
 int g_shrink_stages = 5;
 int g_half_tiles = 1;
 int g_rope_fused = 1;
-int g_head_tiled = 1;
+int g_head_tiled = 2;     // FLATTEN heads: 0 = one warp per output, 1 = CUDA-core 4 x 4 tiles, 2 = mma.sync 16 x 32 tiles
 int g_shrink_fused = 1;   // the LoRA shrink runs as the first work items of the GEMM that consumes it (see pair_gemm.cuh)
 constexpr int kPdlAutoRows = 4096;
 template <typename... KArgs, typename... Args>
@@ -605,7 +606,7 @@ int fmx_destroy(fmx_ctx *c) {
   for (auto &t : c->tasks) { cudaFree(t.head_W); cudaFree(t.head_b); }
   cudaFree(c->d_task_coff); cudaFree(c->d_task_head_kind); cudaFree(c->d_task_head_out); cudaFree(c->d_task_trpad);
   cudaFree(c->d_task_scale); cudaFree(c->d_task_head_W); cudaFree(c->d_task_head_b);
-  cudaFree(c->d_in_stage); cudaFree(c->d_out_stage); cudaFree(c->d_dbg_cu);
+  cudaFree(c->d_in_stage); cudaFree(c->d_out_stage); cudaFree(c->d_dbg_cu); cudaFree(c->d_head_part);
   if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
   for (int i = 0; i < fmx_ctx::kStageSlots; ++i) if (c->stage_ev[i]) cudaEventDestroy(c->stage_ev[i]);
   cudaFreeHost(c->h_stage);
@@ -1122,13 +1123,40 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   ha.task_head_W = (const bf16 *const *)c->d_task_head_W; ha.task_head_b = (const bf16 *const *)c->d_task_head_b;
   ha.out = outputs; ha.d = d.d_model;
   bool any_flat = false, any_pooled = false;
+  int max_out_flat = 0;
   for (int i = 0; i < B; ++i) {
-    if (c->tasks[task_ids[i]].head_kind == FMX_HEAD_FLATTEN) any_flat = true;
+    if (c->tasks[task_ids[i]].head_kind == FMX_HEAD_FLATTEN) { any_flat = true; max_out_flat = std::max(max_out_flat, c->tasks[task_ids[i]].head_out); }
     else any_pooled = true;
   }
   ha.skip_flatten = (any_flat && g_head_tiled) ? 1 : 0;
   if (any_pooled || !ha.skip_flatten) LAUNCH(Lh, F_HEAD, (launch_k(head_kernel, dim3(B, (max_out + 7) / 8), 256, 0, s, ha)));
-  if (ha.skip_flatten) LAUNCH(Lh, F_HEAD, (launch_k(head_flatten_kernel, dim3((B + 3) / 4, (max_out + 3) / 4), 256, 0, s, ha, B)));
+  if (ha.skip_flatten) {
+    // tensor-core path: K (= tokens x d_model, the same for every FLATTEN task of a fixed-length backbone) must split into
+    // n_kc chunks x 8 warps x multiples of 32 features; the chunk-partial scratch is library-owned and grow-only
+    const long long Kf = (long long)d.tokens_per_request * d.d_model;
+    const int groups = (B + 15) / 16, ogs = (max_out_flat + 31) / 32;
+    int n_kc = 0;
+    if (g_head_tiled == 2 && d.tokens_per_request > 0)
+      for (int k = 1; k <= 8; k *= 2)
+        if (Kf % (256ll * k) == 0) { n_kc = k; if ((long long)groups * ogs * k >= c->sm_count) break; }
+    const size_t need = (size_t)groups * ogs * std::max(n_kc, 1) * 512 * sizeof(float);
+    if (n_kc > 0 && need > c->head_part_bytes) {
+      if (graph_capture) n_kc = 0;            // cannot allocate while capturing: this call takes the CUDA-core kernel
+      else {
+        CU_OK(cudaStreamSynchronize(s));
+        cudaFree(c->d_head_part);
+        c->d_head_part = nullptr; c->head_part_bytes = 0;
+        CU_OK(cudaMalloc(&c->d_head_part, align_up(need, 1 << 20)));
+        c->head_part_bytes = align_up(need, 1 << 20);
+      }
+    }
+    if (n_kc > 0) {
+      LAUNCH(Lh, F_HEAD, (launch_k(head_flatten_mma_kernel, dim3(groups, ogs, n_kc), 256, 0, s, ha, B, n_kc, c->d_head_part)));
+      LAUNCH(Lh, F_HEAD, (launch_k(head_flatten_reduce_kernel, dim3(groups, ogs), 512, 0, s, ha, B, n_kc, (const float *)c->d_head_part)));
+    } else {
+      LAUNCH(Lh, F_HEAD, (launch_k(head_flatten_kernel, dim3((B + 3) / 4, (max_out + 3) / 4), 256, 0, s, ha, B)));
+    }
+  }
 
   {
     void *bufs[7] = {w.X, w.Xn, w.QKV, w.AttnO, w.Hid, w.U, w.feat};
@@ -1416,7 +1444,8 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
       g_shrink_fused = value;
       return FMX_OK;
     case FMX_OPT_HEAD_TILED:
-      g_head_tiled = value ? 1 : 0;
+      if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: head_tiled %d", value);
+      g_head_tiled = value;
       return FMX_OK;
     case FMX_OPT_ROPE_FUSED:
       g_rope_fused = value ? 1 : 0;

@@ -588,4 +588,107 @@ __global__ void __launch_bounds__(256) head_flatten_kernel(const HeadArgs a, int
   }
 }
 
+// FLATTEN heads on the tensor cores (mma.sync m16n8k16, fp32 accumulate).  The CUDA-core kernel above moves 1.5 GB through
+// the L2 fabric for cfg2 (every CTA re-reads 4 feature rows and 4 weight rows of 128 KB each) and takes ~0.23 ms; here a
+// warp owns a 16-request x 32-output tile over a K slice, which cuts the traffic to ~0.3 GB.
+//   grid (ceil(B / 16) groups of consecutive SORTED requests, ceil(max_out / 32), n_kc K-chunks); 8 warps split the chunk.
+// The dot product does not care about the order of K, so within every 32 features thread t of a quad loads features
+// [8t, 8t+8) of its rows with ONE 16-byte load and feeds them to two MMAs as "k-slots"; A and B use the same assignment.
+// Requests of a group that belong to different FLATTEN tasks are handled in passes (task boundaries only).  Partial sums
+// of the 8 warps are added in warp order in shared memory; the n_kc chunk partials go to `part` and
+// head_flatten_reduce_kernel adds them in chunk order (deterministic), adds the bias and writes in ORIGINAL request order.
+__device__ __forceinline__ void mma_bf16_16816_h(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
+               : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+               : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+
+__global__ void __launch_bounds__(256) head_flatten_mma_kernel(const HeadArgs a, int B, int n_kc, float *__restrict__ part) {
+  __shared__ float s_part[8][16 * 32];
+  griddep_launch();
+  griddep_wait();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t4 = lane & 3;
+  const int p0 = blockIdx.x * 16, o0 = blockIdx.y * 32, kc = blockIdx.z;
+  // tasks of this thread's two rows (g, g + 8) and of all 16 rows (todo mask is CTA-uniform)
+  unsigned todo = 0;
+  for (int i = 0; i < 16; ++i) {
+    const int p = p0 + i;
+    if (p < B) {
+      const int ti = a.task_sorted[p];
+      if (a.task_head_kind[ti] == 3 && o0 < a.task_head_out[ti]) todo |= 1u << i;
+    }
+  }
+  float fin[4][4];
+#pragma unroll
+  for (int nt = 0; nt < 4; ++nt) fin[nt][0] = fin[nt][1] = fin[nt][2] = fin[nt][3] = 0.0f;
+  while (todo) {
+    const int lead = __ffs(todo) - 1;
+    const int t = a.task_sorted[p0 + lead];
+    unsigned grp = 0;
+    for (int i = 0; i < 16; ++i)
+      if (((todo >> i) & 1u) && a.task_sorted[p0 + i] == t) grp |= 1u << i;
+    todo &= ~grp;
+    const int n_out = a.task_head_out[t];
+    const long long K = (long long)(a.cu_tok[p0 + lead + 1] - a.cu_tok[p0 + lead]) * a.d;
+    const long long k_per_warp = K / (n_kc * 8);                 // host guarantees a multiple of 32
+    const long long k_lo = (long long)(kc * 8 + warp) * k_per_warp;
+    const __nv_bfloat16 *f0 = a.Fn + (size_t)a.cu_tok[p0 + (((grp >> g) & 1u) ? g : lead)] * a.d + k_lo + 8 * t4;
+    const __nv_bfloat16 *f1 = a.Fn + (size_t)a.cu_tok[p0 + (((grp >> (g + 8)) & 1u) ? g + 8 : lead)] * a.d + k_lo + 8 * t4;
+    const __nv_bfloat16 *w[4];
+#pragma unroll
+    for (int nt = 0; nt < 4; ++nt) w[nt] = a.task_head_W[t] + (size_t)min(o0 + nt * 8 + g, n_out - 1) * K + k_lo + 8 * t4;
+    float acc[4][4];
+#pragma unroll
+    for (int nt = 0; nt < 4; ++nt) acc[nt][0] = acc[nt][1] = acc[nt][2] = acc[nt][3] = 0.0f;
+#pragma unroll 2
+    for (long long k = 0; k < k_per_warp; k += 32) {
+      const uint4 A0 = *reinterpret_cast<const uint4 *>(f0 + k), A1 = *reinterpret_cast<const uint4 *>(f1 + k);
+      uint4 Wv[4];
+#pragma unroll
+      for (int nt = 0; nt < 4; ++nt) Wv[nt] = *reinterpret_cast<const uint4 *>(w[nt] + k);
+#pragma unroll
+      for (int nt = 0; nt < 4; ++nt) {
+        mma_bf16_16816_h(acc[nt], A0.x, A1.x, A0.y, A1.y, Wv[nt].x, Wv[nt].y);
+        mma_bf16_16816_h(acc[nt], A0.z, A1.z, A0.w, A1.w, Wv[nt].z, Wv[nt].w);
+      }
+    }
+    // keep the rows of this pass's task (accumulator rows g and g + 8)
+#pragma unroll
+    for (int nt = 0; nt < 4; ++nt) {
+      if ((grp >> g) & 1u) { fin[nt][0] = acc[nt][0]; fin[nt][1] = acc[nt][1]; }
+      if ((grp >> (g + 8)) & 1u) { fin[nt][2] = acc[nt][2]; fin[nt][3] = acc[nt][3]; }
+    }
+  }
+  // ---- add the 8 warps' partial tiles in warp order, one chunk partial per CTA ----
+#pragma unroll
+  for (int nt = 0; nt < 4; ++nt) {
+    const int col = nt * 8 + 2 * t4;
+    s_part[warp][g * 32 + col] = fin[nt][0]; s_part[warp][g * 32 + col + 1] = fin[nt][1];
+    s_part[warp][(g + 8) * 32 + col] = fin[nt][2]; s_part[warp][(g + 8) * 32 + col + 1] = fin[nt][3];
+  }
+  __syncthreads();
+  float *dst = part + ((size_t)(blockIdx.x * gridDim.y + blockIdx.y) * n_kc + kc) * 512;
+  for (int e = threadIdx.x; e < 512; e += 256) {
+    float v = 0.0f;
+#pragma unroll
+    for (int wq = 0; wq < 8; ++wq) v += s_part[wq][e];
+    dst[e] = v;
+  }
+}
+
+__global__ void __launch_bounds__(512) head_flatten_reduce_kernel(const HeadArgs a, int B, int n_kc, const float *__restrict__ part) {
+  griddep_launch();
+  griddep_wait();
+  const int r = threadIdx.x >> 5, o = threadIdx.x & 31;
+  const int p = blockIdx.x * 16 + r, oa = blockIdx.y * 32 + o;
+  if (p >= B) return;
+  const int t = a.task_sorted[p];
+  if (a.task_head_kind[t] != 3 || oa >= a.task_head_out[t]) return;
+  const float *src = part + (size_t)(blockIdx.x * gridDim.y + blockIdx.y) * n_kc * 512 + r * 32 + o;
+  float v = 0.0f;
+  for (int kc = 0; kc < n_kc; ++kc) v += src[(size_t)kc * 512];
+  const __nv_bfloat16 *b = a.task_head_b[t];
+  a.out[a.out_off[a.perm[p]] + oa] = v + (b ? __bfloat162float(b[oa]) : 0.0f);
+}
+
 }  // namespace fmx
