@@ -217,6 +217,18 @@ __global__ void __launch_bounds__(128 + 128 * kQT, kMinBlocks) attention_tc_kern
       const int rsw = r_in_tile & 7;
       float m_ref = 0.0f, l_run = 0.0f;
       uint32_t v[64];
+      if (warp_row_lo >= n) {
+        // No query of this warp exists (cfg3: the third q-tile of a 257-token request holds ONE row): keep the barrier
+        // protocol going and leave the exp2 / issue slots to the warps (and the co-resident CTA) that have rows.
+        for (int j = 0; j < n_tiles; ++j) {
+          mbar_wait(&s_full[q], j & 1);
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&s_free[q]);
+          if (j > 0) mbar_wait(&pv_done[q], (j - 1) & 1);            // p_ready phase j-1 is complete: no arrival can land in it
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&p_ready[q]);
+        }
+      } else {
       for (int j = 0; j < n_tiles; ++j) {
         mbar_wait(&s_full[q], j & 1);
         tc_fence_after();
@@ -304,6 +316,7 @@ __global__ void __launch_bounds__(128 + 128 * kQT, kMinBlocks) attention_tc_kern
                            pack_bf16(__uint_as_float(o[8 * e + 6]) * inv, __uint_as_float(o[8 * e + 7]) * inv));
         }
       }
+      }   // warp with rows
     }
   }
 
