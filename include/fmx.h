@@ -215,7 +215,8 @@ enum {
   FMX_OPT_ATTENTION_IMPL = 0,    /* FMX_ATTN_AUTO | FMX_ATTN_MMA_SYNC | FMX_ATTN_TCGEN05 | FMX_ATTN_LANES */
   FMX_OPT_ATTENTION_VARIANT = 1, /* tcgen05 attention: 0 = one 128-query tile per CTA; 1 = two q-tiles per CTA
                                     sharing K/V.  FMX_ATTN_LANES: 0 / 1 / 2 = 4 / 2 / 3 lanes per CTA (head_dim 64) */
-  FMX_OPT_SHRINK_STAGES = 3,     /* shared-memory pipeline depth of the LoRA shrink kernel: 4 or 5 (default) */
+  FMX_OPT_SHRINK_STAGES = 3,     /* LoRA shrink kernel pipeline: 5 (default) = as deep as ~200 KB allow for the stage size
+                                    (8 / 6 / 5 stages for 1 / 2 / 3 targets), 4 = four 40 KB stages */
   FMX_OPT_HALF_TILES = 4,        /* 1 (default): a short last GEMM wave is cut into 256 x 128 half tiles */
   FMX_OPT_ATTN_SHORT = 5,        /* batches whose requests all have <= 64 tokens: 0 = generic kernels, 1 = pipelined
                                     single-tile mma.sync kernel, 2 (default) = tcgen05 head-pair kernel when head_dim is

@@ -308,8 +308,10 @@ bool norm_dim_supported(int d) {
 }
 
 void launch_shrink(fmx_ctx *c, cudaStream_t s, const GemmParams &p) {
-  if (g_shrink_stages == 5) launch_k(shrink_kernel<5>, c->sm_count, kGemmThreads, shrink_smem_bytes<5>(), s, p);
-  else launch_k(shrink_kernel<4>, c->sm_count, kGemmThreads, shrink_smem_bytes<4>(), s, p);
+  if (g_shrink_stages == 4) launch_k((shrink_kernel<4, 3>), c->sm_count, kGemmThreads, (shrink_smem_bytes<4, 3>()), s, p);
+  else if (p.n_tg == 1) launch_k((shrink_kernel<8, 1>), c->sm_count, kGemmThreads, (shrink_smem_bytes<8, 1>()), s, p);
+  else if (p.n_tg == 2) launch_k((shrink_kernel<6, 2>), c->sm_count, kGemmThreads, (shrink_smem_bytes<6, 2>()), s, p);
+  else launch_k((shrink_kernel<5, 3>), c->sm_count, kGemmThreads, (shrink_smem_bytes<5, 3>()), s, p);
 }
 
 // Pair tiles 256 x 256 when the chunk count is even, else 256 x 128; one cluster of 2 CTAs per SM pair.
@@ -427,8 +429,10 @@ int set_kernel_attrs() {
   CU_OK((cudaFuncSetAttribute(attention_lanes_kernel<128, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_lanes_smem_bytes<128, 2>())));
   CU_OK(cudaFuncSetAttribute(pair_gemm_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<256>()));
   CU_OK(cudaFuncSetAttribute(pair_gemm_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<128>()));
-  CU_OK(cudaFuncSetAttribute(shrink_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<4>()));
-  CU_OK(cudaFuncSetAttribute(shrink_kernel<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<5>()));
+  CU_OK((cudaFuncSetAttribute(shrink_kernel<4, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<4, 3>())));
+  CU_OK((cudaFuncSetAttribute(shrink_kernel<5, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<5, 3>())));
+  CU_OK((cudaFuncSetAttribute(shrink_kernel<6, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<6, 2>())));
+  CU_OK((cudaFuncSetAttribute(shrink_kernel<8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<8, 1>())));
   CU_OK(cudaFuncSetAttribute(attention_pair64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_pair64_smem_bytes()));
   CU_OK(cudaFuncSetAttribute(attention_short_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_short_smem_bytes<32>()));
   CU_OK(cudaFuncSetAttribute(attention_short_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_short_smem_bytes<64>()));
@@ -1426,7 +1430,7 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
       c->opt_attn_impl = value;
       return FMX_OK;
     case FMX_OPT_SHRINK_STAGES:
-      if (value != 4 && value != 5) return fmx_fail(FMX_E_INVALID_ARG, "set_option: shrink stages %d", value);
+      if (value != 4 && value != 5) return fmx_fail(FMX_E_INVALID_ARG, "set_option: shrink stages %d", value);   // 5 = as deep as the stage size allows
       g_shrink_stages = value;
       return FMX_OK;
     case FMX_OPT_ATTN_SHORT:

@@ -107,9 +107,11 @@ __device__ __forceinline__ float silu_f(float x) {
 // targets that read the same input share one pass (N = 64 columns per target).  Single-CTA tcgen05:
 // M = 128, N = n_tg * 64, TMEM accumulator double-buffered; halves with no row of the task skip the
 // loads and MMAs and only write zeros.
-template <int kStages>
+// kTgCap: targets the stage has room for (1..3); the shared-memory ring is as deep as ~200 KB allow for that stage size,
+// because the kernel is bound by bytes in flight per SM: 8 / 6 / 5 stages for 1 / 2 / 3 targets.
+template <int kStages, int kTgCap>
 __global__ void __launch_bounds__(kGemmThreads, 1) shrink_kernel(const __grid_constant__ GemmParams p) {
-  constexpr int kBStageBytes = 3 * 64 * kBK * 2;
+  constexpr int kBStageBytes = kTgCap * 64 * kBK * 2;
   constexpr int kStageBytes = kATileBytes + kBStageBytes;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -241,7 +243,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) shrink_kernel(const __grid_co
   if (warp == 2) tmem_dealloc(tmem_base, 512);
 }
 
-template <int kStages>
-constexpr int shrink_smem_bytes() { return kStages * (kATileBytes + 3 * 64 * kBK * 2) + 1024; }
+template <int kStages, int kTgCap>
+constexpr int shrink_smem_bytes() { return kStages * (kATileBytes + kTgCap * 64 * kBK * 2) + 1024; }
 
 }  // namespace fmx

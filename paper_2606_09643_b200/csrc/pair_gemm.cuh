@@ -257,7 +257,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
               if (p.task_trpad[t * 7 + tg] == 0) continue;
               if (!u_ready) {                               // U is written by the fused-shrink items of all pairs: wait once
                 const unsigned target = 16u * (unsigned)n_u * p.u_epoch;
+                const long long t_wait0 = clock64();
                 while (ld_acquire_gpu(p.u_flag) < target) {
+                  // the shrink items are the FIRST items of every resident pair, so this wait is short; a bound of ~2 s
+                  // of SM clocks turns a scheduling assumption that does not hold into an error instead of a hang
+                  if (clock64() - t_wait0 > (1ll << 32)) __trap();
                 }
                 fence_proxy_async_global();
                 u_ready = true;
