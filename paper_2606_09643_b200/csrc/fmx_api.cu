@@ -259,6 +259,7 @@ struct Launcher {
 int g_pdl = 2, g_pdl_eff = 0;
 int g_shrink_stages = 5;
 int g_half_tiles = 1;
+int g_expand_wide = 1;
 int g_rope_fused = 1;
 int g_head_tiled = 2;     // FLATTEN heads: 0 = one warp per output, 1 = CUDA-core 4 x 4 tiles, 2 = mma.sync 16 x 32 tiles
 int g_shrink_fused = 1;   // the LoRA shrink runs as the first work items of the GEMM that consumes it (see pair_gemm.cuh)
@@ -323,6 +324,7 @@ void launch_pair_gemm(fmx_ctx *c, cudaStream_t s, const PairGemmParams &p) {
     // Wave quantisation: when the last wave would hold at most half as many tiles as there are pairs, its tiles are cut
     // into 256 x 128 halves so that it lasts half a tile time (cfg2 O / FFN-out: 256 tiles on 74 pairs, 4 -> 3.5 waves).
     PairGemmParams q = p;
+    q.expand_wide = g_expand_wide;
     const int rem = tiles % pairs;
     q.n_full = (g_half_tiles && p.mode != GM_OUT_BF16_SWIGLU && !p.rope_cs && tiles > pairs && rem > 0 && 2 * rem <= pairs) ? tiles - rem : -1;
     const int items = q.n_full >= 0 ? q.n_full + 2 * rem : tiles;
@@ -1436,6 +1438,9 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
     case FMX_OPT_ATTN_SHORT:
       if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attn_short %d", value);
       g_attn_short = value;
+      return FMX_OK;
+    case FMX_OPT_EXPAND_WIDE:
+      g_expand_wide = value ? 1 : 0;
       return FMX_OK;
     case FMX_OPT_REVERSE:
       g_reverse = value ? 1 : 0;

@@ -53,6 +53,7 @@ struct PairGemmParams {
   int M, K;
   int n_chunks;            // N / 128
   int n_ptiles;            // ceil(M / 256)
+  int expand_wide;         // 1: same-source whole tiles run their LoRA expand as one N = 256 step per block (A/B knob)
   int reverse;             // 1: row tiles are walked from the last to the first (the producer of this GEMM's input wrote
                            // ascending: its most recent rows are the ones still in L2)
   int n_full;              // kBN = 256: tiles [0, n_full) are 256 x 256; each later tile is cut into two 256 x 128 halves
@@ -154,6 +155,16 @@ __device__ __forceinline__ void pair_decode(const PairGemmParams &p, int item, i
   nch = h >= 0 ? 1 : kCH;
 }
 
+// A whole 256-wide tile whose two chunks come from the same weight source: its LoRA expand runs as ONE N = 256 step per block.
+template <int kBN>
+__device__ __forceinline__ bool pair_expand_wide(const PairGemmParams &p, int c0, int nch) {
+  if (kBN != 256 || nch != 2 || !p.expand_wide) return false;
+  int s0, r0, s1, r1;
+  pair_chunk_source(p, c0, s0, r0);
+  pair_chunk_source(p, c0 + 1, s1, r1);
+  return s0 == s1;
+}
+
 template <int kBN>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pair_gemm_kernel(const __grid_constant__ PairGemmParams p) {
   constexpr int kCH = kBN / kChunk;
@@ -247,7 +258,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
         }
         if (p.has_lora) {
           const int b0 = p.tile_blk_off[m_pt], b1 = p.tile_blk_off[m_pt + 1];
-          for (int c = 0; c < nch; ++c) {
+          // Both chunks of a whole tile from the same source (q | k | v, o, up, down; not SwiGLU's gate / up pairs) read the
+          // SAME U columns: one expand step then covers the tile (U loaded once, each CTA its chunk's 128 slab rows, N = 256).
+          const bool wide = pair_expand_wide<kBN>(p, c0, nch);
+          int rr_wide = 0;
+          if (wide) { int sr; pair_chunk_source(p, c0 + (int)rank, sr, rr_wide); }
+          for (int c = 0; c < (wide ? 1 : nch); ++c) {
             int s, r0;
             pair_chunk_source(p, c0 + c, s, r0);
             const int tg = p.lora_tgt[s];
@@ -269,9 +285,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
               mbar_wait(&empty_bar[stage], phase ^ 1);
               uint8_t *sa = smem + stage * kStageBytes, *sb = sa + kATileBytes;
               const uint32_t fb = mapa_shared(smem_u32(&full_bar[stage]), 0);
-              mbar_arrive_expect_tx_cluster(fb, kExpandBytes);
+              mbar_arrive_expect_tx_cluster(fb, wide ? kExpandBytes + 64 * kBK * 2 : kExpandBytes);
               tma_load_2d_2sm(sa, &p.umap, fb, p.uslot[s] * 64, b * kPairRows + (int)rank * kBM);
-              tma_load_2d_2sm(sb, &p.lmap[s], fb, p.task_coff[t], r0 + (int)rank * 64);
+              if (wide) {
+                tma_load_2d_2sm(sb, &p.lmap[s], fb, p.task_coff[t], rr_wide);
+                tma_load_2d_2sm(sb + 64 * kBK * 2, &p.lmap[s], fb, p.task_coff[t], rr_wide + 64);
+              } else {
+                tma_load_2d_2sm(sb, &p.lmap[s], fb, p.task_coff[t], r0 + (int)rank * 64);
+              }
               if (++stage == kStages) { stage = 0; phase ^= 1; }
             }
           }
@@ -305,7 +326,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
         }
         if (p.has_lora && !u_item) {
           const int b0 = p.tile_blk_off[m_pt], b1 = p.tile_blk_off[m_pt + 1];
-          for (int c = 0; c < nch; ++c) {
+          const bool wide = pair_expand_wide<kBN>(p, c0, nch);
+          for (int c = 0; c < (wide ? 1 : nch); ++c) {
             int s, r0;
             pair_chunk_source(p, c0 + c, s, r0);
             const int tg = p.lora_tgt[s];
@@ -318,7 +340,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
               const uint32_t sa = smem_u32(smem + stage * kStageBytes);
               const uint64_t adesc = make_smem_desc_sw128(sa), bdesc = make_smem_desc_sw128(sa + kATileBytes);
               for (int k = 0; k < ksteps; ++k)
-                umma_bf16_2sm(d_tmem + c * kChunk, adesc + 2 * k, bdesc + 2 * k, idesc_lora, 1);
+                umma_bf16_2sm(d_tmem + c * kChunk, adesc + 2 * k, bdesc + 2 * k, wide ? idesc_whole : idesc_lora, 1);
               umma_commit_2sm(&empty_bar[stage], 3);
               if (++stage == kStages) { stage = 0; phase ^= 1; }
             }
