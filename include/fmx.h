@@ -235,6 +235,8 @@ enum {
                                     directions, so each starts on the rows its producer wrote last (still in L2) */
   FMX_OPT_EXPAND_WIDE = 11,      /* 1 (default): a 256-wide tile whose two chunks share a weight source runs its LoRA
                                     expand as one N = 256 step per block (U loaded once) instead of two N = 128 steps */
+  FMX_OPT_DEEP_PIPE = 12,        /* 1 (default): fp32-output GEMMs (residual, embed) run with one more smem pipeline stage
+                                    and a single epilogue staging buffer per warpgroup */
   FMX_OPT_PDL = 2                /* programmatic dependent launch of the forward's kernels (process-wide):
                                     0 = off, 1 = always, 2 (default) = only for batches of <= 4096 token rows */
 };

@@ -259,6 +259,7 @@ struct Launcher {
 int g_pdl = 2, g_pdl_eff = 0;
 int g_shrink_stages = 5;
 int g_half_tiles = 1;
+int g_deep_pipe = 1;
 int g_expand_wide = 1;
 int g_rope_fused = 1;
 int g_head_tiled = 2;     // FLATTEN heads: 0 = one warp per output, 1 = CUDA-core 4 x 4 tiles, 2 = mma.sync 16 x 32 tiles
@@ -319,6 +320,8 @@ void launch_shrink(fmx_ctx *c, cudaStream_t s, const GemmParams &p) {
 bool pair_wide(const PairGemmParams &p) { return p.n_chunks % 2 == 0; }
 void launch_pair_gemm(fmx_ctx *c, cudaStream_t s, const PairGemmParams &p) {
   const int pairs = c->sm_count / 2;
+  // fp32-output modes (residual reduce-add, embed) take the deep variant: one more pipeline stage, one staging buffer
+  const bool deep = g_deep_pipe && (p.mode == GM_RESID_F32 || p.mode == GM_EMBED_F32 || p.mode == GM_OUT_F32);
   if (pair_wide(p)) {
     const int tiles = p.n_ptiles * (p.n_chunks / 2);
     // Wave quantisation: when the last wave would hold at most half as many tiles as there are pairs, its tiles are cut
@@ -328,10 +331,14 @@ void launch_pair_gemm(fmx_ctx *c, cudaStream_t s, const PairGemmParams &p) {
     const int rem = tiles % pairs;
     q.n_full = (g_half_tiles && p.mode != GM_OUT_BF16_SWIGLU && !p.rope_cs && tiles > pairs && rem > 0 && 2 * rem <= pairs) ? tiles - rem : -1;
     const int items = q.n_full >= 0 ? q.n_full + 2 * rem : tiles;
-    launch_k(pair_gemm_kernel<256>, 2 * (p.n_sh > 0 ? pairs : std::min(items, pairs)), kGemmThreads, pair_smem_bytes<256>(), s, q);
+    const int grid = 2 * (p.n_sh > 0 ? pairs : std::min(items, pairs));
+    if (deep) launch_k((pair_gemm_kernel<256, true>), grid, kGemmThreads, (pair_smem_bytes<256, true>()), s, q);
+    else launch_k((pair_gemm_kernel<256, false>), grid, kGemmThreads, (pair_smem_bytes<256, false>()), s, q);
   } else {
     const int tiles = p.n_ptiles * p.n_chunks;
-    launch_k(pair_gemm_kernel<128>, 2 * (p.n_sh > 0 ? pairs : std::min(tiles, pairs)), kGemmThreads, pair_smem_bytes<128>(), s, p);
+    const int grid = 2 * (p.n_sh > 0 ? pairs : std::min(tiles, pairs));
+    if (deep) launch_k((pair_gemm_kernel<128, true>), grid, kGemmThreads, (pair_smem_bytes<128, true>()), s, p);
+    else launch_k((pair_gemm_kernel<128, false>), grid, kGemmThreads, (pair_smem_bytes<128, false>()), s, p);
   }
 }
 
@@ -429,8 +436,10 @@ int set_kernel_attrs() {
   CU_OK((cudaFuncSetAttribute(attention_lanes_kernel<64, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_lanes_smem_bytes<64, 2>())));
   CU_OK((cudaFuncSetAttribute(attention_lanes_kernel<64, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_lanes_smem_bytes<64, 3>())));
   CU_OK((cudaFuncSetAttribute(attention_lanes_kernel<128, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_lanes_smem_bytes<128, 2>())));
-  CU_OK(cudaFuncSetAttribute(pair_gemm_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<256>()));
-  CU_OK(cudaFuncSetAttribute(pair_gemm_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<128>()));
+  CU_OK((cudaFuncSetAttribute(pair_gemm_kernel<256, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<256, false>())));
+  CU_OK((cudaFuncSetAttribute(pair_gemm_kernel<256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<256, true>())));
+  CU_OK((cudaFuncSetAttribute(pair_gemm_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<128, false>())));
+  CU_OK((cudaFuncSetAttribute(pair_gemm_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<128, true>())));
   CU_OK((cudaFuncSetAttribute(shrink_kernel<4, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<4, 3>())));
   CU_OK((cudaFuncSetAttribute(shrink_kernel<5, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<5, 3>())));
   CU_OK((cudaFuncSetAttribute(shrink_kernel<6, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<6, 2>())));
@@ -572,7 +581,8 @@ int fmx_create(fmx_ctx **out, int device_ordinal) {
       if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess) { cudaGetLastError(); n = 0; }
       return n;
     };
-    const int n256 = max_clusters(pair_gemm_kernel<256>, pair_smem_bytes<256>()), n128 = max_clusters(pair_gemm_kernel<128>, pair_smem_bytes<128>());
+    const int n256 = std::min(max_clusters(pair_gemm_kernel<256, false>, pair_smem_bytes<256, false>()), max_clusters(pair_gemm_kernel<256, true>, pair_smem_bytes<256, true>()));
+    const int n128 = std::min(max_clusters(pair_gemm_kernel<128, false>, pair_smem_bytes<128, false>()), max_clusters(pair_gemm_kernel<128, true>, pair_smem_bytes<128, true>()));
     c->pairs_resident = n256 >= c->sm_count / 2 && n128 >= c->sm_count / 2;
     if (getenv("FMX_DEBUG")) fprintf(stderr, "fmx: max active pair-GEMM clusters %d / %d (need %d): fused shrink %s\n", n256, n128, c->sm_count / 2, c->pairs_resident ? "on" : "off");
   }
@@ -1438,6 +1448,9 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
     case FMX_OPT_ATTN_SHORT:
       if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attn_short %d", value);
       g_attn_short = value;
+      return FMX_OK;
+    case FMX_OPT_DEEP_PIPE:
+      g_deep_pipe = value ? 1 : 0;
       return FMX_OK;
     case FMX_OPT_EXPAND_WIDE:
       g_expand_wide = value ? 1 : 0;

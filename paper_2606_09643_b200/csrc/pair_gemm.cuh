@@ -41,7 +41,11 @@
 namespace fmx {
 
 constexpr int kPairRows = 256;                    // rows of a pair tile (2 x 128)
-constexpr int kStagingBytes = 2 * 2 * 16384;      // 2 warpgroups x 2 buffers x 16 KB
+// Epilogue staging: 2 warpgroups x kBufs buffers x 16 KB.  kDeep = false: two buffers per warpgroup (the bf16 / SwiGLU / RoPE
+// epilogues overlap a box's TMA store with the next box's conversion); kDeep = true: ONE buffer and one more pipeline stage
+// instead, which is what the fp32-residual GEMMs want (short K, mainloop-latency-bound: cfg2 O projection 1.41 -> 1.31 ms).
+template <bool kDeep>
+__host__ __device__ constexpr int pair_staging_bytes() { return 2 * (kDeep ? 1 : 2) * 16384; }
 
 struct PairGemmParams {
   CUtensorMap amap;        // A [M, K] bf16, box {64, 128}
@@ -101,10 +105,10 @@ __device__ __forceinline__ void pair_chunk_source(const PairGemmParams &p, int c
 
 template <int kBN>
 __host__ __device__ constexpr int pair_stage_bytes() { return kATileBytes + (kBN / 2) * kBK * 2; }
-template <int kBN>
-__host__ __device__ constexpr int pair_stages() { return kBN == 256 ? 5 : 6; }
-template <int kBN>
-constexpr int pair_smem_bytes() { return pair_stages<kBN>() * pair_stage_bytes<kBN>() + kStagingBytes + 1024; }
+template <int kBN, bool kDeep>
+__host__ __device__ constexpr int pair_stages() { return (kBN == 256 ? 5 : 6) + (kDeep ? 1 : 0); }
+template <int kBN, bool kDeep>
+constexpr int pair_smem_bytes() { return pair_stages<kBN, kDeep>() * pair_stage_bytes<kBN>() + pair_staging_bytes<kDeep>() + 1024; }
 
 // 32 fp32 accumulator columns (+ bias, activation) -> 4 swizzled 16-byte chunks of bf16 in the staging row.
 __device__ __forceinline__ void stage_bf16_32(const uint32_t (&v)[32], const __nv_bfloat16 *bias, int mode, uint8_t *row_base,
@@ -165,10 +169,11 @@ __device__ __forceinline__ bool pair_expand_wide(const PairGemmParams &p, int c0
   return s0 == s1;
 }
 
-template <int kBN>
+template <int kBN, bool kDeep>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pair_gemm_kernel(const __grid_constant__ PairGemmParams p) {
   constexpr int kCH = kBN / kChunk;
-  constexpr int kStages = pair_stages<kBN>();
+  constexpr int kStages = pair_stages<kBN, kDeep>();
+  constexpr int kBufs = kDeep ? 1 : 2;                    // staging buffers per epilogue warpgroup
   constexpr int kStageBytes = pair_stage_bytes<kBN>();
   constexpr int kBHalf = kBN / 2;                          // W rows per CTA per stage
   constexpr int kExpandBytes = kATileBytes + 64 * kBK * 2; // U half tile + 64 slab rows
@@ -357,7 +362,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
     const int rsw = r_in_tile & 7;
     const bool issuer = (threadIdx.x == 128 + wg * 128);
     const uint32_t bar_id = 1 + wg;
-    uint8_t *stg = staging + wg * 32768;
+    uint8_t *stg = staging + wg * (kBufs * 16384);
     int box_seq = 0;
     int acc = 0; uint32_t accphase = 0;
     const int mode = p.mode;
@@ -410,8 +415,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
         // tile = [gate chunk | up chunk] of the same 128 output features; this warpgroup: 64 of them
         const int r0 = (c0 >> 1) * kChunk;                      // feature offset of the tile (never a half tile)
         const int fcol = wg * 64;
-        uint8_t *buf = stg + (box_seq & 1) * 16384;
-        if (issuer) bulk_wait_read<1>();
+        uint8_t *buf = stg + (box_seq & (kBufs - 1)) * 16384;
+        if (issuer) bulk_wait_read<kBufs - 1>();
         named_bar_sync(bar_id, 128);
         uint8_t *row_base = buf + r_in_tile * 128;
 #pragma unroll 1
@@ -448,7 +453,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
         const int kBoxes = bn / 128;                            // 64-column boxes per warpgroup
         int s_wg, r0_wg;
         pair_chunk_source(p, c0 + (bn == 256 ? wg : 0), s_wg, r0_wg);
-        if (p.rope_cs && bn == 256 && ((p.rope_src_mask >> s_wg) & 1)) {
+        if (!kDeep && p.rope_cs && bn == 256 && ((p.rope_src_mask >> s_wg) & 1)) {   // needs both staging buffers
           // Fused RoPE (rotate-half): this warpgroup's 128 columns are one head; dims j and j + 64 of the thread's row
           // are rotated in fp32 straight from the accumulator (one rounding) and leave as two 64-column boxes.
           const int n_out = (c0 + wg) * kChunk;
@@ -506,8 +511,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
           pair_chunk_source(p, c0 + col / kChunk, s, r0);
           const int n_src = r0 + (col % kChunk);
           const int n_out = c0 * kChunk + col;
-          uint8_t *buf = stg + (box_seq & 1) * 16384;
-          if (issuer) bulk_wait_read<1>();
+          uint8_t *buf = stg + (box_seq & (kBufs - 1)) * 16384;
+          if (issuer) bulk_wait_read<kBufs - 1>();
           named_bar_sync(bar_id, 128);
           tmem_ld_32x32(t_row + col, v);
           tmem_ld_32x32(t_row + col + 32, u);
@@ -538,8 +543,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
           pair_chunk_source(p, c0 + col / kChunk, s, r0);
           const int n_src = r0 + (col % kChunk);
           const int n_out = c0 * kChunk + col;
-          uint8_t *buf = stg + (box_seq & 1) * 16384;
-          if (issuer) bulk_wait_read<1>();
+          uint8_t *buf = stg + (box_seq & (kBufs - 1)) * 16384;
+          if (issuer) bulk_wait_read<kBufs - 1>();
           named_bar_sync(bar_id, 128);
           tmem_ld_32x32(t_row + col, v);
           tmem_ld_wait();

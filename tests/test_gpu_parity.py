@@ -144,7 +144,7 @@ def test_every_kernel_option_gives_the_oracle_result(fmx_mod, cfg, kw):
         for a, b in zip(outs[0], outs[2]):
             assert np.array_equal(a, b), "fused and separate LoRA shrink must be bit-identical"
         s.fmx.set_option("shrink_fused", 1)
-        for opt, val, restore in (("half_tiles", 0, 1), ("rope_fused", 0, 1), ("head_tiled", 0, 2), ("head_tiled", 1, 2), ("reverse", 0, 1), ("expand_wide", 0, 1), ("pdl", 1, 2), ("pdl", 0, 2)):
+        for opt, val, restore in (("half_tiles", 0, 1), ("rope_fused", 0, 1), ("head_tiled", 0, 2), ("head_tiled", 1, 2), ("reverse", 0, 1), ("expand_wide", 0, 1), ("deep_pipe", 0, 1), ("pdl", 1, 2), ("pdl", 0, 2)):
             s.fmx.set_option(opt, val)
             try:
                 check_parity(s.forward_numpy(), ref, f"{cfg} {opt}={val}")
