@@ -27,8 +27,15 @@ float64 arrays (the bf16-rounded values the GPU receives, widened).  Tensor name
 Pins (tests/test_oracle_pins.py): brute-force matmul on tiny shapes; closed forms for the
 norms, softmax, GeLU/SiLU, RoPE; the LoRA merge identity W' = W + s·B·A; zero adapter ==
 backbone-only; pooling/flatten special cases; a hand-expanded 1-layer, 2-token, d=2 example.
-End-to-end outputs have no value printed in the paper: beyond those pins, end-to-end
-parity is unpinned.
+Library pins (tests/test_oracle_library_pins.py, independent PyTorch / Hugging Face code in fp64):
+`attention` vs torch SDPA (causal / full, GQA); the norms and activations vs torch.nn.functional;
+`layer_forward` of both encoder families vs torch.nn.TransformerEncoderLayer(norm_first=True);
+the decoder backbone (RMSNorm, rotate-half RoPE, GQA, causal, SwiGLU) with LoRA on all seven
+targets vs transformers' LlamaModel carrying the merged weights W + (alpha/r) B A.
+The paper prints no value of any forward output, so no pin comes from the paper itself; what
+stays without a library counterpart is only the pooled / flattened head (a mean, a row pick or
+a reshape, then one matrix-vector product), pinned by its special cases; the
+image patch embedding is pinned against torch.nn.Conv2d.
 """
 import math
 

@@ -1,0 +1,199 @@
+"""Pins of the oracle against INDEPENDENT library implementations of the same textbook models (fp64, CPU):
+
+* `attention`              vs torch.nn.functional.scaled_dot_product_attention (causal / full, GQA by repeating KV heads)
+* `layer_norm`, `rms_norm`,
+  `gelu_erf`, `silu`        vs torch.nn.functional
+* `layer_forward` of both encoder families (pre-LN + GeLU + biases: cfg1 / cfg3; RMSNorm + ReLU, no biases: cfg2 / cfg5)
+                            vs torch.nn.TransformerEncoderLayer(norm_first=True) carrying the same weights
+* the whole backbone of the decoder family (RMSNorm, rotate-half RoPE, GQA, causal, SwiGLU: cfg4) WITH per-task LoRA
+                            vs transformers' LlamaModel carrying the merged weights W + (alpha/r) B A
+
+The oracle is numpy, these are PyTorch / Hugging Face code written by other people: a wrong sign in RoPE, a transposed
+operand, a head-grouping mistake, a mis-placed adapter or norm fails here.  None of this touches the CUDA path.
+"""
+import math
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+F = torch.nn.functional
+
+from oracle import vfm_forward as O  # noqa: E402
+
+T64 = dict(dtype=torch.float64)
+
+
+def _rng(seed):
+    return np.random.default_rng(seed)
+
+
+def _t(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).to(torch.float64)
+
+
+# ---------------------------------------------------------------- elementary pieces
+@pytest.mark.parametrize("causal", [0, 1])
+@pytest.mark.parametrize("hq,hkv,dh,n", [(4, 4, 8, 13), (6, 2, 16, 37), (8, 1, 4, 5), (3, 3, 32, 1)])
+def test_attention_matches_torch_sdpa(hq, hkv, dh, n, causal):
+    r = _rng(hq * 100 + n)
+    q, k, v = r.standard_normal((n, hq * dh)), r.standard_normal((n, hkv * dh)), r.standard_normal((n, hkv * dh))
+    got = O.attention(q, k, v, hq, hkv, dh, bool(causal))
+    tq = _t(q).view(n, hq, dh).transpose(0, 1)                                   # [H, n, dh]
+    tk = _t(k).view(n, hkv, dh).transpose(0, 1).repeat_interleave(hq // hkv, dim=0)
+    tv = _t(v).view(n, hkv, dh).transpose(0, 1).repeat_interleave(hq // hkv, dim=0)
+    ref = F.scaled_dot_product_attention(tq[None], tk[None], tv[None], is_causal=bool(causal))[0]
+    ref = ref.transpose(0, 1).reshape(n, hq * dh).numpy()
+    assert np.allclose(got, ref, rtol=1e-11, atol=1e-12)
+
+
+def test_norms_and_activations_match_torch():
+    r = _rng(7)
+    x, g, b = r.standard_normal((9, 24)) * 3, r.standard_normal(24), r.standard_normal(24)
+    assert np.allclose(O.layer_norm(x, g, b, 1e-5), F.layer_norm(_t(x), (24,), _t(g), _t(b), 1e-5).numpy(), rtol=1e-12, atol=1e-13)
+    if hasattr(F, "rms_norm"):
+        assert np.allclose(O.rms_norm(x, g, 1e-6), F.rms_norm(_t(x), (24,), _t(g), 1e-6).numpy(), rtol=1e-12, atol=1e-13)
+    y = np.linspace(-9, 9, 1001)
+    assert np.allclose(O.gelu_erf(y), F.gelu(_t(y), approximate="none").numpy(), rtol=1e-12, atol=1e-14)
+    assert np.allclose(O.silu(y), F.silu(_t(y)).numpy(), rtol=1e-12, atol=1e-14)
+    assert np.allclose(O.relu(y), F.relu(_t(y)).numpy())
+
+
+# ---------------------------------------------------------------- encoder families vs nn.TransformerEncoderLayer
+@pytest.mark.parametrize("norm,act,has_bias", [("ln", "gelu", True),      # cfg1 / cfg3: pre-LayerNorm, exact GeLU, biases
+                                               ("rms", "relu", False)])   # cfg2 / cfg5: RMSNorm, ReLU, no biases
+def test_pre_norm_layers_match_torch_transformer_encoder_layer(norm, act, has_bias):
+    if norm == "rms" and not hasattr(torch.nn, "RMSNorm"):
+        pytest.skip("torch.nn.RMSNorm not available")
+    d, H, Fd, n, L = 32, 4, 80, 19, 2
+    eps = 1e-5 if norm == "ln" else 1e-6
+    r = _rng(2026)
+    W = {}
+    for l in range(L):
+        p = f"L{l:02d}."
+        for nm, shape in (("Wq", (d, d)), ("Wk", (d, d)), ("Wv", (d, d)), ("Wo", (d, d)), ("Wup", (Fd, d)), ("Wdown", (d, Fd))):
+            W[p + nm] = r.standard_normal(shape) * 0.2
+        for nm, m in (("bq", d), ("bk", d), ("bv", d), ("bo", d), ("bup", Fd), ("bdown", d)):
+            W[p + nm] = r.standard_normal(m) * 0.1
+        for nm in ("norm1", "norm2"):
+            W[p + nm + ".g"] = 1 + 0.1 * r.standard_normal(d)
+            W[p + nm + ".b"] = 0.1 * r.standard_normal(d)
+    bb = dict(n_layers=L, d_model=d, n_q_heads=H, n_kv_heads=H, head_dim=d // H, d_ffn=Fd, act=act, norm=norm, norm_eps=eps,
+              causal=False, rope_theta=0.0, input_kind="embedded", patch_dim=0, has_cls=False, has_bias=has_bias, has_pos=False,
+              img_c=0, img_hw=0, patch_hw=0)
+    x = r.standard_normal((n, d))
+    h = x
+    for l in range(L):
+        h = O.layer_forward(bb, W.__getitem__, None, l, h)
+
+    act_fn = (lambda z: F.gelu(z, approximate="none")) if act == "gelu" else F.relu
+    ht = _t(x)[None]
+    for l in range(L):
+        p = f"L{l:02d}."
+        layer = torch.nn.TransformerEncoderLayer(d, H, Fd, dropout=0.0, activation=act_fn, layer_norm_eps=eps, batch_first=True,
+                                                 norm_first=True, bias=has_bias, **T64)
+        if norm == "rms":
+            layer.norm1 = torch.nn.RMSNorm(d, eps=eps, **T64)
+            layer.norm2 = torch.nn.RMSNorm(d, eps=eps, **T64)
+        with torch.no_grad():
+            layer.self_attn.in_proj_weight.copy_(_t(np.concatenate([W[p + "Wq"], W[p + "Wk"], W[p + "Wv"]])))
+            layer.self_attn.out_proj.weight.copy_(_t(W[p + "Wo"]))
+            layer.linear1.weight.copy_(_t(W[p + "Wup"]))
+            layer.linear2.weight.copy_(_t(W[p + "Wdown"]))
+            layer.norm1.weight.copy_(_t(W[p + "norm1.g"]))
+            layer.norm2.weight.copy_(_t(W[p + "norm2.g"]))
+            if has_bias:
+                layer.self_attn.in_proj_bias.copy_(_t(np.concatenate([W[p + "bq"], W[p + "bk"], W[p + "bv"]])))
+                layer.self_attn.out_proj.bias.copy_(_t(W[p + "bo"]))
+                layer.linear1.bias.copy_(_t(W[p + "bup"]))
+                layer.linear2.bias.copy_(_t(W[p + "bdown"]))
+            if norm == "ln":
+                layer.norm1.bias.copy_(_t(W[p + "norm1.b"]))
+                layer.norm2.bias.copy_(_t(W[p + "norm2.b"]))
+        layer.train()                                        # dropout is 0; train mode keeps PyTorch off its fused fast path
+        with torch.no_grad():
+            ht = layer(ht)
+    assert np.allclose(h, ht[0].numpy(), rtol=1e-10, atol=1e-11)
+
+
+# ---------------------------------------------------------------- decoder family (+ LoRA) vs transformers' LlamaModel
+def test_decoder_backbone_with_lora_matches_hf_llama_with_merged_weights():
+    tr = pytest.importorskip("transformers")
+    d, Hq, Hkv, dh, Fd, L, vocab, n = 48, 6, 2, 8, 80, 2, 61, 23
+    theta, eps = 10000.0, 1e-6
+    r = _rng(9643)
+    W = {"embed.table": r.standard_normal((vocab, d)), "final.g": 1 + 0.1 * r.standard_normal(d)}
+    dims = dict(q=(d, Hq * dh), k=(d, Hkv * dh), v=(d, Hkv * dh), o=(Hq * dh, d), gate=(d, Fd), up=(d, Fd), down=(Fd, d))
+    ranks = dict(q=4, k=2, v=8, o=3, gate=5, up=1, down=6)
+    task = dict(id=7, adapters={tg: (ranks[tg], 16.0 / ranks[tg]) for tg in dims}, head_kind="last", head_out=3)
+    for l in range(L):
+        p = f"L{l:02d}."
+        for tg, (din, dout) in dims.items():
+            W[p + "W" + tg] = r.standard_normal((dout, din)) * 0.15
+            W[f"task007.{p}{tg}.A"] = r.standard_normal((ranks[tg], din)) * 0.2
+            W[f"task007.{p}{tg}.B"] = r.standard_normal((dout, ranks[tg])) * 0.2
+        W[p + "norm1.g"] = 1 + 0.1 * r.standard_normal(d)
+        W[p + "norm2.g"] = 1 + 0.1 * r.standard_normal(d)
+    bb = dict(n_layers=L, d_model=d, n_q_heads=Hq, n_kv_heads=Hkv, head_dim=dh, d_ffn=Fd, act="swiglu", norm="rms", norm_eps=eps,
+              causal=True, rope_theta=theta, input_kind="tokens", patch_dim=0, has_cls=False, has_bias=False, has_pos=False,
+              img_c=0, img_hw=0, patch_hw=0)
+    toks = r.integers(0, vocab, size=n)
+    h = O.tokens_from_input(bb, W.__getitem__, toks)
+    for l in range(L):
+        h = O.layer_forward(bb, W.__getitem__, task, l, h)
+    got = O.rms_norm(h, W["final.g"], eps)                      # what head_forward pools from
+
+    cfg = tr.LlamaConfig(vocab_size=vocab, hidden_size=d, intermediate_size=Fd, num_hidden_layers=L, num_attention_heads=Hq,
+                         num_key_value_heads=Hkv, head_dim=dh, hidden_act="silu", max_position_embeddings=64, rms_norm_eps=eps,
+                         rope_theta=theta, attention_bias=False, mlp_bias=False, attention_dropout=0.0, tie_word_embeddings=False)
+    cfg._attn_implementation = "eager"
+    model = tr.LlamaModel(cfg).to(torch.float64).eval()
+    # rotary tables are buffers built in fp32: rebuild them in fp64 so the comparison is not limited by them
+    inv = 1.0 / (theta ** (torch.arange(0, dh, 2, dtype=torch.float64) / dh))
+    model.rotary_emb.inv_freq = inv
+    if hasattr(model.rotary_emb, "original_inv_freq"):
+        model.rotary_emb.original_inv_freq = inv
+
+    def merged(l, tg):
+        p = f"L{l:02d}."
+        s = task["adapters"][tg][1]
+        return _t(W[p + "W" + tg] + s * W[f"task007.{p}{tg}.B"] @ W[f"task007.{p}{tg}.A"])
+
+    with torch.no_grad():
+        model.embed_tokens.weight.copy_(_t(W["embed.table"]))
+        model.norm.weight.copy_(_t(W["final.g"]))
+        for l, layer in enumerate(model.layers):
+            layer.self_attn.q_proj.weight.copy_(merged(l, "q")); layer.self_attn.k_proj.weight.copy_(merged(l, "k"))
+            layer.self_attn.v_proj.weight.copy_(merged(l, "v")); layer.self_attn.o_proj.weight.copy_(merged(l, "o"))
+            layer.mlp.gate_proj.weight.copy_(merged(l, "gate")); layer.mlp.up_proj.weight.copy_(merged(l, "up"))
+            layer.mlp.down_proj.weight.copy_(merged(l, "down"))
+            layer.input_layernorm.weight.copy_(_t(W[f"L{l:02d}.norm1.g"]))
+            layer.post_attention_layernorm.weight.copy_(_t(W[f"L{l:02d}.norm2.g"]))
+        out = model(input_ids=torch.from_numpy(np.asarray(toks, dtype=np.int64))[None]).last_hidden_state[0].numpy()
+    # LlamaRotaryEmbedding evaluates cos / sin in fp32 whatever the model dtype, which bounds the agreement at ~1e-6 relative
+    # per rotation (measured here: 5e-6 absolute on outputs of magnitude 3); any structural mistake is O(0.1 .. 1).
+    err = np.abs(got - out).max()
+    assert err < 5e-5 * max(1.0, np.abs(out).max()), f"oracle vs LlamaModel: max abs {err:.3e}"
+    # sensitivity: the comparison really sees the adapters (an un-merged model differs by far more than the bar)
+    with torch.no_grad():
+        model.layers[0].self_attn.q_proj.weight.copy_(_t(W["L00.Wq"]))
+        out2 = model(input_ids=torch.from_numpy(np.asarray(toks, dtype=np.int64))[None]).last_hidden_state[0].numpy()
+    assert np.abs(got - out2).max() > 1e-3
+
+
+# ---------------------------------------------------------------- image patch embedding vs nn.Conv2d (the ViT formulation)
+def test_image_patch_embedding_matches_conv2d_patchify():
+    C, HW, P, d = 3, 28, 14, 20
+    r = _rng(14)
+    img = r.random((C, HW, HW))
+    W = {"embed.W": r.standard_normal((d, C * P * P)) * 0.1, "embed.b": r.standard_normal(d) * 0.1,
+         "embed.cls": r.standard_normal(d), "embed.pos": r.standard_normal(((HW // P) ** 2 + 1, d)) * 0.1}
+    bb = dict(input_kind="patch", patch_dim=C * P * P, has_cls=True, has_pos=True, img_c=C, img_hw=HW, patch_hw=P)
+    got = O.tokens_from_input(bb, W.__getitem__, img.reshape(-1))
+    conv = torch.nn.Conv2d(C, d, kernel_size=P, stride=P, **T64)
+    with torch.no_grad():
+        conv.weight.copy_(_t(W["embed.W"]).view(d, C, P, P))       # a ViT patch embed IS this convolution
+        conv.bias.copy_(_t(W["embed.b"]))
+        tok = conv(_t(img)[None])[0].flatten(1).transpose(0, 1)      # [grid*grid, d], patches row-major over the grid
+        ref = torch.cat([_t(W["embed.cls"])[None], tok]) + _t(W["embed.pos"])
+    assert got.shape == (5, d) and np.allclose(got, ref.numpy(), rtol=1e-12, atol=1e-13)
