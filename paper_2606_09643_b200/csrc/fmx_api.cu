@@ -63,6 +63,7 @@ struct Backbone {
   bf16 *embed_Wpad = nullptr;              // [d, Kp]
   float *posb = nullptr;                   // [n_pos, d]
   float2 *rope_cs = nullptr;               // [max_seq, dh/2]
+  float2 *rope_cs_t = nullptr;             // [dh/2, max_seq] (the fused-RoPE GEMM epilogue reads this one)
   // weight maps, [0] = box {64,128} (pair tile 256x256: one CTA loads a whole chunk), [1] = box {64,64} (256x128 tiles)
   std::vector<CUtensorMap> mWq[2], mWk[2], mWv[2], mWo[2], mWup[2], mWgate[2], mWdown[2];
   CUtensorMap mEmbedW[2];
@@ -616,7 +617,7 @@ int fmx_destroy(fmx_ctx *c) {
   for (auto e : c->ev_pool) cudaEventDestroy(e);
   for (auto &bp : c->bbs) {
     if (!bp) continue;
-    cudaFree(bp->embed_Wpad); cudaFree(bp->posb); cudaFree(bp->rope_cs);
+    cudaFree(bp->embed_Wpad); cudaFree(bp->posb); cudaFree(bp->rope_cs); cudaFree(bp->rope_cs_t);
     for (int tg = 0; tg < 7; ++tg) { cudaFree(bp->slabA[tg]); cudaFree(bp->slabB[tg]); }
   }
   for (auto &t : c->tasks) { cudaFree(t.head_W); cudaFree(t.head_b); }
@@ -711,6 +712,8 @@ int fmx_register_backbone(fmx_ctx *c, const fmx_backbone_desc *desc, fmx_backbon
     const int n = d.max_seq * (d.head_dim / 2);
     CU_OK(cudaMalloc(&b->rope_cs, sizeof(float2) * n));
     build_rope_table_kernel<<<(n + 255) / 256, 256>>>(b->rope_cs, d.max_seq, d.head_dim, (double)d.rope_theta);
+    CU_OK(cudaMalloc(&b->rope_cs_t, sizeof(float2) * n));
+    transpose_rope_table_kernel<<<(n + 255) / 256, 256>>>(b->rope_cs, b->rope_cs_t, d.max_seq, d.head_dim / 2);
     CU_OK(cudaGetLastError());
   }
   CU_OK(cudaDeviceSynchronize());
@@ -1044,7 +1047,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       p.omap = oQKV;
       // head_dim 128: a 128-column chunk is one head, so RoPE is applied in the GEMM epilogue (fp32, one rounding)
       rope_fused = g_rope_fused && d.rope_theta > 0 && d.head_dim == 128 && pair_wide(p);
-      if (rope_fused) { p.rope_cs = bb.rope_cs; p.rope_src_mask = 3; }
+      if (rope_fused) { p.rope_cs = bb.rope_cs_t; p.rope_ld = d.max_seq; p.rope_src_mask = 3; }
       p.reverse = rev();
       LAUNCH(Lh, F_GEMM_QKV, launch_pair_gemm(c, s, p));
     }

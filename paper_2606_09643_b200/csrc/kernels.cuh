@@ -363,6 +363,15 @@ __global__ void __launch_bounds__(256) rope_kernel(__nv_bfloat16 *qkv, int ld, c
   *reinterpret_cast<uint4 *>(p + half) = make_uint4(bo[0], bo[1], bo[2], bo[3]);
 }
 
+// transposed copy [dh/2][max_seq]: for a fixed pair index, consecutive positions are contiguous, so the threads of a warp
+// (= consecutive token rows = mostly consecutive positions) read it coalesced in the GEMM epilogue
+__global__ void transpose_rope_table_kernel(const float2 *cs, float2 *cs_t, int max_seq, int half) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= max_seq * half) return;
+  const int p = idx / half, j = idx - p * half;
+  cs_t[(size_t)j * max_seq + p] = cs[idx];
+}
+
 __global__ void build_rope_table_kernel(float2 *cs, int max_seq, int dh, double theta) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   const int half = dh >> 1;

@@ -86,7 +86,8 @@ struct PairGemmParams {
   unsigned *u_flag;        // one counter: arrivals of the epilogue warps that wrote a U block (monotonic over a forward)
   unsigned u_epoch;        // 1, 2, ... over the fused launches of a forward: this launch's U is complete when the counter
                            // reaches 16 (epilogue warps of a pair) * n_blk * u_epoch
-  const float2 *rope_cs;   // [max_seq, 64] (cos, sin): fused rotate-half RoPE for head_dim 128 (chunk = head), or NULL
+  const float2 *rope_cs;   // [64, rope_ld] (cos, sin), pair-index major: fused rotate-half RoPE for head_dim 128 (chunk = head), or NULL
+  int rope_ld;             // positions per pair index (= max_seq)
   int rope_src_mask;       // bit s: source s (q | k | v) is rotated
 };
 
@@ -460,7 +461,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
           uint8_t *rowA = stg + r_in_tile * 128, *rowB = rowA + 16384;
           if (issuer) bulk_wait_read<0>();
           named_bar_sync(bar_id, 128);
-          const float2 *cs = p.rope_cs + (size_t)(row < p.M ? p.row_pos[row] : 0) * 64;
+          const float2 *cs = p.rope_cs + (row < p.M ? p.row_pos[row] : 0);          // + j * rope_ld for pair index j
           const __nv_bfloat16 *bias = p.bias[s_wg];
 #pragma unroll 1
           for (int h = 0; h < 2; ++h) {
@@ -484,13 +485,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
                   x2[e] += __bfloat162float(bias[r0_wg + 64 + h * 32 + 8 * q + e]);
                 }
               }
-              const float4 *c4 = reinterpret_cast<const float4 *>(cs + h * 32 + q * 8);
               uint32_t oa[4], ob[4];
 #pragma unroll
               for (int e = 0; e < 4; ++e) {
-                const float4 c = c4[e];                     // (cos, sin) of dims 2e, 2e+1 of this group
-                oa[e] = pack_bf16(x1[2 * e] * c.x - x2[2 * e] * c.y, x1[2 * e + 1] * c.z - x2[2 * e + 1] * c.w);
-                ob[e] = pack_bf16(x2[2 * e] * c.x + x1[2 * e] * c.y, x2[2 * e + 1] * c.z + x1[2 * e + 1] * c.w);
+                // (cos, sin) of dims 2e, 2e+1 of this group: consecutive rows read consecutive addresses
+                const float2 ca = __ldg(cs + (size_t)(h * 32 + q * 8 + 2 * e) * p.rope_ld);
+                const float2 cb = __ldg(cs + (size_t)(h * 32 + q * 8 + 2 * e + 1) * p.rope_ld);
+                oa[e] = pack_bf16(x1[2 * e] * ca.x - x2[2 * e] * ca.y, x1[2 * e + 1] * cb.x - x2[2 * e + 1] * cb.y);
+                ob[e] = pack_bf16(x2[2 * e] * ca.x + x1[2 * e] * ca.y, x2[2 * e + 1] * cb.x + x1[2 * e + 1] * cb.y);
               }
               *reinterpret_cast<uint4 *>(rowA + (((h * 4 + q) ^ rsw) << 4)) = make_uint4(oa[0], oa[1], oa[2], oa[3]);
               *reinterpret_cast<uint4 *>(rowB + (((h * 4 + q) ^ rsw) << 4)) = make_uint4(ob[0], ob[1], ob[2], ob[3]);
