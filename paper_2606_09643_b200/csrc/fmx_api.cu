@@ -1167,6 +1167,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
         c->d_head_part = nullptr; c->head_part_bytes = 0;
         CU_OK(cudaMalloc(&c->d_head_part, align_up(need, 1 << 20)));
         c->head_part_bytes = align_up(need, 1 << 20);
+        ++c->config_gen;                      // a cached forward graph still points at the old scratch buffer
       }
     }
     if (n_kc > 0) {
