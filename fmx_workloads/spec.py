@@ -90,6 +90,7 @@ class TaskSpec:
     head_kind: str      # 'mean' | 'cls' | 'last' | 'flatten'
     head_out: int
     head_std: float = 0.02
+    head_hidden: int = 0   # > 0: MLP decoder head  W2 relu(W feat + b) + b2  (Listing 2, MLPDecoder hidden_dim)
 
     def d_feat(self, bb: BackboneSpec) -> int:
         return bb.d_model * bb.tokens_per_request if self.head_kind == "flatten" else bb.d_model
@@ -159,9 +160,14 @@ class Workload:
             t = int(parts[0][4:])
             ts = self.tasks[t]
             if parts[1] == "head":
+                w1 = ts.head_hidden or ts.head_out                      # rows of the first (or only) layer
                 if parts[2] == "W":
-                    return (ts.head_out, ts.d_feat(bb)), "normal", ts.head_std
-                return (ts.head_out,), "normal", 0.02
+                    return (w1, ts.d_feat(bb)), "normal", ts.head_std
+                if parts[2] == "W2":
+                    return (ts.head_out, ts.head_hidden), "normal", 0.1
+                if parts[2] == "b2":
+                    return (ts.head_out,), "normal", 0.02
+                return (w1,), "normal", 0.02
             tgt, ab = parts[2], parts[3]
             ad = next(a for a in ts.adapters if a.target == tgt)
             d_in, d_out = target_dims(bb, tgt)
@@ -240,6 +246,8 @@ class Workload:
     def task_tensor_names(self, t: int) -> List[str]:
         ts = self.tasks[t]
         names = [f"task{t:03d}.head.W", f"task{t:03d}.head.b"]
+        if self.tasks[t].head_hidden:
+            names += [f"task{t:03d}.head.W2", f"task{t:03d}.head.b2"]
         for l in range(self.bb.n_layers):
             for ad in ts.adapters:
                 names += [f"task{t:03d}.L{l:02d}.{ad.target}.A", f"task{t:03d}.L{l:02d}.{ad.target}.B"]
@@ -322,14 +330,16 @@ def _tasks_for(cfg: str, seed: int, T: int) -> List[TaskSpec]:
 def make_workload(cfg: str, *, n_layers: Optional[int] = None, batch: Optional[int] = None,
                   n_tasks: Optional[int] = None, dist: Optional[str] = None,
                   max_len: Optional[int] = None, adapters: bool = True,
-                  seed_offset: int = 0, lora_std: float = 0.02) -> Workload:
+                  seed_offset: int = 0, lora_std: float = 0.02, mlp_hidden: int = 0) -> Workload:
     """Build the workload of a BASELINE.json config (cfg1..cfg5).
 
     Overrides give the reduced variants the parity tests use (fewer layers, smaller batch);
     with no overrides the result is the full config.  cfg5 takes n_tasks in {1,4,16,48,92}
     and dist in {'uniform','zipf0.8','zipf1.5'}; adapters=False registers head-only tasks
     (the adapter-free reference of reading #19).  lora_std != 0.02 is a STRESS variant for
-    tests that need the adapter delta to dominate the tolerance; it is not a config.
+    tests that need the adapter delta to dominate the tolerance; it is not a config.  mlp_hidden > 0 turns
+    every pooled (non-flatten) head into an MLP decoder head of that hidden width (the
+    paper's Listing 2 uses hidden_dim 128) - a test variant, not a BASELINE.json config.
     """
     bb = _BACKBONES[cfg]
     if n_layers is not None:
@@ -346,6 +356,8 @@ def make_workload(cfg: str, *, n_layers: Optional[int] = None, batch: Optional[i
     tasks = _tasks_for(cfg, seed, T)
     if not adapters:
         tasks = [replace(t, adapters=()) for t in tasks]
+    if mlp_hidden:
+        tasks = [t if t.head_kind == "flatten" else replace(t, head_hidden=mlp_hidden) for t in tasks]
     rng = _stream(seed, "task_ids")
     if cfg == "cfg1":
         while True:                                   # reading #20: every task present

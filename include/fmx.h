@@ -121,6 +121,14 @@ typedef struct fmx_task_desc {
   const void *head_W;          /* DEVICE bf16 [head_out, d_feat]; d_feat = d_model, or
                                   tokens_per_request*d_model for FLATTEN                      */
   const void *head_b;          /* DEVICE bf16 [head_out] or NULL                              */
+  /* MLP decoder head (Listing 2: MLPDecoder(input_dim, hidden_dim, output_dim)).
+   * head_hidden = 0: the linear head above.  head_hidden > 0 (pooled kinds only, <= 4096):
+   *   y = W2 · relu(W · feat + b) + b2   with head_W [head_hidden, d_feat], head_b [head_hidden] or NULL,
+   *   head_W2 DEVICE bf16 [head_out, head_hidden] (required), head_b2 DEVICE bf16 [head_out] or NULL.
+   * The activation is ReLU (the paper names only the three widths; reading 32). */
+  int32_t head_hidden;
+  const void *head_W2;
+  const void *head_b2;
 } fmx_task_desc;
 
 /* ---- lifecycle ---------------------------------------------------------------------- */

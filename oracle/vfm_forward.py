@@ -22,7 +22,7 @@ float64 arrays (the bf16-rounded values the GPU receives, widened).  Tensor name
     L{ll}.norm2.g/.b  final.g/.b
     task{ttt}.L{ll}.{target}.A [r,d_in]  .B [d_out,r]   task{ttt}.head.W [o,d_feat]  .head.b [o]
 `bb` is a dict of hyper-parameters (see `REQUIRED_BB_KEYS`); `task` is a dict
-{id, adapters: {target: (rank, scaling)}, head_kind, head_out}.
+{id, adapters: {target: (rank, scaling)}, head_kind, head_out[, head_hidden]}.
 
 Pins (tests/test_oracle_pins.py): brute-force matmul on tiny shapes; closed forms for the
 norms, softmax, GeLU/SiLU, RoPE; the LoRA merge identity W' = W + s·B·A; zero adapter ==
@@ -222,7 +222,12 @@ def head_forward(bb, get, task, h):
     f = _norm(bb, get, "final", h)
     feat = pooled_feature(f, task["head_kind"])
     p = f"task{task['id']:03d}.head."
-    return get(p + "W") @ feat + get(p + "b")
+    y = get(p + "W") @ feat + get(p + "b")
+    if task.get("head_hidden", 0):
+        # MLP decoder head (Listing 2: MLPDecoder(input_dim, hidden_dim, output_dim)); the paper names the three
+        # widths only - ReLU between the two linear layers is DESIGN.md reading 32
+        y = get(p + "W2") @ relu(y) + get(p + "b2")
+    return y
 
 
 def forward_request(bb, get, task, x):

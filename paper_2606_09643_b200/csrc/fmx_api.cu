@@ -50,8 +50,9 @@ struct TaskRec {
   int coff = 0, rpad = 0;                 // slab columns [coff, coff + rpad)
   unsigned char trpad[7] = {0};
   float scale[7] = {0};
-  int head_kind = 0, head_out = 0;
+  int head_kind = 0, head_out = 0, head_hidden = 0;   // head_hidden > 0: MLP head, head_W is [head_hidden, d_feat]
   bf16 *head_W = nullptr, *head_b = nullptr;   // library-owned copies
+  bf16 *head_W2 = nullptr, *head_b2 = nullptr; // MLP heads: [head_out, head_hidden], [head_out]
 };
 
 struct Backbone {
@@ -92,7 +93,9 @@ struct fmx_ctx {
   int *d_task_coff = nullptr, *d_task_head_kind = nullptr, *d_task_head_out = nullptr;
   unsigned char *d_task_trpad = nullptr;
   float *d_task_scale = nullptr;
-  const bf16 **d_task_head_W = nullptr, **d_task_head_b = nullptr;
+  const bf16 **d_task_head_W = nullptr, **d_task_head_b = nullptr, **d_task_head_W2 = nullptr, **d_task_head_b2 = nullptr;
+  int *d_task_head_w1 = nullptr;           // first-layer width of the head (= head_out for linear heads)
+  float *d_head_hid = nullptr; size_t head_hid_bytes = 0;       // hidden activations of MLP heads [B, max hidden]
   // pinned staging for ids / lengths: a ring (a slot is rewritten only after the copy that read it has run) plus one
   // buffer owned by the cached CUDA graph
   static constexpr int kStageSlots = 4;
@@ -534,6 +537,11 @@ int upload_task_tables(fmx_ctx *c, int t) {
   const bf16 *w = r.head_W, *b = r.head_b;
   CU_OK(cudaMemcpy(c->d_task_head_W + t, &w, sizeof(void *), cudaMemcpyHostToDevice));
   CU_OK(cudaMemcpy(c->d_task_head_b + t, &b, sizeof(void *), cudaMemcpyHostToDevice));
+  const bf16 *w2 = r.head_W2, *b2 = r.head_b2;
+  const int w1 = r.head_hidden > 0 ? r.head_hidden : r.head_out;
+  CU_OK(cudaMemcpy(c->d_task_head_W2 + t, &w2, sizeof(void *), cudaMemcpyHostToDevice));
+  CU_OK(cudaMemcpy(c->d_task_head_b2 + t, &b2, sizeof(void *), cudaMemcpyHostToDevice));
+  CU_OK(cudaMemcpy(c->d_task_head_w1 + t, &w1, sizeof(int), cudaMemcpyHostToDevice));
   return FMX_OK;
 }
 
@@ -595,6 +603,9 @@ int fmx_create(fmx_ctx **out, int device_ordinal) {
   CU_OK(cudaMalloc(&c->d_task_scale, sizeof(float) * 7 * FMX_MAX_TASKS));
   CU_OK(cudaMalloc(&c->d_task_head_W, sizeof(void *) * FMX_MAX_TASKS));
   CU_OK(cudaMalloc(&c->d_task_head_b, sizeof(void *) * FMX_MAX_TASKS));
+  CU_OK(cudaMalloc(&c->d_task_head_W2, sizeof(void *) * FMX_MAX_TASKS));
+  CU_OK(cudaMalloc(&c->d_task_head_b2, sizeof(void *) * FMX_MAX_TASKS));
+  CU_OK(cudaMalloc(&c->d_task_head_w1, sizeof(int) * FMX_MAX_TASKS));
   CU_OK(cudaMemset(c->d_task_coff, 0, sizeof(int) * FMX_MAX_TASKS));
   CU_OK(cudaMemset(c->d_task_head_kind, 0, sizeof(int) * FMX_MAX_TASKS));
   CU_OK(cudaMemset(c->d_task_head_out, 0, sizeof(int) * FMX_MAX_TASKS));
@@ -602,6 +613,9 @@ int fmx_create(fmx_ctx **out, int device_ordinal) {
   CU_OK(cudaMemset(c->d_task_scale, 0, sizeof(float) * 7 * FMX_MAX_TASKS));
   CU_OK(cudaMemset(c->d_task_head_W, 0, sizeof(void *) * FMX_MAX_TASKS));
   CU_OK(cudaMemset(c->d_task_head_b, 0, sizeof(void *) * FMX_MAX_TASKS));
+  CU_OK(cudaMemset(c->d_task_head_W2, 0, sizeof(void *) * FMX_MAX_TASKS));
+  CU_OK(cudaMemset(c->d_task_head_b2, 0, sizeof(void *) * FMX_MAX_TASKS));
+  CU_OK(cudaMemset(c->d_task_head_w1, 0, sizeof(int) * FMX_MAX_TASKS));
   CU_OK(cudaMallocHost(&c->h_stage, sizeof(int) * 2 * FMX_MAX_REQUESTS * (fmx_ctx::kStageSlots + 1)));
   for (int i = 0; i < fmx_ctx::kStageSlots; ++i) CU_OK(cudaEventCreateWithFlags(&c->stage_ev[i], cudaEventDisableTiming));
   *out = c.release();
@@ -620,9 +634,10 @@ int fmx_destroy(fmx_ctx *c) {
     cudaFree(bp->embed_Wpad); cudaFree(bp->posb); cudaFree(bp->rope_cs); cudaFree(bp->rope_cs_t);
     for (int tg = 0; tg < 7; ++tg) { cudaFree(bp->slabA[tg]); cudaFree(bp->slabB[tg]); }
   }
-  for (auto &t : c->tasks) { cudaFree(t.head_W); cudaFree(t.head_b); }
+  for (auto &t : c->tasks) { cudaFree(t.head_W); cudaFree(t.head_b); cudaFree(t.head_W2); cudaFree(t.head_b2); }
   cudaFree(c->d_task_coff); cudaFree(c->d_task_head_kind); cudaFree(c->d_task_head_out); cudaFree(c->d_task_trpad);
   cudaFree(c->d_task_scale); cudaFree(c->d_task_head_W); cudaFree(c->d_task_head_b);
+  cudaFree(c->d_task_head_W2); cudaFree(c->d_task_head_b2); cudaFree(c->d_task_head_w1); cudaFree(c->d_head_hid);
   cudaFree(c->d_in_stage); cudaFree(c->d_out_stage); cudaFree(c->d_dbg_cu); cudaFree(c->d_head_part);
   if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
   for (int i = 0; i < fmx_ctx::kStageSlots; ++i) if (c->stage_ev[i]) cudaEventDestroy(c->stage_ev[i]);
@@ -737,6 +752,9 @@ int fmx_register_task(fmx_ctx *c, fmx_backbone_t h, const fmx_task_desc *desc, f
   if (desc->n_adapters < 0 || desc->n_adapters > 7 || (desc->n_adapters && !desc->adapters)) return fmx_fail(FMX_E_INVALID_ARG, "register_task: bad n_adapters");
   if (desc->head_kind < 0 || desc->head_kind > 3 || desc->head_out < 1 || !desc->head_W) return fmx_fail(FMX_E_INVALID_ARG, "register_task: bad head");
   if (desc->head_kind == FMX_HEAD_FLATTEN && d.tokens_per_request < 1) return fmx_fail(FMX_E_SHAPE, "register_task: FLATTEN head needs a fixed-length backbone");
+  if (desc->head_hidden < 0 || desc->head_hidden > 4096) return fmx_fail(FMX_E_SHAPE, "register_task: head_hidden %d not in [0,4096]", desc->head_hidden);
+  if (desc->head_hidden > 0 && desc->head_kind == FMX_HEAD_FLATTEN) return fmx_fail(FMX_E_SHAPE, "register_task: an MLP head needs a pooled feature (mean / cls / last)");
+  if (desc->head_hidden > 0 && !desc->head_W2) return fmx_fail(FMX_E_INVALID_ARG, "register_task: MLP head without head_W2");
   bool seen[7] = {false};
   int rpad = 0;
   for (int i = 0; i < desc->n_adapters; ++i) {
@@ -755,7 +773,7 @@ int fmx_register_task(fmx_ctx *c, fmx_backbone_t h, const fmx_task_desc *desc, f
   if (slot < 0) return fmx_fail(FMX_E_CAPACITY, "register_task: all %d task slots in use", FMX_MAX_TASKS);
 
   TaskRec r;
-  r.live = true; r.bb = h; r.head_kind = desc->head_kind; r.head_out = desc->head_out; r.rpad = rpad;
+  r.live = true; r.bb = h; r.head_kind = desc->head_kind; r.head_out = desc->head_out; r.head_hidden = desc->head_hidden; r.rpad = rpad;
   // ---- slab columns ----
   if (rpad) {
     int units = rpad / 16, pos = find_columns(*bb, units);
@@ -789,11 +807,20 @@ int fmx_register_task(fmx_ctx *c, fmx_backbone_t h, const fmx_task_desc *desc, f
   }
   // ---- head ----
   const size_t d_feat = desc->head_kind == FMX_HEAD_FLATTEN ? (size_t)d.tokens_per_request * d.d_model : (size_t)d.d_model;
-  CU_OK(cudaMalloc(&r.head_W, sizeof(bf16) * d_feat * desc->head_out));
-  CU_OK(cudaMemcpyAsync(r.head_W, desc->head_W, sizeof(bf16) * d_feat * desc->head_out, cudaMemcpyDeviceToDevice, 0));
+  const size_t w1 = desc->head_hidden > 0 ? (size_t)desc->head_hidden : (size_t)desc->head_out;     // rows of the first layer
+  CU_OK(cudaMalloc(&r.head_W, sizeof(bf16) * d_feat * w1));
+  CU_OK(cudaMemcpyAsync(r.head_W, desc->head_W, sizeof(bf16) * d_feat * w1, cudaMemcpyDeviceToDevice, 0));
   if (desc->head_b) {
-    CU_OK(cudaMalloc(&r.head_b, sizeof(bf16) * desc->head_out));
-    CU_OK(cudaMemcpyAsync(r.head_b, desc->head_b, sizeof(bf16) * desc->head_out, cudaMemcpyDeviceToDevice, 0));
+    CU_OK(cudaMalloc(&r.head_b, sizeof(bf16) * w1));
+    CU_OK(cudaMemcpyAsync(r.head_b, desc->head_b, sizeof(bf16) * w1, cudaMemcpyDeviceToDevice, 0));
+  }
+  if (desc->head_hidden > 0) {
+    CU_OK(cudaMalloc(&r.head_W2, sizeof(bf16) * (size_t)desc->head_out * desc->head_hidden));
+    CU_OK(cudaMemcpyAsync(r.head_W2, desc->head_W2, sizeof(bf16) * (size_t)desc->head_out * desc->head_hidden, cudaMemcpyDeviceToDevice, 0));
+    if (desc->head_b2) {
+      CU_OK(cudaMalloc(&r.head_b2, sizeof(bf16) * desc->head_out));
+      CU_OK(cudaMemcpyAsync(r.head_b2, desc->head_b2, sizeof(bf16) * desc->head_out, cudaMemcpyDeviceToDevice, 0));
+    }
   }
   c->tasks[slot] = r;
   c->n_slots = std::max(c->n_slots, slot + 1);
@@ -826,6 +853,8 @@ int fmx_unregister_task(fmx_ctx *c, fmx_task_t t) {
   for (int u = 0; u < r.rpad / 16; ++u) bb->col_used[r.coff / 16 + u] = 0;
   cudaFree(r.head_W);
   cudaFree(r.head_b);
+  cudaFree(r.head_W2);
+  cudaFree(r.head_b2);
   r = TaskRec();
   if (int e = upload_task_tables(c, t)) return e;
   CU_OK(cudaDeviceSynchronize());
@@ -875,7 +904,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       return fmx_fail(FMX_E_BAD_LENGTH, "forward_mixed: request %d: length %d (max_seq %d, fixed %d)", i, n, d.max_seq, d.tokens_per_request);
     N += n;
     max_len = std::max(max_len, n);
-    max_out = std::max(max_out, c->tasks[t].head_out);
+    max_out = std::max(max_out, c->tasks[t].head_hidden > 0 ? c->tasks[t].head_hidden : c->tasks[t].head_out);   // first-layer width
   }
   if (N > (1ll << 24)) return fmx_fail(FMX_E_CAPACITY, "forward_mixed: %lld tokens > 2^24", N);
   const int T = c->n_slots;
@@ -1141,6 +1170,26 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   ha.task_head_kind = c->d_task_head_kind; ha.task_head_out = c->d_task_head_out;
   ha.task_head_W = (const bf16 *const *)c->d_task_head_W; ha.task_head_b = (const bf16 *const *)c->d_task_head_b;
   ha.out = outputs; ha.d = d.d_model;
+  ha.task_head_w1 = c->d_task_head_w1;
+  ha.task_head_W2 = (const bf16 *const *)c->d_task_head_W2; ha.task_head_b2 = (const bf16 *const *)c->d_task_head_b2;
+  int max_hidden = 0, max_out2 = 0;                      // MLP heads in this batch
+  for (int i = 0; i < B; ++i) {
+    const TaskRec &tr = c->tasks[task_ids[i]];
+    if (tr.head_hidden > 0) { max_hidden = std::max(max_hidden, tr.head_hidden); max_out2 = std::max(max_out2, tr.head_out); }
+  }
+  if (max_hidden > 0) {
+    const size_t need = sizeof(float) * (size_t)B * max_hidden;
+    if (need > c->head_hid_bytes) {
+      if (graph_capture) return fmx_fail(FMX_E_CUDA, "forward_mixed: MLP-head scratch grew during graph capture");
+      CU_OK(cudaStreamSynchronize(s));
+      cudaFree(c->d_head_hid);
+      c->d_head_hid = nullptr; c->head_hid_bytes = 0;
+      CU_OK(cudaMalloc(&c->d_head_hid, align_up(need, 1 << 16)));
+      c->head_hid_bytes = align_up(need, 1 << 16);
+      ++c->config_gen;
+    }
+    ha.hid = c->d_head_hid; ha.ld_hid = max_hidden;
+  }
   bool any_flat = false, any_pooled = false;
   int max_out_flat = 0;
   for (int i = 0; i < B; ++i) {
@@ -1177,6 +1226,9 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       LAUNCH(Lh, F_HEAD, (launch_k(head_flatten_kernel, dim3((B + 3) / 4, (max_out + 3) / 4), 256, 0, s, ha, B)));
     }
   }
+
+  if (max_hidden > 0)                                    // second layer of the MLP heads (the first wrote relu(W feat + b) to hid)
+    LAUNCH(Lh, F_HEAD, (launch_k(head_mlp2_kernel, dim3(B, (max_out2 + 7) / 8), 256, 0, s, ha)));
 
   {
     void *bufs[7] = {w.X, w.Xn, w.QKV, w.AttnO, w.Hid, w.U, w.feat};

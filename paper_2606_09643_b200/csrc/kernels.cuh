@@ -472,6 +472,12 @@ struct HeadArgs {
   const __nv_bfloat16 *const *task_head_W, *const *task_head_b;
   float *out;
   int d;
+  // MLP heads: first-layer width per task (= head_out for linear heads), second-layer weights (NULL = linear head), and the
+  // fp32 hidden scratch [B, ld_hid] indexed by SORTED request
+  const int *task_head_w1;
+  const __nv_bfloat16 *const *task_head_W2, *const *task_head_b2;
+  float *hid;
+  int ld_hid;
   int skip_flatten;                // 1: FLATTEN heads are computed by head_flatten_kernel
 };
 
@@ -483,7 +489,7 @@ __global__ void __launch_bounds__(256) head_kernel(const HeadArgs a) {
   const int p = blockIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int t = a.task_sorted[p];
   const int o = blockIdx.y * 8 + warp;
-  const int n_out = a.task_head_out[t];
+  const int n_out = a.task_head_w1[t];
   if (o >= n_out) return;
   const int kind = a.task_head_kind[t];
   if (kind == 3 && a.skip_flatten) return;
@@ -512,6 +518,30 @@ __global__ void __launch_bounds__(256) head_kernel(const HeadArgs a) {
   for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
   if (lane == 0) {
     const __nv_bfloat16 *b = a.task_head_b[t];
+    const float v = acc + (b ? __bfloat162float(b[o]) : 0.0f);
+    if (a.task_head_W2[t]) a.hid[(size_t)p * a.ld_hid + o] = fmaxf(v, 0.0f);      // hidden layer of an MLP head
+    else a.out[a.out_off[a.perm[p]] + o] = v;
+  }
+}
+
+// Second layer of MLP heads: y = W2 · hid + b2, one warp per (sorted request, output), written in ORIGINAL request order.
+__global__ void __launch_bounds__(256) head_mlp2_kernel(const HeadArgs a) {
+  griddep_launch();
+  griddep_wait();
+  const int p = blockIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int t = a.task_sorted[p];
+  const __nv_bfloat16 *W2 = a.task_head_W2[t];
+  const int o = blockIdx.y * 8 + warp;
+  if (!W2 || o >= a.task_head_out[t]) return;
+  const int K = a.task_head_w1[t];
+  const float *h = a.hid + (size_t)p * a.ld_hid;
+  const __nv_bfloat16 *w = W2 + (size_t)o * K;
+  float acc = 0.0f;
+  for (int c = lane; c < K; c += 32) acc = fmaf(h[c], __bfloat162float(w[c]), acc);
+#pragma unroll
+  for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
+  if (lane == 0) {
+    const __nv_bfloat16 *b = a.task_head_b2[t];
     a.out[a.out_off[a.perm[p]] + o] = acc + (b ? __bfloat162float(b[o]) : 0.0f);
   }
 }

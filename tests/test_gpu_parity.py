@@ -397,3 +397,30 @@ def test_repeated_forwards_are_bit_identical(fmx_mod, cfg, kw):
         again = s.forward_numpy()
         for a, b in zip(first, again):
             assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("cfg,kw", [
+    ("cfg1", dict(mlp_hidden=16)),                                          # mean-pooled MLP heads on the tiny encoder
+    ("cfg2", dict(n_layers=2, batch=24, mlp_hidden=128)),                   # MLP (mean) and linear FLATTEN heads in one batch
+    ("cfg3", dict(n_layers=2, batch=6, mlp_hidden=128)),                    # CLS feature, outputs 10 .. 1000
+    ("cfg4", dict(n_layers=2, batch=8, max_len=200, mlp_hidden=128)),       # last-token feature, scalar regression heads (o = 1)
+])
+def test_mlp_decoder_heads_parity(fmx_mod, cfg, kw):
+    """per-task MLP decoder heads  y = W2 relu(W feat + b) + b2  (the paper's Listing 2 attaches
+    MLPDecoder(input_dim 1024, hidden_dim 128, output_dim 1)); linear and MLP heads mix freely in a batch."""
+    wl = make_workload(cfg, **kw)
+    assert any(t.head_hidden for t in wl.tasks)
+    s = _session(fmx_mod, wl)
+    y = s.forward_numpy()
+    check_segments(s, wl)
+    check_parity(y, G.oracle_outputs(wl), f"{cfg} MLP heads")
+
+
+def test_mlp_head_on_a_flatten_feature_is_rejected(fmx_mod):
+    wl = make_workload("cfg2", n_layers=1, batch=4)
+    s = _session(fmx_mod, wl)
+    W = torch.zeros(128 * 64 * 1024, dtype=torch.bfloat16, device="cuda")
+    W2 = torch.zeros(4 * 128, dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(fmx_mod.FmxError) as e:
+        s.fmx.register_task(s.bb, [], 3, 4, W.data_ptr(), None, 128, W2.data_ptr(), None)
+    assert "pooled" in str(e.value)

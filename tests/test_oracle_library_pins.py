@@ -197,3 +197,34 @@ def test_image_patch_embedding_matches_conv2d_patchify():
         tok = conv(_t(img)[None])[0].flatten(1).transpose(0, 1)      # [grid*grid, d], patches row-major over the grid
         ref = torch.cat([_t(W["embed.cls"])[None], tok]) + _t(W["embed.pos"])
     assert got.shape == (5, d) and np.allclose(got, ref.numpy(), rtol=1e-12, atol=1e-13)
+
+
+# ---------------------------------------------------------------- MLP decoder head vs nn.Sequential
+def test_mlp_head_matches_torch_sequential_and_reduces_to_the_linear_head():
+    d, hidden, out, n = 24, 16, 3, 7
+    r = _rng(128)
+    W = {"final.g": 1 + 0.1 * r.standard_normal(d), "final.b": 0.1 * r.standard_normal(d),
+         "task004.head.W": r.standard_normal((hidden, d)), "task004.head.b": r.standard_normal(hidden),
+         "task004.head.W2": r.standard_normal((out, hidden)), "task004.head.b2": r.standard_normal(out)}
+    bb = dict(norm="ln", norm_eps=1e-5)
+    h = r.standard_normal((n, d))
+    for kind in ("mean", "cls", "last"):
+        task = dict(id=4, adapters={}, head_kind=kind, head_out=out, head_hidden=hidden)
+        got = O.head_forward(bb, W.__getitem__, task, h)
+        f = F.layer_norm(_t(h), (d,), _t(W["final.g"]), _t(W["final.b"]), 1e-5)
+        feat = {"mean": f.mean(0), "cls": f[0], "last": f[-1]}[kind]
+        mlp = torch.nn.Sequential(torch.nn.Linear(d, hidden, **T64), torch.nn.ReLU(), torch.nn.Linear(hidden, out, **T64))
+        with torch.no_grad():
+            mlp[0].weight.copy_(_t(W["task004.head.W"])); mlp[0].bias.copy_(_t(W["task004.head.b"]))
+            mlp[2].weight.copy_(_t(W["task004.head.W2"])); mlp[2].bias.copy_(_t(W["task004.head.b2"]))
+            ref = mlp(feat).numpy()
+        assert got.shape == (out,) and np.allclose(got, ref, rtol=1e-12, atol=1e-12)
+    # special case: identity second layer on a non-negative hidden vector gives the first layer back
+    W["task004.head.W"] = np.abs(W["task004.head.W"]); W["task004.head.b"] = np.abs(W["task004.head.b"])
+    W["task004.head.W2"] = np.eye(hidden); W["task004.head.b2"] = np.zeros(hidden)
+    pos = dict(norm="rms", norm_eps=1e-6)
+    hp = np.abs(h)
+    W["final.g"] = np.abs(W["final.g"])
+    lin = O.head_forward(pos, W.__getitem__, dict(id=4, adapters={}, head_kind="mean", head_out=hidden), hp)
+    mlp_out = O.head_forward(pos, W.__getitem__, dict(id=4, adapters={}, head_kind="mean", head_out=hidden, head_hidden=hidden), hp)
+    assert (lin > 0).all() and np.allclose(lin, mlp_out, rtol=1e-13)
