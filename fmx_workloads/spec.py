@@ -90,6 +90,7 @@ class TaskSpec:
     head_kind: str      # 'mean' | 'cls' | 'last' | 'flatten'
     head_out: int
     head_std: float = 0.02
+    enc_channels: int = 0  # > 1: per-task input encoder, a linear channel combiner C -> 1 (Listing 2)
     head_hidden: int = 0   # > 0: MLP decoder head  W2 relu(W feat + b) + b2  (Listing 2, MLPDecoder hidden_dim)
 
     def d_feat(self, bb: BackboneSpec) -> int:
@@ -159,6 +160,8 @@ class Workload:
         if parts[0].startswith("task"):
             t = int(parts[0][4:])
             ts = self.tasks[t]
+            if parts[1] == "enc":
+                return ((ts.enc_channels,) if parts[2] == "W" else (1,)), "normal", (0.6 if parts[2] == "W" else 0.05)
             if parts[1] == "head":
                 w1 = ts.head_hidden or ts.head_out                      # rows of the first (or only) layer
                 if parts[2] == "W":
@@ -203,10 +206,13 @@ class Workload:
             return rng.integers(0, bb.vocab, size=int(self.lengths[i]), dtype=np.int32)
         if bb.img_c:       # raw image, values U(0,1)
             return f32_to_bf16_bits(rng.random((bb.img_c, bb.img_hw, bb.img_hw), dtype=np.float32))
-        # univariate random walk, z-normalised with the population std (reading #21)
+        # univariate random walk, z-normalised with the population std (reading #21); a task with an input encoder brings
+        # C such channels, channel-major [C, n]
         n = bb.n_patches * bb.patch_dim
-        walk = np.cumsum(rng.standard_normal(n, dtype=np.float64))
-        z = (walk - walk.mean()) / walk.std()
+        C = max(self.tasks[int(self.task_ids[i])].enc_channels, 1)
+        walk = np.cumsum(rng.standard_normal((C, n), dtype=np.float64), axis=1)
+        z = (walk - walk.mean(axis=1, keepdims=True)) / walk.std(axis=1, keepdims=True)
+        z = z[0] if C == 1 else z
         return f32_to_bf16_bits(z.astype(np.float32))
 
     def packed_inputs(self) -> np.ndarray:
@@ -248,6 +254,8 @@ class Workload:
         names = [f"task{t:03d}.head.W", f"task{t:03d}.head.b"]
         if self.tasks[t].head_hidden:
             names += [f"task{t:03d}.head.W2", f"task{t:03d}.head.b2"]
+        if self.tasks[t].enc_channels > 1:
+            names += [f"task{t:03d}.enc.W", f"task{t:03d}.enc.b"]
         for l in range(self.bb.n_layers):
             for ad in ts.adapters:
                 names += [f"task{t:03d}.L{l:02d}.{ad.target}.A", f"task{t:03d}.L{l:02d}.{ad.target}.B"]
@@ -330,7 +338,8 @@ def _tasks_for(cfg: str, seed: int, T: int) -> List[TaskSpec]:
 def make_workload(cfg: str, *, n_layers: Optional[int] = None, batch: Optional[int] = None,
                   n_tasks: Optional[int] = None, dist: Optional[str] = None,
                   max_len: Optional[int] = None, adapters: bool = True,
-                  seed_offset: int = 0, lora_std: float = 0.02, mlp_hidden: int = 0) -> Workload:
+                  seed_offset: int = 0, lora_std: float = 0.02, mlp_hidden: int = 0,
+                  enc_channels: int = 0) -> Workload:
     """Build the workload of a BASELINE.json config (cfg1..cfg5).
 
     Overrides give the reduced variants the parity tests use (fewer layers, smaller batch);
@@ -358,6 +367,8 @@ def make_workload(cfg: str, *, n_layers: Optional[int] = None, batch: Optional[i
         tasks = [replace(t, adapters=()) for t in tasks]
     if mlp_hidden:
         tasks = [t if t.head_kind == "flatten" else replace(t, head_hidden=mlp_hidden) for t in tasks]
+    if enc_channels > 1:          # test variant (NEXT-1): every other task brings enc_channels input channels and a combiner
+        tasks = [replace(t, enc_channels=enc_channels) if i % 2 == 0 else t for i, t in enumerate(tasks)]
     rng = _stream(seed, "task_ids")
     if cfg == "cfg1":
         while True:                                   # reading #20: every task present

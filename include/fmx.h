@@ -129,6 +129,13 @@ typedef struct fmx_task_desc {
   int32_t head_hidden;
   const void *head_W2;
   const void *head_b2;
+  /* Per-task input encoder (Listing 2: LinearChannelCombiner(num_channels = 3, new_num_channels = 1);
+   * SURVEY.md 8(f) NEXT-1).  enc_channels <= 1: none.  enc_channels = C in [2, 16] (PATCH_LINEAR backbones with series
+   * input, img_c = 0, only): a request of this task brings C channels, packed channel-major [C, n_patches * patch_dim], and
+   * the series the backbone sees is  sum_c enc_W[c] * x[c, :] + enc_b.  enc_W DEVICE bf16 [C]; enc_b DEVICE bf16 [1] or NULL. */
+  int32_t enc_channels;
+  const void *enc_W;
+  const void *enc_b;
 } fmx_task_desc;
 
 /* ---- lifecycle ---------------------------------------------------------------------- */

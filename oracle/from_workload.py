@@ -22,7 +22,7 @@ def bb_dict(wl):
 
 def task_dicts(wl):
     return [dict(id=t, adapters={a.target: (a.rank, a.scaling) for a in ts.adapters},
-                 head_kind=ts.head_kind, head_out=ts.head_out, head_hidden=getattr(ts, "head_hidden", 0)) for t, ts in enumerate(wl.tasks)]
+                 head_kind=ts.head_kind, head_out=ts.head_out, head_hidden=getattr(ts, "head_hidden", 0), enc_channels=getattr(ts, "enc_channels", 0)) for t, ts in enumerate(wl.tasks)]
 
 
 def make_get(wl, max_cached_bytes=6 << 30):

@@ -134,9 +134,15 @@ def lora_linear(x, W, b, adapter):
 
 
 # ---------------------------------------------------------------- the definition
-def tokens_from_input(bb, get, x):
-    """Step 1: request input -> h0 [n, d]."""
+def tokens_from_input(bb, get, x, task=None):
+    """Step 1: request input -> h0 [n, d].  A task with an input encoder (Listing 2,
+    LinearChannelCombiner(num_channels = C, new_num_channels = 1)) first maps its C channels to the one series the backbone
+    takes: sum_c w[c] x[c, :] + b."""
     kind = bb["input_kind"]
+    if task is not None and task.get("enc_channels", 0) > 1:
+        C = task["enc_channels"]
+        p = f"task{task['id']:03d}.enc."
+        x = get(p + "W") @ np.asarray(x, dtype=np.float64).reshape(C, -1) + get(p + "b")[0]
     if kind == "embedded":
         return np.array(x, dtype=np.float64)
     if kind == "tokens":
@@ -232,7 +238,7 @@ def head_forward(bb, get, task, h):
 
 def forward_request(bb, get, task, x):
     """The vFM forward of ONE request: backbone + its task's adapter + its task's head."""
-    h = tokens_from_input(bb, get, x)
+    h = tokens_from_input(bb, get, x, task)
     for l in range(bb["n_layers"]):
         h = layer_forward(bb, get, task, l, h)
     return head_forward(bb, get, task, h)
@@ -241,7 +247,7 @@ def forward_request(bb, get, task, x):
 def forward_requests(bb, get, tasks, task_ids, inputs):
     """Every request separately; the layer loop is outermost only so that a caller's `get`
     may widen one layer's weights at a time (each request's arithmetic is untouched)."""
-    hs = [tokens_from_input(bb, get, x) for x in inputs]
+    hs = [tokens_from_input(bb, get, x, tasks[t]) for x, t in zip(inputs, task_ids)]
     for l in range(bb["n_layers"]):
         hs = [layer_forward(bb, get, tasks[t], l, h) for h, t in zip(hs, task_ids)]
     return [head_forward(bb, get, tasks[t], h) for h, t in zip(hs, task_ids)]

@@ -46,7 +46,8 @@ class AdapterDesc(C.Structure):
 class TaskDesc(C.Structure):
     _fields_ = [("n_adapters", C.c_int32), ("adapters", C.POINTER(AdapterDesc)), ("head_kind", C.c_int32),
                 ("head_out", C.c_int32), ("head_W", _vp), ("head_b", _vp),
-                ("head_hidden", C.c_int32), ("head_W2", _vp), ("head_b2", _vp)]
+                ("head_hidden", C.c_int32), ("head_W2", _vp), ("head_b2", _vp),
+                ("enc_channels", C.c_int32), ("enc_W", _vp), ("enc_b", _vp)]
 
 
 class BfqParams(C.Structure):
@@ -173,9 +174,10 @@ class Fmx:
         _check(self.lib.fmx_register_backbone(self.h, C.byref(d), C.byref(out)))
         return out.value
 
-    def register_task(self, bb, adapters, head_kind, head_out, head_W, head_b, head_hidden=0, head_W2=None, head_b2=None):
+    def register_task(self, bb, adapters, head_kind, head_out, head_W, head_b, head_hidden=0, head_W2=None, head_b2=None,
+                      enc_channels=0, enc_W=None, enc_b=None):
         """adapters: list of (target:int, rank:int, scaling:float, A_ptrs:list, B_ptrs:list).  head_hidden > 0: MLP head
-        (head_W [hidden, d_feat], head_b [hidden], head_W2 [head_out, hidden], head_b2 [head_out])."""
+        (head_W [hidden, d_feat], head_b [hidden], head_W2 [head_out, hidden], head_b2 [head_out]).  enc_channels > 1: input channel combiner (enc_W [C], enc_b [1])."""
         n = len(adapters)
         arr = (AdapterDesc * max(n, 1))()
         keep = []
@@ -184,7 +186,7 @@ class Fmx:
             keep += [a, b]
             arr[i].target, arr[i].rank, arr[i].scaling = tg, rank, scaling
             arr[i].A, arr[i].B = C.cast(a, _vpp), C.cast(b, _vpp)
-        d = TaskDesc(n, arr if n else None, head_kind, head_out, head_W, head_b, head_hidden, head_W2, head_b2)
+        d = TaskDesc(n, arr if n else None, head_kind, head_out, head_W, head_b, head_hidden, head_W2, head_b2, enc_channels, enc_W, enc_b)
         out = C.c_int32(-1)
         _check(self.lib.fmx_register_task(self.h, bb, C.byref(d), C.byref(out)))
         return out.value

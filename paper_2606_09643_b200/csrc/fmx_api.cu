@@ -53,6 +53,8 @@ struct TaskRec {
   int head_kind = 0, head_out = 0, head_hidden = 0;   // head_hidden > 0: MLP head, head_W is [head_hidden, d_feat]
   bf16 *head_W = nullptr, *head_b = nullptr;   // library-owned copies
   bf16 *head_W2 = nullptr, *head_b2 = nullptr; // MLP heads: [head_out, head_hidden], [head_out]
+  int enc_channels = 0;                        // per-task input encoder (channel combiner), 0 / 1 = none
+  bf16 *enc_W = nullptr, *enc_b = nullptr;     // [enc_channels], [1]
 };
 
 struct Backbone {
@@ -95,6 +97,8 @@ struct fmx_ctx {
   float *d_task_scale = nullptr;
   const bf16 **d_task_head_W = nullptr, **d_task_head_b = nullptr, **d_task_head_W2 = nullptr, **d_task_head_b2 = nullptr;
   int *d_task_head_w1 = nullptr;           // first-layer width of the head (= head_out for linear heads)
+  int *d_task_enc_ch = nullptr;            // input-encoder channels by task
+  const bf16 **d_task_enc_W = nullptr, **d_task_enc_b = nullptr;
   float *d_head_hid = nullptr; size_t head_hid_bytes = 0;       // hidden activations of MLP heads [B, max hidden]
   // pinned staging for ids / lengths: a ring (a slot is rewritten only after the copy that read it has run) plus one
   // buffer owned by the cached CUDA graph
@@ -542,6 +546,10 @@ int upload_task_tables(fmx_ctx *c, int t) {
   CU_OK(cudaMemcpy(c->d_task_head_W2 + t, &w2, sizeof(void *), cudaMemcpyHostToDevice));
   CU_OK(cudaMemcpy(c->d_task_head_b2 + t, &b2, sizeof(void *), cudaMemcpyHostToDevice));
   CU_OK(cudaMemcpy(c->d_task_head_w1 + t, &w1, sizeof(int), cudaMemcpyHostToDevice));
+  const bf16 *ew = r.enc_W, *eb = r.enc_b;
+  CU_OK(cudaMemcpy(c->d_task_enc_ch + t, &r.enc_channels, sizeof(int), cudaMemcpyHostToDevice));
+  CU_OK(cudaMemcpy(c->d_task_enc_W + t, &ew, sizeof(void *), cudaMemcpyHostToDevice));
+  CU_OK(cudaMemcpy(c->d_task_enc_b + t, &eb, sizeof(void *), cudaMemcpyHostToDevice));
   return FMX_OK;
 }
 
@@ -606,6 +614,9 @@ int fmx_create(fmx_ctx **out, int device_ordinal) {
   CU_OK(cudaMalloc(&c->d_task_head_W2, sizeof(void *) * FMX_MAX_TASKS));
   CU_OK(cudaMalloc(&c->d_task_head_b2, sizeof(void *) * FMX_MAX_TASKS));
   CU_OK(cudaMalloc(&c->d_task_head_w1, sizeof(int) * FMX_MAX_TASKS));
+  CU_OK(cudaMalloc(&c->d_task_enc_ch, sizeof(int) * FMX_MAX_TASKS));
+  CU_OK(cudaMalloc(&c->d_task_enc_W, sizeof(void *) * FMX_MAX_TASKS));
+  CU_OK(cudaMalloc(&c->d_task_enc_b, sizeof(void *) * FMX_MAX_TASKS));
   CU_OK(cudaMemset(c->d_task_coff, 0, sizeof(int) * FMX_MAX_TASKS));
   CU_OK(cudaMemset(c->d_task_head_kind, 0, sizeof(int) * FMX_MAX_TASKS));
   CU_OK(cudaMemset(c->d_task_head_out, 0, sizeof(int) * FMX_MAX_TASKS));
@@ -616,6 +627,9 @@ int fmx_create(fmx_ctx **out, int device_ordinal) {
   CU_OK(cudaMemset(c->d_task_head_W2, 0, sizeof(void *) * FMX_MAX_TASKS));
   CU_OK(cudaMemset(c->d_task_head_b2, 0, sizeof(void *) * FMX_MAX_TASKS));
   CU_OK(cudaMemset(c->d_task_head_w1, 0, sizeof(int) * FMX_MAX_TASKS));
+  CU_OK(cudaMemset(c->d_task_enc_ch, 0, sizeof(int) * FMX_MAX_TASKS));
+  CU_OK(cudaMemset(c->d_task_enc_W, 0, sizeof(void *) * FMX_MAX_TASKS));
+  CU_OK(cudaMemset(c->d_task_enc_b, 0, sizeof(void *) * FMX_MAX_TASKS));
   CU_OK(cudaMallocHost(&c->h_stage, sizeof(int) * 2 * FMX_MAX_REQUESTS * (fmx_ctx::kStageSlots + 1)));
   for (int i = 0; i < fmx_ctx::kStageSlots; ++i) CU_OK(cudaEventCreateWithFlags(&c->stage_ev[i], cudaEventDisableTiming));
   *out = c.release();
@@ -634,10 +648,11 @@ int fmx_destroy(fmx_ctx *c) {
     cudaFree(bp->embed_Wpad); cudaFree(bp->posb); cudaFree(bp->rope_cs); cudaFree(bp->rope_cs_t);
     for (int tg = 0; tg < 7; ++tg) { cudaFree(bp->slabA[tg]); cudaFree(bp->slabB[tg]); }
   }
-  for (auto &t : c->tasks) { cudaFree(t.head_W); cudaFree(t.head_b); cudaFree(t.head_W2); cudaFree(t.head_b2); }
+  for (auto &t : c->tasks) { cudaFree(t.head_W); cudaFree(t.head_b); cudaFree(t.head_W2); cudaFree(t.head_b2); cudaFree(t.enc_W); cudaFree(t.enc_b); }
   cudaFree(c->d_task_coff); cudaFree(c->d_task_head_kind); cudaFree(c->d_task_head_out); cudaFree(c->d_task_trpad);
   cudaFree(c->d_task_scale); cudaFree(c->d_task_head_W); cudaFree(c->d_task_head_b);
   cudaFree(c->d_task_head_W2); cudaFree(c->d_task_head_b2); cudaFree(c->d_task_head_w1); cudaFree(c->d_head_hid);
+  cudaFree(c->d_task_enc_ch); cudaFree(c->d_task_enc_W); cudaFree(c->d_task_enc_b);
   cudaFree(c->d_in_stage); cudaFree(c->d_out_stage); cudaFree(c->d_dbg_cu); cudaFree(c->d_head_part);
   if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
   for (int i = 0; i < fmx_ctx::kStageSlots; ++i) if (c->stage_ev[i]) cudaEventDestroy(c->stage_ev[i]);
@@ -755,6 +770,10 @@ int fmx_register_task(fmx_ctx *c, fmx_backbone_t h, const fmx_task_desc *desc, f
   if (desc->head_hidden < 0 || desc->head_hidden > 4096) return fmx_fail(FMX_E_SHAPE, "register_task: head_hidden %d not in [0,4096]", desc->head_hidden);
   if (desc->head_hidden > 0 && desc->head_kind == FMX_HEAD_FLATTEN) return fmx_fail(FMX_E_SHAPE, "register_task: an MLP head needs a pooled feature (mean / cls / last)");
   if (desc->head_hidden > 0 && !desc->head_W2) return fmx_fail(FMX_E_INVALID_ARG, "register_task: MLP head without head_W2");
+  if (desc->enc_channels < 0 || desc->enc_channels > 16) return fmx_fail(FMX_E_SHAPE, "register_task: enc_channels %d not in [0,16]", desc->enc_channels);
+  if (desc->enc_channels > 1 && (d.input_kind != FMX_INPUT_PATCH_LINEAR || d.img_c))
+    return fmx_fail(FMX_E_SHAPE, "register_task: an input encoder needs a PATCH_LINEAR backbone with series input");
+  if (desc->enc_channels > 1 && !desc->enc_W) return fmx_fail(FMX_E_INVALID_ARG, "register_task: input encoder without enc_W");
   bool seen[7] = {false};
   int rpad = 0;
   for (int i = 0; i < desc->n_adapters; ++i) {
@@ -814,6 +833,15 @@ int fmx_register_task(fmx_ctx *c, fmx_backbone_t h, const fmx_task_desc *desc, f
     CU_OK(cudaMalloc(&r.head_b, sizeof(bf16) * w1));
     CU_OK(cudaMemcpyAsync(r.head_b, desc->head_b, sizeof(bf16) * w1, cudaMemcpyDeviceToDevice, 0));
   }
+  if (desc->enc_channels > 1) {
+    r.enc_channels = desc->enc_channels;
+    CU_OK(cudaMalloc(&r.enc_W, sizeof(bf16) * desc->enc_channels));
+    CU_OK(cudaMemcpyAsync(r.enc_W, desc->enc_W, sizeof(bf16) * desc->enc_channels, cudaMemcpyDeviceToDevice, 0));
+    if (desc->enc_b) {
+      CU_OK(cudaMalloc(&r.enc_b, sizeof(bf16)));
+      CU_OK(cudaMemcpyAsync(r.enc_b, desc->enc_b, sizeof(bf16), cudaMemcpyDeviceToDevice, 0));
+    }
+  }
   if (desc->head_hidden > 0) {
     CU_OK(cudaMalloc(&r.head_W2, sizeof(bf16) * (size_t)desc->head_out * desc->head_hidden));
     CU_OK(cudaMemcpyAsync(r.head_W2, desc->head_W2, sizeof(bf16) * (size_t)desc->head_out * desc->head_hidden, cudaMemcpyDeviceToDevice, 0));
@@ -855,6 +883,8 @@ int fmx_unregister_task(fmx_ctx *c, fmx_task_t t) {
   cudaFree(r.head_b);
   cudaFree(r.head_W2);
   cudaFree(r.head_b2);
+  cudaFree(r.enc_W);
+  cudaFree(r.enc_b);
   r = TaskRec();
   if (int e = upload_task_tables(c, t)) return e;
   CU_OK(cudaDeviceSynchronize());
@@ -940,6 +970,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   }
   SortArgs sa{};
   sa.t = w.t; sa.B = B; sa.T = T; sa.n_tiles = w.n_tiles; sa.tile_rows = kPairRows; sa.task_head_out = c->d_task_head_out;
+  sa.task_enc_ch = (d.input_kind == FMX_INPUT_PATCH_LINEAR && !d.img_c) ? c->d_task_enc_ch : nullptr;
   if (d.input_kind == FMX_INPUT_EMBEDDED) { sa.in_per_tok = d.d_model; sa.in_per_req = 0; }
   else if (d.input_kind == FMX_INPUT_TOKEN_IDS) { sa.in_per_tok = 1; sa.in_per_req = 0; }
   else if (d.img_c) { sa.in_per_tok = 0; sa.in_per_req = (long long)d.img_c * d.img_hw * d.img_hw; }
@@ -1041,6 +1072,9 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     PackArgs pa{};
     pa.inputs = (const bf16 *)inputs; pa.perm = w.t.perm; pa.row_req = w.t.row_req; pa.row_pos = w.t.row_pos; pa.in_off = w.t.in_off;
     pa.N = Ni; pa.patch_dim = d.patch_dim; pa.Kp = bb.Kp; pa.has_cls = d.has_cls; pa.img_c = d.img_c; pa.img_hw = d.img_hw; pa.patch_hw = d.patch_hw;
+    pa.task_ids = w.t.task_ids; pa.task_enc_ch = c->d_task_enc_ch;
+    pa.task_enc_W = (const bf16 *const *)c->d_task_enc_W; pa.task_enc_b = (const bf16 *const *)c->d_task_enc_b;
+    pa.series_len = (d.tokens_per_request - (d.has_cls ? 1 : 0)) * d.patch_dim;
     pa.A = w.Hid;
     LAUNCH(Lh, F_EMBED, (launch_k(pack_patches_kernel, Ni, 128, 0, s, pa)));
     if ((e = encode_2d(c, &mPk, w.Hid, Ni, bb.Kp, bb.Kp, 128))) return e;

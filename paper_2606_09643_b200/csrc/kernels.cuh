@@ -33,6 +33,7 @@ struct SortArgs {
   int tile_rows;                   // rows of a GEMM row tile (256: one CTA-pair tile)
   long long in_per_tok, in_per_req;  // packed-input elements per token / per request
   const int *task_head_out;        // [T]
+  const int *task_enc_ch;          // [T] input channels of the task's encoder (<= 1: none): in_per_req is per channel
 };
 
 constexpr int kSortThreads = 1024;
@@ -139,7 +140,8 @@ __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortAr
   for (int i = tid; i <= T; i += blockDim.x) { const int v = t.cu_tok[s_cnt[i]]; s_tok[i] = v; t.task_tok_off[i] = v; }
   // (5) input / output offsets in ORIGINAL request order
   for (int i = tid; i < B; i += blockDim.x) {
-    t.in_off[i] = (long long)t.lengths[i] * a.in_per_tok + a.in_per_req;
+    const int ch = a.task_enc_ch ? max(a.task_enc_ch[t.task_ids[i]], 1) : 1;
+    t.in_off[i] = (long long)t.lengths[i] * a.in_per_tok + a.in_per_req * ch;
     t.out_off[i] = a.task_head_out[t.task_ids[i]];
   }
   if (tid == 0) { t.in_off[B] = 0; t.out_off[B] = 0; }
@@ -235,6 +237,10 @@ struct PackArgs {
   const long long *in_off;
   int N, patch_dim, Kp, has_cls;
   int img_c, img_hw, patch_hw;     // img_c = 0: input already [n_patches, patch_dim]
+  // per-task input encoder (series input only): channels, weights [C], bias [1] by task; task of each ORIGINAL request
+  const int *task_ids, *task_enc_ch;
+  const __nv_bfloat16 *const *task_enc_W, *const *task_enc_b;
+  int series_len;                  // n_patches * patch_dim (elements of one channel)
   __nv_bfloat16 *A;                // [N, Kp] task-sorted patch rows (CLS rows and the K pad are zero)
 };
 
@@ -256,7 +262,17 @@ __global__ void pack_patches_kernel(const PackArgs a) {
         const int c = e / (P * P), rem = e - c * P * P, py = rem / P, px = rem - py * P;
         v = src[((size_t)c * a.img_hw + gy * P + py) * a.img_hw + gx * P + px];
       } else {
-        v = src[(size_t)pi * a.patch_dim + e];
+        const int t = a.task_ids[i];
+        const int ch = a.task_enc_ch[t];
+        if (ch <= 1) {
+          v = src[(size_t)pi * a.patch_dim + e];
+        } else {                                            // LinearChannelCombiner: sum_c w[c] x[c, k] + b, fp32, one rounding
+          const __nv_bfloat16 *wc = a.task_enc_W[t], *bc = a.task_enc_b[t];
+          float acc = bc ? __bfloat162float(bc[0]) : 0.0f;
+          for (int cc = 0; cc < ch; ++cc)
+            acc = fmaf(__bfloat162float(wc[cc]), __bfloat162float(src[(size_t)cc * a.series_len + (size_t)pi * a.patch_dim + e]), acc);
+          v = __float2bfloat16(acc);
+        }
       }
     }
     dst[e] = v;

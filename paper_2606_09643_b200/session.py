@@ -77,9 +77,11 @@ class Session:
             Bm = [up(f"task{t:03d}.L{l:02d}.{ad.target}.B") for l in range(bb.n_layers)]
             adapters.append((TARGET[ad.target], ad.rank, float(ad.scaling), A, Bm))
         mlp = getattr(ts, "head_hidden", 0)
+        enc = getattr(ts, "enc_channels", 0)
         tid = self.fmx.register_task(self.bb, adapters, HEAD_KIND[ts.head_kind], ts.head_out,
                                      up(f"task{t:03d}.head.W"), up(f"task{t:03d}.head.b"), mlp,
-                                     up(f"task{t:03d}.head.W2") if mlp else None, up(f"task{t:03d}.head.b2") if mlp else None)
+                                     up(f"task{t:03d}.head.W2") if mlp else None, up(f"task{t:03d}.head.b2") if mlp else None,
+                                     enc, up(f"task{t:03d}.enc.W") if enc > 1 else None, up(f"task{t:03d}.enc.b") if enc > 1 else None)
         del tmp      # the library copied everything into its arena
         return tid
 

@@ -424,3 +424,29 @@ def test_mlp_head_on_a_flatten_feature_is_rejected(fmx_mod):
     with pytest.raises(fmx_mod.FmxError) as e:
         s.fmx.register_task(s.bb, [], 3, 4, W.data_ptr(), None, 128, W2.data_ptr(), None)
     assert "pooled" in str(e.value)
+
+
+@pytest.mark.parametrize("cfg,kw", [
+    ("cfg2", dict(n_layers=2, batch=24, enc_channels=3)),                       # every other task brings 3 channels + a combiner
+    ("cfg2", dict(n_layers=2, batch=9, enc_channels=5, mlp_hidden=128)),        # encoder + adapter + MLP decoder: Listing 2's pipeline
+    ("cfg5", dict(n_layers=2, batch=40, n_tasks=16, dist="uniform", enc_channels=2)),
+])
+def test_per_task_input_encoders_parity(fmx_mod, cfg, kw):
+    """per-task input encoders (the paper's LinearChannelCombiner, C channels -> 1) applied while the
+    patches are packed; requests of different tasks bring different numbers of channels, so the packed input is ragged."""
+    wl = make_workload(cfg, **kw)
+    assert any(t.enc_channels > 1 for t in wl.tasks) and any(t.enc_channels <= 1 for t in wl.tasks)
+    s = _session(fmx_mod, wl)
+    y = s.forward_numpy()
+    check_segments(s, wl)
+    check_parity(y, G.oracle_outputs(wl), f"{cfg} input encoders")
+
+
+def test_input_encoder_on_an_image_or_token_backbone_is_rejected(fmx_mod):
+    wl = make_workload("cfg4", n_layers=1, batch=2, max_len=64, n_tasks=2)
+    s = _session(fmx_mod, wl)
+    W = torch.zeros(1536 * 2, dtype=torch.bfloat16, device="cuda")
+    E3 = torch.zeros(3, dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(fmx_mod.FmxError) as e:
+        s.fmx.register_task(s.bb, [], 2, 2, W.data_ptr(), None, 0, None, None, 3, E3.data_ptr(), None)
+    assert "PATCH_LINEAR" in str(e.value)

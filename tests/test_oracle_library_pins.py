@@ -228,3 +228,24 @@ def test_mlp_head_matches_torch_sequential_and_reduces_to_the_linear_head():
     lin = O.head_forward(pos, W.__getitem__, dict(id=4, adapters={}, head_kind="mean", head_out=hidden), hp)
     mlp_out = O.head_forward(pos, W.__getitem__, dict(id=4, adapters={}, head_kind="mean", head_out=hidden, head_hidden=hidden), hp)
     assert (lin > 0).all() and np.allclose(lin, mlp_out, rtol=1e-13)
+
+
+# ---------------------------------------------------------------- per-task input encoder
+def test_input_channel_combiner_is_a_1x1_convolution_and_reduces_to_the_plain_path():
+    C, n_patches, pdim, d = 3, 6, 8, 12
+    r = _rng(31)
+    W = {"embed.W": r.standard_normal((d, pdim)), "embed.b": r.standard_normal(d), "embed.pos": r.standard_normal((n_patches, d)),
+         "task002.enc.W": r.standard_normal(C), "task002.enc.b": r.standard_normal(1)}
+    bb = dict(input_kind="patch", patch_dim=pdim, has_cls=False, has_pos=True, img_c=0, img_hw=0, patch_hw=0)
+    task = dict(id=2, adapters={}, head_kind="mean", head_out=1, enc_channels=C)
+    x = r.standard_normal((C, n_patches * pdim))
+    got = O.tokens_from_input(bb, W.__getitem__, x.reshape(-1), task)
+    conv = torch.nn.Conv1d(C, 1, kernel_size=1, **T64)              # LinearChannelCombiner(C -> 1) is a 1x1 convolution
+    with torch.no_grad():
+        conv.weight.copy_(_t(W["task002.enc.W"]).view(1, C, 1)); conv.bias.copy_(_t(W["task002.enc.b"]))
+        series = conv(_t(x)[None])[0, 0].numpy()
+    ref = O.tokens_from_input(bb, W.__getitem__, series)             # the plain single-channel path on the combined series
+    assert got.shape == (n_patches, d) and np.allclose(got, ref, rtol=1e-12, atol=1e-12)
+    # one-hot weights, zero bias: the encoder picks a channel
+    W["task002.enc.W"] = np.array([0.0, 1.0, 0.0]); W["task002.enc.b"] = np.zeros(1)
+    assert np.allclose(O.tokens_from_input(bb, W.__getitem__, x.reshape(-1), task), O.tokens_from_input(bb, W.__getitem__, x[1]))
