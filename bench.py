@@ -134,8 +134,8 @@ class ClockSampler:
 def build_workload(args):
     from fmx_workloads import make_workload
     if args.workload == "cfg5":
-        return make_workload("cfg5", n_tasks=args.tasks, dist=args.dist, adapters=not args.no_adapters, mlp_hidden=args.mlp_hidden)
-    return make_workload(args.workload, mlp_hidden=args.mlp_hidden)
+        return make_workload("cfg5", n_tasks=args.tasks, dist=args.dist, adapters=not args.no_adapters, mlp_hidden=args.mlp_hidden, enc_channels=args.enc_channels)
+    return make_workload(args.workload, mlp_hidden=args.mlp_hidden, enc_channels=args.enc_channels)
 
 
 # ------------------------------------------------------------------------------------- the oracle legs
@@ -372,7 +372,7 @@ def _measure(args, wl, rank, local_rank, world, with_cpu_baseline=True):
                        "tasks": len(wl.tasks), "tasks_in_batch": int(len(set(wl.task_ids.tolist()))), "dist": wl.notes.get("dist"),
                        "l2": "flushed (256 MB memset) between steps, outside the per-step events" if flush is not None else "no flush",
                        "accumulate": "fp32 (TMEM), fp32 residual stream", "replicas": world,
-                       **({"mlp_heads_hidden": args.mlp_hidden} if args.mlp_hidden else {}),
+                       **({"mlp_heads_hidden": args.mlp_hidden} if args.mlp_hidden else {}), **({"input_encoder_channels": args.enc_channels} if args.enc_channels else {}),
                        "launch": f"CUDA graph replay inside fmx_forward_mixed on {graph_steps} of {args.steps} timed steps" if graph_steps else "plain kernel launches"},
             "pct_bf16_tensor_peak": {"of_burst": round(100 * fl["total"] * world * args.steps / (ms_max * 1e-3) / 1e12 / pk["bf16_tflops"], 2),
                                      "of_sustained": round(100 * fl["total"] * world * args.steps / (ms_max * 1e-3) / 1e12 / pk["bf16_tflops_sustained"], 2),
@@ -433,6 +433,7 @@ def main():
     ap.add_argument("--tasks", type=int, default=92, help="cfg5: number of co-batched tasks")
     ap.add_argument("--dist", default="zipf0.8", choices=["uniform", "zipf0.8", "zipf1.5"])
     ap.add_argument("--no-adapters", action="store_true", help="cfg5: head-only tasks (adapter-free reference)")
+    ap.add_argument("--enc-channels", type=int, default=0, help="NEXT-1 variant: every other task brings this many input channels and a channel combiner (cfg2 / cfg5)")
     ap.add_argument("--mlp-hidden", type=int, default=0, help="NEXT-1 variant: pooled heads become MLP decoder heads of this hidden width")
     ap.add_argument("--no-flush", action="store_true")
     ap.add_argument("--no-graph", action="store_true", help="plain kernel launches in the timed region (FMX_OPT_GRAPH off)")
