@@ -381,6 +381,11 @@ def _measure(args, wl, rank, local_rank, world, with_cpu_baseline=True):
             "clocks": clocks, "roofline": roof, "breakdown": breakdown}
     if rank == 0:
         line["bfq"] = bfq_host_cost(wl)
+        # R2 lifecycle decoupling: take one task off the live context and put it back (the backbone and the other tasks stay)
+        un_ms, reg_ms = sess.task_lifecycle_ms(len(wl.tasks) - 1)
+        line["task_lifecycle"] = {"unregister_ms": round(un_ms, 3), "register_ms": round(reg_ms, 3), "task": len(wl.tasks) - 1,
+                                  "how": "fmx_unregister_task / fmx_register_task on the live context, tensors already on the device; "
+                                         "paper: 25 ms task load vs 5737 ms backbone load for MOMENT-Large on its T4 host (P:L387)"}
     if with_cpu_baseline and rank == 0 and world == 1 and not args.no_cpu_baseline:
         n = min(args.cpu_sample, B)
         idx = list(range(n))

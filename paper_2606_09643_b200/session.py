@@ -2,6 +2,8 @@
 
 Marshalling only — torch provides device memory and streams; every compute step is in libfmx.
 """
+import time
+
 import numpy as np
 import torch
 
@@ -78,12 +80,29 @@ class Session:
             adapters.append((TARGET[ad.target], ad.rank, float(ad.scaling), A, Bm))
         mlp = getattr(ts, "head_hidden", 0)
         enc = getattr(ts, "enc_channels", 0)
+        head = (up(f"task{t:03d}.head.W"), up(f"task{t:03d}.head.b"))
+        torch.cuda.synchronize(self.dev)
+        t0 = time.perf_counter()                         # the fmx_register_task call alone: tensors already on the device
         tid = self.fmx.register_task(self.bb, adapters, HEAD_KIND[ts.head_kind], ts.head_out,
-                                     up(f"task{t:03d}.head.W"), up(f"task{t:03d}.head.b"), mlp,
+                                     head[0], head[1], mlp,
                                      up(f"task{t:03d}.head.W2") if mlp else None, up(f"task{t:03d}.head.b2") if mlp else None,
                                      enc, up(f"task{t:03d}.enc.W") if enc > 1 else None, up(f"task{t:03d}.enc.b") if enc > 1 else None)
+        self.last_register_ms = (time.perf_counter() - t0) * 1e3
         del tmp      # the library copied everything into its arena
         return tid
+
+    def task_lifecycle_ms(self, t):
+        """Unregister and re-register workload task t on the live context (R2 lifecycle decoupling): the
+        backbone and every other task stay registered.  Returns (unregister_ms, register_ms) of the two C-ABI calls; the task
+        keeps its slot (lowest free slot first), so the session's id map stays valid."""
+        tid = self.task_ids_of[t]
+        torch.cuda.synchronize(self.dev)
+        t0 = time.perf_counter()
+        self.fmx.unregister_task(tid)
+        un_ms = (time.perf_counter() - t0) * 1e3
+        new = self._register_task(t)
+        assert new == tid, "a freed slot is reused lowest-first"
+        return un_ms, self.last_register_ms
 
     # ------------------------------------------------------------------ running
     def upload_inputs(self, packed=None):
