@@ -383,7 +383,9 @@ def _measure(args, wl, rank, local_rank, world, with_cpu_baseline=True):
         line["bfq"] = bfq_host_cost(wl)
         # R2 lifecycle decoupling: take one task off the live context and put it back (the backbone and the other tasks stay)
         un_ms, reg_ms = sess.task_lifecycle_ms(len(wl.tasks) - 1)
+        reg_busy_ms, fwd_ms, _ = sess.register_while_serving_ms(len(wl.tasks) - 1, n_forwards=5)
         line["task_lifecycle"] = {"unregister_ms": round(un_ms, 3), "register_ms": round(reg_ms, 3), "task": len(wl.tasks) - 1,
+                                  "register_ms_with_5_forwards_queued": round(reg_busy_ms, 3), "those_5_forwards_ms": round(fwd_ms, 2),
                                   "how": "fmx_unregister_task / fmx_register_task on the live context, tensors already on the device; "
                                          "paper: 25 ms task load vs 5737 ms backbone load for MOMENT-Large on its T4 host (P:L387)"}
     if with_cpu_baseline and rank == 0 and world == 1 and not args.no_cpu_baseline:

@@ -111,6 +111,9 @@ typedef struct fmx_adapter_desc {
 } fmx_adapter_desc;
 
 /* A task's extensions: PEFT adapter(s) + decoder head.
+ * fmx_register_task copies on the library's own registration stream and does not wait for forwards in flight (adding a
+ * task to a serving context costs ~1-2 ms, PAPER.md L92 / L243); the source tensors must be complete (the work that
+ * produced them finished) when the call is made.  Growing the LoRA slab arena (rare) synchronises the device.
  * Ownership: the library COPIES adapters and head into its own arena (task-sorted slabs laid
  * out for the segmented kernels); the caller may free its buffers when the call returns. */
 typedef struct fmx_task_desc {

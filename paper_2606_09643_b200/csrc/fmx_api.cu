@@ -116,6 +116,10 @@ struct fmx_ctx {
              stream == o.stream && gen == o.gen && ids == o.ids && lens == o.lens;
     }
   };
+  // registration runs on its own non-blocking stream: adding a task never waits for (or stalls) forwards in flight
+  cudaStream_t side = nullptr;
+  struct TaskStage { int coff, head_kind, head_out, w1, enc_ch; unsigned char trpad[8]; float scale[7]; const void *ptr[6]; };
+  TaskStage *h_task_stage = nullptr;       // pinned
   int opt_graph = 1;
   unsigned long long config_gen = 0;       // bumped by every registration change and option change
   CallKey last_key, graph_key;
@@ -489,6 +493,7 @@ int alloc_slab(fmx_ctx *c, Backbone &bb, int tg) {
   CU_OK(cudaMalloc(&bb.slabB[tg], nb * sizeof(bf16)));
   CU_OK(cudaMemset(bb.slabA[tg], 0, na * sizeof(bf16)));
   CU_OK(cudaMemset(bb.slabB[tg], 0, nb * sizeof(bf16)));
+  CU_OK(cudaDeviceSynchronize());           // rare path; the registration stream is not ordered after the legacy stream
   return rebuild_slab_maps(c, bb, tg);
 }
 
@@ -513,6 +518,7 @@ int grow_slabs(fmx_ctx *c, Backbone &bb, int new_cap) {
     bb.slabA[tg] = nA;
     bb.slabB[tg] = nB;
   }
+  CU_OK(cudaDeviceSynchronize());           // rare path: forwards in flight used the old slabs, the copies ran on the legacy stream
   bb.Rcap = new_cap;
   bb.col_used.resize(new_cap / 16, 0);
   for (int tg = 0; tg < 7; ++tg)
@@ -532,24 +538,29 @@ int find_columns(const Backbone &bb, int units) {        // first fit, units of 
 }
 
 int upload_task_tables(fmx_ctx *c, int t) {
+  // One task's entries of the device tables, through a pinned staging struct on the registration stream (no legacy-stream
+  // cudaMemcpy: that would wait for forwards running on the default stream).  The caller synchronises c->side afterwards.
   const TaskRec &r = c->tasks[t];
-  CU_OK(cudaMemcpy(c->d_task_coff + t, &r.coff, sizeof(int), cudaMemcpyHostToDevice));
-  CU_OK(cudaMemcpy(c->d_task_trpad + t * 7, r.trpad, 7, cudaMemcpyHostToDevice));
-  CU_OK(cudaMemcpy(c->d_task_scale + t * 7, r.scale, 7 * sizeof(float), cudaMemcpyHostToDevice));
-  CU_OK(cudaMemcpy(c->d_task_head_kind + t, &r.head_kind, sizeof(int), cudaMemcpyHostToDevice));
-  CU_OK(cudaMemcpy(c->d_task_head_out + t, &r.head_out, sizeof(int), cudaMemcpyHostToDevice));
-  const bf16 *w = r.head_W, *b = r.head_b;
-  CU_OK(cudaMemcpy(c->d_task_head_W + t, &w, sizeof(void *), cudaMemcpyHostToDevice));
-  CU_OK(cudaMemcpy(c->d_task_head_b + t, &b, sizeof(void *), cudaMemcpyHostToDevice));
-  const bf16 *w2 = r.head_W2, *b2 = r.head_b2;
-  const int w1 = r.head_hidden > 0 ? r.head_hidden : r.head_out;
-  CU_OK(cudaMemcpy(c->d_task_head_W2 + t, &w2, sizeof(void *), cudaMemcpyHostToDevice));
-  CU_OK(cudaMemcpy(c->d_task_head_b2 + t, &b2, sizeof(void *), cudaMemcpyHostToDevice));
-  CU_OK(cudaMemcpy(c->d_task_head_w1 + t, &w1, sizeof(int), cudaMemcpyHostToDevice));
-  const bf16 *ew = r.enc_W, *eb = r.enc_b;
-  CU_OK(cudaMemcpy(c->d_task_enc_ch + t, &r.enc_channels, sizeof(int), cudaMemcpyHostToDevice));
-  CU_OK(cudaMemcpy(c->d_task_enc_W + t, &ew, sizeof(void *), cudaMemcpyHostToDevice));
-  CU_OK(cudaMemcpy(c->d_task_enc_b + t, &eb, sizeof(void *), cudaMemcpyHostToDevice));
+  CU_OK(cudaStreamSynchronize(c->side));                   // the staging struct is free
+  fmx_ctx::TaskStage &h = *c->h_task_stage;
+  h.coff = r.coff; h.head_kind = r.head_kind; h.head_out = r.head_out; h.w1 = r.head_hidden > 0 ? r.head_hidden : r.head_out;
+  h.enc_ch = r.enc_channels;
+  memcpy(h.trpad, r.trpad, 7); memcpy(h.scale, r.scale, sizeof(r.scale));
+  h.ptr[0] = r.head_W; h.ptr[1] = r.head_b; h.ptr[2] = r.head_W2; h.ptr[3] = r.head_b2; h.ptr[4] = r.enc_W; h.ptr[5] = r.enc_b;
+  auto put = [&](void *dst, const void *src, size_t n) { return cudaMemcpyAsync(dst, src, n, cudaMemcpyHostToDevice, c->side); };
+  CU_OK(put(c->d_task_coff + t, &h.coff, sizeof(int)));
+  CU_OK(put(c->d_task_trpad + t * 7, h.trpad, 7));
+  CU_OK(put(c->d_task_scale + t * 7, h.scale, 7 * sizeof(float)));
+  CU_OK(put(c->d_task_head_kind + t, &h.head_kind, sizeof(int)));
+  CU_OK(put(c->d_task_head_out + t, &h.head_out, sizeof(int)));
+  CU_OK(put(c->d_task_head_w1 + t, &h.w1, sizeof(int)));
+  CU_OK(put(c->d_task_enc_ch + t, &h.enc_ch, sizeof(int)));
+  CU_OK(put(c->d_task_head_W + t, &h.ptr[0], sizeof(void *)));
+  CU_OK(put(c->d_task_head_b + t, &h.ptr[1], sizeof(void *)));
+  CU_OK(put(c->d_task_head_W2 + t, &h.ptr[2], sizeof(void *)));
+  CU_OK(put(c->d_task_head_b2 + t, &h.ptr[3], sizeof(void *)));
+  CU_OK(put(c->d_task_enc_W + t, &h.ptr[4], sizeof(void *)));
+  CU_OK(put(c->d_task_enc_b + t, &h.ptr[5], sizeof(void *)));
   return FMX_OK;
 }
 
@@ -632,6 +643,8 @@ int fmx_create(fmx_ctx **out, int device_ordinal) {
   CU_OK(cudaMemset(c->d_task_enc_b, 0, sizeof(void *) * FMX_MAX_TASKS));
   CU_OK(cudaMallocHost(&c->h_stage, sizeof(int) * 2 * FMX_MAX_REQUESTS * (fmx_ctx::kStageSlots + 1)));
   for (int i = 0; i < fmx_ctx::kStageSlots; ++i) CU_OK(cudaEventCreateWithFlags(&c->stage_ev[i], cudaEventDisableTiming));
+  CU_OK(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
+  CU_OK(cudaMallocHost(&c->h_task_stage, sizeof(fmx_ctx::TaskStage)));
   *out = c.release();
   fmx_clear_error();
   return FMX_OK;
@@ -657,6 +670,8 @@ int fmx_destroy(fmx_ctx *c) {
   if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
   for (int i = 0; i < fmx_ctx::kStageSlots; ++i) if (c->stage_ev[i]) cudaEventDestroy(c->stage_ev[i]);
   cudaFreeHost(c->h_stage);
+  cudaFreeHost(c->h_task_stage);
+  if (c->side) cudaStreamDestroy(c->side);
   delete c;
   return FMX_OK;
 }
@@ -814,9 +829,9 @@ int fmx_register_task(fmx_ctx *c, fmx_backbone_t h, const fmx_task_desc *desc, f
       for (int l = 0; l < L; ++l) {
         bf16 *A = bb->slabA[tg] + ((size_t)l * bb->Rcap + r.coff) * din;
         bf16 *B = bb->slabB[tg] + (size_t)l * dout * bb->Rcap + r.coff;
-        CU_OK(cudaMemcpyAsync(A, a.A[l], (size_t)a.rank * din * sizeof(bf16), cudaMemcpyDeviceToDevice, 0));
+        CU_OK(cudaMemcpyAsync(A, a.A[l], (size_t)a.rank * din * sizeof(bf16), cudaMemcpyDeviceToDevice, c->side));
         CU_OK(cudaMemcpy2DAsync(B, (size_t)bb->Rcap * sizeof(bf16), a.B[l], (size_t)a.rank * sizeof(bf16), (size_t)a.rank * sizeof(bf16),
-                                dout, cudaMemcpyDeviceToDevice, 0));
+                                dout, cudaMemcpyDeviceToDevice, c->side));
       }
       r.trpad[tg] = (unsigned char)((a.rank + 15) / 16 * 16);
       r.scale[tg] = a.scaling;
@@ -828,32 +843,32 @@ int fmx_register_task(fmx_ctx *c, fmx_backbone_t h, const fmx_task_desc *desc, f
   const size_t d_feat = desc->head_kind == FMX_HEAD_FLATTEN ? (size_t)d.tokens_per_request * d.d_model : (size_t)d.d_model;
   const size_t w1 = desc->head_hidden > 0 ? (size_t)desc->head_hidden : (size_t)desc->head_out;     // rows of the first layer
   CU_OK(cudaMalloc(&r.head_W, sizeof(bf16) * d_feat * w1));
-  CU_OK(cudaMemcpyAsync(r.head_W, desc->head_W, sizeof(bf16) * d_feat * w1, cudaMemcpyDeviceToDevice, 0));
+  CU_OK(cudaMemcpyAsync(r.head_W, desc->head_W, sizeof(bf16) * d_feat * w1, cudaMemcpyDeviceToDevice, c->side));
   if (desc->head_b) {
     CU_OK(cudaMalloc(&r.head_b, sizeof(bf16) * w1));
-    CU_OK(cudaMemcpyAsync(r.head_b, desc->head_b, sizeof(bf16) * w1, cudaMemcpyDeviceToDevice, 0));
+    CU_OK(cudaMemcpyAsync(r.head_b, desc->head_b, sizeof(bf16) * w1, cudaMemcpyDeviceToDevice, c->side));
   }
   if (desc->enc_channels > 1) {
     r.enc_channels = desc->enc_channels;
     CU_OK(cudaMalloc(&r.enc_W, sizeof(bf16) * desc->enc_channels));
-    CU_OK(cudaMemcpyAsync(r.enc_W, desc->enc_W, sizeof(bf16) * desc->enc_channels, cudaMemcpyDeviceToDevice, 0));
+    CU_OK(cudaMemcpyAsync(r.enc_W, desc->enc_W, sizeof(bf16) * desc->enc_channels, cudaMemcpyDeviceToDevice, c->side));
     if (desc->enc_b) {
       CU_OK(cudaMalloc(&r.enc_b, sizeof(bf16)));
-      CU_OK(cudaMemcpyAsync(r.enc_b, desc->enc_b, sizeof(bf16), cudaMemcpyDeviceToDevice, 0));
+      CU_OK(cudaMemcpyAsync(r.enc_b, desc->enc_b, sizeof(bf16), cudaMemcpyDeviceToDevice, c->side));
     }
   }
   if (desc->head_hidden > 0) {
     CU_OK(cudaMalloc(&r.head_W2, sizeof(bf16) * (size_t)desc->head_out * desc->head_hidden));
-    CU_OK(cudaMemcpyAsync(r.head_W2, desc->head_W2, sizeof(bf16) * (size_t)desc->head_out * desc->head_hidden, cudaMemcpyDeviceToDevice, 0));
+    CU_OK(cudaMemcpyAsync(r.head_W2, desc->head_W2, sizeof(bf16) * (size_t)desc->head_out * desc->head_hidden, cudaMemcpyDeviceToDevice, c->side));
     if (desc->head_b2) {
       CU_OK(cudaMalloc(&r.head_b2, sizeof(bf16) * desc->head_out));
-      CU_OK(cudaMemcpyAsync(r.head_b2, desc->head_b2, sizeof(bf16) * desc->head_out, cudaMemcpyDeviceToDevice, 0));
+      CU_OK(cudaMemcpyAsync(r.head_b2, desc->head_b2, sizeof(bf16) * desc->head_out, cudaMemcpyDeviceToDevice, c->side));
     }
   }
   c->tasks[slot] = r;
   c->n_slots = std::max(c->n_slots, slot + 1);
   if (int e = upload_task_tables(c, slot)) return e;
-  CU_OK(cudaDeviceSynchronize());
+  CU_OK(cudaStreamSynchronize(c->side));                   // the caller may free its buffers; forwards in flight are not waited for
   *out = slot;
   return FMX_OK;
 }
@@ -873,8 +888,8 @@ int fmx_unregister_task(fmx_ctx *c, fmx_task_t t) {
     for (int l = 0; l < L; ++l) {      // leave unowned columns zero
       bf16 *A = bb->slabA[tg] + ((size_t)l * bb->Rcap + r.coff) * bb->din[tg];
       bf16 *B = bb->slabB[tg] + (size_t)l * bb->dout[tg] * bb->Rcap + r.coff;
-      CU_OK(cudaMemsetAsync(A, 0, (size_t)r.trpad[tg] * bb->din[tg] * sizeof(bf16), 0));
-      CU_OK(cudaMemset2DAsync(B, (size_t)bb->Rcap * sizeof(bf16), 0, (size_t)r.trpad[tg] * sizeof(bf16), bb->dout[tg], 0));
+      CU_OK(cudaMemsetAsync(A, 0, (size_t)r.trpad[tg] * bb->din[tg] * sizeof(bf16), c->side));
+      CU_OK(cudaMemset2DAsync(B, (size_t)bb->Rcap * sizeof(bf16), 0, (size_t)r.trpad[tg] * sizeof(bf16), bb->dout[tg], c->side));
     }
     bb->n_adapters[tg]--;
   }
@@ -887,7 +902,7 @@ int fmx_unregister_task(fmx_ctx *c, fmx_task_t t) {
   cudaFree(r.enc_b);
   r = TaskRec();
   if (int e = upload_task_tables(c, t)) return e;
-  CU_OK(cudaDeviceSynchronize());
+  CU_OK(cudaStreamSynchronize(c->side));
   return FMX_OK;
 }
 

@@ -65,11 +65,13 @@ class Session:
                        embed_table=self._w("embed.table") if bb.input_kind == "tokens" else None)
         return self.fmx.register_backbone(fields, per_layer, singles)
 
-    def _register_task(self, t):
+    def _register_task(self, t, presynced=None):
         wl, bb = self.wl, self.wl.bb
         ts = wl.tasks[t]
         tmp = []
         def up(name):
+            if presynced is not None:                     # tensors uploaded (and synchronised) earlier
+                return presynced[name].data_ptr()
             x = _dev_bf16(wl.tensor(name), self.dev)
             tmp.append(x)
             return x.data_ptr()
@@ -81,7 +83,8 @@ class Session:
         mlp = getattr(ts, "head_hidden", 0)
         enc = getattr(ts, "enc_channels", 0)
         head = (up(f"task{t:03d}.head.W"), up(f"task{t:03d}.head.b"))
-        torch.cuda.synchronize(self.dev)
+        if presynced is None:
+            torch.cuda.synchronize(self.dev)
         t0 = time.perf_counter()                         # the fmx_register_task call alone: tensors already on the device
         tid = self.fmx.register_task(self.bb, adapters, HEAD_KIND[ts.head_kind], ts.head_out,
                                      head[0], head[1], mlp,
@@ -90,6 +93,25 @@ class Session:
         self.last_register_ms = (time.perf_counter() - t0) * 1e3
         del tmp      # the library copied everything into its arena
         return tid
+
+    def _register_task_presynced(self, t):
+        """Upload workload task t's tensors, synchronise, and only then (when called) register: used to time the call while
+        other work is queued on the device."""
+        if not hasattr(self, "_pre"):
+            self._pre = {}
+        if t not in self._pre:
+            names = self.wl.task_tensor_names(t)
+            self._pre[t] = {n: _dev_bf16(self.wl.tensor(n), self.dev) for n in names}
+            torch.cuda.synchronize(self.dev)
+        return self._register_task(t, presynced=self._pre[t])
+
+    def prepare_task_copy(self, t):
+        """Upload (and synchronise) workload task t's tensors ahead of register_while_serving_ms."""
+        if not hasattr(self, "_pre"):
+            self._pre = {}
+        names = self.wl.task_tensor_names(t)
+        self._pre[t] = {n: _dev_bf16(self.wl.tensor(n), self.dev) for n in names}
+        torch.cuda.synchronize(self.dev)
 
     def task_lifecycle_ms(self, t):
         """Unregister and re-register workload task t on the live context (R2 lifecycle decoupling): the
@@ -103,6 +125,25 @@ class Session:
         new = self._register_task(t)
         assert new == tid, "a freed slot is reused lowest-first"
         return un_ms, self.last_register_ms
+
+    def register_while_serving_ms(self, t, n_forwards=5, stream=None):
+        """NEXT-2: add one more task (a copy of workload task t in a fresh slot) while `n_forwards` forwards
+        are queued on the stream; returns (register_ms, forwards_ms, new task id).  fmx_register_task runs on the library's
+        own stream and returns without waiting for the queued forwards."""
+        s = stream if stream is not None else torch.cuda.current_stream(self.dev)
+        if not hasattr(self, "_pre") or t not in self._pre:
+            self.prepare_task_copy(t)
+        self.forward(stream=s)
+        s.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(s)
+        for _ in range(n_forwards):
+            self.forward(stream=s)
+        e1.record(s)
+        tid = self._register_task_presynced(t)
+        reg_ms = self.last_register_ms
+        s.synchronize()
+        return reg_ms, e0.elapsed_time(e1), tid
 
     # ------------------------------------------------------------------ running
     def upload_inputs(self, packed=None):
