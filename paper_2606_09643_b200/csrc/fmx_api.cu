@@ -355,7 +355,7 @@ void launch_pair_gemm(fmx_ctx *c, cudaStream_t s, const PairGemmParams &p) {
 }
 
 // Every request <= 64 tokens: the pipelined single-tile kernel (4 CTAs per SM, each walking a strided item list).
-int g_reverse = 1;       // consecutive kernels of a layer walk the rows in alternating directions (L2 reuse, DESIGN.md 5.1h)
+int g_reverse = 1;       // consecutive kernels of a layer walk the rows in alternating directions (L2 reuse, DESIGN.md 5.1g)
 int g_attn_short = 2;    // 0: generic kernel, 1: pipelined mma.sync kernel, 2: tcgen05 head-pair kernel where it applies (d_h 64, even H_q)
 bool attn_pair64_ok(int dh, int n_q_heads, int max_len) { return g_attn_short == 2 && dh == 64 && n_q_heads % 2 == 0 && max_len <= 64; }
 void launch_attention_pair64(cudaStream_t s, int sm_count, const AttnPairArgs &a) {

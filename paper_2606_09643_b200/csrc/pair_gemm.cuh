@@ -59,7 +59,7 @@ struct PairGemmParams {
   int n_ptiles;            // ceil(M / 256)
   int expand_wide;         // 1: same-source whole tiles run their LoRA expand as one N = 256 step per block (A/B knob)
   int reverse;             // 1: row tiles are walked from the last to the first (the producer of this GEMM's input wrote
-                           // ascending: its most recent rows are the ones still in L2, see DESIGN.md 5.1h)
+                           // ascending: its most recent rows are the ones still in L2, see DESIGN.md 5.1g)
   int n_full;              // kBN = 256: tiles [0, n_full) are 256 x 256; each later tile is cut into two 256 x 128 halves
                            // taken by different pairs, so a short last wave costs half a tile time (-1 = no half tiles)
   int mode;                // GemmMode (not GM_SHRINK)
