@@ -118,3 +118,63 @@ def test_token_level_charging():
     assert [h for _, _, h in q.next_batch(0.0, 99)] == [1, 0, 2]
     q.complete(24.0)               # 1200 tokens -> 0.02 ms/token: 100-token requests cost 2, the 1000-token one 20
     assert q.F_last == [20.0, 4.0] and q.service_ms == [20.0, 4.0]
+
+
+# ------------------------------------------------------------------------------------------------
+# S0 parity of the PRODUCT code: the C++ builder (fmx_bfq_*, csrc/bfq.cpp) against oracle/bfq.py in
+# lock-step on seeded traces (Eq. 1-3).  Tag arithmetic is IEEE
+# double in the same order on both sides, so every comparison is `==`, not a tolerance.  Host only.
+def _lockstep(seed, T, b_max, slo_choices, l_tok, steps=300):
+    from paper_2606_09643_b200.binding import Bfq
+    rng = np.random.default_rng(seed)
+    lat = np.cumsum(rng.uniform(0.5, 3.0, b_max)).tolist()          # increasing latency profile Lat(1..b_max)
+    o = BFQ(T, b_max, lat, l_tok_ms=l_tok)
+    c = Bfq(T, b_max, lat, l_tok_ms=l_tok)
+    for t in range(T):
+        w = float(rng.choice([0.5, 1.0, 2.0, 3.0]))
+        slo = float(rng.choice(slo_choices))
+        o.set_task(t, w, slo); c.set_task(t, w, slo)
+    h, now = 0, 0.0
+    n_batches = n_nonempty = 0
+    for step in range(steps):
+        now += float(rng.uniform(0.0, 4.0))
+        for _ in range(int(rng.integers(0, 2 * b_max + 1))):
+            t = int(rng.integers(0, T))
+            n = int(rng.integers(1, 1025)) if l_tok > 0 else int(rng.integers(1, 9))
+            arr = now - float(rng.uniform(0.0, 2.0))
+            o.enqueue(t, h, n, arr); c.enqueue(t, h, n, arr); h += 1
+        # every queued request's (S, F, v_arr), every task
+        for t in range(T):
+            d, s_ms, queued = c.stats(t)
+            assert queued == len(o.queue[t]) and d == o.dispatched[t] and s_ms == o.service_ms[t]
+            for j, r in enumerate(o.queue[t]):
+                assert c.peek(t, j) == (r["S"], r["F"], r["v_arr"]), (seed, step, t, j)
+        cap = int(rng.choice([0, 1, b_max // 2 + 1, b_max, b_max + 3]))
+        ref = o.next_batch(now, cap)
+        ids, lens, handles = c.next_batch(now, cap)
+        assert [(int(a), int(b), int(d)) for a, b, d in zip(ids, lens, handles)] == ref, (seed, step)
+        n_batches += 1; n_nonempty += bool(ref)
+        measured = 0.0 if rng.random() < 0.5 else float(rng.uniform(0.5, 40.0))
+        o.complete(measured); c.complete(measured)
+    for t in range(T):                                                # after the last retag
+        for j, r in enumerate(o.queue[t]):
+            assert c.peek(t, j) == (r["S"], r["F"], r["v_arr"])
+        assert c.stats(t) == (o.dispatched[t], o.service_ms[t], len(o.queue[t]))
+    assert n_nonempty > steps // 4                                    # the trace really exercised the builder
+    return n_batches
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_cpp_builder_equals_oracle_in_lockstep(seed):
+    rng = np.random.default_rng(1000 + seed)
+    T = int(rng.integers(1, 9))
+    b_max = int(rng.integers(1, 9))
+    slo_choices = [[math.inf], [math.inf, 30.0, 12.0], [30.0, 12.0]][seed % 3]
+    l_tok = 0.0 if seed % 2 == 0 else 0.01                            # both charging modes
+    _lockstep(seed, T, b_max, slo_choices, l_tok)
+
+
+def test_cpp_builder_equals_oracle_at_serving_scale():
+    """92 tasks, B_max 512 (configs[4]'s batch), token charging: the shapes bench.py's `bfq` leg uses."""
+    _lockstep(77, 92, 512, [math.inf, 500.0], 0.01, steps=12)
+    _lockstep(78, 92, 512, [math.inf], 0.0, steps=12)
