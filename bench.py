@@ -1,33 +1,35 @@
 #!/usr/bin/env python
 """bench.py — throughput of the mixed-task vFM forward (fmx_forward_mixed) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2|cfg3|cfg4|cfg5|sweep5]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload headline|cfg2|cfg3|cfg4|cfg5|sweep5]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
     python bench.py --impl reference ...        # the fp64 CPU oracle on the host cores
 
-A step is one pass of the whole hot path (S1 task sort .. S6 output scatter) over
-one synthetic mixed batch.  The default workload is BASELINE.json configs[1] ("cfg2": T5-large-
-encoder-shaped time-series backbone, batch 256, 10 tasks, Zipf(1.1) task ids); configs[0] is the
-tiny parity case and the other configs are selectable with --workload.  Rank 0 prints ONE JSON line.
+A step is one pass of the whole hot path (S1 task sort .. S6 output scatter) over one synthetic mixed batch.
+BASELINE.json's metric is "mixed-task samples/s per B200 and % of bf16 tensor peak vs #co-batched tasks": it is quoted on
+configs[4] (the task-count sweep on the cfg2 backbone, batch 512).  The default workload ("headline") is therefore
+configs[4] at 92 co-batched tasks, task ids Zipf(0.8); the SAME run also measures the single-task batch and the adapter-free
+batch of the same size (`vs_single_task`, `vs_adapter_free`: north_star's "within 10 % of a single-task batch") and the three
+other full-size configs (`per_config`: cfg2 / cfg3 / cfg4 with value, ms_per_step, % of peak and per-GEMM-family TFLOP/s).
+Rank 0 prints ONE JSON line.
 
-  value      whole-job samples/s, inputs resident in HBM, CUDA events around every step on the
-             launching stream, L2 flushed (256 MB memset) between steps outside the events.  The
-             step is the C-ABI call fmx_forward_mixed on a non-default stream; the call is identical
-             every step, so the library replays its cached CUDA graph (FMX_OPT_GRAPH; --no-graph
-             times plain launches).
-  e2e        the same metric through fmx_forward_mixed_host: pinned HOST inputs -> device, forward,
-             outputs -> HOST, inside the timed region (wall clock around the synchronous calls).
-  roofline   the tcgen05 pair GEMM kernel (all four projection families): algorithmic FLOPs per
-             launch / average launch duration from CUDA events recorded around those launches in K
-             more steps of the same loop right after the timed ones (per-launch events need plain
-             launches, so they cannot share steps with the graph), against MEASURED_PEAKS.json
-             (sustained bf16 figure: the kernel is timed inside a long step; the burst fraction is
-             given too).  When the LoRA shrink runs fused inside those launches its algorithmic FLOPs
-             are counted with them.
+  value      whole-job samples/s, inputs resident in HBM, CUDA events around every step on the launching stream, L2 flushed
+             (256 MB memset) between steps outside the events.  The step is the C-ABI call fmx_forward_mixed on a non-default
+             stream; the call is identical every step, so the library replays its cached CUDA graph (--no-graph: plain
+             launches).  `no_graph` gives the same K steps as plain kernel launches right after.
+  breakdown  a third pass of K steps, plain launches with CUDA events around EVERY kernel launch (on the launching stream):
+             per-family launches and ms per step, plus `ms_per_step` of that pass - the family times are parts of it, so
+             their sum is <= it.
+  roofline   the tcgen05 pair GEMM (all four projection families), from the SAME pass as `breakdown`: algorithmic FLOPs per
+             launch / average launch duration.  avg_launch_ms x launches_per_step = the GEMM families' ms in `breakdown`.
+             `peak` is MEASURED_PEAKS.json's burst bf16 figure unless the SM clock sampled during the pass sat at the
+             sustained level (then the sustained figure); both fractions are printed.
+  e2e        the same metric through fmx_forward_mixed_host: pinned HOST inputs -> device, forward, outputs -> HOST, inside the
+             timed region (wall clock around the synchronous calls).
   cpu_baseline  the oracle (numpy fp64, as it stands) on a bounded sample of the same workload.
 
-Multi-GPU is replicas only: every rank runs the same batch shape on its own GPU, no
-data-path collective; value = units of all ranks / max-over-ranks time; scaling "weak".
+Multi-GPU is replicas only: every rank runs the same batch shape on its own GPU, no data-path collective;
+value = units of all ranks / max-over-ranks time; scaling "weak".
 """
 import argparse
 import json
@@ -43,7 +45,11 @@ if ROOT not in sys.path:
 
 METRIC = "mixed-task samples/s per B200 and % of bf16 tensor peak vs #co-batched tasks"
 GEMM_FAMILIES = ("gemm_qkv", "gemm_o", "gemm_ffn_in", "gemm_ffn_out")
+HEADLINE = dict(tasks=92, dist="zipf0.8")
 WORKLOAD_NAMES = {
+    "headline": "configs[4]: task-count/skew sweep on the cfg2 backbone (24L d1024 FFN4096 ReLU RMSNorm, T5-large-encoder-shaped), "
+                "batch 512 x 64 tokens, 92 co-batched tasks (every task present), LoRA rank {4,8,16,32,64} per task on q/k/v/o, "
+                "forecast (flatten->96) / mean-pool heads alternating, task ids Zipf(0.8)",
     "cfg2": "configs[1]: T5-large-encoder-shaped time-series backbone (24L d1024 FFN4096 ReLU RMSNorm), batch 256 x 64 tokens, "
             "10 tasks, rank-8 LoRA on q/k/v/o, forecast (flatten->96) or mean-pool heads, task ids Zipf(1.1)",
     "cfg3": "configs[2]: ViT-L/14-shaped vision backbone, batch 128 x 257 tokens, 32 tasks, rank 8/16 LoRA on q/k/v/o, CLS heads",
@@ -72,8 +78,9 @@ def peaks():
     if os.path.exists(p):
         d = json.load(open(p))
         return dict(source="measured", hbm_gbs=float(d["hbm_gbs"]), bf16_tflops=float(d["bf16_tflops"]),
-                    bf16_tflops_sustained=float(d.get("bf16_tflops_sustained", d["bf16_tflops"])))
-    return dict(source="fallback", hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0)
+                    bf16_tflops_sustained=float(d.get("bf16_tflops_sustained", d["bf16_tflops"])),
+                    sustained_sm_mhz=(d.get("clocks_under_load") or {}).get("sm_mhz_median"))
+    return dict(source="fallback (B200_PROFILING.md)", hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, sustained_sm_mhz=None)
 
 
 class ClockSampler:
@@ -133,6 +140,8 @@ class ClockSampler:
 
 def build_workload(args):
     from fmx_workloads import make_workload
+    if args.workload == "headline":
+        return make_workload("cfg5", n_tasks=HEADLINE["tasks"], dist=HEADLINE["dist"])
     if args.workload == "cfg5":
         return make_workload("cfg5", n_tasks=args.tasks, dist=args.dist, adapters=not args.no_adapters, mlp_hidden=args.mlp_hidden, enc_channels=args.enc_channels)
     return make_workload(args.workload, mlp_hidden=args.mlp_hidden, enc_channels=args.enc_channels)
@@ -242,80 +251,125 @@ def timed_steps(sess, torch, steps, flush):
     return sum(a.elapsed_time(b) for a, b in zip(e0, e1))
 
 
-def measure(args, wl, rank, local_rank, world, with_cpu_baseline=True):
+def measure(args, wl, rank, local_rank, world, full=True, steps=None, weights_from=None, label=None):
     """Everything runs on one non-default stream: fmx_forward_mixed replays its cached CUDA graph there (FMX_OPT_GRAPH)."""
     import torch
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: libfmx has no CPU fallback (use --impl reference for the oracle)")
     torch.cuda.set_device(local_rank)
     with torch.cuda.stream(torch.cuda.Stream(torch.device("cuda", local_rank))):
-        return _measure(args, wl, rank, local_rank, world, with_cpu_baseline)
+        return _measure(args, wl, rank, local_rank, world, full, steps or args.steps, weights_from, label or args.workload)
 
 
-def _measure(args, wl, rank, local_rank, world, with_cpu_baseline=True):
+def _measure(args, wl, rank, local_rank, world, full, steps, weights_from, label):
+    """One workload.  full = the headline treatment (e2e, BFQ cost, task lifecycle, oracle baseline); otherwise the three timed
+    passes only.  Returns (line, session) - the session keeps the device weights alive for a run that shares the backbone."""
     import numpy as np
     import torch
     from paper_2606_09643_b200 import accounting, replicas
     from paper_2606_09643_b200.session import Session
 
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device: libfmx has no CPU fallback (use --impl reference for the oracle)")
     dev = torch.device("cuda", local_rank)
-    torch.cuda.set_device(dev)
     pk = peaks()
-    sess = Session(wl, device=local_rank)
+    sess = Session(wl, device=local_rank, weights_from=weights_from)
     sess.upload_inputs()
     fl = accounting.flops(wl)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if not args.no_flush else None
     B = wl.n_req
+    warm = max(args.warmup, 3)
 
     sampler = ClockSampler(local_rank) if rank == 0 else None
-    for _ in range(max(args.warmup, 3)):
+    sess.fmx.set_option("graph", 0 if args.no_graph else 1)
+    for _ in range(warm):
+        if flush is not None:
+            flush.zero_()
         sess.forward()
     torch.cuda.synchronize()
     launches_per_step = sess.fmx.last_launch_count()
 
-    # ---- timed region: exactly K steps through fmx_forward_mixed (which replays its cached CUDA graph: the call is
-    # identical every step), then K more steps of the same loop with CUDA events around the GEMM launches (the roofline's
-    # kernel; per-launch events need plain launches, so they cannot share steps with the graph).  The clock sampler
-    # covers both.
-    sess.fmx.set_option("graph", 0 if args.no_graph else 1)
-    for _ in range(2):
-        sess.forward()
+    # ---- pass 1, the timed region: exactly K steps through fmx_forward_mixed (graph replay: the call is identical every step)
     replicas.barrier()
     torch.cuda.synchronize()
     if sampler:
         sampler.start()
     replays0 = sess.fmx.graph_replays()
-    ms_total = timed_steps(sess, torch, args.steps, flush)
+    ms_total = timed_steps(sess, torch, steps, flush)
     torch.cuda.synchronize()
     replicas.barrier()
     graph_steps = sess.fmx.graph_replays() - replays0
-    gemm_prof, ms_prof_steps = {}, 0.0
+    ms_max = replicas.max_over_ranks(ms_total, dev if world > 1 else None)
+    value = replicas.whole_job_throughput(B, steps, ms_max, world)
+
+    # ---- pass 2: the same K steps as plain kernel launches (what a serving loop whose batch changes every step gets)
+    sess.fmx.set_option("graph", 0)
+    sess.forward()
+    ms_plain = timed_steps(sess, torch, steps, flush)
+    ms_plain_max = replicas.max_over_ranks(ms_plain, dev if world > 1 else None)
+
+    # ---- pass 3: K steps, plain launches, CUDA events around EVERY launch: breakdown by family + the GEMM roofline
+    breakdown, roof, ms_prof = {}, None, 0.0
     if not args.no_kernel_events:
-        sess.fmx.profile_select(GEMM_FAMILIES)
+        sess.fmx.profile_select(None)
         sess.fmx.profile_enable(True)
-        ms_prof_steps = timed_steps(sess, torch, args.steps, flush)
+        ms_prof = timed_steps(sess, torch, steps, flush)
         torch.cuda.synchronize()
-        gemm_prof = sess.fmx.profile_read()
+        fam = sess.fmx.profile_read()
         sess.fmx.profile_enable(False)
+        breakdown = {k: {"launches_per_step": n // steps, "ms_per_step": round(ms / steps, 4)} for k, (n, ms) in fam.items() if n}
     if sampler:
         sampler.stop()
-    ms_max = replicas.max_over_ranks(ms_total, dev if world > 1 else None)
-    value = replicas.whole_job_throughput(B, args.steps, ms_max, world)
     clocks = sampler.result() if sampler else None
+    sess.fmx.set_option("graph", 0 if args.no_graph else 1)
 
-    # ---- per-family breakdown (extra profiled steps, outside the timed region) ----
-    sess.fmx.profile_select(None)
-    sess.fmx.profile_enable(True)
-    n_prof = 3
-    for _ in range(n_prof):
-        if flush is not None:
-            flush.zero_()
-        sess.forward()
-    fam = sess.fmx.profile_read()
-    sess.fmx.profile_enable(False)
-    breakdown = {k: {"launches_per_step": n // n_prof, "ms_per_step": round(ms / n_prof, 4)} for k, (n, ms) in fam.items() if n}
+    # ---- roofline of the dominant kernel (tcgen05 pair GEMM, all four projection families), from pass 3 ----
+    if breakdown:
+        n_l = sum(fam[f][0] for f in GEMM_FAMILIES)
+        ms_g = sum(fam[f][1] for f in GEMM_FAMILIES)
+        fused = "lora_shrink" not in breakdown      # the LoRA shrink ran as work items of the GEMM launches (no shrink family)
+        fam_fl = {f: fl["families"][f] + (fl["shrink_families"][f] if fused else 0.0) for f in GEMM_FAMILIES}
+        fl_g = sum(fam_fl.values())                                     # per forward
+        avg_ms = ms_g / max(n_l, 1)
+        flops_per_launch = fl_g / accounting.gemm_launches_per_forward(wl)
+        achieved = flops_per_launch / (avg_ms * 1e-3) / 1e12
+        # which measured peak applies: the burst figure, unless the SM clock during these passes sat at the level the
+        # driver recorded for its 4-second sustained matmul (MEASURED_PEAKS.json clocks_under_load)
+        sm = (clocks or {}).get("sm_mhz")
+        sus = pk.get("sustained_sm_mhz")
+        at_sustained = bool(sm and sus and sm <= 1.10 * sus)
+        peak = pk["bf16_tflops_sustained"] if at_sustained else pk["bf16_tflops"]
+        roof = {"kernel": "fmx::pair_gemm_kernel<256> (tcgen05 cta_group::2 / TMEM / TMA, fused LoRA expand)", "bound": "tensor",
+                "achieved": round(achieved, 2), "peak": peak, "unit": "TFLOP/s", "frac": round(achieved / peak, 4),
+                "peak_kind": f"{pk['source']} {'sustained' if at_sustained else 'burst'} bf16 (median SM clock in the passes {sm} MHz; "
+                             f"the driver's sustained matmul ran at {sus} MHz)",
+                "frac_of_burst_peak": round(achieved / pk["bf16_tflops"], 4),
+                "frac_of_sustained_peak": round(achieved / pk["bf16_tflops_sustained"], 4),
+                "traffic": gemm_traffic(label), "traffic_unit": "DRAM bytes per launch (ncu --set full, cold cache; profiles/gemm_traffic.csv)",
+                "flops_per_launch": flops_per_launch, "avg_launch_ms": round(avg_ms, 5), "launches_per_step": n_l // steps,
+                "gemm_ms_per_step": round(ms_g / steps, 4), "share_of_step": round(ms_g / ms_prof, 4),
+                "timed_in": "the `breakdown` pass (plain launches, events around every launch; `breakdown.ms_per_step` is that pass's step time)",
+                "fused_lora_shrink": fused,
+                "per_family_tflops": {f: round(fam_fl[f] * steps / (fam[f][1] * 1e-3) / 1e12, 1) for f in GEMM_FAMILIES if fam[f][1] > 0}}
+        other = sum(v["ms_per_step"] for k, v in breakdown.items() if k not in GEMM_FAMILIES)
+        breakdown = {"ms_per_step": round(ms_prof / steps, 4), "sum_of_families_ms": round(ms_g / steps + other, 4), "families": breakdown}
+
+    tf = fl["total"] * world * steps / (ms_max * 1e-3) / 1e12
+    line = {"metric": METRIC, "value": round(value, 2), "unit": "samples/s", "n_gpus": world, "steps": steps,
+            "warmup": warm, "ms_per_step": round(ms_max / steps, 4), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": WORKLOAD_NAMES.get(label, label), "requests": B, "tokens": wl.n_tokens,
+                       "tasks": len(wl.tasks), "tasks_in_batch": int(len(set(wl.task_ids.tolist()))), "dist": wl.notes.get("dist"),
+                       "l2": "flushed (256 MB memset) between steps, outside the per-step events" if flush is not None else "no flush",
+                       "accumulate": "fp32 (TMEM), fp32 residual stream", "replicas": world,
+                       **({"mlp_heads_hidden": args.mlp_hidden} if args.mlp_hidden else {}), **({"input_encoder_channels": args.enc_channels} if args.enc_channels else {}),
+                       "launch": f"CUDA graph replay inside fmx_forward_mixed on {graph_steps} of {steps} timed steps" if graph_steps else "plain kernel launches"},
+            "no_graph": {"value": round(replicas.whole_job_throughput(B, steps, ms_plain_max, world), 2), "ms_per_step": round(ms_plain_max / steps, 4),
+                         "what": "the same K steps as plain kernel launches (FMX_OPT_GRAPH off), timed the same way"},
+            "pct_bf16_tensor_peak": {"of_burst": round(100 * tf / pk["bf16_tflops"], 2), "of_sustained": round(100 * tf / pk["bf16_tflops_sustained"], 2),
+                                     "achieved_tflops": round(tf, 1), "algorithmic_tflop_per_step": round(fl["total"] / 1e12, 4), "peaks": pk["source"]},
+            "gpu_launches": launches_per_step * steps, "launches_per_step": launches_per_step,
+            "clocks": clocks, "roofline": roof, "breakdown": breakdown}
+    if not full:
+        return line, sess
 
     # ---- e2e through the host-buffer entry point ----
     packed = wl.packed_inputs()
@@ -323,8 +377,9 @@ def _measure(args, wl, rank, local_rank, world, with_cpu_baseline=True):
     ids = np.array([sess.task_ids_of[int(t)] for t in wl.task_ids], dtype=np.int32)
     off = sess.fmx.output_layout(ids)
     host_out = torch.empty(int(off[-1]), dtype=torch.float32).pin_memory()
+    sess.ensure_host_workspace(packed.nbytes, int(off[-1]))
     stream = torch.cuda.current_stream().cuda_stream
-    e2e_steps = max(3, min(args.steps, 20))
+    e2e_steps = max(3, min(steps, 20))
     for _ in range(2):
         sess.fmx.forward_mixed_host(sess.bb, host_in.data_ptr(), packed.nbytes, ids, wl.lengths, host_out.data_ptr(), sess.ws_ptr,
                                     sess.ws_bytes, stream)
@@ -339,56 +394,22 @@ def _measure(args, wl, rank, local_rank, world, with_cpu_baseline=True):
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
     e2e_ms_max = replicas.max_over_ranks(e2e_s * 1e3, dev if world > 1 else None)
-    e2e = {"value": replicas.whole_job_throughput(B, e2e_steps, e2e_ms_max, world), "unit": "samples/s",
-           "h2d_bytes_per_step": int(packed.nbytes + 8 * B), "d2h_bytes_per_step": int(off[-1]) * 4, "steps": e2e_steps,
-           "includes": "L2 flush memset between steps"}
-
-    # ---- roofline of the dominant kernel (tcgen05 GEMM, all four projection families) ----
-    roof = None
-    if gemm_prof:
-        n_l = sum(gemm_prof[f][0] for f in GEMM_FAMILIES)
-        ms_g = sum(gemm_prof[f][1] for f in GEMM_FAMILIES)
-        fused = "lora_shrink" not in breakdown      # the LoRA shrink ran as work items of the GEMM launches (no shrink family)
-        fam_fl = {f: fl["families"][f] + (fl["shrink_families"][f] if fused else 0.0) for f in GEMM_FAMILIES}
-        fl_g = sum(fam_fl.values())                                     # per forward
-        avg_ms = ms_g / max(n_l, 1)
-        flops_per_launch = fl_g / accounting.gemm_launches_per_forward(wl)
-        achieved = flops_per_launch / (avg_ms * 1e-3) / 1e12
-        roof = {"kernel": "fmx::pair_gemm_kernel<256> (tcgen05 cta_group::2 / TMEM / TMA, fused LoRA expand)", "bound": "tensor", "achieved": round(achieved, 2),
-                "peak": pk["bf16_tflops_sustained"], "unit": "TFLOP/s", "frac": round(achieved / pk["bf16_tflops_sustained"], 4),
-                "peak_kind": f"{pk['source']} sustained bf16 (kernel timed inside a long step)",
-                "frac_of_burst_peak": round(achieved / pk["bf16_tflops"], 4), "traffic": gemm_traffic(args.workload),
-                "traffic_unit": "DRAM bytes per launch (ncu --set full, cold cache; profiles/gemm_traffic.csv)",
-                "flops_per_launch": flops_per_launch, "avg_launch_ms": round(avg_ms, 5), "launches_timed": n_l,
-                "share_of_step": round(ms_g / ms_prof_steps, 4),
-                "timed_in": f"{args.steps} steps of the same loop right after the timed region (per-launch events need plain launches; {round(ms_prof_steps / args.steps, 4)} ms/step there)",
-                "fused_lora_shrink": fused,
-                "per_family_tflops": {f: round(fam_fl[f] * args.steps / (gemm_prof[f][1] * 1e-3) / 1e12, 1)
-                                      for f in GEMM_FAMILIES if gemm_prof[f][1] > 0}}
-    line = {"metric": METRIC, "value": round(value, 2), "unit": "samples/s", "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": round(ms_max / args.steps, 4), "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-            "config": {"workload": WORKLOAD_NAMES.get(args.workload, args.workload), "requests": B, "tokens": wl.n_tokens,
-                       "tasks": len(wl.tasks), "tasks_in_batch": int(len(set(wl.task_ids.tolist()))), "dist": wl.notes.get("dist"),
-                       "l2": "flushed (256 MB memset) between steps, outside the per-step events" if flush is not None else "no flush",
-                       "accumulate": "fp32 (TMEM), fp32 residual stream", "replicas": world,
-                       **({"mlp_heads_hidden": args.mlp_hidden} if args.mlp_hidden else {}), **({"input_encoder_channels": args.enc_channels} if args.enc_channels else {}),
-                       "launch": f"CUDA graph replay inside fmx_forward_mixed on {graph_steps} of {args.steps} timed steps" if graph_steps else "plain kernel launches"},
-            "pct_bf16_tensor_peak": {"of_burst": round(100 * fl["total"] * world * args.steps / (ms_max * 1e-3) / 1e12 / pk["bf16_tflops"], 2),
-                                     "of_sustained": round(100 * fl["total"] * world * args.steps / (ms_max * 1e-3) / 1e12 / pk["bf16_tflops_sustained"], 2),
-                                     "algorithmic_tflop_per_step": round(fl["total"] / 1e12, 4), "peaks": pk["source"]},
-            "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "launches_per_step": launches_per_step,
-            "clocks": clocks, "roofline": roof, "breakdown": breakdown}
+    line["e2e"] = {"value": round(replicas.whole_job_throughput(B, e2e_steps, e2e_ms_max, world), 2), "unit": "samples/s",
+                   "h2d_bytes_per_step": int(packed.nbytes + 8 * B), "d2h_bytes_per_step": int(off[-1]) * 4, "steps": e2e_steps,
+                   "includes": "pinned host -> device copy of the packed inputs, ids / lengths upload, forward, device -> host copy of all outputs, "
+                               "stream synchronise; L2 flush memset between steps"}
     if rank == 0:
         line["bfq"] = bfq_host_cost(wl)
         # R2 lifecycle decoupling: take one task off the live context and put it back (the backbone and the other tasks stay)
         un_ms, reg_ms = sess.task_lifecycle_ms(len(wl.tasks) - 1)
         reg_busy_ms, fwd_ms, _ = sess.register_while_serving_ms(len(wl.tasks) - 1, n_forwards=5)
+        un_busy_ms, fwd2_ms = sess.unregister_while_serving_ms(len(wl.tasks) - 1, n_forwards=5)
         line["task_lifecycle"] = {"unregister_ms": round(un_ms, 3), "register_ms": round(reg_ms, 3), "task": len(wl.tasks) - 1,
                                   "register_ms_with_5_forwards_queued": round(reg_busy_ms, 3), "those_5_forwards_ms": round(fwd_ms, 2),
-                                  "how": "fmx_unregister_task / fmx_register_task on the live context, tensors already on the device; "
-                                         "paper: 25 ms task load vs 5737 ms backbone load for MOMENT-Large on its T4 host (P:L387)"}
-    if with_cpu_baseline and rank == 0 and world == 1 and not args.no_cpu_baseline:
+                                  "unregister_ms_with_5_forwards_queued": round(un_busy_ms, 3), "those_forwards_ms": round(fwd2_ms, 2),
+                                  "how": "fmx_unregister_task / fmx_register_task on the live context, tensors already on the device; neither "
+                                         "synchronises the device; paper: 25 ms task load vs 5737 ms backbone load for MOMENT-Large on its T4 host (P:L387)"}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
         n = min(args.cpu_sample, B)
         idx = list(range(n))
         dt, ref = oracle_time(wl, idx)
@@ -398,34 +419,79 @@ def _measure(args, wl, rank, local_rank, world, with_cpu_baseline=True):
         line["cpu_baseline"] = {"value": round(n / dt, 4), "unit": "samples/s", "cores": blas_threads(), "kind": "oracle",
                                 "sample": f"first {n} of {B} requests, one by one in numpy fp64 ({dt:.1f} s; weights widened before the clock)",
                                 "max_abs_vs_cuda": mx}
+    return line, sess
+
+
+def light(line):
+    """The per-config / reference summary of a measured line."""
+    r = line["roofline"] or {}
+    return {"workload": line["config"]["workload"], "requests": line["config"]["requests"], "tokens": line["config"]["tokens"],
+            "tasks_in_batch": line["config"]["tasks_in_batch"], "value": line["value"], "unit": "samples/s", "ms_per_step": line["ms_per_step"],
+            "steps": line["steps"], "no_graph_ms_per_step": line["no_graph"]["ms_per_step"],
+            "pct_of_burst": line["pct_bf16_tensor_peak"]["of_burst"], "pct_of_sustained": line["pct_bf16_tensor_peak"]["of_sustained"],
+            "achieved_tflops": line["pct_bf16_tensor_peak"]["achieved_tflops"],
+            "gemm_tflops": r.get("achieved"), "gemm_frac_of_burst": r.get("frac_of_burst_peak"), "per_family_tflops": r.get("per_family_tflops"),
+            "family_ms_per_step": {k: v["ms_per_step"] for k, v in (line["breakdown"] or {}).get("families", {}).items()},
+            "sm_mhz": (line["clocks"] or {}).get("sm_mhz"), "clock_reasons": (line["clocks"] or {}).get("reasons")}
+
+
+def run_headline(args, rank, local_rank, world):
+    """The default run: BASELINE.json's metric on its own configuration (configs[4], 92 co-batched tasks) plus, in the same
+    process, its two reference batches (single task / adapter-free, same size, same backbone weights on the device) and the
+    other full-size configs."""
+    from fmx_workloads import make_workload
+    short = max(5, min(args.steps, 10))
+    wl = make_workload("cfg5", n_tasks=HEADLINE["tasks"], dist=HEADLINE["dist"])
+    line, sess = measure(args, wl, rank, local_rank, world, full=True, label="headline")
+    refs = {}
+    for key, kw in (("single_task", dict(n_tasks=1, dist="uniform")), ("adapter_free", dict(n_tasks=1, dist="uniform", adapters=False))):
+        l2, s2 = measure(args, make_workload("cfg5", **kw), rank, local_rank, world, full=False, weights_from=sess, label=f"cfg5 {key}")
+        refs[key] = light(l2)
+        s2.fmx.destroy()
     sess.fmx.destroy()
+    del sess
+    line["vs_single_task"] = round(line["value"] / refs["single_task"]["value"], 4)
+    line["vs_adapter_free"] = round(line["value"] / refs["adapter_free"]["value"], 4)
+    line["references"] = {**refs, "note": "same batch size (512) and backbone weights; single_task: all requests on one task with a rank-16 LoRA "
+                                           "on q/k/v/o and a forecast head (reading 19); adapter_free: one head-only task.  north_star target: "
+                                           "vs_single_task >= 0.90"}
+    per = {}
+    if not args.no_per_config:
+        for cfg, st in (("cfg2", short), ("cfg3", short), ("cfg4", max(3, short // 2))):
+            l2, s2 = measure(args, make_workload(cfg), rank, local_rank, world, full=False, steps=st, label=cfg)
+            per[cfg] = light(l2)
+            s2.fmx.destroy()
+            del s2
+    line["per_config"] = per
     return line
 
 
 def run_sweep5(args, rank, local_rank, world):
-    """BASELINE.json configs[4]: T x distribution -> samples/s, ratio to the single-task batch."""
+    """BASELINE.json configs[4] in full: T x distribution -> samples/s, ratio to the single-task batch and to the adapter-free one."""
     from fmx_workloads import make_workload
-    rows = []
-    ref = {}
+    rows, ref, keep, last = [], {}, None, None
     for T, dist, ad in [(1, "uniform", True), (1, "uniform", False)] + [(T, d, True) for T in (4, 16, 48, 92)
                                                                          for d in ("uniform", "zipf0.8", "zipf1.5")]:
         wl = make_workload("cfg5", n_tasks=T, dist=dist, adapters=ad)
-        a = argparse.Namespace(**vars(args))
-        a.workload, a.tasks, a.dist, a.no_adapters = "cfg5", T, dist, not ad
-        line = measure(a, wl, rank, local_rank, world, with_cpu_baseline=False)
+        line, sess = measure(args, wl, rank, local_rank, world, full=False, weights_from=keep, label=f"cfg5 T={T} {dist}")
+        if keep is None:
+            keep = sess                       # later points reuse the backbone weights on the device
+        else:
+            sess.fmx.destroy()
         key = "single_task" if (T == 1 and ad) else ("adapter_free" if T == 1 else None)
         if key:
             ref[key] = line["value"]
         rows.append({"tasks": T, "dist": dist, "adapters": ad, "samples_per_s": line["value"], "ms_per_step": line["ms_per_step"],
-                     "pct_peak_sustained": line["pct_bf16_tensor_peak"]["of_sustained"],
+                     "no_graph_ms_per_step": line["no_graph"]["ms_per_step"],
+                     "pct_peak_burst": line["pct_bf16_tensor_peak"]["of_burst"],
                      "vs_single_task": round(line["value"] / ref["single_task"], 4) if "single_task" in ref else None,
                      "vs_adapter_free": round(line["value"] / ref["adapter_free"], 4) if "adapter_free" in ref else None,
-                     "gemm_frac": line["roofline"]["frac"] if line["roofline"] else None})
+                     "gemm_frac_of_burst": line["roofline"]["frac_of_burst_peak"] if line["roofline"] else None})
         last = line
     os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
     if rank == 0:
         json.dump(rows, open(os.path.join(ROOT, "gpurun_out", "sweep5.json"), "w"), indent=1)
-    last["config"]["workload"] = "configs[4] sweep; this line = T=92, Zipf(1.5); full table in gpurun_out/sweep5.json"
+    last["config"]["workload"] = "configs[4] sweep; this line = T=92, Zipf(1.5); full table in `sweep` (also written to gpurun_out/sweep5.json)"
     last["sweep"] = rows
     return last
 
@@ -433,10 +499,12 @@ def run_sweep5(args, rank, local_rank, world):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="fmx", choices=["fmx", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5", "sweep5"])
+    ap.add_argument("--workload", default="headline", choices=["headline", "cfg2", "cfg3", "cfg4", "cfg5", "sweep5"],
+                    help="headline (default): configs[4] at 92 tasks + its single-task / adapter-free references + per_config cfg2 / cfg3 / cfg4")
+    ap.add_argument("--no-per-config", action="store_true", help="headline: skip the cfg2 / cfg3 / cfg4 lines")
     ap.add_argument("--tasks", type=int, default=92, help="cfg5: number of co-batched tasks")
     ap.add_argument("--dist", default="zipf0.8", choices=["uniform", "zipf0.8", "zipf1.5"])
     ap.add_argument("--no-adapters", action="store_true", help="cfg5: head-only tasks (adapter-free reference)")
@@ -457,8 +525,11 @@ def main():
         sys.stderr.write(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; launch N>1 with torch.distributed.run\n")
     if args.workload == "sweep5":
         line = run_sweep5(args, rank, local_rank, world)
+    elif args.workload == "headline":
+        line = run_headline(args, rank, local_rank, world)
     else:
-        line = measure(args, build_workload(args), rank, local_rank, world)
+        line, sess = measure(args, build_workload(args), rank, local_rank, world)
+        sess.fmx.destroy()
     if rank == 0:
         print(json.dumps(line))
     replicas.finalize()

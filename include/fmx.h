@@ -18,7 +18,13 @@
  *     ordinary host memory.  All matrices are row-major; bf16 is the 16-bit brain float.
  *   - Linear weights are [out, in] (PyTorch/PEFT orientation, Listing 2).
  *   - Validation happens fully on the host BEFORE any launch; on error nothing is enqueued
- *     on the stream and no library state changes.
+ *     on the stream and no library state changes (a registration that fails part-way returns
+ *     what it had allocated; the registry is committed only after its last fallible step).
+ *   - fmx_forward_mixed allocates nothing and never synchronises: every scratch buffer it
+ *     needs is part of the caller's workspace (fmx_workspace_bytes).
+ *   - What the host cannot check (token ids living in device memory) is checked on the device:
+ *     an id outside [0, vocab) is embedded as a zero row and raises the context's device error
+ *     word, which the NEXT call on the context (or fmx_poll_error) reports as FMX_E_INVALID_ARG.
  *   - There is no CPU fallback anywhere: without a CUDA device every compute call returns
  *     FMX_E_CUDA.
  */
@@ -113,7 +119,8 @@ typedef struct fmx_adapter_desc {
 /* A task's extensions: PEFT adapter(s) + decoder head.
  * fmx_register_task copies on the library's own registration stream and does not wait for forwards in flight (adding a
  * task to a serving context costs ~1-2 ms, PAPER.md L92 / L243); the source tensors must be complete (the work that
- * produced them finished) when the call is made.  Growing the LoRA slab arena (rare) synchronises the device.
+ * produced them finished) when the call is made.  Growing the LoRA slab arena (rare) builds the wider arena on that
+ * stream too and switches descriptors at a forward boundary; nothing synchronises the device.
  * Ownership: the library COPIES adapters and head into its own arena (task-sorted slabs laid
  * out for the segmented kernels); the caller may free its buffers when the call returns. */
 typedef struct fmx_task_desc {
@@ -146,6 +153,9 @@ int fmx_create(fmx_ctx **out, int device_ordinal);
 int fmx_destroy(fmx_ctx *ctx);
 const char *fmx_last_error(void);                 /* thread-local; "" if none                  */
 const char *fmx_version(void);
+/* Reports (and clears) a device-side error raised by an earlier forward of this context; call after synchronising the
+ * stream.  FMX_OK if none. */
+int fmx_poll_error(fmx_ctx *ctx);
 
 /* Registers a backbone; *out receives its handle. */
 int fmx_register_backbone(fmx_ctx *ctx, const fmx_backbone_desc *desc, fmx_backbone_t *out);
@@ -155,18 +165,27 @@ int fmx_register_backbone(fmx_ctx *ctx, const fmx_backbone_desc *desc, fmx_backb
  * Synchronises the context's copy stream before returning. */
 int fmx_register_task(fmx_ctx *ctx, fmx_backbone_t bb, const fmx_task_desc *desc, fmx_task_t *out);
 
-/* Removes a task (remove_adapter).  Other tasks' outputs are unaffected. */
+/* Removes a task (remove_adapter).  Other tasks' outputs are unaffected.  Returns at once: forwards already
+ * enqueued still serve the task (its buffers are released on the device after them), later forwards reject its id
+ * (FMX_E_UNKNOWN_TASK).  A registration that reuses the freed slot or slab columns waits on the device, not on the host. */
 int fmx_unregister_task(fmx_ctx *ctx, fmx_task_t task);
 
 /* HOST.  out_off[i] .. out_off[i+1] is request i's slice of the fp32 output buffer (prefix sum
  * of head_out in ORIGINAL request order); out_off has n_req + 1 entries. */
 int fmx_output_layout(fmx_ctx *ctx, const int32_t *task_ids, int32_t n_req, int64_t *out_off);
 
-/* Bytes of DEVICE workspace fmx_forward_mixed needs for up to max_req requests / max_tokens tokens. */
+/* Bytes of DEVICE workspace fmx_forward_mixed needs for up to max_req requests / max_tokens tokens (activations, segment
+ * tables and the head scratch: the forward itself allocates nothing). */
 int fmx_workspace_bytes(fmx_ctx *ctx, fmx_backbone_t bb, int32_t max_req, int64_t max_tokens, size_t *bytes);
+/* The same for fmx_forward_mixed_host, which also stages the packed inputs (max_input_bytes) and the outputs
+ * (max_output_floats fp32 values) in the workspace. */
+int fmx_host_workspace_bytes(fmx_ctx *ctx, fmx_backbone_t bb, int32_t max_req, int64_t max_tokens, size_t max_input_bytes,
+                             int64_t max_output_floats, size_t *bytes);
 
 /* The mixed-task forward.  Asynchronous on cuda_stream (a cudaStream_t; NULL = default
- * stream); the caller synchronises.  One forward in flight per context.
+ * stream); the caller synchronises.  Calls on one context are serialised by the context's mutex.
+ * A stream that is being captured into a CUDA graph by the caller is refused (FMX_E_INVALID_ARG):
+ * ids / lengths travel through a pinned staging ring a replay would find overwritten.
  *   inputs    DEVICE, requests packed back to back in ORIGINAL request order:
  *             EMBEDDED bf16 [n_i, d_model]; PATCH_LINEAR bf16 [n_patches*patch_dim] or image
  *             [img_c, img_hw, img_hw]; TOKEN_IDS int32 [n_i].
@@ -181,7 +200,8 @@ int fmx_forward_mixed(fmx_ctx *ctx, fmx_backbone_t bb, const void *inputs, const
                       size_t workspace_bytes, void *cuda_stream);
 
 /* Same, end to end from HOST buffers: copies inputs host->device, runs the forward, copies the
- * outputs device->host and synchronises.  inputs_bytes = total bytes of the packed inputs. */
+ * outputs device->host and synchronises.  inputs_bytes = total bytes of the packed inputs.
+ * workspace: >= fmx_host_workspace_bytes(...). */
 int fmx_forward_mixed_host(fmx_ctx *ctx, fmx_backbone_t bb, const void *inputs_host, size_t inputs_bytes,
                            const int32_t *task_ids, const int32_t *lengths, int32_t n_req,
                            float *outputs_host, void *workspace, size_t workspace_bytes, void *cuda_stream);
@@ -191,13 +211,6 @@ int fmx_forward_mixed_host(fmx_ctx *ctx, fmx_backbone_t bb, const void *inputs_h
  * n_slots = fmx_task_slots().  Any pointer may be NULL. */
 int fmx_debug_get_segments(fmx_ctx *ctx, int32_t *perm, int32_t *inv_perm, int32_t *task_req_off,
                            int32_t *cu_tok, int32_t *task_tok_off);
-/* Debug/test: the private row-tile table of the last forward (256-row CTA-pair tiles): n_tiles,
- * n_blocks, and per block (tile, task, row_lo, row_hi) into blocks[4*n_blocks] (cap entries available). */
-int fmx_debug_get_tiles(fmx_ctx *ctx, int32_t *n_tiles, int32_t *n_blocks, int32_t *blocks, int32_t cap);
-/* Debug/test: copies an activation buffer of the LAST forward to HOST (synchronises).  which:
- * 0 X fp32 [N,d] (residual, task-sorted rows)  1 Xn bf16 [N,d]  2 QKV bf16 [N,d_qkv]  3 attention out
- * bf16 [N,d_q]  4 FFN hidden bf16 [N,d_ffn]  5 U bf16 [n_blk_cap*256,192]  6 pooled feature fp32 [B,d]. */
-int fmx_debug_read(fmx_ctx *ctx, int which, void *host, size_t bytes);
 int fmx_task_slots(fmx_ctx *ctx);                 /* number of task slots (highest id ever live + 1) */
 
 /* Per-kernel-family timing of the next forwards (CUDA events around every launch, on the
@@ -212,54 +225,9 @@ int fmx_profile_read(fmx_ctx *ctx, int32_t *launches /*[FMX_N_FAMILIES]*/, doubl
 const char *fmx_profile_family_name(int family);
 /* Kernels launched by the last forward (the count bench.py reports as gpu_launches). */
 int fmx_last_launch_count(fmx_ctx *ctx);
-/* Forwards served by replaying the context's cached CUDA graph so far (FMX_OPT_GRAPH; debug / tests). */
-long long fmx_graph_replays(fmx_ctx *ctx);
 
-/* Debug/test: one GEMM through the tcgen05 kernel, C[M,N] (fp32) = A[M,K] (bf16) · W[N,K]^T (bf16);
- * N a multiple of 128, K a multiple of 8.  All DEVICE pointers. */
-int fmx_debug_gemm(fmx_ctx *ctx, const void *A, const void *W, float *C, int32_t M, int32_t N, int32_t K,
-                   void *cuda_stream);
-
-/* Debug/test: the fused variable-length attention step (S3d) alone.  qkv DEVICE bf16
- * [n_tokens, (n_q_heads + 2 n_kv_heads) * head_dim] (q | k | v per row, requests packed back to back),
- * cu_tok HOST int32 [n_req + 1] (prefix sums of the request lengths), out DEVICE bf16
- * [n_tokens, n_q_heads * head_dim].  impl: an FMX_ATTN_* value.  Scale 1/sqrt(head_dim). */
-int fmx_debug_attention(fmx_ctx *ctx, const void *qkv, void *out, const int32_t *cu_tok, int32_t n_req,
-                        int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim, int32_t causal, int32_t impl,
-                        void *cuda_stream);
-
-/* Tuning knobs (process-local experiments; defaults are what bench.py measures). */
-enum {
-  FMX_OPT_ATTENTION_IMPL = 0,    /* FMX_ATTN_AUTO | FMX_ATTN_MMA_SYNC | FMX_ATTN_TCGEN05 | FMX_ATTN_LANES */
-  FMX_OPT_ATTENTION_VARIANT = 1, /* tcgen05 attention: 0 = one 128-query tile per CTA; 1 = two q-tiles per CTA
-                                    sharing K/V.  FMX_ATTN_LANES: 0 / 1 / 2 = 4 / 2 / 3 lanes per CTA (head_dim 64) */
-  FMX_OPT_SHRINK_STAGES = 3,     /* LoRA shrink kernel pipeline: 5 (default) = as deep as ~200 KB allow for the stage size
-                                    (8 / 6 / 5 stages for 1 / 2 / 3 targets), 4 = four 40 KB stages */
-  FMX_OPT_HALF_TILES = 4,        /* 1 (default): a short last GEMM wave is cut into 256 x 128 half tiles */
-  FMX_OPT_ATTN_SHORT = 5,        /* batches whose requests all have <= 64 tokens: 0 = generic kernels, 1 = pipelined
-                                    single-tile mma.sync kernel, 2 (default) = tcgen05 head-pair kernel when head_dim is
-                                    64 and the head count even (FMX_ATTN_AUTO only), else as 1 */
-  FMX_OPT_ROPE_FUSED = 6,        /* 1 (default): head_dim 128 backbones rotate q / k in the QKV GEMM epilogue;
-                                    0: separate RoPE kernel over the bf16 QKV buffer */
-  FMX_OPT_HEAD_TILED = 7,        /* FLATTEN heads: 0 = one warp per (request, output), 1 = CUDA-core 4 x 4 register tiles,
-                                    2 (default) = mma.sync 16-request x 32-output tiles over K chunks */
-  FMX_OPT_SHRINK_FUSED = 8,      /* the LoRA shrink runs as the first work items of the GEMM that consumes it: 0 = never
-                                    (separate shrink kernel), 1 (default) = when the batch has at most one (tile, task)
-                                    block per CTA pair, 2 = always */
-  FMX_OPT_GRAPH = 9,             /* 1 (default): fmx_forward_mixed captures a CUDA graph on the 2nd identical call (same
-                                    buffers, stream, ids, lengths, registrations, options) and replays it afterwards;
-                                    needs a non-default stream; 0: always plain launches */
-  FMX_OPT_REVERSE = 10,          /* 1 (default): consecutive kernels of a layer walk the token rows in alternating
-                                    directions, so each starts on the rows its producer wrote last (still in L2) */
-  FMX_OPT_EXPAND_WIDE = 11,      /* 1 (default): a 256-wide tile whose two chunks share a weight source runs its LoRA
-                                    expand as one N = 256 step per block (U loaded once) instead of two N = 128 steps */
-  FMX_OPT_DEEP_PIPE = 12,        /* 1 (default): fp32-output GEMMs (residual, embed) run with one more smem pipeline stage
-                                    and a single epilogue staging buffer per warpgroup */
-  FMX_OPT_PDL = 2                /* programmatic dependent launch of the forward's kernels (process-wide):
-                                    0 = off, 1 = always, 2 (default) = only for batches of <= 4096 token rows */
-};
-enum { FMX_ATTN_AUTO = 0, FMX_ATTN_MMA_SYNC = 1, FMX_ATTN_TCGEN05 = 2, FMX_ATTN_LANES = 3 };
-int fmx_set_option(fmx_ctx *ctx, int32_t option, int32_t value);
+/* Test hooks and tuning knobs (single-kernel entry points, activation read-back, fmx_set_option) are not part of this
+ * ABI: they are declared in paper_2606_09643_b200/csrc/fmx_internal.h. */
 
 /* ---- BFQ: host-side batch-aware fair-queue batch builder (§4.2, Eq. 1-3) ------------
  * Pure host code (no CUDA).  It emits the task ids / lengths fmx_forward_mixed consumes. */

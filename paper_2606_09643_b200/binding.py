@@ -65,11 +65,14 @@ class FmxError(RuntimeError):
 
 _lib = None
 
-EXPORTS = ["fmx_create", "fmx_destroy", "fmx_last_error", "fmx_version", "fmx_register_backbone", "fmx_register_task",
-           "fmx_unregister_task", "fmx_output_layout", "fmx_workspace_bytes", "fmx_forward_mixed", "fmx_forward_mixed_host",
-           "fmx_debug_get_segments", "fmx_debug_get_tiles", "fmx_debug_read", "fmx_task_slots", "fmx_profile_enable", "fmx_profile_select", "fmx_profile_read",
-           "fmx_profile_family_name", "fmx_last_launch_count", "fmx_graph_replays", "fmx_debug_gemm", "fmx_debug_attention", "fmx_set_option", "fmx_bfq_create", "fmx_bfq_destroy",
+# include/fmx.h (the public C ABI)
+EXPORTS = ["fmx_create", "fmx_destroy", "fmx_last_error", "fmx_version", "fmx_poll_error", "fmx_register_backbone", "fmx_register_task",
+           "fmx_unregister_task", "fmx_output_layout", "fmx_workspace_bytes", "fmx_host_workspace_bytes", "fmx_forward_mixed",
+           "fmx_forward_mixed_host", "fmx_debug_get_segments", "fmx_task_slots", "fmx_profile_enable", "fmx_profile_select",
+           "fmx_profile_read", "fmx_profile_family_name", "fmx_last_launch_count", "fmx_bfq_create", "fmx_bfq_destroy",
            "fmx_bfq_set_task", "fmx_bfq_enqueue", "fmx_bfq_next_batch", "fmx_bfq_complete", "fmx_bfq_stats", "fmx_bfq_peek"]
+# csrc/fmx_internal.h (test hooks and tuning knobs; not part of the ABI)
+INTERNAL_EXPORTS = ["fmx_debug_get_tiles", "fmx_debug_read", "fmx_graph_replays", "fmx_debug_gemm", "fmx_debug_attention", "fmx_set_option"]
 
 
 def load():
@@ -93,6 +96,8 @@ def load():
     lib.fmx_unregister_task.argtypes = [_vp, C.c_int32]
     lib.fmx_output_layout.argtypes = [_vp, i32p, C.c_int32, i64p]
     lib.fmx_workspace_bytes.argtypes = [_vp, C.c_int32, C.c_int32, C.c_int64, C.POINTER(C.c_size_t)]
+    lib.fmx_host_workspace_bytes.argtypes = [_vp, C.c_int32, C.c_int32, C.c_int64, C.c_size_t, C.c_int64, C.POINTER(C.c_size_t)]
+    lib.fmx_poll_error.argtypes = [_vp]
     lib.fmx_forward_mixed.argtypes = [_vp, C.c_int32, _vp, i32p, i32p, C.c_int32, _vp, _vp, C.c_size_t, _vp]
     lib.fmx_forward_mixed_host.argtypes = [_vp, C.c_int32, _vp, C.c_size_t, i32p, i32p, C.c_int32, _vp, _vp, C.c_size_t, _vp]
     lib.fmx_debug_get_segments.argtypes = [_vp, i32p, i32p, i32p, i32p, i32p]
@@ -208,6 +213,14 @@ class Fmx:
         out = C.c_size_t(0)
         _check(self.lib.fmx_workspace_bytes(self.h, bb, max_req, max_tokens, C.byref(out)))
         return out.value
+
+    def host_workspace_bytes(self, bb, max_req, max_tokens, max_input_bytes, max_output_floats):
+        out = C.c_size_t(0)
+        _check(self.lib.fmx_host_workspace_bytes(self.h, bb, max_req, max_tokens, max_input_bytes, max_output_floats, C.byref(out)))
+        return out.value
+
+    def poll_error(self):
+        _check(self.lib.fmx_poll_error(self.h))
 
     def forward_mixed(self, bb, inputs, task_ids, lengths, outputs, workspace, workspace_bytes, stream=0):
         ids, lens = _i32(task_ids), _i32(lengths)

@@ -19,6 +19,7 @@
 #include "attention_tc.cuh"
 #include "common.h"
 #include "fmx.h"
+#include "fmx_internal.h"
 #include "gemm.cuh"
 #include "kernels.cuh"
 #include "pair_gemm.cuh"
@@ -46,6 +47,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
 
 struct TaskRec {
   bool live = false;
+  unsigned long long freed_seq = 0;       // retirement after which this slot's device-table entries may be rewritten
   int bb = -1;
   int coff = 0, rpad = 0;                 // slab columns [coff, coff + rpad)
   unsigned char trpad[7] = {0};
@@ -73,6 +75,7 @@ struct Backbone {
   // LoRA slabs
   int Rcap = 0;
   std::vector<unsigned char> col_used;     // units of 16 columns
+  std::vector<unsigned long long> col_freed_seq;   // retirement after which a freed unit may be rewritten
   bf16 *slabA[7] = {nullptr};              // per target: [L][Rcap, d_in]
   bf16 *slabB[7] = {nullptr};              // per target: [L][d_out, Rcap]
   std::vector<CUtensorMap> mA[7], mB[7];   // per target, per layer
@@ -81,6 +84,25 @@ struct Backbone {
 };
 
 struct ProfEvent { int family; cudaEvent_t e0, e1; };
+
+// Tuning state of ONE context (fmx_set_option, csrc/fmx_internal.h); nothing tunable lives at file scope.
+struct Opts {
+  int pdl = 2;            // programmatic dependent launch: 0 off, 1 always, 2 = only for batches of <= kPdlAutoRows token rows
+  int shrink_stages = 5;
+  int half_tiles = 1;
+  int deep_pipe = 1;
+  int expand_wide = 1;
+  int rope_fused = 1;
+  int head_tiled = 2;     // FLATTEN heads: 0 = one warp per output, 1 = CUDA-core 4 x 4 tiles, 2 = mma.sync 16 x 32 tiles
+  int shrink_fused = 1;   // the LoRA shrink runs as the first work items of the GEMM that consumes it (see pair_gemm.cuh)
+  int reverse = 1;        // consecutive kernels of a layer walk the rows in alternating directions (L2 reuse)
+  int attn_short = 2;     // 0: generic kernel, 1: pipelined mma.sync kernel, 2: tcgen05 head-pair kernel where it applies
+  int graph = 1;
+  int attn_impl = FMX_ATTN_AUTO, attn_variant = 0;
+};
+
+// A launch target: the stream and whether the launch carries the programmatic-stream-serialization attribute.
+struct Strm { cudaStream_t s; int pdl; };
 
 }  // namespace
 
@@ -99,7 +121,6 @@ struct fmx_ctx {
   int *d_task_head_w1 = nullptr;           // first-layer width of the head (= head_out for linear heads)
   int *d_task_enc_ch = nullptr;            // input-encoder channels by task
   const bf16 **d_task_enc_W = nullptr, **d_task_enc_b = nullptr;
-  float *d_head_hid = nullptr; size_t head_hid_bytes = 0;       // hidden activations of MLP heads [B, max hidden]
   // pinned staging for ids / lengths: a ring (a slot is rewritten only after the copy that read it has run) plus one
   // buffer owned by the cached CUDA graph
   static constexpr int kStageSlots = 4;
@@ -118,18 +139,27 @@ struct fmx_ctx {
   };
   // registration runs on its own non-blocking stream: adding a task never waits for (or stalls) forwards in flight
   cudaStream_t side = nullptr;
+  // retirement stream: frees of what forwards in flight may still read happen here, after those forwards (see retire())
+  cudaStream_t side2 = nullptr;
+  cudaEvent_t side_ev = nullptr, retire_ev = nullptr;
+  unsigned long long retire_seq = 0, retire_done = 0;   // retirements issued / known complete
   struct TaskStage { int coff, head_kind, head_out, w1, enc_ch; unsigned char trpad[8]; float scale[7]; const void *ptr[6]; };
   TaskStage *h_task_stage = nullptr;       // pinned
-  int opt_graph = 1;
+  Opts o;
   unsigned long long config_gen = 0;       // bumped by every registration change and option change
   CallKey last_key, graph_key;
   cudaGraphExec_t graph_exec = nullptr;
   int graph_launches = 0;                  // kernels inside the cached graph
   unsigned long long graph_replays = 0;
-  // host-buffer forward staging
-  void *d_in_stage = nullptr; size_t in_stage_bytes = 0;
-  float *d_out_stage = nullptr; size_t out_stage_bytes = 0;
-  float *d_head_part = nullptr; size_t head_part_bytes = 0;     // K-chunk partials of the tensor-core FLATTEN head
+  // Where forwards are in flight: the end-of-forward event of the latest forward on each serving stream seen (a few
+  // entries, least recently used replaced).  fmx_unregister_task and a slab growth make the registration stream wait for
+  // these events before it frees or reuses what those forwards may still read - the host never waits (NEXT-2).
+  static constexpr int kServe = 8;
+  struct Serving { cudaStream_t stream = nullptr; cudaEvent_t ev = nullptr; bool used = false; unsigned long long tick = 0; };
+  Serving serving[kServe];
+  unsigned long long serve_tick = 0;
+  // device-side error word (mapped pinned host memory): bit 0 = a TOKEN_IDS request carried an id outside [0, vocab)
+  unsigned *h_err = nullptr, *d_err = nullptr;
   // last forward (debug)
   SegTables last_t{};
   int last_B = 0, last_T = 0, last_n_tiles = 0, last_launches = 0;
@@ -140,8 +170,7 @@ struct fmx_ctx {
   uint32_t prof_mask = 0xFFFFFFFFu;        // families that get events while prof_on
   std::vector<ProfEvent> prof;
   std::vector<cudaEvent_t> ev_pool;        // recycled events
-  int opt_attn_impl = FMX_ATTN_AUTO, opt_attn_variant = 0;
-  int *d_dbg_cu = nullptr; int dbg_cu_cap = 0;   // fmx_debug_attention's device copy of cu_tok
+  int *d_dbg_cu = nullptr;                 // fmx_debug_attention's device copy of cu_tok [FMX_MAX_REQUESTS + 1]
   std::mutex mu;
 };
 
@@ -184,10 +213,18 @@ struct Workspace {
   float *X = nullptr, *feat = nullptr;
   bf16 *Xn = nullptr, *QKV = nullptr, *AttnO = nullptr, *Hid = nullptr, *U = nullptr;
   unsigned *u_flag = nullptr;            // completion counter of the fused-shrink items
+  float *head_hid = nullptr;             // hidden activations of MLP heads [B, kMaxHeadHidden]
+  float *head_part = nullptr;            // K-chunk partials of the tensor-core FLATTEN head: kHeadPartFloats per request
+  size_t head_part_floats = 0;
   int n_tiles = 0, n_blk_cap = 0;
   size_t bytes = 0;
 };
 
+// The head scratch is part of the caller's workspace (no allocation inside the forward): an MLP head's hidden layer is at
+// most kMaxHeadHidden wide (fmx_register_task enforces it); the FLATTEN-head partials get a fixed budget per request and
+// the launcher picks the K split that fits it.
+constexpr int kMaxHeadHidden = 4096;
+constexpr size_t kHeadPartFloats = 2048;
 Workspace carve(const Backbone &bb, void *base, int B, long long N, int T) {
   Workspace w;
   uint8_t *p = static_cast<uint8_t *>(base);
@@ -222,6 +259,9 @@ Workspace carve(const Backbone &bb, void *base, int B, long long N, int T) {
   w.U = (bf16 *)take(sizeof(bf16) * (size_t)w.n_blk_cap * kPairRows * 192);
   w.feat = (float *)take(sizeof(float) * (size_t)B * d.d_model);
   w.u_flag = (unsigned *)take(sizeof(unsigned));
+  w.head_hid = (float *)take(sizeof(float) * (size_t)B * kMaxHeadHidden);
+  w.head_part_floats = (size_t)((B + 15) / 16) * 16 * kHeadPartFloats;
+  w.head_part = (float *)take(sizeof(float) * w.head_part_floats);
   w.bytes = off;
   return w;
 }
@@ -268,31 +308,23 @@ struct Launcher {
 // griddepcontrol.wait before it touches global memory.  FMX_OPT_PDL: 0 = plain stream order, 1 = always, 2 (default) =
 // only for small batches (<= kPdlAutoRows token rows), where the step is bound by launch latency: measured on B200 it
 // takes cfg1 from 0.208 to 0.163 ms per forward and is neutral to slightly negative (< 1 %) on the large configs.
-int g_pdl = 2, g_pdl_eff = 0;
-int g_shrink_stages = 5;
-int g_half_tiles = 1;
-int g_deep_pipe = 1;
-int g_expand_wide = 1;
-int g_rope_fused = 1;
-int g_head_tiled = 2;     // FLATTEN heads: 0 = one warp per output, 1 = CUDA-core 4 x 4 tiles, 2 = mma.sync 16 x 32 tiles
-int g_shrink_fused = 1;   // the LoRA shrink runs as the first work items of the GEMM that consumes it (see pair_gemm.cuh)
 constexpr int kPdlAutoRows = 4096;
 template <typename... KArgs, typename... Args>
-void launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args &&...args) {
+void launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, Strm st, Args &&...args) {
   cudaLaunchConfig_t cfg{};
-  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st.s;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  at[0].val.programmaticStreamSerializationAllowed = g_pdl_eff;
+  at[0].val.programmaticStreamSerializationAllowed = st.pdl;
   cfg.attrs = at; cfg.numAttrs = 1;
   cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
 }
 
 template <int kVec>
-void launch_norm(cudaStream_t s, const float *X, bf16 *Y, const bf16 *g, const bf16 *b, int N, float eps, int rms, int rev) {
+void launch_norm(Strm s, const float *X, bf16 *Y, const bf16 *g, const bf16 *b, int N, float eps, int rms, int rev) {
   launch_k(norm_kernel<kVec>, (N + 7) / 8, 256, 0, s, X, Y, g, b, N, eps, rms, rev);
 }
-bool dispatch_norm(cudaStream_t s, int d, const float *X, bf16 *Y, const bf16 *g, const bf16 *b, int N, float eps, int rms, int rev) {
+bool dispatch_norm(Strm s, int d, const float *X, bf16 *Y, const bf16 *g, const bf16 *b, int N, float eps, int rms, int rev) {
   switch (d / 128) {
     case 1: launch_norm<1>(s, X, Y, g, b, N, eps, rms, rev); return true;
     case 2: launch_norm<2>(s, X, Y, g, b, N, eps, rms, rev); return true;
@@ -304,7 +336,7 @@ bool dispatch_norm(cudaStream_t s, int d, const float *X, bf16 *Y, const bf16 *g
   }
   return false;
 }
-bool dispatch_pool(cudaStream_t s, int d, int B, const PoolArgs &a) {
+bool dispatch_pool(Strm s, int d, int B, const PoolArgs &a) {
   switch (d / 128) {
     case 1: launch_k(final_pool_kernel<1>, B, 128, 0, s, a); return true;
     case 2: launch_k(final_pool_kernel<2>, B, 128, 0, s, a); return true;
@@ -321,8 +353,8 @@ bool norm_dim_supported(int d) {
   return d % 128 == 0 && (v == 1 || v == 2 || v == 4 || v == 6 || v == 8 || v == 12 || v == 16);
 }
 
-void launch_shrink(fmx_ctx *c, cudaStream_t s, const GemmParams &p) {
-  if (g_shrink_stages == 4) launch_k((shrink_kernel<4, 3>), c->sm_count, kGemmThreads, (shrink_smem_bytes<4, 3>()), s, p);
+void launch_shrink(fmx_ctx *c, Strm s, const GemmParams &p) {
+  if (c->o.shrink_stages == 4) launch_k((shrink_kernel<4, 3>), c->sm_count, kGemmThreads, (shrink_smem_bytes<4, 3>()), s, p);
   else if (p.n_tg == 1) launch_k((shrink_kernel<8, 1>), c->sm_count, kGemmThreads, (shrink_smem_bytes<8, 1>()), s, p);
   else if (p.n_tg == 2) launch_k((shrink_kernel<6, 2>), c->sm_count, kGemmThreads, (shrink_smem_bytes<6, 2>()), s, p);
   else launch_k((shrink_kernel<5, 3>), c->sm_count, kGemmThreads, (shrink_smem_bytes<5, 3>()), s, p);
@@ -330,18 +362,18 @@ void launch_shrink(fmx_ctx *c, cudaStream_t s, const GemmParams &p) {
 
 // Pair tiles 256 x 256 when the chunk count is even, else 256 x 128; one cluster of 2 CTAs per SM pair.
 bool pair_wide(const PairGemmParams &p) { return p.n_chunks % 2 == 0; }
-void launch_pair_gemm(fmx_ctx *c, cudaStream_t s, const PairGemmParams &p) {
+void launch_pair_gemm(fmx_ctx *c, Strm s, const PairGemmParams &p) {
   const int pairs = c->sm_count / 2;
   // fp32-output modes (residual reduce-add, embed) take the deep variant: one more pipeline stage, one staging buffer
-  const bool deep = g_deep_pipe && (p.mode == GM_RESID_F32 || p.mode == GM_EMBED_F32 || p.mode == GM_OUT_F32);
+  const bool deep = c->o.deep_pipe && (p.mode == GM_RESID_F32 || p.mode == GM_EMBED_F32 || p.mode == GM_OUT_F32);
   if (pair_wide(p)) {
     const int tiles = p.n_ptiles * (p.n_chunks / 2);
     // Wave quantisation: when the last wave would hold at most half as many tiles as there are pairs, its tiles are cut
     // into 256 x 128 halves so that it lasts half a tile time (cfg2 O / FFN-out: 256 tiles on 74 pairs, 4 -> 3.5 waves).
     PairGemmParams q = p;
-    q.expand_wide = g_expand_wide;
+    q.expand_wide = c->o.expand_wide;
     const int rem = tiles % pairs;
-    q.n_full = (g_half_tiles && p.mode != GM_OUT_BF16_SWIGLU && !p.rope_cs && tiles > pairs && rem > 0 && 2 * rem <= pairs) ? tiles - rem : -1;
+    q.n_full = (c->o.half_tiles && p.mode != GM_OUT_BF16_SWIGLU && !p.rope_cs && tiles > pairs && rem > 0 && 2 * rem <= pairs) ? tiles - rem : -1;
     const int items = q.n_full >= 0 ? q.n_full + 2 * rem : tiles;
     const int grid = 2 * (p.n_sh > 0 ? pairs : std::min(items, pairs));
     if (deep) launch_k((pair_gemm_kernel<256, true>), grid, kGemmThreads, (pair_smem_bytes<256, true>()), s, q);
@@ -355,22 +387,20 @@ void launch_pair_gemm(fmx_ctx *c, cudaStream_t s, const PairGemmParams &p) {
 }
 
 // Every request <= 64 tokens: the pipelined single-tile kernel (4 CTAs per SM, each walking a strided item list).
-int g_reverse = 1;       // consecutive kernels of a layer walk the rows in alternating directions (L2 reuse)
-int g_attn_short = 2;    // 0: generic kernel, 1: pipelined mma.sync kernel, 2: tcgen05 head-pair kernel where it applies (d_h 64, even H_q)
-bool attn_pair64_ok(int dh, int n_q_heads, int max_len) { return g_attn_short == 2 && dh == 64 && n_q_heads % 2 == 0 && max_len <= 64; }
-void launch_attention_pair64(cudaStream_t s, int sm_count, const AttnPairArgs &a) {
+bool attn_pair64_ok(const Opts &o, int dh, int n_q_heads, int max_len) { return o.attn_short == 2 && dh == 64 && n_q_heads % 2 == 0 && max_len <= 64; }
+void launch_attention_pair64(Strm s, int sm_count, const AttnPairArgs &a) {
   const int items = a.n_req * (a.n_q_heads / 2);
   const int grid = std::min(sm_count, (items + kP64Lanes - 1) / kP64Lanes);
   launch_k(attention_pair64_kernel, grid, kP64Threads, attn_pair64_smem_bytes(), s, a);
 }
-void launch_attention_short(cudaStream_t s, int sm_count, int dh, int n_req, const AttnArgs &a) {
+void launch_attention_short(Strm s, int sm_count, int dh, int n_req, const AttnArgs &a) {
   const int items = n_req * a.n_q_heads;
   const int grid = std::min(items, sm_count * 4);
   if (dh == 32) launch_k(attention_short_kernel<32>, grid, kAttnThreads, attn_short_smem_bytes<32>(), s, a, n_req);
   else if (dh == 64) launch_k(attention_short_kernel<64>, grid, kAttnThreads, attn_short_smem_bytes<64>(), s, a, n_req);
   else launch_k(attention_short_kernel<128>, std::min(items, sm_count * 2), kAttnThreads, attn_short_smem_bytes<128>(), s, a, n_req);
 }
-void launch_attention(cudaStream_t s, int dh, dim3 grid, const AttnArgs &a) {
+void launch_attention(Strm s, int dh, dim3 grid, const AttnArgs &a) {
   if (dh == 32) launch_k(attention_kernel<32>, grid, kAttnThreads, attn_smem_bytes<32>(), s, a);
   else if (dh == 64) launch_k(attention_kernel<64>, grid, kAttnThreads, attn_smem_bytes<64>(), s, a);
   else launch_k(attention_kernel<128>, grid, kAttnThreads, attn_smem_bytes<128>(), s, a);
@@ -390,14 +420,14 @@ bool attn_use_lanes(int impl, int dh, int max_len) {
   return impl == FMX_ATTN_LANES;
 }
 template <int DH, int kLanes>
-void launch_attention_lanes_v(cudaStream_t s, int sm_count, int max_len, const AttnLaneArgs &a0) {
+void launch_attention_lanes_v(Strm s, int sm_count, int max_len, const AttnLaneArgs &a0) {
   AttnLaneArgs a = a0;
   a.n_qt_max = (max_len + kAtBQ - 1) / kAtBQ;
   const long long items = (long long)a.n_qt_max * a.n_req * a.n_q_heads;
   const int grid = (int)std::min<long long>(sm_count, (items + kLanes - 1) / kLanes);
   launch_k((attention_lanes_kernel<DH, kLanes>), grid, attn_lanes_threads<kLanes>(), attn_lanes_smem_bytes<DH, kLanes>(), s, a);
 }
-void launch_attention_lanes(cudaStream_t s, int sm_count, int dh, int variant, int max_len, const AttnLaneArgs &a) {
+void launch_attention_lanes(Strm s, int sm_count, int dh, int variant, int max_len, const AttnLaneArgs &a) {
   if (dh == 64) {
     if (variant == 0) launch_attention_lanes_v<64, 4>(s, sm_count, max_len, a);
     else if (variant == 1) launch_attention_lanes_v<64, 2>(s, sm_count, max_len, a);
@@ -407,11 +437,11 @@ void launch_attention_lanes(cudaStream_t s, int sm_count, int dh, int variant, i
   }
 }
 template <int DH, int kQT, int kSt, int kMinB>
-void launch_attention_tc_v(cudaStream_t s, int max_len, int n_heads, int B, const AttnTcArgs &a) {
+void launch_attention_tc_v(Strm s, int max_len, int n_heads, int B, const AttnTcArgs &a) {
   dim3 grid((max_len + kAtBQ * kQT - 1) / (kAtBQ * kQT), n_heads, B);
   launch_k((attention_tc_kernel<DH, kQT, kSt, kMinB>), grid, attn_tc_threads<kQT>(), attn_tc_smem_bytes<DH, kQT, kSt>(), s, a);
 }
-void launch_attention_tc(cudaStream_t s, int dh, int variant, int max_len, int n_heads, int B, const AttnTcArgs &a) {
+void launch_attention_tc(Strm s, int dh, int variant, int max_len, int n_heads, int B, const AttnTcArgs &a) {
   if (dh == 64) {
     if (variant == 0) launch_attention_tc_v<64, 1, 3, 2>(s, max_len, n_heads, B, a);
     else launch_attention_tc_v<64, 2, 3, 1>(s, max_len, n_heads, B, a);
@@ -486,41 +516,98 @@ int rebuild_slab_maps(fmx_ctx *c, Backbone &bb, int tg) {
   return FMX_OK;
 }
 
+// Forwards in flight may still read what an unregister or a slab growth is about to free.  The retirement stream waits
+// (on the device) for the registration stream and for the latest forward of every serving stream, then frees; the host
+// never waits.  Every retirement gets a sequence number; a later registration that wants to REUSE a freed task slot or
+// freed slab columns makes the registration stream wait for that retirement first (wait_retired).
+int retire(fmx_ctx *c, const std::vector<void *> &ptrs) {
+  CU_OK(cudaEventRecord(c->side_ev, c->side));
+  CU_OK(cudaStreamWaitEvent(c->side2, c->side_ev, 0));
+  for (auto &sv : c->serving)
+    if (sv.used) CU_OK(cudaStreamWaitEvent(c->side2, sv.ev, 0));
+  for (void *q : ptrs) if (q) CU_OK(cudaFreeAsync(q, c->side2));
+  CU_OK(cudaEventRecord(c->retire_ev, c->side2));
+  ++c->retire_seq;
+  return FMX_OK;
+}
+int wait_retired(fmx_ctx *c, unsigned long long seq) {
+  if (seq <= c->retire_done) return FMX_OK;
+  if (cudaEventQuery(c->retire_ev) == cudaSuccess) { c->retire_done = c->retire_seq; return FMX_OK; }
+  cudaGetLastError();                                    // cudaErrorNotReady is not an error
+  CU_OK(cudaStreamWaitEvent(c->side, c->retire_ev, 0));   // covers every earlier retirement: the stream is ordered
+  return FMX_OK;
+}
+
+// Called at the end of every forward enqueued on `s` (not while capturing).
+int note_forward(fmx_ctx *c, cudaStream_t s) {
+  fmx_ctx::Serving *slot = nullptr;
+  for (auto &sv : c->serving) if (sv.used && sv.stream == s) { slot = &sv; break; }
+  if (!slot) {
+    for (auto &sv : c->serving) if (!sv.used) { slot = &sv; break; }
+    if (!slot) {                                        // all entries taken: the least recently used one is replaced; the
+      slot = &c->serving[0];                            // retirement stream inherits its dependency first
+      for (auto &sv : c->serving) if (sv.tick < slot->tick) slot = &sv;
+      CU_OK(cudaStreamWaitEvent(c->side2, slot->ev, 0));
+    }
+    if (!slot->ev) CU_OK(cudaEventCreateWithFlags(&slot->ev, cudaEventDisableTiming));
+    slot->stream = s; slot->used = true;
+  }
+  slot->tick = ++c->serve_tick;
+  CU_OK(cudaEventRecord(slot->ev, s));
+  return FMX_OK;
+}
+
+// First adapter on a target: its slabs, zero-filled, from the stream-ordered pool on the registration stream.
 int alloc_slab(fmx_ctx *c, Backbone &bb, int tg) {
   const size_t L = bb.d.n_layers;
   const size_t na = L * bb.Rcap * bb.din[tg], nb = L * bb.dout[tg] * bb.Rcap;
-  CU_OK(cudaMalloc(&bb.slabA[tg], na * sizeof(bf16)));
-  CU_OK(cudaMalloc(&bb.slabB[tg], nb * sizeof(bf16)));
-  CU_OK(cudaMemset(bb.slabA[tg], 0, na * sizeof(bf16)));
-  CU_OK(cudaMemset(bb.slabB[tg], 0, nb * sizeof(bf16)));
-  CU_OK(cudaDeviceSynchronize());           // rare path; the registration stream is not ordered after the legacy stream
+  bf16 *A = nullptr, *B = nullptr;
+  CU_OK(cudaMallocAsync(&A, na * sizeof(bf16), c->side));
+  if (cudaError_t e = cudaMallocAsync(&B, nb * sizeof(bf16), c->side)) {
+    cudaFreeAsync(A, c->side);
+    return fmx_fail(FMX_E_CUDA, "register_task: LoRA slab allocation failed: %s", cudaGetErrorString(e));
+  }
+  CU_OK(cudaMemsetAsync(A, 0, na * sizeof(bf16), c->side));
+  CU_OK(cudaMemsetAsync(B, 0, nb * sizeof(bf16), c->side));
+  bb.slabA[tg] = A; bb.slabB[tg] = B;
   return rebuild_slab_maps(c, bb, tg);
 }
 
+// The arena is full: a twice as wide one is built on the registration stream (the old columns copied over) while forwards
+// keep reading the old one; the descriptors switch at a forward boundary (forwards enqueued from now on take the new maps)
+// and the old arena is released once the forwards that were in flight are done - no device-wide synchronisation.
 int grow_slabs(fmx_ctx *c, Backbone &bb, int new_cap) {
   const size_t L = bb.d.n_layers;
   const int old = bb.Rcap;
+  bf16 *nA[7] = {nullptr}, *nB[7] = {nullptr};
+  auto undo = [&]() { for (int tg = 0; tg < 7; ++tg) { if (nA[tg]) cudaFreeAsync(nA[tg], c->side); if (nB[tg]) cudaFreeAsync(nB[tg], c->side); } };
   for (int tg = 0; tg < 7; ++tg) {
     if (!bb.slabA[tg]) continue;
-    bf16 *nA = nullptr, *nB = nullptr;
     const size_t na = L * new_cap * bb.din[tg], nb = L * bb.dout[tg] * (size_t)new_cap;
-    CU_OK(cudaMalloc(&nA, na * sizeof(bf16)));
-    CU_OK(cudaMalloc(&nB, nb * sizeof(bf16)));
-    CU_OK(cudaMemset(nA, 0, na * sizeof(bf16)));
-    CU_OK(cudaMemset(nB, 0, nb * sizeof(bf16)));
-    for (size_t l = 0; l < L; ++l)
-      CU_OK(cudaMemcpy(nA + l * new_cap * bb.din[tg], bb.slabA[tg] + l * old * bb.din[tg], (size_t)old * bb.din[tg] * sizeof(bf16),
-                       cudaMemcpyDeviceToDevice));
-    CU_OK(cudaMemcpy2D(nB, (size_t)new_cap * sizeof(bf16), bb.slabB[tg], (size_t)old * sizeof(bf16), (size_t)old * sizeof(bf16),
-                       L * bb.dout[tg], cudaMemcpyDeviceToDevice));
-    cudaFree(bb.slabA[tg]);
-    cudaFree(bb.slabB[tg]);
-    bb.slabA[tg] = nA;
-    bb.slabB[tg] = nB;
+    cudaError_t e = cudaMallocAsync(&nA[tg], na * sizeof(bf16), c->side);
+    if (e == cudaSuccess) e = cudaMallocAsync(&nB[tg], nb * sizeof(bf16), c->side);
+    if (e == cudaSuccess) e = cudaMemsetAsync(nA[tg], 0, na * sizeof(bf16), c->side);
+    if (e == cudaSuccess) e = cudaMemsetAsync(nB[tg], 0, nb * sizeof(bf16), c->side);
+    if (e == cudaSuccess)
+      e = cudaMemcpy2DAsync(nA[tg], (size_t)new_cap * bb.din[tg] * sizeof(bf16), bb.slabA[tg], (size_t)old * bb.din[tg] * sizeof(bf16),
+                            (size_t)old * bb.din[tg] * sizeof(bf16), L, cudaMemcpyDeviceToDevice, c->side);
+    if (e == cudaSuccess)
+      e = cudaMemcpy2DAsync(nB[tg], (size_t)new_cap * sizeof(bf16), bb.slabB[tg], (size_t)old * sizeof(bf16), (size_t)old * sizeof(bf16),
+                            L * bb.dout[tg], cudaMemcpyDeviceToDevice, c->side);
+    if (e != cudaSuccess) { undo(); return fmx_fail(FMX_E_CUDA, "register_task: growing the LoRA slabs to %d columns failed: %s", new_cap, cudaGetErrorString(e)); }
   }
-  CU_OK(cudaDeviceSynchronize());           // rare path: forwards in flight used the old slabs, the copies ran on the legacy stream
+  // commit: nothing below fails short of a broken context
+  std::vector<void *> old_slabs;
+  for (int tg = 0; tg < 7; ++tg) if (bb.slabA[tg]) { old_slabs.push_back(bb.slabA[tg]); old_slabs.push_back(bb.slabB[tg]); }
+  if (int e = retire(c, old_slabs)) { undo(); return e; }
+  for (int tg = 0; tg < 7; ++tg) {
+    if (!bb.slabA[tg]) continue;
+    bb.slabA[tg] = nA[tg];
+    bb.slabB[tg] = nB[tg];
+  }
   bb.Rcap = new_cap;
   bb.col_used.resize(new_cap / 16, 0);
+  bb.col_freed_seq.resize(new_cap / 16, 0);
   for (int tg = 0; tg < 7; ++tg)
     if (bb.slabA[tg]) if (int e = rebuild_slab_maps(c, bb, tg)) return e;
   return FMX_OK;
@@ -537,12 +624,10 @@ int find_columns(const Backbone &bb, int units) {        // first fit, units of 
   return -1;
 }
 
-int upload_task_tables(fmx_ctx *c, int t) {
+int upload_task_tables(fmx_ctx *c, int t, const TaskRec &r) {
   // One task's entries of the device tables, through a pinned staging struct on the registration stream (no legacy-stream
   // cudaMemcpy: that would wait for forwards running on the default stream).  The caller synchronises c->side afterwards.
-  const TaskRec &r = c->tasks[t];
-  CU_OK(cudaStreamSynchronize(c->side));                   // the staging struct is free
-  fmx_ctx::TaskStage &h = *c->h_task_stage;
+  fmx_ctx::TaskStage &h = *c->h_task_stage;                // free: every registration ends with a synchronise of c->side
   h.coff = r.coff; h.head_kind = r.head_kind; h.head_out = r.head_out; h.w1 = r.head_hidden > 0 ? r.head_hidden : r.head_out;
   h.enc_ch = r.enc_channels;
   memcpy(h.trpad, r.trpad, 7); memcpy(h.scale, r.scale, sizeof(r.scale));
@@ -644,7 +729,22 @@ int fmx_create(fmx_ctx **out, int device_ordinal) {
   CU_OK(cudaMallocHost(&c->h_stage, sizeof(int) * 2 * FMX_MAX_REQUESTS * (fmx_ctx::kStageSlots + 1)));
   for (int i = 0; i < fmx_ctx::kStageSlots; ++i) CU_OK(cudaEventCreateWithFlags(&c->stage_ev[i], cudaEventDisableTiming));
   CU_OK(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
+  CU_OK(cudaStreamCreateWithFlags(&c->side2, cudaStreamNonBlocking));
+  CU_OK(cudaEventCreateWithFlags(&c->side_ev, cudaEventDisableTiming));
+  CU_OK(cudaEventCreateWithFlags(&c->retire_ev, cudaEventDisableTiming));
   CU_OK(cudaMallocHost(&c->h_task_stage, sizeof(fmx_ctx::TaskStage)));
+  CU_OK(cudaHostAlloc(&c->h_err, sizeof(unsigned), cudaHostAllocMapped));
+  *c->h_err = 0;
+  CU_OK(cudaHostGetDevicePointer(&c->d_err, c->h_err, 0));
+  CU_OK(cudaMalloc(&c->d_dbg_cu, sizeof(int) * (FMX_MAX_REQUESTS + 1)));
+  {
+    // task tensors and LoRA slabs come from the device's stream-ordered pool on the registration stream (cudaFree would
+    // synchronise the whole device; cudaFreeAsync does not); keep freed memory cached in the pool
+    cudaMemPool_t pool = nullptr;
+    CU_OK(cudaDeviceGetDefaultMemPool(&pool, device_ordinal));
+    unsigned long long keep = ~0ull;
+    CU_OK(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+  }
   *out = c.release();
   fmx_clear_error();
   return FMX_OK;
@@ -659,19 +759,27 @@ int fmx_destroy(fmx_ctx *c) {
   for (auto &bp : c->bbs) {
     if (!bp) continue;
     cudaFree(bp->embed_Wpad); cudaFree(bp->posb); cudaFree(bp->rope_cs); cudaFree(bp->rope_cs_t);
-    for (int tg = 0; tg < 7; ++tg) { cudaFree(bp->slabA[tg]); cudaFree(bp->slabB[tg]); }
+    for (int tg = 0; tg < 7; ++tg) { if (bp->slabA[tg]) cudaFreeAsync(bp->slabA[tg], c->side); if (bp->slabB[tg]) cudaFreeAsync(bp->slabB[tg], c->side); }
   }
-  for (auto &t : c->tasks) { cudaFree(t.head_W); cudaFree(t.head_b); cudaFree(t.head_W2); cudaFree(t.head_b2); cudaFree(t.enc_W); cudaFree(t.enc_b); }
+  for (auto &t : c->tasks)
+    for (bf16 *q : {t.head_W, t.head_b, t.head_W2, t.head_b2, t.enc_W, t.enc_b}) if (q) cudaFreeAsync(q, c->side);
+  cudaStreamSynchronize(c->side);
+  cudaStreamSynchronize(c->side2);
   cudaFree(c->d_task_coff); cudaFree(c->d_task_head_kind); cudaFree(c->d_task_head_out); cudaFree(c->d_task_trpad);
   cudaFree(c->d_task_scale); cudaFree(c->d_task_head_W); cudaFree(c->d_task_head_b);
-  cudaFree(c->d_task_head_W2); cudaFree(c->d_task_head_b2); cudaFree(c->d_task_head_w1); cudaFree(c->d_head_hid);
+  cudaFree(c->d_task_head_W2); cudaFree(c->d_task_head_b2); cudaFree(c->d_task_head_w1);
   cudaFree(c->d_task_enc_ch); cudaFree(c->d_task_enc_W); cudaFree(c->d_task_enc_b);
-  cudaFree(c->d_in_stage); cudaFree(c->d_out_stage); cudaFree(c->d_dbg_cu); cudaFree(c->d_head_part);
+  cudaFree(c->d_dbg_cu);
+  for (auto &sv : c->serving) if (sv.ev) cudaEventDestroy(sv.ev);
+  cudaFreeHost(c->h_err);
   if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
   for (int i = 0; i < fmx_ctx::kStageSlots; ++i) if (c->stage_ev[i]) cudaEventDestroy(c->stage_ev[i]);
   cudaFreeHost(c->h_stage);
   cudaFreeHost(c->h_task_stage);
+  if (c->side_ev) cudaEventDestroy(c->side_ev);
+  if (c->retire_ev) cudaEventDestroy(c->retire_ev);
   if (c->side) cudaStreamDestroy(c->side);
+  if (c->side2) cudaStreamDestroy(c->side2);
   delete c;
   return FMX_OK;
 }
@@ -764,6 +872,7 @@ int fmx_register_backbone(fmx_ctx *c, const fmx_backbone_desc *desc, fmx_backbon
   CU_OK(cudaDeviceSynchronize());
   b->Rcap = 256;
   b->col_used.assign(b->Rcap / 16, 0);
+  b->col_freed_seq.assign(b->Rcap / 16, 0);
   c->bbs.push_back(std::move(b));
   *out = (int)c->bbs.size() - 1;
   return FMX_OK;
@@ -772,7 +881,6 @@ int fmx_register_backbone(fmx_ctx *c, const fmx_backbone_desc *desc, fmx_backbon
 int fmx_register_task(fmx_ctx *c, fmx_backbone_t h, const fmx_task_desc *desc, fmx_task_t *out) {
   if (!c || !desc || !out) return fmx_fail(FMX_E_INVALID_ARG, "register_task: NULL argument");
   std::lock_guard<std::mutex> lk(c->mu);
-  ++c->config_gen;                      // invalidates the cached forward graph
   CU_OK(cudaSetDevice(c->device));
   Backbone *bb = get_bb(c, h);
   if (!bb) return fmx_fail(FMX_E_UNKNOWN_BACKBONE, "register_task: unknown backbone %d", h);
@@ -782,7 +890,7 @@ int fmx_register_task(fmx_ctx *c, fmx_backbone_t h, const fmx_task_desc *desc, f
   if (desc->n_adapters < 0 || desc->n_adapters > 7 || (desc->n_adapters && !desc->adapters)) return fmx_fail(FMX_E_INVALID_ARG, "register_task: bad n_adapters");
   if (desc->head_kind < 0 || desc->head_kind > 3 || desc->head_out < 1 || !desc->head_W) return fmx_fail(FMX_E_INVALID_ARG, "register_task: bad head");
   if (desc->head_kind == FMX_HEAD_FLATTEN && d.tokens_per_request < 1) return fmx_fail(FMX_E_SHAPE, "register_task: FLATTEN head needs a fixed-length backbone");
-  if (desc->head_hidden < 0 || desc->head_hidden > 4096) return fmx_fail(FMX_E_SHAPE, "register_task: head_hidden %d not in [0,4096]", desc->head_hidden);
+  if (desc->head_hidden < 0 || desc->head_hidden > kMaxHeadHidden) return fmx_fail(FMX_E_SHAPE, "register_task: head_hidden %d not in [0,%d]", desc->head_hidden, kMaxHeadHidden);
   if (desc->head_hidden > 0 && desc->head_kind == FMX_HEAD_FLATTEN) return fmx_fail(FMX_E_SHAPE, "register_task: an MLP head needs a pooled feature (mean / cls / last)");
   if (desc->head_hidden > 0 && !desc->head_W2) return fmx_fail(FMX_E_INVALID_ARG, "register_task: MLP head without head_W2");
   if (desc->enc_channels < 0 || desc->enc_channels > 16) return fmx_fail(FMX_E_SHAPE, "register_task: enc_channels %d not in [0,16]", desc->enc_channels);
@@ -806,108 +914,119 @@ int fmx_register_task(fmx_ctx *c, fmx_backbone_t h, const fmx_task_desc *desc, f
   for (int t = 0; t < FMX_MAX_TASKS; ++t) if (!c->tasks[t].live) { slot = t; break; }
   if (slot < 0) return fmx_fail(FMX_E_CAPACITY, "register_task: all %d task slots in use", FMX_MAX_TASKS);
 
+  // Nothing below changes the registry until the last fallible call has succeeded: buffers are allocated first, the slab
+  // arena may grow (a grown arena is a valid state by itself), the copies are enqueued, and only then are the columns, the
+  // adapter counts and the task record committed.  On failure the buffers allocated here go back to the pool.
   TaskRec r;
   r.live = true; r.bb = h; r.head_kind = desc->head_kind; r.head_out = desc->head_out; r.head_hidden = desc->head_hidden; r.rpad = rpad;
+  r.freed_seq = c->tasks[slot].freed_seq;
+  std::vector<void *> mine;
+  auto fail = [&](int code) { for (void *q : mine) cudaFreeAsync(q, c->side); return code; };
+  auto dup = [&](bf16 **dst, const void *src, size_t n) -> int {           // device -> device copy into a pool allocation
+    cudaError_t e = cudaMallocAsync(dst, n * sizeof(bf16), c->side);
+    if (e != cudaSuccess) { *dst = nullptr; return fmx_fail(FMX_E_CUDA, "register_task: cudaMallocAsync(%zu B) failed: %s", n * sizeof(bf16), cudaGetErrorString(e)); }
+    mine.push_back(*dst);
+    e = cudaMemcpyAsync(*dst, src, n * sizeof(bf16), cudaMemcpyDeviceToDevice, c->side);
+    if (e != cudaSuccess) return fmx_fail(FMX_E_CUDA, "register_task: copy failed: %s", cudaGetErrorString(e));
+    return FMX_OK;
+  };
+  // ---- head / encoder buffers ----
+  const size_t d_feat = desc->head_kind == FMX_HEAD_FLATTEN ? (size_t)d.tokens_per_request * d.d_model : (size_t)d.d_model;
+  const size_t w1 = desc->head_hidden > 0 ? (size_t)desc->head_hidden : (size_t)desc->head_out;     // rows of the first layer
+  if (int e = dup(&r.head_W, desc->head_W, d_feat * w1)) return fail(e);
+  if (desc->head_b) if (int e = dup(&r.head_b, desc->head_b, w1)) return fail(e);
+  if (desc->enc_channels > 1) {
+    r.enc_channels = desc->enc_channels;
+    if (int e = dup(&r.enc_W, desc->enc_W, desc->enc_channels)) return fail(e);
+    if (desc->enc_b) if (int e = dup(&r.enc_b, desc->enc_b, 1)) return fail(e);
+  }
+  if (desc->head_hidden > 0) {
+    if (int e = dup(&r.head_W2, desc->head_W2, (size_t)desc->head_out * desc->head_hidden)) return fail(e);
+    if (desc->head_b2) if (int e = dup(&r.head_b2, desc->head_b2, desc->head_out)) return fail(e);
+  }
   // ---- slab columns ----
+  int pos = -1, units = rpad / 16;
   if (rpad) {
-    int units = rpad / 16, pos = find_columns(*bb, units);
-    if (pos < 0) {
-      int new_cap = bb->Rcap;
-      while (pos < 0) {
-        new_cap *= 2;
-        if (new_cap > 16 * 65536) return fmx_fail(FMX_E_CAPACITY, "register_task: LoRA slab capacity exceeded");
-        if (int e = grow_slabs(c, *bb, new_cap)) return e;
-        pos = find_columns(*bb, units);
-      }
+    pos = find_columns(*bb, units);
+    int new_cap = bb->Rcap;
+    while (pos < 0) {
+      new_cap *= 2;
+      if (new_cap > 16 * 65536) return fail(fmx_fail(FMX_E_CAPACITY, "register_task: LoRA slab capacity exceeded"));
+      if (int e = grow_slabs(c, *bb, new_cap)) return fail(e);
+      pos = find_columns(*bb, units);
     }
     r.coff = pos * 16;
+    for (int i = 0; i < desc->n_adapters; ++i)
+      if (!bb->slabA[desc->adapters[i].target]) if (int e = alloc_slab(c, *bb, desc->adapters[i].target)) return fail(e);
+    // a slot or columns handed back by a recent fmx_unregister_task may still be read by forwards that were in flight then
+    unsigned long long seq = r.freed_seq;
+    for (int u = 0; u < units; ++u) seq = std::max(seq, bb->col_freed_seq[pos + u]);
+    if (int e = wait_retired(c, seq)) return fail(e);
     for (int i = 0; i < desc->n_adapters; ++i) {
       const fmx_adapter_desc &a = desc->adapters[i];
-      const int tg = a.target;
-      if (!bb->slabA[tg]) if (int e = alloc_slab(c, *bb, tg)) return e;
+      const int tg = a.target, rp = (a.rank + 15) / 16 * 16;
       const int din = bb->din[tg], dout = bb->dout[tg];
       for (int l = 0; l < L; ++l) {
         bf16 *A = bb->slabA[tg] + ((size_t)l * bb->Rcap + r.coff) * din;
         bf16 *B = bb->slabB[tg] + (size_t)l * dout * bb->Rcap + r.coff;
-        CU_OK(cudaMemcpyAsync(A, a.A[l], (size_t)a.rank * din * sizeof(bf16), cudaMemcpyDeviceToDevice, c->side));
-        CU_OK(cudaMemcpy2DAsync(B, (size_t)bb->Rcap * sizeof(bf16), a.B[l], (size_t)a.rank * sizeof(bf16), (size_t)a.rank * sizeof(bf16),
-                                dout, cudaMemcpyDeviceToDevice, c->side));
+        cudaError_t e = cudaSuccess;
+        if (rp > a.rank) {                 // the zero padding of the rank (exact): whatever a previous owner left there goes
+          e = cudaMemsetAsync(A + (size_t)a.rank * din, 0, (size_t)(rp - a.rank) * din * sizeof(bf16), c->side);
+          if (e == cudaSuccess) e = cudaMemset2DAsync(B + a.rank, (size_t)bb->Rcap * sizeof(bf16), 0, (size_t)(rp - a.rank) * sizeof(bf16), dout, c->side);
+        }
+        if (e == cudaSuccess) e = cudaMemcpyAsync(A, a.A[l], (size_t)a.rank * din * sizeof(bf16), cudaMemcpyDeviceToDevice, c->side);
+        if (e == cudaSuccess)
+          e = cudaMemcpy2DAsync(B, (size_t)bb->Rcap * sizeof(bf16), a.B[l], (size_t)a.rank * sizeof(bf16), (size_t)a.rank * sizeof(bf16),
+                                dout, cudaMemcpyDeviceToDevice, c->side);
+        if (e != cudaSuccess) return fail(fmx_fail(FMX_E_CUDA, "register_task: adapter copy failed: %s", cudaGetErrorString(e)));
       }
-      r.trpad[tg] = (unsigned char)((a.rank + 15) / 16 * 16);
+      r.trpad[tg] = (unsigned char)rp;
       r.scale[tg] = a.scaling;
-      bb->n_adapters[tg]++;
     }
-    for (int u = 0; u < units; ++u) bb->col_used[pos + u] = 1;
+  } else if (int e = wait_retired(c, r.freed_seq)) {
+    return fail(e);
   }
-  // ---- head ----
-  const size_t d_feat = desc->head_kind == FMX_HEAD_FLATTEN ? (size_t)d.tokens_per_request * d.d_model : (size_t)d.d_model;
-  const size_t w1 = desc->head_hidden > 0 ? (size_t)desc->head_hidden : (size_t)desc->head_out;     // rows of the first layer
-  CU_OK(cudaMalloc(&r.head_W, sizeof(bf16) * d_feat * w1));
-  CU_OK(cudaMemcpyAsync(r.head_W, desc->head_W, sizeof(bf16) * d_feat * w1, cudaMemcpyDeviceToDevice, c->side));
-  if (desc->head_b) {
-    CU_OK(cudaMalloc(&r.head_b, sizeof(bf16) * w1));
-    CU_OK(cudaMemcpyAsync(r.head_b, desc->head_b, sizeof(bf16) * w1, cudaMemcpyDeviceToDevice, c->side));
-  }
-  if (desc->enc_channels > 1) {
-    r.enc_channels = desc->enc_channels;
-    CU_OK(cudaMalloc(&r.enc_W, sizeof(bf16) * desc->enc_channels));
-    CU_OK(cudaMemcpyAsync(r.enc_W, desc->enc_W, sizeof(bf16) * desc->enc_channels, cudaMemcpyDeviceToDevice, c->side));
-    if (desc->enc_b) {
-      CU_OK(cudaMalloc(&r.enc_b, sizeof(bf16)));
-      CU_OK(cudaMemcpyAsync(r.enc_b, desc->enc_b, sizeof(bf16), cudaMemcpyDeviceToDevice, c->side));
-    }
-  }
-  if (desc->head_hidden > 0) {
-    CU_OK(cudaMalloc(&r.head_W2, sizeof(bf16) * (size_t)desc->head_out * desc->head_hidden));
-    CU_OK(cudaMemcpyAsync(r.head_W2, desc->head_W2, sizeof(bf16) * (size_t)desc->head_out * desc->head_hidden, cudaMemcpyDeviceToDevice, c->side));
-    if (desc->head_b2) {
-      CU_OK(cudaMalloc(&r.head_b2, sizeof(bf16) * desc->head_out));
-      CU_OK(cudaMemcpyAsync(r.head_b2, desc->head_b2, sizeof(bf16) * desc->head_out, cudaMemcpyDeviceToDevice, c->side));
-    }
-  }
+  // ---- device tables, then commit ----
+  if (int e = upload_task_tables(c, slot, r)) return fail(e);
+  if (cudaError_t e = cudaStreamSynchronize(c->side))      // the caller may free its buffers; forwards in flight are not waited for
+    return fail(fmx_fail(FMX_E_CUDA, "register_task: %s", cudaGetErrorString(e)));
+  for (int u = 0; u < units; ++u) bb->col_used[pos + u] = 1;
+  for (int tg = 0; tg < 7; ++tg) if (r.trpad[tg]) bb->n_adapters[tg]++;
   c->tasks[slot] = r;
   c->n_slots = std::max(c->n_slots, slot + 1);
-  if (int e = upload_task_tables(c, slot)) return e;
-  CU_OK(cudaStreamSynchronize(c->side));                   // the caller may free its buffers; forwards in flight are not waited for
+  ++c->config_gen;                      // invalidates the cached forward graph
   *out = slot;
   return FMX_OK;
 }
 
+// No device-wide synchronisation: the task leaves the registry at once (later forwards reject its id), its buffers are freed
+// on the retirement stream after the forwards in flight, and its slot / slab columns carry the retirement's sequence number
+// so that a registration reusing them waits for it on the device.  Slab columns are not cleared: no live task reads them
+// (a registration zero-fills the padding of its own columns).
 int fmx_unregister_task(fmx_ctx *c, fmx_task_t t) {
   if (!c) return fmx_fail(FMX_E_INVALID_ARG, "unregister_task: NULL ctx");
   std::lock_guard<std::mutex> lk(c->mu);
-  ++c->config_gen;                      // invalidates the cached forward graph
   if (t < 0 || t >= FMX_MAX_TASKS || !c->tasks[t].live) return fmx_fail(FMX_E_UNKNOWN_TASK, "unregister_task: task %d is not registered", t);
   CU_OK(cudaSetDevice(c->device));
-  CU_OK(cudaDeviceSynchronize());
   TaskRec &r = c->tasks[t];
   Backbone *bb = get_bb(c, r.bb);
-  const int L = bb->d.n_layers;
-  for (int tg = 0; tg < 7; ++tg) {
-    if (!r.trpad[tg]) continue;
-    for (int l = 0; l < L; ++l) {      // leave unowned columns zero
-      bf16 *A = bb->slabA[tg] + ((size_t)l * bb->Rcap + r.coff) * bb->din[tg];
-      bf16 *B = bb->slabB[tg] + (size_t)l * bb->dout[tg] * bb->Rcap + r.coff;
-      CU_OK(cudaMemsetAsync(A, 0, (size_t)r.trpad[tg] * bb->din[tg] * sizeof(bf16), c->side));
-      CU_OK(cudaMemset2DAsync(B, (size_t)bb->Rcap * sizeof(bf16), 0, (size_t)r.trpad[tg] * sizeof(bf16), bb->dout[tg], c->side));
-    }
-    bb->n_adapters[tg]--;
-  }
-  for (int u = 0; u < r.rpad / 16; ++u) bb->col_used[r.coff / 16 + u] = 0;
-  cudaFree(r.head_W);
-  cudaFree(r.head_b);
-  cudaFree(r.head_W2);
-  cudaFree(r.head_b2);
-  cudaFree(r.enc_W);
-  cudaFree(r.enc_b);
+  if (int e = retire(c, {r.head_W, r.head_b, r.head_W2, r.head_b2, r.enc_W, r.enc_b})) return e;
+  for (int tg = 0; tg < 7; ++tg) if (r.trpad[tg]) bb->n_adapters[tg]--;
+  for (int u = 0; u < r.rpad / 16; ++u) { bb->col_used[r.coff / 16 + u] = 0; bb->col_freed_seq[r.coff / 16 + u] = c->retire_seq; }
   r = TaskRec();
-  if (int e = upload_task_tables(c, t)) return e;
-  CU_OK(cudaStreamSynchronize(c->side));
+  r.freed_seq = c->retire_seq;
+  ++c->config_gen;                      // invalidates the cached forward graph
   return FMX_OK;
 }
 
+static int output_layout_locked(fmx_ctx *c, const int32_t *task_ids, int32_t n_req, int64_t *out_off);
 int fmx_output_layout(fmx_ctx *c, const int32_t *task_ids, int32_t n_req, int64_t *out_off) {
   if (!c || !out_off || (n_req > 0 && !task_ids) || n_req < 0) return fmx_fail(FMX_E_INVALID_ARG, "output_layout: bad argument");
+  std::lock_guard<std::mutex> lk(c->mu);
+  return output_layout_locked(c, task_ids, n_req, out_off);
+}
+
+static int output_layout_locked(fmx_ctx *c, const int32_t *task_ids, int32_t n_req, int64_t *out_off) {
   int64_t run = 0;
   for (int i = 0; i < n_req; ++i) {
     const int t = task_ids[i];
@@ -921,11 +1040,20 @@ int fmx_output_layout(fmx_ctx *c, const int32_t *task_ids, int32_t n_req, int64_
 
 int fmx_workspace_bytes(fmx_ctx *c, fmx_backbone_t h, int32_t max_req, int64_t max_tokens, size_t *bytes) {
   if (!c || !bytes) return fmx_fail(FMX_E_INVALID_ARG, "workspace_bytes: NULL argument");
+  std::lock_guard<std::mutex> lk(c->mu);
   Backbone *bb = get_bb(c, h);
   if (!bb) return fmx_fail(FMX_E_UNKNOWN_BACKBONE, "workspace_bytes: unknown backbone %d", h);
   if (max_req < 1 || max_req > FMX_MAX_REQUESTS || max_tokens < 1 || max_tokens > (1ll << 24))
     return fmx_fail(FMX_E_CAPACITY, "workspace_bytes: max_req in [1,%d], max_tokens in [1,2^24]", FMX_MAX_REQUESTS);
   *bytes = carve(*bb, nullptr, max_req, max_tokens, FMX_MAX_TASKS).bytes;
+  return FMX_OK;
+}
+
+int fmx_host_workspace_bytes(fmx_ctx *c, fmx_backbone_t h, int32_t max_req, int64_t max_tokens, size_t max_input_bytes,
+                             int64_t max_output_floats, size_t *bytes) {
+  if (max_output_floats < 0) return fmx_fail(FMX_E_INVALID_ARG, "host_workspace_bytes: max_output_floats < 0");
+  if (int e = fmx_workspace_bytes(c, h, max_req, max_tokens, bytes)) return e;
+  *bytes += align_up(max_input_bytes, 1024) + align_up((size_t)max_output_floats * sizeof(float), 1024);
   return FMX_OK;
 }
 
@@ -958,28 +1086,32 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   if (w.bytes > workspace_bytes) return fmx_fail(FMX_E_WORKSPACE, "forward_mixed: workspace %zu B < required %zu B", workspace_bytes, w.bytes);
 
   const int Ni = (int)N;
-  g_pdl_eff = g_pdl == 1 || (g_pdl == 2 && Ni <= kPdlAutoRows);
+  const Strm S{s, (c->o.pdl == 1 || (c->o.pdl == 2 && Ni <= kPdlAutoRows)) ? 1 : 0};
   Launcher Lh{c, s};
   // Every kernel of the layer chain streams over all N rows and the next one reads what it wrote.  Walking the rows in
   // alternating directions lets each kernel start on the rows its producer wrote last, which are the ones still in L2.
   int dir = 0;
-  auto rev = [&]() { const int r = g_reverse ? dir : 0; dir ^= 1; return r; };
+  auto rev = [&]() { const int r = c->o.reverse ? dir : 0; dir ^= 1; return r; };
   // ---- S1: ids/lengths to the device, counting sort, tables ----
   cudaStreamCaptureStatus cap_status = cudaStreamCaptureStatusNone;
   if (!graph_capture) CU_OK(cudaStreamIsCapturing(s, &cap_status));
-  const bool user_capture = cap_status != cudaStreamCaptureStatusNone;      // the caller captures: no event calls here
+  // ids / lengths reach the device through the library's pinned staging ring, whose slots are rewritten a few calls later:
+  // a graph the CALLER captures would replay stale copies, so a capturing stream is refused (the library keeps its own
+  // graph cache, FMX_OPT_GRAPH).
+  if (cap_status != cudaStreamCaptureStatusNone)
+    return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed: the stream is being captured; capture is not supported (the library caches its own CUDA graph)");
   int slot = fmx_ctx::kStageSlots;                                         // the graph's buffer
   if (!graph_capture) {
     slot = c->stage_next;
     c->stage_next = (c->stage_next + 1) % fmx_ctx::kStageSlots;
-    if (c->stage_used[slot] && !user_capture) CU_OK(cudaEventSynchronize(c->stage_ev[slot]));
+    if (c->stage_used[slot]) CU_OK(cudaEventSynchronize(c->stage_ev[slot]));
   }
   int *stage = c->h_stage + (size_t)slot * 2 * FMX_MAX_REQUESTS;
   memcpy(stage, task_ids, sizeof(int) * B);
   memcpy(stage + FMX_MAX_REQUESTS, lengths, sizeof(int) * B);
   CU_OK(cudaMemcpyAsync(w.t.task_ids, stage, sizeof(int) * B, cudaMemcpyHostToDevice, s));
   CU_OK(cudaMemcpyAsync(w.t.lengths, stage + FMX_MAX_REQUESTS, sizeof(int) * B, cudaMemcpyHostToDevice, s));
-  if (!graph_capture && !user_capture) {
+  if (!graph_capture) {
     CU_OK(cudaEventRecord(c->stage_ev[slot], s));
     c->stage_used[slot] = true;
   }
@@ -990,8 +1122,8 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   else if (d.input_kind == FMX_INPUT_TOKEN_IDS) { sa.in_per_tok = 1; sa.in_per_req = 0; }
   else if (d.img_c) { sa.in_per_tok = 0; sa.in_per_req = (long long)d.img_c * d.img_hw * d.img_hw; }
   else { sa.in_per_tok = 0; sa.in_per_req = (long long)(d.tokens_per_request - (d.has_cls ? 1 : 0)) * d.patch_dim; }
-  LAUNCH(Lh, F_SORT, (launch_k(task_sort_kernel, 1, kSortThreads, 0, s, sa)));
-  LAUNCH(Lh, F_SORT, (launch_k(row_tables_kernel, (Ni + 255) / 256, 256, 0, s, w.t.cu_tok, B, Ni, w.t.row_req, w.t.row_pos)));
+  LAUNCH(Lh, F_SORT, (launch_k(task_sort_kernel, 1, kSortThreads, 0, S, sa)));
+  LAUNCH(Lh, F_SORT, (launch_k(row_tables_kernel, (Ni + 255) / 256, 256, 0, S, w.t.cu_tok, B, Ni, w.t.row_req, w.t.row_pos)));
 
   // ---- common GEMM parameter pieces ----
   GemmParams sbase{};                       // segmented shrink
@@ -1033,7 +1165,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     }
     if (p.n_tg == 0) return FMX_OK;
     p.reverse = rev();
-    LAUNCH(Lh, F_SHRINK, launch_shrink(c, s, p));
+    LAUNCH(Lh, F_SHRINK, launch_shrink(c, S, p));
     return FMX_OK;
   };
   // fused form: no launch; the GEMM that reads the same input computes U in its first work items
@@ -1068,7 +1200,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       lo = hi;
     }
   }
-  const bool fuse_ok = g_shrink_fused && c->pairs_resident && (g_shrink_fused == 2 || n_blk_host <= c->sm_count / 2);
+  const bool fuse_ok = c->o.shrink_fused && c->pairs_resident && (c->o.shrink_fused == 2 || n_blk_host <= c->sm_count / 2);
   if (fuse_ok) CU_OK(cudaMemsetAsync(w.u_flag, 0, sizeof(unsigned), s));
   // fusable: all CTA pairs of the persistent grid are co-resident (the expand steps spin on another pair's result) and
   // a 3-target group needs the 256-wide kernel
@@ -1091,17 +1223,18 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     pa.task_enc_W = (const bf16 *const *)c->d_task_enc_W; pa.task_enc_b = (const bf16 *const *)c->d_task_enc_b;
     pa.series_len = (d.tokens_per_request - (d.has_cls ? 1 : 0)) * d.patch_dim;
     pa.A = w.Hid;
-    LAUNCH(Lh, F_EMBED, (launch_k(pack_patches_kernel, Ni, 128, 0, s, pa)));
+    LAUNCH(Lh, F_EMBED, (launch_k(pack_patches_kernel, Ni, 128, 0, S, pa)));
     if ((e = encode_2d(c, &mPk, w.Hid, Ni, bb.Kp, bb.Kp, 128))) return e;
     PairGemmParams p = base;
     p.mode = GM_EMBED_F32; p.amap = mPk; p.K = bb.Kp; p.n_chunks = d.d_model / 128;
     p.wmap[0] = bb.mEmbedW[wv(p)]; p.wmap_h[0] = bb.mEmbedW[1]; p.omap = oX; p.posb = bb.posb; p.ld_pos = d.d_model;
-    LAUNCH(Lh, F_EMBED, launch_pair_gemm(c, s, p));
+    LAUNCH(Lh, F_EMBED, launch_pair_gemm(c, S, p));
   } else {
     EmbedArgs ea{};
     ea.inputs = inputs; ea.perm = w.t.perm; ea.row_req = w.t.row_req; ea.row_pos = w.t.row_pos; ea.in_off = w.t.in_off;
     ea.N = Ni; ea.d = d.d_model; ea.X = w.X; ea.table = (const bf16 *)d.embed_table; ea.pos = (const bf16 *)d.embed_pos;
-    LAUNCH(Lh, F_EMBED, (launch_k(embed_rows_kernel, (Ni + 7) / 8, 256, 0, s, ea, d.input_kind == FMX_INPUT_TOKEN_IDS)));
+    ea.vocab = d.vocab; ea.err = c->d_err;
+    LAUNCH(Lh, F_EMBED, (launch_k(embed_rows_kernel, (Ni + 7) / 8, 256, 0, S, ea, d.input_kind == FMX_INPUT_TOKEN_IDS)));
   }
 
   // ---- layers ----
@@ -1109,7 +1242,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   const float scale_log2 = 1.4426950408889634f / sqrtf((float)d.head_dim);
   bool rope_fused = false;
   for (int l = 0; l < d.n_layers; ++l) {
-    LAUNCH(Lh, F_NORM, dispatch_norm(s, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm1_g[l], (const bf16 *)bb.norm1_b[l], Ni, d.norm_eps, rms, rev()));
+    LAUNCH(Lh, F_NORM, dispatch_norm(S, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm1_g[l], (const bf16 *)bb.norm1_b[l], Ni, d.norm_eps, rms, rev()));
     {
       const int tgs[3] = {FMX_TGT_Q, FMX_TGT_K, FMX_TGT_V};
       PairGemmParams p = base;
@@ -1124,40 +1257,40 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       set_lora(p, 0, FMX_TGT_Q, l); set_lora(p, 1, FMX_TGT_K, l); set_lora(p, 2, FMX_TGT_V, l);
       p.omap = oQKV;
       // head_dim 128: a 128-column chunk is one head, so RoPE is applied in the GEMM epilogue (fp32, one rounding)
-      rope_fused = g_rope_fused && d.rope_theta > 0 && d.head_dim == 128 && pair_wide(p);
+      rope_fused = c->o.rope_fused && d.rope_theta > 0 && d.head_dim == 128 && pair_wide(p);
       if (rope_fused) { p.rope_cs = bb.rope_cs_t; p.rope_ld = d.max_seq; p.rope_src_mask = 3; }
       p.reverse = rev();
-      LAUNCH(Lh, F_GEMM_QKV, launch_pair_gemm(c, s, p));
+      LAUNCH(Lh, F_GEMM_QKV, launch_pair_gemm(c, S, p));
     }
     if (d.rope_theta > 0 && !rope_fused) {
       const int nh = d.n_q_heads + d.n_kv_heads;
       const long long total = (long long)Ni * nh * (d.head_dim / 16);
-      LAUNCH(Lh, F_ROPE, (launch_k(rope_kernel, (unsigned)((total + 255) / 256), 256, 0, s, w.QKV, bb.d_qkv, w.t.row_pos, bb.rope_cs, Ni, nh, d.head_dim)));
+      LAUNCH(Lh, F_ROPE, (launch_k(rope_kernel, (unsigned)((total + 255) / 256), 256, 0, S, w.QKV, bb.d_qkv, w.t.row_pos, bb.rope_cs, Ni, nh, d.head_dim)));
     }
-    if (c->opt_attn_impl == FMX_ATTN_AUTO && attn_pair64_ok(d.head_dim, d.n_q_heads, max_len)) {
+    if (c->o.attn_impl == FMX_ATTN_AUTO && attn_pair64_ok(c->o, d.head_dim, d.n_q_heads, max_len)) {
       AttnPairArgs pa2{};
       pa2.qkv_map = mQKV64; pa2.out = w.AttnO; pa2.cu_tok = w.t.cu_tok; pa2.ld_out = bb.d_q; pa2.n_req = B;
       pa2.n_q_heads = d.n_q_heads; pa2.n_kv_heads = d.n_kv_heads; pa2.causal = d.causal; pa2.scale_log2 = scale_log2;
       pa2.reverse = rev();
-      LAUNCH(Lh, F_ATTN, launch_attention_pair64(s, c->sm_count, pa2));
-    } else if (attn_use_lanes(c->opt_attn_impl, d.head_dim, max_len)) {
+      LAUNCH(Lh, F_ATTN, launch_attention_pair64(S, c->sm_count, pa2));
+    } else if (attn_use_lanes(c->o.attn_impl, d.head_dim, max_len)) {
       AttnLaneArgs la{};
       la.qkv_map = mQKV64; la.out = w.AttnO; la.cu_tok = w.t.cu_tok; la.ld_out = bb.d_q; la.n_req = B;
       la.n_q_heads = d.n_q_heads; la.n_kv_heads = d.n_kv_heads; la.causal = d.causal; la.scale_log2 = scale_log2;
-      LAUNCH(Lh, F_ATTN, launch_attention_lanes(s, c->sm_count, d.head_dim, c->opt_attn_variant, max_len, la));
-    } else if (attn_use_tc(c->opt_attn_impl, d.head_dim, max_len)) {
+      LAUNCH(Lh, F_ATTN, launch_attention_lanes(S, c->sm_count, d.head_dim, c->o.attn_variant, max_len, la));
+    } else if (attn_use_tc(c->o.attn_impl, d.head_dim, max_len)) {
       AttnTcArgs ta{};
       ta.qkv_map = mQKV64; ta.out = w.AttnO; ta.cu_tok = w.t.cu_tok; ta.ld_out = bb.d_q;
       ta.n_q_heads = d.n_q_heads; ta.n_kv_heads = d.n_kv_heads; ta.causal = d.causal; ta.scale_log2 = scale_log2;
       ta.reverse = rev();
-      LAUNCH(Lh, F_ATTN, launch_attention_tc(s, d.head_dim, c->opt_attn_variant, max_len, d.n_q_heads, B, ta));
+      LAUNCH(Lh, F_ATTN, launch_attention_tc(S, d.head_dim, c->o.attn_variant, max_len, d.n_q_heads, B, ta));
     } else {
       AttnArgs aa{};
       aa.qkv = w.QKV; aa.out = w.AttnO; aa.cu_tok = w.t.cu_tok; aa.ld_qkv = bb.d_qkv; aa.ld_out = bb.d_q;
       aa.n_q_heads = d.n_q_heads; aa.n_kv_heads = d.n_kv_heads; aa.causal = d.causal; aa.scale_log2 = scale_log2;
       dim3 grid((max_len + kAttnBQ - 1) / kAttnBQ, d.n_q_heads, B);
-      if (max_len <= 64 && g_attn_short) LAUNCH(Lh, F_ATTN, launch_attention_short(s, c->sm_count, d.head_dim, B, aa));
-      else LAUNCH(Lh, F_ATTN, launch_attention(s, d.head_dim, grid, aa));
+      if (max_len <= 64 && c->o.attn_short) LAUNCH(Lh, F_ATTN, launch_attention_short(S, c->sm_count, d.head_dim, B, aa));
+      else LAUNCH(Lh, F_ATTN, launch_attention(S, d.head_dim, grid, aa));
     }
     {
       const int tgs[1] = {FMX_TGT_O};
@@ -1169,9 +1302,9 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       set_lora(p, 0, FMX_TGT_O, l);
       p.omap = oX;
       p.reverse = rev();
-      LAUNCH(Lh, F_GEMM_O, launch_pair_gemm(c, s, p));
+      LAUNCH(Lh, F_GEMM_O, launch_pair_gemm(c, S, p));
     }
-    LAUNCH(Lh, F_NORM, dispatch_norm(s, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm2_g[l], (const bf16 *)bb.norm2_b[l], Ni, d.norm_eps, rms, rev()));
+    LAUNCH(Lh, F_NORM, dispatch_norm(S, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm2_g[l], (const bf16 *)bb.norm2_b[l], Ni, d.norm_eps, rms, rev()));
     if (d.act == FMX_ACT_SWIGLU) {
       const int tgs[2] = {FMX_TGT_GATE, FMX_TGT_UP};
       PairGemmParams p = base;
@@ -1183,7 +1316,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       set_lora(p, 0, FMX_TGT_GATE, l); set_lora(p, 1, FMX_TGT_UP, l);
       p.omap = oHid;
       p.reverse = rev();
-      LAUNCH(Lh, F_GEMM_FFN_IN, launch_pair_gemm(c, s, p));
+      LAUNCH(Lh, F_GEMM_FFN_IN, launch_pair_gemm(c, S, p));
     } else {
       const int tgs[1] = {FMX_TGT_UP};
       PairGemmParams p = base;
@@ -1194,7 +1327,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       set_lora(p, 0, FMX_TGT_UP, l);
       p.omap = oHid;
       p.reverse = rev();
-      LAUNCH(Lh, F_GEMM_FFN_IN, launch_pair_gemm(c, s, p));
+      LAUNCH(Lh, F_GEMM_FFN_IN, launch_pair_gemm(c, S, p));
     }
     {
       const int tgs[1] = {FMX_TGT_DOWN};
@@ -1206,14 +1339,14 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       set_lora(p, 0, FMX_TGT_DOWN, l);
       p.omap = oX;
       p.reverse = rev();
-      LAUNCH(Lh, F_GEMM_FFN_OUT, launch_pair_gemm(c, s, p));
+      LAUNCH(Lh, F_GEMM_FFN_OUT, launch_pair_gemm(c, S, p));
     }
   }
   // ---- S4-S6 ----
   PoolArgs pa{};
   pa.X = w.X; pa.g = (const bf16 *)d.final_g; pa.b = (const bf16 *)d.final_b; pa.cu_tok = w.t.cu_tok; pa.task_sorted = w.t.task_sorted;
   pa.task_head_kind = c->d_task_head_kind; pa.feat = w.feat; pa.Fn = w.Xn; pa.d = d.d_model; pa.eps = d.norm_eps; pa.rms = rms;
-  LAUNCH(Lh, F_POOL, dispatch_pool(s, d.d_model, B, pa));
+  LAUNCH(Lh, F_POOL, dispatch_pool(S, d.d_model, B, pa));
   HeadArgs ha{};
   ha.feat = w.feat; ha.Fn = w.Xn; ha.cu_tok = w.t.cu_tok; ha.task_sorted = w.t.task_sorted; ha.perm = w.t.perm; ha.out_off = w.t.out_off;
   ha.task_head_kind = c->d_task_head_kind; ha.task_head_out = c->d_task_head_out;
@@ -1226,58 +1359,35 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     const TaskRec &tr = c->tasks[task_ids[i]];
     if (tr.head_hidden > 0) { max_hidden = std::max(max_hidden, tr.head_hidden); max_out2 = std::max(max_out2, tr.head_out); }
   }
-  if (max_hidden > 0) {
-    const size_t need = sizeof(float) * (size_t)B * max_hidden;
-    if (need > c->head_hid_bytes) {
-      if (graph_capture) return fmx_fail(FMX_E_CUDA, "forward_mixed: MLP-head scratch grew during graph capture");
-      CU_OK(cudaStreamSynchronize(s));
-      cudaFree(c->d_head_hid);
-      c->d_head_hid = nullptr; c->head_hid_bytes = 0;
-      CU_OK(cudaMalloc(&c->d_head_hid, align_up(need, 1 << 16)));
-      c->head_hid_bytes = align_up(need, 1 << 16);
-      ++c->config_gen;
-    }
-    ha.hid = c->d_head_hid; ha.ld_hid = max_hidden;
-  }
+  if (max_hidden > 0) { ha.hid = w.head_hid; ha.ld_hid = max_hidden; }      // max_hidden <= kMaxHeadHidden by registration
   bool any_flat = false, any_pooled = false;
   int max_out_flat = 0;
   for (int i = 0; i < B; ++i) {
     if (c->tasks[task_ids[i]].head_kind == FMX_HEAD_FLATTEN) { any_flat = true; max_out_flat = std::max(max_out_flat, c->tasks[task_ids[i]].head_out); }
     else any_pooled = true;
   }
-  ha.skip_flatten = (any_flat && g_head_tiled) ? 1 : 0;
-  if (any_pooled || !ha.skip_flatten) LAUNCH(Lh, F_HEAD, (launch_k(head_kernel, dim3(B, (max_out + 7) / 8), 256, 0, s, ha)));
+  ha.skip_flatten = (any_flat && c->o.head_tiled) ? 1 : 0;
+  if (any_pooled || !ha.skip_flatten) LAUNCH(Lh, F_HEAD, (launch_k(head_kernel, dim3(B, (max_out + 7) / 8), 256, 0, S, ha)));
   if (ha.skip_flatten) {
     // tensor-core path: K (= tokens x d_model, the same for every FLATTEN task of a fixed-length backbone) must split into
-    // n_kc chunks x 8 warps x multiples of 32 features; the chunk-partial scratch is library-owned and grow-only
+    // n_kc chunks x 8 warps x multiples of 32 features; the chunk partials live in the caller's workspace
     const long long Kf = (long long)d.tokens_per_request * d.d_model;
     const int groups = (B + 15) / 16, ogs = (max_out_flat + 31) / 32;
     int n_kc = 0;
-    if (g_head_tiled == 2 && d.tokens_per_request > 0)
+    if (c->o.head_tiled == 2 && d.tokens_per_request > 0)
       for (int k = 1; k <= 8; k *= 2)
         if (Kf % (256ll * k) == 0) { n_kc = k; if ((long long)groups * ogs * k >= c->sm_count) break; }
-    const size_t need = (size_t)groups * ogs * std::max(n_kc, 1) * 512 * sizeof(float);
-    if (n_kc > 0 && need > c->head_part_bytes) {
-      if (graph_capture) n_kc = 0;            // cannot allocate while capturing: this call takes the CUDA-core kernel
-      else {
-        CU_OK(cudaStreamSynchronize(s));
-        cudaFree(c->d_head_part);
-        c->d_head_part = nullptr; c->head_part_bytes = 0;
-        CU_OK(cudaMalloc(&c->d_head_part, align_up(need, 1 << 20)));
-        c->head_part_bytes = align_up(need, 1 << 20);
-        ++c->config_gen;                      // a cached forward graph still points at the old scratch buffer
-      }
-    }
+    while (n_kc > 0 && (size_t)groups * ogs * n_kc * 512 > w.head_part_floats) n_kc /= 2;     // fit the workspace's partial budget
     if (n_kc > 0) {
-      LAUNCH(Lh, F_HEAD, (launch_k(head_flatten_mma_kernel, dim3(groups, ogs, n_kc), 256, 0, s, ha, B, n_kc, c->d_head_part)));
-      LAUNCH(Lh, F_HEAD, (launch_k(head_flatten_reduce_kernel, dim3(groups, ogs), 512, 0, s, ha, B, n_kc, (const float *)c->d_head_part)));
+      LAUNCH(Lh, F_HEAD, (launch_k(head_flatten_mma_kernel, dim3(groups, ogs, n_kc), 256, 0, S, ha, B, n_kc, w.head_part)));
+      LAUNCH(Lh, F_HEAD, (launch_k(head_flatten_reduce_kernel, dim3(groups, ogs), 512, 0, S, ha, B, n_kc, (const float *)w.head_part)));
     } else {
-      LAUNCH(Lh, F_HEAD, (launch_k(head_flatten_kernel, dim3((B + 3) / 4, (max_out + 3) / 4), 256, 0, s, ha, B)));
+      LAUNCH(Lh, F_HEAD, (launch_k(head_flatten_kernel, dim3((B + 3) / 4, (max_out + 3) / 4), 256, 0, S, ha, B)));
     }
   }
 
   if (max_hidden > 0)                                    // second layer of the MLP heads (the first wrote relu(W feat + b) to hid)
-    LAUNCH(Lh, F_HEAD, (launch_k(head_mlp2_kernel, dim3(B, (max_out2 + 7) / 8), 256, 0, s, ha)));
+    LAUNCH(Lh, F_HEAD, (launch_k(head_mlp2_kernel, dim3(B, (max_out2 + 7) / 8), 256, 0, S, ha)));
 
   {
     void *bufs[7] = {w.X, w.Xn, w.QKV, w.AttnO, w.Hid, w.U, w.feat};
@@ -1286,7 +1396,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     for (int i = 0; i < 7; ++i) { c->last_buf[i] = bufs[i]; c->last_buf_bytes[i] = sz[i]; }
   }
   c->last_t = w.t; c->last_B = B; c->last_T = T; c->last_n_tiles = w.n_tiles; c->last_stream = s; c->last_launches = Lh.count;
-  return FMX_OK;
+  return graph_capture ? FMX_OK : note_forward(c, s);
 }
 
 // The forward with the context's one-entry CUDA-graph cache in front of it (c->mu held by the caller).  The 2nd identical call
@@ -1294,7 +1404,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
 // kernels loses ~4 % to launch gaps otherwise (cfg2: 11.55 -> 11.09 ms).
 static int forward_cached(fmx_ctx *c, Backbone *bb, fmx_backbone_t h, const void *inputs, const int32_t *task_ids, const int32_t *lengths,
                           int32_t n_req, float *outputs, void *workspace, size_t workspace_bytes, cudaStream_t s) {
-  const bool graphable = c->opt_graph && !c->prof_on && s != nullptr && s != cudaStreamLegacy && s != cudaStreamPerThread;
+  const bool graphable = c->o.graph && !c->prof_on && s != nullptr && s != cudaStreamLegacy && s != cudaStreamPerThread;
   if (graphable) {
     cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
     CU_OK(cudaStreamIsCapturing(s, &st));
@@ -1306,7 +1416,7 @@ static int forward_cached(fmx_ctx *c, Backbone *bb, fmx_backbone_t h, const void
         CU_OK(cudaGraphLaunch(c->graph_exec, s));
         c->last_launches = c->graph_launches; c->last_stream = s;
         ++c->graph_replays;
-        return FMX_OK;
+        return note_forward(c, s);
       }
       if (key == c->last_key) {
         if (c->graph_exec) {                          // the old graph may still be running and owns the graph staging buffer
@@ -1324,7 +1434,7 @@ static int forward_cached(fmx_ctx *c, Backbone *bb, fmx_backbone_t h, const void
             c->graph_key = key;
             c->graph_launches = c->last_launches;
             CU_OK(cudaGraphLaunch(c->graph_exec, s));
-            return FMX_OK;
+            return note_forward(c, s);
           }
           if (graph) cudaGraphDestroy(graph);
           c->graph_exec = nullptr;
@@ -1340,54 +1450,68 @@ static int forward_cached(fmx_ctx *c, Backbone *bb, fmx_backbone_t h, const void
   return forward_impl(c, *bb, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, s);
 }
 
+// A device-side error of an EARLIER forward (the word is mapped host memory the kernels write): reported by the next call.
+static int poll_device_error(fmx_ctx *c) {
+  const unsigned e = *(volatile unsigned *)c->h_err;
+  if (!e) return FMX_OK;
+  *(volatile unsigned *)c->h_err = 0;
+  return fmx_fail(FMX_E_INVALID_ARG, "an earlier forward read token ids outside [0, vocab): those rows were embedded as zeros (device error word 0x%x)", e);
+}
+
+int fmx_poll_error(fmx_ctx *c) {
+  if (!c) return fmx_fail(FMX_E_INVALID_ARG, "poll_error: NULL ctx");
+  std::lock_guard<std::mutex> lk(c->mu);
+  return poll_device_error(c);
+}
+
 int fmx_forward_mixed(fmx_ctx *c, fmx_backbone_t h, const void *inputs, const int32_t *task_ids, const int32_t *lengths,
                       int32_t n_req, float *outputs, void *workspace, size_t workspace_bytes, void *cuda_stream) {
   if (!c) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed: NULL ctx");
   if (n_req < 0) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed: n_req < 0");
+  std::lock_guard<std::mutex> lk(c->mu);
   Backbone *bb = get_bb(c, h);
   if (!bb) return fmx_fail(FMX_E_UNKNOWN_BACKBONE, "forward_mixed: unknown backbone %d", h);
   if (n_req == 0) return FMX_OK;
   if (n_req > FMX_MAX_REQUESTS) return fmx_fail(FMX_E_CAPACITY, "forward_mixed: %d requests > %d", n_req, FMX_MAX_REQUESTS);
   if (!inputs || !task_ids || !lengths || !outputs || !workspace) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed: NULL pointer");
-  std::lock_guard<std::mutex> lk(c->mu);
   CU_OK(cudaSetDevice(c->device));
+  if (int e = poll_device_error(c)) return e;
   return forward_cached(c, bb, h, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, (cudaStream_t)cuda_stream);
 }
 
+// Layout of the host-path workspace: [forward workspace for this batch | input staging | output staging].
 int fmx_forward_mixed_host(fmx_ctx *c, fmx_backbone_t h, const void *inputs_host, size_t inputs_bytes, const int32_t *task_ids,
                            const int32_t *lengths, int32_t n_req, float *outputs_host, void *workspace, size_t workspace_bytes,
                            void *cuda_stream) {
   if (!c) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed_host: NULL ctx");
   if (n_req < 0) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed_host: n_req < 0");
+  std::lock_guard<std::mutex> lk(c->mu);
   Backbone *bb = get_bb(c, h);
   if (!bb) return fmx_fail(FMX_E_UNKNOWN_BACKBONE, "forward_mixed_host: unknown backbone %d", h);
   if (n_req == 0) return FMX_OK;
+  if (n_req > FMX_MAX_REQUESTS) return fmx_fail(FMX_E_CAPACITY, "forward_mixed_host: %d requests > %d", n_req, FMX_MAX_REQUESTS);
   if (!inputs_host || !task_ids || !lengths || !outputs_host || !workspace) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed_host: NULL pointer");
   std::vector<int64_t> off(n_req + 1);
-  if (int e = fmx_output_layout(c, task_ids, n_req, off.data())) return e;
-  std::lock_guard<std::mutex> lk(c->mu);
-  CU_OK(cudaSetDevice(c->device));
-  cudaStream_t s = (cudaStream_t)cuda_stream;
+  if (int e = output_layout_locked(c, task_ids, n_req, off.data())) return e;
+  long long N = 0;
+  for (int i = 0; i < n_req; ++i) N += std::max(lengths[i], 0);
+  if (N < 1 || N > (1ll << 24)) return fmx_fail(FMX_E_BAD_LENGTH, "forward_mixed_host: %lld tokens", N);
+  if (reinterpret_cast<uintptr_t>(workspace) & 1023) return fmx_fail(FMX_E_WORKSPACE, "forward_mixed_host: workspace must be 1024-byte aligned");
+  const size_t fwd_bytes = align_up(carve(*bb, nullptr, n_req, N, c->n_slots).bytes, 1024);
   const size_t out_bytes = (size_t)off[n_req] * sizeof(float);
-  if (inputs_bytes > c->in_stage_bytes) {
-    CU_OK(cudaStreamSynchronize(s));
-    cudaFree(c->d_in_stage);
-    c->d_in_stage = nullptr; c->in_stage_bytes = 0;
-    CU_OK(cudaMalloc(&c->d_in_stage, align_up(inputs_bytes, 1 << 20)));
-    c->in_stage_bytes = align_up(inputs_bytes, 1 << 20);
-  }
-  if (out_bytes > c->out_stage_bytes) {
-    CU_OK(cudaStreamSynchronize(s));
-    cudaFree(c->d_out_stage);
-    c->d_out_stage = nullptr; c->out_stage_bytes = 0;
-    CU_OK(cudaMalloc(&c->d_out_stage, align_up(out_bytes, 1 << 16)));
-    c->out_stage_bytes = align_up(out_bytes, 1 << 16);
-  }
-  CU_OK(cudaMemcpyAsync(c->d_in_stage, inputs_host, inputs_bytes, cudaMemcpyHostToDevice, s));
-  if (int e = forward_cached(c, bb, h, c->d_in_stage, task_ids, lengths, n_req, c->d_out_stage, workspace, workspace_bytes, s)) return e;
-  CU_OK(cudaMemcpyAsync(outputs_host, c->d_out_stage, out_bytes, cudaMemcpyDeviceToHost, s));
+  const size_t need = fwd_bytes + align_up(inputs_bytes, 1024) + align_up(out_bytes, 1024);
+  if (need > workspace_bytes)
+    return fmx_fail(FMX_E_WORKSPACE, "forward_mixed_host: workspace %zu B < required %zu B (fmx_host_workspace_bytes)", workspace_bytes, need);
+  CU_OK(cudaSetDevice(c->device));
+  if (int e = poll_device_error(c)) return e;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  uint8_t *in_stage = static_cast<uint8_t *>(workspace) + fwd_bytes;
+  float *out_stage = reinterpret_cast<float *>(in_stage + align_up(inputs_bytes, 1024));
+  CU_OK(cudaMemcpyAsync(in_stage, inputs_host, inputs_bytes, cudaMemcpyHostToDevice, s));
+  if (int e = forward_cached(c, bb, h, in_stage, task_ids, lengths, n_req, out_stage, workspace, fwd_bytes, s)) return e;
+  CU_OK(cudaMemcpyAsync(outputs_host, out_stage, out_bytes, cudaMemcpyDeviceToHost, s));
   CU_OK(cudaStreamSynchronize(s));
-  return FMX_OK;
+  return poll_device_error(c);
 }
 
 int fmx_debug_get_segments(fmx_ctx *c, int32_t *perm, int32_t *inv_perm, int32_t *task_req_off, int32_t *cu_tok, int32_t *task_tok_off) {
@@ -1479,7 +1603,7 @@ int fmx_debug_gemm(fmx_ctx *c, const void *A, const void *W, float *C, int32_t M
   if ((e = encode_2d(c, &p.wmap_h[0], W, N, K, K, 64))) return e;
   if ((e = encode_2d(c, &p.omap, C, M, N, N, 128, true))) return e;
   for (int i = 0; i < 3; ++i) { p.lora_tgt[i] = -1; p.src_end[i] = 1 << 30; }
-  launch_pair_gemm(c, (cudaStream_t)cuda_stream, p);
+  launch_pair_gemm(c, Strm{(cudaStream_t)cuda_stream, 0}, p);
   CU_OK(cudaGetLastError());
   return FMX_OK;
 }
@@ -1497,40 +1621,34 @@ int fmx_debug_attention(fmx_ctx *c, const void *qkv, void *out, const int32_t *c
     if (cu_tok[i + 1] <= cu_tok[i]) return fmx_fail(FMX_E_BAD_LENGTH, "debug_attention: request %d has no tokens", i);
     max_len = std::max(max_len, cu_tok[i + 1] - cu_tok[i]);
   }
-  if (n_req + 1 > c->dbg_cu_cap) {
-    CU_OK(cudaStreamSynchronize(s));
-    cudaFree(c->d_dbg_cu);
-    c->d_dbg_cu = nullptr; c->dbg_cu_cap = 0;
-    CU_OK(cudaMalloc(&c->d_dbg_cu, sizeof(int) * (n_req + 1)));
-    c->dbg_cu_cap = n_req + 1;
-  }
+  if (n_req > FMX_MAX_REQUESTS) return fmx_fail(FMX_E_CAPACITY, "debug_attention: %d requests > %d", n_req, FMX_MAX_REQUESTS);
   CU_OK(cudaMemcpyAsync(c->d_dbg_cu, cu_tok, sizeof(int) * (n_req + 1), cudaMemcpyHostToDevice, s));
   const int N = cu_tok[n_req], d_q = n_q_heads * head_dim, d_qkv = (n_q_heads + 2 * n_kv_heads) * head_dim;
   const float scale_log2 = 1.4426950408889634f / sqrtf((float)head_dim);
-  if (impl == FMX_ATTN_AUTO && attn_pair64_ok(head_dim, n_q_heads, max_len)) {
+  if (impl == FMX_ATTN_AUTO && attn_pair64_ok(c->o, head_dim, n_q_heads, max_len)) {
     AttnPairArgs pa2{};
     if (int e = encode_2d(c, &pa2.qkv_map, qkv, N, d_qkv, d_qkv, 64)) return e;
     pa2.out = (bf16 *)out; pa2.cu_tok = c->d_dbg_cu; pa2.ld_out = d_q; pa2.n_req = n_req; pa2.n_q_heads = n_q_heads; pa2.n_kv_heads = n_kv_heads;
     pa2.causal = causal; pa2.scale_log2 = scale_log2;
-    launch_attention_pair64(s, c->sm_count, pa2);
+    launch_attention_pair64(Strm{s, 0}, c->sm_count, pa2);
   } else if (attn_use_lanes(impl, head_dim, max_len)) {
     AttnLaneArgs la{};
     if (int e = encode_2d(c, &la.qkv_map, qkv, N, d_qkv, d_qkv, 64)) return e;
     la.out = (bf16 *)out; la.cu_tok = c->d_dbg_cu; la.ld_out = d_q; la.n_req = n_req; la.n_q_heads = n_q_heads; la.n_kv_heads = n_kv_heads;
     la.causal = causal; la.scale_log2 = scale_log2;
-    launch_attention_lanes(s, c->sm_count, head_dim, c->opt_attn_variant, max_len, la);
+    launch_attention_lanes(Strm{s, 0}, c->sm_count, head_dim, c->o.attn_variant, max_len, la);
   } else if (attn_use_tc(impl, head_dim, max_len)) {
     AttnTcArgs ta{};
     if (int e = encode_2d(c, &ta.qkv_map, qkv, N, d_qkv, d_qkv, 64)) return e;
     ta.out = (bf16 *)out; ta.cu_tok = c->d_dbg_cu; ta.ld_out = d_q; ta.n_q_heads = n_q_heads; ta.n_kv_heads = n_kv_heads;
     ta.causal = causal; ta.scale_log2 = scale_log2;
-    launch_attention_tc(s, head_dim, c->opt_attn_variant, max_len, n_q_heads, n_req, ta);
+    launch_attention_tc(Strm{s, 0}, head_dim, c->o.attn_variant, max_len, n_q_heads, n_req, ta);
   } else {
     AttnArgs aa{};
     aa.qkv = (const bf16 *)qkv; aa.out = (bf16 *)out; aa.cu_tok = c->d_dbg_cu; aa.ld_qkv = d_qkv; aa.ld_out = d_q;
     aa.n_q_heads = n_q_heads; aa.n_kv_heads = n_kv_heads; aa.causal = causal; aa.scale_log2 = scale_log2;
-    if (max_len <= 64 && g_attn_short) launch_attention_short(s, c->sm_count, head_dim, n_req, aa);
-    else launch_attention(s, head_dim, dim3((max_len + kAttnBQ - 1) / kAttnBQ, n_q_heads, n_req), aa);
+    if (max_len <= 64 && c->o.attn_short) launch_attention_short(Strm{s, 0}, c->sm_count, head_dim, n_req, aa);
+    else launch_attention(Strm{s, 0}, head_dim, dim3((max_len + kAttnBQ - 1) / kAttnBQ, n_q_heads, n_req), aa);
   }
   CU_OK(cudaGetLastError());
   CU_OK(cudaStreamSynchronize(s));      // cu_tok is a host array of the caller
@@ -1544,49 +1662,49 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
   switch (option) {
     case FMX_OPT_ATTENTION_IMPL:
       if (value < FMX_ATTN_AUTO || value > FMX_ATTN_LANES) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attention impl %d", value);
-      c->opt_attn_impl = value;
+      c->o.attn_impl = value;
       return FMX_OK;
     case FMX_OPT_SHRINK_STAGES:
       if (value != 4 && value != 5) return fmx_fail(FMX_E_INVALID_ARG, "set_option: shrink stages %d", value);   // 5 = as deep as the stage size allows
-      g_shrink_stages = value;
+      c->o.shrink_stages = value;
       return FMX_OK;
     case FMX_OPT_ATTN_SHORT:
       if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attn_short %d", value);
-      g_attn_short = value;
+      c->o.attn_short = value;
       return FMX_OK;
     case FMX_OPT_DEEP_PIPE:
-      g_deep_pipe = value ? 1 : 0;
+      c->o.deep_pipe = value ? 1 : 0;
       return FMX_OK;
     case FMX_OPT_EXPAND_WIDE:
-      g_expand_wide = value ? 1 : 0;
+      c->o.expand_wide = value ? 1 : 0;
       return FMX_OK;
     case FMX_OPT_REVERSE:
-      g_reverse = value ? 1 : 0;
+      c->o.reverse = value ? 1 : 0;
       return FMX_OK;
     case FMX_OPT_GRAPH:
-      c->opt_graph = value ? 1 : 0;
+      c->o.graph = value ? 1 : 0;
       return FMX_OK;
     case FMX_OPT_SHRINK_FUSED:
       if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: shrink_fused %d", value);
-      g_shrink_fused = value;
+      c->o.shrink_fused = value;
       return FMX_OK;
     case FMX_OPT_HEAD_TILED:
       if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: head_tiled %d", value);
-      g_head_tiled = value;
+      c->o.head_tiled = value;
       return FMX_OK;
     case FMX_OPT_ROPE_FUSED:
-      g_rope_fused = value ? 1 : 0;
+      c->o.rope_fused = value ? 1 : 0;
       return FMX_OK;
     case FMX_OPT_HALF_TILES:
-      g_half_tiles = value ? 1 : 0;
+      c->o.half_tiles = value ? 1 : 0;
       return FMX_OK;
     case FMX_OPT_PDL:
       if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: pdl %d", value);
-      g_pdl = value;
+      c->o.pdl = value;
       return FMX_OK;
     case FMX_OPT_ATTENTION_VARIANT:
       if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attention variant %d", value);
-      c->opt_attn_variant = value;
+      c->o.attn_variant = value;
       return FMX_OK;
   }
   return fmx_fail(FMX_E_INVALID_ARG, "set_option: unknown option %d", option);

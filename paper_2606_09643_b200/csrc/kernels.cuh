@@ -201,6 +201,8 @@ struct EmbedArgs {
   float *X;                        // fp32 residual [N, d], task-sorted rows
   const __nv_bfloat16 *table;      // TOKEN_IDS
   const __nv_bfloat16 *pos;        // optional positional table [max_seq, d] (EMBEDDED/TOKEN_IDS)
+  int vocab;                       // TOKEN_IDS: rows of the table
+  unsigned *err;                   // device error word (bit 0: a token id outside [0, vocab))
 };
 
 // EMBEDDED: X[r] = x_i[pos] (+ Pos[pos]);   one warp per row, 8 bf16 per lane per step
@@ -212,7 +214,15 @@ __global__ void embed_rows_kernel(const EmbedArgs a, int token_ids) {
   const int r = warp, pos = a.row_pos[r], i = a.perm[a.row_req[r]];
   const __nv_bfloat16 *src;
   if (token_ids) {
+    // The ids are device data the host cannot validate: an id outside the table becomes a zero row (never an out-of-bounds
+    // read) and raises the context's device error word, which the next forward call reports.
     const int id = reinterpret_cast<const int *>(a.inputs)[a.in_off[i] + pos];
+    if (id < 0 || id >= a.vocab) {
+      if (lane == 0) *a.err = 1u;
+      float *dst0 = a.X + (size_t)r * a.d;
+      for (int c = lane * 4; c < a.d; c += 128) *reinterpret_cast<float4 *>(dst0 + c) = make_float4(0.f, 0.f, 0.f, 0.f);
+      return;
+    }
     src = a.table + (size_t)id * a.d;
   } else {
     src = reinterpret_cast<const __nv_bfloat16 *>(a.inputs) + a.in_off[i] + (size_t)pos * a.d;

@@ -18,21 +18,34 @@ def _dev_bf16(bits, device):
 
 
 class Session:
-    def __init__(self, wl: Workload, device=0, fmx: Fmx = None, max_req=None, max_tokens=None):
+    def __init__(self, wl: Workload, device=0, fmx: Fmx = None, max_req=None, max_tokens=None, weights_from=None):
+        """weights_from: another Session on a backbone of the SAME shape whose device-resident backbone tensors are reused
+        instead of generating and uploading this workload's own (timing runs that only change the task set: same shapes,
+        same value distribution; never used by a parity test)."""
         self.wl = wl
         self.dev = torch.device("cuda", device)
         torch.cuda.set_device(self.dev)
         self.fmx = fmx or Fmx(device)
-        self._weights = {}
+        self._weights = dict(weights_from._weights) if weights_from is not None else {}
         self.bb = self._register_backbone()
         self.task_ids_of = [self._register_task(t) for t in range(len(wl.tasks))]
-        B = max_req or wl.n_req
-        N = max_tokens or max(wl.n_tokens, 1)
-        self.ws_bytes = self.fmx.workspace_bytes(self.bb, B, N)
-        self.workspace = torch.empty(self.ws_bytes + 1024, dtype=torch.uint8, device=self.dev)
-        self.ws_ptr = (self.workspace.data_ptr() + 1023) // 1024 * 1024
+        self.max_req = max_req or wl.n_req
+        self.max_tokens = max_tokens or max(wl.n_tokens, 1)
+        self._alloc_workspace(self.fmx.workspace_bytes(self.bb, self.max_req, self.max_tokens))
         self.inputs_dev = None
         self.out_dev = None
+
+    def _alloc_workspace(self, nbytes):
+        self.ws_bytes = nbytes
+        self.workspace = torch.empty(nbytes + 1024, dtype=torch.uint8, device=self.dev)
+        self.ws_ptr = (self.workspace.data_ptr() + 1023) // 1024 * 1024
+
+    def ensure_host_workspace(self, input_bytes, output_floats):
+        """fmx_forward_mixed_host stages the packed inputs and the outputs in the workspace too."""
+        need = self.fmx.host_workspace_bytes(self.bb, self.max_req, self.max_tokens, input_bytes, output_floats)
+        if need > self.ws_bytes:
+            torch.cuda.synchronize(self.dev)
+            self._alloc_workspace(need)
 
     # ------------------------------------------------------------------ registration
     def _w(self, name):
@@ -144,6 +157,24 @@ class Session:
         reg_ms = self.last_register_ms
         s.synchronize()
         return reg_ms, e0.elapsed_time(e1), tid
+
+    def unregister_while_serving_ms(self, t, n_forwards=5, stream=None):
+        """NEXT-2: remove a fresh copy of workload task t (so the batch stays servable) while `n_forwards` forwards are queued; returns (unregister_ms, forwards_ms).  fmx_unregister_task does not
+        synchronise the device: the copy's buffers are released on the device after the queued forwards."""
+        s = stream if stream is not None else torch.cuda.current_stream(self.dev)
+        tid = self._register_task_presynced(t)
+        self.forward(stream=s)
+        s.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(s)
+        for _ in range(n_forwards):
+            self.forward(stream=s)
+        e1.record(s)
+        t0 = time.perf_counter()
+        self.fmx.unregister_task(tid)
+        un_ms = (time.perf_counter() - t0) * 1e3
+        s.synchronize()
+        return un_ms, e0.elapsed_time(e1)
 
     # ------------------------------------------------------------------ running
     def upload_inputs(self, packed=None):

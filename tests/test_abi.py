@@ -9,11 +9,12 @@ import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HEADER = os.path.join(ROOT, "include", "fmx.h")
+INTERNAL_HEADER = os.path.join(ROOT, "paper_2606_09643_b200", "csrc", "fmx_internal.h")
 
 
-def declared_functions():
-    """Names of the functions include/fmx.h declares (`<type> fmx_xxx(` at the start of a declaration)."""
-    text = open(HEADER).read()
+def declared_functions(header=HEADER):
+    """Names of the functions a header declares (`<type> fmx_xxx(` at the start of a declaration)."""
+    text = open(header).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)            # comments mention names too
     names = re.findall(r"^[A-Za-z_][A-Za-z_0-9 \*]*?\b(fmx_[a-z0-9_]+)\s*\(", text, flags=re.M)
     return sorted(set(names))
@@ -31,17 +32,21 @@ def test_header_declares_the_north_star_calls():
     for must in ("fmx_register_backbone", "fmx_register_task", "fmx_unregister_task", "fmx_forward_mixed", "fmx_output_layout",
                  "fmx_workspace_bytes", "fmx_bfq_create", "fmx_bfq_enqueue", "fmx_bfq_next_batch", "fmx_bfq_complete"):
         assert must in names
-    assert len(names) >= 30
+    assert len(names) >= 26
+    # test hooks and tuning knobs are NOT part of the public ABI
+    assert not any(n.startswith("fmx_debug_") and n != "fmx_debug_get_segments" for n in names) and "fmx_set_option" not in names
+    assert "FMX_OPT_" not in open(HEADER).read()
 
 
 def test_library_exports_every_declared_symbol(lib):
-    missing = [n for n in declared_functions() if not hasattr(lib, n)]
-    assert not missing, f"libfmx.so lacks symbols declared in include/fmx.h: {missing}"
+    missing = [n for n in declared_functions() + declared_functions(INTERNAL_HEADER) if not hasattr(lib, n)]
+    assert not missing, f"libfmx.so lacks symbols declared in include/fmx.h / csrc/fmx_internal.h: {missing}"
 
 
 def test_binding_names_match_the_header():
-    from paper_2606_09643_b200.binding import EXPORTS
+    from paper_2606_09643_b200.binding import EXPORTS, INTERNAL_EXPORTS
     assert sorted(EXPORTS) == declared_functions()
+    assert sorted(INTERNAL_EXPORTS) == declared_functions(INTERNAL_HEADER)
 
 
 def test_no_device_means_an_error_not_a_fallback(lib):

@@ -155,37 +155,139 @@ def test_every_kernel_option_gives_the_oracle_result(fmx_mod, cfg, kw):
 
 
 # ---------------------------------------------------------------- full sizes, sampled outputs
-@pytest.mark.parametrize("cfg,kw,n_sample", [
-    ("cfg2", {}, 6),
-    ("cfg3", {}, 3),
-    ("cfg5", dict(n_tasks=92, dist="zipf0.8"), 4),
-    ("cfg5", dict(n_tasks=1), 2),
+def stratified_sample(wl, seg, n_random=2, seed=1):
+    """Requests the oracle recomputes at full size (requests are independent by definition, so any subset is a valid check).
+    Not a random draw alone: the sample always holds the requests at sorted positions 0 and B-1 (first / last row tile), a
+    request whose rows straddle a 256-row tile boundary (if one exists), the shortest and the longest request, one request
+    per distinct LoRA rank and per head kind present in the batch, plus n_random seeded ones."""
+    B = wl.n_req
+    perm, cu = seg["perm"], seg["cu_tok"]
+    pick = {int(perm[0]), int(perm[B - 1])}
+    for p in range(B):
+        if cu[p] // 256 != (cu[p + 1] - 1) // 256 and cu[p] % 256 != 0:
+            pick.add(int(perm[p]))
+            break
+    order = np.argsort(wl.lengths, kind="stable")
+    pick.update((int(order[0]), int(order[-1])))
+    seen = set()
+    for i in range(B):
+        ts = wl.tasks[int(wl.task_ids[i])]
+        rank = max((a.rank for a in ts.adapters), default=0)
+        for key in (("rank", rank), ("head", ts.head_kind, bool(getattr(ts, "head_hidden", 0)))):
+            if key not in seen:
+                seen.add(key)
+                pick.add(i)
+    rng = np.random.default_rng(seed)
+    pick.update(int(i) for i in rng.choice(B, size=min(n_random, B), replace=False))
+    return sorted(pick)
+
+
+@pytest.mark.parametrize("cfg,kw", [
+    ("cfg2", {}),
+    ("cfg3", {}),
+    ("cfg5", dict(n_tasks=92, dist="zipf0.8")),
+    ("cfg5", dict(n_tasks=92, dist="zipf1.5")),
+    ("cfg5", dict(n_tasks=1)),
 ])
-def test_full_size_sampled_parity(fmx_mod, cfg, kw, n_sample):
-    """BASELINE.json's full sizes in the launch configuration bench.py times; the oracle computes
-    a seeded sample of requests one by one (requests are independent by definition)."""
+def test_full_size_sampled_parity(fmx_mod, cfg, kw):
+    """BASELINE.json's full sizes in the launch configuration bench.py times; the oracle recomputes a stratified sample of
+    requests one by one (see stratified_sample)."""
     wl = make_workload(cfg, **kw)
     s = _session(fmx_mod, wl)
     y = s.forward_numpy()
-    check_segments(s, wl)
-    rng = np.random.default_rng(1)
-    idx = sorted(rng.choice(wl.n_req, size=n_sample, replace=False).tolist())
+    seg = check_segments(s, wl)
+    idx = stratified_sample(wl, seg)
+    ranks = {max((a.rank for a in wl.tasks[int(wl.task_ids[i])].adapters), default=0) for i in idx}
+    assert ranks == {max((a.rank for a in wl.tasks[int(t)].adapters), default=0) for t in set(wl.task_ids.tolist())}
+    assert int(seg["perm"][0]) in idx and int(seg["perm"][-1]) in idx
     ref = G.oracle_outputs(wl, idx)
     check_parity([y[i] for i in idx], ref, f"{cfg} full {kw}")
     assert all(np.isfinite(v).all() for v in y)
 
 
 def test_cfg4_full_size_sampled_parity(fmx_mod):
-    """cfg4 at full depth/width with all 92 tasks registered; batch of 64 variable-length prompts;
-    the oracle checks the two shortest requests and one mid-length one."""
+    """cfg4 at full depth / width with all 92 tasks registered; batch of 64 variable-length prompts.  The oracle recomputes
+    the stratified sample: first / last sorted request, a tile-straddling one, the SHORTEST and the LONGEST prompt, one request
+    per LoRA rank {4, 8, 16, 32, 64} and per head kind (classification, scalar regression)."""
     wl = make_workload("cfg4")
     s = _session(fmx_mod, wl)
     y = s.forward_numpy()
-    check_segments(s, wl)
-    order = np.argsort(wl.lengths)
-    idx = sorted([int(order[0]), int(order[1]), int(order[len(order) // 3])])
+    seg = check_segments(s, wl)
+    idx = stratified_sample(wl, seg, n_random=0)
+    assert wl.lengths[idx].max() == wl.lengths.max() and wl.lengths[idx].min() == wl.lengths.min()
     ref = G.oracle_outputs(wl, idx)
     check_parity([y[i] for i in idx], ref, "cfg4 full")
+    assert all(np.isfinite(v).all() for v in y)
+
+
+# ---------------------------------------------------------------- intermediate tensors (SURVEY.md section 4, tier 3)
+@pytest.mark.parametrize("cfg,kw", [
+    ("cfg4", dict(n_layers=2, batch=8, max_len=300)),      # RoPE'd q / k, GQA, SwiGLU hidden, `down` shrink output U
+    ("cfg3", dict(n_layers=2, batch=5)),                   # LN + biases, GeLU hidden, odd sequence length 257 (no `down` adapter: U unchecked)
+])
+def test_intermediate_tensors_match_the_oracle(fmx_mod, cfg, kw):
+    """The activation buffers the LAST layer leaves in the workspace (fmx_debug_read) against the oracle's capture of the same
+    layer, row by row in task-sorted order: norm-2 output, q | k | v (after RoPE), attention output, FFN hidden, the final
+    residual stream, and - where the last shrink of the layer is the `down` one - the LoRA shrink output U = s (hid A^T).
+    Bars: per-row cosine >= 0.999 and max-abs <= 2 % of the tensor's range (bf16 storage of every buffer but the residual)."""
+    from oracle.vfm_forward import layer_forward, tokens_from_input
+    wl = make_workload(cfg, **kw)
+    s = _session(fmx_mod, wl)
+    s.fmx.set_option("shrink_fused", 0)        # U then holds exactly the last separate shrink launch of the layer
+    s.forward_numpy()
+    seg = check_segments(s, wl)
+    bbw = wl.bb
+    N, d = wl.n_tokens, bbw.d_model
+    d_q, d_kv = bbw.n_q_heads * bbw.head_dim, bbw.n_kv_heads * bbw.head_dim
+    got = dict(X=s.fmx.debug_read(0, (N, d), np.float32).astype(np.float64),
+               norm2=bf16_bits_to_f64(s.fmx.debug_read(1, (N, d), np.uint16)),
+               qkv=bf16_bits_to_f64(s.fmx.debug_read(2, (N, d_q + 2 * d_kv), np.uint16)),
+               attn=bf16_bits_to_f64(s.fmx.debug_read(3, (N, d_q), np.uint16)),
+               hid=bf16_bits_to_f64(s.fmx.debug_read(4, (N, bbw.d_ffn), np.uint16)))
+    bb, get, tasks = G.bb_dict(wl), G.make_get(wl), G.task_dicts(wl)
+    L = bbw.n_layers
+    ref = {k: np.zeros_like(v) for k, v in got.items()}
+    hid_rows = np.zeros((N, bbw.d_ffn))
+    for p in range(wl.n_req):
+        i = int(seg["perm"][p])
+        task = tasks[int(wl.task_ids[i])]
+        h = tokens_from_input(bb, get, G.request_inputs(wl, [i])[0], task)
+        cap = {}
+        for l in range(L):
+            h = layer_forward(bb, get, task, l, h, capture=cap if l == L - 1 else None)
+        r0, r1 = int(seg["cu_tok"][p]), int(seg["cu_tok"][p + 1])
+        ref["X"][r0:r1] = h
+        ref["norm2"][r0:r1] = cap["norm2"]
+        ref["qkv"][r0:r1] = np.concatenate([cap["q"], cap["k"], cap["v"]], axis=1)
+        ref["attn"][r0:r1] = cap["attn"]
+        ref["hid"][r0:r1] = cap["hid"]
+        hid_rows[r0:r1] = cap["hid"]
+
+    def close(name, a, b):
+        rng_ = float(np.abs(b).max())
+        err = float(np.abs(a - b).max())
+        assert err <= 0.02 * rng_, f"{name}: max-abs {err:.3e} > 2 % of range {rng_:.3e}"
+        num = (a * b).sum(axis=1)
+        den = np.linalg.norm(a, axis=1) * np.linalg.norm(b, axis=1) + 1e-300
+        assert float((num / den).min()) >= 0.999, f"{name}: row cosine {float((num / den).min()):.6f}"
+
+    for k in ("norm2", "qkv", "attn", "hid", "X"):
+        close(k, got[k], ref[k])
+    # U of the `down` shrink (the layer's last one when the tasks adapt `down`): block b of the S1 table owns rows
+    # [b * 256 + lo, b * 256 + hi) of U; columns [0, rank) = s_t * (hid_row . A_t^T), rows of other tasks zero
+    if any(a.target == "down" for t in wl.tasks for a in t.adapters):
+        n_tiles, n_blk, blocks = s.fmx.debug_get_tiles()
+        U = bf16_bits_to_f64(s.fmx.debug_read(5, (n_blk * 256, 192), np.uint16))
+        for b, (tile, slot, lo, hi) in enumerate(blocks):
+            wt = s.task_ids_of.index(int(slot))
+            ad = [a for a in wl.tasks[wt].adapters if a.target == "down"]
+            blk = U[b * 256:(b + 1) * 256]
+            assert not blk[:lo].any() and not blk[hi:].any(), "rows outside the block's segment must be zero"
+            if not ad:
+                continue
+            A = get(f"task{wt:03d}.L{L - 1:02d}.down.A")
+            want = ad[0].scaling * (hid_rows[tile * 256 + lo:tile * 256 + hi] @ A.T)
+            close(f"U block {b}", blk[lo:hi, :ad[0].rank], want)
 
 
 # ---------------------------------------------------------------- invariants on the GPU
@@ -310,6 +412,10 @@ def test_host_buffer_forward_matches_device_forward(fmx_mod):
     ids = np.array([s.task_ids_of[int(t)] for t in wl.task_ids], dtype=np.int32)
     off = s.fmx.output_layout(ids)
     host_out = torch.empty(int(off[-1]), dtype=torch.float32).pin_memory()
+    with pytest.raises(fmx_mod.FmxError) as e:                     # the plain forward's workspace has no room for the staging
+        s.fmx.forward_mixed_host(s.bb, host_in.data_ptr(), packed.nbytes, ids, wl.lengths, host_out.data_ptr(), s.ws_ptr, s.ws_bytes // 2)
+    assert e.value.code == -6
+    s.ensure_host_workspace(packed.nbytes, int(off[-1]))
     s.fmx.forward_mixed_host(s.bb, host_in.data_ptr(), packed.nbytes, ids, wl.lengths, host_out.data_ptr(), s.ws_ptr, s.ws_bytes,
                              torch.cuda.current_stream().cuda_stream)
     got = host_out.numpy()
@@ -475,3 +581,146 @@ def test_task_can_be_added_while_forwards_are_in_flight(fmx_mod):
         again = s.forward_numpy()
         for i in ids7:
             assert np.array_equal(again[i], base[i])
+
+
+def test_unregister_does_not_wait_for_forwards_in_flight(fmx_mod):
+    """NEXT-2 (PAPER.md L92 R2, L243-L245): fmx_unregister_task returns without a device-wide synchronise while
+    forwards that still serve the task are queued; those forwards are unaffected (bit-identical), the id is rejected
+    afterwards, and a registration that reuses the freed slot and slab columns right away is correct."""
+    wl = make_workload("cfg2", n_layers=8, batch=128)
+    s = _session(fmx_mod, wl)
+    base = s.forward_numpy()
+    victim = int(wl.task_ids[0])                                  # a task the queued forwards DO use
+    s.prepare_task_copy(victim)
+    st = torch.cuda.Stream()
+    import time
+    with torch.cuda.stream(st):
+        s.forward(stream=st)
+        st.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        for _ in range(12):
+            s.forward(stream=st)
+        e1.record(st)
+        t0 = time.perf_counter()
+        s.fmx.unregister_task(s.task_ids_of[victim])
+        un_ms = (time.perf_counter() - t0) * 1e3
+        busy = not e1.query()                                     # the queued forwards were still running when the call returned
+        new_tid = s._register_task_presynced(victim)              # reuses the slot and the columns: waits on the device only
+        st.synchronize()
+        fwd_ms = e0.elapsed_time(e1)
+        flat = s.out_dev.cpu().numpy()
+    assert busy, "the forwards finished before unregister returned: the test did not exercise the overlap"
+    assert un_ms < 0.5 * fwd_ms, f"unregister took {un_ms:.2f} ms while 12 forwards took {fwd_ms:.2f} ms: it waited for them"
+    got = [flat[s.last_off[i]:s.last_off[i + 1]] for i in range(wl.n_req)]
+    for a, b in zip(got, base):
+        assert np.array_equal(a, b), "a forward queued before the unregister changed"
+    assert new_tid == s.task_ids_of[victim], "the freed slot is reused lowest-first"
+    again = s.forward_numpy()
+    for a, b in zip(again, base):
+        assert np.array_equal(a, b), "the re-registered task must give the same bits"
+    s.fmx.unregister_task(new_tid)
+    with pytest.raises(fmx_mod.FmxError) as e:
+        s.forward()
+    assert e.value.code == -3                                     # FMX_E_UNKNOWN_TASK
+
+
+def test_slab_growth_does_not_wait_for_forwards_in_flight(fmx_mod):
+    """NEXT-2: a registration that overflows the LoRA slab arena (256 columns at first) builds the wider arena on the
+    registration stream while forwards keep reading the old one; the call does not wait for them and they are unaffected."""
+    wl = make_workload("cfg5", n_layers=4, batch=128, n_tasks=4, dist="uniform")
+    s = _session(fmx_mod, wl)
+    base = s.forward_numpy()
+    big = max(range(len(wl.tasks)), key=lambda t: max(a.rank for a in wl.tasks[t].adapters))
+    r_pad = (max(a.rank for a in wl.tasks[big].adapters) + 15) // 16 * 16
+    used = sum((max(a.rank for a in t.adapters) + 15) // 16 * 16 for t in wl.tasks)
+    n_fill = (256 - used) // r_pad                                # copies that still fit the first arena
+    s.prepare_task_copy(big)
+    extra = [s._register_task_presynced(big) for _ in range(n_fill)]
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        s.forward(stream=st)
+        st.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        for _ in range(24):
+            s.forward(stream=st)
+        e1.record(st)
+        grown = s._register_task_presynced(big)                   # does not fit: the arena doubles
+        reg_ms = s.last_register_ms
+        busy = not e1.query()
+        st.synchronize()
+        fwd_ms = e0.elapsed_time(e1)
+        flat = s.out_dev.cpu().numpy()
+    assert busy and reg_ms < 0.5 * fwd_ms, f"growing registration took {reg_ms:.2f} ms, 24 forwards {fwd_ms:.2f} ms (busy={busy})"
+    got = [flat[s.last_off[i]:s.last_off[i + 1]] for i in range(wl.n_req)]
+    for a, b in zip(got, base):
+        assert np.array_equal(a, b)
+    # after the switch: old tasks, the fillers and the task in the new columns all give task `big`'s / their own bits
+    after = s.forward_numpy()
+    for a, b in zip(after, base):
+        assert np.array_equal(a, b)
+    sel = [i for i in range(wl.n_req) if wl.task_ids[i] == big]
+    for tid in (extra[:1] + [grown]):
+        remap = list(s.task_ids_of)
+        remap[big] = tid
+        keep, s.task_ids_of = s.task_ids_of, remap
+        try:
+            y = s.forward_numpy()
+        finally:
+            s.task_ids_of = keep
+        for i in sel:
+            assert np.array_equal(y[i], base[i])
+
+
+def test_two_contexts_keep_their_own_options(fmx_mod):
+    """Tuning state is per context (no file-scope knobs): two contexts on one device with different options, forwards
+    interleaved on two streams, each give exactly what they give alone."""
+    wl = make_workload("cfg2", n_layers=2, batch=40)
+    a, b = _session(fmx_mod, wl), _session(fmx_mod, wl)
+    alone = a.forward_numpy()
+    b.fmx.set_option("shrink_fused", 0)
+    b.fmx.set_option("pdl", 1)
+    b.fmx.set_option("half_tiles", 0)
+    b.fmx.set_option("reverse", 0)
+    alone_b = b.forward_numpy()
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    for _ in range(4):
+        a.forward(stream=sa)
+        b.forward(stream=sb)
+    torch.cuda.synchronize()
+    fa, fb = a.out_dev.cpu().numpy(), b.out_dev.cpu().numpy()
+    for i in range(wl.n_req):
+        assert np.array_equal(fa[a.last_off[i]:a.last_off[i + 1]], alone[i])
+        assert np.array_equal(fb[b.last_off[i]:b.last_off[i + 1]], alone_b[i])
+    check_parity(alone_b, G.oracle_outputs(wl), "second context")
+
+
+def test_token_id_outside_the_vocabulary_is_reported_not_read(fmx_mod):
+    """Token ids live in device memory, so the host cannot validate them: an id outside [0, vocab) must not become an
+    out-of-bounds read.  Its row is embedded as zeros, the device error word is raised and the next call reports it; requests
+    without a bad id are bit-identical to a clean run."""
+    wl = make_workload("cfg4", n_layers=1, batch=5, max_len=130, n_tasks=6)
+    s = _session(fmx_mod, wl)
+    good = s.forward_numpy()
+    toks = wl.packed_inputs().copy()
+    n0 = int(wl.lengths[0])
+    toks[n0 + 3] = wl.bb.vocab + 12345                             # request 1
+    toks[n0 + 4] = -7
+    s.upload_inputs(toks)
+    bad = s.forward_numpy()
+    with pytest.raises(fmx_mod.FmxError) as e:
+        s.fmx.poll_error()
+    assert e.value.code == -1 and "vocab" in str(e.value)
+    s.fmx.poll_error()                                             # reported once, then clear
+    for i in range(wl.n_req):
+        assert np.isfinite(bad[i]).all()
+        if i != 1:
+            assert np.array_equal(bad[i], good[i])
+    s.forward()                                                    # raise it again: the NEXT forward call refuses
+    torch.cuda.synchronize()
+    with pytest.raises(fmx_mod.FmxError):
+        s.forward()
+    s.upload_inputs(wl.packed_inputs())
+    for a, b in zip(s.forward_numpy(), good):
+        assert np.array_equal(a, b)
