@@ -272,6 +272,9 @@ def _measure(args, wl, rank, local_rank, world, full, steps, weights_from, label
     dev = torch.device("cuda", local_rank)
     pk = peaks()
     sess = Session(wl, device=local_rank, weights_from=weights_from)
+    for kv in args.opt:
+        name, val = kv.split("=")
+        sess.fmx.set_option(name, int(val))
     sess.upload_inputs()
     fl = accounting.flops(wl)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if not args.no_flush else None
@@ -359,7 +362,7 @@ def _measure(args, wl, rank, local_rank, world, full, steps, weights_from, label
             "config": {"workload": WORKLOAD_NAMES.get(label, label), "requests": B, "tokens": wl.n_tokens,
                        "tasks": len(wl.tasks), "tasks_in_batch": int(len(set(wl.task_ids.tolist()))), "dist": wl.notes.get("dist"),
                        "l2": "flushed (256 MB memset) between steps, outside the per-step events" if flush is not None else "no flush",
-                       "accumulate": "fp32 (TMEM), fp32 residual stream", "replicas": world,
+                       "accumulate": "fp32 (TMEM), fp32 residual stream", "replicas": world, **({"options": args.opt} if args.opt else {}),
                        **({"mlp_heads_hidden": args.mlp_hidden} if args.mlp_hidden else {}), **({"input_encoder_channels": args.enc_channels} if args.enc_channels else {}),
                        "launch": f"CUDA graph replay inside fmx_forward_mixed on {graph_steps} of {steps} timed steps" if graph_steps else "plain kernel launches"},
             "no_graph": {"value": round(replicas.whole_job_throughput(B, steps, ms_plain_max, world), 2), "ms_per_step": round(ms_plain_max / steps, 4),
@@ -510,6 +513,8 @@ def main():
     ap.add_argument("--no-adapters", action="store_true", help="cfg5: head-only tasks (adapter-free reference)")
     ap.add_argument("--enc-channels", type=int, default=0, help="NEXT-1 variant: every other task brings this many input channels and a channel combiner (cfg2 / cfg5)")
     ap.add_argument("--mlp-hidden", type=int, default=0, help="NEXT-1 variant: pooled heads become MLP decoder heads of this hidden width")
+    ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
+                    help="fmx_set_option experiment knob (csrc/fmx_internal.h), e.g. --opt attention_impl=3; recorded in config.options")
     ap.add_argument("--no-flush", action="store_true")
     ap.add_argument("--no-graph", action="store_true", help="plain kernel launches in the timed region (FMX_OPT_GRAPH off)")
     ap.add_argument("--no-kernel-events", action="store_true", help="no per-GEMM events inside the timed region (no roofline)")

@@ -17,6 +17,7 @@
 #include "attention_lanes.cuh"
 #include "attention_pair64.cuh"
 #include "attention_tc.cuh"
+#include "attention_fa.cuh"
 #include "common.h"
 #include "fmx.h"
 #include "fmx_internal.h"
@@ -94,7 +95,8 @@ struct Opts {
   int expand_wide = 1;
   int rope_fused = 1;
   int head_tiled = 2;     // FLATTEN heads: 0 = one warp per output, 1 = CUDA-core 4 x 4 tiles, 2 = mma.sync 16 x 32 tiles
-  int shrink_fused = 1;   // the LoRA shrink runs as the first work items of the GEMM that consumes it (see pair_gemm.cuh)
+  int shrink_fused = 0;   // 1 / 2: the LoRA shrink runs as the first work items of the GEMM that consumes it (see pair_gemm.cuh);
+                          // opt-in: it needs every CTA pair of the grid resident at once, i.e. the GPU to itself
   int reverse = 1;        // consecutive kernels of a layer walk the rows in alternating directions (L2 reuse)
   int attn_short = 2;     // 0: generic kernel, 1: pipelined mma.sync kernel, 2: tcgen05 head-pair kernel where it applies
   int graph = 1;
@@ -105,6 +107,16 @@ struct Opts {
 struct Strm { cudaStream_t s; int pdl; };
 
 }  // namespace
+
+struct BatchShape {
+  long long N = 0;
+  int max_len = 0, max_out = 0, max_hidden = 0, max_out2 = 0, max_out_flat = 0, n_blk = 0;
+  bool any_flat = false, any_pooled = false;
+  bool operator==(const BatchShape &o) const {
+    return N == o.N && max_len == o.max_len && max_out == o.max_out && max_hidden == o.max_hidden && max_out2 == o.max_out2 &&
+           max_out_flat == o.max_out_flat && any_flat == o.any_flat && any_pooled == o.any_pooled;
+  }
+};
 
 struct fmx_ctx {
   int device = 0, sm_count = 0;
@@ -121,20 +133,19 @@ struct fmx_ctx {
   int *d_task_head_w1 = nullptr;           // first-layer width of the head (= head_out for linear heads)
   int *d_task_enc_ch = nullptr;            // input-encoder channels by task
   const bf16 **d_task_enc_W = nullptr, **d_task_enc_b = nullptr;
-  // pinned staging for ids / lengths: a ring (a slot is rewritten only after the copy that read it has run) plus one
-  // buffer owned by the cached CUDA graph
+  // pinned staging for ids / lengths: a ring (a slot is rewritten only after the copy that read it has run)
   static constexpr int kStageSlots = 4;
   int *h_stage = nullptr;                  // [kStageSlots + 1][2 * FMX_MAX_REQUESTS]
   cudaEvent_t stage_ev[kStageSlots] = {nullptr, nullptr, nullptr, nullptr};
   bool stage_used[kStageSlots] = {false, false, false, false};
   int stage_next = 0;
-  // CUDA-graph cache of the forward (FMX_OPT_GRAPH): the third identical call onwards replays one captured graph
+  // CUDA-graph cache of the forward (FMX_OPT_GRAPH): keyed by buffers + BatchShape, not by the ids (see forward_cached)
   struct CallKey {
     int bb = -1, B = 0; const void *inputs = nullptr; float *outputs = nullptr; void *workspace = nullptr; size_t ws_bytes = 0;
-    cudaStream_t stream = nullptr; unsigned long long gen = 0; std::vector<int> ids, lens;
+    cudaStream_t stream = nullptr; unsigned long long gen = 0; BatchShape shape; bool fuse = false;
     bool operator==(const CallKey &o) const {
       return bb == o.bb && B == o.B && inputs == o.inputs && outputs == o.outputs && workspace == o.workspace && ws_bytes == o.ws_bytes &&
-             stream == o.stream && gen == o.gen && ids == o.ids && lens == o.lens;
+             stream == o.stream && gen == o.gen && shape == o.shape && fuse == o.fuse;
     }
   };
   // registration runs on its own non-blocking stream: adding a task never waits for (or stalls) forwards in flight
@@ -442,6 +453,13 @@ void launch_attention_tc_v(Strm s, int max_len, int n_heads, int B, const AttnTc
   launch_k((attention_tc_kernel<DH, kQT, kSt, kMinB>), grid, attn_tc_threads<kQT>(), attn_tc_smem_bytes<DH, kQT, kSt>(), s, a);
 }
 void launch_attention_tc(Strm s, int dh, int variant, int max_len, int n_heads, int B, const AttnTcArgs &a) {
+  if (variant == 0) {        // the light one-q-tile CTA (attention_fa.cuh): 4 CTAs per SM for head_dim 64, 2 for 128
+    dim3 grid((max_len + kAtBQ - 1) / kAtBQ, n_heads, B);
+    if (dh == 64) launch_k((attention_fa_kernel<64, 1, 4>), grid, kFaThreads, attn_fa_smem_bytes<64>(), s, a);
+    else launch_k((attention_fa_kernel<128, 2, 2>), grid, kFaThreads, attn_fa_smem_bytes<128>(), s, a);
+    return;
+  }
+  variant -= 1;
   if (dh == 64) {
     if (variant == 0) launch_attention_tc_v<64, 1, 3, 2>(s, max_len, n_heads, B, a);
     else launch_attention_tc_v<64, 2, 3, 1>(s, max_len, n_heads, B, a);
@@ -469,7 +487,24 @@ cudaError_t set_attn_tc_attr() {
   return e;
 }
 
+template <int DH, int kSBuf, int kMinB>
+cudaError_t set_attn_fa_attr() {
+  cudaError_t e = cudaFuncSetAttribute(attention_fa_kernel<DH, kSBuf, kMinB>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_fa_smem_bytes<DH>());
+  // without this the driver sizes the L1/shared split for ONE block and further CTAs never become resident
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(attention_fa_kernel<DH, kSBuf, kMinB>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  if (e == cudaSuccess && getenv("FMX_DEBUG")) {
+    int nb = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, attention_fa_kernel<DH, kSBuf, kMinB>, kFaThreads, attn_fa_smem_bytes<DH>());
+    cudaFuncAttributes fa{};
+    cudaFuncGetAttributes(&fa, attention_fa_kernel<DH, kSBuf, kMinB>);
+    fprintf(stderr, "fmx: attention_fa<%d,%d,%d>: %d B smem, %d CTA/SM, %d regs\n", DH, kSBuf, kMinB, attn_fa_smem_bytes<DH>(), nb, fa.numRegs);
+  }
+  return e;
+}
+
 int set_kernel_attrs() {
+  CU_OK((set_attn_fa_attr<64, 1, 4>()));
+  CU_OK((set_attn_fa_attr<128, 2, 2>()));
   CU_OK((set_attn_tc_attr<64, 1, 3, 2>()));
   CU_OK((set_attn_tc_attr<64, 2, 3, 1>()));
   CU_OK((set_attn_tc_attr<128, 1, 2, 2>()));
@@ -1058,16 +1093,15 @@ int fmx_host_workspace_bytes(fmx_ctx *c, fmx_backbone_t h, int32_t max_req, int6
 }
 
 // ---------------------------------------------------------------- the forward
-// graph_capture: the stream is being captured into the context's cached graph: ids / lengths go through the graph's own
-// pinned buffer and no event is recorded.
-static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int32_t *task_ids, const int32_t *lengths,
-                        int32_t B, float *outputs, void *workspace, size_t workspace_bytes, cudaStream_t s, bool graph_capture = false) {
+// What the launch sequence of a forward depends on, beyond the buffers: everything the host derives from the caller's
+// ids / lengths.  Two batches with the same BatchShape run the SAME kernels with the same grids (the ids / lengths
+// themselves travel to the device tables), so one captured CUDA graph serves both.
+// Host validation of a batch (nothing is enqueued on failure) and its BatchShape.
+static int batch_shape(fmx_ctx *c, const Backbone &bb, const int32_t *task_ids, const int32_t *lengths, int32_t B, BatchShape &bs) {
   const fmx_backbone_desc &d = bb.d;
-  // ---- host validation (nothing is enqueued on failure) ----
-  long long N = 0;
-  int max_len = 0, max_out = 0;
   int bb_index = -1;
   for (size_t i = 0; i < c->bbs.size(); ++i) if (c->bbs[i].get() == &bb) bb_index = (int)i;
+  bs = BatchShape();
   for (int i = 0; i < B; ++i) {
     const int t = task_ids[i];
     if (t < 0 || t >= FMX_MAX_TASKS || !c->tasks[t].live || c->tasks[t].bb != bb_index)
@@ -1075,11 +1109,53 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     const int n = lengths[i];
     if (n < 1 || n > d.max_seq || (d.tokens_per_request && n != d.tokens_per_request))
       return fmx_fail(FMX_E_BAD_LENGTH, "forward_mixed: request %d: length %d (max_seq %d, fixed %d)", i, n, d.max_seq, d.tokens_per_request);
-    N += n;
-    max_len = std::max(max_len, n);
-    max_out = std::max(max_out, c->tasks[t].head_hidden > 0 ? c->tasks[t].head_hidden : c->tasks[t].head_out);   // first-layer width
+    const TaskRec &tr = c->tasks[t];
+    bs.N += n;
+    bs.max_len = std::max(bs.max_len, n);
+    bs.max_out = std::max(bs.max_out, tr.head_hidden > 0 ? tr.head_hidden : tr.head_out);   // first-layer width
+    if (tr.head_hidden > 0) { bs.max_hidden = std::max(bs.max_hidden, tr.head_hidden); bs.max_out2 = std::max(bs.max_out2, tr.head_out); }
+    if (tr.head_kind == FMX_HEAD_FLATTEN) { bs.any_flat = true; bs.max_out_flat = std::max(bs.max_out_flat, tr.head_out); }
+    else bs.any_pooled = true;
   }
-  if (N > (1ll << 24)) return fmx_fail(FMX_E_CAPACITY, "forward_mixed: %lld tokens > 2^24", N);
+  if (bs.N > (1ll << 24)) return fmx_fail(FMX_E_CAPACITY, "forward_mixed: %lld tokens > 2^24", bs.N);
+  // (tile, task) blocks of the task-sorted batch (the device computes the same number in S1)
+  const int T = c->n_slots;
+  std::vector<long long> tok(T + 1, 0);
+  for (int i = 0; i < B; ++i) tok[task_ids[i]] += lengths[i];
+  long long lo = 0;
+  for (int t = 0; t < T; ++t) {
+    if (tok[t] == 0) continue;
+    const long long hi = lo + tok[t];
+    bs.n_blk += (int)((hi - 1) / kPairRows - lo / kPairRows + 1);
+    lo = hi;
+  }
+  return FMX_OK;
+}
+
+// ids / lengths -> the device tables, through the pinned staging ring (a slot is rewritten only after the copy that read it
+// has run).  Never part of a captured graph: a replay serves a NEW batch, so these copies are enqueued before every launch.
+static int stage_ids(fmx_ctx *c, const Workspace &w, const int32_t *task_ids, const int32_t *lengths, int32_t B, cudaStream_t s) {
+  const int slot = c->stage_next;
+  c->stage_next = (c->stage_next + 1) % fmx_ctx::kStageSlots;
+  if (c->stage_used[slot]) CU_OK(cudaEventSynchronize(c->stage_ev[slot]));
+  int *stage = c->h_stage + (size_t)slot * 2 * FMX_MAX_REQUESTS;
+  memcpy(stage, task_ids, sizeof(int) * B);
+  memcpy(stage + FMX_MAX_REQUESTS, lengths, sizeof(int) * B);
+  CU_OK(cudaMemcpyAsync(w.t.task_ids, stage, sizeof(int) * B, cudaMemcpyHostToDevice, s));
+  CU_OK(cudaMemcpyAsync(w.t.lengths, stage + FMX_MAX_REQUESTS, sizeof(int) * B, cudaMemcpyHostToDevice, s));
+  CU_OK(cudaEventRecord(c->stage_ev[slot], s));
+  c->stage_used[slot] = true;
+  return FMX_OK;
+}
+
+// graph_capture: the stream is being captured into the context's cached graph: ids / lengths go through the graph's own
+// pinned buffer and no event is recorded.
+static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int32_t *task_ids, const int32_t *lengths,
+                        int32_t B, float *outputs, void *workspace, size_t workspace_bytes, cudaStream_t s, const BatchShape &bs,
+                        bool graph_capture = false) {
+  const fmx_backbone_desc &d = bb.d;
+  const long long N = bs.N;
+  const int max_len = bs.max_len, max_out = bs.max_out;
   const int T = c->n_slots;
   if (reinterpret_cast<uintptr_t>(workspace) & 1023) return fmx_fail(FMX_E_WORKSPACE, "forward_mixed: workspace must be 1024-byte aligned");
   Workspace w = carve(bb, workspace, B, N, T);
@@ -1093,27 +1169,15 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   int dir = 0;
   auto rev = [&]() { const int r = c->o.reverse ? dir : 0; dir ^= 1; return r; };
   // ---- S1: ids/lengths to the device, counting sort, tables ----
-  cudaStreamCaptureStatus cap_status = cudaStreamCaptureStatusNone;
-  if (!graph_capture) CU_OK(cudaStreamIsCapturing(s, &cap_status));
-  // ids / lengths reach the device through the library's pinned staging ring, whose slots are rewritten a few calls later:
-  // a graph the CALLER captures would replay stale copies, so a capturing stream is refused (the library keeps its own
-  // graph cache, FMX_OPT_GRAPH).
-  if (cap_status != cudaStreamCaptureStatusNone)
-    return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed: the stream is being captured; capture is not supported (the library caches its own CUDA graph)");
-  int slot = fmx_ctx::kStageSlots;                                         // the graph's buffer
   if (!graph_capture) {
-    slot = c->stage_next;
-    c->stage_next = (c->stage_next + 1) % fmx_ctx::kStageSlots;
-    if (c->stage_used[slot]) CU_OK(cudaEventSynchronize(c->stage_ev[slot]));
-  }
-  int *stage = c->h_stage + (size_t)slot * 2 * FMX_MAX_REQUESTS;
-  memcpy(stage, task_ids, sizeof(int) * B);
-  memcpy(stage + FMX_MAX_REQUESTS, lengths, sizeof(int) * B);
-  CU_OK(cudaMemcpyAsync(w.t.task_ids, stage, sizeof(int) * B, cudaMemcpyHostToDevice, s));
-  CU_OK(cudaMemcpyAsync(w.t.lengths, stage + FMX_MAX_REQUESTS, sizeof(int) * B, cudaMemcpyHostToDevice, s));
-  if (!graph_capture) {
-    CU_OK(cudaEventRecord(c->stage_ev[slot], s));
-    c->stage_used[slot] = true;
+    // ids / lengths reach the device through the library's pinned staging ring, whose slots are rewritten a few calls later:
+    // a graph the CALLER captures would replay stale copies, so a capturing stream is refused (the library keeps its own
+    // graph cache, FMX_OPT_GRAPH).
+    cudaStreamCaptureStatus cap_status = cudaStreamCaptureStatusNone;
+    CU_OK(cudaStreamIsCapturing(s, &cap_status));
+    if (cap_status != cudaStreamCaptureStatusNone)
+      return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed: the stream is being captured; capture is not supported (the library caches its own CUDA graph)");
+    if (int e = stage_ids(c, w, task_ids, lengths, B, s)) return e;
   }
   SortArgs sa{};
   sa.t = w.t; sa.B = B; sa.T = T; sa.n_tiles = w.n_tiles; sa.tile_rows = kPairRows; sa.task_head_out = c->d_task_head_out;
@@ -1182,24 +1246,12 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     }
     if (p.n_sh == 0) return;
     p.blk_tile = w.t.blk_tile; p.blk_lo = w.t.blk_lo; p.blk_hi = w.t.blk_hi; p.n_blk = w.t.n_blk;
-    p.task_scale = c->d_task_scale; p.U = w.U; p.u_flag = w.u_flag; p.u_epoch = ++u_epoch;
+    p.task_scale = c->d_task_scale; p.U = w.U; p.u_flag = w.u_flag; p.u_epoch = ++u_epoch; p.err = c->d_err;
   };
-  // (tile, task) blocks of the sorted batch, counted on the host from the caller's ids / lengths (the device computes the
-  // same number in S1).  Measured on B200: fusing pays when the shrink items fit ONE wave of the persistent grid (cfg2:
-  // 73 blocks on 74 pairs, -0.4 ms per step); with more blocks the items' low arithmetic intensity costs as much as the
-  // separate shrink launches (cfg3 / cfg4 / cfg5 at 92 tasks: +-0), so those keep the dedicated kernel.
-  int n_blk_host = 0;
-  {
-    std::vector<long long> tok(T + 1, 0);
-    for (int i = 0; i < B; ++i) tok[task_ids[i]] += lengths[i];
-    long long lo = 0;
-    for (int t = 0; t < T; ++t) {
-      if (tok[t] == 0) continue;
-      const long long hi = lo + tok[t];
-      n_blk_host += (int)((hi - 1) / kPairRows - lo / kPairRows + 1);
-      lo = hi;
-    }
-  }
+  // (tile, task) blocks of the sorted batch (bs.n_blk, counted on the host).  Measured on B200: fusing pays when the shrink
+  // items fit ONE wave of the persistent grid (cfg2: 73 blocks on 74 pairs, -0.4 ms per step); with more blocks the items'
+  // low arithmetic intensity costs as much as the separate shrink launches (cfg3 / cfg4 / cfg5 at 92 tasks: +-0).
+  const int n_blk_host = bs.n_blk;
   const bool fuse_ok = c->o.shrink_fused && c->pairs_resident && (c->o.shrink_fused == 2 || n_blk_host <= c->sm_count / 2);
   if (fuse_ok) CU_OK(cudaMemsetAsync(w.u_flag, 0, sizeof(unsigned), s));
   // fusable: all CTA pairs of the persistent grid are co-resident (the expand steps spin on another pair's result) and
@@ -1354,18 +1406,10 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   ha.out = outputs; ha.d = d.d_model;
   ha.task_head_w1 = c->d_task_head_w1;
   ha.task_head_W2 = (const bf16 *const *)c->d_task_head_W2; ha.task_head_b2 = (const bf16 *const *)c->d_task_head_b2;
-  int max_hidden = 0, max_out2 = 0;                      // MLP heads in this batch
-  for (int i = 0; i < B; ++i) {
-    const TaskRec &tr = c->tasks[task_ids[i]];
-    if (tr.head_hidden > 0) { max_hidden = std::max(max_hidden, tr.head_hidden); max_out2 = std::max(max_out2, tr.head_out); }
-  }
+  const int max_hidden = bs.max_hidden, max_out2 = bs.max_out2;      // MLP heads in this batch
   if (max_hidden > 0) { ha.hid = w.head_hid; ha.ld_hid = max_hidden; }      // max_hidden <= kMaxHeadHidden by registration
-  bool any_flat = false, any_pooled = false;
-  int max_out_flat = 0;
-  for (int i = 0; i < B; ++i) {
-    if (c->tasks[task_ids[i]].head_kind == FMX_HEAD_FLATTEN) { any_flat = true; max_out_flat = std::max(max_out_flat, c->tasks[task_ids[i]].head_out); }
-    else any_pooled = true;
-  }
+  const bool any_flat = bs.any_flat, any_pooled = bs.any_pooled;
+  const int max_out_flat = bs.max_out_flat;
   ha.skip_flatten = (any_flat && c->o.head_tiled) ? 1 : 0;
   if (any_pooled || !ha.skip_flatten) LAUNCH(Lh, F_HEAD, (launch_k(head_kernel, dim3(B, (max_out + 7) / 8), 256, 0, S, ha)));
   if (ha.skip_flatten) {
@@ -1399,11 +1443,15 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   return graph_capture ? FMX_OK : note_forward(c, s);
 }
 
-// The forward with the context's one-entry CUDA-graph cache in front of it (c->mu held by the caller).  The 2nd identical call
-// (same buffers, stream, ids, lengths, registrations, options) is captured, later ones replay it; a step of ~200 short
-// kernels loses ~4 % to launch gaps otherwise (cfg2: 11.55 -> 11.09 ms).
+// The forward with the context's one-entry CUDA-graph cache in front of it (c->mu held by the caller).  The graph holds the
+// kernels only; ids / lengths are copied to the device tables before every launch, so the graph is keyed by the call's
+// buffers and BatchShape, not by the ids: a serving loop whose batches change but keep their shape (a fixed-length backbone
+// at a fixed batch size) replays it on every step.  The 2nd call with the same key is captured, later ones replay; a step
+// of ~200 short kernels loses ~4 % to launch gaps otherwise (cfg2: 11.55 -> 11.09 ms).
 static int forward_cached(fmx_ctx *c, Backbone *bb, fmx_backbone_t h, const void *inputs, const int32_t *task_ids, const int32_t *lengths,
                           int32_t n_req, float *outputs, void *workspace, size_t workspace_bytes, cudaStream_t s) {
+  BatchShape bs;
+  if (int e = batch_shape(c, *bb, task_ids, lengths, n_req, bs)) return e;
   const bool graphable = c->o.graph && !c->prof_on && s != nullptr && s != cudaStreamLegacy && s != cudaStreamPerThread;
   if (graphable) {
     cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
@@ -1411,23 +1459,30 @@ static int forward_cached(fmx_ctx *c, Backbone *bb, fmx_backbone_t h, const void
     if (st == cudaStreamCaptureStatusNone) {
       fmx_ctx::CallKey key;
       key.bb = h; key.B = n_req; key.inputs = inputs; key.outputs = outputs; key.workspace = workspace; key.ws_bytes = workspace_bytes;
-      key.stream = s; key.gen = c->config_gen; key.ids.assign(task_ids, task_ids + n_req); key.lens.assign(lengths, lengths + n_req);
-      if (c->graph_exec && key == c->graph_key) {
-        CU_OK(cudaGraphLaunch(c->graph_exec, s));
-        c->last_launches = c->graph_launches; c->last_stream = s;
-        ++c->graph_replays;
-        return note_forward(c, s);
-      }
-      if (key == c->last_key) {
-        if (c->graph_exec) {                          // the old graph may still be running and owns the graph staging buffer
+      key.stream = s; key.gen = c->config_gen; key.shape = bs;
+      key.fuse = c->o.shrink_fused == 2 || (c->o.shrink_fused == 1 && bs.n_blk <= c->sm_count / 2);
+      const bool hit = c->graph_exec && key == c->graph_key;
+      if (hit || key == c->last_key) {
+        if (reinterpret_cast<uintptr_t>(workspace) & 1023) return fmx_fail(FMX_E_WORKSPACE, "forward_mixed: workspace must be 1024-byte aligned");
+        const Workspace w = carve(*bb, workspace, n_req, bs.N, c->n_slots);
+        if (w.bytes > workspace_bytes) return fmx_fail(FMX_E_WORKSPACE, "forward_mixed: workspace %zu B < required %zu B", workspace_bytes, w.bytes);
+        if (hit) {
+          if (int e = stage_ids(c, w, task_ids, lengths, n_req, s)) return e;
+          CU_OK(cudaGraphLaunch(c->graph_exec, s));
+          c->last_launches = c->graph_launches; c->last_stream = s;
+          c->last_t = w.t; c->last_B = n_req; c->last_T = c->n_slots; c->last_n_tiles = w.n_tiles;
+          ++c->graph_replays;
+          return note_forward(c, s);
+        }
+        if (c->graph_exec) {                          // the old graph may still be running
           CU_OK(cudaStreamSynchronize(c->graph_key.stream));
           cudaGraphExecDestroy(c->graph_exec);
           c->graph_exec = nullptr;
         }
-        CU_OK(cudaStreamSynchronize(s));
+        if (int e = stage_ids(c, w, task_ids, lengths, n_req, s)) return e;
         cudaGraph_t graph = nullptr;
         if (cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
-          const int e = forward_impl(c, *bb, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, s, true);
+          const int e = forward_impl(c, *bb, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, s, bs, true);
           const cudaError_t ce = cudaStreamEndCapture(s, &graph);
           if (e == FMX_OK && ce == cudaSuccess && graph && cudaGraphInstantiate(&c->graph_exec, graph, 0) == cudaSuccess) {
             cudaGraphDestroy(graph);
@@ -1443,11 +1498,14 @@ static int forward_cached(fmx_ctx *c, Backbone *bb, fmx_backbone_t h, const void
         } else {
           cudaGetLastError();
         }
+        // capture failed: the ids are staged already; run the kernels plainly (graph_capture = true skips the staging only)
+        if (int e = forward_impl(c, *bb, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, s, bs, true)) return e;
+        return note_forward(c, s);
       }
       c->last_key = std::move(key);
     }
   }
-  return forward_impl(c, *bb, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, s);
+  return forward_impl(c, *bb, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, s, bs);
 }
 
 // A device-side error of an EARLIER forward (the word is mapped host memory the kernels write): reported by the next call.
@@ -1455,6 +1513,9 @@ static int poll_device_error(fmx_ctx *c) {
   const unsigned e = *(volatile unsigned *)c->h_err;
   if (!e) return FMX_OK;
   *(volatile unsigned *)c->h_err = 0;
+  if (e & 2u)
+    return fmx_fail(FMX_E_CUDA, "an earlier forward's fused LoRA shrink timed out waiting for CTA pairs that never became resident (another "
+                                "kernel held their SMs); its outputs are invalid.  FMX_OPT_SHRINK_FUSED needs the GPU to itself (device error word 0x%x)", e);
   return fmx_fail(FMX_E_INVALID_ARG, "an earlier forward read token ids outside [0, vocab): those rows were embedded as zeros (device error word 0x%x)", e);
 }
 
@@ -1703,7 +1764,7 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
       c->o.pdl = value;
       return FMX_OK;
     case FMX_OPT_ATTENTION_VARIANT:
-      if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attention variant %d", value);
+      if (value < 0 || value > 3) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attention variant %d", value);
       c->o.attn_variant = value;
       return FMX_OK;
   }

@@ -50,9 +50,11 @@ enum {
                                     0: separate RoPE kernel over the bf16 QKV buffer */
   FMX_OPT_HEAD_TILED = 7,        /* FLATTEN heads: 0 = one warp per (request, output), 1 = CUDA-core 4 x 4 register tiles,
                                     2 (default) = mma.sync 16-request x 32-output tiles over K chunks */
-  FMX_OPT_SHRINK_FUSED = 8,      /* the LoRA shrink runs as the first work items of the GEMM that consumes it: 0 = never
-                                    (separate shrink kernel), 1 (default) = when the batch has at most one (tile, task)
-                                    block per CTA pair, 2 = always */
+  FMX_OPT_SHRINK_FUSED = 8,      /* the LoRA shrink runs as the first work items of the GEMM that consumes it: 0 (default) = never
+                                    (separate shrink kernel), 1 = when the batch has at most one (tile, task) block per CTA pair,
+                                    2 = always.  Opt-in: a pair waits for blocks computed by OTHER pairs, so every cluster of the
+                                    grid must be resident at once - true only when no other kernel holds SMs of the device.  A wait
+                                    that times out (~2 s) raises the device error word (fmx_poll_error); it does not trap. */
   FMX_OPT_GRAPH = 9,             /* 1 (default): fmx_forward_mixed captures a CUDA graph on the 2nd identical call (same
                                     buffers, stream, ids, lengths, registrations, options) and replays it afterwards;
                                     needs a non-default stream; 0: always plain launches */

@@ -38,62 +38,47 @@ struct SortArgs {
 
 constexpr int kSortThreads = 1024;
 
-// Block-wide exclusive scan of n ints (global or shared), in place; returns the total.
-// Every thread of the block must call it.  scratch: kSortThreads + 1 ints of shared memory.
-__device__ inline long long block_exclusive_scan_ll(long long *a, int n, long long *scratch) {
-  const int tid = threadIdx.x, nt = blockDim.x;
+// Block-wide exclusive scan of n values (global or shared), in place; returns the total.  Every thread of the block
+// (kSortThreads of them) must call it.  Each thread owns a run of consecutive elements; the run sums are scanned with warp
+// shuffles (one pass inside each warp, one over the 32 warp totals): two block barriers per scan, no serial loop.
+// scratch: 33 values of shared memory.
+template <typename V>
+__device__ inline V block_exclusive_scan(V *a, int n, V *scratch) {
+  const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, wid = tid >> 5;
   const int per = (n + nt - 1) / nt;
   const int lo = min(tid * per, n), hi = min(lo + per, n);
-  long long s = 0;
+  V s = 0;
   for (int i = lo; i < hi; ++i) s += a[i];
-  scratch[tid] = s;
+  V incl = s;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const V v = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += v; }
+  if (lane == 31) scratch[wid] = incl;
   __syncthreads();
-  if (tid == 0) {
-    long long run = 0;
-    for (int i = 0; i < nt; ++i) { long long v = scratch[i]; scratch[i] = run; run += v; }
-    scratch[nt] = run;
+  if (wid == 0) {
+    const V w = lane < (nt >> 5) ? scratch[lane] : V(0);
+    V wi = w;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const V v = __shfl_up_sync(0xffffffffu, wi, d); if (lane >= d) wi += v; }
+    scratch[lane] = wi - w;                       // exclusive offset of warp `lane`
+    if (lane == 31) scratch[32] = wi;             // grand total
   }
   __syncthreads();
-  long long run = scratch[tid];
-  for (int i = lo; i < hi; ++i) { long long v = a[i]; a[i] = run; run += v; }
-  const long long total = scratch[nt];
+  V run = scratch[wid] + incl - s;
+  for (int i = lo; i < hi; ++i) { const V v = a[i]; a[i] = run; run += v; }
+  const V total = scratch[32];
   __syncthreads();
   return total;
 }
-
-__device__ inline int block_exclusive_scan_i(int *a, int n, int *scratch) {
-  const int tid = threadIdx.x, nt = blockDim.x;
-  const int per = (n + nt - 1) / nt;
-  const int lo = min(tid * per, n), hi = min(lo + per, n);
-  int s = 0;
-  for (int i = lo; i < hi; ++i) s += a[i];
-  scratch[tid] = s;
-  __syncthreads();
-  if (tid < 32) {                                  // warp 0 scans the 1024 partials, 32 per lane
-    const int seg = nt / 32;
-    int part = 0;
-    for (int i = 0; i < seg; ++i) part += scratch[tid * seg + i];
-    int incl = part;
-    for (int d = 1; d < 32; d <<= 1) { int v = __shfl_up_sync(0xffffffffu, incl, d); if (tid >= d) incl += v; }
-    int run = incl - part;
-    for (int i = 0; i < seg; ++i) { int v = scratch[tid * seg + i]; scratch[tid * seg + i] = run; run += v; }
-    if (tid == 31) scratch[nt] = incl;
-  }
-  __syncthreads();
-  int run = scratch[tid];
-  for (int i = lo; i < hi; ++i) { int v = a[i]; a[i] = run; run += v; }
-  const int total = scratch[nt];
-  __syncthreads();
-  return total;
-}
+__device__ inline long long block_exclusive_scan_ll(long long *a, int n, long long *scratch) { return block_exclusive_scan<long long>(a, n, scratch); }
+__device__ inline int block_exclusive_scan_i(int *a, int n, int *scratch) { return block_exclusive_scan<int>(a, n, scratch); }
 
 // One CTA.  Stable counting sort of request indices by task id, then the prefix tables and the
 // (row-tile, task) block table the segmented GEMMs walk.  Integer only; deterministic.
 __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortArgs a) {
   __shared__ int s_cnt[1024 + 1];          // per-task count, then task_req_off
   __shared__ int s_tok[1024 + 1];          // task_tok_off
-  __shared__ int s_scratch[kSortThreads + 1];
-  __shared__ long long s_scratch_ll[kSortThreads + 1];
+  __shared__ int s_scratch[33];
+  __shared__ long long s_scratch_ll[33];
   __shared__ int s_rank[4096];             // rank of request i within its task
   const int tid = threadIdx.x, B = a.B, T = a.T;
   const SegTables &t = a.t;

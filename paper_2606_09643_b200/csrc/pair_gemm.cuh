@@ -84,6 +84,7 @@ struct PairGemmParams {
   const float *task_scale; // [T*7] alpha / r
   __nv_bfloat16 *U;        // [n_blk_cap*256, 192]
   unsigned *u_flag;        // one counter: arrivals of the epilogue warps that wrote a U block (monotonic over a forward)
+  unsigned *err;           // the context's device error word (bit 1: the fused-shrink wait timed out)
   unsigned u_epoch;        // 1, 2, ... over the fused launches of a forward: this launch's U is complete when the counter
                            // reaches 16 (epilogue warps of a pair) * n_blk * u_epoch
   const float2 *rope_cs;   // [64, rope_ld] (cos, sin), pair-index major: fused rotate-half RoPE for head_dim 128 (chunk = head), or NULL
@@ -283,7 +284,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
                 while (ld_acquire_gpu(p.u_flag) < target) {
                   // the shrink items are the FIRST items of every resident pair, so this wait is short; a bound of ~2 s
                   // of SM clocks turns a scheduling assumption that does not hold into an error instead of a hang
-                  if (clock64() - t_wait0 > (1ll << 32)) __trap();
+                  if (clock64() - t_wait0 > (1ll << 32)) { *p.err = 2u; break; }   // reported by the next call; no trap
                 }
                 fence_proxy_async_global();
                 u_ready = true;

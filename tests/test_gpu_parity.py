@@ -143,7 +143,7 @@ def test_every_kernel_option_gives_the_oracle_result(fmx_mod, cfg, kw):
             check_parity(outs[fused], ref, f"{cfg} shrink_fused={fused}")
         for a, b in zip(outs[0], outs[2]):
             assert np.array_equal(a, b), "fused and separate LoRA shrink must be bit-identical"
-        s.fmx.set_option("shrink_fused", 1)
+        s.fmx.set_option("shrink_fused", 0)
         for opt, val, restore in (("half_tiles", 0, 1), ("rope_fused", 0, 1), ("head_tiled", 0, 2), ("head_tiled", 1, 2), ("reverse", 0, 1), ("expand_wide", 0, 1), ("deep_pipe", 0, 1), ("pdl", 1, 2), ("pdl", 0, 2)):
             s.fmx.set_option(opt, val)
             try:
@@ -151,7 +151,7 @@ def test_every_kernel_option_gives_the_oracle_result(fmx_mod, cfg, kw):
             finally:
                 s.fmx.set_option(opt, restore)
     finally:
-        s.fmx.set_option("shrink_fused", 1)
+        s.fmx.set_option("shrink_fused", 0)
 
 
 # ---------------------------------------------------------------- full sizes, sampled outputs
@@ -423,35 +423,44 @@ def test_host_buffer_forward_matches_device_forward(fmx_mod):
         assert np.array_equal(got[off[i]:off[i + 1]], dev[i])
 
 
-def test_cuda_graph_cache_replays_only_identical_calls(fmx_mod):
-    """FMX_OPT_GRAPH: on a non-default stream the 2nd identical call is captured and later ones replay the graph.  The
-    replayed result equals the plain one bit for bit; different task ids, a registration change or the default stream
-    never replay a stale graph."""
+def test_cuda_graph_cache_is_keyed_by_shape_not_by_ids(fmx_mod):
+    """FMX_OPT_GRAPH: on a non-default stream the 2nd call with the same buffers and batch SHAPE is captured and later ones
+    replay the graph - also when the task ids change (ids / lengths are copied to the device tables before every launch, the
+    graph holds the kernels only), which is what a serving loop with changing batches needs.  Replayed results equal the plain
+    ones bit for bit; a different batch size, a registration / option change or the default stream never replay a stale graph."""
     wl = make_workload("cfg2", n_layers=2, batch=20)
     s = _session(fmx_mod, wl)
     plain = s.forward_numpy()                                    # torch's default stream: never graphed
     assert s.fmx.graph_replays() == 0
+    variants = [np.roll(wl.task_ids, k) for k in (1, 3, 7)] + [wl.task_ids[::-1].copy()]
+    plain_v = [s.forward_numpy(task_ids=v) for v in variants]
     st = torch.cuda.Stream()
+
+    def run(ids=None, n=None):
+        s.forward(task_ids=ids, stream=st) if n is None else s.forward(task_ids=ids[:n], lengths=wl.lengths[:n], stream=st)
+        st.synchronize()
+        flat = s.out_dev.cpu().numpy()
+        return [flat[s.last_off[i]:s.last_off[i + 1]].copy() for i in range(len(s.last_off) - 1)]
+
     with torch.cuda.stream(st):
-        outs = []
-        for _ in range(4):
-            s.forward(stream=st)
-            st.synchronize()
-            flat = s.out_dev.cpu().numpy()
-            outs.append([flat[s.last_off[i]:s.last_off[i + 1]].copy() for i in range(wl.n_req)])
+        outs = [run() for _ in range(4)]
         assert s.fmx.graph_replays() == 2                        # call 1 plain, call 2 capture + launch, calls 3-4 replay
         for o in outs:
             for a, b in zip(o, plain):
                 assert np.array_equal(a, b)
-        # other task ids, same shapes: must run the new batch, not the cached graph
-        ids2 = np.roll(wl.task_ids, 1)
-        s.forward(task_ids=ids2, stream=st)
-        st.synchronize()
-        assert s.fmx.graph_replays() == 2
-        flat = s.out_dev.cpu().numpy()
-        got = [flat[s.last_off[i]:s.last_off[i + 1]].copy() for i in range(wl.n_req)]
-    ref = s.forward_numpy(task_ids=ids2)
-    for a, b in zip(got, ref):
+        # other task ids, same shape: the SAME graph serves the new batch
+        for v, want in zip(variants, plain_v):
+            got = run(v)
+            for a, b in zip(got, want):
+                assert np.array_equal(a, b), "a replayed graph must serve the ids of THIS call"
+        shapes_equal = all(set(np.asarray(v).tolist()) == set(wl.task_ids.tolist()) for v in variants)
+        assert shapes_equal and s.fmx.graph_replays() == 2 + len(variants)
+        # a smaller batch: another shape, no replay
+        n0 = s.fmx.graph_replays()
+        got = run(wl.task_ids, n=12)
+        assert s.fmx.graph_replays() == n0
+    ref12 = s.forward_numpy(task_ids=wl.task_ids[:12], lengths=wl.lengths[:12])
+    for a, b in zip(got, ref12):
         assert np.array_equal(a, b)
     # option change invalidates the cached graph
     with torch.cuda.stream(st):
@@ -679,7 +688,7 @@ def test_two_contexts_keep_their_own_options(fmx_mod):
     wl = make_workload("cfg2", n_layers=2, batch=40)
     a, b = _session(fmx_mod, wl), _session(fmx_mod, wl)
     alone = a.forward_numpy()
-    b.fmx.set_option("shrink_fused", 0)
+    b.fmx.set_option("expand_wide", 0)
     b.fmx.set_option("pdl", 1)
     b.fmx.set_option("half_tiles", 0)
     b.fmx.set_option("reverse", 0)
