@@ -77,13 +77,14 @@ __device__ __forceinline__ float fa_chunk_exp(const uint32_t (&v)[NC], uint32_t 
   return (r4[0] + r4[1]) + (r4[2] + r4[3]);
 }
 
-template <int DH, int kSBuf, int kMinBlocks>
+template <int DH, int kSBuf, int kMinBlocks, bool kOnePass>
 __global__ void __launch_bounds__(kFaThreads, kMinBlocks) attention_fa_kernel(const __grid_constant__ AttnTcArgs a) {
   constexpr int kKB = DH / 64;                        // 64-column blocks of the head
   constexpr int kQBytes = kKB * 16384;                // the q-tile
   constexpr int kKVBytes = kKB * 8192;                // one K (or V) tile
-  constexpr uint32_t kTmemCols = kSBuf * 64 + DH;     // [S / P : 64] x kSBuf, [O : DH]
-  static_assert(kTmemCols == 128 || kTmemCols == 256, "TMEM allocation is a power of two");
+  constexpr uint32_t kTmemUsed = kSBuf * 64 + DH;     // [S / P : 64] x kSBuf, [O : DH]
+  constexpr uint32_t kTmemCols = kTmemUsed <= 128 ? 128 : 256;      // the allocation is a power of two
+  static_assert(kTmemUsed <= 256, "TMEM budget");
   extern __shared__ uint8_t fa_smem_raw[];
   const uint32_t raw_addr = smem_u32(fa_smem_raw);
   const uint32_t pad = (1024u - (raw_addr & 1023u)) & 1023u;
@@ -97,9 +98,14 @@ __global__ void __launch_bounds__(kFaThreads, kMinBlocks) attention_fa_kernel(co
   uint64_t &q_full = bars[0];
   uint64_t *k_full = bars + 1, *k_empty = k_full + kFaStages, *v_full = k_empty + kFaStages, *v_empty = v_full + kFaStages;
   uint64_t *s_full = v_empty + kFaStages;             // [kSBuf]
-  uint64_t &p_ready = s_full[kSBuf], &pv_done = s_full[kSBuf + 1];
-  uint32_t &tmem_base_slot = *reinterpret_cast<uint32_t *>(&s_full[kSBuf + 2]);
-  static_assert((1 + 4 * kFaStages + kSBuf + 2 + 1) * 8 <= 128, "barrier block");
+  // one p_ready barrier per S buffer: with a single one a softmax warp that runs ahead into tile j + 1 (its S is already there
+  // when S is double-buffered) would complete phase j with its second arrival
+  uint64_t *p_ready = s_full + kSBuf;                 // [kSBuf]
+  // pv_done: one phase per PV (the rare O rescale of tile j waits for PV_(j-1): at that point at most one phase is pending);
+  // o_full: completes once, after the LAST PV - the epilogue cannot use pv_done, a fast tail tile may be two phases ahead
+  uint64_t &pv_done = s_full[2 * kSBuf], &o_full = s_full[2 * kSBuf + 1];
+  uint32_t &tmem_base_slot = *reinterpret_cast<uint32_t *>(&s_full[2 * kSBuf + 2]);
+  static_assert((1 + 4 * kFaStages + 2 * kSBuf + 2) * 8 + 4 <= 128, "barrier block");
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int p = a.reverse ? (int)gridDim.z - 1 - (int)blockIdx.z : (int)blockIdx.z, head = blockIdx.y;
@@ -117,9 +123,9 @@ __global__ void __launch_bounds__(kFaThreads, kMinBlocks) attention_fa_kernel(co
   if (threadIdx.x == 0) {
     mbar_init(&q_full, 1);
     for (int s = 0; s < kFaStages; ++s) { mbar_init(&k_full[s], 1); mbar_init(&k_empty[s], 1); mbar_init(&v_full[s], 1); mbar_init(&v_empty[s], 1); }
-    for (int s = 0; s < kSBuf; ++s) mbar_init(&s_full[s], 1);
-    mbar_init(&p_ready, 4);
+    for (int s = 0; s < kSBuf; ++s) { mbar_init(&s_full[s], 1); mbar_init(&p_ready[s], 4); }
     mbar_init(&pv_done, 1);
+    mbar_init(&o_full, 1);
     fence_barrier_init();
   }
   if (warp == 1) {
@@ -188,7 +194,7 @@ __global__ void __launch_bounds__(kFaThreads, kMinBlocks) attention_fa_kernel(co
           tc_fence_after();
           issue_s(j + 1, nstage);
         }
-        mbar_wait(&p_ready, j & 1);                    // P_j sits in TMEM (over S_j), O rescaled if it had to be
+        mbar_wait(&p_ready[kSBuf == 2 ? (j & 1) : 0], kSBuf == 2 ? ((j >> 1) & 1) : (j & 1));   // P_j sits in TMEM (over S_j), O rescaled if it had to be
         mbar_wait(&v_full[stage], phase);
         tc_fence_after();
         const uint32_t t_p = tmem_base + (kSBuf == 2 ? (j & 1) * 64 : 0);
@@ -198,6 +204,7 @@ __global__ void __launch_bounds__(kFaThreads, kMinBlocks) attention_fa_kernel(co
           umma_bf16_ts(tm_o, t_p + 8 * k, make_smem_desc_sw128_mn(va + k * 2048, 8192), idesc_o, (j | k) != 0);
         umma_commit(&v_empty[stage]);
         umma_commit(&pv_done);
+        if (j + 1 == nkv) umma_commit(&o_full);
         if (kSBuf == 1 && j + 1 < nkv) {               // same S buffer: in pipe order after PV_j has read P_j
           mbar_wait(&k_full[nstage], nphase);
           tc_fence_after();
@@ -226,64 +233,66 @@ __global__ void __launch_bounds__(kFaThreads, kMinBlocks) attention_fa_kernel(co
         const uint32_t t_s = tmem_base + sb * 64 + lane_sel;
         const int key0 = j * kAtBKV;
         const bool need_mask = key0 + cols > n || (a.causal && key0 + cols - 1 > warp_row_lo);
-        // ---- pass 1: the row maximum of the tile ----
-        float mx;
-        if (cols == 64) {
-          uint32_t v[32];
-          tmem_ld_32x32(t_s, v);
-          tmem_ld_wait();
-          mx = fa_chunk_max<32>(v, key0, lim, need_mask);
-          tmem_ld_32x32(t_s + 32, v);
-          tmem_ld_wait();
-          mx = fmaxf(mx, fa_chunk_max<32>(v, key0 + 32, lim, need_mask));
-        } else {
-          uint32_t v[16];
-          tmem_ld_32x16(t_s, v);
-          tmem_ld_wait();
-          mx = fa_chunk_max<16>(v, key0, lim, need_mask);
-        }
-        mx *= a.scale_log2;                                          // scale > 0; -inf stays -inf
+        // the reference maximum moves lazily; when it does, O (quiescent once PV_(j-1) has completed) is rescaled in TMEM
         float factor = 1.0f;
-        bool rescale = false;
-        if (j == 0) {
-          m_ref = (mx == -INFINITY) ? 0.0f : mx;
-        } else if (mx > m_ref + 8.0f) {
-          factor = fast_exp2(m_ref - mx);
-          m_ref = mx;
-          rescale = true;
-        }
-        if (j > 0 && __any_sync(0xffffffffu, rescale)) {
-          mbar_wait(&pv_done, (j - 1) & 1);                          // O is quiescent: PV_(j-1) has completed
-          tc_fence_after();
-#pragma unroll 1
-          for (int c = 0; c < DH; c += 32) {
-            uint32_t o[32];
-            tmem_ld_32x32(t_o + c, o);
-            tmem_ld_wait();
-#pragma unroll
-            for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * factor);
-            tmem_st_32x32(t_o + c, o);
+        auto update_ref = [&](float mx) {
+          mx *= a.scale_log2;                                        // scale > 0; -inf stays -inf
+          bool rescale = false;
+          if (j == 0) {
+            m_ref = (mx == -INFINITY) ? 0.0f : mx;
+          } else if (mx > m_ref + 8.0f) {
+            factor = fast_exp2(m_ref - mx);
+            m_ref = mx;
+            rescale = true;
           }
-        }
-        // ---- pass 2: P = exp2(S c - m_ref) over S's own columns (chunk c of P lands on columns S chunk <= c occupied) ----
+          if (j > 0 && __any_sync(0xffffffffu, rescale)) {
+            mbar_wait(&pv_done, (j - 1) & 1);
+            tc_fence_after();
+#pragma unroll 1
+            for (int c = 0; c < DH; c += 32) {
+              uint32_t o[32];
+              tmem_ld_32x32(t_o + c, o);
+              tmem_ld_wait();
+#pragma unroll
+              for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * factor);
+              tmem_st_32x32(t_o + c, o);
+            }
+          }
+        };
+        // P = exp2(S c - m_ref) goes back over S's own columns (chunk c of P lands on columns that S chunks <= c occupied)
         float rs;
-        if (cols == 64) {
+        if (cols == 64 && kOnePass) {
+          // all 64 scores of the row in registers: one TMEM round trip
+          uint32_t v0[32], v1[32], pk[16];
+          tmem_ld_32x32(t_s, v0);
+          tmem_ld_32x32(t_s + 32, v1);
+          tmem_ld_wait();
+          update_ref(fmaxf(fa_chunk_max<32>(v0, key0, lim, need_mask), fa_chunk_max<32>(v1, key0 + 32, lim, need_mask)));
+          rs = fa_chunk_exp<32>(v0, pk, a.scale_log2, m_ref);
+          tmem_st_32x16(t_s, pk);
+          rs += fa_chunk_exp<32>(v1, pk, a.scale_log2, m_ref);
+          tmem_st_32x16(t_s + 16, pk);
+        } else if (cols == 64) {
+          // two passes over S in 32-column chunks: half the live registers, twice the TMEM loads
           uint32_t v[32], pk[16];
           tmem_ld_32x32(t_s, v);
           tmem_ld_wait();
-          if (need_mask) fa_chunk_max<32>(v, key0, lim, true);
-          rs = fa_chunk_exp<32>(v, pk, a.scale_log2, m_ref);
+          float mx = fa_chunk_max<32>(v, key0, lim, need_mask);
           tmem_ld_32x32(t_s + 32, v);
           tmem_ld_wait();
-          tmem_st_32x16(t_s, pk);
-          if (need_mask) fa_chunk_max<32>(v, key0 + 32, lim, true);
-          rs += fa_chunk_exp<32>(v, pk, a.scale_log2, m_ref);
+          update_ref(fmaxf(mx, fa_chunk_max<32>(v, key0 + 32, lim, need_mask)));
+          rs = fa_chunk_exp<32>(v, pk, a.scale_log2, m_ref);         // second chunk first: it is in registers
+          tmem_ld_32x32(t_s, v);
+          tmem_ld_wait();
           tmem_st_32x16(t_s + 16, pk);
+          if (need_mask) fa_chunk_max<32>(v, key0, lim, true);
+          rs += fa_chunk_exp<32>(v, pk, a.scale_log2, m_ref);
+          tmem_st_32x16(t_s, pk);
         } else {
           uint32_t v[16], pk[8];
           tmem_ld_32x16(t_s, v);
           tmem_ld_wait();
-          if (need_mask) fa_chunk_max<16>(v, key0, lim, true);
+          update_ref(fa_chunk_max<16>(v, key0, lim, need_mask));
           rs = fa_chunk_exp<16>(v, pk, a.scale_log2, m_ref);
           tmem_st_32x8(t_s, pk);
         }
@@ -292,11 +301,11 @@ __global__ void __launch_bounds__(kFaThreads, kMinBlocks) attention_fa_kernel(co
         tc_fence_before();
       }
       __syncwarp();
-      if (lane == 0) mbar_arrive(&p_ready);
+      if (lane == 0) mbar_arrive(&p_ready[sb]);
     }
     // ---- O / l -> bf16 -> global ----
     if (warp_valid) {
-      mbar_wait(&pv_done, (nkv - 1) & 1);
+      mbar_wait(&o_full, 0);
       tc_fence_after();
       const float inv = 1.0f / l_run;
       __nv_bfloat16 *dst = a.out + (size_t)(r0 + qrow) * a.ld_out + head * DH;

@@ -453,13 +453,15 @@ void launch_attention_tc_v(Strm s, int max_len, int n_heads, int B, const AttnTc
   launch_k((attention_tc_kernel<DH, kQT, kSt, kMinB>), grid, attn_tc_threads<kQT>(), attn_tc_smem_bytes<DH, kQT, kSt>(), s, a);
 }
 void launch_attention_tc(Strm s, int dh, int variant, int max_len, int n_heads, int B, const AttnTcArgs &a) {
-  if (variant == 0) {        // the light one-q-tile CTA (attention_fa.cuh): 4 CTAs per SM for head_dim 64, 2 for 128
+  if (variant <= 1) {        // the light one-q-tile CTA (attention_fa.cuh); variant 1 = the other softmax register / occupancy trade
     dim3 grid((max_len + kAtBQ - 1) / kAtBQ, n_heads, B);
-    if (dh == 64) launch_k((attention_fa_kernel<64, 1, 4>), grid, kFaThreads, attn_fa_smem_bytes<64>(), s, a);
-    else launch_k((attention_fa_kernel<128, 2, 2>), grid, kFaThreads, attn_fa_smem_bytes<128>(), s, a);
+    if (dh == 64 && variant == 0) launch_k((attention_fa_kernel<64, 1, 4, false>), grid, kFaThreads, attn_fa_smem_bytes<64>(), s, a);
+    else if (dh == 64) launch_k((attention_fa_kernel<64, 1, 3, true>), grid, kFaThreads, attn_fa_smem_bytes<64>(), s, a);
+    else if (variant == 0) launch_k((attention_fa_kernel<128, 2, 2, true>), grid, kFaThreads, attn_fa_smem_bytes<128>(), s, a);
+    else launch_k((attention_fa_kernel<128, 2, 2, false>), grid, kFaThreads, attn_fa_smem_bytes<128>(), s, a);
     return;
   }
-  variant -= 1;
+  variant -= 2;
   if (dh == 64) {
     if (variant == 0) launch_attention_tc_v<64, 1, 3, 2>(s, max_len, n_heads, B, a);
     else launch_attention_tc_v<64, 2, 3, 1>(s, max_len, n_heads, B, a);
@@ -487,24 +489,26 @@ cudaError_t set_attn_tc_attr() {
   return e;
 }
 
-template <int DH, int kSBuf, int kMinB>
+template <int DH, int kSBuf, int kMinB, bool kOne>
 cudaError_t set_attn_fa_attr() {
-  cudaError_t e = cudaFuncSetAttribute(attention_fa_kernel<DH, kSBuf, kMinB>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_fa_smem_bytes<DH>());
+  cudaError_t e = cudaFuncSetAttribute(attention_fa_kernel<DH, kSBuf, kMinB, kOne>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_fa_smem_bytes<DH>());
   // without this the driver sizes the L1/shared split for ONE block and further CTAs never become resident
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(attention_fa_kernel<DH, kSBuf, kMinB>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(attention_fa_kernel<DH, kSBuf, kMinB, kOne>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
   if (e == cudaSuccess && getenv("FMX_DEBUG")) {
     int nb = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, attention_fa_kernel<DH, kSBuf, kMinB>, kFaThreads, attn_fa_smem_bytes<DH>());
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, attention_fa_kernel<DH, kSBuf, kMinB, kOne>, kFaThreads, attn_fa_smem_bytes<DH>());
     cudaFuncAttributes fa{};
-    cudaFuncGetAttributes(&fa, attention_fa_kernel<DH, kSBuf, kMinB>);
-    fprintf(stderr, "fmx: attention_fa<%d,%d,%d>: %d B smem, %d CTA/SM, %d regs\n", DH, kSBuf, kMinB, attn_fa_smem_bytes<DH>(), nb, fa.numRegs);
+    cudaFuncGetAttributes(&fa, attention_fa_kernel<DH, kSBuf, kMinB, kOne>);
+    fprintf(stderr, "fmx: attention_fa<%d,%d,%d,%d>: %d B smem, %d CTA/SM, %d regs\n", DH, kSBuf, kMinB, (int)kOne, attn_fa_smem_bytes<DH>(), nb, fa.numRegs);
   }
   return e;
 }
 
 int set_kernel_attrs() {
-  CU_OK((set_attn_fa_attr<64, 1, 4>()));
-  CU_OK((set_attn_fa_attr<128, 2, 2>()));
+  CU_OK((set_attn_fa_attr<64, 1, 4, false>()));
+  CU_OK((set_attn_fa_attr<64, 1, 3, true>()));
+  CU_OK((set_attn_fa_attr<128, 2, 2, true>()));
+  CU_OK((set_attn_fa_attr<128, 2, 2, false>()));
   CU_OK((set_attn_tc_attr<64, 1, 3, 2>()));
   CU_OK((set_attn_tc_attr<64, 2, 3, 1>()));
   CU_OK((set_attn_tc_attr<128, 1, 2, 2>()));
@@ -1420,7 +1424,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     int n_kc = 0;
     if (c->o.head_tiled == 2 && d.tokens_per_request > 0)
       for (int k = 1; k <= 8; k *= 2)
-        if (Kf % (256ll * k) == 0) { n_kc = k; if ((long long)groups * ogs * k >= c->sm_count) break; }
+        if (Kf % (256ll * k) == 0) { n_kc = k; if ((long long)groups * ogs * k >= 2ll * c->sm_count) break; }   // >= 2 CTAs per SM: a CTA streams one task's weights per pass at single-SM bandwidth
     while (n_kc > 0 && (size_t)groups * ogs * n_kc * 512 > w.head_part_floats) n_kc /= 2;     // fit the workspace's partial budget
     if (n_kc > 0) {
       LAUNCH(Lh, F_HEAD, (launch_k(head_flatten_mma_kernel, dim3(groups, ogs, n_kc), 256, 0, S, ha, B, n_kc, w.head_part)));
@@ -1764,7 +1768,7 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
       c->o.pdl = value;
       return FMX_OK;
     case FMX_OPT_ATTENTION_VARIANT:
-      if (value < 0 || value > 3) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attention variant %d", value);
+      if (value < 0 || value > 4) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attention variant %d", value);
       c->o.attn_variant = value;
       return FMX_OK;
   }
