@@ -117,12 +117,15 @@ def test_pre_norm_layers_match_torch_transformer_encoder_layer(norm, act, has_bi
 
 
 # ---------------------------------------------------------------- decoder family (+ LoRA) vs transformers' LlamaModel
-def test_decoder_backbone_with_lora_matches_hf_llama_with_merged_weights():
-    tr = pytest.importorskip("transformers")
-    d, Hq, Hkv, dh, Fd, L, vocab, n = 48, 6, 2, 8, 80, 2, 61, 23
+def _llama_fixture(tr):
+    """A 2-layer Llama-shaped decoder (RMSNorm, rotate-half RoPE, GQA 3:1, causal, SwiGLU) with one task's LoRA on all 7
+    targets: the oracle's weight dict / task, and transformers' LlamaForCausalLM carrying the MERGED weights
+    W + (alpha / r) B A and an untied LM head."""
+    d, Hq, Hkv, dh, Fd, L, vocab = 48, 6, 2, 8, 80, 2, 61
     theta, eps = 10000.0, 1e-6
     r = _rng(9643)
-    W = {"embed.table": r.standard_normal((vocab, d)), "final.g": 1 + 0.1 * r.standard_normal(d)}
+    W = {"embed.table": r.standard_normal((vocab, d)), "final.g": 1 + 0.1 * r.standard_normal(d),
+         "lm_head.W": r.standard_normal((vocab, d)) * 0.3}
     dims = dict(q=(d, Hq * dh), k=(d, Hkv * dh), v=(d, Hkv * dh), o=(Hq * dh, d), gate=(d, Fd), up=(d, Fd), down=(Fd, d))
     ranks = dict(q=4, k=2, v=8, o=3, gate=5, up=1, down=6)
     task = dict(id=7, adapters={tg: (ranks[tg], 16.0 / ranks[tg]) for tg in dims}, head_kind="last", head_out=3)
@@ -137,17 +140,12 @@ def test_decoder_backbone_with_lora_matches_hf_llama_with_merged_weights():
     bb = dict(n_layers=L, d_model=d, n_q_heads=Hq, n_kv_heads=Hkv, head_dim=dh, d_ffn=Fd, act="swiglu", norm="rms", norm_eps=eps,
               causal=True, rope_theta=theta, input_kind="tokens", patch_dim=0, has_cls=False, has_bias=False, has_pos=False,
               img_c=0, img_hw=0, patch_hw=0)
-    toks = r.integers(0, vocab, size=n)
-    h = O.tokens_from_input(bb, W.__getitem__, toks)
-    for l in range(L):
-        h = O.layer_forward(bb, W.__getitem__, task, l, h)
-    got = O.rms_norm(h, W["final.g"], eps)                      # what head_forward pools from
-
     cfg = tr.LlamaConfig(vocab_size=vocab, hidden_size=d, intermediate_size=Fd, num_hidden_layers=L, num_attention_heads=Hq,
                          num_key_value_heads=Hkv, head_dim=dh, hidden_act="silu", max_position_embeddings=64, rms_norm_eps=eps,
                          rope_theta=theta, attention_bias=False, mlp_bias=False, attention_dropout=0.0, tie_word_embeddings=False)
     cfg._attn_implementation = "eager"
-    model = tr.LlamaModel(cfg).to(torch.float64).eval()
+    lm = tr.LlamaForCausalLM(cfg).to(torch.float64).eval()
+    model = lm.model
     # rotary tables are buffers built in fp32: rebuild them in fp64 so the comparison is not limited by them
     inv = 1.0 / (theta ** (torch.arange(0, dh, 2, dtype=torch.float64) / dh))
     model.rotary_emb.inv_freq = inv
@@ -162,6 +160,7 @@ def test_decoder_backbone_with_lora_matches_hf_llama_with_merged_weights():
     with torch.no_grad():
         model.embed_tokens.weight.copy_(_t(W["embed.table"]))
         model.norm.weight.copy_(_t(W["final.g"]))
+        lm.lm_head.weight.copy_(_t(W["lm_head.W"]))
         for l, layer in enumerate(model.layers):
             layer.self_attn.q_proj.weight.copy_(merged(l, "q")); layer.self_attn.k_proj.weight.copy_(merged(l, "k"))
             layer.self_attn.v_proj.weight.copy_(merged(l, "v")); layer.self_attn.o_proj.weight.copy_(merged(l, "o"))
@@ -169,6 +168,19 @@ def test_decoder_backbone_with_lora_matches_hf_llama_with_merged_weights():
             layer.mlp.down_proj.weight.copy_(merged(l, "down"))
             layer.input_layernorm.weight.copy_(_t(W[f"L{l:02d}.norm1.g"]))
             layer.post_attention_layernorm.weight.copy_(_t(W[f"L{l:02d}.norm2.g"]))
+    return bb, W, task, lm, r
+
+
+def test_decoder_backbone_with_lora_matches_hf_llama_with_merged_weights():
+    tr = pytest.importorskip("transformers")
+    bb, W, task, lm, r = _llama_fixture(tr)
+    model, eps, n = lm.model, bb["norm_eps"], 23
+    toks = r.integers(0, W["embed.table"].shape[0], size=n)
+    h = O.tokens_from_input(bb, W.__getitem__, toks)
+    for l in range(bb["n_layers"]):
+        h = O.layer_forward(bb, W.__getitem__, task, l, h)
+    got = O.rms_norm(h, W["final.g"], eps)                      # what head_forward pools from
+    with torch.no_grad():
         out = model(input_ids=torch.from_numpy(np.asarray(toks, dtype=np.int64))[None]).last_hidden_state[0].numpy()
     # LlamaRotaryEmbedding evaluates cos / sin in fp32 whatever the model dtype, which bounds the agreement at ~1e-6 relative
     # per rotation (measured here: 5e-6 absolute on outputs of magnitude 3); any structural mistake is O(0.1 .. 1).
@@ -179,6 +191,43 @@ def test_decoder_backbone_with_lora_matches_hf_llama_with_merged_weights():
         model.layers[0].self_attn.q_proj.weight.copy_(_t(W["L00.Wq"]))
         out2 = model(input_ids=torch.from_numpy(np.asarray(toks, dtype=np.int64))[None]).last_hidden_state[0].numpy()
     assert np.abs(got - out2).max() > 1e-3
+
+
+def test_token_decode_matches_hf_llama_incremental_decoding_with_a_kv_cache():
+    """oracle.decode recomputes the whole prefix for every new token - the definition.  transformers'
+    LlamaForCausalLM decodes INCREMENTALLY: the prompt once, then one token per call against its key / value cache
+    (`past_key_values`).  Both must give the same next-token scores at every step and the same greedy continuation: this
+    pins the definition and, independently, the claim that a KV cache does not change it."""
+    tr = pytest.importorskip("transformers")
+    from oracle import decode as D
+    bb, W, task, lm, r = _llama_fixture(tr)
+    vocab = W["embed.table"].shape[0]
+    prompt = r.integers(0, vocab, size=9)
+    n_new = 7
+    toks, scores = D.greedy_decode(bb, W.__getitem__, task, prompt, n_new)
+    with torch.no_grad():
+        out = lm(input_ids=torch.from_numpy(np.asarray(prompt, dtype=np.int64))[None], use_cache=True)
+        past, hf_scores, hf_toks = out.past_key_values, [out.logits[0, -1].numpy()], []
+        for s in range(n_new):
+            nxt = int(np.argmax(hf_scores[-1]))
+            hf_toks.append(nxt)
+            if s + 1 < n_new:
+                out = lm(input_ids=torch.tensor([[nxt]]), past_key_values=past, use_cache=True)
+                past = out.past_key_values
+                hf_scores.append(out.logits[0, -1].numpy())
+    assert toks == hf_toks, f"greedy continuation differs: {toks} vs {hf_toks}"
+    for s, (a, b) in enumerate(zip(scores, hf_scores)):
+        err = np.abs(a - b).max()
+        assert err < 5e-5 * max(1.0, np.abs(b).max()), f"step {s}: oracle vs incremental HF decode: max abs {err:.3e}"
+    # the scores of a step are the LM head on the last row of the plain forward over the prefix (the definition, re-stated
+    # with the forward's own pieces) and they DO depend on the adapters
+    seq = list(prompt) + toks[:3]
+    h = O.tokens_from_input(bb, W.__getitem__, np.asarray(seq))
+    for l in range(bb["n_layers"]):
+        h = O.layer_forward(bb, W.__getitem__, task, l, h)
+    assert np.allclose(scores[3], W["lm_head.W"] @ O.rms_norm(h, W["final.g"], bb["norm_eps"])[-1], rtol=1e-12, atol=1e-12)
+    no_adapter = dict(task, adapters={})
+    assert np.abs(D.lm_scores(bb, W.__getitem__, no_adapter, seq) - scores[3]).max() > 1e-2
 
 
 # ---------------------------------------------------------------- image patch embedding vs nn.Conv2d (the ViT formulation)
