@@ -54,7 +54,7 @@ class BfqParams(C.Structure):
     _fields_ = [("n_tasks", C.c_int32), ("b_max", C.c_int32), ("lat_ms", C.POINTER(C.c_double)), ("l_tok_ms", C.c_double)]
 
 
-OPTIONS = {"attention_impl": 0, "attention_variant": 1, "pdl": 2, "shrink_stages": 3, "half_tiles": 4, "attn_short": 5, "rope_fused": 6, "head_tiled": 7, "shrink_fused": 8, "graph": 9, "reverse": 10, "expand_wide": 11, "deep_pipe": 12}
+OPTIONS = {"attention_impl": 0, "pdl": 2, "shrink_stages": 3, "half_tiles": 4, "attn_short": 5, "rope_fused": 6, "head_tiled": 7, "shrink_fused": 8, "graph": 9, "reverse": 10, "expand_wide": 11, "deep_pipe": 12}
 
 
 class FmxError(RuntimeError):
@@ -288,7 +288,7 @@ class Fmx:
                                             n_kv_heads, head_dim, int(causal), impl, stream or None))
 
     def set_option(self, option, value):
-        """option: 'attention_impl' (0 auto, 1 mma.sync, 2 tcgen05, 3 lanes), 'attention_variant', 'pdl' (0/1)."""
+        """option: a key of OPTIONS (csrc/fmx_internal.h), e.g. 'attention_impl' (0 auto, 1 mma.sync, 2 tcgen05), 'pdl' (0 / 1 / 2)."""
         _check(self.lib.fmx_set_option(self.h, OPTIONS[option], int(value)))
 
 

@@ -30,19 +30,55 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#include "attention_lanes.cuh"
 #include "ptx.cuh"
 
 namespace fmx {
 
+constexpr int kAtBQ = 128;       // queries per q-tile (TMEM lanes)
+constexpr int kAtBKV = 64;       // keys per KV tile
 constexpr int kFaThreads = 192;
 constexpr int kFaStages = 2;     // K / V ring depth
+
+struct AttnTcArgs {
+  CUtensorMap qkv_map;           // [N, d_qkv] bf16, box {64 columns, 64 rows}, 128B swizzle
+  __nv_bfloat16 *out;
+  const int *cu_tok;
+  int ld_out;
+  int n_q_heads, n_kv_heads;
+  int causal;
+  float scale_log2;              // log2(e) / sqrt(d_h)
+  int reverse;                   // 1: requests are walked from the last to the first (blockIdx.z reversed)
+};
 
 template <int DH>
 __host__ __device__ constexpr int attn_fa_tile_bytes() { return (DH / 64) * (16384 + 2 * kFaStages * 8192); }
 template <int DH>
 constexpr int attn_fa_smem_bytes() { return attn_fa_tile_bytes<DH>() + 1024; }
 
+// MN-major, 128B-swizzled B operand: [K rows of 128 bytes][64-column blocks lbo_bytes apart]
+__device__ __forceinline__ uint64_t make_smem_desc_sw128_mn(uint32_t smem_addr, uint32_t lbo_bytes) {
+  uint64_t d = 0;
+  d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);
+  d |= (uint64_t)(lbo_bytes >> 4) << 16;                 // next 64 MN elements
+  d |= (uint64_t)(1024u >> 4) << 32;                     // next 8 K rows
+  d |= (uint64_t)1 << 46;
+  d |= (uint64_t)2 << 61;
+  return d;
+}
+// D[tmem] (+)= A[tmem] * B[smem]^T : A = bf16 pairs in TMEM (lane = row, 32-bit column c = elements 2c, 2c+1)
+__device__ __forceinline__ void umma_bf16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}\n" ::"r"(d_tmem),
+      "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_st_32x8(uint32_t taddr, const uint32_t (&v)[8]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};\n" ::"r"(taddr), "r"(v[0]),
+               "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7])
+               : "memory");
+}
 __device__ __forceinline__ void tmem_st_32x16(uint32_t taddr, const uint32_t (&v)[16]) {
   asm volatile(
       "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};\n" ::"r"(taddr),

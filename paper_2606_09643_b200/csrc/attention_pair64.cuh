@@ -18,7 +18,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#include "attention_lanes.cuh"
+#include "attention_fa.cuh"
 #include "ptx.cuh"
 
 namespace fmx {

@@ -14,9 +14,7 @@
 #include <vector>
 
 #include "attention.cuh"
-#include "attention_lanes.cuh"
 #include "attention_pair64.cuh"
-#include "attention_tc.cuh"
 #include "attention_fa.cuh"
 #include "common.h"
 #include "fmx.h"
@@ -100,7 +98,7 @@ struct Opts {
   int reverse = 1;        // consecutive kernels of a layer walk the rows in alternating directions (L2 reuse)
   int attn_short = 2;     // 0: generic kernel, 1: pipelined mma.sync kernel, 2: tcgen05 head-pair kernel where it applies
   int graph = 1;
-  int attn_impl = FMX_ATTN_AUTO, attn_variant = 0;
+  int attn_impl = FMX_ATTN_AUTO;
 };
 
 // A launch target: the stream and whether the launch carries the programmatic-stream-serialization attribute.
@@ -426,69 +424,14 @@ bool attn_use_tc(int impl, int dh, int max_len) {
   if (impl == FMX_ATTN_AUTO) return max_len > 64;
   return impl != FMX_ATTN_MMA_SYNC;
 }
-bool attn_use_lanes(int impl, int dh, int max_len) {
-  if (dh != 64 && dh != 128) return false;
-  return impl == FMX_ATTN_LANES;
+// head_dim 64: four light CTAs per SM (single S buffer, two-pass softmax: 80 registers); head_dim 128: TMEM (2 x 64 + 128
+// columns) allows two CTAs per SM, which double-buffer S and keep a tile's 64 scores in registers.  Measured against the other
+// trades (profiles/r2_02): head_dim 64 one-pass at 3 CTAs per SM 5.2 vs 3.5 ms per cfg3 step; head_dim 128 two-pass 6.7 vs 6.4 ms.
+void launch_attention_tc(Strm s, int dh, int max_len, int n_heads, int B, const AttnTcArgs &a) {
+  dim3 grid((max_len + kAtBQ - 1) / kAtBQ, n_heads, B);
+  if (dh == 64) launch_k((attention_fa_kernel<64, 1, 4, false>), grid, kFaThreads, attn_fa_smem_bytes<64>(), s, a);
+  else launch_k((attention_fa_kernel<128, 2, 2, true>), grid, kFaThreads, attn_fa_smem_bytes<128>(), s, a);
 }
-template <int DH, int kLanes>
-void launch_attention_lanes_v(Strm s, int sm_count, int max_len, const AttnLaneArgs &a0) {
-  AttnLaneArgs a = a0;
-  a.n_qt_max = (max_len + kAtBQ - 1) / kAtBQ;
-  const long long items = (long long)a.n_qt_max * a.n_req * a.n_q_heads;
-  const int grid = (int)std::min<long long>(sm_count, (items + kLanes - 1) / kLanes);
-  launch_k((attention_lanes_kernel<DH, kLanes>), grid, attn_lanes_threads<kLanes>(), attn_lanes_smem_bytes<DH, kLanes>(), s, a);
-}
-void launch_attention_lanes(Strm s, int sm_count, int dh, int variant, int max_len, const AttnLaneArgs &a) {
-  if (dh == 64) {
-    if (variant == 0) launch_attention_lanes_v<64, 4>(s, sm_count, max_len, a);
-    else if (variant == 1) launch_attention_lanes_v<64, 2>(s, sm_count, max_len, a);
-    else launch_attention_lanes_v<64, 3>(s, sm_count, max_len, a);
-  } else {
-    launch_attention_lanes_v<128, 2>(s, sm_count, max_len, a);
-  }
-}
-template <int DH, int kQT, int kSt, int kMinB>
-void launch_attention_tc_v(Strm s, int max_len, int n_heads, int B, const AttnTcArgs &a) {
-  dim3 grid((max_len + kAtBQ * kQT - 1) / (kAtBQ * kQT), n_heads, B);
-  launch_k((attention_tc_kernel<DH, kQT, kSt, kMinB>), grid, attn_tc_threads<kQT>(), attn_tc_smem_bytes<DH, kQT, kSt>(), s, a);
-}
-void launch_attention_tc(Strm s, int dh, int variant, int max_len, int n_heads, int B, const AttnTcArgs &a) {
-  if (variant <= 1) {        // the light one-q-tile CTA (attention_fa.cuh); variant 1 = the other softmax register / occupancy trade
-    dim3 grid((max_len + kAtBQ - 1) / kAtBQ, n_heads, B);
-    if (dh == 64 && variant == 0) launch_k((attention_fa_kernel<64, 1, 4, false>), grid, kFaThreads, attn_fa_smem_bytes<64>(), s, a);
-    else if (dh == 64) launch_k((attention_fa_kernel<64, 1, 3, true>), grid, kFaThreads, attn_fa_smem_bytes<64>(), s, a);
-    else if (variant == 0) launch_k((attention_fa_kernel<128, 2, 2, true>), grid, kFaThreads, attn_fa_smem_bytes<128>(), s, a);
-    else launch_k((attention_fa_kernel<128, 2, 2, false>), grid, kFaThreads, attn_fa_smem_bytes<128>(), s, a);
-    return;
-  }
-  variant -= 2;
-  if (dh == 64) {
-    if (variant == 0) launch_attention_tc_v<64, 1, 3, 2>(s, max_len, n_heads, B, a);
-    else launch_attention_tc_v<64, 2, 3, 1>(s, max_len, n_heads, B, a);
-  } else {
-    if (variant == 0) launch_attention_tc_v<128, 1, 2, 2>(s, max_len, n_heads, B, a);
-    else launch_attention_tc_v<128, 2, 3, 1>(s, max_len, n_heads, B, a);
-  }
-}
-template <int DH, int kQT, int kSt, int kMinB>
-cudaError_t set_attn_tc_attr() {
-  cudaError_t e = cudaFuncSetAttribute(attention_tc_kernel<DH, kQT, kSt, kMinB>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_tc_smem_bytes<DH, kQT, kSt>());
-  // without this the driver sizes the L1/shared split for ONE block and a second CTA never becomes resident
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(attention_tc_kernel<DH, kQT, kSt, kMinB>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-  if (e == cudaSuccess && getenv("FMX_DEBUG")) {
-    int nb = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, attention_tc_kernel<DH, kQT, kSt, kMinB>, attn_tc_threads<kQT>(), attn_tc_smem_bytes<DH, kQT, kSt>());
-    cudaFuncAttributes fa{};
-    cudaFuncGetAttributes(&fa, attention_tc_kernel<DH, kQT, kSt, kMinB>);
-    cudaDeviceProp pr{};
-    cudaGetDeviceProperties(&pr, 0);
-    fprintf(stderr, "fmx: attention_tc<%d,%d,%d,%d>: %d B smem, %d CTA/SM; regs %d static %zu maxdyn %d carveout %d; SM smem %zu regs %d reserved %zu\n",
-            DH, kQT, kSt, kMinB, attn_tc_smem_bytes<DH, kQT, kSt>(), nb, fa.numRegs, fa.sharedSizeBytes, fa.maxDynamicSharedSizeBytes,
-            fa.preferredShmemCarveout, pr.sharedMemPerMultiprocessor, pr.regsPerMultiprocessor, pr.reservedSharedMemPerBlock);
-  }
-  return e;
-}
-
 template <int DH, int kSBuf, int kMinB, bool kOne>
 cudaError_t set_attn_fa_attr() {
   cudaError_t e = cudaFuncSetAttribute(attention_fa_kernel<DH, kSBuf, kMinB, kOne>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_fa_smem_bytes<DH>());
@@ -506,17 +449,7 @@ cudaError_t set_attn_fa_attr() {
 
 int set_kernel_attrs() {
   CU_OK((set_attn_fa_attr<64, 1, 4, false>()));
-  CU_OK((set_attn_fa_attr<64, 1, 3, true>()));
   CU_OK((set_attn_fa_attr<128, 2, 2, true>()));
-  CU_OK((set_attn_fa_attr<128, 2, 2, false>()));
-  CU_OK((set_attn_tc_attr<64, 1, 3, 2>()));
-  CU_OK((set_attn_tc_attr<64, 2, 3, 1>()));
-  CU_OK((set_attn_tc_attr<128, 1, 2, 2>()));
-  CU_OK((set_attn_tc_attr<128, 2, 3, 1>()));
-  CU_OK((cudaFuncSetAttribute(attention_lanes_kernel<64, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_lanes_smem_bytes<64, 4>())));
-  CU_OK((cudaFuncSetAttribute(attention_lanes_kernel<64, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_lanes_smem_bytes<64, 2>())));
-  CU_OK((cudaFuncSetAttribute(attention_lanes_kernel<64, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_lanes_smem_bytes<64, 3>())));
-  CU_OK((cudaFuncSetAttribute(attention_lanes_kernel<128, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_lanes_smem_bytes<128, 2>())));
   CU_OK((cudaFuncSetAttribute(pair_gemm_kernel<256, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<256, false>())));
   CU_OK((cudaFuncSetAttribute(pair_gemm_kernel<256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<256, true>())));
   CU_OK((cudaFuncSetAttribute(pair_gemm_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<128, false>())));
@@ -1329,17 +1262,12 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       pa2.n_q_heads = d.n_q_heads; pa2.n_kv_heads = d.n_kv_heads; pa2.causal = d.causal; pa2.scale_log2 = scale_log2;
       pa2.reverse = rev();
       LAUNCH(Lh, F_ATTN, launch_attention_pair64(S, c->sm_count, pa2));
-    } else if (attn_use_lanes(c->o.attn_impl, d.head_dim, max_len)) {
-      AttnLaneArgs la{};
-      la.qkv_map = mQKV64; la.out = w.AttnO; la.cu_tok = w.t.cu_tok; la.ld_out = bb.d_q; la.n_req = B;
-      la.n_q_heads = d.n_q_heads; la.n_kv_heads = d.n_kv_heads; la.causal = d.causal; la.scale_log2 = scale_log2;
-      LAUNCH(Lh, F_ATTN, launch_attention_lanes(S, c->sm_count, d.head_dim, c->o.attn_variant, max_len, la));
     } else if (attn_use_tc(c->o.attn_impl, d.head_dim, max_len)) {
       AttnTcArgs ta{};
       ta.qkv_map = mQKV64; ta.out = w.AttnO; ta.cu_tok = w.t.cu_tok; ta.ld_out = bb.d_q;
       ta.n_q_heads = d.n_q_heads; ta.n_kv_heads = d.n_kv_heads; ta.causal = d.causal; ta.scale_log2 = scale_log2;
       ta.reverse = rev();
-      LAUNCH(Lh, F_ATTN, launch_attention_tc(S, d.head_dim, c->o.attn_variant, max_len, d.n_q_heads, B, ta));
+      LAUNCH(Lh, F_ATTN, launch_attention_tc(S, d.head_dim, max_len, d.n_q_heads, B, ta));
     } else {
       AttnArgs aa{};
       aa.qkv = w.QKV; aa.out = w.AttnO; aa.cu_tok = w.t.cu_tok; aa.ld_qkv = bb.d_qkv; aa.ld_out = bb.d_q;
@@ -1696,18 +1624,12 @@ int fmx_debug_attention(fmx_ctx *c, const void *qkv, void *out, const int32_t *c
     pa2.out = (bf16 *)out; pa2.cu_tok = c->d_dbg_cu; pa2.ld_out = d_q; pa2.n_req = n_req; pa2.n_q_heads = n_q_heads; pa2.n_kv_heads = n_kv_heads;
     pa2.causal = causal; pa2.scale_log2 = scale_log2;
     launch_attention_pair64(Strm{s, 0}, c->sm_count, pa2);
-  } else if (attn_use_lanes(impl, head_dim, max_len)) {
-    AttnLaneArgs la{};
-    if (int e = encode_2d(c, &la.qkv_map, qkv, N, d_qkv, d_qkv, 64)) return e;
-    la.out = (bf16 *)out; la.cu_tok = c->d_dbg_cu; la.ld_out = d_q; la.n_req = n_req; la.n_q_heads = n_q_heads; la.n_kv_heads = n_kv_heads;
-    la.causal = causal; la.scale_log2 = scale_log2;
-    launch_attention_lanes(Strm{s, 0}, c->sm_count, head_dim, c->o.attn_variant, max_len, la);
   } else if (attn_use_tc(impl, head_dim, max_len)) {
     AttnTcArgs ta{};
     if (int e = encode_2d(c, &ta.qkv_map, qkv, N, d_qkv, d_qkv, 64)) return e;
     ta.out = (bf16 *)out; ta.cu_tok = c->d_dbg_cu; ta.ld_out = d_q; ta.n_q_heads = n_q_heads; ta.n_kv_heads = n_kv_heads;
     ta.causal = causal; ta.scale_log2 = scale_log2;
-    launch_attention_tc(Strm{s, 0}, head_dim, c->o.attn_variant, max_len, n_q_heads, n_req, ta);
+    launch_attention_tc(Strm{s, 0}, head_dim, max_len, n_q_heads, n_req, ta);
   } else {
     AttnArgs aa{};
     aa.qkv = (const bf16 *)qkv; aa.out = (bf16 *)out; aa.cu_tok = c->d_dbg_cu; aa.ld_qkv = d_qkv; aa.ld_out = d_q;
@@ -1726,7 +1648,7 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
   ++c->config_gen;                      // invalidates the cached forward graph
   switch (option) {
     case FMX_OPT_ATTENTION_IMPL:
-      if (value < FMX_ATTN_AUTO || value > FMX_ATTN_LANES) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attention impl %d", value);
+      if (value < FMX_ATTN_AUTO || value > FMX_ATTN_TCGEN05) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attention impl %d", value);
       c->o.attn_impl = value;
       return FMX_OK;
     case FMX_OPT_SHRINK_STAGES:
@@ -1766,10 +1688,6 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
     case FMX_OPT_PDL:
       if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: pdl %d", value);
       c->o.pdl = value;
-      return FMX_OK;
-    case FMX_OPT_ATTENTION_VARIANT:
-      if (value < 0 || value > 4) return fmx_fail(FMX_E_INVALID_ARG, "set_option: attention variant %d", value);
-      c->o.attn_variant = value;
       return FMX_OK;
   }
   return fmx_fail(FMX_E_INVALID_ARG, "set_option: unknown option %d", option);

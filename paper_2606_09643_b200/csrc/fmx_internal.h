@@ -37,9 +37,7 @@ int fmx_debug_attention(fmx_ctx *ctx, const void *qkv, void *out, const int32_t 
 
 /* Tuning knobs of one context (experiments; the defaults are what bench.py measures). */
 enum {
-  FMX_OPT_ATTENTION_IMPL = 0,    /* FMX_ATTN_AUTO | FMX_ATTN_MMA_SYNC | FMX_ATTN_TCGEN05 | FMX_ATTN_LANES */
-  FMX_OPT_ATTENTION_VARIANT = 1, /* tcgen05 attention: 0 = one 128-query tile per CTA; 1 = two q-tiles per CTA
-                                    sharing K/V.  FMX_ATTN_LANES: 0 / 1 / 2 = 4 / 2 / 3 lanes per CTA (head_dim 64) */
+  FMX_OPT_ATTENTION_IMPL = 0,    /* FMX_ATTN_AUTO | FMX_ATTN_MMA_SYNC | FMX_ATTN_TCGEN05 (head_dim 64 / 128 only) */
   FMX_OPT_SHRINK_STAGES = 3,     /* LoRA shrink kernel pipeline: 5 (default) = as deep as ~200 KB allow for the stage size
                                     (8 / 6 / 5 stages for 1 / 2 / 3 targets), 4 = four 40 KB stages */
   FMX_OPT_HALF_TILES = 4,        /* 1 (default): a short last GEMM wave is cut into 256 x 128 half tiles */
@@ -67,7 +65,7 @@ enum {
   FMX_OPT_PDL = 2                /* programmatic dependent launch of the forward's kernels:
                                     0 = off, 1 = always, 2 (default) = only for batches of <= 4096 token rows */
 };
-enum { FMX_ATTN_AUTO = 0, FMX_ATTN_MMA_SYNC = 1, FMX_ATTN_TCGEN05 = 2, FMX_ATTN_LANES = 3 };
+enum { FMX_ATTN_AUTO = 0, FMX_ATTN_MMA_SYNC = 1, FMX_ATTN_TCGEN05 = 2 };
 int fmx_set_option(fmx_ctx *ctx, int32_t option, int32_t value);
 
 #ifdef __cplusplus

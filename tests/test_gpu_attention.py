@@ -16,7 +16,7 @@ pytestmark = pytest.mark.gpu
 from fmx_workloads import bf16_bits_to_f64, f32_to_bf16_bits  # noqa: E402
 from oracle.vfm_forward import attention  # noqa: E402
 
-MMA_SYNC, TCGEN05, LANES = 1, 2, 3
+MMA_SYNC, TCGEN05 = 1, 2
 
 
 @pytest.fixture(scope="module")
@@ -73,51 +73,28 @@ CASES = [
 ]
 
 
-@pytest.mark.parametrize("variant", [0, 1])       # 0: one q-tile per CTA, two CTAs per SM; 1: two q-tiles per CTA
-@pytest.mark.parametrize("lengths,hq,hkv,dh,causal", CASES)
-def test_tcgen05_attention_matches_oracle(fmx, lengths, hq, hkv, dh, causal, variant):
-    fmx.set_option("attention_variant", variant)
-    try:
-        run_case(fmx, lengths, hq, hkv, dh, causal, TCGEN05, seed=len(lengths) * 131 + dh)
-    finally:
-        fmx.set_option("attention_variant", 0)
+MORE_CASES = [
+    ([17] * 40 + [257] * 9,           16, 16, 64, 0),    # many short requests next to cfg3-like ones: CTAs that exit at once
+    ([130, 66, 80, 129, 193, 16, 15], 2, 2, 128, 0),     # head_dim 128 with last KV tiles of 2, 2, 16, 1, 1 keys (N = 16 tail MMA)
+    ([200, 72],                       12, 2, 128, 1),    # causal tail: keys 192..199 visible to the last rows only
+    ([513, 1000],                     4, 2, 64, 1),      # head_dim 64 causal, 9 and 16 KV tiles (single S buffer)
+]
+
+
+@pytest.mark.parametrize("lengths,hq,hkv,dh,causal", CASES + MORE_CASES)
+def test_tcgen05_attention_matches_oracle(fmx, lengths, hq, hkv, dh, causal):
+    run_case(fmx, lengths, hq, hkv, dh, causal, TCGEN05, seed=len(lengths) * 131 + dh)
 
 
 @pytest.mark.parametrize("lengths,hq,hkv,dh,causal", [
     ([300, 700], 2, 2, 64, 0),
     ([1024, 90], 6, 1, 128, 1),
+    ([257, 130], 2, 2, 128, 0),                          # rescale with a fast 16-key tail tile running ahead (double-buffered S)
 ])
-@pytest.mark.parametrize("variant", [0, 1])
-def test_tcgen05_attention_large_scores_rescale_path(fmx, lengths, hq, hkv, dh, causal, variant):
+def test_tcgen05_attention_large_scores_rescale_path(fmx, lengths, hq, hkv, dh, causal):
     """Scores of magnitude ~10^2 in the log2 domain with the largest ones late in the sequence: the
     lazily updated reference maximum must move (more than once) and O in TMEM must be rescaled."""
-    fmx.set_option("attention_variant", variant)
-    try:
-        run_case(fmx, lengths, hq, hkv, dh, causal, TCGEN05, seed=7, q_scale=6.0, ramp=3.0)
-    finally:
-        fmx.set_option("attention_variant", 0)
-
-
-@pytest.mark.parametrize("variant", [0, 1, 2])    # 4, 2, 3 lanes per CTA (head_dim 128: always 2)
-@pytest.mark.parametrize("lengths,hq,hkv,dh,causal", CASES + [([17] * 40 + [257] * 9, 16, 16, 64, 0)])
-def test_lanes_attention_matches_oracle(fmx, lengths, hq, hkv, dh, causal, variant):
-    """Persistent multi-lane tcgen05 kernel (P kept in TMEM, 16-key tail tile): more work items than lanes, so every
-    lane walks several items and the Q / K / V rings wrap."""
-    if dh == 128 and variant > 0:
-        pytest.skip("head_dim 128 has one lane count")
-    fmx.set_option("attention_variant", variant)
-    try:
-        run_case(fmx, lengths, hq, hkv, dh, causal, LANES, seed=len(lengths) * 17 + dh)
-    finally:
-        fmx.set_option("attention_variant", 0)
-
-
-@pytest.mark.parametrize("lengths,hq,hkv,dh,causal", [
-    ([300, 700], 2, 2, 64, 0),
-    ([1024, 90], 6, 1, 128, 1),
-])
-def test_lanes_attention_large_scores_rescale_path(fmx, lengths, hq, hkv, dh, causal):
-    run_case(fmx, lengths, hq, hkv, dh, causal, LANES, seed=7, q_scale=6.0, ramp=3.0)
+    run_case(fmx, lengths, hq, hkv, dh, causal, TCGEN05, seed=7, q_scale=6.0, ramp=3.0)
 
 
 @pytest.mark.parametrize("lengths,hq,hkv,dh,causal", [
