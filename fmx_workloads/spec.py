@@ -140,6 +140,8 @@ class Workload:
                 return (bb.tokens_per_request, bb.d_model), bb.pos_kind, bb.std
             if what == "table":
                 return (bb.vocab, bb.d_model), "normal", bb.std_embed
+        if parts[0] == "lm_head":          # NEXT-3: untied language-model head [vocab, d_model] (reading 34)
+            return (bb.vocab, bb.d_model), "normal", 0.02
         if parts[0] == "final":
             return (bb.d_model,), ("gain" if parts[1] == "g" else "normal"), bb.std
         if parts[0].startswith("L") and len(parts[0]) == 3:

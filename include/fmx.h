@@ -206,6 +206,45 @@ int fmx_forward_mixed_host(fmx_ctx *ctx, fmx_backbone_t bb, const void *inputs_h
                            const int32_t *task_ids, const int32_t *lengths, int32_t n_req,
                            float *outputs_host, void *workspace, size_t workspace_bytes, void *cuda_stream);
 
+/* ---- token decode with a key / value cache ---------------------------------------------------
+ * The paper serves "token-based FMs (e.g., LLMs with continuous batching and long-lived decode iterations)" through the
+ * same vFM boundary (fourth difference) and charges "token-level work in service-time units" (L168).  What a
+ * decode iteration computes (the paper gives no arithmetic; reading 34): the next-token scores of a request that
+ * has seen x_0 .. x_{n-1} are  lm_head · FinalNorm(Backbone_t(x_0 .. x_{n-1}))[n-1]  with its task's adapters - the last row
+ * of the ordinary causal forward over the whole prefix.  The cache stores every layer's k / v rows (after RoPE) so that a
+ * step feeds ONE new token per request; it must not change the value (tests compare with the no-cache definition).
+ * Requests of different tasks decode in one batch (task-sorted rows, segmented LoRA as in fmx_forward_mixed), and the batch
+ * may change from step to step (continuous batching): a step names, per request, its task, its cache slot and how many
+ * tokens the slot already holds.
+ *
+ * kv_cache: DEVICE, caller-owned, fmx_kv_cache_bytes(n_slots) bytes, 16-byte aligned; layout
+ * [slot][layer][k | v][max_seq][n_kv_heads * head_dim] bf16.  The library keeps no per-slot state: `positions` is the
+ * caller's.  Causal backbones only (FMX_E_SHAPE otherwise). */
+
+/* The language-model head of a backbone: W DEVICE bf16 [vocab, d_model], caller-owned (not copied), vocab a multiple of
+ * 128.  Register it BEFORE sizing workspaces: fmx_workspace_bytes then includes the [max_req, vocab] fp32 score buffer. */
+int fmx_register_lm_head(fmx_ctx *ctx, fmx_backbone_t bb, const void *W, int32_t vocab);
+int fmx_kv_cache_bytes(fmx_ctx *ctx, fmx_backbone_t bb, int32_t n_slots, size_t *bytes);
+
+/* Prefill: fmx_forward_mixed that also writes every request's k / v rows into cache slot slots[i] (positions 0 .. n_i - 1).
+ *   slots        HOST int32 [n_req], distinct, each in [0, n_slots)
+ *   outputs      DEVICE fp32 task-head outputs as fmx_forward_mixed, or NULL to skip the heads
+ *   scores       DEVICE fp32 [n_req, vocab] next-token scores in ORIGINAL request order, or NULL
+ *   next_tokens  DEVICE int32 [n_req] greedy next token (argmax, lowest index on ties), or NULL
+ * Asynchronous on cuda_stream; never replayed from the graph cache. */
+int fmx_prefill(fmx_ctx *ctx, fmx_backbone_t bb, const void *inputs, const int32_t *task_ids, const int32_t *lengths,
+                const int32_t *slots, int32_t n_req, float *outputs, float *scores, int32_t *next_tokens, void *kv_cache,
+                int32_t n_slots, void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* One decode iteration: request i appends token tokens[i] at position positions[i] of its slot (the slot must hold exactly
+ * positions[i] tokens, < max_seq) and receives the scores / greedy choice of the NEXT token.
+ *   tokens     DEVICE int32 [n_req] (e.g. the next_tokens buffer of the previous call), TOKEN_IDS backbones only
+ *   positions  HOST int32 [n_req]
+ * workspace: >= fmx_workspace_bytes(n_req, n_req tokens). */
+int fmx_decode_step(fmx_ctx *ctx, fmx_backbone_t bb, const int32_t *tokens, const int32_t *task_ids, const int32_t *slots,
+                    const int32_t *positions, int32_t n_req, float *scores, int32_t *next_tokens, void *kv_cache,
+                    int32_t n_slots, void *workspace, size_t workspace_bytes, void *cuda_stream);
+
 /* Debug/test: copies the segment tables of the LAST forward to HOST arrays (synchronises).
  * Sizes: perm, inv_perm [n_req]; task_req_off, task_tok_off [n_slots+1]; cu_tok [n_req+1];
  * n_slots = fmx_task_slots().  Any pointer may be NULL. */

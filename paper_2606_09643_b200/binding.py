@@ -68,7 +68,7 @@ _lib = None
 # include/fmx.h (the public C ABI)
 EXPORTS = ["fmx_create", "fmx_destroy", "fmx_last_error", "fmx_version", "fmx_poll_error", "fmx_register_backbone", "fmx_register_task",
            "fmx_unregister_task", "fmx_output_layout", "fmx_workspace_bytes", "fmx_host_workspace_bytes", "fmx_forward_mixed",
-           "fmx_forward_mixed_host", "fmx_debug_get_segments", "fmx_task_slots", "fmx_profile_enable", "fmx_profile_select",
+           "fmx_forward_mixed_host", "fmx_register_lm_head", "fmx_kv_cache_bytes", "fmx_prefill", "fmx_decode_step", "fmx_debug_get_segments", "fmx_task_slots", "fmx_profile_enable", "fmx_profile_select",
            "fmx_profile_read", "fmx_profile_family_name", "fmx_last_launch_count", "fmx_bfq_create", "fmx_bfq_destroy",
            "fmx_bfq_set_task", "fmx_bfq_enqueue", "fmx_bfq_next_batch", "fmx_bfq_complete", "fmx_bfq_stats", "fmx_bfq_peek"]
 # csrc/fmx_internal.h (test hooks and tuning knobs; not part of the ABI)
@@ -100,6 +100,10 @@ def load():
     lib.fmx_poll_error.argtypes = [_vp]
     lib.fmx_forward_mixed.argtypes = [_vp, C.c_int32, _vp, i32p, i32p, C.c_int32, _vp, _vp, C.c_size_t, _vp]
     lib.fmx_forward_mixed_host.argtypes = [_vp, C.c_int32, _vp, C.c_size_t, i32p, i32p, C.c_int32, _vp, _vp, C.c_size_t, _vp]
+    lib.fmx_register_lm_head.argtypes = [_vp, C.c_int32, _vp, C.c_int32]
+    lib.fmx_kv_cache_bytes.argtypes = [_vp, C.c_int32, C.c_int32, C.POINTER(C.c_size_t)]
+    lib.fmx_prefill.argtypes = [_vp, C.c_int32, _vp, i32p, i32p, i32p, C.c_int32, _vp, _vp, _vp, _vp, C.c_int32, _vp, C.c_size_t, _vp]
+    lib.fmx_decode_step.argtypes = [_vp, C.c_int32, _vp, i32p, i32p, i32p, C.c_int32, _vp, _vp, _vp, C.c_int32, _vp, C.c_size_t, _vp]
     lib.fmx_debug_get_segments.argtypes = [_vp, i32p, i32p, i32p, i32p, i32p]
     lib.fmx_debug_get_tiles.argtypes = [_vp, i32p, i32p, i32p, C.c_int32]
     lib.fmx_task_slots.argtypes = [_vp]
@@ -235,6 +239,26 @@ class Fmx:
         _check(self.lib.fmx_forward_mixed_host(self.h, bb, inputs_host, inputs_bytes, ids.ctypes.data_as(p),
                                                lens.ctypes.data_as(p), len(ids), outputs_host, workspace,
                                                workspace_bytes, stream or None))
+
+    def register_lm_head(self, bb, W, vocab):
+        _check(self.lib.fmx_register_lm_head(self.h, bb, W, vocab))
+
+    def kv_cache_bytes(self, bb, n_slots):
+        out = C.c_size_t(0)
+        _check(self.lib.fmx_kv_cache_bytes(self.h, bb, n_slots, C.byref(out)))
+        return out.value
+
+    def prefill(self, bb, inputs, task_ids, lengths, slots, outputs, scores, next_tokens, kv_cache, n_slots, workspace, workspace_bytes, stream=0):
+        ids, lens, sl = _i32(task_ids), _i32(lengths), _i32(slots)
+        p = C.POINTER(C.c_int32)
+        _check(self.lib.fmx_prefill(self.h, bb, inputs, ids.ctypes.data_as(p), lens.ctypes.data_as(p), sl.ctypes.data_as(p), len(ids),
+                                    outputs or None, scores or None, next_tokens or None, kv_cache, n_slots, workspace, workspace_bytes, stream or None))
+
+    def decode_step(self, bb, tokens, task_ids, slots, positions, scores, next_tokens, kv_cache, n_slots, workspace, workspace_bytes, stream=0):
+        ids, sl, pos = _i32(task_ids), _i32(slots), _i32(positions)
+        p = C.POINTER(C.c_int32)
+        _check(self.lib.fmx_decode_step(self.h, bb, tokens, ids.ctypes.data_as(p), sl.ctypes.data_as(p), pos.ctypes.data_as(p), len(ids),
+                                        scores or None, next_tokens or None, kv_cache, n_slots, workspace, workspace_bytes, stream or None))
 
     def debug_get_segments(self, n_req):
         T = self.task_slots()

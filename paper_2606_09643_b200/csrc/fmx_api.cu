@@ -71,6 +71,10 @@ struct Backbone {
   // weight maps, [0] = box {64,128} (pair tile 256x256: one CTA loads a whole chunk), [1] = box {64,64} (256x128 tiles)
   std::vector<CUtensorMap> mWq[2], mWk[2], mWv[2], mWo[2], mWup[2], mWgate[2], mWdown[2];
   CUtensorMap mEmbedW[2];
+  // language-model head for token decode (NEXT-3): caller-owned bf16 [lm_vocab, d_model]
+  const bf16 *lm_head = nullptr;
+  int lm_vocab = 0;
+  CUtensorMap mLm[2];
   // LoRA slabs
   int Rcap = 0;
   std::vector<unsigned char> col_used;     // units of 16 columns
@@ -133,7 +137,7 @@ struct fmx_ctx {
   const bf16 **d_task_enc_W = nullptr, **d_task_enc_b = nullptr;
   // pinned staging for ids / lengths: a ring (a slot is rewritten only after the copy that read it has run)
   static constexpr int kStageSlots = 4;
-  int *h_stage = nullptr;                  // [kStageSlots + 1][2 * FMX_MAX_REQUESTS]
+  int *h_stage = nullptr;                  // [kStageSlots][4 * FMX_MAX_REQUESTS]: ids, lengths, cache slots, cache positions
   cudaEvent_t stage_ev[kStageSlots] = {nullptr, nullptr, nullptr, nullptr};
   bool stage_used[kStageSlots] = {false, false, false, false};
   int stage_next = 0;
@@ -225,6 +229,10 @@ struct Workspace {
   float *head_hid = nullptr;             // hidden activations of MLP heads [B, kMaxHeadHidden]
   float *head_part = nullptr;            // K-chunk partials of the tensor-core FLATTEN head: kHeadPartFloats per request
   size_t head_part_floats = 0;
+  // token decode (NEXT-3): cache slot / position per request (original order) and per token row; LM-head operands
+  int *slots = nullptr, *pos0 = nullptr, *row_slot = nullptr, *row_cpos = nullptr;
+  bf16 *Fl = nullptr;                    // [B, d] final-normed last rows, sorted request order
+  float *lm_scores = nullptr;            // [B, lm_vocab] sorted request order
   int n_tiles = 0, n_blk_cap = 0;
   size_t bytes = 0;
 };
@@ -271,6 +279,14 @@ Workspace carve(const Backbone &bb, void *base, int B, long long N, int T) {
   w.head_hid = (float *)take(sizeof(float) * (size_t)B * kMaxHeadHidden);
   w.head_part_floats = (size_t)((B + 15) / 16) * 16 * kHeadPartFloats;
   w.head_part = (float *)take(sizeof(float) * w.head_part_floats);
+  w.slots = (int *)take(sizeof(int) * B);
+  w.pos0 = (int *)take(sizeof(int) * B);
+  w.row_slot = (int *)take(sizeof(int) * N);
+  w.row_cpos = (int *)take(sizeof(int) * N);
+  if (bb.lm_head) {
+    w.Fl = (bf16 *)take(sizeof(bf16) * (size_t)B * d.d_model);
+    w.lm_scores = (float *)take(sizeof(float) * (size_t)B * bb.lm_vocab);
+  }
   w.bytes = off;
   return w;
 }
@@ -698,7 +714,7 @@ int fmx_create(fmx_ctx **out, int device_ordinal) {
   CU_OK(cudaMemset(c->d_task_enc_ch, 0, sizeof(int) * FMX_MAX_TASKS));
   CU_OK(cudaMemset(c->d_task_enc_W, 0, sizeof(void *) * FMX_MAX_TASKS));
   CU_OK(cudaMemset(c->d_task_enc_b, 0, sizeof(void *) * FMX_MAX_TASKS));
-  CU_OK(cudaMallocHost(&c->h_stage, sizeof(int) * 2 * FMX_MAX_REQUESTS * (fmx_ctx::kStageSlots + 1)));
+  CU_OK(cudaMallocHost(&c->h_stage, sizeof(int) * 4 * FMX_MAX_REQUESTS * fmx_ctx::kStageSlots));
   for (int i = 0; i < fmx_ctx::kStageSlots; ++i) CU_OK(cudaEventCreateWithFlags(&c->stage_ev[i], cudaEventDisableTiming));
   CU_OK(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
   CU_OK(cudaStreamCreateWithFlags(&c->side2, cudaStreamNonBlocking));
@@ -1071,25 +1087,46 @@ static int batch_shape(fmx_ctx *c, const Backbone &bb, const int32_t *task_ids, 
 
 // ids / lengths -> the device tables, through the pinned staging ring (a slot is rewritten only after the copy that read it
 // has run).  Never part of a captured graph: a replay serves a NEW batch, so these copies are enqueued before every launch.
-static int stage_ids(fmx_ctx *c, const Workspace &w, const int32_t *task_ids, const int32_t *lengths, int32_t B, cudaStream_t s) {
+static int stage_ids(fmx_ctx *c, const Workspace &w, const int32_t *task_ids, const int32_t *lengths, int32_t B, cudaStream_t s,
+                     const int32_t *slots = nullptr, const int32_t *pos0 = nullptr) {
   const int slot = c->stage_next;
   c->stage_next = (c->stage_next + 1) % fmx_ctx::kStageSlots;
   if (c->stage_used[slot]) CU_OK(cudaEventSynchronize(c->stage_ev[slot]));
-  int *stage = c->h_stage + (size_t)slot * 2 * FMX_MAX_REQUESTS;
+  int *stage = c->h_stage + (size_t)slot * 4 * FMX_MAX_REQUESTS;
   memcpy(stage, task_ids, sizeof(int) * B);
   memcpy(stage + FMX_MAX_REQUESTS, lengths, sizeof(int) * B);
   CU_OK(cudaMemcpyAsync(w.t.task_ids, stage, sizeof(int) * B, cudaMemcpyHostToDevice, s));
   CU_OK(cudaMemcpyAsync(w.t.lengths, stage + FMX_MAX_REQUESTS, sizeof(int) * B, cudaMemcpyHostToDevice, s));
+  if (slots) {
+    memcpy(stage + 2 * FMX_MAX_REQUESTS, slots, sizeof(int) * B);
+    CU_OK(cudaMemcpyAsync(w.slots, stage + 2 * FMX_MAX_REQUESTS, sizeof(int) * B, cudaMemcpyHostToDevice, s));
+  }
+  if (pos0) {
+    memcpy(stage + 3 * FMX_MAX_REQUESTS, pos0, sizeof(int) * B);
+    CU_OK(cudaMemcpyAsync(w.pos0, stage + 3 * FMX_MAX_REQUESTS, sizeof(int) * B, cudaMemcpyHostToDevice, s));
+  }
   CU_OK(cudaEventRecord(c->stage_ev[slot], s));
   c->stage_used[slot] = true;
   return FMX_OK;
 }
 
+// A forward that also maintains a key / value cache (NEXT-3): prefill writes every request's k / v rows into its slot,
+// a decode step appends ONE token per request and attends the cached positions.
+struct KvCall {
+  bf16 *cache = nullptr;
+  int n_slots = 0;
+  const int32_t *slots = nullptr;        // HOST [B]
+  const int32_t *pos0 = nullptr;         // HOST [B] tokens already cached per request (decode); NULL = prefill from 0
+  float *scores = nullptr;               // DEVICE fp32 [B, lm_vocab] or NULL
+  int32_t *next_tokens = nullptr;        // DEVICE int32 [B] or NULL
+  bool decode = false;
+};
+
 // graph_capture: the stream is being captured into the context's cached graph: ids / lengths go through the graph's own
 // pinned buffer and no event is recorded.
 static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int32_t *task_ids, const int32_t *lengths,
                         int32_t B, float *outputs, void *workspace, size_t workspace_bytes, cudaStream_t s, const BatchShape &bs,
-                        bool graph_capture = false) {
+                        bool graph_capture = false, const KvCall *kv = nullptr) {
   const fmx_backbone_desc &d = bb.d;
   const long long N = bs.N;
   const int max_len = bs.max_len, max_out = bs.max_out;
@@ -1114,7 +1151,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     CU_OK(cudaStreamIsCapturing(s, &cap_status));
     if (cap_status != cudaStreamCaptureStatusNone)
       return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed: the stream is being captured; capture is not supported (the library caches its own CUDA graph)");
-    if (int e = stage_ids(c, w, task_ids, lengths, B, s)) return e;
+    if (int e = stage_ids(c, w, task_ids, lengths, B, s, kv ? kv->slots : nullptr, kv ? kv->pos0 : nullptr)) return e;
   }
   SortArgs sa{};
   sa.t = w.t; sa.B = B; sa.T = T; sa.n_tiles = w.n_tiles; sa.tile_rows = kPairRows; sa.task_head_out = c->d_task_head_out;
@@ -1125,6 +1162,15 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   else { sa.in_per_tok = 0; sa.in_per_req = (long long)(d.tokens_per_request - (d.has_cls ? 1 : 0)) * d.patch_dim; }
   LAUNCH(Lh, F_SORT, (launch_k(task_sort_kernel, 1, kSortThreads, 0, S, sa)));
   LAUNCH(Lh, F_SORT, (launch_k(row_tables_kernel, (Ni + 255) / 256, 256, 0, S, w.t.cu_tok, B, Ni, w.t.row_req, w.t.row_pos)));
+  KvArgs ka{};
+  if (kv) {
+    ka.cache = kv->cache; ka.d_kv = bb.d_kv; ka.max_seq = d.max_seq;
+    ka.kv_stride = (long long)d.max_seq * bb.d_kv; ka.layer_stride = 2 * ka.kv_stride; ka.slot_stride = (long long)d.n_layers * ka.layer_stride;
+    ka.row_slot = w.row_slot; ka.row_cpos = w.row_cpos;
+    LAUNCH(Lh, F_SORT, (launch_k(kv_rows_kernel, (Ni + 255) / 256, 256, 0, S, (const int *)w.t.row_req, (const int *)w.t.row_pos, (const int *)w.t.perm,
+                                 (const int *)w.slots, kv->pos0 ? (const int *)w.pos0 : (const int *)nullptr, Ni, w.row_slot, w.row_cpos)));
+  }
+  const int *rope_pos = kv ? w.row_cpos : w.t.row_pos;        // RoPE position of a row = its position in the request's WHOLE sequence
 
   // ---- common GEMM parameter pieces ----
   GemmParams sbase{};                       // segmented shrink
@@ -1247,16 +1293,23 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       p.omap = oQKV;
       // head_dim 128: a 128-column chunk is one head, so RoPE is applied in the GEMM epilogue (fp32, one rounding)
       rope_fused = c->o.rope_fused && d.rope_theta > 0 && d.head_dim == 128 && pair_wide(p);
-      if (rope_fused) { p.rope_cs = bb.rope_cs_t; p.rope_ld = d.max_seq; p.rope_src_mask = 3; }
+      if (rope_fused) { p.rope_cs = bb.rope_cs_t; p.rope_ld = d.max_seq; p.rope_src_mask = 3; p.row_pos = rope_pos; }
       p.reverse = rev();
       LAUNCH(Lh, F_GEMM_QKV, launch_pair_gemm(c, S, p));
     }
     if (d.rope_theta > 0 && !rope_fused) {
       const int nh = d.n_q_heads + d.n_kv_heads;
       const long long total = (long long)Ni * nh * (d.head_dim / 16);
-      LAUNCH(Lh, F_ROPE, (launch_k(rope_kernel, (unsigned)((total + 255) / 256), 256, 0, S, w.QKV, bb.d_qkv, w.t.row_pos, bb.rope_cs, Ni, nh, d.head_dim)));
+      LAUNCH(Lh, F_ROPE, (launch_k(rope_kernel, (unsigned)((total + 255) / 256), 256, 0, S, w.QKV, bb.d_qkv, rope_pos, bb.rope_cs, Ni, nh, d.head_dim)));
     }
-    if (c->o.attn_impl == FMX_ATTN_AUTO && attn_pair64_ok(c->o, d.head_dim, d.n_q_heads, max_len)) {
+    if (kv) LAUNCH(Lh, F_ATTN, (launch_k(kv_append_kernel, (Ni + 7) / 8, 256, 0, S, (const bf16 *)w.QKV, bb.d_qkv, bb.d_q, bb.d_q + bb.d_kv, Ni, l, ka)));
+    if (kv && kv->decode) {
+      dim3 grid(B, d.n_kv_heads);
+      if (d.head_dim == 32) LAUNCH(Lh, F_ATTN, (launch_k(decode_attention_kernel<32>, grid, 256, 0, S, (const bf16 *)w.QKV, bb.d_qkv, w.AttnO, bb.d_q, d.n_q_heads, d.n_kv_heads, scale_log2, l, ka)));
+      else if (d.head_dim == 64) LAUNCH(Lh, F_ATTN, (launch_k(decode_attention_kernel<64>, grid, 256, 0, S, (const bf16 *)w.QKV, bb.d_qkv, w.AttnO, bb.d_q, d.n_q_heads, d.n_kv_heads, scale_log2, l, ka)));
+      else LAUNCH(Lh, F_ATTN, (launch_k(decode_attention_kernel<128>, grid, 256, 0, S, (const bf16 *)w.QKV, bb.d_qkv, w.AttnO, bb.d_q, d.n_q_heads, d.n_kv_heads, scale_log2, l, ka)));
+      rev();
+    } else if (c->o.attn_impl == FMX_ATTN_AUTO && attn_pair64_ok(c->o, d.head_dim, d.n_q_heads, max_len)) {
       AttnPairArgs pa2{};
       pa2.qkv_map = mQKV64; pa2.out = w.AttnO; pa2.cu_tok = w.t.cu_tok; pa2.ld_out = bb.d_q; pa2.n_req = B;
       pa2.n_q_heads = d.n_q_heads; pa2.n_kv_heads = d.n_kv_heads; pa2.causal = d.causal; pa2.scale_log2 = scale_log2;
@@ -1326,7 +1379,8 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       LAUNCH(Lh, F_GEMM_FFN_OUT, launch_pair_gemm(c, S, p));
     }
   }
-  // ---- S4-S6 ----
+  // ---- S4-S6 (skipped by a decode step that wants LM scores only) ----
+  if (outputs != nullptr) {
   PoolArgs pa{};
   pa.X = w.X; pa.g = (const bf16 *)d.final_g; pa.b = (const bf16 *)d.final_b; pa.cu_tok = w.t.cu_tok; pa.task_sorted = w.t.task_sorted;
   pa.task_head_kind = c->d_task_head_kind; pa.feat = w.feat; pa.Fn = w.Xn; pa.d = d.d_model; pa.eps = d.norm_eps; pa.rms = rms;
@@ -1364,6 +1418,25 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
 
   if (max_hidden > 0)                                    // second layer of the MLP heads (the first wrote relu(W feat + b) to hid)
     LAUNCH(Lh, F_HEAD, (launch_k(head_mlp2_kernel, dim3(B, (max_out2 + 7) / 8), 256, 0, S, ha)));
+  }
+
+  // ---- LM head (NEXT-3): scores of every request's last token, greedy next token; original request order ----
+  if (kv && (kv->scores || kv->next_tokens)) {
+    switch (d.d_model / 128) {
+#define FMX_LRN(V) case V: LAUNCH(Lh, F_POOL, (launch_k(last_row_norm_kernel<V>, (B + 7) / 8, 256, 0, S, (const float *)w.X, (const int *)w.t.cu_tok, w.Fl, (const bf16 *)d.final_g, (const bf16 *)d.final_b, B, d.norm_eps, rms))); break;
+      FMX_LRN(1) FMX_LRN(2) FMX_LRN(4) FMX_LRN(6) FMX_LRN(8) FMX_LRN(12) FMX_LRN(16)
+#undef FMX_LRN
+    }
+    PairGemmParams p{};
+    p.M = B; p.K = d.d_model; p.n_chunks = bb.lm_vocab / 128; p.n_ptiles = (B + kPairRows - 1) / kPairRows; p.mode = GM_OUT_F32;
+    for (int i = 0; i < 3; ++i) { p.lora_tgt[i] = -1; p.src_end[i] = 1 << 30; }
+    CUtensorMap mFl, oLm;
+    if ((e = encode_2d(c, &mFl, w.Fl, B, d.d_model, d.d_model, 128))) return e;
+    if ((e = encode_2d(c, &oLm, w.lm_scores, B, bb.lm_vocab, bb.lm_vocab, 128, true))) return e;
+    p.amap = mFl; p.omap = oLm; p.wmap[0] = bb.mLm[pair_wide(p) ? 0 : 1]; p.wmap_h[0] = bb.mLm[1];
+    LAUNCH(Lh, F_HEAD, launch_pair_gemm(c, S, p));
+    LAUNCH(Lh, F_HEAD, (launch_k(scores_out_kernel, B, 256, 0, S, (const float *)w.lm_scores, (const int *)w.t.perm, bb.lm_vocab, kv->scores, kv->next_tokens)));
+  }
 
   {
     void *bufs[7] = {w.X, w.Xn, w.QKV, w.AttnO, w.Hid, w.U, w.feat};
@@ -1505,6 +1578,90 @@ int fmx_forward_mixed_host(fmx_ctx *c, fmx_backbone_t h, const void *inputs_host
   CU_OK(cudaMemcpyAsync(outputs_host, out_stage, out_bytes, cudaMemcpyDeviceToHost, s));
   CU_OK(cudaStreamSynchronize(s));
   return poll_device_error(c);
+}
+
+// ---------------------------------------------------------------- token decode with a key / value cache (NEXT-3)
+int fmx_register_lm_head(fmx_ctx *c, fmx_backbone_t h, const void *W, int32_t vocab) {
+  if (!c || !W) return fmx_fail(FMX_E_INVALID_ARG, "register_lm_head: NULL argument");
+  std::lock_guard<std::mutex> lk(c->mu);
+  Backbone *bb = get_bb(c, h);
+  if (!bb) return fmx_fail(FMX_E_UNKNOWN_BACKBONE, "register_lm_head: unknown backbone %d", h);
+  if (vocab < 128 || vocab % 128) return fmx_fail(FMX_E_SHAPE, "register_lm_head: vocab %d must be a positive multiple of 128", vocab);
+  CUtensorMap m0, m1;
+  if (int e = encode_2d(c, &m0, W, vocab, bb->d.d_model, bb->d.d_model, 128)) return e;
+  if (int e = encode_2d(c, &m1, W, vocab, bb->d.d_model, bb->d.d_model, 64)) return e;
+  bb->lm_head = (const bf16 *)W; bb->lm_vocab = vocab; bb->mLm[0] = m0; bb->mLm[1] = m1;
+  ++c->config_gen;
+  return FMX_OK;
+}
+
+int fmx_kv_cache_bytes(fmx_ctx *c, fmx_backbone_t h, int32_t n_slots, size_t *bytes) {
+  if (!c || !bytes) return fmx_fail(FMX_E_INVALID_ARG, "kv_cache_bytes: NULL argument");
+  std::lock_guard<std::mutex> lk(c->mu);
+  Backbone *bb = get_bb(c, h);
+  if (!bb) return fmx_fail(FMX_E_UNKNOWN_BACKBONE, "kv_cache_bytes: unknown backbone %d", h);
+  if (n_slots < 1 || n_slots > (1 << 20)) return fmx_fail(FMX_E_CAPACITY, "kv_cache_bytes: n_slots %d", n_slots);
+  *bytes = (size_t)n_slots * bb->d.n_layers * 2 * bb->d.max_seq * bb->d_kv * sizeof(bf16);
+  return FMX_OK;
+}
+
+// Shared validation + launch of fmx_prefill / fmx_decode_step (c->mu held).
+static int kv_forward(fmx_ctx *c, fmx_backbone_t h, const char *who, const void *inputs, const int32_t *task_ids, const int32_t *lengths,
+                      const int32_t *slots, const int32_t *pos0, int32_t n_req, float *outputs, float *scores, int32_t *next_tokens,
+                      void *kv_cache, int32_t n_slots, void *workspace, size_t workspace_bytes, cudaStream_t s) {
+  Backbone *bb = get_bb(c, h);
+  if (!bb) return fmx_fail(FMX_E_UNKNOWN_BACKBONE, "%s: unknown backbone %d", who, h);
+  if (n_req == 0) return FMX_OK;
+  if (n_req > FMX_MAX_REQUESTS) return fmx_fail(FMX_E_CAPACITY, "%s: %d requests > %d", who, n_req, FMX_MAX_REQUESTS);
+  if (!inputs || !task_ids || !slots || !kv_cache || !workspace) return fmx_fail(FMX_E_INVALID_ARG, "%s: NULL pointer", who);
+  const fmx_backbone_desc &d = bb->d;
+  if (!d.causal) return fmx_fail(FMX_E_SHAPE, "%s: a key / value cache needs a causal backbone", who);
+  if ((scores || next_tokens) && !bb->lm_head) return fmx_fail(FMX_E_INVALID_ARG, "%s: scores / next_tokens need fmx_register_lm_head", who);
+  if (reinterpret_cast<uintptr_t>(kv_cache) & 15) return fmx_fail(FMX_E_INVALID_ARG, "%s: kv_cache must be 16-byte aligned", who);
+  if (n_slots < 1) return fmx_fail(FMX_E_INVALID_ARG, "%s: n_slots < 1", who);
+  std::vector<unsigned char> seen((size_t)n_slots, 0);
+  std::vector<int32_t> ones;
+  if (pos0) { ones.assign(n_req, 1); lengths = ones.data(); }          // a decode step: one token per request
+  else if (!lengths) return fmx_fail(FMX_E_INVALID_ARG, "%s: NULL lengths", who);
+  for (int i = 0; i < n_req; ++i) {
+    if (slots[i] < 0 || slots[i] >= n_slots) return fmx_fail(FMX_E_INVALID_ARG, "%s: request %d: cache slot %d not in [0, %d)", who, i, slots[i], n_slots);
+    if (seen[slots[i]]) return fmx_fail(FMX_E_INVALID_ARG, "%s: cache slot %d is used by two requests of the batch", who, slots[i]);
+    seen[slots[i]] = 1;
+    if (pos0 && (pos0[i] < 0 || pos0[i] >= d.max_seq))
+      return fmx_fail(FMX_E_BAD_LENGTH, "%s: request %d: %d cached tokens, the cache holds max_seq = %d", who, i, pos0[i], d.max_seq);
+  }
+  BatchShape bs;
+  if (int e = batch_shape(c, *bb, task_ids, lengths, n_req, bs)) return e;
+  CU_OK(cudaSetDevice(c->device));
+  if (int e = poll_device_error(c)) return e;
+  KvCall kv;
+  kv.cache = (bf16 *)kv_cache; kv.n_slots = n_slots; kv.slots = slots; kv.pos0 = pos0; kv.scores = scores; kv.next_tokens = next_tokens;
+  kv.decode = pos0 != nullptr;
+  return forward_impl(c, *bb, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, s, bs, false, &kv);
+}
+
+int fmx_prefill(fmx_ctx *c, fmx_backbone_t h, const void *inputs, const int32_t *task_ids, const int32_t *lengths, const int32_t *slots,
+                int32_t n_req, float *outputs, float *scores, int32_t *next_tokens, void *kv_cache, int32_t n_slots, void *workspace,
+                size_t workspace_bytes, void *cuda_stream) {
+  if (!c) return fmx_fail(FMX_E_INVALID_ARG, "prefill: NULL ctx");
+  if (n_req < 0) return fmx_fail(FMX_E_INVALID_ARG, "prefill: n_req < 0");
+  std::lock_guard<std::mutex> lk(c->mu);
+  return kv_forward(c, h, "prefill", inputs, task_ids, lengths, slots, nullptr, n_req, outputs, scores, next_tokens, kv_cache, n_slots,
+                    workspace, workspace_bytes, (cudaStream_t)cuda_stream);
+}
+
+int fmx_decode_step(fmx_ctx *c, fmx_backbone_t h, const int32_t *tokens, const int32_t *task_ids, const int32_t *slots, const int32_t *positions,
+                    int32_t n_req, float *scores, int32_t *next_tokens, void *kv_cache, int32_t n_slots, void *workspace,
+                    size_t workspace_bytes, void *cuda_stream) {
+  if (!c) return fmx_fail(FMX_E_INVALID_ARG, "decode_step: NULL ctx");
+  if (n_req < 0) return fmx_fail(FMX_E_INVALID_ARG, "decode_step: n_req < 0");
+  if (n_req > 0 && !positions) return fmx_fail(FMX_E_INVALID_ARG, "decode_step: NULL positions");
+  std::lock_guard<std::mutex> lk(c->mu);
+  Backbone *bb = get_bb(c, h);
+  if (bb && bb->d.input_kind != FMX_INPUT_TOKEN_IDS) return fmx_fail(FMX_E_SHAPE, "decode_step: the backbone does not take token ids");
+  if (n_req > 0 && !scores && !next_tokens) return fmx_fail(FMX_E_INVALID_ARG, "decode_step: neither scores nor next_tokens requested");
+  return kv_forward(c, h, "decode_step", tokens, task_ids, nullptr, slots, positions, n_req, nullptr, scores, next_tokens, kv_cache, n_slots,
+                    workspace, workspace_bytes, (cudaStream_t)cuda_stream);
 }
 
 int fmx_debug_get_segments(fmx_ctx *c, int32_t *perm, int32_t *inv_perm, int32_t *task_req_off, int32_t *cu_tok, int32_t *task_tok_off) {

@@ -741,4 +741,201 @@ __global__ void __launch_bounds__(512) head_flatten_reduce_kernel(const HeadArgs
   a.out[a.out_off[a.perm[p]] + oa] = v + (b ? __bfloat162float(b[oa]) : 0.0f);
 }
 
+// ============================================================================= token decode with a KV cache (NEXT-3)
+// Cache layout (caller-owned device memory, fmx_kv_cache_bytes): [slot][layer][k | v][max_seq][d_kv] bf16.
+struct KvArgs {
+  __nv_bfloat16 *cache;
+  long long slot_stride, layer_stride, kv_stride;   // elements: per slot, per layer, k -> v
+  int d_kv, max_seq;
+  const int *row_slot, *row_cpos;                   // [N] cache slot / cache position of every token row
+};
+
+// row -> (cache slot, cache position = RoPE position).  slots / pos0 are per ORIGINAL request; pos0 NULL = 0 (prefill).
+__global__ void kv_rows_kernel(const int *__restrict__ row_req, const int *__restrict__ row_pos, const int *__restrict__ perm,
+                               const int *__restrict__ slots, const int *__restrict__ pos0, int N, int *__restrict__ row_slot,
+                               int *__restrict__ row_cpos) {
+  griddep_launch();
+  griddep_wait();
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= N) return;
+  const int i = perm[row_req[r]];
+  row_slot[r] = slots[i];
+  row_cpos[r] = (pos0 ? pos0[i] : 0) + row_pos[r];
+}
+
+// Appends this layer's k and v rows (after RoPE) of every token row to the cache.  One warp per row, 16-byte copies.
+__global__ void kv_append_kernel(const __nv_bfloat16 *__restrict__ qkv, int ld_qkv, int col_k, int col_v, int N, int layer, const KvArgs a) {
+  griddep_launch();
+  griddep_wait();
+  const int r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (r >= N) return;
+  __nv_bfloat16 *dst = a.cache + (long long)a.row_slot[r] * a.slot_stride + (long long)layer * a.layer_stride + (long long)a.row_cpos[r] * a.d_kv;
+  const __nv_bfloat16 *src = qkv + (size_t)r * ld_qkv;
+  for (int c = lane * 8; c < a.d_kv; c += 256) {
+    *reinterpret_cast<uint4 *>(dst + c) = *reinterpret_cast<const uint4 *>(src + col_k + c);
+    *reinterpret_cast<uint4 *>(dst + a.kv_stride + c) = *reinterpret_cast<const uint4 *>(src + col_v + c);
+  }
+}
+
+// Decode attention: every request has ONE query token (row p of the task-sorted batch) that attends the cache positions
+// 0 .. cpos (its own k / v were appended just before).  One CTA per (request, KV head); the query heads of the GQA group share
+// the K / V rows.  Warp w walks keys w, w + 8, ...; a lane owns DH / 32 consecutive dims of a row (coalesced row reads),
+// the dot products are reduced with shuffles, every warp keeps an online softmax per head and the eight partial states
+// (m, l, o) are merged in warp order in shared memory (deterministic).  Memory-bound: 2 * (cpos + 1) * DH * 2 bytes per CTA.
+constexpr int kDecGroupMax = 8;
+template <int VPT>
+__device__ __forceinline__ void load_bf16_vec(const __nv_bfloat16 *p, float (&f)[VPT]) {      // one aligned load of VPT = 1 / 2 / 4 values
+  if constexpr (VPT == 4) {
+    const uint2 u = *reinterpret_cast<const uint2 *>(p);
+    f[0] = bf16_lo(u.x); f[1] = bf16_hi(u.x); f[2] = bf16_lo(u.y); f[3] = bf16_hi(u.y);
+  } else if constexpr (VPT == 2) {
+    const uint32_t u = *reinterpret_cast<const uint32_t *>(p);
+    f[0] = bf16_lo(u); f[1] = bf16_hi(u);
+  } else {
+    f[0] = __bfloat162float(p[0]);
+  }
+}
+template <int DH>
+__global__ void __launch_bounds__(256) decode_attention_kernel(const __nv_bfloat16 *__restrict__ qkv, int ld_qkv, __nv_bfloat16 *__restrict__ out,
+                                                               int ld_out, int n_q_heads, int n_kv_heads, float scale_log2, int layer, const KvArgs a) {
+  constexpr int VPT = DH / 32;
+  __shared__ float s_m[8][kDecGroupMax], s_l[8][kDecGroupMax];
+  __shared__ float s_o[8][kDecGroupMax][DH];
+  griddep_launch();
+  griddep_wait();
+  const int p = blockIdx.x, kvh = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int group = n_q_heads / n_kv_heads;
+  const int n_keys = a.row_cpos[p] + 1;
+  const __nv_bfloat16 *K = a.cache + (long long)a.row_slot[p] * a.slot_stride + (long long)layer * a.layer_stride + kvh * DH + lane * VPT;
+  const __nv_bfloat16 *V = K + a.kv_stride;
+  float q[kDecGroupMax][VPT], acc[kDecGroupMax][VPT], m[kDecGroupMax], l[kDecGroupMax];
+#pragma unroll
+  for (int g = 0; g < kDecGroupMax; ++g) {
+    m[g] = -INFINITY; l[g] = 0.0f;
+#pragma unroll
+    for (int e = 0; e < VPT; ++e) {
+      acc[g][e] = 0.0f;
+      q[g][e] = g < group ? __bfloat162float(qkv[(size_t)p * ld_qkv + (kvh * group + g) * DH + lane * VPT + e]) * scale_log2 : 0.0f;
+    }
+  }
+  for (int k = warp; k < n_keys; k += 8) {
+    float kf[VPT], vf[VPT];
+    load_bf16_vec<VPT>(K + (long long)k * a.d_kv, kf);
+    load_bf16_vec<VPT>(V + (long long)k * a.d_kv, vf);
+#pragma unroll
+    for (int g = 0; g < kDecGroupMax; ++g) {
+      if (g >= group) break;
+      float s = 0.0f;
+#pragma unroll
+      for (int e = 0; e < VPT; ++e) s = fmaf(q[g][e], kf[e], s);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+      const float mn = fmaxf(m[g], s);
+      const float f = fast_exp2(m[g] - mn), pw = fast_exp2(s - mn);
+      m[g] = mn;
+      l[g] = l[g] * f + pw;
+#pragma unroll
+      for (int e = 0; e < VPT; ++e) acc[g][e] = fmaf(pw, vf[e], acc[g][e] * f);
+    }
+  }
+#pragma unroll
+  for (int g = 0; g < kDecGroupMax; ++g) {
+    if (g >= group) break;
+    if (lane == 0) { s_m[warp][g] = m[g]; s_l[warp][g] = l[g]; }
+#pragma unroll
+    for (int e = 0; e < VPT; ++e) s_o[warp][g][lane * VPT + e] = acc[g][e];
+  }
+  __syncthreads();
+  for (int idx = threadIdx.x; idx < group * DH; idx += blockDim.x) {
+    const int g = idx / DH, d = idx - g * DH;
+    float mx = -INFINITY;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) mx = fmaxf(mx, s_m[w][g]);
+    float L = 0.0f, O = 0.0f;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) {
+      const float f = fast_exp2(s_m[w][g] - mx);           // a warp that saw no key: m = -inf -> f = 0
+      L = fmaf(s_l[w][g], f, L);
+      O = fmaf(s_o[w][g][d], f, O);
+    }
+    out[(size_t)p * ld_out + (kvh * group + g) * DH + d] = __float2bfloat16(O / L);
+  }
+}
+
+// Final norm of every request's LAST token row -> bf16 [B, d] (sorted request order): the A operand of the LM-head GEMM.
+template <int kVec>
+__global__ void __launch_bounds__(256) last_row_norm_kernel(const float *__restrict__ X, const int *__restrict__ cu_tok, __nv_bfloat16 *__restrict__ Y,
+                                                            const __nv_bfloat16 *__restrict__ g, const __nv_bfloat16 *__restrict__ b, int B, float eps, int rms) {
+  griddep_launch();
+  griddep_wait();
+  const int p = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (p >= B) return;
+  constexpr int d = 128 * kVec;
+  const float4 *x = reinterpret_cast<const float4 *>(X + (size_t)(cu_tok[p + 1] - 1) * d);
+  float4 v[kVec];
+  float s = 0.0f;
+#pragma unroll
+  for (int j = 0; j < kVec; ++j) { v[j] = x[j * 32 + lane]; s += v[j].x + v[j].y + v[j].z + v[j].w; }
+  float mean = 0.0f;
+  if (!rms) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    mean = s * (1.0f / d);
+  }
+  float qq = 0.0f;
+#pragma unroll
+  for (int j = 0; j < kVec; ++j) {
+    const float a0 = v[j].x - mean, a1 = v[j].y - mean, a2 = v[j].z - mean, a3 = v[j].w - mean;
+    qq += a0 * a0 + a1 * a1 + a2 * a2 + a3 * a3;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) qq += __shfl_xor_sync(0xffffffffu, qq, o);
+  const float inv = rsqrtf(qq * (1.0f / d) + eps);
+  uint2 *y = reinterpret_cast<uint2 *>(Y + (size_t)p * d);
+#pragma unroll
+  for (int j = 0; j < kVec; ++j) {
+    const int c4 = j * 32 + lane;
+    const uint2 gg = reinterpret_cast<const uint2 *>(g)[c4];
+    float o0 = (v[j].x - mean) * inv * bf16_lo(gg.x), o1 = (v[j].y - mean) * inv * bf16_hi(gg.x);
+    float o2 = (v[j].z - mean) * inv * bf16_lo(gg.y), o3 = (v[j].w - mean) * inv * bf16_hi(gg.y);
+    if (b) {
+      const uint2 bb = reinterpret_cast<const uint2 *>(b)[c4];
+      o0 += bf16_lo(bb.x); o1 += bf16_hi(bb.x); o2 += bf16_lo(bb.y); o3 += bf16_hi(bb.y);
+    }
+    y[c4] = make_uint2(pack_bf16(o0, o1), pack_bf16(o2, o3));
+  }
+}
+
+// LM scores of sorted request p -> the caller's buffers in ORIGINAL request order: scores[perm[p], :] (optional) and the greedy
+// next token argmax (lowest index on ties; optional).  One CTA per request.
+__global__ void __launch_bounds__(256) scores_out_kernel(const float *__restrict__ sorted_scores, const int *__restrict__ perm, int vocab,
+                                                         float *__restrict__ scores, int *__restrict__ next_tokens) {
+  __shared__ float s_v[8];
+  __shared__ int s_i[8];
+  griddep_launch();
+  griddep_wait();
+  const int p = blockIdx.x, i = perm[p], warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const float *src = sorted_scores + (size_t)p * vocab;
+  float best = -INFINITY;
+  int bi = 0x7fffffff;
+  for (int c = threadIdx.x; c < vocab; c += blockDim.x) {
+    const float v = src[c];
+    if (scores) scores[(size_t)i * vocab + c] = v;
+    if (v > best) { best = v; bi = c; }                   // ascending c per thread: the first maximum is kept
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const float ov = __shfl_xor_sync(0xffffffffu, best, o);
+    const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+    if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+  }
+  if (lane == 0) { s_v[warp] = best; s_i[warp] = bi; }
+  __syncthreads();
+  if (threadIdx.x == 0 && next_tokens) {
+    for (int w = 1; w < 8; ++w)
+      if (s_v[w] > best || (s_v[w] == best && s_i[w] < bi)) { best = s_v[w]; bi = s_i[w]; }
+    next_tokens[i] = bi;
+  }
+}
+
 }  // namespace fmx

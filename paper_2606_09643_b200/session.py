@@ -176,6 +176,55 @@ class Session:
         s.synchronize()
         return un_ms, e0.elapsed_time(e1)
 
+    # ------------------------------------------------------------------ token decode (NEXT-3)
+    def enable_decode(self, n_slots, max_req=None):
+        """Register the workload's LM head, allocate the KV cache for n_slots sequences and re-size the workspace (the LM
+        scores buffer is part of it)."""
+        self._lm = _dev_bf16(self.wl.tensor("lm_head.W"), self.dev)
+        self.fmx.register_lm_head(self.bb, self._lm.data_ptr(), self.wl.bb.vocab)
+        self.n_slots = n_slots
+        self.kv_cache = torch.zeros(self.fmx.kv_cache_bytes(self.bb, n_slots) + 16, dtype=torch.uint8, device=self.dev)
+        self.kv_ptr = (self.kv_cache.data_ptr() + 15) // 16 * 16
+        if max_req:
+            self.max_req = max_req
+        self._alloc_workspace(self.fmx.workspace_bytes(self.bb, self.max_req, self.max_tokens))
+        vocab = self.wl.bb.vocab
+        self.scores_dev = torch.empty(self.max_req * vocab, dtype=torch.float32, device=self.dev)
+        self.next_dev = torch.empty(self.max_req, dtype=torch.int32, device=self.dev)
+
+    def prefill(self, tokens, task_ids, lengths, slots, with_heads=True, stream=None):
+        """tokens: packed int32 prompts.  Returns (scores [B, vocab], next tokens [B], head outputs or None) as numpy."""
+        ids = np.asarray([self.task_ids_of[int(t)] for t in task_ids], dtype=np.int32)
+        B, vocab = len(ids), self.wl.bb.vocab
+        tok = torch.from_numpy(np.ascontiguousarray(tokens, dtype=np.int32)).to(self.dev)
+        out = None
+        if with_heads:
+            off = self.fmx.output_layout(ids)
+            out = torch.empty(max(int(off[-1]), 1), dtype=torch.float32, device=self.dev)
+        s = stream if stream is not None else torch.cuda.current_stream(self.dev)
+        self.fmx.prefill(self.bb, tok.data_ptr(), ids, lengths, slots, out.data_ptr() if with_heads else 0, self.scores_dev.data_ptr(),
+                         self.next_dev.data_ptr(), self.kv_ptr, self.n_slots, self.ws_ptr, self.ws_bytes, s.cuda_stream)
+        torch.cuda.synchronize(self.dev)
+        heads = None
+        if with_heads:
+            flat = out.cpu().numpy()
+            heads = [flat[off[i]:off[i + 1]].copy() for i in range(B)]
+        return self.scores_dev[:B * vocab].cpu().numpy().reshape(B, vocab), self.next_dev[:B].cpu().numpy(), heads
+
+    def decode_step(self, tokens_dev_ptr, task_ids, slots, positions, want_scores=True, stream=None, sync=True):
+        """One decode iteration; tokens_dev_ptr: device address of int32 [B].  Returns (scores or None, next tokens) as numpy
+        when sync, else nothing (results stay in self.scores_dev / self.next_dev)."""
+        ids = np.asarray([self.task_ids_of[int(t)] for t in task_ids], dtype=np.int32)
+        B, vocab = len(ids), self.wl.bb.vocab
+        s = stream if stream is not None else torch.cuda.current_stream(self.dev)
+        self.fmx.decode_step(self.bb, tokens_dev_ptr, ids, slots, positions, self.scores_dev.data_ptr() if want_scores else 0,
+                             self.next_dev.data_ptr(), self.kv_ptr, self.n_slots, self.ws_ptr, self.ws_bytes, s.cuda_stream)
+        if not sync:
+            return None
+        torch.cuda.synchronize(self.dev)
+        sc = self.scores_dev[:B * vocab].cpu().numpy().reshape(B, vocab) if want_scores else None
+        return sc, self.next_dev[:B].cpu().numpy()
+
     # ------------------------------------------------------------------ running
     def upload_inputs(self, packed=None):
         packed = self.wl.packed_inputs() if packed is None else packed

@@ -1,0 +1,112 @@
+"""GPU parity of token decode with a KV cache ("token-based FMs ... continuous batching
+and long-lived decode iterations", L168) through the C ABI (fmx_prefill / fmx_decode_step) against oracle.decode, which has no
+cache: it recomputes the whole prefix of every request for every step in fp64 (the definition).
+
+Bars: next-token scores max-abs <= 2e-2 and cosine >= 0.999 per request and step (BASELINE.json's tolerance; the LM head is
+N(0, 0.02), scores are O(1)).  The greedy token is an argmax over floating-point scores: the GPU's choice must be within twice
+the tolerance of the oracle's best score, and the oracle is teacher-forced with the GPU's tokens so that a near-tie cannot make
+the two sequences diverge."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from fmx_workloads import make_workload  # noqa: E402
+from oracle import decode as D  # noqa: E402
+from oracle import from_workload as G  # noqa: E402
+
+MAX_ABS, MIN_COS = 2e-2, 0.999
+
+
+@pytest.fixture(scope="module")
+def fmx_mod():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test needs a CUDA device; the product has no CPU fallback")
+    import paper_2606_09643_b200 as pkg
+    return pkg
+
+
+def check_scores(got, ref, label):
+    err = float(np.abs(got - ref).max())
+    cos = float(got @ ref / (np.linalg.norm(got) * np.linalg.norm(ref)))
+    assert np.isfinite(got).all() and err <= MAX_ABS and cos >= MIN_COS, f"{label}: max-abs {err:.3e}, cosine {cos:.6f}"
+
+
+def check_token(tok, ref, label):
+    assert ref[int(tok)] >= ref.max() - 2 * MAX_ABS, f"{label}: token {tok} scores {ref[int(tok)]:.4f}, the best is {ref.max():.4f}"
+
+
+@pytest.mark.parametrize("cfg,kw,opts", [
+    ("cfg4", dict(n_layers=2, batch=6, max_len=90, n_tasks=8), {}),    # head_dim 128, GQA 6:1, RoPE fused in the QKV epilogue, SwiGLU, 7 LoRA targets
+    ("cfg4", dict(n_layers=2, batch=5, max_len=140, n_tasks=8), dict(rope_fused=0, pdl=1)),   # separate RoPE kernel reading cache positions; PDL on
+])
+def test_prefill_and_decode_match_the_no_cache_definition(fmx_mod, cfg, kw, opts):
+    from paper_2606_09643_b200.session import Session
+    wl = make_workload(cfg, **kw)
+    B = wl.n_req
+    s = Session(wl, max_req=8, max_tokens=max(wl.n_tokens, 64))
+    for k, v in opts.items():
+        s.fmx.set_option(k, v)
+    plain_heads = s.forward_numpy()
+    s.enable_decode(n_slots=8)
+    bb, get, tasks = G.bb_dict(wl), G.make_get(wl), G.task_dicts(wl)
+    prompts = [wl.request_input(i) for i in range(B)]
+    slots = np.array([3, 0, 5, 1, 4, 2][:B], dtype=np.int32)
+    # ---- prefill: task heads equal the plain forward bit for bit; scores follow the definition ----
+    scores, nxt, heads = s.prefill(wl.packed_inputs(), wl.task_ids, wl.lengths, slots)
+    for a, b in zip(heads, plain_heads):
+        assert np.array_equal(a, b), "prefill changes the task-head outputs"
+    seqs = [list(map(int, p)) for p in prompts]
+    for i in range(B):
+        ref = D.lm_scores(bb, get, tasks[int(wl.task_ids[i])], seqs[i])
+        check_scores(scores[i], ref, f"prefill request {i}")
+        check_token(nxt[i], ref, f"prefill request {i}")
+    # ---- decode with a changing batch (continuous batching): all, a subset in another order, all again ----
+    pending = {i: int(nxt[i]) for i in range(B)}                 # the token each request appends next
+    for step, members in enumerate([list(range(B)), [4, 0, 2], list(range(B))[::-1], [1, 3, 5, 0]]):
+        members = [m for m in members if m < B]
+        toks = torch.tensor([pending[i] for i in members], dtype=torch.int32, device="cuda")
+        pos = np.array([len(seqs[i]) for i in members], dtype=np.int32)
+        sc, nx = s.decode_step(toks.data_ptr(), wl.task_ids[members], slots[members], pos)
+        for j, i in enumerate(members):
+            seqs[i].append(pending[i])
+            ref = D.lm_scores(bb, get, tasks[int(wl.task_ids[i])], seqs[i])
+            check_scores(sc[j], ref, f"decode step {step} request {i} (position {pos[j]})")
+            check_token(nx[j], ref, f"decode step {step} request {i}")
+            pending[i] = int(nx[j])
+    # ---- a request's decode does not depend on who shares the batch: alone == in the batch, bit for bit ----
+    i = 2
+    toks = torch.tensor([pending[k] for k in range(B)], dtype=torch.int32, device="cuda")
+    pos = np.array([len(seqs[k]) for k in range(B)], dtype=np.int32)
+    sc_all, _ = s.decode_step(toks.data_ptr(), wl.task_ids, slots, pos)
+    sc_one, _ = s.decode_step(toks[i:i + 1].data_ptr(), wl.task_ids[i:i + 1], slots[i:i + 1], pos[i:i + 1])   # rewrites the same cache row
+    assert np.array_equal(sc_all[i], sc_one[0])
+
+
+def test_decode_argument_errors(fmx_mod):
+    from paper_2606_09643_b200.session import Session
+    wl = make_workload("cfg4", n_layers=1, batch=3, max_len=70, n_tasks=4)
+    s = Session(wl, max_req=4, max_tokens=256)
+    E = fmx_mod.FmxError
+    tok = torch.zeros(4, dtype=torch.int32, device="cuda")
+    kv = torch.zeros(1 << 20, dtype=torch.uint8, device="cuda")
+    with pytest.raises(E) as e:                                   # no LM head registered
+        s.fmx.decode_step(s.bb, tok.data_ptr(), [0], [0], [5], 0, tok.data_ptr(), kv.data_ptr(), 1, s.ws_ptr, s.ws_bytes)
+    assert e.value.code == -1
+    s.enable_decode(n_slots=4)
+    args = (s.scores_dev.data_ptr(), s.next_dev.data_ptr(), s.kv_ptr, 4, s.ws_ptr, s.ws_bytes)
+    with pytest.raises(E) as e:                                   # two requests on one slot
+        s.fmx.decode_step(s.bb, tok.data_ptr(), [0, 1], [2, 2], [5, 5], *args)
+    assert e.value.code == -1 and "slot" in str(e.value)
+    with pytest.raises(E) as e:                                   # cache full
+        s.fmx.decode_step(s.bb, tok.data_ptr(), [0], [1], [wl.bb.max_seq], *args)
+    assert e.value.code == -5
+    with pytest.raises(E) as e:                                   # slot out of range
+        s.fmx.decode_step(s.bb, tok.data_ptr(), [0], [4], [0], *args)
+    assert e.value.code == -1
+    wl2 = make_workload("cfg2", n_layers=1, batch=2)
+    s2 = Session(wl2)
+    with pytest.raises(E) as e:                                   # not a causal backbone
+        s2.fmx.prefill(s2.bb, tok.data_ptr(), [0], [64], [0], 0, 0, 0, kv.data_ptr(), 1, s2.ws_ptr, s2.ws_bytes)
+    assert e.value.code == -4
