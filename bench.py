@@ -434,7 +434,7 @@ def measure_decode(sess, wl, steps=16, warm=3):
     import torch
     bb = wl.bb
     B = wl.n_req
-    room = steps + warm + 2
+    room = steps + warm + 4
     lens = np.minimum(wl.lengths, bb.max_seq - room).astype(np.int32)
     toks = np.concatenate([wl.request_input(i)[:lens[i]] for i in range(B)]).astype(np.int32)
     sess.enable_decode(n_slots=B, max_req=B)
@@ -457,6 +457,14 @@ def measure_decode(sess, wl, steps=16, warm=3):
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / steps
     launches = sess.fmx.last_launch_count()
+    sess.fmx.profile_select(None)
+    sess.fmx.profile_enable(True)
+    for _ in range(2):
+        sess.decode_step(ptr, wl.task_ids, slots, pos, want_scores=False, sync=False)
+        pos += 1
+    fam = sess.fmx.profile_read()
+    sess.fmx.profile_enable(False)
+    families = {k: {"launches_per_step": n // 2, "ms_per_step": round(t / 2, 4)} for k, (n, t) in fam.items() if n}
     per_layer = 2 * (bb.d_model * (bb.d_q + 2 * bb.d_kv) + bb.d_q * bb.d_model + (3 if bb.act == "swiglu" else 2) * bb.d_model * bb.d_ffn)
     weight_bytes = bb.n_layers * per_layer + 2 * bb.vocab * bb.d_model          # backbone matrices + LM head, bf16
     kv_bytes = kv_rows / steps * bb.n_layers * 2 * bb.d_kv * 2
@@ -464,7 +472,7 @@ def measure_decode(sess, wl, steps=16, warm=3):
     gbs = (weight_bytes + kv_bytes) / (ms * 1e-3) / 1e9
     return {"what": "fmx_decode_step: one new token for each of the batch's sequences per iteration, KV cache, mixed tasks, greedy tokens fed back on the device",
             "requests": B, "tokens_per_s": round(B / (ms * 1e-3), 1), "ms_per_step": round(ms, 4), "steps": steps, "launches_per_step": launches,
-            "mean_cached_tokens": round(kv_rows / steps / B, 1),
+            "mean_cached_tokens": round(kv_rows / steps / B, 1), "families": families,
             "roofline": {"bound": "hbm", "achieved": round(gbs, 1), "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": round(gbs / pk["hbm_gbs"], 4),
                          "bytes_per_step": int(weight_bytes + kv_bytes),
                          "note": "algorithmic bytes = every backbone and LM-head weight once + the cached k / v rows read; the projection GEMMs here are the "

@@ -231,7 +231,8 @@ int fmx_kv_cache_bytes(fmx_ctx *ctx, fmx_backbone_t bb, int32_t n_slots, size_t 
  *   outputs      DEVICE fp32 task-head outputs as fmx_forward_mixed, or NULL to skip the heads
  *   scores       DEVICE fp32 [n_req, vocab] next-token scores in ORIGINAL request order, or NULL
  *   next_tokens  DEVICE int32 [n_req] greedy next token (argmax, lowest index on ties), or NULL
- * Asynchronous on cuda_stream; never replayed from the graph cache. */
+ * Asynchronous on cuda_stream.  Decode iterations of one batch shape replay the context's cached CUDA graph on a non-default
+ * stream (ids, slots and positions are copied before every launch, as in fmx_forward_mixed). */
 int fmx_prefill(fmx_ctx *ctx, fmx_backbone_t bb, const void *inputs, const int32_t *task_ids, const int32_t *lengths,
                 const int32_t *slots, int32_t n_req, float *outputs, float *scores, int32_t *next_tokens, void *kv_cache,
                 int32_t n_slots, void *workspace, size_t workspace_bytes, void *cuda_stream);

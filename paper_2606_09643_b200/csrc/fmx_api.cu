@@ -145,9 +145,11 @@ struct fmx_ctx {
   struct CallKey {
     int bb = -1, B = 0; const void *inputs = nullptr; float *outputs = nullptr; void *workspace = nullptr; size_t ws_bytes = 0;
     cudaStream_t stream = nullptr; unsigned long long gen = 0; BatchShape shape; bool fuse = false;
+    const void *kv_cache = nullptr, *scores = nullptr, *next_tokens = nullptr; int kv_mode = 0, n_slots = 0;   // 0 plain, 1 prefill, 2 decode
     bool operator==(const CallKey &o) const {
       return bb == o.bb && B == o.B && inputs == o.inputs && outputs == o.outputs && workspace == o.workspace && ws_bytes == o.ws_bytes &&
-             stream == o.stream && gen == o.gen && shape == o.shape && fuse == o.fuse;
+             stream == o.stream && gen == o.gen && shape == o.shape && fuse == o.fuse && kv_cache == o.kv_cache && scores == o.scores &&
+             next_tokens == o.next_tokens && kv_mode == o.kv_mode && n_slots == o.n_slots;
     }
   };
   // registration runs on its own non-blocking stream: adding a task never waits for (or stalls) forwards in flight
@@ -1454,7 +1456,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
 // at a fixed batch size) replays it on every step.  The 2nd call with the same key is captured, later ones replay; a step
 // of ~200 short kernels loses ~4 % to launch gaps otherwise (cfg2: 11.55 -> 11.09 ms).
 static int forward_cached(fmx_ctx *c, Backbone *bb, fmx_backbone_t h, const void *inputs, const int32_t *task_ids, const int32_t *lengths,
-                          int32_t n_req, float *outputs, void *workspace, size_t workspace_bytes, cudaStream_t s) {
+                          int32_t n_req, float *outputs, void *workspace, size_t workspace_bytes, cudaStream_t s, const KvCall *kv = nullptr) {
   BatchShape bs;
   if (int e = batch_shape(c, *bb, task_ids, lengths, n_req, bs)) return e;
   const bool graphable = c->o.graph && !c->prof_on && s != nullptr && s != cudaStreamLegacy && s != cudaStreamPerThread;
@@ -1466,13 +1468,14 @@ static int forward_cached(fmx_ctx *c, Backbone *bb, fmx_backbone_t h, const void
       key.bb = h; key.B = n_req; key.inputs = inputs; key.outputs = outputs; key.workspace = workspace; key.ws_bytes = workspace_bytes;
       key.stream = s; key.gen = c->config_gen; key.shape = bs;
       key.fuse = c->o.shrink_fused == 2 || (c->o.shrink_fused == 1 && bs.n_blk <= c->sm_count / 2);
+      if (kv) { key.kv_cache = kv->cache; key.scores = kv->scores; key.next_tokens = kv->next_tokens; key.kv_mode = kv->decode ? 2 : 1; key.n_slots = kv->n_slots; }
       const bool hit = c->graph_exec && key == c->graph_key;
       if (hit || key == c->last_key) {
         if (reinterpret_cast<uintptr_t>(workspace) & 1023) return fmx_fail(FMX_E_WORKSPACE, "forward_mixed: workspace must be 1024-byte aligned");
         const Workspace w = carve(*bb, workspace, n_req, bs.N, c->n_slots);
         if (w.bytes > workspace_bytes) return fmx_fail(FMX_E_WORKSPACE, "forward_mixed: workspace %zu B < required %zu B", workspace_bytes, w.bytes);
         if (hit) {
-          if (int e = stage_ids(c, w, task_ids, lengths, n_req, s)) return e;
+          if (int e = stage_ids(c, w, task_ids, lengths, n_req, s, kv ? kv->slots : nullptr, kv ? kv->pos0 : nullptr)) return e;
           CU_OK(cudaGraphLaunch(c->graph_exec, s));
           c->last_launches = c->graph_launches; c->last_stream = s;
           c->last_t = w.t; c->last_B = n_req; c->last_T = c->n_slots; c->last_n_tiles = w.n_tiles;
@@ -1484,10 +1487,10 @@ static int forward_cached(fmx_ctx *c, Backbone *bb, fmx_backbone_t h, const void
           cudaGraphExecDestroy(c->graph_exec);
           c->graph_exec = nullptr;
         }
-        if (int e = stage_ids(c, w, task_ids, lengths, n_req, s)) return e;
+        if (int e = stage_ids(c, w, task_ids, lengths, n_req, s, kv ? kv->slots : nullptr, kv ? kv->pos0 : nullptr)) return e;
         cudaGraph_t graph = nullptr;
         if (cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
-          const int e = forward_impl(c, *bb, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, s, bs, true);
+          const int e = forward_impl(c, *bb, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, s, bs, true, kv);
           const cudaError_t ce = cudaStreamEndCapture(s, &graph);
           if (e == FMX_OK && ce == cudaSuccess && graph && cudaGraphInstantiate(&c->graph_exec, graph, 0) == cudaSuccess) {
             cudaGraphDestroy(graph);
@@ -1504,13 +1507,13 @@ static int forward_cached(fmx_ctx *c, Backbone *bb, fmx_backbone_t h, const void
           cudaGetLastError();
         }
         // capture failed: the ids are staged already; run the kernels plainly (graph_capture = true skips the staging only)
-        if (int e = forward_impl(c, *bb, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, s, bs, true)) return e;
+        if (int e = forward_impl(c, *bb, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, s, bs, true, kv)) return e;
         return note_forward(c, s);
       }
       c->last_key = std::move(key);
     }
   }
-  return forward_impl(c, *bb, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, s, bs);
+  return forward_impl(c, *bb, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, s, bs, false, kv);
 }
 
 // A device-side error of an EARLIER forward (the word is mapped host memory the kernels write): reported by the next call.
@@ -1630,14 +1633,12 @@ static int kv_forward(fmx_ctx *c, fmx_backbone_t h, const char *who, const void 
     if (pos0 && (pos0[i] < 0 || pos0[i] >= d.max_seq))
       return fmx_fail(FMX_E_BAD_LENGTH, "%s: request %d: %d cached tokens, the cache holds max_seq = %d", who, i, pos0[i], d.max_seq);
   }
-  BatchShape bs;
-  if (int e = batch_shape(c, *bb, task_ids, lengths, n_req, bs)) return e;
   CU_OK(cudaSetDevice(c->device));
   if (int e = poll_device_error(c)) return e;
   KvCall kv;
   kv.cache = (bf16 *)kv_cache; kv.n_slots = n_slots; kv.slots = slots; kv.pos0 = pos0; kv.scores = scores; kv.next_tokens = next_tokens;
   kv.decode = pos0 != nullptr;
-  return forward_impl(c, *bb, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, s, bs, false, &kv);
+  return forward_cached(c, bb, h, inputs, task_ids, lengths, n_req, outputs, workspace, workspace_bytes, s, &kv);
 }
 
 int fmx_prefill(fmx_ctx *c, fmx_backbone_t h, const void *inputs, const int32_t *task_ids, const int32_t *lengths, const int32_t *slots,

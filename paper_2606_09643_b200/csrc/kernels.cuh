@@ -779,9 +779,13 @@ __global__ void kv_append_kernel(const __nv_bfloat16 *__restrict__ qkv, int ld_q
 
 // Decode attention: every request has ONE query token (row p of the task-sorted batch) that attends the cache positions
 // 0 .. cpos (its own k / v were appended just before).  One CTA per (request, KV head); the query heads of the GQA group share
-// the K / V rows.  Warp w walks keys w, w + 8, ...; a lane owns DH / 32 consecutive dims of a row (coalesced row reads),
-// the dot products are reduced with shuffles, every warp keeps an online softmax per head and the eight partial states
-// (m, l, o) are merged in warp order in shared memory (deterministic).  Memory-bound: 2 * (cpos + 1) * DH * 2 bytes per CTA.
+// the K / V rows.  A warp takes 32 keys at a time:
+//   scores   lane = key: the lane reads its key row with 16-byte loads and takes the dot product with every head's query
+//            (queries, pre-scaled, sit in shared memory and are read as broadcast float4s) - no shuffles in the hot loop;
+//   softmax  online per head over the warp's chunks (one warp max / sum per chunk and head);
+//   P V      lane = DH / 32 output dims: the chunk's probabilities go through shared memory, V rows are read coalesced.
+// The eight warps' partial states (m, l, o) are merged in warp order in shared memory (deterministic).
+// Memory-bound: 2 * (cpos + 1) * DH * 2 bytes per CTA.
 constexpr int kDecGroupMax = 8;
 template <int VPT>
 __device__ __forceinline__ void load_bf16_vec(const __nv_bfloat16 *p, float (&f)[VPT]) {      // one aligned load of VPT = 1 / 2 / 4 values
@@ -799,47 +803,89 @@ template <int DH>
 __global__ void __launch_bounds__(256) decode_attention_kernel(const __nv_bfloat16 *__restrict__ qkv, int ld_qkv, __nv_bfloat16 *__restrict__ out,
                                                                int ld_out, int n_q_heads, int n_kv_heads, float scale_log2, int layer, const KvArgs a) {
   constexpr int VPT = DH / 32;
-  __shared__ float s_m[8][kDecGroupMax], s_l[8][kDecGroupMax];
-  __shared__ float s_o[8][kDecGroupMax][DH];
+  constexpr int G = kDecGroupMax;
+  __shared__ __align__(16) float s_q[G][DH];              // queries of the group, times scale * log2(e)
+  __shared__ __align__(16) float s_p[8][G][32];           // a warp's probabilities of its current 32-key chunk
+  __shared__ float s_m[8][G], s_l[8][G];
+  __shared__ float s_o[8][G][DH];
   griddep_launch();
   griddep_wait();
   const int p = blockIdx.x, kvh = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int group = n_q_heads / n_kv_heads;
   const int n_keys = a.row_cpos[p] + 1;
-  const __nv_bfloat16 *K = a.cache + (long long)a.row_slot[p] * a.slot_stride + (long long)layer * a.layer_stride + kvh * DH + lane * VPT;
+  for (int idx = threadIdx.x; idx < G * DH; idx += blockDim.x) {
+    const int g = idx / DH, d = idx - g * DH;
+    s_q[g][d] = g < group ? __bfloat162float(qkv[(size_t)p * ld_qkv + (kvh * group + g) * DH + d]) * scale_log2 : 0.0f;
+  }
+  __syncthreads();
+  const __nv_bfloat16 *K = a.cache + (long long)a.row_slot[p] * a.slot_stride + (long long)layer * a.layer_stride + kvh * DH;
   const __nv_bfloat16 *V = K + a.kv_stride;
-  float q[kDecGroupMax][VPT], acc[kDecGroupMax][VPT], m[kDecGroupMax], l[kDecGroupMax];
+  float acc[G][VPT], m[G], l[G];
 #pragma unroll
-  for (int g = 0; g < kDecGroupMax; ++g) {
+  for (int g = 0; g < G; ++g) {
     m[g] = -INFINITY; l[g] = 0.0f;
 #pragma unroll
-    for (int e = 0; e < VPT; ++e) {
-      acc[g][e] = 0.0f;
-      q[g][e] = g < group ? __bfloat162float(qkv[(size_t)p * ld_qkv + (kvh * group + g) * DH + lane * VPT + e]) * scale_log2 : 0.0f;
-    }
+    for (int e = 0; e < VPT; ++e) acc[g][e] = 0.0f;
   }
-  for (int k = warp; k < n_keys; k += 8) {
-    float kf[VPT], vf[VPT];
-    load_bf16_vec<VPT>(K + (long long)k * a.d_kv, kf);
-    load_bf16_vec<VPT>(V + (long long)k * a.d_kv, vf);
+  for (int k0 = warp * 32; k0 < n_keys; k0 += 8 * 32) {
+    const int key = k0 + lane;
+    const bool valid = key < n_keys;
+    // ---- scores of this lane's key against every head of the group ----
+    float s[G];
 #pragma unroll
-    for (int g = 0; g < kDecGroupMax; ++g) {
+    for (int g = 0; g < G; ++g) s[g] = 0.0f;
+    const uint4 *kp = reinterpret_cast<const uint4 *>(K + (long long)(valid ? key : k0) * a.d_kv);
+#pragma unroll 4
+    for (int v = 0; v < DH / 8; ++v) {
+      const uint4 u = kp[v];
+      const float kf[8] = {bf16_lo(u.x), bf16_hi(u.x), bf16_lo(u.y), bf16_hi(u.y), bf16_lo(u.z), bf16_hi(u.z), bf16_lo(u.w), bf16_hi(u.w)};
+#pragma unroll
+      for (int g = 0; g < G; ++g) {
+        if (g >= group) break;
+        const float4 qa = *reinterpret_cast<const float4 *>(&s_q[g][8 * v]), qb = *reinterpret_cast<const float4 *>(&s_q[g][8 * v + 4]);
+        s[g] = fmaf(qa.x, kf[0], s[g]); s[g] = fmaf(qa.y, kf[1], s[g]); s[g] = fmaf(qa.z, kf[2], s[g]); s[g] = fmaf(qa.w, kf[3], s[g]);
+        s[g] = fmaf(qb.x, kf[4], s[g]); s[g] = fmaf(qb.y, kf[5], s[g]); s[g] = fmaf(qb.z, kf[6], s[g]); s[g] = fmaf(qb.w, kf[7], s[g]);
+      }
+    }
+    // ---- online softmax per head over the chunk ----
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
       if (g >= group) break;
-      float s = 0.0f;
+      const float sv = valid ? s[g] : -INFINITY;
+      float mc = sv;
 #pragma unroll
-      for (int e = 0; e < VPT; ++e) s = fmaf(q[g][e], kf[e], s);
+      for (int o = 16; o > 0; o >>= 1) mc = fmaxf(mc, __shfl_xor_sync(0xffffffffu, mc, o));
+      const float mn = fmaxf(m[g], mc);                     // finite: the chunk holds at least one valid key
+      const float f = fast_exp2(m[g] - mn), pw = fast_exp2(sv - mn);
+      float lc = pw;
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-      const float mn = fmaxf(m[g], s);
-      const float f = fast_exp2(m[g] - mn), pw = fast_exp2(s - mn);
+      for (int o = 16; o > 0; o >>= 1) lc += __shfl_xor_sync(0xffffffffu, lc, o);
       m[g] = mn;
-      l[g] = l[g] * f + pw;
+      l[g] = l[g] * f + lc;
 #pragma unroll
-      for (int e = 0; e < VPT; ++e) acc[g][e] = fmaf(pw, vf[e], acc[g][e] * f);
+      for (int e = 0; e < VPT; ++e) acc[g][e] *= f;
+      s_p[warp][g][lane] = pw;
     }
+    __syncwarp();
+    // ---- O += P V: the lane owns VPT dims of every head's output ----
+    const int nk = min(32, n_keys - k0);
+    const __nv_bfloat16 *vp = V + (long long)k0 * a.d_kv + lane * VPT;
+    for (int kk = 0; kk < nk; kk += 4) {
+      float vf[4][VPT];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) load_bf16_vec<VPT>(vp + (long long)min(kk + j, nk - 1) * a.d_kv, vf[j]);
+#pragma unroll
+      for (int g = 0; g < G; ++g) {
+        if (g >= group) break;
+        const float4 pw = *reinterpret_cast<const float4 *>(&s_p[warp][g][kk]);     // invalid keys of the chunk hold 0
+#pragma unroll
+        for (int e = 0; e < VPT; ++e) acc[g][e] = fmaf(pw.x, vf[0][e], fmaf(pw.y, vf[1][e], fmaf(pw.z, vf[2][e], fmaf(pw.w, vf[3][e], acc[g][e]))));
+      }
+    }
+    __syncwarp();
   }
 #pragma unroll
-  for (int g = 0; g < kDecGroupMax; ++g) {
+  for (int g = 0; g < G; ++g) {
     if (g >= group) break;
     if (lane == 0) { s_m[warp][g] = m[g]; s_l[warp][g] = l[g]; }
 #pragma unroll

@@ -84,6 +84,37 @@ def test_prefill_and_decode_match_the_no_cache_definition(fmx_mod, cfg, kw, opts
     assert np.array_equal(sc_all[i], sc_one[0])
 
 
+def test_decode_steps_replay_the_cached_graph_with_identical_results(fmx_mod):
+    """On a non-default stream the decode iterations of one batch shape are captured once and replayed, positions and slots
+    changing from step to step: the tokens and scores equal those of plain launches bit for bit."""
+    from paper_2606_09643_b200.session import Session
+    wl = make_workload("cfg4", n_layers=2, batch=6, max_len=80, n_tasks=8)
+    B = wl.n_req
+    slots = np.arange(B, dtype=np.int32)[::-1].copy()
+    runs = []
+    for use_stream in (False, True):
+        s = Session(wl, max_req=8, max_tokens=max(wl.n_tokens, 64))
+        s.enable_decode(n_slots=8)
+        st = torch.cuda.Stream() if use_stream else None
+        _, nxt, _ = s.prefill(wl.packed_inputs(), wl.task_ids, wl.lengths, slots, with_heads=False)
+        pos = wl.lengths.astype(np.int32).copy()
+        trace = [nxt.copy()]
+        r0 = s.fmx.graph_replays()
+        for _ in range(6):
+            if st is not None:
+                with torch.cuda.stream(st):
+                    sc, nx = s.decode_step(s.next_dev.data_ptr(), wl.task_ids, slots, pos, stream=st)
+            else:
+                sc, nx = s.decode_step(s.next_dev.data_ptr(), wl.task_ids, slots, pos)
+            trace += [nx.copy(), sc.copy()]
+            pos += 1
+        runs.append(trace)
+        if use_stream:
+            assert s.fmx.graph_replays() - r0 == 4            # step 1 plain, step 2 captured, steps 3-6 replayed
+    for a, b in zip(*runs):
+        assert np.array_equal(a, b)
+
+
 def test_decode_argument_errors(fmx_mod):
     from paper_2606_09643_b200.session import Session
     wl = make_workload("cfg4", n_layers=1, batch=3, max_len=70, n_tasks=4)
