@@ -226,8 +226,12 @@ def pooled_feature(f, head_kind):
 def head_forward(bb, get, task, h):
     """Steps 3-5: final norm, pool, linear head."""
     f = _norm(bb, get, "final", h)
-    feat = pooled_feature(f, task["head_kind"])
     p = f"task{task['id']:03d}.head."
+    if task["head_kind"] == "dense":
+        # dense (per-token) decoder, PAPER.md L70 "dense decoders for ... detection, and segmentation" (SURVEY.md 8(f) NEXT-1;
+        # DESIGN.md reading 35): the head is applied to EVERY token row; the output is [n, o_t] row-major (token, then class)
+        return (f @ get(p + "W").T + get(p + "b")).reshape(-1)
+    feat = pooled_feature(f, task["head_kind"])
     y = get(p + "W") @ feat + get(p + "b")
     if task.get("head_hidden", 0):
         # MLP decoder head (PAPER.md L546 Listing 2: MLPDecoder(input_dim, hidden_dim, output_dim)); the paper names the three

@@ -733,3 +733,38 @@ def test_token_id_outside_the_vocabulary_is_reported_not_read(fmx_mod):
     s.upload_inputs(wl.packed_inputs())
     for a, b in zip(s.forward_numpy(), good):
         assert np.array_equal(a, b)
+
+
+def test_two_backbones_share_one_context(fmx_mod):
+    """SURVEY.md 8(f) NEXT-4, first part (PAPER.md L253 / L293: several FM instances on one accelerator): two different backbones -
+    the time-series encoder and the decoder LM - are registered in ONE context with their own tasks, LoRA slab arenas and
+    workspaces.  Forwards of the two, interleaved on two streams, give exactly what each gives in a context of its own; a
+    task id of one backbone is rejected on the other."""
+    from paper_2606_09643_b200.session import Session
+    wl_a = make_workload("cfg2", n_layers=2, batch=24)
+    wl_b = make_workload("cfg4", n_layers=2, batch=6, max_len=150, n_tasks=8)
+    alone_a = Session(wl_a).forward_numpy()
+    alone_b = Session(wl_b).forward_numpy()
+    ctx = fmx_mod.Fmx(0)
+    a = Session(wl_a, fmx=ctx)
+    b = Session(wl_b, fmx=ctx)
+    assert a.bb != b.bb and set(a.task_ids_of).isdisjoint(b.task_ids_of)
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    for _ in range(3):
+        a.forward(stream=sa)
+        b.forward(stream=sb)
+    torch.cuda.synchronize()
+    fa, fb = a.out_dev.cpu().numpy(), b.out_dev.cpu().numpy()
+    for i in range(wl_a.n_req):
+        assert np.array_equal(fa[a.last_off[i]:a.last_off[i + 1]], alone_a[i])
+    for i in range(wl_b.n_req):
+        assert np.array_equal(fb[b.last_off[i]:b.last_off[i + 1]], alone_b[i])
+    check_parity(alone_b, G.oracle_outputs(wl_b), "decoder backbone beside the encoder")
+    with pytest.raises(fmx_mod.FmxError) as e:            # a task of backbone A on backbone B
+        ctx.forward_mixed(b.bb, b.inputs_dev.data_ptr(), np.array([a.task_ids_of[0]]), np.array([64]), b.out_dev.data_ptr(), b.ws_ptr, b.ws_bytes)
+    assert e.value.code == -3
+    # removing a task of one backbone leaves the other backbone's outputs untouched
+    ctx.unregister_task(a.task_ids_of[max(set(range(len(wl_a.tasks))) - set(wl_a.task_ids.tolist()), default=len(wl_a.tasks) - 1)]) \
+        if set(range(len(wl_a.tasks))) - set(wl_a.task_ids.tolist()) else None
+    for x, y in zip(b.forward_numpy(), alone_b):
+        assert np.array_equal(x, y)
