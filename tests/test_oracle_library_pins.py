@@ -279,6 +279,33 @@ def test_mlp_head_matches_torch_sequential_and_reduces_to_the_linear_head():
     assert (lin > 0).all() and np.allclose(lin, mlp_out, rtol=1e-13)
 
 
+def test_dense_head_is_a_1x1_convolution_over_tokens_and_reduces_to_the_last_token_head():
+    """SURVEY.md 8(f) NEXT-1, dense decoders: the head applied to every token row.  Pinned against
+    torch.nn.Conv1d(d, o, kernel_size=1) over the token axis (the standard segmentation-style linear decoder), against the
+    per-token scalar evaluation, and against the special case that its last row IS the last-token head."""
+    d, out, n = 24, 5, 9
+    r = _rng(70)
+    W = {"final.g": 1 + 0.1 * r.standard_normal(d), "final.b": 0.1 * r.standard_normal(d),
+         "task002.head.W": r.standard_normal((out, d)), "task002.head.b": r.standard_normal(out)}
+    bb = dict(norm="ln", norm_eps=1e-5)
+    h = r.standard_normal((n, d))
+    got = O.head_forward(bb, W.__getitem__, dict(id=2, adapters={}, head_kind="dense", head_out=out), h)
+    assert got.shape == (n * out,)
+    f = F.layer_norm(_t(h), (d,), _t(W["final.g"]), _t(W["final.b"]), 1e-5)
+    conv = torch.nn.Conv1d(d, out, kernel_size=1, **T64)
+    with torch.no_grad():
+        conv.weight.copy_(_t(W["task002.head.W"])[:, :, None]); conv.bias.copy_(_t(W["task002.head.b"]))
+        ref = conv(f.T[None])[0].T.numpy()                       # [n, out]
+    assert np.allclose(got.reshape(n, out), ref, rtol=1e-12, atol=1e-12)
+    fn = f.numpy()
+    for tok in (0, 4, n - 1):
+        for o in range(out):
+            want = sum(W["task002.head.W"][o, c] * fn[tok, c] for c in range(d)) + W["task002.head.b"][o]
+            assert abs(got[tok * out + o] - want) < 1e-12        # layout: token-major, then class
+    last = O.head_forward(bb, W.__getitem__, dict(id=2, adapters={}, head_kind="last", head_out=out), h)
+    assert np.allclose(got.reshape(n, out)[-1], last, rtol=1e-13, atol=1e-13)
+
+
 # ---------------------------------------------------------------- per-task input encoder (SURVEY.md 8(f) NEXT-1)
 def test_input_channel_combiner_is_a_1x1_convolution_and_reduces_to_the_plain_path():
     C, n_patches, pdim, d = 3, 6, 8, 12
