@@ -87,7 +87,7 @@ class AdapterSpec:
 @dataclass(frozen=True)
 class TaskSpec:
     adapters: Tuple[AdapterSpec, ...]
-    head_kind: str      # 'mean' | 'cls' | 'last' | 'flatten'
+    head_kind: str      # 'mean' | 'cls' | 'last' | 'flatten' | 'dense' (per token: output [n_i, head_out])
     head_out: int
     head_std: float = 0.02
     enc_channels: int = 0  # > 1: per-task input encoder, a linear channel combiner C -> 1 (Listing 2)
@@ -273,7 +273,8 @@ class Workload:
         return int(np.sum(self.lengths))
 
     def out_offsets(self) -> np.ndarray:
-        o = np.array([self.tasks[t].head_out for t in self.task_ids], dtype=np.int64)
+        o = np.array([self.tasks[t].head_out * (int(n) if self.tasks[t].head_kind == "dense" else 1)
+                      for t, n in zip(self.task_ids, self.lengths)], dtype=np.int64)
         return np.concatenate([[0], np.cumsum(o)])
 
 
@@ -341,7 +342,7 @@ def make_workload(cfg: str, *, n_layers: Optional[int] = None, batch: Optional[i
                   n_tasks: Optional[int] = None, dist: Optional[str] = None,
                   max_len: Optional[int] = None, adapters: bool = True,
                   seed_offset: int = 0, lora_std: float = 0.02, mlp_hidden: int = 0,
-                  enc_channels: int = 0) -> Workload:
+                  enc_channels: int = 0, dense_heads: bool = False) -> Workload:
     """Build the workload of a BASELINE.json config (cfg1..cfg5).
 
     Overrides give the reduced variants the parity tests use (fewer layers, smaller batch);
@@ -369,6 +370,9 @@ def make_workload(cfg: str, *, n_layers: Optional[int] = None, batch: Optional[i
         tasks = [replace(t, adapters=()) for t in tasks]
     if mlp_hidden:
         tasks = [t if t.head_kind == "flatten" else replace(t, head_hidden=mlp_hidden) for t in tasks]
+    if dense_heads:               # test variant (NEXT-1): every third task decodes EVERY token (dense / segmentation-style head)
+        tasks = [replace(t, head_kind="dense", head_hidden=0, head_std=0.02, head_out=min(t.head_out, 21)) if i % 3 == 1 else t
+                 for i, t in enumerate(tasks)]
     if enc_channels > 1:          # test variant (NEXT-1): every other task brings enc_channels input channels and a combiner
         tasks = [replace(t, enc_channels=enc_channels) if i % 2 == 0 else t for i, t in enumerate(tasks)]
     rng = _stream(seed, "task_ids")

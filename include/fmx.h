@@ -67,7 +67,10 @@ typedef enum { FMX_TGT_Q = 0, FMX_TGT_K, FMX_TGT_V, FMX_TGT_O, FMX_TGT_GATE, FMX
 typedef enum { FMX_HEAD_POOL_MEAN = 0,  /* mean over the request's n_i normed rows            */
                FMX_HEAD_POOL_CLS = 1,   /* row 0                                               */
                FMX_HEAD_POOL_LAST = 2,  /* row n_i - 1                                         */
-               FMX_HEAD_FLATTEN = 3     /* all rows, token-major then channel (fixed-length backbones only) */
+               FMX_HEAD_FLATTEN = 3,    /* all rows, token-major then channel (fixed-length backbones only) */
+               FMX_HEAD_DENSE = 4       /* dense (per-token) decoder, "dense decoders for ... detection, and
+                                           segmentation": the linear head is applied to EVERY normed token row; the request's
+                                           output is [n_i, head_out] row-major (token, then class).  d_feat = d_model; no MLP form */
 } fmx_head_kind;
 
 /* Backbone: a pre-norm transformer stack.  Plain data, no architecture enum.
@@ -173,6 +176,9 @@ int fmx_unregister_task(fmx_ctx *ctx, fmx_task_t task);
 /* HOST.  out_off[i] .. out_off[i+1] is request i's slice of the fp32 output buffer (prefix sum
  * of head_out in ORIGINAL request order); out_off has n_req + 1 entries. */
 int fmx_output_layout(fmx_ctx *ctx, const int32_t *task_ids, int32_t n_req, int64_t *out_off);
+/* The same with the requests' token counts (HOST int32 [n_req]): a FMX_HEAD_DENSE task contributes lengths[i] * head_out values.
+ * fmx_output_layout serves dense tasks only on fixed-length backbones (it uses tokens_per_request), else FMX_E_BAD_LENGTH. */
+int fmx_output_layout_len(fmx_ctx *ctx, const int32_t *task_ids, const int32_t *lengths, int32_t n_req, int64_t *out_off);
 
 /* Bytes of DEVICE workspace fmx_forward_mixed needs for up to max_req requests / max_tokens tokens (activations, segment
  * tables and the head scratch: the forward itself allocates nothing). */

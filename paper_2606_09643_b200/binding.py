@@ -21,7 +21,7 @@ ACT = {"gelu": 0, "relu": 1, "swiglu": 2}
 NORM = {"ln": 0, "rms": 1}
 INPUT_KIND = {"embedded": 0, "patch": 1, "tokens": 2}
 TARGET = {"q": 0, "k": 1, "v": 2, "o": 3, "gate": 4, "up": 5, "down": 6}
-HEAD_KIND = {"mean": 0, "cls": 1, "last": 2, "flatten": 3}
+HEAD_KIND = {"mean": 0, "cls": 1, "last": 2, "flatten": 3, "dense": 4}
 N_FAMILIES = 12
 MAX_TASKS = 1024
 
@@ -67,7 +67,7 @@ _lib = None
 
 # include/fmx.h (the public C ABI)
 EXPORTS = ["fmx_create", "fmx_destroy", "fmx_last_error", "fmx_version", "fmx_poll_error", "fmx_register_backbone", "fmx_register_task",
-           "fmx_unregister_task", "fmx_output_layout", "fmx_workspace_bytes", "fmx_host_workspace_bytes", "fmx_forward_mixed",
+           "fmx_unregister_task", "fmx_output_layout", "fmx_output_layout_len", "fmx_workspace_bytes", "fmx_host_workspace_bytes", "fmx_forward_mixed",
            "fmx_forward_mixed_host", "fmx_register_lm_head", "fmx_kv_cache_bytes", "fmx_prefill", "fmx_decode_step", "fmx_debug_get_segments", "fmx_task_slots", "fmx_profile_enable", "fmx_profile_select",
            "fmx_profile_read", "fmx_profile_family_name", "fmx_last_launch_count", "fmx_bfq_create", "fmx_bfq_destroy",
            "fmx_bfq_set_task", "fmx_bfq_enqueue", "fmx_bfq_next_batch", "fmx_bfq_complete", "fmx_bfq_stats", "fmx_bfq_peek"]
@@ -95,6 +95,7 @@ def load():
     lib.fmx_register_task.argtypes = [_vp, C.c_int32, C.POINTER(TaskDesc), i32p]
     lib.fmx_unregister_task.argtypes = [_vp, C.c_int32]
     lib.fmx_output_layout.argtypes = [_vp, i32p, C.c_int32, i64p]
+    lib.fmx_output_layout_len.argtypes = [_vp, i32p, i32p, C.c_int32, i64p]
     lib.fmx_workspace_bytes.argtypes = [_vp, C.c_int32, C.c_int32, C.c_int64, C.POINTER(C.c_size_t)]
     lib.fmx_host_workspace_bytes.argtypes = [_vp, C.c_int32, C.c_int32, C.c_int64, C.c_size_t, C.c_int64, C.POINTER(C.c_size_t)]
     lib.fmx_poll_error.argtypes = [_vp]
@@ -206,11 +207,16 @@ class Fmx:
     def task_slots(self):
         return self.lib.fmx_task_slots(self.h)
 
-    def output_layout(self, task_ids):
+    def output_layout(self, task_ids, lengths=None):
+        """lengths: needed when a task with a dense (per-token) head runs on a variable-length backbone."""
         ids = _i32(task_ids)
         off = np.zeros(len(ids) + 1, dtype=np.int64)
-        _check(self.lib.fmx_output_layout(self.h, ids.ctypes.data_as(C.POINTER(C.c_int32)), len(ids),
-                                          off.ctypes.data_as(C.POINTER(C.c_int64))))
+        p = C.POINTER(C.c_int32)
+        if lengths is None:
+            _check(self.lib.fmx_output_layout(self.h, ids.ctypes.data_as(p), len(ids), off.ctypes.data_as(C.POINTER(C.c_int64))))
+        else:
+            lens = _i32(lengths)
+            _check(self.lib.fmx_output_layout_len(self.h, ids.ctypes.data_as(p), lens.ctypes.data_as(p), len(ids), off.ctypes.data_as(C.POINTER(C.c_int64))))
         return off
 
     def workspace_bytes(self, bb, max_req, max_tokens):

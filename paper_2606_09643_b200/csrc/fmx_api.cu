@@ -113,10 +113,12 @@ struct Strm { cudaStream_t s; int pdl; };
 struct BatchShape {
   long long N = 0;
   int max_len = 0, max_out = 0, max_hidden = 0, max_out2 = 0, max_out_flat = 0, n_blk = 0;
-  bool any_flat = false, any_pooled = false;
+  bool any_flat = false, any_pooled = false, any_dense = false;
+  int max_out_dense = 0;
   bool operator==(const BatchShape &o) const {
     return N == o.N && max_len == o.max_len && max_out == o.max_out && max_hidden == o.max_hidden && max_out2 == o.max_out2 &&
-           max_out_flat == o.max_out_flat && any_flat == o.any_flat && any_pooled == o.any_pooled;
+           max_out_flat == o.max_out_flat && any_flat == o.any_flat && any_pooled == o.any_pooled && any_dense == o.any_dense &&
+           max_out_dense == o.max_out_dense;
   }
 };
 
@@ -878,10 +880,11 @@ int fmx_register_task(fmx_ctx *c, fmx_backbone_t h, const fmx_task_desc *desc, f
   const int L = d.n_layers;
   // ---- validate everything before touching state ----
   if (desc->n_adapters < 0 || desc->n_adapters > 7 || (desc->n_adapters && !desc->adapters)) return fmx_fail(FMX_E_INVALID_ARG, "register_task: bad n_adapters");
-  if (desc->head_kind < 0 || desc->head_kind > 3 || desc->head_out < 1 || !desc->head_W) return fmx_fail(FMX_E_INVALID_ARG, "register_task: bad head");
+  if (desc->head_kind < 0 || desc->head_kind > FMX_HEAD_DENSE || desc->head_out < 1 || !desc->head_W) return fmx_fail(FMX_E_INVALID_ARG, "register_task: bad head");
   if (desc->head_kind == FMX_HEAD_FLATTEN && d.tokens_per_request < 1) return fmx_fail(FMX_E_SHAPE, "register_task: FLATTEN head needs a fixed-length backbone");
   if (desc->head_hidden < 0 || desc->head_hidden > kMaxHeadHidden) return fmx_fail(FMX_E_SHAPE, "register_task: head_hidden %d not in [0,%d]", desc->head_hidden, kMaxHeadHidden);
-  if (desc->head_hidden > 0 && desc->head_kind == FMX_HEAD_FLATTEN) return fmx_fail(FMX_E_SHAPE, "register_task: an MLP head needs a pooled feature (mean / cls / last)");
+  if (desc->head_hidden > 0 && (desc->head_kind == FMX_HEAD_FLATTEN || desc->head_kind == FMX_HEAD_DENSE))
+    return fmx_fail(FMX_E_SHAPE, "register_task: an MLP head needs a pooled feature (mean / cls / last)");
   if (desc->head_hidden > 0 && !desc->head_W2) return fmx_fail(FMX_E_INVALID_ARG, "register_task: MLP head without head_W2");
   if (desc->enc_channels < 0 || desc->enc_channels > 16) return fmx_fail(FMX_E_SHAPE, "register_task: enc_channels %d not in [0,16]", desc->enc_channels);
   if (desc->enc_channels > 1 && (d.input_kind != FMX_INPUT_PATCH_LINEAR || d.img_c))
@@ -1009,20 +1012,30 @@ int fmx_unregister_task(fmx_ctx *c, fmx_task_t t) {
   return FMX_OK;
 }
 
-static int output_layout_locked(fmx_ctx *c, const int32_t *task_ids, int32_t n_req, int64_t *out_off);
+static int output_layout_locked(fmx_ctx *c, const int32_t *task_ids, const int32_t *lengths, int32_t n_req, int64_t *out_off);
 int fmx_output_layout(fmx_ctx *c, const int32_t *task_ids, int32_t n_req, int64_t *out_off) {
   if (!c || !out_off || (n_req > 0 && !task_ids) || n_req < 0) return fmx_fail(FMX_E_INVALID_ARG, "output_layout: bad argument");
   std::lock_guard<std::mutex> lk(c->mu);
-  return output_layout_locked(c, task_ids, n_req, out_off);
+  return output_layout_locked(c, task_ids, nullptr, n_req, out_off);
+}
+int fmx_output_layout_len(fmx_ctx *c, const int32_t *task_ids, const int32_t *lengths, int32_t n_req, int64_t *out_off) {
+  if (!c || !out_off || (n_req > 0 && (!task_ids || !lengths)) || n_req < 0) return fmx_fail(FMX_E_INVALID_ARG, "output_layout_len: bad argument");
+  std::lock_guard<std::mutex> lk(c->mu);
+  return output_layout_locked(c, task_ids, lengths, n_req, out_off);
 }
 
-static int output_layout_locked(fmx_ctx *c, const int32_t *task_ids, int32_t n_req, int64_t *out_off) {
+static int output_layout_locked(fmx_ctx *c, const int32_t *task_ids, const int32_t *lengths, int32_t n_req, int64_t *out_off) {
   int64_t run = 0;
   for (int i = 0; i < n_req; ++i) {
     const int t = task_ids[i];
     if (t < 0 || t >= FMX_MAX_TASKS || !c->tasks[t].live) return fmx_fail(FMX_E_UNKNOWN_TASK, "output_layout: request %d: task %d is not registered", i, t);
     out_off[i] = run;
-    run += c->tasks[t].head_out;
+    int64_t rows = 1;
+    if (c->tasks[t].head_kind == FMX_HEAD_DENSE) {                  // one output row per token
+      rows = lengths ? lengths[i] : get_bb(c, c->tasks[t].bb)->d.tokens_per_request;
+      if (rows < 1) return fmx_fail(FMX_E_BAD_LENGTH, "output_layout: request %d: a dense head on a variable-length backbone needs fmx_output_layout_len", i);
+    }
+    run += rows * c->tasks[t].head_out;
   }
   out_off[n_req] = run;
   return FMX_OK;
@@ -1070,6 +1083,7 @@ static int batch_shape(fmx_ctx *c, const Backbone &bb, const int32_t *task_ids, 
     bs.max_out = std::max(bs.max_out, tr.head_hidden > 0 ? tr.head_hidden : tr.head_out);   // first-layer width
     if (tr.head_hidden > 0) { bs.max_hidden = std::max(bs.max_hidden, tr.head_hidden); bs.max_out2 = std::max(bs.max_out2, tr.head_out); }
     if (tr.head_kind == FMX_HEAD_FLATTEN) { bs.any_flat = true; bs.max_out_flat = std::max(bs.max_out_flat, tr.head_out); }
+    else if (tr.head_kind == FMX_HEAD_DENSE) { bs.any_dense = true; bs.max_out_dense = std::max(bs.max_out_dense, tr.head_out); }
     else bs.any_pooled = true;
   }
   if (bs.N > (1ll << 24)) return fmx_fail(FMX_E_CAPACITY, "forward_mixed: %lld tokens > 2^24", bs.N);
@@ -1156,7 +1170,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     if (int e = stage_ids(c, w, task_ids, lengths, B, s, kv ? kv->slots : nullptr, kv ? kv->pos0 : nullptr)) return e;
   }
   SortArgs sa{};
-  sa.t = w.t; sa.B = B; sa.T = T; sa.n_tiles = w.n_tiles; sa.tile_rows = kPairRows; sa.task_head_out = c->d_task_head_out;
+  sa.t = w.t; sa.B = B; sa.T = T; sa.n_tiles = w.n_tiles; sa.tile_rows = kPairRows; sa.task_head_out = c->d_task_head_out; sa.task_head_kind = c->d_task_head_kind;
   sa.task_enc_ch = (d.input_kind == FMX_INPUT_PATCH_LINEAR && !d.img_c) ? c->d_task_enc_ch : nullptr;
   if (d.input_kind == FMX_INPUT_EMBEDDED) { sa.in_per_tok = d.d_model; sa.in_per_req = 0; }
   else if (d.input_kind == FMX_INPUT_TOKEN_IDS) { sa.in_per_tok = 1; sa.in_per_req = 0; }
@@ -1418,6 +1432,8 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     }
   }
 
+  if (bs.any_dense)                                      // dense (per-token) heads: one warp per token row of a dense task's request
+    LAUNCH(Lh, F_HEAD, (launch_k(head_dense_kernel, (Ni + 7) / 8, 256, 0, S, ha, Ni, (const int *)w.t.row_req, (const int *)w.t.row_pos)));
   if (max_hidden > 0)                                    // second layer of the MLP heads (the first wrote relu(W feat + b) to hid)
     LAUNCH(Lh, F_HEAD, (launch_k(head_mlp2_kernel, dim3(B, (max_out2 + 7) / 8), 256, 0, S, ha)));
   }
@@ -1561,7 +1577,7 @@ int fmx_forward_mixed_host(fmx_ctx *c, fmx_backbone_t h, const void *inputs_host
   if (n_req > FMX_MAX_REQUESTS) return fmx_fail(FMX_E_CAPACITY, "forward_mixed_host: %d requests > %d", n_req, FMX_MAX_REQUESTS);
   if (!inputs_host || !task_ids || !lengths || !outputs_host || !workspace) return fmx_fail(FMX_E_INVALID_ARG, "forward_mixed_host: NULL pointer");
   std::vector<int64_t> off(n_req + 1);
-  if (int e = output_layout_locked(c, task_ids, n_req, off.data())) return e;
+  if (int e = output_layout_locked(c, task_ids, lengths, n_req, off.data())) return e;
   long long N = 0;
   for (int i = 0; i < n_req; ++i) N += std::max(lengths[i], 0);
   if (N < 1 || N > (1ll << 24)) return fmx_fail(FMX_E_BAD_LENGTH, "forward_mixed_host: %lld tokens", N);

@@ -33,6 +33,7 @@ struct SortArgs {
   int tile_rows;                   // rows of a GEMM row tile (256: one CTA-pair tile)
   long long in_per_tok, in_per_req;  // packed-input elements per token / per request
   const int *task_head_out;        // [T]
+  const int *task_head_kind;       // [T] (a dense head writes one output row per token)
   const int *task_enc_ch;          // [T] input channels of the task's encoder (<= 1: none): in_per_req is per channel
 };
 
@@ -127,7 +128,7 @@ __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortAr
   for (int i = tid; i < B; i += blockDim.x) {
     const int ch = a.task_enc_ch ? max(a.task_enc_ch[t.task_ids[i]], 1) : 1;
     t.in_off[i] = (long long)t.lengths[i] * a.in_per_tok + a.in_per_req * ch;
-    t.out_off[i] = a.task_head_out[t.task_ids[i]];
+    t.out_off[i] = (long long)a.task_head_out[t.task_ids[i]] * (a.task_head_kind[t.task_ids[i]] == 4 ? t.lengths[i] : 1);
   }
   if (tid == 0) { t.in_off[B] = 0; t.out_off[B] = 0; }
   __syncthreads();
@@ -399,7 +400,7 @@ struct PoolArgs {
   const int *cu_tok, *task_sorted;
   const int *task_head_kind;       // [T]
   float *feat;                     // [B, d] fp32 pooled feature per SORTED request (mean / cls / last)
-  __nv_bfloat16 *Fn;               // [N, d] bf16 normed rows (written for FLATTEN requests only)
+  __nv_bfloat16 *Fn;               // [N, d] bf16 normed rows (written for FLATTEN / DENSE requests only)
   int d;
   float eps;
   int rms;
@@ -453,14 +454,14 @@ __global__ void __launch_bounds__(128) final_pool_kernel(const PoolArgs a) {
         const uint2 bb = reinterpret_cast<const uint2 *>(a.b)[c4];
         o0 += bf16_lo(bb.x); o1 += bf16_hi(bb.x); o2 += bf16_lo(bb.y); o3 += bf16_hi(bb.y);
       }
-      if (kind == 3) {
+      if (kind >= 3) {                                    // FLATTEN and DENSE heads read every normed row
         reinterpret_cast<uint2 *>(a.Fn + (size_t)(r0 + i) * d)[c4] = make_uint2(pack_bf16(o0, o1), pack_bf16(o2, o3));
       } else {
         accv[j].x += o0; accv[j].y += o1; accv[j].z += o2; accv[j].w += o3;
       }
     }
   }
-  if (kind == 3) return;
+  if (kind >= 3) return;
 #pragma unroll
   for (int j = 0; j < kVec; ++j) reinterpret_cast<float4 *>(s_part[warp])[j * 32 + lane] = accv[j];
   __syncthreads();
@@ -503,7 +504,7 @@ __global__ void __launch_bounds__(256) head_kernel(const HeadArgs a) {
   const int n_out = a.task_head_w1[t];
   if (o >= n_out) return;
   const int kind = a.task_head_kind[t];
-  if (kind == 3 && a.skip_flatten) return;
+  if ((kind == 3 && a.skip_flatten) || kind == 4) return;       // FLATTEN on the tensor-core path; dense heads have their own kernel
   const int r0 = a.cu_tok[p], n = a.cu_tok[p + 1] - r0;
   const long long K = kind == 3 ? (long long)n * a.d : a.d;
   const __nv_bfloat16 *w = a.task_head_W[t] + (size_t)o * K;
@@ -532,6 +533,35 @@ __global__ void __launch_bounds__(256) head_kernel(const HeadArgs a) {
     const float v = acc + (b ? __bfloat162float(b[o]) : 0.0f);
     if (a.task_head_W2[t]) a.hid[(size_t)p * a.ld_hid + o] = fmaxf(v, 0.0f);      // hidden layer of an MLP head
     else a.out[a.out_off[a.perm[p]] + o] = v;
+  }
+}
+
+// Dense (per-token) heads (FMX_HEAD_DENSE): y[token, :] = W_t f[token] + b_t for every token row of a dense task's request,
+// f = the final-normed row (bf16, written by final_pool_kernel).  One warp per token row: the row sits in registers, the
+// task's weight rows stream through (L1 / L2 hits: consecutive rows share the task), one shuffle reduction per output.
+// Written at out_off[request] + position * head_out in ORIGINAL request order.
+__global__ void __launch_bounds__(256) head_dense_kernel(const HeadArgs a, int N, const int *__restrict__ row_req, const int *__restrict__ row_pos) {
+  griddep_launch();
+  griddep_wait();
+  const int r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (r >= N) return;
+  const int p = row_req[r], t = a.task_sorted[p];
+  if (a.task_head_kind[t] != 4) return;
+  const int n_out = a.task_head_out[t];
+  const __nv_bfloat16 *f = a.Fn + (size_t)r * a.d, *W = a.task_head_W[t], *b = a.task_head_b[t];
+  float *dst = a.out + a.out_off[a.perm[p]] + (long long)row_pos[r] * n_out;
+  for (int o = 0; o < n_out; ++o) {
+    const __nv_bfloat16 *w = W + (size_t)o * a.d;
+    float acc = 0.0f;
+    for (int c = lane * 8; c < a.d; c += 256) {
+      const uint4 wv = *reinterpret_cast<const uint4 *>(w + c), fv = *reinterpret_cast<const uint4 *>(f + c);
+      acc += bf16_lo(wv.x) * bf16_lo(fv.x) + bf16_hi(wv.x) * bf16_hi(fv.x) + bf16_lo(wv.y) * bf16_lo(fv.y) +
+             bf16_hi(wv.y) * bf16_hi(fv.y) + bf16_lo(wv.z) * bf16_lo(fv.z) + bf16_hi(wv.z) * bf16_hi(fv.z) +
+             bf16_lo(wv.w) * bf16_lo(fv.w) + bf16_hi(wv.w) * bf16_hi(fv.w);
+    }
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
+    if (lane == 0) dst[o] = acc + (b ? __bfloat162float(b[o]) : 0.0f);
   }
 }
 

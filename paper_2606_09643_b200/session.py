@@ -241,7 +241,7 @@ class Session:
         lens = wl.lengths if lengths is None else lengths
         if self.inputs_dev is None:
             self.upload_inputs()
-        off = self.fmx.output_layout(ids)
+        off = self.fmx.output_layout(ids, lens)
         if self.out_dev is None or self.out_dev.numel() < int(off[-1]):
             self.out_dev = torch.empty(max(int(off[-1]), 1), dtype=torch.float32, device=self.dev)
         s = stream if stream is not None else torch.cuda.current_stream(self.dev)

@@ -531,6 +531,26 @@ def test_mlp_decoder_heads_parity(fmx_mod, cfg, kw):
     check_parity(y, G.oracle_outputs(wl), f"{cfg} MLP heads")
 
 
+@pytest.mark.parametrize("cfg,kw", [
+    ("cfg1", dict(dense_heads=True)),                                       # tiny encoder: dense next to mean-pooled heads
+    ("cfg3", dict(n_layers=2, batch=6, dense_heads=True)),                  # ViT shape: per-patch classes (segmentation-style), CLS heads beside
+    ("cfg4", dict(n_layers=2, batch=8, max_len=200, dense_heads=True)),     # variable lengths: ragged [n_i, o_t] outputs (fmx_output_layout_len)
+    ("cfg2", dict(n_layers=2, batch=24, dense_heads=True, mlp_hidden=64)),  # dense + FLATTEN + MLP heads in one batch
+])
+def test_dense_per_token_heads_parity(fmx_mod, cfg, kw):
+    """SURVEY.md 8(f) NEXT-1, dense decoders ("dense decoders for ... detection, and segmentation"): a task's linear
+    head applied to EVERY token of its requests; a request's output is [n_i, o_t]."""
+    wl = make_workload(cfg, **kw)
+    assert any(t.head_kind == "dense" for t in wl.tasks) and any(t.head_kind != "dense" for t in wl.tasks)
+    s = _session(fmx_mod, wl)
+    y = s.forward_numpy()
+    check_segments(s, wl)
+    assert np.array_equal(s.last_off, wl.out_offsets())
+    check_parity(y, G.oracle_outputs(wl), f"{cfg} dense heads")
+    dense_req = [i for i in range(wl.n_req) if wl.tasks[int(wl.task_ids[i])].head_kind == "dense"]
+    assert dense_req and all(len(y[i]) == int(wl.lengths[i]) * wl.tasks[int(wl.task_ids[i])].head_out for i in dense_req)
+
+
 def test_mlp_head_on_a_flatten_feature_is_rejected(fmx_mod):
     wl = make_workload("cfg2", n_layers=1, batch=4)
     s = _session(fmx_mod, wl)
