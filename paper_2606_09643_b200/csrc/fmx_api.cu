@@ -237,6 +237,9 @@ struct Workspace {
   int *slots = nullptr, *pos0 = nullptr, *row_slot = nullptr, *row_cpos = nullptr;
   bf16 *Fl = nullptr;                    // [B, d] final-normed last rows, sorted request order
   float *lm_scores = nullptr;            // [B, lm_vocab] sorted request order
+  float *splitk = nullptr;               // partials of the small-M (decode) projections: [k_split, 256, N] fp32, k_split * N <= splitk_cols
+  float *delta = nullptr;                // row-wise LoRA deltas of a projection group: [256, proj_max_n] fp32
+  float *rowu = nullptr;                 // row-wise shrink outputs [256, 3, 64] fp32
   int n_tiles = 0, n_blk_cap = 0;
   size_t bytes = 0;
 };
@@ -245,6 +248,11 @@ struct Workspace {
 // most kMaxHeadHidden wide (fmx_register_task enforces it); the FLATTEN-head partials get a fixed budget per request and
 // the launcher picks the K split that fits it.
 constexpr int kMaxHeadHidden = 4096;
+constexpr int kSplitMax = 16;            // most K splits of a small-M projection
+// widest projection output of a backbone (SwiGLU: gate and up interleaved), and the columns of the split-K partial buffer:
+// k_split * N <= (CTA pairs) * 256 by construction, or N itself when the projection is not split
+int proj_max_n(const Backbone &bb) { return std::max(std::max(bb.d_qkv, bb.d.d_model), (bb.d.act == FMX_ACT_SWIGLU ? 2 : 1) * bb.d.d_ffn); }
+size_t splitk_cols(const Backbone &bb) { return (size_t)std::max(80 * 256, proj_max_n(bb)); }
 constexpr size_t kHeadPartFloats = 2048;
 Workspace carve(const Backbone &bb, void *base, int B, long long N, int T) {
   Workspace w;
@@ -290,6 +298,9 @@ Workspace carve(const Backbone &bb, void *base, int B, long long N, int T) {
   if (bb.lm_head) {
     w.Fl = (bf16 *)take(sizeof(bf16) * (size_t)B * d.d_model);
     w.lm_scores = (float *)take(sizeof(float) * (size_t)B * bb.lm_vocab);
+    w.splitk = (float *)take(sizeof(float) * kPairRows * splitk_cols(bb));
+    w.delta = (float *)take(sizeof(float) * (size_t)kPairRows * proj_max_n(bb));
+    w.rowu = (float *)take(sizeof(float) * (size_t)kPairRows * 3 * 64);
   }
   w.bytes = off;
   return w;
@@ -394,7 +405,7 @@ bool pair_wide(const PairGemmParams &p) { return p.n_chunks % 2 == 0; }
 void launch_pair_gemm(fmx_ctx *c, Strm s, const PairGemmParams &p) {
   const int pairs = c->sm_count / 2;
   // fp32-output modes (residual reduce-add, embed) take the deep variant: one more pipeline stage, one staging buffer
-  const bool deep = c->o.deep_pipe && (p.mode == GM_RESID_F32 || p.mode == GM_EMBED_F32 || p.mode == GM_OUT_F32);
+  const bool deep = c->o.deep_pipe && (p.mode == GM_RESID_F32 || p.mode == GM_EMBED_F32 || p.mode == GM_OUT_F32 || p.k_split > 0);
   if (pair_wide(p)) {
     const int tiles = p.n_ptiles * (p.n_chunks / 2);
     // Wave quantisation: when the last wave would hold at most half as many tiles as there are pairs, its tiles are cut
@@ -402,13 +413,13 @@ void launch_pair_gemm(fmx_ctx *c, Strm s, const PairGemmParams &p) {
     PairGemmParams q = p;
     q.expand_wide = c->o.expand_wide;
     const int rem = tiles % pairs;
-    q.n_full = (c->o.half_tiles && p.mode != GM_OUT_BF16_SWIGLU && !p.rope_cs && tiles > pairs && rem > 0 && 2 * rem <= pairs) ? tiles - rem : -1;
-    const int items = q.n_full >= 0 ? q.n_full + 2 * rem : tiles;
+    q.n_full = (c->o.half_tiles && p.k_split == 0 && p.mode != GM_OUT_BF16_SWIGLU && !p.rope_cs && tiles > pairs && rem > 0 && 2 * rem <= pairs) ? tiles - rem : -1;
+    const int items = p.k_split > 0 ? tiles * p.k_split : (q.n_full >= 0 ? q.n_full + 2 * rem : tiles);
     const int grid = 2 * (p.n_sh > 0 ? pairs : std::min(items, pairs));
     if (deep) launch_k((pair_gemm_kernel<256, true>), grid, kGemmThreads, (pair_smem_bytes<256, true>()), s, q);
     else launch_k((pair_gemm_kernel<256, false>), grid, kGemmThreads, (pair_smem_bytes<256, false>()), s, q);
   } else {
-    const int tiles = p.n_ptiles * p.n_chunks;
+    const int tiles = p.n_ptiles * p.n_chunks * std::max(p.k_split, 1);
     const int grid = 2 * (p.n_sh > 0 ? pairs : std::min(tiles, pairs));
     if (deep) launch_k((pair_gemm_kernel<128, true>), grid, kGemmThreads, (pair_smem_bytes<128, true>()), s, p);
     else launch_k((pair_gemm_kernel<128, false>), grid, kGemmThreads, (pair_smem_bytes<128, false>()), s, p);
@@ -1216,6 +1227,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   // shrink over an input group: targets tgs[0..n) that currently have adapters; fills uslot_of[tg]
   int uslot_of[7] = {-1, -1, -1, -1, -1, -1, -1};
   auto shrink = [&](const CUtensorMap &amap, int K, const int *tgs, int n, int layer) -> int {
+    if (kv && kv->decode && w.splitk && w.n_tiles == 1) return FMX_OK;     // row_mode: row_shrink_kernel + row_expand_kernel do shrink and expand
     GemmParams p = sbase;
     p.mode = GM_SHRINK; p.amap = amap; p.K = K; p.out = w.U; p.ld_out = 192; p.n_tg = 0;
     for (int i = 0; i < n; ++i) {
@@ -1251,7 +1263,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   // items fit ONE wave of the persistent grid (cfg2: 73 blocks on 74 pairs, -0.4 ms per step); with more blocks the items'
   // low arithmetic intensity costs as much as the separate shrink launches (cfg3 / cfg4 / cfg5 at 92 tasks: +-0).
   const int n_blk_host = bs.n_blk;
-  const bool fuse_ok = c->o.shrink_fused && c->pairs_resident && (c->o.shrink_fused == 2 || n_blk_host <= c->sm_count / 2);
+  const bool fuse_ok = !(kv && kv->decode && w.splitk && w.n_tiles == 1) && c->o.shrink_fused && c->pairs_resident && (c->o.shrink_fused == 2 || n_blk_host <= c->sm_count / 2);
   if (fuse_ok) CU_OK(cudaMemsetAsync(w.u_flag, 0, sizeof(unsigned), s));
   // fusable: all CTA pairs of the persistent grid are co-resident (the expand steps spin on another pair's result) and
   // a 3-target group needs the 256-wide kernel
@@ -1260,9 +1272,59 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   };
 
   auto set_lora = [&](PairGemmParams &p, int src, int tg, int layer) {
+    if (kv && kv->decode && w.splitk && w.n_tiles == 1) return;
     if (bb.n_adapters[tg] > 0 && uslot_of[tg] >= 0) {
       p.lora_tgt[src] = tg; p.uslot[src] = uslot_of[tg]; p.lmap[src] = bb.mB[tg][layer]; p.has_lora = 1;
     }
+  };
+
+  // Decode iterations (one row tile of <= 256 rows, a few rows per task).  The segmented tensor-core LoRA path would load a 256-row U
+  // tile and a slab block per (tile, task) for a few rows of work, and a projection with few N tiles would be streamed by a handful
+  // of CTA pairs.  So in this mode (row_mode): (1) row_shrink_kernel + row_expand_kernel compute every row's LoRA delta on CUDA cores, (2) the GEMM runs
+  // without shrink / expand and stores raw fp32 partials, its K axis split over ~all CTA pairs when it has few tiles, (3)
+  // splitk_reduce_kernel adds the partials in split order, the delta and the bias and applies activation / SwiGLU / the residual
+  // update.  Every choice depends on the projection's shape only, never on the batch, so a request decodes to the same bits alone
+  // and in a batch.  (Prefill keeps the fused path: its outputs must not depend on the batch size.)
+  const bool row_mode = kv && kv->decode && w.splitk && w.n_tiles == 1;
+  auto project = [&](PairGemmParams &p, int family, __nv_bfloat16 *out_bf16, int ld_out, const __nv_bfloat16 *x, const int *tgs, int n_tg, int layer) -> int {
+    if (!row_mode) { LAUNCH(Lh, family, launch_pair_gemm(c, S, p)); return FMX_OK; }
+    const int Nn = p.n_chunks * 128;
+    bool any = false;
+    for (int i = 0; i < n_tg; ++i) any = any || bb.n_adapters[tgs[i]] > 0;
+    if (any) {
+      RowLoraArgs la{};
+      la.x = x; la.M = Ni; la.K = p.K; la.ld_delta = Nn; la.delta = w.delta; la.n_tg = n_tg; la.interleave2 = p.interleave2; la.Rcap = bb.Rcap;
+      la.row_req = w.t.row_req; la.task_sorted = w.t.task_sorted; la.task_coff = c->d_task_coff; la.task_trpad = c->d_task_trpad; la.task_scale = c->d_task_scale;
+      int col = 0;
+      for (int i = 0; i < n_tg; ++i) {
+        const int tg = tgs[i];
+        la.tg[i] = tg; la.d_out[i] = bb.dout[tg]; la.col0[i] = col; col += bb.dout[tg];
+        la.slabA[i] = bb.slabA[tg] ? bb.slabA[tg] + (size_t)layer * bb.Rcap * bb.din[tg] : nullptr;
+        la.slabB[i] = bb.slabB[tg] ? bb.slabB[tg] + (size_t)layer * bb.dout[tg] * bb.Rcap : nullptr;
+      }
+      int max_dout = 0;
+      for (int i = 0; i < n_tg; ++i) max_dout = std::max(max_dout, bb.dout[tgs[i]]);
+      LAUNCH(Lh, F_SHRINK, (launch_k(row_shrink_kernel, dim3(Ni, n_tg, FMX_MAX_RANK / 16), 256, 0, S, la, w.rowu)));
+      LAUNCH(Lh, F_SHRINK, (launch_k(row_expand_kernel, dim3(Ni, n_tg, (max_dout + kRowExpandCols - 1) / kRowExpandCols), 256, 0, S, la, (const float *)w.rowu)));
+    }
+    const int tiles = pair_wide(p) ? p.n_chunks / 2 : p.n_chunks, pairs = c->sm_count / 2, nK = (p.K + kBK - 1) / kBK;
+    int ks = 1, kbps = nK;
+    if (2 * tiles <= pairs) {
+      ks = std::min(kSplitMax, pairs / tiles);
+      kbps = (nK + ks - 1) / ks;
+      ks = (nK + kbps - 1) / kbps;
+    }
+    if (int e2 = encode_2d(c, &p.pmap, w.splitk, (uint64_t)ks * kPairRows, Nn, Nn, 128, true)) return e2;
+    p.k_split = ks; p.kb_per_split = kbps; p.split_rows = kPairRows;
+    LAUNCH(Lh, family, launch_pair_gemm(c, S, p));
+    SplitKReduceArgs ra{};
+    ra.partial = w.splitk; ra.k_split = ks; ra.split_rows = kPairRows; ra.M = Ni; ra.N = Nn; ra.delta = any ? w.delta : nullptr;
+    ra.mode = p.mode == GM_RESID_F32 ? 3 : p.mode == GM_OUT_BF16_SWIGLU ? 4 : p.mode == GM_OUT_BF16_GELU ? 1 : p.mode == GM_OUT_BF16_RELU ? 2 : 0;
+    for (int i = 0; i < 3; ++i) { ra.bias[i] = p.bias[i]; ra.src_end_col[i] = p.src_end[i] >= (1 << 20) ? (1 << 30) : p.src_end[i] * 128; }
+    ra.out_bf16 = out_bf16; ra.X = w.X; ra.ld_out = ld_out;
+    const long long n_thr = (long long)Ni * (ra.mode == 4 ? Nn / 8 : Nn / 4);
+    LAUNCH(Lh, family, (launch_k(splitk_reduce_kernel, (unsigned)((n_thr + 255) / 256), 256, 0, S, ra)));
+    return FMX_OK;
   };
 
   // ---- S2: embed ----
@@ -1308,10 +1370,11 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       set_lora(p, 0, FMX_TGT_Q, l); set_lora(p, 1, FMX_TGT_K, l); set_lora(p, 2, FMX_TGT_V, l);
       p.omap = oQKV;
       // head_dim 128: a 128-column chunk is one head, so RoPE is applied in the GEMM epilogue (fp32, one rounding)
-      rope_fused = c->o.rope_fused && d.rope_theta > 0 && d.head_dim == 128 && pair_wide(p);
+      // (a decode iteration splits the K axis of this GEMM and rotates q / k with rope_kernel after the reduction)
+      rope_fused = c->o.rope_fused && d.rope_theta > 0 && d.head_dim == 128 && pair_wide(p) && !(kv && kv->decode && w.splitk && w.n_tiles == 1);
       if (rope_fused) { p.rope_cs = bb.rope_cs_t; p.rope_ld = d.max_seq; p.rope_src_mask = 3; p.row_pos = rope_pos; }
       p.reverse = rev();
-      LAUNCH(Lh, F_GEMM_QKV, launch_pair_gemm(c, S, p));
+      if ((e = project(p, F_GEMM_QKV, w.QKV, bb.d_qkv, w.Xn, tgs, 3, l))) return e;
     }
     if (d.rope_theta > 0 && !rope_fused) {
       const int nh = d.n_q_heads + d.n_kv_heads;
@@ -1355,7 +1418,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       set_lora(p, 0, FMX_TGT_O, l);
       p.omap = oX;
       p.reverse = rev();
-      LAUNCH(Lh, F_GEMM_O, launch_pair_gemm(c, S, p));
+      if ((e = project(p, F_GEMM_O, nullptr, d.d_model, w.AttnO, tgs, 1, l))) return e;
     }
     LAUNCH(Lh, F_NORM, dispatch_norm(S, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm2_g[l], (const bf16 *)bb.norm2_b[l], Ni, d.norm_eps, rms, rev()));
     if (d.act == FMX_ACT_SWIGLU) {
@@ -1369,7 +1432,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       set_lora(p, 0, FMX_TGT_GATE, l); set_lora(p, 1, FMX_TGT_UP, l);
       p.omap = oHid;
       p.reverse = rev();
-      LAUNCH(Lh, F_GEMM_FFN_IN, launch_pair_gemm(c, S, p));
+      if ((e = project(p, F_GEMM_FFN_IN, w.Hid, d.d_ffn, w.Xn, tgs, 2, l))) return e;
     } else {
       const int tgs[1] = {FMX_TGT_UP};
       PairGemmParams p = base;
@@ -1380,7 +1443,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       set_lora(p, 0, FMX_TGT_UP, l);
       p.omap = oHid;
       p.reverse = rev();
-      LAUNCH(Lh, F_GEMM_FFN_IN, launch_pair_gemm(c, S, p));
+      if ((e = project(p, F_GEMM_FFN_IN, w.Hid, d.d_ffn, w.Xn, tgs, 1, l))) return e;
     }
     {
       const int tgs[1] = {FMX_TGT_DOWN};
@@ -1392,7 +1455,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       set_lora(p, 0, FMX_TGT_DOWN, l);
       p.omap = oX;
       p.reverse = rev();
-      LAUNCH(Lh, F_GEMM_FFN_OUT, launch_pair_gemm(c, S, p));
+      if ((e = project(p, F_GEMM_FFN_OUT, nullptr, d.d_model, w.Hid, tgs, 1, l))) return e;
     }
   }
   // ---- S4-S6 (skipped by a decode step that wants LM scores only) ----

@@ -1014,4 +1014,166 @@ __global__ void __launch_bounds__(256) scores_out_kernel(const float *__restrict
   }
 }
 
+// ============================================================================= small-M projections (decode): split-K reduce, row-wise shrink
+// Sums the fp32 partial accumulators of a split-K projection in split order (deterministic) and applies the epilogue the GEMM
+// would have applied: + bias of the column's weight source, then either the fp32 residual update (X += ...) or activation and a
+// bf16 store.  One thread per 4 consecutive columns of a row.
+struct SplitKReduceArgs {
+  const float *partial;            // [k_split, split_rows, N]
+  int k_split, split_rows, M, N;
+  int mode;                        // 0 bf16 out, 1 bf16 out + GeLU(erf), 2 bf16 out + ReLU, 3 fp32 residual X += ., 4 SwiGLU (N = 2 d_ffn,
+                                   //   128-column chunks alternate gate / up; bf16 out [M, N / 2])
+  const float *delta;              // [M, N] fp32 LoRA delta of the rows' tasks (row_expand_kernel), added before bias / activation; or NULL
+  const __nv_bfloat16 *bias[3];    // per weight source (NULL = none)
+  int src_end_col[3];              // first column AFTER source s (cumulative)
+  __nv_bfloat16 *out_bf16;
+  float *X;
+  int ld_out;
+};
+__device__ __forceinline__ float splitk_gelu(float x) { return 0.5f * x * (1.0f + erff(x * 0.70710678118654752f)); }
+__global__ void __launch_bounds__(256) splitk_reduce_kernel(const SplitKReduceArgs a) {
+  griddep_launch();
+  griddep_wait();
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  auto column_sum = [&](int r, int c) {
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int ks = 0; ks < a.k_split; ++ks) {
+      const float4 v = *reinterpret_cast<const float4 *>(a.partial + ((size_t)ks * a.split_rows + r) * a.N + c);
+      acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
+    }
+    if (a.delta) {
+      const float4 v = *reinterpret_cast<const float4 *>(a.delta + (size_t)r * a.N + c);
+      acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
+    }
+    return acc;
+  };
+  if (a.mode == 4) {                                    // SwiGLU: feature f = 128 q + j -> gate column 256 q + j, up column 256 q + 128 + j
+    const int f4 = a.N / 8;
+    if (idx >= (long long)a.M * f4) return;
+    const int r = (int)(idx / f4), f = (int)(idx - (long long)r * f4) * 4;
+    const int cg = (f >> 7) * 256 + (f & 127);
+    float4 g = column_sum(r, cg), u = column_sum(r, cg + 128);
+    if (const __nv_bfloat16 *b = a.bias[0]) { const uint2 bv = *reinterpret_cast<const uint2 *>(b + f); g.x += bf16_lo(bv.x); g.y += bf16_hi(bv.x); g.z += bf16_lo(bv.y); g.w += bf16_hi(bv.y); }
+    if (const __nv_bfloat16 *b = a.bias[1]) { const uint2 bv = *reinterpret_cast<const uint2 *>(b + f); u.x += bf16_lo(bv.x); u.y += bf16_hi(bv.x); u.z += bf16_lo(bv.y); u.w += bf16_hi(bv.y); }
+    auto silu = [](float x) { return x / (1.0f + __expf(-x)); };
+    *reinterpret_cast<uint2 *>(a.out_bf16 + (size_t)r * a.ld_out + f) =
+        make_uint2(pack_bf16(silu(g.x) * u.x, silu(g.y) * u.y), pack_bf16(silu(g.z) * u.z, silu(g.w) * u.w));
+    return;
+  }
+  const int n4 = a.N / 4;
+  if (idx >= (long long)a.M * n4) return;
+  const int r = (int)(idx / n4), c = (int)(idx - (long long)r * n4) * 4;
+  float4 acc = column_sum(r, c);
+  int s = 0, begin = 0;
+  if (c >= a.src_end_col[0]) { s = 1; begin = a.src_end_col[0]; }
+  if (c >= a.src_end_col[1]) { s = 2; begin = a.src_end_col[1]; }
+  if (const __nv_bfloat16 *b = a.bias[s]) {
+    const uint2 bv = *reinterpret_cast<const uint2 *>(b + (c - begin));
+    acc.x += bf16_lo(bv.x); acc.y += bf16_hi(bv.x); acc.z += bf16_lo(bv.y); acc.w += bf16_hi(bv.y);
+  }
+  if (a.mode == 3) {
+    float4 *x = reinterpret_cast<float4 *>(a.X + (size_t)r * a.ld_out + c);
+    float4 o = *x;
+    o.x += acc.x; o.y += acc.y; o.z += acc.z; o.w += acc.w;
+    *x = o;
+    return;
+  }
+  if (a.mode == 1) { acc.x = splitk_gelu(acc.x); acc.y = splitk_gelu(acc.y); acc.z = splitk_gelu(acc.z); acc.w = splitk_gelu(acc.w); }
+  else if (a.mode == 2) { acc.x = fmaxf(acc.x, 0.f); acc.y = fmaxf(acc.y, 0.f); acc.z = fmaxf(acc.z, 0.f); acc.w = fmaxf(acc.w, 0.f); }
+  *reinterpret_cast<uint2 *>(a.out_bf16 + (size_t)r * a.ld_out + c) = make_uint2(pack_bf16(acc.x, acc.y), pack_bf16(acc.z, acc.w));
+}
+
+// Row-wise LoRA for small batches (decode iterations): delta[row, cols of target] = s_t (x_row A_t^T) B_t^T for every target of an
+// input group, on CUDA cores (row_shrink_kernel, then row_expand_kernel).  With a handful of rows per task the segmented tensor-core path would
+// load a 256-row U tile and a slab block per (tile, task) for a few rows of work; here a row reads its own task's slab columns
+// once.  Rows whose task has no adapter on the target get zeros (the reduce kernel adds the delta unconditionally).
+struct RowLoraArgs {
+  const __nv_bfloat16 *x;          // [M, K] bf16 input of the projection group
+  int M, K, ld_delta;
+  float *delta;                    // [M, ld_delta] fp32
+  int n_tg;
+  int tg[3];                       // target ids
+  const __nv_bfloat16 *slabA[3];   // [Rcap, K] of this layer
+  const __nv_bfloat16 *slabB[3];   // [d_out, Rcap] of this layer
+  int d_out[3], col0[3];           // output width of the target, its first column in delta
+  int interleave2;                 // SwiGLU: target i owns the 128-column chunks 2 q + i (feature 128 q + j -> column 256 q + 128 i + j)
+  int Rcap;
+  const int *row_req, *task_sorted, *task_coff;
+  const unsigned char *task_trpad;
+  const float *task_scale;
+};
+// Both kernels are latency-bound (a few KB per thread block from scattered slab rows), so the work is cut fine - (row, target, 16 ranks)
+// and (row, target, 512 columns) - and every thread issues all its loads of a round before it uses any.
+constexpr int kRowExpandCols = 512;
+// u[row, i, j] = s_t <x_row, A_t[j, :]> for the 16 ranks j = 16 z .. of target i (fp32, [M, 3, 64])
+__global__ void __launch_bounds__(256) row_shrink_kernel(const RowLoraArgs a, float *__restrict__ u) {
+  griddep_launch();
+  griddep_wait();
+  const int r = blockIdx.x, i = blockIdx.y, z = blockIdx.z, tg = a.tg[i], warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int t = a.task_sorted[a.row_req[r]];
+  const int rp = a.task_trpad[t * 7 + tg];               // padded rank (multiple of 16); 0 = no adapter on this target
+  if (16 * z >= rp) return;
+  const float sc = a.task_scale[t * 7 + tg];
+  const __nv_bfloat16 *x = a.x + (size_t)r * a.K;
+  const int j0 = 16 * z + warp;                          // this warp: ranks j0 and j0 + 8
+  const __nv_bfloat16 *a0 = a.slabA[i] + (size_t)(a.task_coff[t] + j0) * a.K, *a1 = a0 + (size_t)8 * a.K;
+  float acc0 = 0.0f, acc1 = 0.0f;
+#pragma unroll 4
+  for (int k = lane * 8; k < a.K; k += 256) {
+    const uint4 xv = *reinterpret_cast<const uint4 *>(x + k), v0 = *reinterpret_cast<const uint4 *>(a0 + k), v1 = *reinterpret_cast<const uint4 *>(a1 + k);
+    acc0 += bf16_lo(v0.x) * bf16_lo(xv.x) + bf16_hi(v0.x) * bf16_hi(xv.x) + bf16_lo(v0.y) * bf16_lo(xv.y) + bf16_hi(v0.y) * bf16_hi(xv.y) +
+            bf16_lo(v0.z) * bf16_lo(xv.z) + bf16_hi(v0.z) * bf16_hi(xv.z) + bf16_lo(v0.w) * bf16_lo(xv.w) + bf16_hi(v0.w) * bf16_hi(xv.w);
+    acc1 += bf16_lo(v1.x) * bf16_lo(xv.x) + bf16_hi(v1.x) * bf16_hi(xv.x) + bf16_lo(v1.y) * bf16_lo(xv.y) + bf16_hi(v1.y) * bf16_hi(xv.y) +
+            bf16_lo(v1.z) * bf16_lo(xv.z) + bf16_hi(v1.z) * bf16_hi(xv.z) + bf16_lo(v1.w) * bf16_lo(xv.w) + bf16_hi(v1.w) * bf16_hi(xv.w);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { acc0 += __shfl_xor_sync(0xffffffffu, acc0, o); acc1 += __shfl_xor_sync(0xffffffffu, acc1, o); }
+  if (lane == 0) {
+    float *dst = u + ((size_t)r * 3 + i) * 64;
+    dst[j0] = acc0 * sc;
+    dst[j0 + 8] = acc1 * sc;
+  }
+}
+// delta[row, column of (target i, c)] = <u[row, i, :rp], B_t[c, :rp]> for 512 columns per CTA, two per thread
+__global__ void __launch_bounds__(256) row_expand_kernel(const RowLoraArgs a, const float *__restrict__ u) {
+  __shared__ float s_u[64];
+  griddep_launch();
+  griddep_wait();
+  const int r = blockIdx.x, i = blockIdx.y, tg = a.tg[i];
+  const int dout = a.d_out[i];
+  const int c_lo = blockIdx.z * kRowExpandCols;
+  if (c_lo >= dout) return;
+  const int t = a.task_sorted[a.row_req[r]];
+  const int rp = a.task_trpad[t * 7 + tg];
+  float *dst = a.delta + (size_t)r * a.ld_delta;
+  auto col_of = [&](int c) { return a.interleave2 ? ((c >> 7) * 256 + i * 128 + (c & 127)) : a.col0[i] + c; };
+  const int c0 = c_lo + threadIdx.x, c1 = c0 + 256;
+  if (rp == 0) {                                         // no adapter: the reduce kernel adds the delta unconditionally
+    if (c0 < dout) dst[col_of(c0)] = 0.0f;
+    if (c1 < dout) dst[col_of(c1)] = 0.0f;
+    return;
+  }
+  if (threadIdx.x < 64) s_u[threadIdx.x] = threadIdx.x < rp ? u[((size_t)r * 3 + i) * 64 + threadIdx.x] : 0.0f;
+  const __nv_bfloat16 *b0 = a.slabB[i] + (size_t)min(c0, dout - 1) * a.Rcap + a.task_coff[t];
+  const __nv_bfloat16 *b1 = a.slabB[i] + (size_t)min(c1, dout - 1) * a.Rcap + a.task_coff[t];
+  uint4 v0[8], v1[8];
+#pragma unroll
+  for (int q = 0; q < 8; ++q) {                          // every load of the thread is in flight before the first use
+    v0[q] = 8 * q < rp ? *reinterpret_cast<const uint4 *>(b0 + 8 * q) : make_uint4(0, 0, 0, 0);
+    v1[q] = 8 * q < rp ? *reinterpret_cast<const uint4 *>(b1 + 8 * q) : make_uint4(0, 0, 0, 0);
+  }
+  __syncthreads();
+  float acc0 = 0.0f, acc1 = 0.0f;
+#pragma unroll
+  for (int q = 0; q < 8; ++q) {
+    const float *uu = s_u + 8 * q;
+    acc0 += uu[0] * bf16_lo(v0[q].x) + uu[1] * bf16_hi(v0[q].x) + uu[2] * bf16_lo(v0[q].y) + uu[3] * bf16_hi(v0[q].y) +
+            uu[4] * bf16_lo(v0[q].z) + uu[5] * bf16_hi(v0[q].z) + uu[6] * bf16_lo(v0[q].w) + uu[7] * bf16_hi(v0[q].w);
+    acc1 += uu[0] * bf16_lo(v1[q].x) + uu[1] * bf16_hi(v1[q].x) + uu[2] * bf16_lo(v1[q].y) + uu[3] * bf16_hi(v1[q].y) +
+            uu[4] * bf16_lo(v1[q].z) + uu[5] * bf16_hi(v1[q].z) + uu[6] * bf16_lo(v1[q].w) + uu[7] * bf16_hi(v1[q].w);
+  }
+  if (c0 < dout) dst[col_of(c0)] = acc0;
+  if (c1 < dout) dst[col_of(c1)] = acc1;
+}
+
 }  // namespace fmx

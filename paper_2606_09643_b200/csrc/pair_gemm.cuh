@@ -87,6 +87,13 @@ struct PairGemmParams {
   unsigned *err;           // the context's device error word (bit 1: the fused-shrink wait timed out)
   unsigned u_epoch;        // 1, 2, ... over the fused launches of a forward: this launch's U is complete when the counter
                            // reaches 16 (epilogue warps of a pair) * n_blk * u_epoch
+  // ---- partial-output mode / split-K (small M: a weight matrix with few N tiles would be streamed by a handful of CTA pairs).
+  // k_split >= 1 (0 = off): work item
+  // (tile, ks) runs k-blocks [ks * kb_per_split, ...) of a whole tile and stores its fp32 partial accumulator with a plain TMA
+  // store to pmap rows [ks * split_rows + row, ...); splitk_reduce_kernel adds the partials in split order (deterministic) and
+  // applies the epilogue.  The LoRA expand steps belong to split 0.
+  CUtensorMap pmap;        // partials [k_split * split_rows, N] fp32, box {32, 128}
+  int k_split, kb_per_split, split_rows;
   const float2 *rope_cs;   // [64, rope_ld] (cos, sin), pair-index major: fused rotate-half RoPE for head_dim 128 (chunk = head), or NULL
   int rope_ld;             // positions per pair index (= max_seq)
   int rope_src_mask;       // bit s: source s (q | k | v) is rotated
@@ -210,7 +217,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
   griddep_launch();
   griddep_wait();
   const int n_u = p.n_sh > 0 ? *p.n_blk : 0;                // fused-shrink items come first in the work list
-  const int total_tiles = n_u + n_full + 2 * (whole_tiles - n_full);
+  const bool part = p.k_split > 0;                           // partial-output mode (k_split >= 1): item = tile * ksp + ks, whole tiles only, no shrink items
+  const int ksp = part ? p.k_split : 1;
+  const int total_tiles = part ? whole_tiles * ksp : n_u + n_full + 2 * (whole_tiles - n_full);
 
   if (warp == 0) {
     // ================================ TMA producer (both CTAs) ================================
@@ -220,7 +229,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
       int stage = 0; uint32_t phase = 0;
       bool u_ready = p.n_sh == 0;
       for (int tile = tile0; tile < total_tiles; tile += tile_step) {
-        if (tile < n_u) {
+        if (!part && tile < n_u) {
           // ---- fused-shrink item: block `tile` of the S1 table; B = the task's A-slab rows of each shrink target.
           // u_n = 256: CTA 0 loads targets 0, 1 and CTA 1 target 2; u_n = 128: CTA r loads target r.
           const int m0 = p.blk_tile[tile] * kPairRows + (int)rank * kBM;
@@ -240,7 +249,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
           continue;
         }
         int m_pt, c0, nch;
-        pair_decode<kCH>(p, tile - n_u, n_ntiles, n_full, m_pt, c0, nch);
+        const int ks = part ? tile % ksp : 0;
+        pair_decode<kCH>(p, part ? tile / ksp : tile - n_u, n_ntiles, n_full, m_pt, c0, nch);
+        const int kb0 = ks * p.kb_per_split, kb1 = part ? min(nK, kb0 + p.kb_per_split) : nK;
         const int m0 = m_pt * kPairRows + (int)rank * kBM;
         int bsrc, brow;
         const CUtensorMap *wm;
@@ -254,7 +265,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
           wm = kBN == 256 ? &p.wmap_h[bsrc] : &p.wmap[bsrc];
           stage_tx = kATileBytes + 64 * kBK * 2;
         }
-        for (int kb = 0; kb < nK; ++kb) {
+        for (int kb = kb0; kb < kb1; ++kb) {
           mbar_wait(&empty_bar[stage], phase ^ 1);
           uint8_t *sa = smem + stage * kStageBytes, *sb = sa + kATileBytes;
           const uint32_t fb = mapa_shared(smem_u32(&full_bar[stage]), 0);
@@ -263,7 +274,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
           tma_load_2d_2sm(sb, wm, fb, kb * kBK, brow);
           if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
-        if (p.has_lora) {
+        if (p.has_lora && ks == 0) {
           const int b0 = p.tile_blk_off[m_pt], b1 = p.tile_blk_off[m_pt + 1];
           // Both chunks of a whole tile from the same source (q | k | v, o, up, down; not SwiGLU's gate / up pairs) read the
           // SAME U columns: one expand step then covers the tile (U loaded once, each CTA its chunk's 128 slab rows, N = 256).
@@ -314,24 +325,26 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
       constexpr uint32_t idesc_lora = make_idesc_bf16(kPairRows, kChunk);
       for (int tile = tile0; tile < total_tiles; tile += tile_step) {
         int m_pt = 0, c0 = 0, nch = 0;
-        const bool u_item = tile < n_u;
-        if (!u_item) pair_decode<kCH>(p, tile - n_u, n_ntiles, n_full, m_pt, c0, nch);
+        const bool u_item = !part && tile < n_u;
+        const int ks = part ? tile % ksp : 0;
+        if (!u_item) pair_decode<kCH>(p, part ? tile / ksp : tile - n_u, n_ntiles, n_full, m_pt, c0, nch);
+        const int kb0 = ks * p.kb_per_split, kb1 = part ? min(nK, kb0 + p.kb_per_split) : nK;
         const uint32_t idesc_main = u_item ? (u_n == 256 ? make_idesc_bf16(kPairRows, 256) : idesc_lora) : (nch == kCH ? idesc_whole : idesc_lora);
         mbar_wait_cluster(&tempty_bar[acc], accphase ^ 1);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + acc * kAccStride;
-        for (int kb = 0; kb < nK; ++kb) {
+        for (int kb = kb0; kb < kb1; ++kb) {
           mbar_wait_cluster(&full_bar[stage], phase);
           tc_fence_after();
           const uint32_t sa = smem_u32(smem + stage * kStageBytes);
           const uint64_t adesc = make_smem_desc_sw128(sa), bdesc = make_smem_desc_sw128(sa + kATileBytes);
 #pragma unroll
           for (int k = 0; k < kBK / 16; ++k)
-            umma_bf16_2sm(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc_main, (kb | k) != 0);
+            umma_bf16_2sm(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc_main, ((kb - kb0) | k) != 0);
           umma_commit_2sm(&empty_bar[stage], 3);
           if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
-        if (p.has_lora && !u_item) {
+        if (p.has_lora && !u_item && ks == 0) {
           const int b0 = p.tile_blk_off[m_pt], b1 = p.tile_blk_off[m_pt + 1];
           const bool wide = pair_expand_wide<kBN>(p, c0, nch);
           for (int c = 0; c < (wide ? 1 : nch); ++c) {
@@ -367,9 +380,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
     uint8_t *stg = staging + wg * (kBufs * 16384);
     int box_seq = 0;
     int acc = 0; uint32_t accphase = 0;
-    const int mode = p.mode;
+    const int mode = part ? (int)GM_OUT_F32 : p.mode;          // partial mode: every item stores its raw fp32 partial
     for (int tile = tile0; tile < total_tiles; tile += tile_step) {
-      if (tile < n_u) {
+      if (!part && tile < n_u) {
         // ---- fused-shrink item: U_blk[row, slot*64 + j] = bf16(s_t · acc), rows outside the block's task zeroed ----
         const int b = tile, t = p.blk_task[b];
         const int rp = (int)rank * kBM + r_in_tile;             // row within the 256-row tile
@@ -403,7 +416,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
         continue;
       }
       int m_pt, c0, nch;
-      pair_decode<kCH>(p, tile - n_u, n_ntiles, n_full, m_pt, c0, nch);
+      const int ks = part ? tile % ksp : 0;
+      pair_decode<kCH>(p, part ? tile / ksp : tile - n_u, n_ntiles, n_full, m_pt, c0, nch);
       const int bn = nch * kChunk;                              // columns of this work item (a half tile has 128)
       const int row0_cta = m_pt * kPairRows + (int)rank * kBM;
       const int row = row0_cta + r_in_tile;
@@ -559,7 +573,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
           float f[32];
 #pragma unroll
           for (int e = 0; e < 32; ++e) f[e] = __uint_as_float(v[e]);
-          const __nv_bfloat16 *bias = p.bias[s];
+          const __nv_bfloat16 *bias = part ? nullptr : p.bias[s];        // partial mode: the reduce kernel adds the bias once
           if (bias) {
             const uint4 *bp = reinterpret_cast<const uint4 *>(bias + n_src);
 #pragma unroll
@@ -586,7 +600,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1) pai
           fence_proxy_async();
           named_bar_sync(bar_id, 128);
           if (issuer) {
-            if (mode == GM_RESID_F32) tma_reduce_add_2d(&p.omap, buf, n_out, row0_cta);
+            if (part) tma_store_2d(&p.pmap, buf, n_out, ks * p.split_rows + row0_cta);
+            else if (mode == GM_RESID_F32) tma_reduce_add_2d(&p.omap, buf, n_out, row0_cta);
             else tma_store_2d(&p.omap, buf, n_out, row0_cta);
             bulk_commit();
           }
