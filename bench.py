@@ -513,7 +513,9 @@ def run_headline(args, rank, local_rank, world):
                                            "on q/k/v/o and a forecast head (reading 19); adapter_free: one head-only task.  north_star target: "
                                            "vs_single_task >= 0.90"}
     per = {}
-    if not args.no_per_config:
+    if world > 1:
+        line["config"]["per_config"] = "skipped under torchrun (N > 1): the scaling run needs the headline only; run N = 1 for the other configs"
+    elif not args.no_per_config:
         for cfg, st in (("cfg2", short), ("cfg3", short), ("cfg4", max(3, short // 2))):
             wl2 = make_workload(cfg)
             l2, s2 = measure(args, wl2, rank, local_rank, world, full=False, steps=st, label=cfg)

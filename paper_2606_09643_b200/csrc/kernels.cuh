@@ -865,9 +865,12 @@ __global__ void __launch_bounds__(256) decode_attention_kernel(const __nv_bfloat
 #pragma unroll
     for (int g = 0; g < G; ++g) s[g] = 0.0f;
     const uint4 *kp = reinterpret_cast<const uint4 *>(K + (long long)(valid ? key : k0) * a.d_kv);
-#pragma unroll 4
+    uint4 kv[DH / 8];
+#pragma unroll
+    for (int v = 0; v < DH / 8; ++v) kv[v] = kp[v];             // the whole key row in flight before the first use
+#pragma unroll
     for (int v = 0; v < DH / 8; ++v) {
-      const uint4 u = kp[v];
+      const uint4 u = kv[v];
       const float kf[8] = {bf16_lo(u.x), bf16_hi(u.x), bf16_lo(u.y), bf16_hi(u.y), bf16_lo(u.z), bf16_hi(u.z), bf16_lo(u.w), bf16_hi(u.w)};
 #pragma unroll
       for (int g = 0; g < G; ++g) {
@@ -900,16 +903,18 @@ __global__ void __launch_bounds__(256) decode_attention_kernel(const __nv_bfloat
     // ---- O += P V: the lane owns VPT dims of every head's output ----
     const int nk = min(32, n_keys - k0);
     const __nv_bfloat16 *vp = V + (long long)k0 * a.d_kv + lane * VPT;
-    for (int kk = 0; kk < nk; kk += 4) {
-      float vf[4][VPT];
+    for (int kk = 0; kk < nk; kk += 8) {                         // eight V rows in flight at a time
+      float vf[8][VPT];
 #pragma unroll
-      for (int j = 0; j < 4; ++j) load_bf16_vec<VPT>(vp + (long long)min(kk + j, nk - 1) * a.d_kv, vf[j]);
+      for (int j = 0; j < 8; ++j) load_bf16_vec<VPT>(vp + (long long)min(kk + j, nk - 1) * a.d_kv, vf[j]);
 #pragma unroll
       for (int g = 0; g < G; ++g) {
         if (g >= group) break;
-        const float4 pw = *reinterpret_cast<const float4 *>(&s_p[warp][g][kk]);     // invalid keys of the chunk hold 0
+        const float4 pa = *reinterpret_cast<const float4 *>(&s_p[warp][g][kk]), pb = *reinterpret_cast<const float4 *>(&s_p[warp][g][kk + 4]);   // invalid keys of the chunk hold 0
 #pragma unroll
-        for (int e = 0; e < VPT; ++e) acc[g][e] = fmaf(pw.x, vf[0][e], fmaf(pw.y, vf[1][e], fmaf(pw.z, vf[2][e], fmaf(pw.w, vf[3][e], acc[g][e]))));
+        for (int e = 0; e < VPT; ++e)
+          acc[g][e] = fmaf(pa.x, vf[0][e], fmaf(pa.y, vf[1][e], fmaf(pa.z, vf[2][e], fmaf(pa.w, vf[3][e],
+                      fmaf(pb.x, vf[4][e], fmaf(pb.y, vf[5][e], fmaf(pb.z, vf[6][e], fmaf(pb.w, vf[7][e], acc[g][e]))))))));
       }
     }
     __syncwarp();
