@@ -528,6 +528,26 @@ def run_headline(args, rank, local_rank, world):
     return line
 
 
+def run_decode(args, rank, local_rank, world):
+    """NEXT-3 only: decode iterations on the cfg4 backbone (64 sequences, 92 tasks); the line's value is tokens per second."""
+    import torch
+    from fmx_workloads import make_workload
+    from paper_2606_09643_b200.session import Session
+    torch.cuda.set_device(local_rank)
+    wl = make_workload("cfg4")
+    with torch.cuda.stream(torch.cuda.Stream(torch.device("cuda", local_rank))):
+        sess = Session(wl, device=local_rank)
+        for k, v in (o.split("=") for o in args.opt):
+            sess.fmx.set_option(k, int(v))
+        d = measure_decode(sess, wl, steps=args.steps, warm=max(3, args.warmup))
+        sess.fmx.destroy()
+    return {"metric": "decode tokens per second, mixed-task batch", "value": d["tokens_per_s"], "unit": "tokens/s", "n_gpus": 1, "steps": args.steps,
+            "warmup": max(3, args.warmup), "ms_per_step": d["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "bf16", "data": "synthetic", "config": {"workload": "cfg4 decode: 64 sequences, 92 registered tasks, prompts cut to leave room in the cache",
+                                                             "options": args.opt}, "gpu_launches": d["launches_per_step"] * args.steps,
+            "roofline": d["roofline"], "decode": d}
+
+
 def run_sweep5(args, rank, local_rank, world):
     """BASELINE.json configs[4] in full: T x distribution -> samples/s, ratio to the single-task batch and to the adapter-free one."""
     from fmx_workloads import make_workload
@@ -564,7 +584,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="fmx", choices=["fmx", "reference"])
-    ap.add_argument("--workload", default="headline", choices=["headline", "cfg2", "cfg3", "cfg4", "cfg5", "sweep5"],
+    ap.add_argument("--workload", default="headline", choices=["headline", "cfg2", "cfg3", "cfg4", "cfg5", "sweep5", "decode"],
                     help="headline (default): configs[4] at 92 tasks + its single-task / adapter-free references + per_config cfg2 / cfg3 / cfg4")
     ap.add_argument("--no-per-config", action="store_true", help="headline: skip the cfg2 / cfg3 / cfg4 lines")
     ap.add_argument("--tasks", type=int, default=92, help="cfg5: number of co-batched tasks")
@@ -591,6 +611,8 @@ def main():
         line = run_sweep5(args, rank, local_rank, world)
     elif args.workload == "headline":
         line = run_headline(args, rank, local_rank, world)
+    elif args.workload == "decode":
+        line = run_decode(args, rank, local_rank, world)
     else:
         wl = build_workload(args)
         line, sess = measure(args, wl, rank, local_rank, world)

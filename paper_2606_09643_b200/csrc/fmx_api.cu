@@ -103,6 +103,7 @@ struct Opts {
   int attn_short = 2;     // 0: generic kernel, 1: pipelined mma.sync kernel, 2: tcgen05 head-pair kernel where it applies
   int graph = 1;
   int attn_impl = FMX_ATTN_AUTO;
+  int decode_fork = 1;    // decode iterations: row-wise LoRA kernels on the auxiliary stream beside the projection GEMM
 };
 
 // A launch target: the stream and whether the launch carries the programmatic-stream-serialization attribute.
@@ -159,6 +160,8 @@ struct fmx_ctx {
   // retirement stream: frees of what forwards in flight may still read happen here, after those forwards (see retire())
   cudaStream_t side2 = nullptr;
   cudaEvent_t side_ev = nullptr, retire_ev = nullptr;
+  cudaStream_t aux = nullptr;              // decode iterations fork the row-wise LoRA kernels onto this stream (FMX_OPT_DECODE_FORK)
+  cudaEvent_t fork_ev = nullptr, join_ev = nullptr;
   unsigned long long retire_seq = 0, retire_done = 0;   // retirements issued / known complete
   struct TaskStage { int coff, head_kind, head_out, w1, enc_ch; unsigned char trpad[8]; float scale[7]; const void *ptr[6]; };
   TaskStage *h_task_stage = nullptr;       // pinned
@@ -239,7 +242,9 @@ struct Workspace {
   float *lm_scores = nullptr;            // [B, lm_vocab] sorted request order
   float *splitk = nullptr;               // partials of the small-M (decode) projections: [k_split, 256, N] fp32, k_split * N <= splitk_cols
   float *delta = nullptr;                // row-wise LoRA deltas of a projection group: [256, proj_max_n] fp32
-  float *rowu = nullptr;                 // row-wise shrink outputs [256, 3, 64] fp32
+  float *dec_part = nullptr;             // decode attention: per (request, q head, chunk) partial (o, m, l)
+  unsigned *dec_cnt = nullptr;           // decode attention: chunks finished per (request, KV head)
+  float *rowu = nullptr;                 // row-wise shrink partial sums [nkc, 256, 3, 64] fp32 (nkc = 512-column chunks of the widest input)
   int n_tiles = 0, n_blk_cap = 0;
   size_t bytes = 0;
 };
@@ -254,6 +259,11 @@ constexpr int kSplitMax = 16;            // most K splits of a small-M projectio
 int proj_max_n(const Backbone &bb) { return std::max(std::max(bb.d_qkv, bb.d.d_model), (bb.d.act == FMX_ACT_SWIGLU ? 2 : 1) * bb.d.d_ffn); }
 size_t splitk_cols(const Backbone &bb) { return (size_t)std::max(80 * 256, proj_max_n(bb)); }
 constexpr size_t kHeadPartFloats = 2048;
+int row_shrink_chunks(int K) { return (K + kRowShrinkK - 1) / kRowShrinkK; }
+// Decode attention splits a sequence's cached positions into chunks of kc_keys (a property of the backbone: the longest sequence
+// has at most 16 chunks), one CTA each.
+int dec_chunk_keys(int max_seq) { int kc = kDecKeys; while (kc * 16 < max_seq) kc *= 2; return kc; }
+int dec_chunks_cap(int max_seq) { const int kc = dec_chunk_keys(max_seq); return (max_seq + kc - 1) / kc; }
 Workspace carve(const Backbone &bb, void *base, int B, long long N, int T) {
   Workspace w;
   uint8_t *p = static_cast<uint8_t *>(base);
@@ -300,7 +310,9 @@ Workspace carve(const Backbone &bb, void *base, int B, long long N, int T) {
     w.lm_scores = (float *)take(sizeof(float) * (size_t)B * bb.lm_vocab);
     w.splitk = (float *)take(sizeof(float) * kPairRows * splitk_cols(bb));
     w.delta = (float *)take(sizeof(float) * (size_t)kPairRows * proj_max_n(bb));
-    w.rowu = (float *)take(sizeof(float) * (size_t)kPairRows * 3 * 64);
+    w.dec_part = (float *)take(sizeof(float) * (size_t)B * d.n_q_heads * dec_chunks_cap(d.max_seq) * (d.head_dim + 2));
+    w.dec_cnt = (unsigned *)take(sizeof(unsigned) * (size_t)B * d.n_kv_heads);
+    w.rowu = (float *)take(sizeof(float) * (size_t)row_shrink_chunks(std::max({d.d_model, d.d_ffn, bb.d_q})) * kPairRows * 3 * 64);
   }
   w.bytes = off;
   return w;
@@ -485,6 +497,9 @@ int set_kernel_attrs() {
   CU_OK((cudaFuncSetAttribute(pair_gemm_kernel<256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<256, true>())));
   CU_OK((cudaFuncSetAttribute(pair_gemm_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<128, false>())));
   CU_OK((cudaFuncSetAttribute(pair_gemm_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<128, true>())));
+  CU_OK((cudaFuncSetAttribute(decode_attention_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, decode_attention_smem<32>())));
+  CU_OK((cudaFuncSetAttribute(decode_attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, decode_attention_smem<64>())));
+  CU_OK((cudaFuncSetAttribute(decode_attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, decode_attention_smem<128>())));
   CU_OK((cudaFuncSetAttribute(shrink_kernel<4, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<4, 3>())));
   CU_OK((cudaFuncSetAttribute(shrink_kernel<5, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<5, 3>())));
   CU_OK((cudaFuncSetAttribute(shrink_kernel<6, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, shrink_smem_bytes<6, 2>())));
@@ -734,6 +749,9 @@ int fmx_create(fmx_ctx **out, int device_ordinal) {
   CU_OK(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
   CU_OK(cudaStreamCreateWithFlags(&c->side2, cudaStreamNonBlocking));
   CU_OK(cudaEventCreateWithFlags(&c->side_ev, cudaEventDisableTiming));
+  CU_OK(cudaStreamCreateWithFlags(&c->aux, cudaStreamNonBlocking));
+  CU_OK(cudaEventCreateWithFlags(&c->fork_ev, cudaEventDisableTiming));
+  CU_OK(cudaEventCreateWithFlags(&c->join_ev, cudaEventDisableTiming));
   CU_OK(cudaEventCreateWithFlags(&c->retire_ev, cudaEventDisableTiming));
   CU_OK(cudaMallocHost(&c->h_task_stage, sizeof(fmx_ctx::TaskStage)));
   CU_OK(cudaHostAlloc(&c->h_err, sizeof(unsigned), cudaHostAllocMapped));
@@ -781,6 +799,9 @@ int fmx_destroy(fmx_ctx *c) {
   cudaFreeHost(c->h_task_stage);
   if (c->side_ev) cudaEventDestroy(c->side_ev);
   if (c->retire_ev) cudaEventDestroy(c->retire_ev);
+  if (c->fork_ev) cudaEventDestroy(c->fork_ev);
+  if (c->join_ev) cudaEventDestroy(c->join_ev);
+  if (c->aux) cudaStreamDestroy(c->aux);
   if (c->side) cudaStreamDestroy(c->side);
   if (c->side2) cudaStreamDestroy(c->side2);
   delete c;
@@ -1265,6 +1286,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   const int n_blk_host = bs.n_blk;
   const bool fuse_ok = !(kv && kv->decode && w.splitk && w.n_tiles == 1) && c->o.shrink_fused && c->pairs_resident && (c->o.shrink_fused == 2 || n_blk_host <= c->sm_count / 2);
   if (fuse_ok) CU_OK(cudaMemsetAsync(w.u_flag, 0, sizeof(unsigned), s));
+  if (kv && kv->decode) CU_OK(cudaMemsetAsync(w.dec_cnt, 0, sizeof(unsigned) * (size_t)B * d.n_kv_heads, s));   // the last chunk's CTA resets its counter; this covers an aborted launch
   // fusable: all CTA pairs of the persistent grid are co-resident (the expand steps spin on another pair's result) and
   // a 3-target group needs the 256-wide kernel
   auto can_fuse = [&](const PairGemmParams &p, int n_targets) {
@@ -1291,6 +1313,8 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     const int Nn = p.n_chunks * 128;
     bool any = false;
     for (int i = 0; i < n_tg; ++i) any = any || bb.n_adapters[tgs[i]] > 0;
+    // the LoRA kernels and the GEMM are independent until the reduction: fork them (not while per-launch profiling events are on)
+    const bool fork = any && c->o.decode_fork && !c->prof_on;
     if (any) {
       RowLoraArgs la{};
       la.x = x; la.M = Ni; la.K = p.K; la.ld_delta = Nn; la.delta = w.delta; la.n_tg = n_tg; la.interleave2 = p.interleave2; la.Rcap = bb.Rcap;
@@ -1304,8 +1328,12 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       }
       int max_dout = 0;
       for (int i = 0; i < n_tg; ++i) max_dout = std::max(max_dout, bb.dout[tgs[i]]);
-      LAUNCH(Lh, F_SHRINK, (launch_k(row_shrink_kernel, dim3(Ni, n_tg, FMX_MAX_RANK / 16), 256, 0, S, la, w.rowu)));
-      LAUNCH(Lh, F_SHRINK, (launch_k(row_expand_kernel, dim3(Ni, n_tg, (max_dout + kRowExpandCols - 1) / kRowExpandCols), 256, 0, S, la, (const float *)w.rowu)));
+      const int nkc = row_shrink_chunks(p.K);
+      const Strm SL = fork ? Strm{c->aux, 0} : S;
+      if (fork) { CU_OK(cudaEventRecord(c->fork_ev, s)); CU_OK(cudaStreamWaitEvent(c->aux, c->fork_ev, 0)); }
+      LAUNCH(Lh, F_SHRINK, (launch_k(row_shrink_kernel, dim3(Ni, n_tg, nkc), 256, 0, SL, la, w.rowu)));
+      LAUNCH(Lh, F_SHRINK, (launch_k(row_expand_kernel, dim3(Ni, n_tg, (max_dout + kRowExpandCols - 1) / kRowExpandCols), 256, 0, SL, la, (const float *)w.rowu, nkc)));
+      if (fork) CU_OK(cudaEventRecord(c->join_ev, c->aux));
     }
     const int tiles = pair_wide(p) ? p.n_chunks / 2 : p.n_chunks, pairs = c->sm_count / 2, nK = (p.K + kBK - 1) / kBK;
     int ks = 1, kbps = nK;
@@ -1317,6 +1345,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     if (int e2 = encode_2d(c, &p.pmap, w.splitk, (uint64_t)ks * kPairRows, Nn, Nn, 128, true)) return e2;
     p.k_split = ks; p.kb_per_split = kbps; p.split_rows = kPairRows;
     LAUNCH(Lh, family, launch_pair_gemm(c, S, p));
+    if (fork) CU_OK(cudaStreamWaitEvent(s, c->join_ev, 0));
     SplitKReduceArgs ra{};
     ra.partial = w.splitk; ra.k_split = ks; ra.split_rows = kPairRows; ra.M = Ni; ra.N = Nn; ra.delta = any ? w.delta : nullptr;
     ra.mode = p.mode == GM_RESID_F32 ? 3 : p.mode == GM_OUT_BF16_SWIGLU ? 4 : p.mode == GM_OUT_BF16_GELU ? 1 : p.mode == GM_OUT_BF16_RELU ? 2 : 0;
@@ -1383,10 +1412,13 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     }
     if (kv) LAUNCH(Lh, F_ATTN, (launch_k(kv_append_kernel, (Ni + 7) / 8, 256, 0, S, (const bf16 *)w.QKV, bb.d_qkv, bb.d_q, bb.d_q + bb.d_kv, Ni, l, ka)));
     if (kv && kv->decode) {
-      dim3 grid(B, d.n_kv_heads);
-      if (d.head_dim == 32) LAUNCH(Lh, F_ATTN, (launch_k(decode_attention_kernel<32>, grid, 256, 0, S, (const bf16 *)w.QKV, bb.d_qkv, w.AttnO, bb.d_q, d.n_q_heads, d.n_kv_heads, scale_log2, l, ka)));
-      else if (d.head_dim == 64) LAUNCH(Lh, F_ATTN, (launch_k(decode_attention_kernel<64>, grid, 256, 0, S, (const bf16 *)w.QKV, bb.d_qkv, w.AttnO, bb.d_q, d.n_q_heads, d.n_kv_heads, scale_log2, l, ka)));
-      else LAUNCH(Lh, F_ATTN, (launch_k(decode_attention_kernel<128>, grid, 256, 0, S, (const bf16 *)w.QKV, bb.d_qkv, w.AttnO, bb.d_q, d.n_q_heads, d.n_kv_heads, scale_log2, l, ka)));
+      DecAttnArgs da{};
+      da.qkv = w.QKV; da.out = w.AttnO; da.ld_qkv = bb.d_qkv; da.ld_out = bb.d_q; da.n_q_heads = d.n_q_heads; da.n_kv_heads = d.n_kv_heads;
+      da.layer = l; da.scale_log2 = scale_log2; da.kc_keys = dec_chunk_keys(d.max_seq); da.part = w.dec_part; da.cnt = w.dec_cnt;
+      dim3 grid(B, d.n_kv_heads, dec_chunks_cap(d.max_seq));
+      if (d.head_dim == 32) LAUNCH(Lh, F_ATTN, (launch_k(decode_attention_kernel<32>, grid, 128, decode_attention_smem<32>(), S, da, ka)));
+      else if (d.head_dim == 64) LAUNCH(Lh, F_ATTN, (launch_k(decode_attention_kernel<64>, grid, 128, decode_attention_smem<64>(), S, da, ka)));
+      else LAUNCH(Lh, F_ATTN, (launch_k(decode_attention_kernel<128>, grid, 128, decode_attention_smem<128>(), S, da, ka)));
       rev();
     } else if (c->o.attn_impl == FMX_ATTN_AUTO && attn_pair64_ok(c->o, d.head_dim, d.n_q_heads, max_len)) {
       AttnPairArgs pa2{};
@@ -1921,6 +1953,9 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
       return FMX_OK;
     case FMX_OPT_HALF_TILES:
       c->o.half_tiles = value ? 1 : 0;
+      return FMX_OK;
+    case FMX_OPT_DECODE_FORK:
+      c->o.decode_fork = value ? 1 : 0;
       return FMX_OK;
     case FMX_OPT_PDL:
       if (value < 0 || value > 2) return fmx_fail(FMX_E_INVALID_ARG, "set_option: pdl %d", value);

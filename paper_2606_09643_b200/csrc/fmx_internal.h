@@ -62,6 +62,9 @@ enum {
                                     expand as one N = 256 step per block (U loaded once) instead of two N = 128 steps */
   FMX_OPT_DEEP_PIPE = 12,        /* 1 (default): fp32-output GEMMs (residual, embed) run with one more smem pipeline stage
                                     and a single epilogue staging buffer per warpgroup */
+  FMX_OPT_DECODE_FORK = 13,      /* 1 (default): in a decode iteration the row-wise LoRA kernels of a projection run on the
+                                    context's auxiliary stream beside the projection GEMM (both are latency-bound) and join
+                                    before the reduction; set 0 when the serving stream belongs to an SM partition */
   FMX_OPT_PDL = 2                /* programmatic dependent launch of the forward's kernels:
                                     0 = off, 1 = always, 2 (default) = only for batches of <= 4096 token rows */
 };

@@ -807,139 +807,211 @@ __global__ void kv_append_kernel(const __nv_bfloat16 *__restrict__ qkv, int ld_q
   }
 }
 
-// Decode attention: every request has ONE query token (row p of the task-sorted batch) that attends the cache positions
-// 0 .. cpos (its own k / v were appended just before).  One CTA per (request, KV head); the query heads of the GQA group share
-// the K / V rows.  A warp takes 32 keys at a time:
-//   scores   lane = key: the lane reads its key row with 16-byte loads and takes the dot product with every head's query
-//            (queries, pre-scaled, sit in shared memory and are read as broadcast float4s) - no shuffles in the hot loop;
-//   softmax  online per head over the warp's chunks (one warp max / sum per chunk and head);
-//   P V      lane = DH / 32 output dims: the chunk's probabilities go through shared memory, V rows are read coalesced.
-// The eight warps' partial states (m, l, o) are merged in warp order in shared memory (deterministic).
-// Memory-bound: 2 * (cpos + 1) * DH * 2 bytes per CTA.
+// Decode attention (split over the keys): every request has ONE query token (row p of the task-sorted batch) that attends the cache
+// positions 0 .. cpos (its own k / v were appended just before).  One CTA per (request, KV head, chunk of kc_keys cached
+// positions); the query heads of the GQA group share the K / V rows.  Per 128 keys:
+//   load     the K and V rows go to shared memory with 16-byte cp.async copies, all in flight at once (coalesced; rows padded by
+//            16 bytes so that ldmatrix reads are bank-conflict free);
+//   scores   S = Q K^T on mma.sync m16n8k16: the M = 16 rows are the group's query heads (padded with zeros), a warp takes 32 keys;
+//   softmax  online per head over the warp's keys, in the accumulator registers (fp32, exp2 with the scale folded in);
+//   P V      P (bf16) stays in registers as the A operand, V through ldmatrix.trans.
+// (A first version did the two products with scalar FMAs, lane = key: 10 M instructions per launch at two warps per scheduler made
+// it latency-bound at 48 us per layer for 37 MB of cache.)
+// The four warps' states (m, l, o) are merged in warp order (deterministic).  A request with one chunk writes its output; with
+// more, every chunk's CTA stores (o, m, l) per head and the LAST CTA to finish (a counter per (request, KV head), reset by that
+// CTA) merges them in chunk order - the result depends on the request's own length only, never on the batch or on timing.
+// Memory-bound: 2 * (cpos + 1) * DH * 2 bytes per (request, KV head).
 constexpr int kDecGroupMax = 8;
-template <int VPT>
-__device__ __forceinline__ void load_bf16_vec(const __nv_bfloat16 *p, float (&f)[VPT]) {      // one aligned load of VPT = 1 / 2 / 4 values
-  if constexpr (VPT == 4) {
-    const uint2 u = *reinterpret_cast<const uint2 *>(p);
-    f[0] = bf16_lo(u.x); f[1] = bf16_hi(u.x); f[2] = bf16_lo(u.y); f[3] = bf16_hi(u.y);
-  } else if constexpr (VPT == 2) {
-    const uint32_t u = *reinterpret_cast<const uint32_t *>(p);
-    f[0] = bf16_lo(u); f[1] = bf16_hi(u);
-  } else {
-    f[0] = __bfloat162float(p[0]);
-  }
-}
+constexpr int kDecKeys = 128;                       // keys per pass of a CTA (4 warps x 32)
 template <int DH>
-__global__ void __launch_bounds__(256) decode_attention_kernel(const __nv_bfloat16 *__restrict__ qkv, int ld_qkv, __nv_bfloat16 *__restrict__ out,
-                                                               int ld_out, int n_q_heads, int n_kv_heads, float scale_log2, int layer, const KvArgs a) {
-  constexpr int VPT = DH / 32;
-  constexpr int G = kDecGroupMax;
-  __shared__ __align__(16) float s_q[G][DH];              // queries of the group, times scale * log2(e)
-  __shared__ __align__(16) float s_p[8][G][32];           // a warp's probabilities of its current 32-key chunk
-  __shared__ float s_m[8][G], s_l[8][G];
-  __shared__ float s_o[8][G][DH];
+constexpr size_t decode_attention_smem() {
+  return sizeof(__nv_bfloat16) * (2 * kDecKeys + 16) * (DH + 8) + sizeof(float) * 2 * 4 * kDecGroupMax;
+}
+struct DecAttnArgs {
+  const __nv_bfloat16 *qkv;
+  __nv_bfloat16 *out;
+  int ld_qkv, ld_out, n_q_heads, n_kv_heads, layer;
+  float scale_log2;
+  int kc_keys;                     // cached positions per chunk (multiple of kDecKeys); gridDim.z = chunks of the longest possible sequence
+  float *part;                     // [request, q head, chunk, DH + 2] (o unnormalised, m, l)
+  unsigned *cnt;                   // [request, KV head], zero between launches
+};
+template <int DH>
+__global__ void __launch_bounds__(128) decode_attention_kernel(const DecAttnArgs d, const KvArgs a) {
+  constexpr int G = kDecGroupMax, KS = DH + 8;
+  extern __shared__ __align__(16) unsigned char dec_smem[];
+  __nv_bfloat16 *s_k = reinterpret_cast<__nv_bfloat16 *>(dec_smem);           // [128][DH + 8]
+  __nv_bfloat16 *s_v = s_k + kDecKeys * KS;                                   // [128][DH + 8]
+  __nv_bfloat16 *s_q = s_v + kDecKeys * KS;                                   // [16][DH + 8] queries of the group, rows >= group zero
+  float *s_m = reinterpret_cast<float *>(s_q + 16 * KS), *s_l = s_m + 4 * G;  // [4][G]
+  float *s_o = reinterpret_cast<float *>(s_k);                                // [4][G][DH], reuses the K rows after the last pass
+  __shared__ int s_last;
   griddep_launch();
   griddep_wait();
-  const int p = blockIdx.x, kvh = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int group = n_q_heads / n_kv_heads;
+  const int p = blockIdx.x, kvh = blockIdx.y, chunk = blockIdx.z, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int group = d.n_q_heads / d.n_kv_heads;
   const int n_keys = a.row_cpos[p] + 1;
-  for (int idx = threadIdx.x; idx < G * DH; idx += blockDim.x) {
-    const int g = idx / DH, d = idx - g * DH;
-    s_q[g][d] = g < group ? __bfloat162float(qkv[(size_t)p * ld_qkv + (kvh * group + g) * DH + d]) * scale_log2 : 0.0f;
+  const int key_lo = chunk * d.kc_keys;
+  if (key_lo >= n_keys) return;
+  const int key_hi = min(n_keys, key_lo + d.kc_keys), n_chunks = (n_keys + d.kc_keys - 1) / d.kc_keys;
+  for (int idx = threadIdx.x; idx < 16 * (DH / 8); idx += blockDim.x) {
+    const int g = idx / (DH / 8), pc = idx - g * (DH / 8);
+    *reinterpret_cast<uint4 *>(s_q + g * KS + pc * 8) =
+        g < group ? *reinterpret_cast<const uint4 *>(d.qkv + (size_t)p * d.ld_qkv + (kvh * group + g) * DH + pc * 8) : make_uint4(0, 0, 0, 0);
   }
-  __syncthreads();
-  const __nv_bfloat16 *K = a.cache + (long long)a.row_slot[p] * a.slot_stride + (long long)layer * a.layer_stride + kvh * DH;
+  const __nv_bfloat16 *K = a.cache + (long long)a.row_slot[p] * a.slot_stride + (long long)d.layer * a.layer_stride + kvh * DH;
   const __nv_bfloat16 *V = K + a.kv_stride;
-  float acc[G][VPT], m[G], l[G];
+  // this thread's softmax row = head hr = lane / 4 of the group (accumulator rows 8 .. 15 of the 16-row MMA tile are padding)
+  float oacc[DH / 8][4], m = -INFINITY, l = 0.0f;
 #pragma unroll
-  for (int g = 0; g < G; ++g) {
-    m[g] = -INFINITY; l[g] = 0.0f;
+  for (int nt = 0; nt < DH / 8; ++nt) oacc[nt][0] = oacc[nt][1] = oacc[nt][2] = oacc[nt][3] = 0.0f;
+  for (int k0 = key_lo; k0 < key_hi; k0 += kDecKeys) {
+    const int nk_cta = min(kDecKeys, key_hi - k0), rows = (nk_cta + 31) & ~31;
+    if (k0 > key_lo) __syncthreads();                           // the previous pass is done with the buffers
+    for (int idx = threadIdx.x; idx < nk_cta * (DH / 8); idx += blockDim.x) {
+      const int row = idx / (DH / 8), pc = idx - row * (DH / 8);
+      cp_async_16(s_k + row * KS + pc * 8, K + (long long)(k0 + row) * a.d_kv + pc * 8, 16);
+    }
+    cp_async_commit();
+    for (int idx = threadIdx.x; idx < rows * (DH / 8); idx += blockDim.x) {      // rows past the last key are zero (0 * stale bits could be NaN)
+      const int row = idx / (DH / 8), pc = idx - row * (DH / 8);
+      const bool ok = row < nk_cta;
+      cp_async_16(s_v + row * KS + pc * 8, V + (long long)(k0 + (ok ? row : 0)) * a.d_kv + pc * 8, ok ? 16 : 0);
+    }
+    cp_async_commit();
+    cp_async_wait<1>();
+    __syncthreads();                                            // K rows (and, first pass, the queries) are in shared memory
+    const int nk = min(32, nk_cta - warp * 32);                 // this warp's keys in the pass (<= 0: none)
+    uint32_t ap[2][4];
+    if (nk > 0) {
+      // ---- S = Q K^T: 16 (heads, padded) x 32 keys ----
+      float sacc[4][4];
 #pragma unroll
-    for (int e = 0; e < VPT; ++e) acc[g][e] = 0.0f;
-  }
-  for (int k0 = warp * 32; k0 < n_keys; k0 += 8 * 32) {
-    const int key = k0 + lane;
-    const bool valid = key < n_keys;
-    // ---- scores of this lane's key against every head of the group ----
-    float s[G];
+      for (int nt = 0; nt < 4; ++nt) sacc[nt][0] = sacc[nt][1] = sacc[nt][2] = sacc[nt][3] = 0.0f;
 #pragma unroll
-    for (int g = 0; g < G; ++g) s[g] = 0.0f;
-    const uint4 *kp = reinterpret_cast<const uint4 *>(K + (long long)(valid ? key : k0) * a.d_kv);
-    uint4 kv[DH / 8];
+      for (int ks = 0; ks < DH / 16; ++ks) {
+        uint32_t aq[4];
+        ldmatrix_x4(aq, s_q + (lane & 15) * KS + ks * 16 + (lane >> 4) * 8);
 #pragma unroll
-    for (int v = 0; v < DH / 8; ++v) kv[v] = kp[v];             // the whole key row in flight before the first use
+        for (int np = 0; np < 2; ++np) {
+          uint32_t bk[4];
+          ldmatrix_x4(bk, s_k + (warp * 32 + np * 16 + (lane >> 4) * 8 + (lane & 7)) * KS + ks * 16 + ((lane >> 3) & 1) * 8);
+          const uint32_t b0[2] = {bk[0], bk[1]}, b1[2] = {bk[2], bk[3]};
+          mma_bf16_16816(sacc[2 * np], aq, b0);
+          mma_bf16_16816(sacc[2 * np + 1], aq, b1);
+        }
+      }
+      // ---- online softmax of row hr over the warp's keys (the thread holds keys 8 nt + 2 (lane % 4) + {0, 1}) ----
+      float mc = -INFINITY;
 #pragma unroll
-    for (int v = 0; v < DH / 8; ++v) {
-      const uint4 u = kv[v];
-      const float kf[8] = {bf16_lo(u.x), bf16_hi(u.x), bf16_lo(u.y), bf16_hi(u.y), bf16_lo(u.z), bf16_hi(u.z), bf16_lo(u.w), bf16_hi(u.w)};
+      for (int nt = 0; nt < 4; ++nt)
 #pragma unroll
-      for (int g = 0; g < G; ++g) {
-        if (g >= group) break;
-        const float4 qa = *reinterpret_cast<const float4 *>(&s_q[g][8 * v]), qb = *reinterpret_cast<const float4 *>(&s_q[g][8 * v + 4]);
-        s[g] = fmaf(qa.x, kf[0], s[g]); s[g] = fmaf(qa.y, kf[1], s[g]); s[g] = fmaf(qa.z, kf[2], s[g]); s[g] = fmaf(qa.w, kf[3], s[g]);
-        s[g] = fmaf(qb.x, kf[4], s[g]); s[g] = fmaf(qb.y, kf[5], s[g]); s[g] = fmaf(qb.z, kf[6], s[g]); s[g] = fmaf(qb.w, kf[7], s[g]);
+        for (int e = 0; e < 2; ++e) {
+          const bool valid = nt * 8 + 2 * (lane & 3) + e < nk;
+          sacc[nt][e] = valid ? sacc[nt][e] * d.scale_log2 : -INFINITY;
+          mc = fmaxf(mc, sacc[nt][e]);
+        }
+      mc = fmaxf(mc, __shfl_xor_sync(0xffffffffu, mc, 1));
+      mc = fmaxf(mc, __shfl_xor_sync(0xffffffffu, mc, 2));
+      const float mn = fmaxf(m, mc);                            // finite: the warp holds at least one valid key
+      const float f = fast_exp2(m - mn);
+      float lc = 0.0f;
+#pragma unroll
+      for (int nt = 0; nt < 4; ++nt) {
+        sacc[nt][0] = fast_exp2(sacc[nt][0] - mn);
+        sacc[nt][1] = fast_exp2(sacc[nt][1] - mn);
+        lc += sacc[nt][0] + sacc[nt][1];
+      }
+      lc += __shfl_xor_sync(0xffffffffu, lc, 1);
+      lc += __shfl_xor_sync(0xffffffffu, lc, 2);
+      m = mn;
+      l = l * f + lc;
+#pragma unroll
+      for (int nt = 0; nt < DH / 8; ++nt) { oacc[nt][0] *= f; oacc[nt][1] *= f; }
+#pragma unroll
+      for (int kk = 0; kk < 2; ++kk) {                          // P as the A operand of P V: keys 16 kk .. 16 kk + 15
+        ap[kk][0] = pack_bf16(sacc[2 * kk][0], sacc[2 * kk][1]);
+        ap[kk][2] = pack_bf16(sacc[2 * kk + 1][0], sacc[2 * kk + 1][1]);
+        ap[kk][1] = ap[kk][3] = 0u;
       }
     }
-    // ---- online softmax per head over the chunk ----
+    cp_async_wait<0>();
+    __syncthreads();                                            // V rows are in shared memory
+    if (nk > 0) {
+      // ---- O += P V: 16 x DH ----
 #pragma unroll
-    for (int g = 0; g < G; ++g) {
-      if (g >= group) break;
-      const float sv = valid ? s[g] : -INFINITY;
-      float mc = sv;
+      for (int kk = 0; kk < 2; ++kk)
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) mc = fmaxf(mc, __shfl_xor_sync(0xffffffffu, mc, o));
-      const float mn = fmaxf(m[g], mc);                     // finite: the chunk holds at least one valid key
-      const float f = fast_exp2(m[g] - mn), pw = fast_exp2(sv - mn);
-      float lc = pw;
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) lc += __shfl_xor_sync(0xffffffffu, lc, o);
-      m[g] = mn;
-      l[g] = l[g] * f + lc;
-#pragma unroll
-      for (int e = 0; e < VPT; ++e) acc[g][e] *= f;
-      s_p[warp][g][lane] = pw;
+        for (int dp = 0; dp < DH / 16; ++dp) {
+          uint32_t bv[4];
+          ldmatrix_x4_trans(bv, s_v + (warp * 32 + kk * 16 + ((lane >> 3) & 1) * 8 + (lane & 7)) * KS + (2 * dp + (lane >> 4)) * 8);
+          const uint32_t b0[2] = {bv[0], bv[1]}, b1[2] = {bv[2], bv[3]};
+          mma_bf16_16816(oacc[2 * dp], ap[kk], b0);
+          mma_bf16_16816(oacc[2 * dp + 1], ap[kk], b1);
+        }
     }
-    __syncwarp();
-    // ---- O += P V: the lane owns VPT dims of every head's output ----
-    const int nk = min(32, n_keys - k0);
-    const __nv_bfloat16 *vp = V + (long long)k0 * a.d_kv + lane * VPT;
-    for (int kk = 0; kk < nk; kk += 8) {                         // eight V rows in flight at a time
-      float vf[8][VPT];
-#pragma unroll
-      for (int j = 0; j < 8; ++j) load_bf16_vec<VPT>(vp + (long long)min(kk + j, nk - 1) * a.d_kv, vf[j]);
-#pragma unroll
-      for (int g = 0; g < G; ++g) {
-        if (g >= group) break;
-        const float4 pa = *reinterpret_cast<const float4 *>(&s_p[warp][g][kk]), pb = *reinterpret_cast<const float4 *>(&s_p[warp][g][kk + 4]);   // invalid keys of the chunk hold 0
-#pragma unroll
-        for (int e = 0; e < VPT; ++e)
-          acc[g][e] = fmaf(pa.x, vf[0][e], fmaf(pa.y, vf[1][e], fmaf(pa.z, vf[2][e], fmaf(pa.w, vf[3][e],
-                      fmaf(pb.x, vf[4][e], fmaf(pb.y, vf[5][e], fmaf(pb.z, vf[6][e], fmaf(pb.w, vf[7][e], acc[g][e]))))))));
-      }
-    }
-    __syncwarp();
   }
+  __syncthreads();                                              // every warp is done with the K rows: s_o may overwrite them
+  {
+    const int hr = lane >> 2;
+    if ((lane & 3) == 0) { s_m[warp * G + hr] = m; s_l[warp * G + hr] = l; }
 #pragma unroll
-  for (int g = 0; g < G; ++g) {
-    if (g >= group) break;
-    if (lane == 0) { s_m[warp][g] = m[g]; s_l[warp][g] = l[g]; }
-#pragma unroll
-    for (int e = 0; e < VPT; ++e) s_o[warp][g][lane * VPT + e] = acc[g][e];
+    for (int nt = 0; nt < DH / 8; ++nt)
+      *reinterpret_cast<float2 *>(&s_o[(warp * G + hr) * DH + nt * 8 + 2 * (lane & 3)]) = make_float2(oacc[nt][0], oacc[nt][1]);
   }
   __syncthreads();
+  const int n_cap = gridDim.z;
   for (int idx = threadIdx.x; idx < group * DH; idx += blockDim.x) {
-    const int g = idx / DH, d = idx - g * DH;
+    const int g = idx / DH, e = idx - g * DH;
     float mx = -INFINITY;
 #pragma unroll
-    for (int w = 0; w < 8; ++w) mx = fmaxf(mx, s_m[w][g]);
+    for (int w = 0; w < 4; ++w) mx = fmaxf(mx, s_m[w * G + g]);
     float L = 0.0f, O = 0.0f;
 #pragma unroll
-    for (int w = 0; w < 8; ++w) {
-      const float f = fast_exp2(s_m[w][g] - mx);           // a warp that saw no key: m = -inf -> f = 0
-      L = fmaf(s_l[w][g], f, L);
-      O = fmaf(s_o[w][g][d], f, O);
+    for (int w = 0; w < 4; ++w) {
+      const float f = fast_exp2(s_m[w * G + g] - mx);        // a warp that saw no key: m = -inf -> f = 0
+      L = fmaf(s_l[w * G + g], f, L);
+      O = fmaf(s_o[(w * G + g) * DH + e], f, O);
     }
-    out[(size_t)p * ld_out + (kvh * group + g) * DH + d] = __float2bfloat16(O / L);
+    if (n_chunks == 1) {
+      d.out[(size_t)p * d.ld_out + (kvh * group + g) * DH + e] = __float2bfloat16(O / L);
+    } else {
+      float *dst = d.part + (((size_t)p * d.n_q_heads + kvh * group + g) * n_cap + chunk) * (DH + 2);
+      dst[e] = O;
+      if (e == 0) { dst[DH] = mx; dst[DH + 1] = L; }
+    }
+  }
+  if (n_chunks == 1) return;
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) s_last = atomicAdd(&d.cnt[p * d.n_kv_heads + kvh], 1u) == (unsigned)(n_chunks - 1);
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  if (threadIdx.x == 0) d.cnt[p * d.n_kv_heads + kvh] = 0u;      // ready for the next launch
+  for (int idx = threadIdx.x; idx < group * DH; idx += blockDim.x) {
+    const int g = idx / DH, e = idx - g * DH;
+    const float *src = d.part + (((size_t)p * d.n_q_heads + kvh * group + g) * n_cap) * (DH + 2);
+    float cm[16], cl[16], co[16];                          // every chunk's (m, l, o) in flight at once (n_cap <= 16)
+#pragma unroll
+    for (int c = 0; c < 16; ++c) {
+      const bool ok = c < n_chunks;
+      const float *q = src + (size_t)(ok ? c : 0) * (DH + 2);
+      cm[c] = ok ? __ldcg(q + DH) : -INFINITY;
+      cl[c] = ok ? __ldcg(q + DH + 1) : 0.0f;
+      co[c] = ok ? __ldcg(q + e) : 0.0f;
+    }
+    float mx = -INFINITY;
+#pragma unroll
+    for (int c = 0; c < 16; ++c) mx = fmaxf(mx, cm[c]);
+    float L = 0.0f, O = 0.0f;
+#pragma unroll
+    for (int c = 0; c < 16; ++c) {                         // chunk order; a chunk past the end has f = 0
+      const float f = fast_exp2(cm[c] - mx);
+      L = fmaf(cl[c], f, L);
+      O = fmaf(co[c], f, O);
+    }
+    d.out[(size_t)p * d.ld_out + (kvh * group + g) * DH + e] = __float2bfloat16(O / L);
   }
 }
 
@@ -1107,78 +1179,99 @@ struct RowLoraArgs {
   const unsigned char *task_trpad;
   const float *task_scale;
 };
-// Both kernels are latency-bound (a few KB per thread block from scattered slab rows), so the work is cut fine - (row, target, 16 ranks)
-// and (row, target, 512 columns) - and every thread issues all its loads of a round before it uses any.
+// Both kernels are bound by memory latency and by the number of separate cache lines they touch, not by arithmetic, so
+//  * the work is cut fine - (row, target, 512 input columns) and (row, target, 512 output columns) - and every thread issues all
+//    its loads before it uses any;
+//  * adjacent lanes read adjacent 16 bytes: a shrink warp reads 512 contiguous bytes of a slab row per instruction, an expand warp
+//    covers the r_pad * 2 contiguous bytes of a column of B with r_pad / 8 adjacent lanes (one cache-line lookup per column instead
+//    of one per 16 bytes).
 constexpr int kRowExpandCols = 512;
-// u[row, i, j] = s_t <x_row, A_t[j, :]> for the 16 ranks j = 16 z .. of target i (fp32, [M, 3, 64])
+constexpr int kRowShrinkK = 512;
+// u_part[kc, row, i, j] = s_t <x_row[kc-th 512 columns], A_t[j, same columns]> for every rank j of target i (fp32, [nkc, M, 3, 64]);
+// the expand kernel adds the nkc partial sums in kc order.  Warp w takes the ranks w, w + 8, ...
 __global__ void __launch_bounds__(256) row_shrink_kernel(const RowLoraArgs a, float *__restrict__ u) {
   griddep_launch();
   griddep_wait();
-  const int r = blockIdx.x, i = blockIdx.y, z = blockIdx.z, tg = a.tg[i], warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int r = blockIdx.x, i = blockIdx.y, kc = blockIdx.z, tg = a.tg[i], warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int t = a.task_sorted[a.row_req[r]];
   const int rp = a.task_trpad[t * 7 + tg];               // padded rank (multiple of 16); 0 = no adapter on this target
-  if (16 * z >= rp) return;
+  if (rp == 0) return;
   const float sc = a.task_scale[t * 7 + tg];
+  const int nj = rp >> 3;                                // ranks of this warp: warp + 8 jj, jj < nj
+  const int k0 = kc * kRowShrinkK + lane * 8, k1 = k0 + 256;
+  const bool ok0 = k0 < a.K, ok1 = k1 < a.K;
   const __nv_bfloat16 *x = a.x + (size_t)r * a.K;
-  const int j0 = 16 * z + warp;                          // this warp: ranks j0 and j0 + 8
-  const __nv_bfloat16 *a0 = a.slabA[i] + (size_t)(a.task_coff[t] + j0) * a.K, *a1 = a0 + (size_t)8 * a.K;
-  float acc0 = 0.0f, acc1 = 0.0f;
-#pragma unroll 4
-  for (int k = lane * 8; k < a.K; k += 256) {
-    const uint4 xv = *reinterpret_cast<const uint4 *>(x + k), v0 = *reinterpret_cast<const uint4 *>(a0 + k), v1 = *reinterpret_cast<const uint4 *>(a1 + k);
-    acc0 += bf16_lo(v0.x) * bf16_lo(xv.x) + bf16_hi(v0.x) * bf16_hi(xv.x) + bf16_lo(v0.y) * bf16_lo(xv.y) + bf16_hi(v0.y) * bf16_hi(xv.y) +
-            bf16_lo(v0.z) * bf16_lo(xv.z) + bf16_hi(v0.z) * bf16_hi(xv.z) + bf16_lo(v0.w) * bf16_lo(xv.w) + bf16_hi(v0.w) * bf16_hi(xv.w);
-    acc1 += bf16_lo(v1.x) * bf16_lo(xv.x) + bf16_hi(v1.x) * bf16_hi(xv.x) + bf16_lo(v1.y) * bf16_lo(xv.y) + bf16_hi(v1.y) * bf16_hi(xv.y) +
-            bf16_lo(v1.z) * bf16_lo(xv.z) + bf16_hi(v1.z) * bf16_hi(xv.z) + bf16_lo(v1.w) * bf16_lo(xv.w) + bf16_hi(v1.w) * bf16_hi(xv.w);
-  }
+  const __nv_bfloat16 *A = a.slabA[i] + (size_t)(a.task_coff[t] + warp) * a.K;
+  const uint4 z4 = make_uint4(0, 0, 0, 0);
+  const uint4 x0 = ok0 ? *reinterpret_cast<const uint4 *>(x + k0) : z4, x1 = ok1 ? *reinterpret_cast<const uint4 *>(x + k1) : z4;
+  uint4 v0[8], v1[8];
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) { acc0 += __shfl_xor_sync(0xffffffffu, acc0, o); acc1 += __shfl_xor_sync(0xffffffffu, acc1, o); }
-  if (lane == 0) {
-    float *dst = u + ((size_t)r * 3 + i) * 64;
-    dst[j0] = acc0 * sc;
-    dst[j0 + 8] = acc1 * sc;
+  for (int jj = 0; jj < 8; ++jj) {
+    const __nv_bfloat16 *row = A + (size_t)(8 * jj) * a.K;
+    v0[jj] = (jj < nj && ok0) ? *reinterpret_cast<const uint4 *>(row + k0) : z4;
+    v1[jj] = (jj < nj && ok1) ? *reinterpret_cast<const uint4 *>(row + k1) : z4;
+  }
+  auto dot8 = [](const uint4 &p, const uint4 &q) {
+    return bf16_lo(p.x) * bf16_lo(q.x) + bf16_hi(p.x) * bf16_hi(q.x) + bf16_lo(p.y) * bf16_lo(q.y) + bf16_hi(p.y) * bf16_hi(q.y) +
+           bf16_lo(p.z) * bf16_lo(q.z) + bf16_hi(p.z) * bf16_hi(q.z) + bf16_lo(p.w) * bf16_lo(q.w) + bf16_hi(p.w) * bf16_hi(q.w);
+  };
+  float *dst = u + (((size_t)kc * a.M + r) * 3 + i) * 64;
+#pragma unroll
+  for (int jj = 0; jj < 8; ++jj) {
+    if (jj >= nj) break;
+    float acc = dot8(v0[jj], x0) + dot8(v1[jj], x1);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) dst[warp + 8 * jj] = acc * sc;
   }
 }
-// delta[row, column of (target i, c)] = <u[row, i, :rp], B_t[c, :rp]> for 512 columns per CTA, two per thread
-__global__ void __launch_bounds__(256) row_expand_kernel(const RowLoraArgs a, const float *__restrict__ u) {
-  __shared__ float s_u[64];
+// delta[row, column of (target i, c)] = <u[row, i, :rp], B_t[c, :rp]>: 512 columns per CTA, 64 per warp.  lpc = 2 / 4 / 8 adjacent
+// lanes share a column (lane q of them owns the ranks 8 q .. 8 q + 7), so a warp load covers 32 / lpc whole columns.
+__global__ void __launch_bounds__(256) row_expand_kernel(const RowLoraArgs a, const float *__restrict__ u, int nkc) {
   griddep_launch();
   griddep_wait();
-  const int r = blockIdx.x, i = blockIdx.y, tg = a.tg[i];
+  const int r = blockIdx.x, i = blockIdx.y, tg = a.tg[i], warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int dout = a.d_out[i];
-  const int c_lo = blockIdx.z * kRowExpandCols;
-  if (c_lo >= dout) return;
+  const int c_base = blockIdx.z * kRowExpandCols + warp * 64;
+  if (c_base >= dout) return;
   const int t = a.task_sorted[a.row_req[r]];
   const int rp = a.task_trpad[t * 7 + tg];
   float *dst = a.delta + (size_t)r * a.ld_delta;
   auto col_of = [&](int c) { return a.interleave2 ? ((c >> 7) * 256 + i * 128 + (c & 127)) : a.col0[i] + c; };
-  const int c0 = c_lo + threadIdx.x, c1 = c0 + 256;
   if (rp == 0) {                                         // no adapter: the reduce kernel adds the delta unconditionally
-    if (c0 < dout) dst[col_of(c0)] = 0.0f;
-    if (c1 < dout) dst[col_of(c1)] = 0.0f;
+    if (c_base + lane < dout) dst[col_of(c_base + lane)] = 0.0f;
+    if (c_base + 32 + lane < dout) dst[col_of(c_base + 32 + lane)] = 0.0f;
     return;
   }
-  if (threadIdx.x < 64) s_u[threadIdx.x] = threadIdx.x < rp ? u[((size_t)r * 3 + i) * 64 + threadIdx.x] : 0.0f;
-  const __nv_bfloat16 *b0 = a.slabB[i] + (size_t)min(c0, dout - 1) * a.Rcap + a.task_coff[t];
-  const __nv_bfloat16 *b1 = a.slabB[i] + (size_t)min(c1, dout - 1) * a.Rcap + a.task_coff[t];
-  uint4 v0[8], v1[8];
+  const int lpc = rp <= 16 ? 2 : rp <= 32 ? 4 : 8, sh = rp <= 16 ? 1 : rp <= 32 ? 2 : 3;
+  const int q = lane & (lpc - 1), cs = lane >> sh, cpi = 32 >> sh, n_ld = 64 / cpi;   // 4 / 8 / 16 loads per lane
+  const bool live = 8 * q < rp;
+  const uint4 z4 = make_uint4(0, 0, 0, 0);
+  const __nv_bfloat16 *B = a.slabB[i] + a.task_coff[t] + 8 * q;
+  uint4 v[16];
 #pragma unroll
-  for (int q = 0; q < 8; ++q) {                          // every load of the thread is in flight before the first use
-    v0[q] = 8 * q < rp ? *reinterpret_cast<const uint4 *>(b0 + 8 * q) : make_uint4(0, 0, 0, 0);
-    v1[q] = 8 * q < rp ? *reinterpret_cast<const uint4 *>(b1 + 8 * q) : make_uint4(0, 0, 0, 0);
+  for (int n = 0; n < 16; ++n) {
+    const int c = c_base + n * cpi + cs;
+    v[n] = (n < n_ld && live && c < dout) ? *reinterpret_cast<const uint4 *>(B + (size_t)c * a.Rcap) : z4;
   }
-  __syncthreads();
-  float acc0 = 0.0f, acc1 = 0.0f;
+  float uu[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  if (live)
+    for (int kc = 0; kc < nkc; ++kc) {
+      const float4 *src = reinterpret_cast<const float4 *>(u + (((size_t)kc * a.M + r) * 3 + i) * 64 + 8 * q);
+      const float4 p0 = src[0], p1 = src[1];
+      uu[0] += p0.x; uu[1] += p0.y; uu[2] += p0.z; uu[3] += p0.w; uu[4] += p1.x; uu[5] += p1.y; uu[6] += p1.z; uu[7] += p1.w;
+    }
 #pragma unroll
-  for (int q = 0; q < 8; ++q) {
-    const float *uu = s_u + 8 * q;
-    acc0 += uu[0] * bf16_lo(v0[q].x) + uu[1] * bf16_hi(v0[q].x) + uu[2] * bf16_lo(v0[q].y) + uu[3] * bf16_hi(v0[q].y) +
-            uu[4] * bf16_lo(v0[q].z) + uu[5] * bf16_hi(v0[q].z) + uu[6] * bf16_lo(v0[q].w) + uu[7] * bf16_hi(v0[q].w);
-    acc1 += uu[0] * bf16_lo(v1[q].x) + uu[1] * bf16_hi(v1[q].x) + uu[2] * bf16_lo(v1[q].y) + uu[3] * bf16_hi(v1[q].y) +
-            uu[4] * bf16_lo(v1[q].z) + uu[5] * bf16_hi(v1[q].z) + uu[6] * bf16_lo(v1[q].w) + uu[7] * bf16_hi(v1[q].w);
+  for (int n = 0; n < 16; ++n) {
+    if (n >= n_ld) break;
+    float acc = uu[0] * bf16_lo(v[n].x) + uu[1] * bf16_hi(v[n].x) + uu[2] * bf16_lo(v[n].y) + uu[3] * bf16_hi(v[n].y) +
+                uu[4] * bf16_lo(v[n].z) + uu[5] * bf16_hi(v[n].z) + uu[6] * bf16_lo(v[n].w) + uu[7] * bf16_hi(v[n].w);
+    acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+    if (lpc > 2) acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+    if (lpc > 4) acc += __shfl_xor_sync(0xffffffffu, acc, 4);
+    const int c = c_base + n * cpi + cs;
+    if (q == 0 && c < dout) dst[col_of(c)] = acc;
   }
-  if (c0 < dout) dst[col_of(c0)] = acc0;
-  if (c1 < dout) dst[col_of(c1)] = acc1;
 }
 
 }  // namespace fmx
