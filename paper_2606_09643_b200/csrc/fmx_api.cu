@@ -81,6 +81,9 @@ struct Backbone {
   std::vector<unsigned long long> col_freed_seq;   // retirement after which a freed unit may be rewritten
   bf16 *slabA[7] = {nullptr};              // per target: [L][Rcap, d_in]
   bf16 *slabB[7] = {nullptr};              // per target: [L][d_out, Rcap]
+  bf16 *slabBt[7] = {nullptr};             // decoder backbones only (row_bt): the same B, rank-major [L][Rcap, d_out] - a task's rank rows are
+                                           //   contiguous, which is what the row-wise expand of a decode iteration streams
+  bool row_bt = false;
   std::vector<CUtensorMap> mA[7], mB[7];   // per target, per layer
   int n_adapters[7] = {0};                 // live adapters per target
   int din[7], dout[7];
@@ -579,15 +582,19 @@ int note_forward(fmx_ctx *c, cudaStream_t s) {
 int alloc_slab(fmx_ctx *c, Backbone &bb, int tg) {
   const size_t L = bb.d.n_layers;
   const size_t na = L * bb.Rcap * bb.din[tg], nb = L * bb.dout[tg] * bb.Rcap;
-  bf16 *A = nullptr, *B = nullptr;
+  bf16 *A = nullptr, *B = nullptr, *Bt = nullptr;
   CU_OK(cudaMallocAsync(&A, na * sizeof(bf16), c->side));
-  if (cudaError_t e = cudaMallocAsync(&B, nb * sizeof(bf16), c->side)) {
+  cudaError_t e = cudaMallocAsync(&B, nb * sizeof(bf16), c->side);
+  if (e == cudaSuccess && bb.row_bt) e = cudaMallocAsync(&Bt, nb * sizeof(bf16), c->side);
+  if (e != cudaSuccess) {
     cudaFreeAsync(A, c->side);
+    if (B) cudaFreeAsync(B, c->side);
     return fmx_fail(FMX_E_CUDA, "register_task: LoRA slab allocation failed: %s", cudaGetErrorString(e));
   }
   CU_OK(cudaMemsetAsync(A, 0, na * sizeof(bf16), c->side));
   CU_OK(cudaMemsetAsync(B, 0, nb * sizeof(bf16), c->side));
-  bb.slabA[tg] = A; bb.slabB[tg] = B;
+  if (Bt) CU_OK(cudaMemsetAsync(Bt, 0, nb * sizeof(bf16), c->side));
+  bb.slabA[tg] = A; bb.slabB[tg] = B; bb.slabBt[tg] = Bt;
   return rebuild_slab_maps(c, bb, tg);
 }
 
@@ -597,8 +604,10 @@ int alloc_slab(fmx_ctx *c, Backbone &bb, int tg) {
 int grow_slabs(fmx_ctx *c, Backbone &bb, int new_cap) {
   const size_t L = bb.d.n_layers;
   const int old = bb.Rcap;
-  bf16 *nA[7] = {nullptr}, *nB[7] = {nullptr};
-  auto undo = [&]() { for (int tg = 0; tg < 7; ++tg) { if (nA[tg]) cudaFreeAsync(nA[tg], c->side); if (nB[tg]) cudaFreeAsync(nB[tg], c->side); } };
+  bf16 *nA[7] = {nullptr}, *nB[7] = {nullptr}, *nBt[7] = {nullptr};
+  auto undo = [&]() {
+    for (int tg = 0; tg < 7; ++tg) { if (nA[tg]) cudaFreeAsync(nA[tg], c->side); if (nB[tg]) cudaFreeAsync(nB[tg], c->side); if (nBt[tg]) cudaFreeAsync(nBt[tg], c->side); }
+  };
   for (int tg = 0; tg < 7; ++tg) {
     if (!bb.slabA[tg]) continue;
     const size_t na = L * new_cap * bb.din[tg], nb = L * bb.dout[tg] * (size_t)new_cap;
@@ -612,16 +621,24 @@ int grow_slabs(fmx_ctx *c, Backbone &bb, int new_cap) {
     if (e == cudaSuccess)
       e = cudaMemcpy2DAsync(nB[tg], (size_t)new_cap * sizeof(bf16), bb.slabB[tg], (size_t)old * sizeof(bf16), (size_t)old * sizeof(bf16),
                             L * bb.dout[tg], cudaMemcpyDeviceToDevice, c->side);
+    if (e == cudaSuccess && bb.slabBt[tg]) {
+      e = cudaMallocAsync(&nBt[tg], nb * sizeof(bf16), c->side);
+      if (e == cudaSuccess) e = cudaMemsetAsync(nBt[tg], 0, nb * sizeof(bf16), c->side);
+      if (e == cudaSuccess)
+        e = cudaMemcpy2DAsync(nBt[tg], (size_t)new_cap * bb.dout[tg] * sizeof(bf16), bb.slabBt[tg], (size_t)old * bb.dout[tg] * sizeof(bf16),
+                              (size_t)old * bb.dout[tg] * sizeof(bf16), L, cudaMemcpyDeviceToDevice, c->side);
+    }
     if (e != cudaSuccess) { undo(); return fmx_fail(FMX_E_CUDA, "register_task: growing the LoRA slabs to %d columns failed: %s", new_cap, cudaGetErrorString(e)); }
   }
   // commit: nothing below fails short of a broken context
   std::vector<void *> old_slabs;
-  for (int tg = 0; tg < 7; ++tg) if (bb.slabA[tg]) { old_slabs.push_back(bb.slabA[tg]); old_slabs.push_back(bb.slabB[tg]); }
+  for (int tg = 0; tg < 7; ++tg) if (bb.slabA[tg]) { old_slabs.push_back(bb.slabA[tg]); old_slabs.push_back(bb.slabB[tg]); old_slabs.push_back(bb.slabBt[tg]); }
   if (int e = retire(c, old_slabs)) { undo(); return e; }
   for (int tg = 0; tg < 7; ++tg) {
     if (!bb.slabA[tg]) continue;
     bb.slabA[tg] = nA[tg];
     bb.slabB[tg] = nB[tg];
+    bb.slabBt[tg] = nBt[tg];
   }
   bb.Rcap = new_cap;
   bb.col_used.resize(new_cap / 16, 0);
@@ -780,7 +797,7 @@ int fmx_destroy(fmx_ctx *c) {
   for (auto &bp : c->bbs) {
     if (!bp) continue;
     cudaFree(bp->embed_Wpad); cudaFree(bp->posb); cudaFree(bp->rope_cs); cudaFree(bp->rope_cs_t);
-    for (int tg = 0; tg < 7; ++tg) { if (bp->slabA[tg]) cudaFreeAsync(bp->slabA[tg], c->side); if (bp->slabB[tg]) cudaFreeAsync(bp->slabB[tg], c->side); }
+    for (int tg = 0; tg < 7; ++tg) { if (bp->slabA[tg]) cudaFreeAsync(bp->slabA[tg], c->side); if (bp->slabB[tg]) cudaFreeAsync(bp->slabB[tg], c->side); if (bp->slabBt[tg]) cudaFreeAsync(bp->slabBt[tg], c->side); }
   }
   for (auto &t : c->tasks)
     for (bf16 *q : {t.head_W, t.head_b, t.head_W2, t.head_b2, t.enc_W, t.enc_b}) if (q) cudaFreeAsync(q, c->side);
@@ -895,6 +912,7 @@ int fmx_register_backbone(fmx_ctx *c, const fmx_backbone_desc *desc, fmx_backbon
   }
   CU_OK(cudaDeviceSynchronize());
   b->Rcap = 256;
+  b->row_bt = d.input_kind == FMX_INPUT_TOKEN_IDS && d.causal;      // a decoder: may serve decode iterations (row-wise LoRA reads B rank-major)
   b->col_used.assign(b->Rcap / 16, 0);
   b->col_freed_seq.assign(b->Rcap / 16, 0);
   c->bbs.push_back(std::move(b));
@@ -1003,6 +1021,11 @@ int fmx_register_task(fmx_ctx *c, fmx_backbone_t h, const fmx_task_desc *desc, f
         if (e == cudaSuccess)
           e = cudaMemcpy2DAsync(B, (size_t)bb->Rcap * sizeof(bf16), a.B[l], (size_t)a.rank * sizeof(bf16), (size_t)a.rank * sizeof(bf16),
                                 dout, cudaMemcpyDeviceToDevice, c->side);
+        if (e == cudaSuccess && bb->slabBt[tg]) {          // rank-major copy, padding rows zeroed
+          bf16 *Bt = bb->slabBt[tg] + ((size_t)l * bb->Rcap + r.coff) * dout;
+          lora_bt_fill_kernel<<<(unsigned)(((size_t)dout * rp + 255) / 256), 256, 0, c->side>>>((const bf16 *)a.B[l], Bt, dout, a.rank, rp);
+          e = cudaGetLastError();
+        }
         if (e != cudaSuccess) return fail(fmx_fail(FMX_E_CUDA, "register_task: adapter copy failed: %s", cudaGetErrorString(e)));
       }
       r.trpad[tg] = (unsigned char)rp;
@@ -1248,7 +1271,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   // shrink over an input group: targets tgs[0..n) that currently have adapters; fills uslot_of[tg]
   int uslot_of[7] = {-1, -1, -1, -1, -1, -1, -1};
   auto shrink = [&](const CUtensorMap &amap, int K, const int *tgs, int n, int layer) -> int {
-    if (kv && kv->decode && w.splitk && w.n_tiles == 1) return FMX_OK;     // row_mode: row_shrink_kernel + row_expand_kernel do shrink and expand
+    if (kv && kv->decode && w.splitk && bb.row_bt && w.n_tiles == 1) return FMX_OK;     // row_mode: row_shrink_kernel + row_expand_kernel do shrink and expand
     GemmParams p = sbase;
     p.mode = GM_SHRINK; p.amap = amap; p.K = K; p.out = w.U; p.ld_out = 192; p.n_tg = 0;
     for (int i = 0; i < n; ++i) {
@@ -1284,7 +1307,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   // items fit ONE wave of the persistent grid (cfg2: 73 blocks on 74 pairs, -0.4 ms per step); with more blocks the items'
   // low arithmetic intensity costs as much as the separate shrink launches (cfg3 / cfg4 / cfg5 at 92 tasks: +-0).
   const int n_blk_host = bs.n_blk;
-  const bool fuse_ok = !(kv && kv->decode && w.splitk && w.n_tiles == 1) && c->o.shrink_fused && c->pairs_resident && (c->o.shrink_fused == 2 || n_blk_host <= c->sm_count / 2);
+  const bool fuse_ok = !(kv && kv->decode && w.splitk && bb.row_bt && w.n_tiles == 1) && c->o.shrink_fused && c->pairs_resident && (c->o.shrink_fused == 2 || n_blk_host <= c->sm_count / 2);
   if (fuse_ok) CU_OK(cudaMemsetAsync(w.u_flag, 0, sizeof(unsigned), s));
   if (kv && kv->decode) CU_OK(cudaMemsetAsync(w.dec_cnt, 0, sizeof(unsigned) * (size_t)B * d.n_kv_heads, s));   // the last chunk's CTA resets its counter; this covers an aborted launch
   // fusable: all CTA pairs of the persistent grid are co-resident (the expand steps spin on another pair's result) and
@@ -1294,7 +1317,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   };
 
   auto set_lora = [&](PairGemmParams &p, int src, int tg, int layer) {
-    if (kv && kv->decode && w.splitk && w.n_tiles == 1) return;
+    if (kv && kv->decode && w.splitk && bb.row_bt && w.n_tiles == 1) return;
     if (bb.n_adapters[tg] > 0 && uslot_of[tg] >= 0) {
       p.lora_tgt[src] = tg; p.uslot[src] = uslot_of[tg]; p.lmap[src] = bb.mB[tg][layer]; p.has_lora = 1;
     }
@@ -1307,7 +1330,10 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   // splitk_reduce_kernel adds the partials in split order, the delta and the bias and applies activation / SwiGLU / the residual
   // update.  Every choice depends on the projection's shape only, never on the batch, so a request decodes to the same bits alone
   // and in a batch.  (Prefill keeps the fused path: its outputs must not depend on the batch size.)
-  const bool row_mode = kv && kv->decode && w.splitk && w.n_tiles == 1;
+  const bool row_mode = kv && kv->decode && w.splitk && bb.row_bt && w.n_tiles == 1;
+  // row mode fuses what follows a reduction into it: RoPE + the cache append after q / k / v, the next norm after a residual update
+  const bool row_norm_fused = row_mode && d.d_model <= 4096;
+  const bf16 *next_norm_g = nullptr, *next_norm_b = nullptr;
   auto project = [&](PairGemmParams &p, int family, __nv_bfloat16 *out_bf16, int ld_out, const __nv_bfloat16 *x, const int *tgs, int n_tg, int layer) -> int {
     if (!row_mode) { LAUNCH(Lh, family, launch_pair_gemm(c, S, p)); return FMX_OK; }
     const int Nn = p.n_chunks * 128;
@@ -1324,14 +1350,14 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
         const int tg = tgs[i];
         la.tg[i] = tg; la.d_out[i] = bb.dout[tg]; la.col0[i] = col; col += bb.dout[tg];
         la.slabA[i] = bb.slabA[tg] ? bb.slabA[tg] + (size_t)layer * bb.Rcap * bb.din[tg] : nullptr;
-        la.slabB[i] = bb.slabB[tg] ? bb.slabB[tg] + (size_t)layer * bb.dout[tg] * bb.Rcap : nullptr;
+        la.slabB[i] = bb.slabBt[tg] ? bb.slabBt[tg] + (size_t)layer * bb.Rcap * bb.dout[tg] : nullptr;
       }
       int max_dout = 0;
       for (int i = 0; i < n_tg; ++i) max_dout = std::max(max_dout, bb.dout[tgs[i]]);
-      const int nkc = row_shrink_chunks(p.K);
+      const int nkc = row_shrink_chunks(p.K), k_range = ((p.K + nkc - 1) / nkc + 255) / 256 * 256;
       const Strm SL = fork ? Strm{c->aux, 0} : S;
       if (fork) { CU_OK(cudaEventRecord(c->fork_ev, s)); CU_OK(cudaStreamWaitEvent(c->aux, c->fork_ev, 0)); }
-      LAUNCH(Lh, F_SHRINK, (launch_k(row_shrink_kernel, dim3(Ni, n_tg, nkc), 256, 0, SL, la, w.rowu)));
+      LAUNCH(Lh, F_SHRINK, (launch_k(row_shrink_kernel, dim3(Ni, n_tg, nkc), 256, 0, SL, la, w.rowu, k_range)));
       LAUNCH(Lh, F_SHRINK, (launch_k(row_expand_kernel, dim3(Ni, n_tg, (max_dout + kRowExpandCols - 1) / kRowExpandCols), 256, 0, SL, la, (const float *)w.rowu, nkc)));
       if (fork) CU_OK(cudaEventRecord(c->join_ev, c->aux));
     }
@@ -1346,6 +1372,23 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     p.k_split = ks; p.kb_per_split = kbps; p.split_rows = kPairRows;
     LAUNCH(Lh, family, launch_pair_gemm(c, S, p));
     if (fork) CU_OK(cudaStreamWaitEvent(s, c->join_ev, 0));
+    if (family == F_GEMM_QKV) {                              // + RoPE at the cache position + append k / v to the cache
+      QkvReduceArgs qa{};
+      qa.partial = w.splitk; qa.k_split = ks; qa.split_rows = kPairRows; qa.M = Ni; qa.N = Nn; qa.delta = any ? w.delta : nullptr;
+      for (int i = 0; i < 3; ++i) qa.bias[i] = p.bias[i];
+      qa.qkv = out_bf16; qa.n_q_heads = d.n_q_heads; qa.n_kv_heads = d.n_kv_heads; qa.dh = d.head_dim; qa.layer = layer;
+      qa.rope_cs = d.rope_theta > 0 ? bb.rope_cs : nullptr;
+      const long long n_thr = (long long)Ni * (d.n_q_heads + 2 * d.n_kv_heads) * (d.head_dim / 8);
+      LAUNCH(Lh, family, (launch_k(qkv_reduce_rope_kernel, (unsigned)((n_thr + 255) / 256), 256, 0, S, qa, ka)));
+      return FMX_OK;
+    }
+    if (p.mode == GM_RESID_F32 && row_norm_fused) {          // + the norm that follows the residual update
+      ReduceNormArgs na{};
+      na.partial = w.splitk; na.k_split = ks; na.split_rows = kPairRows; na.N = Nn; na.delta = any ? w.delta : nullptr; na.bias = p.bias[0];
+      na.X = w.X; na.Y = w.Xn; na.g = next_norm_g; na.b = next_norm_b; na.eps = d.norm_eps; na.rms = d.norm == FMX_NORM_RMSNORM;
+      LAUNCH(Lh, family, (launch_k(reduce_resid_norm_kernel, (unsigned)Ni, 128, 0, S, na)));
+      return FMX_OK;
+    }
     SplitKReduceArgs ra{};
     ra.partial = w.splitk; ra.k_split = ks; ra.split_rows = kPairRows; ra.M = Ni; ra.N = Nn; ra.delta = any ? w.delta : nullptr;
     ra.mode = p.mode == GM_RESID_F32 ? 3 : p.mode == GM_OUT_BF16_SWIGLU ? 4 : p.mode == GM_OUT_BF16_GELU ? 1 : p.mode == GM_OUT_BF16_RELU ? 2 : 0;
@@ -1384,7 +1427,8 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   const float scale_log2 = 1.4426950408889634f / sqrtf((float)d.head_dim);
   bool rope_fused = false;
   for (int l = 0; l < d.n_layers; ++l) {
-    LAUNCH(Lh, F_NORM, dispatch_norm(S, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm1_g[l], (const bf16 *)bb.norm1_b[l], Ni, d.norm_eps, rms, rev()));
+    if (!(row_norm_fused && l > 0))                          // (row mode: the previous layer's FFN-down reduction wrote Xn)
+      LAUNCH(Lh, F_NORM, dispatch_norm(S, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm1_g[l], (const bf16 *)bb.norm1_b[l], Ni, d.norm_eps, rms, rev()));
     {
       const int tgs[3] = {FMX_TGT_Q, FMX_TGT_K, FMX_TGT_V};
       PairGemmParams p = base;
@@ -1400,17 +1444,17 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       p.omap = oQKV;
       // head_dim 128: a 128-column chunk is one head, so RoPE is applied in the GEMM epilogue (fp32, one rounding)
       // (a decode iteration splits the K axis of this GEMM and rotates q / k with rope_kernel after the reduction)
-      rope_fused = c->o.rope_fused && d.rope_theta > 0 && d.head_dim == 128 && pair_wide(p) && !(kv && kv->decode && w.splitk && w.n_tiles == 1);
+      rope_fused = c->o.rope_fused && d.rope_theta > 0 && d.head_dim == 128 && pair_wide(p) && !(kv && kv->decode && w.splitk && bb.row_bt && w.n_tiles == 1);
       if (rope_fused) { p.rope_cs = bb.rope_cs_t; p.rope_ld = d.max_seq; p.rope_src_mask = 3; p.row_pos = rope_pos; }
       p.reverse = rev();
       if ((e = project(p, F_GEMM_QKV, w.QKV, bb.d_qkv, w.Xn, tgs, 3, l))) return e;
     }
-    if (d.rope_theta > 0 && !rope_fused) {
+    if (d.rope_theta > 0 && !rope_fused && !row_mode) {
       const int nh = d.n_q_heads + d.n_kv_heads;
       const long long total = (long long)Ni * nh * (d.head_dim / 16);
       LAUNCH(Lh, F_ROPE, (launch_k(rope_kernel, (unsigned)((total + 255) / 256), 256, 0, S, w.QKV, bb.d_qkv, rope_pos, bb.rope_cs, Ni, nh, d.head_dim)));
     }
-    if (kv) LAUNCH(Lh, F_ATTN, (launch_k(kv_append_kernel, (Ni + 7) / 8, 256, 0, S, (const bf16 *)w.QKV, bb.d_qkv, bb.d_q, bb.d_q + bb.d_kv, Ni, l, ka)));
+    if (kv && !row_mode) LAUNCH(Lh, F_ATTN, (launch_k(kv_append_kernel, (Ni + 7) / 8, 256, 0, S, (const bf16 *)w.QKV, bb.d_qkv, bb.d_q, bb.d_q + bb.d_kv, Ni, l, ka)));
     if (kv && kv->decode) {
       DecAttnArgs da{};
       da.qkv = w.QKV; da.out = w.AttnO; da.ld_qkv = bb.d_qkv; da.ld_out = bb.d_q; da.n_q_heads = d.n_q_heads; da.n_kv_heads = d.n_kv_heads;
@@ -1450,9 +1494,11 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       set_lora(p, 0, FMX_TGT_O, l);
       p.omap = oX;
       p.reverse = rev();
+      next_norm_g = (const bf16 *)bb.norm2_g[l]; next_norm_b = (const bf16 *)bb.norm2_b[l];
       if ((e = project(p, F_GEMM_O, nullptr, d.d_model, w.AttnO, tgs, 1, l))) return e;
     }
-    LAUNCH(Lh, F_NORM, dispatch_norm(S, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm2_g[l], (const bf16 *)bb.norm2_b[l], Ni, d.norm_eps, rms, rev()));
+    if (!row_norm_fused)
+      LAUNCH(Lh, F_NORM, dispatch_norm(S, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm2_g[l], (const bf16 *)bb.norm2_b[l], Ni, d.norm_eps, rms, rev()));
     if (d.act == FMX_ACT_SWIGLU) {
       const int tgs[2] = {FMX_TGT_GATE, FMX_TGT_UP};
       PairGemmParams p = base;
@@ -1487,6 +1533,8 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       set_lora(p, 0, FMX_TGT_DOWN, l);
       p.omap = oX;
       p.reverse = rev();
+      next_norm_g = l + 1 < d.n_layers ? (const bf16 *)bb.norm1_g[l + 1] : nullptr;
+      next_norm_b = l + 1 < d.n_layers ? (const bf16 *)bb.norm1_b[l + 1] : nullptr;
       if ((e = project(p, F_GEMM_FFN_OUT, nullptr, d.d_model, w.Hid, tgs, 1, l))) return e;
     }
   }

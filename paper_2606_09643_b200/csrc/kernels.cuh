@@ -1160,6 +1160,147 @@ __global__ void __launch_bounds__(256) splitk_reduce_kernel(const SplitKReduceAr
   *reinterpret_cast<uint2 *>(a.out_bf16 + (size_t)r * a.ld_out + c) = make_uint2(pack_bf16(acc.x, acc.y), pack_bf16(acc.z, acc.w));
 }
 
+// The reduction of a residual projection (attention output, FFN down) fused with the norm that follows it: one CTA of 128 threads
+// per row.  X[row] += sum of the partials (split order) + delta + bias, then LayerNorm / RMSNorm of the updated row -> bf16 Y (the
+// same arithmetic as norm_kernel: mean, then the sum of squared deviations, fp32).  g == NULL: no norm follows (last layer).
+struct ReduceNormArgs {
+  const float *partial;            // [k_split, split_rows, N]
+  int k_split, split_rows, N;      // N = d_model (a multiple of 4, <= 4096)
+  const float *delta;              // [M, N] or NULL
+  const __nv_bfloat16 *bias;       // [N] or NULL
+  float *X;                        // [M, N] fp32 residual stream, updated in place
+  __nv_bfloat16 *Y;                // [M, N] bf16 normalised rows
+  const __nv_bfloat16 *g, *b;      // norm weight / bias (b NULL for RMSNorm)
+  float eps;
+  int rms;
+};
+__device__ __forceinline__ float block128_sum(float v, float *s_red) {        // every thread gets the sum; fixed order
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  __syncthreads();                                                            // s_red free again
+  if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = v;
+  __syncthreads();
+  return (s_red[0] + s_red[1]) + (s_red[2] + s_red[3]);
+}
+__global__ void __launch_bounds__(128) reduce_resid_norm_kernel(const ReduceNormArgs a) {
+  __shared__ float s_red[4];
+  griddep_launch();
+  griddep_wait();
+  const int r = blockIdx.x, n4 = a.N >> 2;
+  float4 v[8];
+  float s = 0.0f;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    const int c4 = threadIdx.x + 128 * j;
+    v[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (c4 >= n4) continue;
+    const int c = 4 * c4;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int ks = 0; ks < a.k_split; ++ks) {
+      const float4 q = *reinterpret_cast<const float4 *>(a.partial + ((size_t)ks * a.split_rows + r) * a.N + c);
+      acc.x += q.x; acc.y += q.y; acc.z += q.z; acc.w += q.w;
+    }
+    if (a.delta) {
+      const float4 q = *reinterpret_cast<const float4 *>(a.delta + (size_t)r * a.N + c);
+      acc.x += q.x; acc.y += q.y; acc.z += q.z; acc.w += q.w;
+    }
+    if (a.bias) {
+      const uint2 bv = *reinterpret_cast<const uint2 *>(a.bias + c);
+      acc.x += bf16_lo(bv.x); acc.y += bf16_hi(bv.x); acc.z += bf16_lo(bv.y); acc.w += bf16_hi(bv.y);
+    }
+    float4 *x = reinterpret_cast<float4 *>(a.X + (size_t)r * a.N + c);
+    float4 o = *x;
+    o.x += acc.x; o.y += acc.y; o.z += acc.z; o.w += acc.w;
+    *x = o;
+    v[j] = o;
+    s += o.x + o.y + o.z + o.w;
+  }
+  if (!a.g) return;
+  float mean = 0.0f;
+  if (!a.rms) mean = block128_sum(s, s_red) * (1.0f / a.N);
+  float q = 0.0f;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    if (threadIdx.x + 128 * j >= n4) continue;
+    const float a0 = v[j].x - mean, a1 = v[j].y - mean, a2 = v[j].z - mean, a3 = v[j].w - mean;
+    q += a0 * a0 + a1 * a1 + a2 * a2 + a3 * a3;
+  }
+  const float inv = rsqrtf(block128_sum(q, s_red) * (1.0f / a.N) + a.eps);
+  uint2 *y = reinterpret_cast<uint2 *>(a.Y + (size_t)r * a.N);
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    const int c4 = threadIdx.x + 128 * j;
+    if (c4 >= n4) continue;
+    const uint2 gg = reinterpret_cast<const uint2 *>(a.g)[c4];
+    float o0 = (v[j].x - mean) * inv * bf16_lo(gg.x), o1 = (v[j].y - mean) * inv * bf16_hi(gg.x);
+    float o2 = (v[j].z - mean) * inv * bf16_lo(gg.y), o3 = (v[j].w - mean) * inv * bf16_hi(gg.y);
+    if (a.b) {
+      const uint2 bb = reinterpret_cast<const uint2 *>(a.b)[c4];
+      o0 += bf16_lo(bb.x); o1 += bf16_hi(bb.x); o2 += bf16_lo(bb.y); o3 += bf16_hi(bb.y);
+    }
+    y[c4] = make_uint2(pack_bf16(o0, o1), pack_bf16(o2, o3));
+  }
+}
+
+// The reduction of the fused q / k / v projection of a decode iteration, with what follows it: + delta + bias, RoPE at the row's
+// cache position (rotate-half pairs (j, j + dh/2), applied in fp32 to the unrounded sums - one rounding, as in the prefill GEMM's
+// fused epilogue), bf16 store to the qkv buffer, and the k / v heads appended to the KV cache.  One thread per (row, head, 4 pairs).
+struct QkvReduceArgs {
+  const float *partial;
+  int k_split, split_rows, M, N;   // N = d_q + 2 d_kv
+  const float *delta;              // [M, N] or NULL
+  const __nv_bfloat16 *bias[3];    // q / k / v
+  __nv_bfloat16 *qkv;              // [M, N]
+  int n_q_heads, n_kv_heads, dh, layer;
+  const float2 *rope_cs;           // [max_seq, dh / 2] (cos, sin), or NULL: no rotation
+};
+__global__ void __launch_bounds__(256) qkv_reduce_rope_kernel(const QkvReduceArgs a, const KvArgs kv) {
+  griddep_launch();
+  griddep_wait();
+  const int half = a.dh >> 1, vph = half >> 2, n_heads = a.n_q_heads + 2 * a.n_kv_heads;
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (long long)a.M * n_heads * vph) return;
+  const int jv = (int)(idx % vph), h = (int)((idx / vph) % n_heads), r = (int)(idx / ((long long)vph * n_heads));
+  const int src = h < a.n_q_heads ? 0 : h < a.n_q_heads + a.n_kv_heads ? 1 : 2;
+  const int c = h * a.dh + 4 * jv;                                  // first-half columns c .. c + 3, second half c + half ..
+  const int c_src = c - (src == 0 ? 0 : src == 1 ? a.n_q_heads * a.dh : (a.n_q_heads + a.n_kv_heads) * a.dh);
+  auto column_sum = [&](int col, int col_src) {
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int ks = 0; ks < a.k_split; ++ks) {
+      const float4 q = *reinterpret_cast<const float4 *>(a.partial + ((size_t)ks * a.split_rows + r) * a.N + col);
+      acc.x += q.x; acc.y += q.y; acc.z += q.z; acc.w += q.w;
+    }
+    if (a.delta) {
+      const float4 q = *reinterpret_cast<const float4 *>(a.delta + (size_t)r * a.N + col);
+      acc.x += q.x; acc.y += q.y; acc.z += q.z; acc.w += q.w;
+    }
+    if (const __nv_bfloat16 *b = a.bias[src]) {
+      const uint2 bv = *reinterpret_cast<const uint2 *>(b + col_src);
+      acc.x += bf16_lo(bv.x); acc.y += bf16_hi(bv.x); acc.z += bf16_lo(bv.y); acc.w += bf16_hi(bv.y);
+    }
+    return acc;
+  };
+  float4 x1 = column_sum(c, c_src), x2 = column_sum(c + half, c_src + half);
+  const int pos = kv.row_cpos[r];
+  if (a.rope_cs && src < 2) {
+    const float4 *cs = reinterpret_cast<const float4 *>(a.rope_cs + (size_t)pos * half + 4 * jv);
+    const float4 ca = cs[0], cb = cs[1];                            // (cos, sin) of pairs 4 jv, 4 jv + 1 | 4 jv + 2, 4 jv + 3
+    const float4 y1 = make_float4(x1.x * ca.x - x2.x * ca.y, x1.y * ca.z - x2.y * ca.w, x1.z * cb.x - x2.z * cb.y, x1.w * cb.z - x2.w * cb.w);
+    const float4 y2 = make_float4(x2.x * ca.x + x1.x * ca.y, x2.y * ca.z + x1.y * ca.w, x2.z * cb.x + x1.z * cb.y, x2.w * cb.z + x1.w * cb.w);
+    x1 = y1; x2 = y2;
+  }
+  const uint2 o1 = make_uint2(pack_bf16(x1.x, x1.y), pack_bf16(x1.z, x1.w)), o2 = make_uint2(pack_bf16(x2.x, x2.y), pack_bf16(x2.z, x2.w));
+  __nv_bfloat16 *q = a.qkv + (size_t)r * a.N + c;
+  *reinterpret_cast<uint2 *>(q) = o1;
+  *reinterpret_cast<uint2 *>(q + half) = o2;
+  if (src > 0) {                                                    // k / v head: append to the cache
+    __nv_bfloat16 *dst = kv.cache + (long long)kv.row_slot[r] * kv.slot_stride + (long long)a.layer * kv.layer_stride + (src == 2 ? kv.kv_stride : 0) +
+                         (long long)pos * kv.d_kv + c_src;
+    *reinterpret_cast<uint2 *>(dst) = o1;
+    *reinterpret_cast<uint2 *>(dst + half) = o2;
+  }
+}
+
 // Row-wise LoRA for small batches (decode iterations): delta[row, cols of target] = s_t (x_row A_t^T) B_t^T for every target of an
 // input group, on CUDA cores (row_shrink_kernel, then row_expand_kernel).  With a handful of rows per task the segmented tensor-core path would
 // load a 256-row U tile and a slab block per (tile, task) for a few rows of work; here a row reads its own task's slab columns
@@ -1171,7 +1312,7 @@ struct RowLoraArgs {
   int n_tg;
   int tg[3];                       // target ids
   const __nv_bfloat16 *slabA[3];   // [Rcap, K] of this layer
-  const __nv_bfloat16 *slabB[3];   // [d_out, Rcap] of this layer
+  const __nv_bfloat16 *slabB[3];   // RANK-MAJOR [Rcap, d_out] of this layer (Backbone::slabBt)
   int d_out[3], col0[3];           // output width of the target, its first column in delta
   int interleave2;                 // SwiGLU: target i owns the 128-column chunks 2 q + i (feature 128 q + j -> column 256 q + 128 i + j)
   int Rcap;
@@ -1180,98 +1321,128 @@ struct RowLoraArgs {
   const float *task_scale;
 };
 // Both kernels are bound by memory latency and by the number of separate cache lines they touch, not by arithmetic, so
-//  * the work is cut fine - (row, target, 512 input columns) and (row, target, 512 output columns) - and every thread issues all
-//    its loads before it uses any;
+//  * a warp streams its share in batches of eight 16-byte loads per lane, the next batch in flight while the current one is used;
 //  * adjacent lanes read adjacent 16 bytes: a shrink warp reads 512 contiguous bytes of a slab row per instruction, an expand warp
 //    covers the r_pad * 2 contiguous bytes of a column of B with r_pad / 8 adjacent lanes (one cache-line lookup per column instead
 //    of one per 16 bytes).
-constexpr int kRowExpandCols = 512;
-constexpr int kRowShrinkK = 512;
-// u_part[kc, row, i, j] = s_t <x_row[kc-th 512 columns], A_t[j, same columns]> for every rank j of target i (fp32, [nkc, M, 3, 64]);
-// the expand kernel adds the nkc partial sums in kc order.  Warp w takes the ranks w, w + 8, ...
-__global__ void __launch_bounds__(256) row_shrink_kernel(const RowLoraArgs a, float *__restrict__ u) {
+constexpr int kRowShrinkK = 2048;                   // longest input range of one shrink warp
+__device__ __forceinline__ float dot8_bf16(const uint4 &p, const uint4 &q) {
+  return bf16_lo(p.x) * bf16_lo(q.x) + bf16_hi(p.x) * bf16_hi(q.x) + bf16_lo(p.y) * bf16_lo(q.y) + bf16_hi(p.y) * bf16_hi(q.y) +
+         bf16_lo(p.z) * bf16_lo(q.z) + bf16_hi(p.z) * bf16_hi(q.z) + bf16_lo(p.w) * bf16_lo(q.w) + bf16_hi(p.w) * bf16_hi(q.w);
+}
+// u_part[kc, row, i, j] = s_t <x_row[range kc], A_t[j, range kc]> for every rank j of target i (fp32, [nkc, M, 3, 64]); the expand
+// kernel adds the nkc partial sums in kc order.  Warp w of the CTA (row, target, range) takes the ranks 8 w .. 8 w + 7.
+__global__ void __launch_bounds__(256) row_shrink_kernel(const RowLoraArgs a, float *__restrict__ u, int k_range) {
   griddep_launch();
   griddep_wait();
   const int r = blockIdx.x, i = blockIdx.y, kc = blockIdx.z, tg = a.tg[i], warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int t = a.task_sorted[a.row_req[r]];
   const int rp = a.task_trpad[t * 7 + tg];               // padded rank (multiple of 16); 0 = no adapter on this target
-  if (rp == 0) return;
+  if (8 * warp >= rp) return;
   const float sc = a.task_scale[t * 7 + tg];
-  const int nj = rp >> 3;                                // ranks of this warp: warp + 8 jj, jj < nj
-  const int k0 = kc * kRowShrinkK + lane * 8, k1 = k0 + 256;
-  const bool ok0 = k0 < a.K, ok1 = k1 < a.K;
-  const __nv_bfloat16 *x = a.x + (size_t)r * a.K;
-  const __nv_bfloat16 *A = a.slabA[i] + (size_t)(a.task_coff[t] + warp) * a.K;
+  const int k_lo = kc * k_range, k_hi = min(a.K, k_lo + k_range);
+  const __nv_bfloat16 *x = a.x + (size_t)r * a.K + lane * 8;
+  const __nv_bfloat16 *A = a.slabA[i] + (size_t)(a.task_coff[t] + 8 * warp) * a.K + lane * 8;
   const uint4 z4 = make_uint4(0, 0, 0, 0);
-  const uint4 x0 = ok0 ? *reinterpret_cast<const uint4 *>(x + k0) : z4, x1 = ok1 ? *reinterpret_cast<const uint4 *>(x + k1) : z4;
-  uint4 v0[8], v1[8];
+  float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  auto load = [&](uint4 &xv, uint4 (&v)[8], int k0) {
+    const bool ok = k0 + lane * 8 < k_hi;
+    xv = ok ? *reinterpret_cast<const uint4 *>(x + k0) : z4;
 #pragma unroll
-  for (int jj = 0; jj < 8; ++jj) {
-    const __nv_bfloat16 *row = A + (size_t)(8 * jj) * a.K;
-    v0[jj] = (jj < nj && ok0) ? *reinterpret_cast<const uint4 *>(row + k0) : z4;
-    v1[jj] = (jj < nj && ok1) ? *reinterpret_cast<const uint4 *>(row + k1) : z4;
-  }
-  auto dot8 = [](const uint4 &p, const uint4 &q) {
-    return bf16_lo(p.x) * bf16_lo(q.x) + bf16_hi(p.x) * bf16_hi(q.x) + bf16_lo(p.y) * bf16_lo(q.y) + bf16_hi(p.y) * bf16_hi(q.y) +
-           bf16_lo(p.z) * bf16_lo(q.z) + bf16_hi(p.z) * bf16_hi(q.z) + bf16_lo(p.w) * bf16_lo(q.w) + bf16_hi(p.w) * bf16_hi(q.w);
+    for (int j = 0; j < 8; ++j) v[j] = ok ? *reinterpret_cast<const uint4 *>(A + (size_t)j * a.K + k0) : z4;
   };
-  float *dst = u + (((size_t)kc * a.M + r) * 3 + i) * 64;
+  auto comp = [&](const uint4 &xv, const uint4 (&v)[8]) {
 #pragma unroll
-  for (int jj = 0; jj < 8; ++jj) {
-    if (jj >= nj) break;
-    float acc = dot8(v0[jj], x0) + dot8(v1[jj], x1);
+    for (int j = 0; j < 8; ++j) acc[j] += dot8_bf16(v[j], xv);
+  };
+  uint4 xa, xb, va[8], vb[8];
+  load(xa, va, k_lo);
+  for (int k0 = k_lo; k0 < k_hi; k0 += 512) {
+    const bool more1 = k0 + 256 < k_hi, more2 = k0 + 512 < k_hi;
+    if (more1) load(xb, vb, k0 + 256);
+    comp(xa, va);
+    if (more2) load(xa, va, k0 + 512);
+    if (more1) comp(xb, vb);
+  }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    if (lane == 0) dst[warp + 8 * jj] = acc * sc;
+  for (int j = 0; j < 8; ++j)
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc[j] += __shfl_xor_sync(0xffffffffu, acc[j], o);
+  if (lane == 0) {
+    float4 *dst = reinterpret_cast<float4 *>(u + (((size_t)kc * a.M + r) * 3 + i) * 64 + 8 * warp);
+    dst[0] = make_float4(acc[0] * sc, acc[1] * sc, acc[2] * sc, acc[3] * sc);
+    dst[1] = make_float4(acc[4] * sc, acc[5] * sc, acc[6] * sc, acc[7] * sc);
   }
 }
-// delta[row, column of (target i, c)] = <u[row, i, :rp], B_t[c, :rp]>: 512 columns per CTA, 64 per warp.  lpc = 2 / 4 / 8 adjacent
-// lanes share a column (lane q of them owns the ranks 8 q .. 8 q + 7), so a warp load covers 32 / lpc whole columns.
+// delta[row, column of (target i, c)] = sum_j u[row, i, j] Bt_t[j, c] for the CTA's 512 columns.  B is read RANK-MAJOR (slabBt:
+// [Rcap, d_out], a task's rank rows contiguous): the column-major copy the tensor-core path uses would make every column a separate
+// 32 - 128 byte access 2 Rcap bytes apart, which DRAM serves at a fraction of its streaming rate (measured: 1.8 TB/s, 31 us for the
+// gate / up pair).  Thread (g = tid / 64, cg = tid % 64) takes the ranks 16 g .. 16 g + 15 of the columns 8 cg .. 8 cg + 7 - sixteen
+// 16-byte loads, all in flight at once, a warp reading 512 contiguous bytes per load - and the four rank groups are added in g order
+// through shared memory.
+constexpr int kRowExpandCols = 512;
 __global__ void __launch_bounds__(256) row_expand_kernel(const RowLoraArgs a, const float *__restrict__ u, int nkc) {
+  __shared__ float s_u[64];
+  __shared__ __align__(16) float s_acc[4][kRowExpandCols];
   griddep_launch();
   griddep_wait();
-  const int r = blockIdx.x, i = blockIdx.y, tg = a.tg[i], warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int r = blockIdx.x, i = blockIdx.y, tg = a.tg[i], g = threadIdx.x >> 6, cg = threadIdx.x & 63;
   const int dout = a.d_out[i];
-  const int c_base = blockIdx.z * kRowExpandCols + warp * 64;
+  const int c_base = blockIdx.z * kRowExpandCols;
   if (c_base >= dout) return;
   const int t = a.task_sorted[a.row_req[r]];
   const int rp = a.task_trpad[t * 7 + tg];
   float *dst = a.delta + (size_t)r * a.ld_delta;
-  auto col_of = [&](int c) { return a.interleave2 ? ((c >> 7) * 256 + i * 128 + (c & 127)) : a.col0[i] + c; };
+  const int c2 = c_base + 2 * threadIdx.x;               // the two columns this thread writes at the end
+  const int o2 = a.interleave2 ? ((c2 >> 7) * 256 + i * 128 + (c2 & 127)) : a.col0[i] + c2;
   if (rp == 0) {                                         // no adapter: the reduce kernel adds the delta unconditionally
-    if (c_base + lane < dout) dst[col_of(c_base + lane)] = 0.0f;
-    if (c_base + 32 + lane < dout) dst[col_of(c_base + 32 + lane)] = 0.0f;
+    if (c2 < dout) *reinterpret_cast<float2 *>(dst + o2) = make_float2(0.f, 0.f);
     return;
   }
-  const int lpc = rp <= 16 ? 2 : rp <= 32 ? 4 : 8, sh = rp <= 16 ? 1 : rp <= 32 ? 2 : 3;
-  const int q = lane & (lpc - 1), cs = lane >> sh, cpi = 32 >> sh, n_ld = 64 / cpi;   // 4 / 8 / 16 loads per lane
-  const bool live = 8 * q < rp;
+  const int c = c_base + 8 * cg;
+  const bool live = 16 * g < rp && c < dout;
   const uint4 z4 = make_uint4(0, 0, 0, 0);
-  const __nv_bfloat16 *B = a.slabB[i] + a.task_coff[t] + 8 * q;
+  const __nv_bfloat16 *B = a.slabB[i] + (size_t)(a.task_coff[t] + 16 * g) * dout + c;
   uint4 v[16];
 #pragma unroll
-  for (int n = 0; n < 16; ++n) {
-    const int c = c_base + n * cpi + cs;
-    v[n] = (n < n_ld && live && c < dout) ? *reinterpret_cast<const uint4 *>(B + (size_t)c * a.Rcap) : z4;
+  for (int j = 0; j < 16; ++j) v[j] = live ? *reinterpret_cast<const uint4 *>(B + (size_t)j * dout) : z4;
+  if (threadIdx.x < 64) {
+    float s = 0.0f;
+    if ((int)threadIdx.x < rp)
+      for (int kc = 0; kc < nkc; ++kc) s += u[(((size_t)kc * a.M + r) * 3 + i) * 64 + threadIdx.x];
+    s_u[threadIdx.x] = s;
   }
-  float uu[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  if (live)
-    for (int kc = 0; kc < nkc; ++kc) {
-      const float4 *src = reinterpret_cast<const float4 *>(u + (((size_t)kc * a.M + r) * 3 + i) * 64 + 8 * q);
-      const float4 p0 = src[0], p1 = src[1];
-      uu[0] += p0.x; uu[1] += p0.y; uu[2] += p0.z; uu[3] += p0.w; uu[4] += p1.x; uu[5] += p1.y; uu[6] += p1.z; uu[7] += p1.w;
-    }
+  __syncthreads();
+  float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-  for (int n = 0; n < 16; ++n) {
-    if (n >= n_ld) break;
-    float acc = uu[0] * bf16_lo(v[n].x) + uu[1] * bf16_hi(v[n].x) + uu[2] * bf16_lo(v[n].y) + uu[3] * bf16_hi(v[n].y) +
-                uu[4] * bf16_lo(v[n].z) + uu[5] * bf16_hi(v[n].z) + uu[6] * bf16_lo(v[n].w) + uu[7] * bf16_hi(v[n].w);
-    acc += __shfl_xor_sync(0xffffffffu, acc, 1);
-    if (lpc > 2) acc += __shfl_xor_sync(0xffffffffu, acc, 2);
-    if (lpc > 4) acc += __shfl_xor_sync(0xffffffffu, acc, 4);
-    const int c = c_base + n * cpi + cs;
-    if (q == 0 && c < dout) dst[col_of(c)] = acc;
+  for (int j = 0; j < 16; ++j) {
+    const float uj = s_u[16 * g + j];
+    acc[0] = fmaf(uj, bf16_lo(v[j].x), acc[0]); acc[1] = fmaf(uj, bf16_hi(v[j].x), acc[1]);
+    acc[2] = fmaf(uj, bf16_lo(v[j].y), acc[2]); acc[3] = fmaf(uj, bf16_hi(v[j].y), acc[3]);
+    acc[4] = fmaf(uj, bf16_lo(v[j].z), acc[4]); acc[5] = fmaf(uj, bf16_hi(v[j].z), acc[5]);
+    acc[6] = fmaf(uj, bf16_lo(v[j].w), acc[6]); acc[7] = fmaf(uj, bf16_hi(v[j].w), acc[7]);
   }
+  *reinterpret_cast<float4 *>(&s_acc[g][8 * cg]) = make_float4(acc[0], acc[1], acc[2], acc[3]);
+  *reinterpret_cast<float4 *>(&s_acc[g][8 * cg + 4]) = make_float4(acc[4], acc[5], acc[6], acc[7]);
+  __syncthreads();
+  if (c2 < dout) {
+    const int cl = 2 * threadIdx.x;
+    float2 o = *reinterpret_cast<const float2 *>(&s_acc[0][cl]);
+#pragma unroll
+    for (int gg = 1; gg < 4; ++gg) {                     // rank groups past the task's rank hold zeros
+      const float2 q = *reinterpret_cast<const float2 *>(&s_acc[gg][cl]);
+      o.x += q.x; o.y += q.y;
+    }
+    *reinterpret_cast<float2 *>(dst + o2) = o;
+  }
+}
+
+// Registration: the rank-major copy of one layer's B of an adapter, Bt[j, c] = B[c, j] for j < rank, zero for the padding ranks.
+__global__ void lora_bt_fill_kernel(const __nv_bfloat16 *__restrict__ B, __nv_bfloat16 *__restrict__ Bt, int dout, int rank, int rp) {
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (size_t)dout * rp) return;
+  const int j = (int)(idx / dout), c = (int)(idx - (size_t)j * dout);
+  Bt[idx] = j < rank ? B[(size_t)c * rank + j] : __float2bfloat16(0.0f);
 }
 
 }  // namespace fmx
