@@ -468,15 +468,25 @@ def measure_decode(sess, wl, steps=16, warm=3):
     per_layer = 2 * (bb.d_model * (bb.d_q + 2 * bb.d_kv) + bb.d_q * bb.d_model + (3 if bb.act == "swiglu" else 2) * bb.d_model * bb.d_ffn)
     weight_bytes = bb.n_layers * per_layer + 2 * bb.vocab * bb.d_model          # backbone matrices + LM head, bf16
     kv_bytes = kv_rows / steps * bb.n_layers * 2 * bb.d_kv * 2
+    from fmx_workloads.spec import target_dims
+    adapter_bytes = 0                                                            # A and B of every adapter of the DISTINCT tasks in the batch, once
+    for t in sorted(set(int(x) for x in wl.task_ids)):
+        for ad in wl.tasks[t].adapters:
+            d_in, d_out = target_dims(bb, ad.target)
+            adapter_bytes += bb.n_layers * 2 * ad.rank * (d_in + d_out)
     pk = peaks()
-    gbs = (weight_bytes + kv_bytes) / (ms * 1e-3) / 1e9
+    total = weight_bytes + kv_bytes + adapter_bytes
+    gbs = total / (ms * 1e-3) / 1e9
     return {"what": "fmx_decode_step: one new token for each of the batch's sequences per iteration, KV cache, mixed tasks, greedy tokens fed back on the device",
             "requests": B, "tokens_per_s": round(B / (ms * 1e-3), 1), "ms_per_step": round(ms, 4), "steps": steps, "launches_per_step": launches,
-            "mean_cached_tokens": round(kv_rows / steps / B, 1), "families": families,
+            "mean_cached_tokens": round(kv_rows / steps / B, 1), "distinct_tasks": len(set(int(x) for x in wl.task_ids)), "families": families,
             "roofline": {"bound": "hbm", "achieved": round(gbs, 1), "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": round(gbs / pk["hbm_gbs"], 4),
-                         "bytes_per_step": int(weight_bytes + kv_bytes),
-                         "note": "algorithmic bytes = every backbone and LM-head weight once + the cached k / v rows read; the projection GEMMs here are the "
-                                 "prefill kernel at M = batch rows (one 256-row tile): few CTAs stream the weights, a small-M split-K kernel is the next step"}}
+                         "bytes_per_step": int(total),
+                         "bytes": {"backbone_and_lm_head": int(weight_bytes), "kv_cache": int(kv_bytes), "lora_adapters": int(adapter_bytes)},
+                         "note": "algorithmic bytes = every backbone and LM-head weight once + the cached k / v rows read + the LoRA matrices of the "
+                                 "distinct tasks in the batch once (unpadded ranks).  The iteration is bound by kernel count and dependent memory "
+                                 "latency (17 launches per layer), not by bandwidth; families are timed with plain launches and an event pair per "
+                                 "launch, so their sum exceeds the graph-replayed iteration"}}
 
 
 def light(line):

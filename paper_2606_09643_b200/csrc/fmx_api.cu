@@ -22,6 +22,7 @@
 #include "gemm.cuh"
 #include "kernels.cuh"
 #include "pair_gemm.cuh"
+#include "row_gemm.cuh"
 
 using namespace fmx;
 typedef __nv_bfloat16 bf16;
@@ -106,6 +107,7 @@ struct Opts {
   int attn_short = 2;     // 0: generic kernel, 1: pipelined mma.sync kernel, 2: tcgen05 head-pair kernel where it applies
   int graph = 1;
   int attn_impl = FMX_ATTN_AUTO;
+  int decode_rowgemm = 1; // decode iterations of <= 128 rows: projections on the lean mma.sync kernel (row_gemm.cuh) instead of the pair GEMM
   int decode_fork = 1;    // decode iterations: row-wise LoRA kernels on the auxiliary stream beside the projection GEMM
 };
 
@@ -500,6 +502,10 @@ int set_kernel_attrs() {
   CU_OK((cudaFuncSetAttribute(pair_gemm_kernel<256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<256, true>())));
   CU_OK((cudaFuncSetAttribute(pair_gemm_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<128, false>())));
   CU_OK((cudaFuncSetAttribute(pair_gemm_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<128, true>())));
+  CU_OK((cudaFuncSetAttribute(row_gemm_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, row_gemm_smem<1>())));
+  CU_OK((cudaFuncSetAttribute(row_gemm_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, row_gemm_smem<2>())));
+  CU_OK((cudaFuncSetAttribute(row_gemm_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, row_gemm_smem<4>())));
+  CU_OK((cudaFuncSetAttribute(row_gemm_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, row_gemm_smem<8>())));
   CU_OK((cudaFuncSetAttribute(decode_attention_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, decode_attention_smem<32>())));
   CU_OK((cudaFuncSetAttribute(decode_attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, decode_attention_smem<64>())));
   CU_OK((cudaFuncSetAttribute(decode_attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, decode_attention_smem<128>())));
@@ -1334,7 +1340,8 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
   // row mode fuses what follows a reduction into it: RoPE + the cache append after q / k / v, the next norm after a residual update
   const bool row_norm_fused = row_mode && d.d_model <= 4096;
   const bf16 *next_norm_g = nullptr, *next_norm_b = nullptr;
-  auto project = [&](PairGemmParams &p, int family, __nv_bfloat16 *out_bf16, int ld_out, const __nv_bfloat16 *x, const int *tgs, int n_tg, int layer) -> int {
+  auto project = [&](PairGemmParams &p, int family, __nv_bfloat16 *out_bf16, int ld_out, const __nv_bfloat16 *x, const int *tgs, int n_tg, int layer,
+                     const void *W0, const void *W1, const void *W2) -> int {
     if (!row_mode) { LAUNCH(Lh, family, launch_pair_gemm(c, S, p)); return FMX_OK; }
     const int Nn = p.n_chunks * 128;
     bool any = false;
@@ -1361,20 +1368,42 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       LAUNCH(Lh, F_SHRINK, (launch_k(row_expand_kernel, dim3(Ni, n_tg, (max_dout + kRowExpandCols - 1) / kRowExpandCols), 256, 0, SL, la, (const float *)w.rowu, nkc)));
       if (fork) CU_OK(cudaEventRecord(c->join_ev, c->aux));
     }
-    const int tiles = pair_wide(p) ? p.n_chunks / 2 : p.n_chunks, pairs = c->sm_count / 2, nK = (p.K + kBK - 1) / kBK;
-    int ks = 1, kbps = nK;
-    if (2 * tiles <= pairs) {
-      ks = std::min(kSplitMax, pairs / tiles);
-      kbps = (nK + ks - 1) / ks;
-      ks = (nK + kbps - 1) / kbps;
+    const int nK = (p.K + kBK - 1) / kBK;
+    int ks = 1, split_rows = kPairRows;
+    if (Ni <= 128 && c->o.decode_rowgemm) {
+      // the lean small-M kernel (row_gemm.cuh): 128-column slices x K slices, ~2 CTAs per SM, at least two 64-wide chunks per slice
+      RowGemmArgs ga{};
+      ga.x = x; ga.M = Ni; ga.K = p.K; ga.N = Nn; ga.interleave2 = p.interleave2;
+      ga.W[0] = (const bf16 *)W0; ga.W[1] = (const bf16 *)W1; ga.W[2] = (const bf16 *)W2;
+      for (int i = 0; i < 3; ++i) ga.src_end_col[i] = p.src_end[i] >= (1 << 20) ? (1 << 30) : p.src_end[i] * 128;
+      const int n_slices = Nn / kRgCols;
+      split_rows = (Ni + 15) / 16 * 16;
+      ks = std::max(1, std::min((2 * c->sm_count + n_slices - 1) / n_slices, nK / 2));
+      while (ks > 1 && (size_t)ks * split_rows * Nn > (size_t)kPairRows * splitk_cols(bb)) --ks;      // the partials' workspace
+      const int cps = (nK + ks - 1) / ks;
+      ks = (nK + cps - 1) / cps;
+      ga.chunks_per_split = cps; ga.split_rows = split_rows; ga.partial = w.splitk;
+      const dim3 grid(n_slices, ks);
+      if (Ni <= 16) LAUNCH(Lh, family, (launch_k(row_gemm_kernel<1>, grid, 256, row_gemm_smem<1>(), S, ga)));
+      else if (Ni <= 32) LAUNCH(Lh, family, (launch_k(row_gemm_kernel<2>, grid, 256, row_gemm_smem<2>(), S, ga)));
+      else if (Ni <= 64) LAUNCH(Lh, family, (launch_k(row_gemm_kernel<4>, grid, 256, row_gemm_smem<4>(), S, ga)));
+      else LAUNCH(Lh, family, (launch_k(row_gemm_kernel<8>, grid, 256, row_gemm_smem<8>(), S, ga)));
+    } else {
+      const int tiles = pair_wide(p) ? p.n_chunks / 2 : p.n_chunks, pairs = c->sm_count / 2;
+      int kbps = nK;
+      if (2 * tiles <= pairs) {
+        ks = std::min(kSplitMax, pairs / tiles);
+        kbps = (nK + ks - 1) / ks;
+        ks = (nK + kbps - 1) / kbps;
+      }
+      if (int e2 = encode_2d(c, &p.pmap, w.splitk, (uint64_t)ks * kPairRows, Nn, Nn, 128, true)) return e2;
+      p.k_split = ks; p.kb_per_split = kbps; p.split_rows = kPairRows;
+      LAUNCH(Lh, family, launch_pair_gemm(c, S, p));
     }
-    if (int e2 = encode_2d(c, &p.pmap, w.splitk, (uint64_t)ks * kPairRows, Nn, Nn, 128, true)) return e2;
-    p.k_split = ks; p.kb_per_split = kbps; p.split_rows = kPairRows;
-    LAUNCH(Lh, family, launch_pair_gemm(c, S, p));
     if (fork) CU_OK(cudaStreamWaitEvent(s, c->join_ev, 0));
     if (family == F_GEMM_QKV) {                              // + RoPE at the cache position + append k / v to the cache
       QkvReduceArgs qa{};
-      qa.partial = w.splitk; qa.k_split = ks; qa.split_rows = kPairRows; qa.M = Ni; qa.N = Nn; qa.delta = any ? w.delta : nullptr;
+      qa.partial = w.splitk; qa.k_split = ks; qa.split_rows = split_rows; qa.M = Ni; qa.N = Nn; qa.delta = any ? w.delta : nullptr;
       for (int i = 0; i < 3; ++i) qa.bias[i] = p.bias[i];
       qa.qkv = out_bf16; qa.n_q_heads = d.n_q_heads; qa.n_kv_heads = d.n_kv_heads; qa.dh = d.head_dim; qa.layer = layer;
       qa.rope_cs = d.rope_theta > 0 ? bb.rope_cs : nullptr;
@@ -1384,13 +1413,13 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     }
     if (p.mode == GM_RESID_F32 && row_norm_fused) {          // + the norm that follows the residual update
       ReduceNormArgs na{};
-      na.partial = w.splitk; na.k_split = ks; na.split_rows = kPairRows; na.N = Nn; na.delta = any ? w.delta : nullptr; na.bias = p.bias[0];
+      na.partial = w.splitk; na.k_split = ks; na.split_rows = split_rows; na.N = Nn; na.delta = any ? w.delta : nullptr; na.bias = p.bias[0];
       na.X = w.X; na.Y = w.Xn; na.g = next_norm_g; na.b = next_norm_b; na.eps = d.norm_eps; na.rms = d.norm == FMX_NORM_RMSNORM;
       LAUNCH(Lh, family, (launch_k(reduce_resid_norm_kernel, (unsigned)Ni, 128, 0, S, na)));
       return FMX_OK;
     }
     SplitKReduceArgs ra{};
-    ra.partial = w.splitk; ra.k_split = ks; ra.split_rows = kPairRows; ra.M = Ni; ra.N = Nn; ra.delta = any ? w.delta : nullptr;
+    ra.partial = w.splitk; ra.k_split = ks; ra.split_rows = split_rows; ra.M = Ni; ra.N = Nn; ra.delta = any ? w.delta : nullptr;
     ra.mode = p.mode == GM_RESID_F32 ? 3 : p.mode == GM_OUT_BF16_SWIGLU ? 4 : p.mode == GM_OUT_BF16_GELU ? 1 : p.mode == GM_OUT_BF16_RELU ? 2 : 0;
     for (int i = 0; i < 3; ++i) { ra.bias[i] = p.bias[i]; ra.src_end_col[i] = p.src_end[i] >= (1 << 20) ? (1 << 30) : p.src_end[i] * 128; }
     ra.out_bf16 = out_bf16; ra.X = w.X; ra.ld_out = ld_out;
@@ -1447,7 +1476,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       rope_fused = c->o.rope_fused && d.rope_theta > 0 && d.head_dim == 128 && pair_wide(p) && !(kv && kv->decode && w.splitk && bb.row_bt && w.n_tiles == 1);
       if (rope_fused) { p.rope_cs = bb.rope_cs_t; p.rope_ld = d.max_seq; p.rope_src_mask = 3; p.row_pos = rope_pos; }
       p.reverse = rev();
-      if ((e = project(p, F_GEMM_QKV, w.QKV, bb.d_qkv, w.Xn, tgs, 3, l))) return e;
+      if ((e = project(p, F_GEMM_QKV, w.QKV, bb.d_qkv, w.Xn, tgs, 3, l, bb.Wq[l], bb.Wk[l], bb.Wv[l]))) return e;
     }
     if (d.rope_theta > 0 && !rope_fused && !row_mode) {
       const int nh = d.n_q_heads + d.n_kv_heads;
@@ -1495,7 +1524,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       p.omap = oX;
       p.reverse = rev();
       next_norm_g = (const bf16 *)bb.norm2_g[l]; next_norm_b = (const bf16 *)bb.norm2_b[l];
-      if ((e = project(p, F_GEMM_O, nullptr, d.d_model, w.AttnO, tgs, 1, l))) return e;
+      if ((e = project(p, F_GEMM_O, nullptr, d.d_model, w.AttnO, tgs, 1, l, bb.Wo[l], nullptr, nullptr))) return e;
     }
     if (!row_norm_fused)
       LAUNCH(Lh, F_NORM, dispatch_norm(S, d.d_model, w.X, w.Xn, (const bf16 *)bb.norm2_g[l], (const bf16 *)bb.norm2_b[l], Ni, d.norm_eps, rms, rev()));
@@ -1510,7 +1539,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       set_lora(p, 0, FMX_TGT_GATE, l); set_lora(p, 1, FMX_TGT_UP, l);
       p.omap = oHid;
       p.reverse = rev();
-      if ((e = project(p, F_GEMM_FFN_IN, w.Hid, d.d_ffn, w.Xn, tgs, 2, l))) return e;
+      if ((e = project(p, F_GEMM_FFN_IN, w.Hid, d.d_ffn, w.Xn, tgs, 2, l, bb.Wgate[l], bb.Wup[l], nullptr))) return e;
     } else {
       const int tgs[1] = {FMX_TGT_UP};
       PairGemmParams p = base;
@@ -1521,7 +1550,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       set_lora(p, 0, FMX_TGT_UP, l);
       p.omap = oHid;
       p.reverse = rev();
-      if ((e = project(p, F_GEMM_FFN_IN, w.Hid, d.d_ffn, w.Xn, tgs, 1, l))) return e;
+      if ((e = project(p, F_GEMM_FFN_IN, w.Hid, d.d_ffn, w.Xn, tgs, 1, l, bb.Wup[l], nullptr, nullptr))) return e;
     }
     {
       const int tgs[1] = {FMX_TGT_DOWN};
@@ -1535,7 +1564,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       p.reverse = rev();
       next_norm_g = l + 1 < d.n_layers ? (const bf16 *)bb.norm1_g[l + 1] : nullptr;
       next_norm_b = l + 1 < d.n_layers ? (const bf16 *)bb.norm1_b[l + 1] : nullptr;
-      if ((e = project(p, F_GEMM_FFN_OUT, nullptr, d.d_model, w.Hid, tgs, 1, l))) return e;
+      if ((e = project(p, F_GEMM_FFN_OUT, nullptr, d.d_model, w.Hid, tgs, 1, l, bb.Wdown[l], nullptr, nullptr))) return e;
     }
   }
   // ---- S4-S6 (skipped by a decode step that wants LM scores only) ----
@@ -2001,6 +2030,9 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
       return FMX_OK;
     case FMX_OPT_HALF_TILES:
       c->o.half_tiles = value ? 1 : 0;
+      return FMX_OK;
+    case FMX_OPT_DECODE_ROWGEMM:
+      c->o.decode_rowgemm = value ? 1 : 0;
       return FMX_OK;
     case FMX_OPT_DECODE_FORK:
       c->o.decode_fork = value ? 1 : 0;

@@ -65,6 +65,8 @@ enum {
   FMX_OPT_DECODE_FORK = 13,      /* 1 (default): in a decode iteration the row-wise LoRA kernels of a projection run on the
                                     context's auxiliary stream beside the projection GEMM (both are latency-bound) and join
                                     before the reduction; set 0 when the serving stream belongs to an SM partition */
+  FMX_OPT_DECODE_ROWGEMM = 14,   /* 1 (default): decode iterations of <= 128 rows run their projections on the lean mma.sync
+                                    kernel (row_gemm.cuh); 0 = the pair GEMM in partial-output mode */
   FMX_OPT_PDL = 2                /* programmatic dependent launch of the forward's kernels:
                                     0 = off, 1 = always, 2 (default) = only for batches of <= 4096 token rows */
 };

@@ -73,19 +73,60 @@ __device__ inline V block_exclusive_scan(V *a, int n, V *scratch) {
 __device__ inline long long block_exclusive_scan_ll(long long *a, int n, long long *scratch) { return block_exclusive_scan<long long>(a, n, scratch); }
 __device__ inline int block_exclusive_scan_i(int *a, int n, int *scratch) { return block_exclusive_scan<int>(a, n, scratch); }
 
+// Exclusive scan of f(0) .. f(n - 1) written to out[0 .. n) (global), f evaluated twice per element; returns the total.
+template <typename V, typename F>
+__device__ inline V block_exclusive_scan_fn(int n, F f, V *out, V *scratch) {
+  const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, wid = tid >> 5;
+  const int per = (n + nt - 1) / nt;
+  const int lo = min(tid * per, n), hi = min(lo + per, n);
+  V s = 0;
+  for (int i = lo; i < hi; ++i) s += f(i);
+  V incl = s;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const V v = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += v; }
+  if (lane == 31) scratch[wid] = incl;
+  __syncthreads();
+  if (wid == 0) {
+    const V w = lane < (nt >> 5) ? scratch[lane] : V(0);
+    V wi = w;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const V v = __shfl_up_sync(0xffffffffu, wi, d); if (lane >= d) wi += v; }
+    scratch[lane] = wi - w;
+    if (lane == 31) scratch[32] = wi;
+  }
+  __syncthreads();
+  V run = scratch[wid] + incl - s;
+  for (int i = lo; i < hi; ++i) { out[i] = run; run += f(i); }
+  const V total = scratch[32];
+  __syncthreads();
+  return total;
+}
+
 // One CTA.  Stable counting sort of request indices by task id, then the prefix tables and the
 // (row-tile, task) block table the segmented GEMMs walk.  Integer only; deterministic.
+// The ids and lengths are read from global memory once (ids to shared memory, lengths to registers); ranking and the scans of the
+// counts and the sorted lengths run in shared memory, the offset tables are scanned from their defining expressions and written
+// once - the kernel's time is the handful of dependent global round trips that remain, not arithmetic.
 __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortArgs a) {
   __shared__ int s_cnt[1024 + 1];          // per-task count, then task_req_off
   __shared__ int s_tok[1024 + 1];          // task_tok_off
   __shared__ int s_scratch[33];
   __shared__ long long s_scratch_ll[33];
-  __shared__ int s_rank[4096];             // rank of request i within its task
+  __shared__ unsigned short s_task[4096];  // task id of request i (T <= 1024)
+  __shared__ unsigned short s_rank[4096];  // rank of request i within its task
+  __shared__ int s_slen[4096 + 1];         // lengths in sorted order, then cu_tok
   const int tid = threadIdx.x, B = a.B, T = a.T;
   const SegTables &t = a.t;
   griddep_launch();
   griddep_wait();
 
+  int len_r[4];                            // lengths of the requests tid, tid + 1024, ... (B <= 4096)
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const int i = tid + k * kSortThreads;
+    len_r[k] = i < B ? t.lengths[i] : 0;
+    if (i < B) s_task[i] = (unsigned short)t.task_ids[i];
+  }
   for (int i = tid; i <= T; i += blockDim.x) s_cnt[i] = 0;
   __syncthreads();
   // (1) stable rank within task: warp 0 walks the requests 32 at a time, in order.
@@ -93,14 +134,14 @@ __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortAr
     for (int base = 0; base < B; base += 32) {
       const int i = base + tid;
       const bool ok = i < B;
-      const int key = ok ? t.task_ids[i] : -1 - tid;           // inactive lanes get unique keys
+      const int key = ok ? (int)s_task[i] : -1 - tid;          // inactive lanes get unique keys
       const unsigned m = __match_any_sync(0xffffffffu, key);
       const int leader = __ffs(m) - 1;
       const int rank_in_chunk = __popc(m & ((1u << tid) - 1u));
       int start = 0;
       if (ok && tid == leader) { start = s_cnt[key]; s_cnt[key] = start + __popc(m); }
       start = __shfl_sync(0xffffffffu, start, leader);
-      if (ok) s_rank[i] = start + rank_in_chunk;
+      if (ok) s_rank[i] = (unsigned short)(start + rank_in_chunk);
       __syncwarp();
     }
   }
@@ -111,29 +152,34 @@ __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortAr
   block_exclusive_scan_i(s_cnt, T + 1, s_scratch);
   for (int i = tid; i <= T; i += blockDim.x) t.task_req_off[i] = s_cnt[i];
   // (3) perm / inv_perm / sorted lengths
-  for (int i = tid; i < B; i += blockDim.x) {
-    const int tk = t.task_ids[i];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const int i = tid + k * kSortThreads;
+    if (i >= B) continue;
+    const int tk = s_task[i];
     const int pos = s_cnt[tk] + s_rank[i];
     t.perm[pos] = i;
     t.inv_perm[i] = pos;
     t.task_sorted[pos] = tk;
-    t.cu_tok[pos] = t.lengths[i];
+    s_slen[pos] = len_r[k];
   }
-  if (tid == 0) t.cu_tok[B] = 0;
+  if (tid == 0) s_slen[B] = 0;
   __syncthreads();
   // (4) cu_tok = exclusive scan of the sorted lengths; task_tok_off
-  block_exclusive_scan_i(t.cu_tok, B + 1, s_scratch);
-  for (int i = tid; i <= T; i += blockDim.x) { const int v = t.cu_tok[s_cnt[i]]; s_tok[i] = v; t.task_tok_off[i] = v; }
+  block_exclusive_scan_i(s_slen, B + 1, s_scratch);
+  for (int i = tid; i <= B; i += blockDim.x) t.cu_tok[i] = s_slen[i];
+  for (int i = tid; i <= T; i += blockDim.x) { const int v = s_slen[s_cnt[i]]; s_tok[i] = v; t.task_tok_off[i] = v; }
   // (5) input / output offsets in ORIGINAL request order
-  for (int i = tid; i < B; i += blockDim.x) {
-    const int ch = a.task_enc_ch ? max(a.task_enc_ch[t.task_ids[i]], 1) : 1;
-    t.in_off[i] = (long long)t.lengths[i] * a.in_per_tok + a.in_per_req * ch;
-    t.out_off[i] = (long long)a.task_head_out[t.task_ids[i]] * (a.task_head_kind[t.task_ids[i]] == 4 ? t.lengths[i] : 1);
-  }
-  if (tid == 0) { t.in_off[B] = 0; t.out_off[B] = 0; }
-  __syncthreads();
-  block_exclusive_scan_ll(t.in_off, B + 1, s_scratch_ll);
-  block_exclusive_scan_ll(t.out_off, B + 1, s_scratch_ll);
+  block_exclusive_scan_fn<long long>(B + 1, [&](int i) -> long long {
+    if (i >= B) return 0;
+    const int ch = a.task_enc_ch ? max(a.task_enc_ch[s_task[i]], 1) : 1;
+    return (long long)t.lengths[i] * a.in_per_tok + a.in_per_req * ch;
+  }, t.in_off, s_scratch_ll);
+  block_exclusive_scan_fn<long long>(B + 1, [&](int i) -> long long {
+    if (i >= B) return 0;
+    const int tk = s_task[i];
+    return (long long)a.task_head_out[tk] * (a.task_head_kind[tk] == 4 ? t.lengths[i] : 1);
+  }, t.out_off, s_scratch_ll);
   // (6) block table: for each row tile, the non-empty task segments that intersect it.
   const int n_tok = s_tok[T];
   auto first_task_after = [&](int row) {     // smallest task with tok_off[task+1] > row
@@ -141,15 +187,13 @@ __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortAr
     while (lo < hi) { int mid = (lo + hi) >> 1; if (s_tok[mid + 1] > row) hi = mid; else lo = mid + 1; }
     return lo;
   };
-  for (int m = tid; m < a.n_tiles; m += blockDim.x) {
+  auto tile_blocks = [&](int m) {
     const int r0 = m * a.tile_rows, r1 = min(r0 + a.tile_rows, n_tok);
     int cnt = 0;
     for (int k = first_task_after(r0); k < T && s_tok[k] < r1; ++k) cnt += (s_tok[k + 1] > s_tok[k]);
-    t.tile_blk_off[m] = cnt;
-  }
-  if (tid == 0) t.tile_blk_off[a.n_tiles] = 0;
-  __syncthreads();
-  const int n_blk = block_exclusive_scan_i(t.tile_blk_off, a.n_tiles + 1, s_scratch);
+    return cnt;
+  };
+  const int n_blk = block_exclusive_scan_fn<int>(a.n_tiles + 1, [&](int m) { return m < a.n_tiles ? tile_blocks(m) : 0; }, t.tile_blk_off, s_scratch);
   if (tid == 0) *t.n_blk = n_blk;
   for (int m = tid; m < a.n_tiles; m += blockDim.x) {
     const int r0 = m * a.tile_rows, r1 = min(r0 + a.tile_rows, n_tok);
