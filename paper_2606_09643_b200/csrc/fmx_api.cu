@@ -1378,7 +1378,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       for (int i = 0; i < 3; ++i) ga.src_end_col[i] = p.src_end[i] >= (1 << 20) ? (1 << 30) : p.src_end[i] * 128;
       const int n_slices = Nn / kRgCols;
       split_rows = (Ni + 15) / 16 * 16;
-      ks = std::max(1, std::min((2 * c->sm_count + n_slices - 1) / n_slices, nK / 2));
+      ks = std::max(1, std::min(2 * c->sm_count / n_slices, nK / 2));      // one wave at two CTAs per SM
       while (ks > 1 && (size_t)ks * split_rows * Nn > (size_t)kPairRows * splitk_cols(bb)) --ks;      // the partials' workspace
       const int cps = (nK + ks - 1) / ks;
       ks = (nK + cps - 1) / cps;

@@ -1158,6 +1158,7 @@ __global__ void __launch_bounds__(256) splitk_reduce_kernel(const SplitKReduceAr
   const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   auto column_sum = [&](int r, int c) {
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 8
     for (int ks = 0; ks < a.k_split; ++ks) {
       const float4 v = *reinterpret_cast<const float4 *>(a.partial + ((size_t)ks * a.split_rows + r) * a.N + c);
       acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
@@ -1232,18 +1233,25 @@ __global__ void __launch_bounds__(128) reduce_resid_norm_kernel(const ReduceNorm
   griddep_wait();
   const int r = blockIdx.x, n4 = a.N >> 2;
   float4 v[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) v[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+  const float *part = a.partial + (size_t)r * a.N + 4 * threadIdx.x;
+#pragma unroll 4
+  for (int ks = 0; ks < a.k_split; ++ks) {                      // split order; the loads of four splits in flight at a time
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      if (threadIdx.x + 128 * j >= n4) continue;
+      const float4 q = *reinterpret_cast<const float4 *>(part + (size_t)ks * a.split_rows * a.N + 512 * j);
+      v[j].x += q.x; v[j].y += q.y; v[j].z += q.z; v[j].w += q.w;
+    }
+  }
   float s = 0.0f;
 #pragma unroll
   for (int j = 0; j < 8; ++j) {
     const int c4 = threadIdx.x + 128 * j;
-    v[j] = make_float4(0.f, 0.f, 0.f, 0.f);
     if (c4 >= n4) continue;
     const int c = 4 * c4;
-    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int ks = 0; ks < a.k_split; ++ks) {
-      const float4 q = *reinterpret_cast<const float4 *>(a.partial + ((size_t)ks * a.split_rows + r) * a.N + c);
-      acc.x += q.x; acc.y += q.y; acc.z += q.z; acc.w += q.w;
-    }
+    float4 acc = v[j];
     if (a.delta) {
       const float4 q = *reinterpret_cast<const float4 *>(a.delta + (size_t)r * a.N + c);
       acc.x += q.x; acc.y += q.y; acc.z += q.z; acc.w += q.w;
@@ -1310,6 +1318,7 @@ __global__ void __launch_bounds__(256) qkv_reduce_rope_kernel(const QkvReduceArg
   const int c_src = c - (src == 0 ? 0 : src == 1 ? a.n_q_heads * a.dh : (a.n_q_heads + a.n_kv_heads) * a.dh);
   auto column_sum = [&](int col, int col_src) {
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 8
     for (int ks = 0; ks < a.k_split; ++ks) {
       const float4 q = *reinterpret_cast<const float4 *>(a.partial + ((size_t)ks * a.split_rows + r) * a.N + col);
       acc.x += q.x; acc.y += q.y; acc.z += q.z; acc.w += q.w;
