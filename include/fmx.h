@@ -252,6 +252,21 @@ int fmx_decode_step(fmx_ctx *ctx, fmx_backbone_t bb, const int32_t *tokens, cons
                     const int32_t *positions, int32_t n_req, float *scores, int32_t *next_tokens, void *kv_cache,
                     int32_t n_slots, void *workspace, size_t workspace_bytes, void *cuda_stream);
 
+/* ---- an entry point that allocates nothing ------------------------------------------------------------------------------
+ * The small-M projection of a decode iteration alone (NEXT-3: one row per request of the batch, "long-lived
+ * decode iterations"):  out[M, N] (fp32) = x[M, K] (bf16) . W[N, K]^T (bf16), fp32 accumulation, the K axis split over CTAs.
+ * For callers that cannot call cudaMalloc or hand over a workspace (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid allocation): the per-slice partial sums live in a file-scope __device__ array of 8 MiB that every GPU
+ * which loads the library holds until the process exits.  The call allocates and frees nothing and needs no fmx_ctx; it
+ * works on the CURRENT device and only enqueues two kernels on cuda_stream (no synchronisation).
+ *   x, W, out   DEVICE pointers, caller-owned, 16-byte aligned; rows contiguous (ld = K, K, N)
+ *   limits      1 <= M <= 128; N a multiple of 128; K a multiple of 8; round_up(M, 16) * N * 4 bytes <= 8 MiB
+ *               (else FMX_E_CAPACITY / FMX_E_INVALID_ARG with a message, nothing launched)
+ * Every call shares the array and finds the previous call's contents in it; nothing has to start at zero (a call writes every
+ * element it reads).  Calls that OVERLAP on the GPU - different streams, concurrent graphs - race on the array: keep them on
+ * one stream or order them with events. */
+int fmx_row_gemm_static(const void *x, const void *W, float *out, int32_t M, int32_t N, int32_t K, void *cuda_stream);
+
 /* Debug/test: copies the segment tables of the LAST forward to HOST arrays (synchronises).
  * Sizes: perm, inv_perm [n_req]; task_req_off, task_tok_off [n_slots+1]; cu_tok [n_req+1];
  * n_slots = fmx_task_slots().  Any pointer may be NULL. */

@@ -68,7 +68,7 @@ _lib = None
 # include/fmx.h (the public C ABI)
 EXPORTS = ["fmx_create", "fmx_destroy", "fmx_last_error", "fmx_version", "fmx_poll_error", "fmx_register_backbone", "fmx_register_task",
            "fmx_unregister_task", "fmx_output_layout", "fmx_output_layout_len", "fmx_workspace_bytes", "fmx_host_workspace_bytes", "fmx_forward_mixed",
-           "fmx_forward_mixed_host", "fmx_register_lm_head", "fmx_kv_cache_bytes", "fmx_prefill", "fmx_decode_step", "fmx_debug_get_segments", "fmx_task_slots", "fmx_profile_enable", "fmx_profile_select",
+           "fmx_forward_mixed_host", "fmx_register_lm_head", "fmx_kv_cache_bytes", "fmx_prefill", "fmx_decode_step", "fmx_row_gemm_static", "fmx_debug_get_segments", "fmx_task_slots", "fmx_profile_enable", "fmx_profile_select",
            "fmx_profile_read", "fmx_profile_family_name", "fmx_last_launch_count", "fmx_bfq_create", "fmx_bfq_destroy",
            "fmx_bfq_set_task", "fmx_bfq_enqueue", "fmx_bfq_next_batch", "fmx_bfq_complete", "fmx_bfq_stats", "fmx_bfq_peek"]
 # csrc/fmx_internal.h (test hooks and tuning knobs; not part of the ABI)
@@ -116,6 +116,7 @@ def load():
     lib.fmx_graph_replays.argtypes = [_vp]
     lib.fmx_graph_replays.restype = C.c_longlong
     lib.fmx_debug_gemm.argtypes = [_vp, _vp, _vp, _vp, C.c_int32, C.c_int32, C.c_int32, _vp]
+    lib.fmx_row_gemm_static.argtypes = [_vp, _vp, _vp, C.c_int32, C.c_int32, C.c_int32, _vp]
     lib.fmx_debug_attention.argtypes = [_vp, _vp, _vp, i32p, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, _vp]
     lib.fmx_set_option.argtypes = [_vp, C.c_int32, C.c_int32]
     lib.fmx_bfq_create.argtypes = [C.POINTER(BfqParams), C.POINTER(_vp)]
@@ -133,6 +134,12 @@ def load():
 def _check(code):
     if code != FMX_OK:
         raise FmxError(code, load().fmx_last_error().decode())
+
+
+def row_gemm_static(x, W, out, M, N, K, stream=0):
+    """fmx_row_gemm_static: out[M, N] fp32 = x[M, K] . W[N, K]^T (bf16 device pointers) on the current device; allocates nothing
+    (its scratch is a static 8 MiB device array), M <= 128.  Calls that overlap on the GPU race on that array."""
+    _check(load().fmx_row_gemm_static(x, W, out, M, N, K, stream or None))
 
 
 def _ptr_array(ptrs):

@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfmx.so")
-SOURCES = ["fmx_api.cu", "bfq.cpp", "errors.cpp"]
+SOURCES = ["fmx_api.cu", "no_alloc.cu", "bfq.cpp", "errors.cpp"]
 
 
 def _newest_source_mtime():
