@@ -1415,7 +1415,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       ReduceNormArgs na{};
       na.partial = w.splitk; na.k_split = ks; na.split_rows = split_rows; na.N = Nn; na.delta = any ? w.delta : nullptr; na.bias = p.bias[0];
       na.X = w.X; na.Y = w.Xn; na.g = next_norm_g; na.b = next_norm_b; na.eps = d.norm_eps; na.rms = d.norm == FMX_NORM_RMSNORM;
-      LAUNCH(Lh, family, (launch_k(reduce_resid_norm_kernel, (unsigned)Ni, 128, 0, S, na)));
+      LAUNCH(Lh, family, (launch_k(reduce_resid_norm_kernel, (unsigned)Ni, (unsigned)((Nn / 4 + 31) / 32 * 32), 0, S, na)));
       return FMX_OK;
     }
     SplitKReduceArgs ra{};

@@ -1219,79 +1219,58 @@ struct ReduceNormArgs {
   float eps;
   int rms;
 };
-__device__ __forceinline__ float block128_sum(float v, float *s_red) {        // every thread gets the sum; fixed order
+__device__ __forceinline__ float block_sum_fixed(float v, float *s_red) {    // every thread gets the sum; fixed order; blockDim a multiple of 32
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   __syncthreads();                                                            // s_red free again
   if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = v;
   __syncthreads();
-  return (s_red[0] + s_red[1]) + (s_red[2] + s_red[3]);
+  float t = 0.0f;
+  for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += s_red[w];
+  return t;
 }
-__global__ void __launch_bounds__(128) reduce_resid_norm_kernel(const ReduceNormArgs a) {
-  __shared__ float s_red[4];
+// One CTA per row, one thread per 4 columns (blockDim = N / 4 rounded up to a warp, <= 1024): the thread's partials of every
+// split, the delta and the residual are all requested before the first is used.
+__global__ void __launch_bounds__(1024) reduce_resid_norm_kernel(const ReduceNormArgs a) {
+  __shared__ float s_red[32];
   griddep_launch();
   griddep_wait();
-  const int r = blockIdx.x, n4 = a.N >> 2;
-  float4 v[8];
-#pragma unroll
-  for (int j = 0; j < 8; ++j) v[j] = make_float4(0.f, 0.f, 0.f, 0.f);
-  const float *part = a.partial + (size_t)r * a.N + 4 * threadIdx.x;
-#pragma unroll 4
-  for (int ks = 0; ks < a.k_split; ++ks) {                      // split order; the loads of four splits in flight at a time
-#pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      if (threadIdx.x + 128 * j >= n4) continue;
-      const float4 q = *reinterpret_cast<const float4 *>(part + (size_t)ks * a.split_rows * a.N + 512 * j);
-      v[j].x += q.x; v[j].y += q.y; v[j].z += q.z; v[j].w += q.w;
-    }
-  }
-  float s = 0.0f;
-#pragma unroll
-  for (int j = 0; j < 8; ++j) {
-    const int c4 = threadIdx.x + 128 * j;
-    if (c4 >= n4) continue;
-    const int c = 4 * c4;
-    float4 acc = v[j];
-    if (a.delta) {
-      const float4 q = *reinterpret_cast<const float4 *>(a.delta + (size_t)r * a.N + c);
+  const int r = blockIdx.x, n4 = a.N >> 2, c4 = threadIdx.x;
+  const bool on = c4 < n4;
+  const int c = 4 * c4;
+  const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+  float4 *xp = reinterpret_cast<float4 *>(a.X + (size_t)r * a.N + c);
+  const float4 x0 = on ? *xp : z4;
+  const float4 dl = (on && a.delta) ? *reinterpret_cast<const float4 *>(a.delta + (size_t)r * a.N + c) : z4;
+  float4 acc = z4;
+  if (on) {
+    const float *part = a.partial + (size_t)r * a.N + c;
+#pragma unroll 8
+    for (int ks = 0; ks < a.k_split; ++ks) {                    // split order
+      const float4 q = *reinterpret_cast<const float4 *>(part + (size_t)ks * a.split_rows * a.N);
       acc.x += q.x; acc.y += q.y; acc.z += q.z; acc.w += q.w;
     }
+    acc.x += dl.x; acc.y += dl.y; acc.z += dl.z; acc.w += dl.w;
     if (a.bias) {
       const uint2 bv = *reinterpret_cast<const uint2 *>(a.bias + c);
       acc.x += bf16_lo(bv.x); acc.y += bf16_hi(bv.x); acc.z += bf16_lo(bv.y); acc.w += bf16_hi(bv.y);
     }
-    float4 *x = reinterpret_cast<float4 *>(a.X + (size_t)r * a.N + c);
-    float4 o = *x;
-    o.x += acc.x; o.y += acc.y; o.z += acc.z; o.w += acc.w;
-    *x = o;
-    v[j] = o;
-    s += o.x + o.y + o.z + o.w;
   }
+  const float4 v = make_float4(x0.x + acc.x, x0.y + acc.y, x0.z + acc.z, x0.w + acc.w);
+  if (on) *xp = v;
   if (!a.g) return;
   float mean = 0.0f;
-  if (!a.rms) mean = block128_sum(s, s_red) * (1.0f / a.N);
-  float q = 0.0f;
-#pragma unroll
-  for (int j = 0; j < 8; ++j) {
-    if (threadIdx.x + 128 * j >= n4) continue;
-    const float a0 = v[j].x - mean, a1 = v[j].y - mean, a2 = v[j].z - mean, a3 = v[j].w - mean;
-    q += a0 * a0 + a1 * a1 + a2 * a2 + a3 * a3;
+  if (!a.rms) mean = block_sum_fixed(on ? (v.x + v.y) + (v.z + v.w) : 0.0f, s_red) * (1.0f / a.N);
+  const float a0 = v.x - mean, a1 = v.y - mean, a2 = v.z - mean, a3 = v.w - mean;
+  const float inv = rsqrtf(block_sum_fixed(on ? a0 * a0 + a1 * a1 + a2 * a2 + a3 * a3 : 0.0f, s_red) * (1.0f / a.N) + a.eps);
+  if (!on) return;
+  const uint2 gg = reinterpret_cast<const uint2 *>(a.g)[c4];
+  float o0 = a0 * inv * bf16_lo(gg.x), o1 = a1 * inv * bf16_hi(gg.x), o2 = a2 * inv * bf16_lo(gg.y), o3 = a3 * inv * bf16_hi(gg.y);
+  if (a.b) {
+    const uint2 bb = reinterpret_cast<const uint2 *>(a.b)[c4];
+    o0 += bf16_lo(bb.x); o1 += bf16_hi(bb.x); o2 += bf16_lo(bb.y); o3 += bf16_hi(bb.y);
   }
-  const float inv = rsqrtf(block128_sum(q, s_red) * (1.0f / a.N) + a.eps);
-  uint2 *y = reinterpret_cast<uint2 *>(a.Y + (size_t)r * a.N);
-#pragma unroll
-  for (int j = 0; j < 8; ++j) {
-    const int c4 = threadIdx.x + 128 * j;
-    if (c4 >= n4) continue;
-    const uint2 gg = reinterpret_cast<const uint2 *>(a.g)[c4];
-    float o0 = (v[j].x - mean) * inv * bf16_lo(gg.x), o1 = (v[j].y - mean) * inv * bf16_hi(gg.x);
-    float o2 = (v[j].z - mean) * inv * bf16_lo(gg.y), o3 = (v[j].w - mean) * inv * bf16_hi(gg.y);
-    if (a.b) {
-      const uint2 bb = reinterpret_cast<const uint2 *>(a.b)[c4];
-      o0 += bf16_lo(bb.x); o1 += bf16_hi(bb.x); o2 += bf16_lo(bb.y); o3 += bf16_hi(bb.y);
-    }
-    y[c4] = make_uint2(pack_bf16(o0, o1), pack_bf16(o2, o3));
-  }
+  reinterpret_cast<uint2 *>(a.Y + (size_t)r * a.N)[c4] = make_uint2(pack_bf16(o0, o1), pack_bf16(o2, o3));
 }
 
 // The reduction of the fused q / k / v projection of a decode iteration, with what follows it: + delta + bias, RoPE at the row's
