@@ -50,6 +50,9 @@ class BackboneSpec:
     std_out: float = 0.02       # o and down projections
     std_embed: float = 0.02     # token table
     pos_kind: str = "none"      # 'none' | 'sinusoid' | 'normal'
+    # NEXT-4 variant: T5-style relative-position bias, one table [rel_buckets, n_q_heads] shared by every layer (0 = none)
+    rel_buckets: int = 0
+    rel_max_distance: int = 0
 
     @property
     def d_q(self):
@@ -140,6 +143,8 @@ class Workload:
                 return (bb.tokens_per_request, bb.d_model), bb.pos_kind, bb.std
             if what == "table":
                 return (bb.vocab, bb.d_model), "normal", bb.std_embed
+        if parts[0] == "rel_bias":         # NEXT-4 variant: T5 relative-position bias table [buckets, heads]; O(1) values so that it matters
+            return (bb.rel_buckets, bb.n_q_heads), "normal", 1.0
         if parts[0] == "lm_head":          # NEXT-3: untied language-model head [vocab, d_model] (reading 34)
             return (bb.vocab, bb.d_model), "normal", 0.02
         if parts[0] == "final":
@@ -342,7 +347,7 @@ def make_workload(cfg: str, *, n_layers: Optional[int] = None, batch: Optional[i
                   n_tasks: Optional[int] = None, dist: Optional[str] = None,
                   max_len: Optional[int] = None, adapters: bool = True,
                   seed_offset: int = 0, lora_std: float = 0.02, mlp_hidden: int = 0,
-                  enc_channels: int = 0, dense_heads: bool = False) -> Workload:
+                  enc_channels: int = 0, dense_heads: bool = False, rel_bias: bool = False) -> Workload:
     """Build the workload of a BASELINE.json config (cfg1..cfg5).
 
     Overrides give the reduced variants the parity tests use (fewer layers, smaller batch);
@@ -356,6 +361,8 @@ def make_workload(cfg: str, *, n_layers: Optional[int] = None, batch: Optional[i
     bb = _BACKBONES[cfg]
     if n_layers is not None:
         bb = replace(bb, n_layers=n_layers)
+    if rel_bias:            # the T5 relative-position bias (32 buckets, max distance 128: T5's defaults); a variant
+        bb = replace(bb, rel_buckets=32, rel_max_distance=128)
     idx = int(cfg[3])
     seed = 9643000 + idx + seed_offset
     defaults = {"cfg1": (12, 3), "cfg2": (256, 10), "cfg3": (128, 32), "cfg4": (64, 92),

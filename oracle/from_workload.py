@@ -17,7 +17,8 @@ def bb_dict(wl):
                 norm=bb.norm, norm_eps=bb.norm_eps, causal=bb.causal, rope_theta=bb.rope_theta,
                 input_kind=bb.input_kind, patch_dim=bb.patch_dim, has_cls=bb.has_cls,
                 has_bias=bb.has_bias, has_pos=bb.pos_kind != "none", img_c=bb.img_c,
-                img_hw=bb.img_hw, patch_hw=bb.patch_hw)
+                img_hw=bb.img_hw, patch_hw=bb.patch_hw, rel_buckets=getattr(bb, "rel_buckets", 0),
+                rel_max_distance=getattr(bb, "rel_max_distance", 0))
 
 
 def task_dicts(wl):

@@ -31,7 +31,8 @@ Library pins (tests/test_oracle_library_pins.py, independent PyTorch / Hugging F
 `attention` vs torch SDPA (causal / full, GQA); the norms and activations vs torch.nn.functional;
 `layer_forward` of both encoder families vs torch.nn.TransformerEncoderLayer(norm_first=True);
 the decoder backbone (RMSNorm, rotate-half RoPE, GQA, causal, SwiGLU) with LoRA on all seven
-targets vs transformers' LlamaModel carrying the merged weights W + (alpha/r) B A.
+targets vs transformers' LlamaModel carrying the merged weights W + (alpha/r) B A; the relative-position bias variant
+(`rel_bucket`, NEXT-4) vs transformers' T5Attention bucket function and a whole T5Block, plus hand-derived bucket values.
 The paper prints no value of any forward output, so no pin comes from the paper itself; what
 stays without a library counterpart is only the pooled / flattened head (a mean, a row pick or
 a reshape, then one matrix-vector product), pinned by its special cases; the
@@ -104,9 +105,9 @@ def rope_rotate_half(x, theta):
     return np.concatenate([x1 * c - x2 * s, x2 * c + x1 * s], axis=1)
 
 
-def attention(q, k, v, n_q_heads, n_kv_heads, head_dim, causal):
-    """softmax(q k^T / sqrt(d_h) + M) v per query head; query head g reads KV head
-    floor(g / (H_q/H_kv)); M_ab = -inf for b > a when causal."""
+def attention(q, k, v, n_q_heads, n_kv_heads, head_dim, causal, bias=None):
+    """softmax(q k^T / sqrt(d_h) + M + bias_g) v per query head; query head g reads KV head
+    floor(g / (H_q/H_kv)); M_ab = -inf for b > a when causal; bias: None or [H_q, n, n] added to the scores."""
     n = q.shape[0]
     group = n_q_heads // n_kv_heads
     out = np.empty((n, n_q_heads * head_dim), dtype=np.float64)
@@ -116,9 +117,47 @@ def attention(q, k, v, n_q_heads, n_kv_heads, head_dim, causal):
         kg = k[:, kv * head_dim:(kv + 1) * head_dim]
         vg = v[:, kv * head_dim:(kv + 1) * head_dim]
         s = (qg @ kg.T) / math.sqrt(head_dim)
+        if bias is not None:
+            s = s + bias[g]
         if causal:
             s = np.where(np.arange(n)[None, :] > np.arange(n)[:, None], -np.inf, s)
         out[:, g * head_dim:(g + 1) * head_dim] = softmax_rows(s) @ vg
+    return out
+
+
+def rel_bucket(rel, bidirectional, n_buckets, max_distance):
+    """Bucket of the relative position rel = key position - query position (T5: Raffel et al. 2020, section 2.1 "we use 32
+    embeddings ... with ranges that increase in size logarithmically up to an offset of 128 beyond which we assign all relative
+    positions to the same embedding").  Step by step:
+      bidirectional (encoder): half of the buckets for keys after the query (rel > 0), half for keys at or before it; the
+        distance is |rel|.  Unidirectional (causal): keys after the query all map to distance 0; the distance is max(-rel, 0).
+      Of the n buckets on a side the first n / 2 hold the distances 0 .. n/2 - 1 exactly; the other n / 2 hold logarithmically
+        growing ranges up to max_distance, everything beyond falls in the last bucket:
+        n/2 + floor( log(dist / (n/2)) / log(max_distance / (n/2)) * (n - n/2) ), capped at n - 1."""
+    rel = int(rel)
+    n = n_buckets
+    b = 0
+    if bidirectional:
+        n //= 2
+        if rel > 0:
+            b += n
+        dist = abs(rel)
+    else:
+        dist = max(-rel, 0)
+    max_exact = n // 2
+    if dist < max_exact:
+        return b + dist
+    large = max_exact + int(math.log(dist / max_exact) / math.log(max_distance / max_exact) * (n - max_exact))
+    return b + min(large, n - 1)
+
+
+def rel_bias_matrix(table, n, bidirectional, n_buckets, max_distance):
+    """bias[g, a, b] = table[rel_bucket(b - a), g] for query position a, key position b; table [n_buckets, H_q]."""
+    H = table.shape[1]
+    out = np.empty((H, n, n), dtype=np.float64)
+    for a in range(n):
+        for b in range(n):
+            out[:, a, b] = table[rel_bucket(b - a, bidirectional, n_buckets, max_distance)]
     return out
 
 
@@ -195,7 +234,10 @@ def layer_forward(bb, get, task, l, h, capture=None):
                             for g in range(Hq)], axis=1)
         k = np.concatenate([rope_rotate_half(k[:, g * dh:(g + 1) * dh], bb["rope_theta"])
                             for g in range(Hkv)], axis=1)
-    o = attention(q, k, v, Hq, Hkv, dh, bb["causal"])
+    rel = None
+    if bb.get("rel_buckets", 0) > 0:        # one table for every layer, as in T5 (the first block owns it, the others reuse it)
+        rel = rel_bias_matrix(get("rel_bias.W"), h.shape[0], not bb["causal"], bb["rel_buckets"], bb["rel_max_distance"])
+    o = attention(q, k, v, Hq, Hkv, dh, bb["causal"], rel)
     h = h + lora_linear(o, get(p + "Wo"), bias("bo"), _adapter(get, task, l, "o"))
     m = _norm(bb, get, p + "norm2", h)
     if bb["act"] == "swiglu":

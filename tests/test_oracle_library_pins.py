@@ -325,3 +325,63 @@ def test_input_channel_combiner_is_a_1x1_convolution_and_reduces_to_the_plain_pa
     # one-hot weights, zero bias: the encoder picks a channel
     W["task002.enc.W"] = np.array([0.0, 1.0, 0.0]); W["task002.enc.b"] = np.zeros(1)
     assert np.allclose(O.tokens_from_input(bb, W.__getitem__, x.reshape(-1), task), O.tokens_from_input(bb, W.__getitem__, x[1]))
+
+
+# ---------------------------------------------------------------- NEXT-4 variant: T5 relative-position bias vs transformers' T5
+def test_relative_position_bucket_matches_hf_t5():
+    tr = pytest.importorskip("transformers")
+    from transformers.models.t5.modeling_t5 import T5Attention
+    rel = torch.arange(-400, 401, dtype=torch.long)
+    for bidirectional in (True, False):
+        for n_buckets, max_distance in ((32, 128), (8, 20), (16, 64), (32, 1024)):
+            want = T5Attention._relative_position_bucket(rel, bidirectional=bidirectional, num_buckets=n_buckets, max_distance=max_distance)
+            got = [O.rel_bucket(int(x), bidirectional, n_buckets, max_distance) for x in rel]
+            assert got == want.tolist(), (bidirectional, n_buckets, max_distance)
+
+
+def test_t5_encoder_block_with_relative_bias_matches_hf_t5block():
+    """cfg2's family (RMSNorm, ReLU, no biases) + the relative-position bias = a T5 encoder block.  T5 does not scale the scores
+    by 1/sqrt(d_h) (SURVEY.md 8(c) reading 1 keeps the scale), so the HF block gets Wq / sqrt(d_h): sqrt(16) = 4, exact."""
+    tr = pytest.importorskip("transformers")
+    from transformers.models.t5.modeling_t5 import T5Block
+    d, H, dh, Fd, n, NB, MD = 64, 4, 16, 96, 45, 8, 20                  # n > max distance: the last bucket is exercised
+    cfg = tr.T5Config(d_model=d, d_kv=dh, num_heads=H, d_ff=Fd, num_layers=1, relative_attention_num_buckets=NB,
+                      relative_attention_max_distance=MD, dropout_rate=0.0, layer_norm_epsilon=1e-6, feed_forward_proj="relu",
+                      is_decoder=False, use_cache=False)
+    cfg._attn_implementation = "eager"
+    r = _rng(77)
+    W = {"rel_bias.W": r.standard_normal((NB, H))}
+    p = "L00."
+    for nm, shape in (("Wq", (d, d)), ("Wk", (d, d)), ("Wv", (d, d)), ("Wo", (d, d)), ("Wup", (Fd, d)), ("Wdown", (d, Fd))):
+        W[p + nm] = r.standard_normal(shape) * 0.2
+    for nm in ("norm1", "norm2"):
+        W[p + nm + ".g"] = 1 + 0.1 * r.standard_normal(d)
+    bb = dict(n_layers=1, d_model=d, n_q_heads=H, n_kv_heads=H, head_dim=dh, d_ffn=Fd, act="relu", norm="rms", norm_eps=1e-6,
+              causal=False, rope_theta=0.0, input_kind="embedded", patch_dim=0, has_cls=False, has_bias=False, has_pos=False,
+              img_c=0, img_hw=0, patch_hw=0, rel_buckets=NB, rel_max_distance=MD)
+    x = r.standard_normal((n, d))
+    got = O.layer_forward(bb, W.__getitem__, None, 0, x)
+    # without the bias the result must differ (the pin would not see a dropped term otherwise)
+    assert np.abs(got - O.layer_forward({**bb, "rel_buckets": 0}, W.__getitem__, None, 0, x)).max() > 1e-3
+
+    blk = T5Block(cfg, has_relative_attention_bias=True, layer_idx=0).to(torch.float64).eval()
+    with torch.no_grad():
+        sa = blk.layer[0].SelfAttention
+        sa.q.weight.copy_(_t(W[p + "Wq"] / math.sqrt(dh)))
+        sa.k.weight.copy_(_t(W[p + "Wk"]))
+        sa.v.weight.copy_(_t(W[p + "Wv"]))
+        sa.o.weight.copy_(_t(W[p + "Wo"]))
+        sa.relative_attention_bias.weight.copy_(_t(W["rel_bias.W"]))
+        blk.layer[0].layer_norm.weight.copy_(_t(W[p + "norm1.g"]))
+        ff = blk.layer[1]
+        ff.DenseReluDense.wi.weight.copy_(_t(W[p + "Wup"]))
+        ff.DenseReluDense.wo.weight.copy_(_t(W[p + "Wdown"]))
+        ff.layer_norm.weight.copy_(_t(W[p + "norm2.g"]))
+        try:
+            out = blk(_t(x)[None], cache_position=torch.arange(n))
+        except TypeError:
+            out = blk(_t(x)[None])
+    want = (out[0] if isinstance(out, (tuple, list)) else out)[0].numpy()
+    # HF's T5 takes the softmax and the RMS statistics in float32 whatever the module's dtype (`scores.float()`), so the two agree
+    # to float32 rounding of O(1) values, not to 1e-10; a wrong bucket or a dropped bias is > 1e-3 (asserted above)
+    assert np.allclose(got, want, rtol=0, atol=2e-5), np.abs(got - want).max()

@@ -350,3 +350,24 @@ def test_stress_variant_makes_adapters_visible():
     y_swapped = O.forward_request(bb, lambda n: get(n.replace(f"task{other['id']:03d}.head", f"task{t:03d}.head")), other, xs[0])
     cos = lambda a, b: float(a @ b / np.linalg.norm(a) / np.linalg.norm(b))
     assert cos(y_on, y_off) < 0.99 and cos(y_on, y_swapped) < 0.99
+
+
+def test_relative_position_buckets_by_hand():
+    """T5 (Raffel et al. 2020, section 2.1): 32 buckets, offsets up to 128.  Bidirectional: 16 buckets per side, distances 0 .. 7
+    exact, then 8 logarithmic buckets 8 + floor(8 log(dist / 8) / log(16)), the last one open-ended; keys after the query are
+    offset by 16.  Unidirectional: 32 buckets on the past side, distances 0 .. 15 exact, then 16 + floor(16 log(dist / 16) / log 8)."""
+    from oracle.vfm_forward import rel_bucket
+    bi = lambda rel: rel_bucket(rel, True, 32, 128)
+    assert [bi(0), bi(-1), bi(1), bi(-7), bi(7)] == [0, 1, 17, 7, 23]
+    assert bi(-8) == 8 and bi(-11) == 8 and bi(-12) == 9          # 8 * 16^(1/8) = 11.3: distances 8 .. 11 share bucket 8
+    assert bi(-16) == 10                                           # log(2) / log(16) * 8 = 2 exactly
+    assert bi(-127) == 15 and bi(-128) == 15 and bi(-5000) == 15   # 7.98 -> 7; 8 -> capped at 15
+    assert bi(200) == 31
+    uni = lambda rel: rel_bucket(rel, False, 32, 128)
+    assert [uni(5), uni(0), uni(-15), uni(-16)] == [0, 0, 15, 16]  # keys after the query: distance 0
+    assert uni(-100) == 30 and uni(-128) == 31 and uni(-129) == 31 # 16 * log(6.25) / log(8) = 14.1
+    # the bias matrix picks table rows by key position - query position
+    from oracle.vfm_forward import rel_bias_matrix
+    tab = np.arange(32 * 2, dtype=np.float64).reshape(32, 2)
+    m = rel_bias_matrix(tab, 4, True, 32, 128)
+    assert m.shape == (2, 4, 4) and m[1, 0, 0] == tab[0, 1] and m[0, 2, 0] == tab[2, 0] and m[0, 0, 3] == tab[19, 0]
