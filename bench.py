@@ -143,8 +143,9 @@ def build_workload(args):
     if args.workload == "headline":
         return make_workload("cfg5", n_tasks=HEADLINE["tasks"], dist=HEADLINE["dist"])
     if args.workload == "cfg5":
-        return make_workload("cfg5", n_tasks=args.tasks, dist=args.dist, adapters=not args.no_adapters, mlp_hidden=args.mlp_hidden, enc_channels=args.enc_channels)
-    return make_workload(args.workload, mlp_hidden=args.mlp_hidden, enc_channels=args.enc_channels)
+        return make_workload("cfg5", n_tasks=args.tasks, dist=args.dist, adapters=not args.no_adapters, mlp_hidden=args.mlp_hidden, enc_channels=args.enc_channels,
+                             rel_bias=args.rel_bias)
+    return make_workload(args.workload, mlp_hidden=args.mlp_hidden, enc_channels=args.enc_channels, rel_bias=args.rel_bias)
 
 
 # ------------------------------------------------------------------------------------- the oracle legs
@@ -602,6 +603,7 @@ def main():
     ap.add_argument("--no-adapters", action="store_true", help="cfg5: head-only tasks (adapter-free reference)")
     ap.add_argument("--enc-channels", type=int, default=0, help="NEXT-1 variant: every other task brings this many input channels and a channel combiner (cfg2 / cfg5)")
     ap.add_argument("--mlp-hidden", type=int, default=0, help="NEXT-1 variant: pooled heads become MLP decoder heads of this hidden width")
+    ap.add_argument("--rel-bias", action="store_true", help="NEXT-4 variant: the backbone carries a T5-style relative-position bias (32 buckets, max distance 128)")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
                     help="fmx_set_option experiment knob (csrc/fmx_internal.h), e.g. --opt attention_impl=3; recorded in config.options")
     ap.add_argument("--no-flush", action="store_true")

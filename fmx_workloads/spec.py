@@ -238,6 +238,8 @@ class Workload:
             names.append("embed.table")
         if bb.pos_kind != "none":
             names.append("embed.pos")
+        if bb.rel_buckets:
+            names.append("rel_bias.W")
         for l in range(bb.n_layers):
             names += self.layer_tensor_names(l)
         names.append("final.g")

@@ -36,7 +36,7 @@ class BackboneDesc(C.Structure):
                [(n, _vp) for n in ("embed_W", "embed_b", "embed_cls", "embed_pos", "embed_table")] + \
                [(n, _vpp) for n in ("norm1_g", "norm1_b", "Wq", "Wk", "Wv", "Wo", "bq", "bk", "bv", "bo", "norm2_g", "norm2_b",
                                     "Wup", "Wgate", "Wdown", "bup", "bgate", "bdown")] + \
-               [("final_g", _vp), ("final_b", _vp)]
+               [("final_g", _vp), ("final_b", _vp), ("rel_bias", _vp), ("rel_buckets", C.c_int32), ("rel_max_distance", C.c_int32)]
 
 
 class AdapterDesc(C.Structure):

@@ -23,6 +23,9 @@ struct AttnArgs {
   int n_q_heads, n_kv_heads;
   int causal;
   float scale_log2;      // log2(e) / sqrt(d_h)
+  // optional relative-position bias (attention_kernel only): relb[head * relb_ld + (key - query) + relb_off], already times log2(e)
+  const float *relb;
+  int relb_ld, relb_off;
 };
 
 
@@ -116,7 +119,11 @@ __global__ void __launch_bounds__(kAttnThreads) attention_kernel(const AttnArgs 
         const int key = key0 + nt * 8 + t * 2 + (e & 1);
         const int qrow = (e < 2) ? qrow_a : qrow_b;
         const bool masked = key >= n || (a.causal && key > qrow);
-        const float v = masked ? -1e30f : s[nt][e] * a.scale_log2;
+        float v = -1e30f;
+        if (!masked) {
+          v = s[nt][e] * a.scale_log2;
+          if (a.relb) v += __ldg(a.relb + head * a.relb_ld + max((key - qrow) + a.relb_off, 0));   // (rows past the request's end are padding)
+        }
         s[nt][e] = v;
         mx[e >> 1] = fmaxf(mx[e >> 1], v);
       }

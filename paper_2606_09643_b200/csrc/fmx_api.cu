@@ -69,6 +69,7 @@ struct Backbone {
   float *posb = nullptr;                   // [n_pos, d]
   float2 *rope_cs = nullptr;               // [max_seq, dh/2]
   float2 *rope_cs_t = nullptr;             // [dh/2, max_seq] (the fused-RoPE GEMM epilogue reads this one)
+  float *relb = nullptr;                   // relative-position bias by distance: [n_q_heads, 2 max_seq - 1] fp32, times log2(e); index (key - query) + max_seq - 1
   // weight maps, [0] = box {64,128} (pair tile 256x256: one CTA loads a whole chunk), [1] = box {64,64} (256x128 tiles)
   std::vector<CUtensorMap> mWq[2], mWk[2], mWv[2], mWo[2], mWup[2], mWgate[2], mWdown[2];
   CUtensorMap mEmbedW[2];
@@ -802,7 +803,7 @@ int fmx_destroy(fmx_ctx *c) {
   for (auto e : c->ev_pool) cudaEventDestroy(e);
   for (auto &bp : c->bbs) {
     if (!bp) continue;
-    cudaFree(bp->embed_Wpad); cudaFree(bp->posb); cudaFree(bp->rope_cs); cudaFree(bp->rope_cs_t);
+    cudaFree(bp->embed_Wpad); cudaFree(bp->posb); cudaFree(bp->rope_cs); cudaFree(bp->rope_cs_t); cudaFree(bp->relb);
     for (int tg = 0; tg < 7; ++tg) { if (bp->slabA[tg]) cudaFreeAsync(bp->slabA[tg], c->side); if (bp->slabB[tg]) cudaFreeAsync(bp->slabB[tg], c->side); if (bp->slabBt[tg]) cudaFreeAsync(bp->slabBt[tg], c->side); }
   }
   for (auto &t : c->tasks)
@@ -864,6 +865,12 @@ int fmx_register_backbone(fmx_ctx *c, const fmx_backbone_desc *desc, fmx_backbon
   }
   if (d.input_kind == FMX_INPUT_TOKEN_IDS && (!d.embed_table || d.vocab < 1)) return fmx_fail(FMX_E_INVALID_ARG, "register_backbone: TOKEN_IDS needs embed_table, vocab");
   if (d.rope_theta > 0 && d.head_dim % 2) return fmx_fail(FMX_E_SHAPE, "register_backbone: RoPE needs even head_dim");
+  if (d.rel_bias && d.rel_buckets != 0) {
+    const int side = d.causal ? d.rel_buckets : d.rel_buckets / 2;           // buckets per direction
+    if (d.rel_buckets < 2 || d.rel_buckets > 256 || d.rel_buckets % 2 || side < 2 || d.rel_max_distance <= side / 2)
+      return fmx_fail(FMX_E_SHAPE, "register_backbone: relative-position bias needs an even rel_buckets in 2..256 (>= 4 when not causal) and rel_max_distance > buckets-per-side / 2 (got %d, %d)",
+                      d.rel_buckets, d.rel_max_distance);
+  }
 
   std::unique_ptr<Backbone> b(new Backbone());
   b->d = d;
@@ -915,6 +922,30 @@ int fmx_register_backbone(fmx_ctx *c, const fmx_backbone_desc *desc, fmx_backbon
     CU_OK(cudaMalloc(&b->rope_cs_t, sizeof(float2) * n));
     transpose_rope_table_kernel<<<(n + 255) / 256, 256>>>(b->rope_cs, b->rope_cs_t, d.max_seq, d.head_dim / 2);
     CU_OK(cudaGetLastError());
+  }
+  if (d.rel_bias && d.rel_buckets > 0) {
+    // bias by relative distance, for every head: the bucket of each distance is taken here on the host (T5's bucket function in
+    // double precision, reading 36), the table row is the caller's bf16 value; stored times log2(e) for the exp2 softmax
+    const int nb = d.rel_buckets, H = d.n_q_heads, S = d.max_seq, ld = 2 * S - 1;
+    std::vector<uint16_t> tab((size_t)nb * H);
+    CU_OK(cudaMemcpy(tab.data(), d.rel_bias, tab.size() * sizeof(uint16_t), cudaMemcpyDeviceToHost));
+    std::vector<float> dense((size_t)H * ld);
+    for (int rel = -(S - 1); rel <= S - 1; ++rel) {
+      int n = nb, bucket = 0, dist;
+      if (!d.causal) { n /= 2; if (rel > 0) bucket += n; dist = rel < 0 ? -rel : rel; }
+      else dist = rel < 0 ? -rel : 0;
+      const int max_exact = n / 2;
+      if (dist < max_exact) bucket += dist;
+      else bucket += std::min(max_exact + (int)(std::log((double)dist / max_exact) / std::log((double)d.rel_max_distance / max_exact) * (n - max_exact)), n - 1);
+      for (int g = 0; g < H; ++g) {
+        const uint32_t bits = (uint32_t)tab[(size_t)bucket * H + g] << 16;
+        float v;
+        memcpy(&v, &bits, sizeof(v));
+        dense[(size_t)g * ld + rel + S - 1] = v * 1.4426950408889634f;
+      }
+    }
+    CU_OK(cudaMalloc(&b->relb, dense.size() * sizeof(float)));
+    CU_OK(cudaMemcpy(b->relb, dense.data(), dense.size() * sizeof(float), cudaMemcpyHostToDevice));
   }
   CU_OK(cudaDeviceSynchronize());
   b->Rcap = 256;
@@ -1493,13 +1524,13 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       else if (d.head_dim == 64) LAUNCH(Lh, F_ATTN, (launch_k(decode_attention_kernel<64>, grid, 128, decode_attention_smem<64>(), S, da, ka)));
       else LAUNCH(Lh, F_ATTN, (launch_k(decode_attention_kernel<128>, grid, 128, decode_attention_smem<128>(), S, da, ka)));
       rev();
-    } else if (c->o.attn_impl == FMX_ATTN_AUTO && attn_pair64_ok(c->o, d.head_dim, d.n_q_heads, max_len)) {
+    } else if (!bb.relb && c->o.attn_impl == FMX_ATTN_AUTO && attn_pair64_ok(c->o, d.head_dim, d.n_q_heads, max_len)) {
       AttnPairArgs pa2{};
       pa2.qkv_map = mQKV64; pa2.out = w.AttnO; pa2.cu_tok = w.t.cu_tok; pa2.ld_out = bb.d_q; pa2.n_req = B;
       pa2.n_q_heads = d.n_q_heads; pa2.n_kv_heads = d.n_kv_heads; pa2.causal = d.causal; pa2.scale_log2 = scale_log2;
       pa2.reverse = rev();
       LAUNCH(Lh, F_ATTN, launch_attention_pair64(S, c->sm_count, pa2));
-    } else if (attn_use_tc(c->o.attn_impl, d.head_dim, max_len)) {
+    } else if (!bb.relb && attn_use_tc(c->o.attn_impl, d.head_dim, max_len)) {
       AttnTcArgs ta{};
       ta.qkv_map = mQKV64; ta.out = w.AttnO; ta.cu_tok = w.t.cu_tok; ta.ld_out = bb.d_q;
       ta.n_q_heads = d.n_q_heads; ta.n_kv_heads = d.n_kv_heads; ta.causal = d.causal; ta.scale_log2 = scale_log2;
@@ -1509,8 +1540,9 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       AttnArgs aa{};
       aa.qkv = w.QKV; aa.out = w.AttnO; aa.cu_tok = w.t.cu_tok; aa.ld_qkv = bb.d_qkv; aa.ld_out = bb.d_q;
       aa.n_q_heads = d.n_q_heads; aa.n_kv_heads = d.n_kv_heads; aa.causal = d.causal; aa.scale_log2 = scale_log2;
+      aa.relb = bb.relb; aa.relb_ld = 2 * d.max_seq - 1; aa.relb_off = d.max_seq - 1;     // relative-position bias: the generic kernel only
       dim3 grid((max_len + kAttnBQ - 1) / kAttnBQ, d.n_q_heads, B);
-      if (max_len <= 64 && c->o.attn_short) LAUNCH(Lh, F_ATTN, launch_attention_short(S, c->sm_count, d.head_dim, B, aa));
+      if (max_len <= 64 && c->o.attn_short && !bb.relb) LAUNCH(Lh, F_ATTN, launch_attention_short(S, c->sm_count, d.head_dim, B, aa));
       else LAUNCH(Lh, F_ATTN, launch_attention(S, d.head_dim, grid, aa));
     }
     {
@@ -1778,6 +1810,7 @@ int fmx_register_lm_head(fmx_ctx *c, fmx_backbone_t h, const void *W, int32_t vo
   Backbone *bb = get_bb(c, h);
   if (!bb) return fmx_fail(FMX_E_UNKNOWN_BACKBONE, "register_lm_head: unknown backbone %d", h);
   if (vocab < 128 || vocab % 128) return fmx_fail(FMX_E_SHAPE, "register_lm_head: vocab %d must be a positive multiple of 128", vocab);
+  if (bb->relb) return fmx_fail(FMX_E_SHAPE, "register_lm_head: backbones with a relative-position bias do not serve token decode");
   CUtensorMap m0, m1;
   if (int e = encode_2d(c, &m0, W, vocab, bb->d.d_model, bb->d.d_model, 128)) return e;
   if (int e = encode_2d(c, &m1, W, vocab, bb->d.d_model, bb->d.d_model, 64)) return e;

@@ -60,7 +60,8 @@ class Session:
                       head_dim=bb.head_dim, d_ffn=bb.d_ffn, act=ACT[bb.act], norm=NORM[bb.norm], norm_eps=bb.norm_eps,
                       causal=int(bb.causal), rope_theta=bb.rope_theta, input_kind=INPUT_KIND[bb.input_kind],
                       patch_dim=bb.patch_dim, tokens_per_request=bb.tokens_per_request, has_cls=int(bb.has_cls),
-                      vocab=bb.vocab, max_seq=bb.max_seq, img_c=bb.img_c, img_hw=bb.img_hw, patch_hw=bb.patch_hw)
+                      vocab=bb.vocab, max_seq=bb.max_seq, img_c=bb.img_c, img_hw=bb.img_hw, patch_hw=bb.patch_hw,
+                      rel_buckets=getattr(bb, "rel_buckets", 0), rel_max_distance=getattr(bb, "rel_max_distance", 0))
         lay = lambda n: [self._w(f"L{l:02d}.{n}") for l in range(L)]
         per_layer = dict(norm1_g=lay("norm1.g"), norm2_g=lay("norm2.g"), Wq=lay("Wq"), Wk=lay("Wk"), Wv=lay("Wv"),
                          Wo=lay("Wo"), Wup=lay("Wup"), Wdown=lay("Wdown"),
@@ -75,7 +76,8 @@ class Session:
                        embed_b=self._w("embed.b") if bb.input_kind == "patch" else None,
                        embed_cls=self._w("embed.cls") if bb.has_cls else None,
                        embed_pos=self._w("embed.pos") if bb.pos_kind != "none" else None,
-                       embed_table=self._w("embed.table") if bb.input_kind == "tokens" else None)
+                       embed_table=self._w("embed.table") if bb.input_kind == "tokens" else None,
+                       rel_bias=self._w("rel_bias.W") if getattr(bb, "rel_buckets", 0) else None)
         return self.fmx.register_backbone(fields, per_layer, singles)
 
     def _register_task(self, t, presynced=None):

@@ -845,3 +845,31 @@ def test_two_backbones_on_disjoint_sm_partitions(fmx_mod):
     # the board's power budget (measured on B200: 2.0 -> 2.8 ms with the other partition busy; on shared SMs 1.3 -> 1.9 ms).
     assert busy <= 2.0 * quiet, f"partitioned forward slowed from {quiet:.3f} to {busy:.3f} ms by the other partition"
     part.close()
+
+
+# ---------------------------------------------------------------- NEXT-4 variant: T5 relative-position bias
+@pytest.mark.parametrize("cfg,kw", [
+    ("cfg2", dict(n_layers=2, batch=24, rel_bias=True)),                 # the T5-encoder-shaped family: bidirectional buckets, 64 tokens
+    ("cfg3", dict(n_layers=2, batch=6, rel_bias=True)),                  # 257 tokens: distances beyond max_distance (last bucket), 5 key tiles
+    ("cfg4", dict(n_layers=2, batch=8, max_len=300, rel_bias=True)),     # causal: unidirectional buckets, ragged lengths, with RoPE and GQA
+])
+def test_relative_position_bias_variant_parity(fmx_mod, cfg, kw):
+    """SURVEY.md 8(f) NEXT-4 / DESIGN.md reading 36: one T5-style bias table [buckets, heads] added to the scores of every layer."""
+    wl = make_workload(cfg, **kw)
+    assert wl.bb.rel_buckets == 32
+    s = _session(fmx_mod, wl)
+    y = s.forward_numpy()
+    check_segments(s, wl)
+    ref = G.oracle_outputs(wl)
+    check_parity(y, ref, f"{cfg} relative-position bias")
+    # the bias matters at this tolerance: a path that dropped it would fail the max-abs bar (0.21 / 0.085 / 0.036 on these three)
+    plain = G.oracle_outputs(make_workload(cfg, **{**kw, "rel_bias": False}))
+    assert max(float(np.abs(a - b).max()) for a, b in zip(ref, plain)) > 1.5 * MAX_ABS
+
+
+def test_relative_position_bias_backbone_refuses_token_decode(fmx_mod):
+    wl = make_workload("cfg4", n_layers=1, batch=2, max_len=16, rel_bias=True)
+    s = _session(fmx_mod, wl)
+    with pytest.raises(fmx_mod.FmxError) as e:
+        s.enable_decode(n_slots=2, max_req=2)
+    assert "relative-position bias" in str(e.value)
