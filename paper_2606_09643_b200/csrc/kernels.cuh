@@ -1357,7 +1357,7 @@ struct RowLoraArgs {
 //  * adjacent lanes read adjacent 16 bytes: a shrink warp reads 512 contiguous bytes of a slab row per instruction, an expand warp
 //    covers the r_pad * 2 contiguous bytes of a column of B with r_pad / 8 adjacent lanes (one cache-line lookup per column instead
 //    of one per 16 bytes).
-constexpr int kRowShrinkK = 2048;                   // longest input range of one shrink warp
+constexpr int kRowShrinkK = 1024;                   // longest input range of one shrink warp
 __device__ __forceinline__ float dot8_bf16(const uint4 &p, const uint4 &q) {
   return bf16_lo(p.x) * bf16_lo(q.x) + bf16_hi(p.x) * bf16_hi(q.x) + bf16_lo(p.y) * bf16_lo(q.y) + bf16_hi(p.y) * bf16_hi(q.y) +
          bf16_lo(p.z) * bf16_lo(q.z) + bf16_hi(p.z) * bf16_hi(q.z) + bf16_lo(p.w) * bf16_lo(q.w) + bf16_hi(p.w) * bf16_hi(q.w);
