@@ -53,6 +53,7 @@ __global__ void __launch_bounds__(kAttnThreads) attention_kernel(const AttnArgs 
   __nv_bfloat16 *sQ = reinterpret_cast<__nv_bfloat16 *>(attn_smem);
   __nv_bfloat16 *sK = sQ + kAttnBQ * LD;                // 2 stages
   __nv_bfloat16 *sV = sK + 2 * kAttnBKV * LD;           // 2 stages
+  __shared__ float s_rel[kAttnBQ + kAttnBKV];           // relative-position bias of the current (query tile, key tile): index (key - key0) - (query - q0) + 63
 
   const int p = blockIdx.z, head = blockIdx.y, q0 = blockIdx.x * kAttnBQ;
   griddep_launch();
@@ -82,6 +83,10 @@ __global__ void __launch_bounds__(kAttnThreads) attention_kernel(const AttnArgs 
 
   for (int j = 0; j < n_kv_tiles; ++j) {
     const int st = j & 1;
+    if (a.relb && threadIdx.x < kAttnBQ + kAttnBKV - 1) {      // the previous iteration ended with a block barrier: s_rel is free
+      const int rel = j * kAttnBKV - q0 - (kAttnBQ - 1) + (int)threadIdx.x;
+      s_rel[threadIdx.x] = __ldg(a.relb + head * a.relb_ld + min(max(rel + a.relb_off, 0), a.relb_ld - 1));   // (clamped: padding rows / keys only)
+    }
     if (j + 1 < n_kv_tiles) {
       load_tile_async<DH>(sK + (st ^ 1) * kAttnBKV * LD, gk, a.ld_qkv, (j + 1) * kAttnBKV, n);
       load_tile_async<DH>(sV + (st ^ 1) * kAttnBKV * LD, gv, a.ld_qkv, (j + 1) * kAttnBKV, n);
@@ -122,7 +127,7 @@ __global__ void __launch_bounds__(kAttnThreads) attention_kernel(const AttnArgs 
         float v = -1e30f;
         if (!masked) {
           v = s[nt][e] * a.scale_log2;
-          if (a.relb) v += __ldg(a.relb + head * a.relb_ld + max((key - qrow) + a.relb_off, 0));   // (rows past the request's end are padding)
+          if (a.relb) v += s_rel[(key - key0) - (qrow - q0) + (kAttnBQ - 1)];
         }
         s[nt][e] = v;
         mx[e >> 1] = fmaxf(mx[e >> 1], v);
