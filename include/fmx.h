@@ -111,8 +111,8 @@ typedef struct fmx_backbone_desc {
   /* Optional T5-style relative-position bias (reading 36): bias[g][a][b] =
    * rel_bias[bucket(b - a)][g] is added to the scaled scores of query head g, query position a, key position b, in every
    * layer.  Buckets as in T5: half per direction when !causal, exact up to n/2 - 1, then logarithmic up to rel_max_distance,
-   * the last one open-ended.  rel_bias NULL / rel_buckets 0 = none.  Backbones with a bias run their attention on the
-   * generic mma.sync kernel and do not serve token decode (fmx_register_lm_head: FMX_E_SHAPE). */
+   * the last one open-ended.  rel_bias NULL / rel_buckets 0 = none.  Backbones with a bias do not serve token decode
+   * (fmx_register_lm_head: FMX_E_SHAPE). */
   const void *rel_bias;        /* DEVICE bf16 [rel_buckets, n_q_heads] or NULL; copied at registration */
   int32_t rel_buckets;         /* even, 2 .. 256 (causal: 2 .. 256)                                    */
   int32_t rel_max_distance;    /* > rel_buckets                                                        */

@@ -48,6 +48,10 @@ struct AttnTcArgs {
   int causal;
   float scale_log2;              // log2(e) / sqrt(d_h)
   int reverse;                   // 1: requests are walked from the last to the first (blockIdx.z reversed)
+  // kBias instantiations only: relative-position bias by distance, relb[head * relb_ld + (key - query) + relb_off], times log2(e);
+  // the table is padded so that the padding rows / keys of a tile index inside it
+  const float *relb;
+  int relb_ld, relb_off;
 };
 
 template <int DH>
@@ -99,6 +103,13 @@ __device__ __forceinline__ float fa_chunk_max(uint32_t (&v)[NC], int key0, int l
   for (int c = 0; c < NC; ++c) m4[c & 3] = fmaxf(m4[c & 3], __uint_as_float(v[c]));
   return fmaxf(fmaxf(m4[0], m4[1]), fmaxf(m4[2], m4[3]));
 }
+// kBias: raw scores -> scores in the log2 domain with the relative-position bias of the row added (rel = the row's table entry for
+// the chunk's first key); the maximum / exponent steps then run with a scale of 1.
+template <int NC>
+__device__ __forceinline__ void fa_chunk_bias(uint32_t (&v)[NC], float scale_log2, const float *__restrict__ rel) {
+#pragma unroll
+  for (int c = 0; c < NC; ++c) v[c] = __float_as_uint(fmaf(__uint_as_float(v[c]), scale_log2, __ldg(rel + c)));
+}
 // ... -> P = exp2(S c - m_ref) as NC / 2 packed bf16 pairs; returns the row sum of the chunk.
 template <int NC>
 __device__ __forceinline__ float fa_chunk_exp(const uint32_t (&v)[NC], uint32_t (&pk)[NC / 2], float scale_log2, float m_ref) {
@@ -113,7 +124,7 @@ __device__ __forceinline__ float fa_chunk_exp(const uint32_t (&v)[NC], uint32_t 
   return (r4[0] + r4[1]) + (r4[2] + r4[3]);
 }
 
-template <int DH, int kSBuf, int kMinBlocks, bool kOnePass>
+template <int DH, int kSBuf, int kMinBlocks, bool kOnePass, bool kBias = false>
 __global__ void __launch_bounds__(kFaThreads, kMinBlocks) attention_fa_kernel(const __grid_constant__ AttnTcArgs a) {
   constexpr int kKB = DH / 64;                        // 64-column blocks of the head
   constexpr int kQBytes = kKB * 16384;                // the q-tile
@@ -260,6 +271,8 @@ __global__ void __launch_bounds__(kFaThreads, kMinBlocks) attention_fa_kernel(co
     const uint32_t t_o = tm_o + lane_sel;
     const int lim = a.causal ? min(n, qrow + 1) : n;                 // keys [0, lim) are visible to this row
     float m_ref = 0.0f, l_run = 0.0f;
+    const float sc = kBias ? 1.0f : a.scale_log2;                    // kBias: fa_chunk_bias has already scaled the scores
+    const float *relrow = kBias ? a.relb + head * a.relb_ld + a.relb_off - qrow : nullptr;    // + key = this row's bias for that key
     for (int j = 0; j < nkv; ++j) {
       const int cols = j == nkv - 1 ? tail_cols : 64;
       const int sb = kSBuf == 2 ? (j & 1) : 0;
@@ -272,7 +285,7 @@ __global__ void __launch_bounds__(kFaThreads, kMinBlocks) attention_fa_kernel(co
         // the reference maximum moves lazily; when it does, O (quiescent once PV_(j-1) has completed) is rescaled in TMEM
         float factor = 1.0f;
         auto update_ref = [&](float mx) {
-          mx *= a.scale_log2;                                        // scale > 0; -inf stays -inf
+          mx *= sc;                                                  // scale > 0; -inf stays -inf
           bool rescale = false;
           if (j == 0) {
             m_ref = (mx == -INFINITY) ? 0.0f : mx;
@@ -303,33 +316,38 @@ __global__ void __launch_bounds__(kFaThreads, kMinBlocks) attention_fa_kernel(co
           tmem_ld_32x32(t_s, v0);
           tmem_ld_32x32(t_s + 32, v1);
           tmem_ld_wait();
+          if constexpr (kBias) { fa_chunk_bias<32>(v0, a.scale_log2, relrow + key0); fa_chunk_bias<32>(v1, a.scale_log2, relrow + key0 + 32); }
           update_ref(fmaxf(fa_chunk_max<32>(v0, key0, lim, need_mask), fa_chunk_max<32>(v1, key0 + 32, lim, need_mask)));
-          rs = fa_chunk_exp<32>(v0, pk, a.scale_log2, m_ref);
+          rs = fa_chunk_exp<32>(v0, pk, sc, m_ref);
           tmem_st_32x16(t_s, pk);
-          rs += fa_chunk_exp<32>(v1, pk, a.scale_log2, m_ref);
+          rs += fa_chunk_exp<32>(v1, pk, sc, m_ref);
           tmem_st_32x16(t_s + 16, pk);
         } else if (cols == 64) {
           // two passes over S in 32-column chunks: half the live registers, twice the TMEM loads
           uint32_t v[32], pk[16];
           tmem_ld_32x32(t_s, v);
           tmem_ld_wait();
+          if constexpr (kBias) fa_chunk_bias<32>(v, a.scale_log2, relrow + key0);
           float mx = fa_chunk_max<32>(v, key0, lim, need_mask);
           tmem_ld_32x32(t_s + 32, v);
           tmem_ld_wait();
+          if constexpr (kBias) fa_chunk_bias<32>(v, a.scale_log2, relrow + key0 + 32);
           update_ref(fmaxf(mx, fa_chunk_max<32>(v, key0 + 32, lim, need_mask)));
-          rs = fa_chunk_exp<32>(v, pk, a.scale_log2, m_ref);         // second chunk first: it is in registers
+          rs = fa_chunk_exp<32>(v, pk, sc, m_ref);                   // second chunk first: it is in registers
           tmem_ld_32x32(t_s, v);
           tmem_ld_wait();
           tmem_st_32x16(t_s + 16, pk);
+          if constexpr (kBias) fa_chunk_bias<32>(v, a.scale_log2, relrow + key0);
           if (need_mask) fa_chunk_max<32>(v, key0, lim, true);
-          rs += fa_chunk_exp<32>(v, pk, a.scale_log2, m_ref);
+          rs += fa_chunk_exp<32>(v, pk, sc, m_ref);
           tmem_st_32x16(t_s, pk);
         } else {
           uint32_t v[16], pk[8];
           tmem_ld_32x16(t_s, v);
           tmem_ld_wait();
+          if constexpr (kBias) fa_chunk_bias<16>(v, a.scale_log2, relrow + key0);
           update_ref(fa_chunk_max<16>(v, key0, lim, need_mask));
-          rs = fa_chunk_exp<16>(v, pk, a.scale_log2, m_ref);
+          rs = fa_chunk_exp<16>(v, pk, sc, m_ref);
           tmem_st_32x8(t_s, pk);
         }
         l_run = l_run * factor + rs;

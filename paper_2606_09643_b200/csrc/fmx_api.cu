@@ -69,7 +69,8 @@ struct Backbone {
   float *posb = nullptr;                   // [n_pos, d]
   float2 *rope_cs = nullptr;               // [max_seq, dh/2]
   float2 *rope_cs_t = nullptr;             // [dh/2, max_seq] (the fused-RoPE GEMM epilogue reads this one)
-  float *relb = nullptr;                   // relative-position bias by distance: [n_q_heads, 2 max_seq - 1] fp32, times log2(e); index (key - query) + max_seq - 1
+  float *relb = nullptr;                   // relative-position bias by distance: [n_q_heads, relb_ld] fp32, times log2(e); index (key - query) + relb_off;
+  int relb_ld = 0, relb_off = 0;           //   padded by 128 / 127 zeros so that a tile's padding rows / keys index inside the table
   // weight maps, [0] = box {64,128} (pair tile 256x256: one CTA loads a whole chunk), [1] = box {64,64} (256x128 tiles)
   std::vector<CUtensorMap> mWq[2], mWk[2], mWv[2], mWo[2], mWup[2], mWgate[2], mWdown[2];
   CUtensorMap mEmbedW[2];
@@ -478,19 +479,24 @@ bool attn_use_tc(int impl, int dh, int max_len) {
 // trades (profiles/r2_02): head_dim 64 one-pass at 3 CTAs per SM 5.2 vs 3.5 ms per cfg3 step; head_dim 128 two-pass 6.7 vs 6.4 ms.
 void launch_attention_tc(Strm s, int dh, int max_len, int n_heads, int B, const AttnTcArgs &a) {
   dim3 grid((max_len + kAtBQ - 1) / kAtBQ, n_heads, B);
+  if (a.relb) {              // relative-position bias: the same kernels with the bias added to each score (d_h 64: 3 CTAs per SM for the registers)
+    if (dh == 64) launch_k((attention_fa_kernel<64, 1, 3, false, true>), grid, kFaThreads, attn_fa_smem_bytes<64>(), s, a);
+    else launch_k((attention_fa_kernel<128, 2, 2, true, true>), grid, kFaThreads, attn_fa_smem_bytes<128>(), s, a);
+    return;
+  }
   if (dh == 64) launch_k((attention_fa_kernel<64, 1, 4, false>), grid, kFaThreads, attn_fa_smem_bytes<64>(), s, a);
   else launch_k((attention_fa_kernel<128, 2, 2, true>), grid, kFaThreads, attn_fa_smem_bytes<128>(), s, a);
 }
-template <int DH, int kSBuf, int kMinB, bool kOne>
+template <int DH, int kSBuf, int kMinB, bool kOne, bool kBias = false>
 cudaError_t set_attn_fa_attr() {
-  cudaError_t e = cudaFuncSetAttribute(attention_fa_kernel<DH, kSBuf, kMinB, kOne>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_fa_smem_bytes<DH>());
+  cudaError_t e = cudaFuncSetAttribute(attention_fa_kernel<DH, kSBuf, kMinB, kOne, kBias>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_fa_smem_bytes<DH>());
   // without this the driver sizes the L1/shared split for ONE block and further CTAs never become resident
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(attention_fa_kernel<DH, kSBuf, kMinB, kOne>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(attention_fa_kernel<DH, kSBuf, kMinB, kOne, kBias>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
   if (e == cudaSuccess && getenv("FMX_DEBUG")) {
     int nb = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, attention_fa_kernel<DH, kSBuf, kMinB, kOne>, kFaThreads, attn_fa_smem_bytes<DH>());
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, attention_fa_kernel<DH, kSBuf, kMinB, kOne, kBias>, kFaThreads, attn_fa_smem_bytes<DH>());
     cudaFuncAttributes fa{};
-    cudaFuncGetAttributes(&fa, attention_fa_kernel<DH, kSBuf, kMinB, kOne>);
+    cudaFuncGetAttributes(&fa, attention_fa_kernel<DH, kSBuf, kMinB, kOne, kBias>);
     fprintf(stderr, "fmx: attention_fa<%d,%d,%d,%d>: %d B smem, %d CTA/SM, %d regs\n", DH, kSBuf, kMinB, (int)kOne, attn_fa_smem_bytes<DH>(), nb, fa.numRegs);
   }
   return e;
@@ -499,6 +505,8 @@ cudaError_t set_attn_fa_attr() {
 int set_kernel_attrs() {
   CU_OK((set_attn_fa_attr<64, 1, 4, false>()));
   CU_OK((set_attn_fa_attr<128, 2, 2, true>()));
+  CU_OK((set_attn_fa_attr<64, 1, 3, false, true>()));
+  CU_OK((set_attn_fa_attr<128, 2, 2, true, true>()));
   CU_OK((cudaFuncSetAttribute(pair_gemm_kernel<256, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<256, false>())));
   CU_OK((cudaFuncSetAttribute(pair_gemm_kernel<256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<256, true>())));
   CU_OK((cudaFuncSetAttribute(pair_gemm_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pair_smem_bytes<128, false>())));
@@ -926,10 +934,10 @@ int fmx_register_backbone(fmx_ctx *c, const fmx_backbone_desc *desc, fmx_backbon
   if (d.rel_bias && d.rel_buckets > 0) {
     // bias by relative distance, for every head: the bucket of each distance is taken here on the host (T5's bucket function in
     // double precision, reading 36), the table row is the caller's bf16 value; stored times log2(e) for the exp2 softmax
-    const int nb = d.rel_buckets, H = d.n_q_heads, S = d.max_seq, ld = 2 * S - 1;
+    const int nb = d.rel_buckets, H = d.n_q_heads, S = d.max_seq, off = S - 1 + 128, ld = 2 * S - 1 + 255;
     std::vector<uint16_t> tab((size_t)nb * H);
     CU_OK(cudaMemcpy(tab.data(), d.rel_bias, tab.size() * sizeof(uint16_t), cudaMemcpyDeviceToHost));
-    std::vector<float> dense((size_t)H * ld);
+    std::vector<float> dense((size_t)H * ld, 0.0f);
     for (int rel = -(S - 1); rel <= S - 1; ++rel) {
       int n = nb, bucket = 0, dist;
       if (!d.causal) { n /= 2; if (rel > 0) bucket += n; dist = rel < 0 ? -rel : rel; }
@@ -941,11 +949,12 @@ int fmx_register_backbone(fmx_ctx *c, const fmx_backbone_desc *desc, fmx_backbon
         const uint32_t bits = (uint32_t)tab[(size_t)bucket * H + g] << 16;
         float v;
         memcpy(&v, &bits, sizeof(v));
-        dense[(size_t)g * ld + rel + S - 1] = v * 1.4426950408889634f;
+        dense[(size_t)g * ld + rel + off] = v * 1.4426950408889634f;
       }
     }
     CU_OK(cudaMalloc(&b->relb, dense.size() * sizeof(float)));
     CU_OK(cudaMemcpy(b->relb, dense.data(), dense.size() * sizeof(float), cudaMemcpyHostToDevice));
+    b->relb_ld = ld; b->relb_off = off;
   }
   CU_OK(cudaDeviceSynchronize());
   b->Rcap = 256;
@@ -1530,8 +1539,9 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       pa2.n_q_heads = d.n_q_heads; pa2.n_kv_heads = d.n_kv_heads; pa2.causal = d.causal; pa2.scale_log2 = scale_log2;
       pa2.reverse = rev();
       LAUNCH(Lh, F_ATTN, launch_attention_pair64(S, c->sm_count, pa2));
-    } else if (!bb.relb && attn_use_tc(c->o.attn_impl, d.head_dim, max_len)) {
+    } else if (attn_use_tc(c->o.attn_impl, d.head_dim, max_len)) {
       AttnTcArgs ta{};
+      ta.relb = bb.relb; ta.relb_ld = bb.relb_ld; ta.relb_off = bb.relb_off;
       ta.qkv_map = mQKV64; ta.out = w.AttnO; ta.cu_tok = w.t.cu_tok; ta.ld_out = bb.d_q;
       ta.n_q_heads = d.n_q_heads; ta.n_kv_heads = d.n_kv_heads; ta.causal = d.causal; ta.scale_log2 = scale_log2;
       ta.reverse = rev();
@@ -1540,7 +1550,7 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
       AttnArgs aa{};
       aa.qkv = w.QKV; aa.out = w.AttnO; aa.cu_tok = w.t.cu_tok; aa.ld_qkv = bb.d_qkv; aa.ld_out = bb.d_q;
       aa.n_q_heads = d.n_q_heads; aa.n_kv_heads = d.n_kv_heads; aa.causal = d.causal; aa.scale_log2 = scale_log2;
-      aa.relb = bb.relb; aa.relb_ld = 2 * d.max_seq - 1; aa.relb_off = d.max_seq - 1;     // relative-position bias: the generic kernel only
+      aa.relb = bb.relb; aa.relb_ld = bb.relb_ld; aa.relb_off = bb.relb_off;
       dim3 grid((max_len + kAttnBQ - 1) / kAttnBQ, d.n_q_heads, B);
       if (max_len <= 64 && c->o.attn_short && !bb.relb) LAUNCH(Lh, F_ATTN, launch_attention_short(S, c->sm_count, d.head_dim, B, aa));
       else LAUNCH(Lh, F_ATTN, launch_attention(S, d.head_dim, grid, aa));
