@@ -12,7 +12,8 @@
 //   mma.sync m16n8k16 (bf16 in, fp32 accumulate): warp w owns columns 16 w .. 16 w + 15 of the slice for every 16-row tile;
 //   the raw fp32 partial goes to [k_split, split_rows, N]; splitk_reduce_kernel / qkv_reduce_rope_kernel /
 //        reduce_resid_norm_kernel add the slices in order, the LoRA delta and the bias, and apply what follows.
-// k_split depends on the projection's shape only, never on the batch: a request decodes to the same bits alone and in a batch.
+// k_split depends on the projection's shape only, never on the batch, and a row's accumulation does not depend on the other rows:
+// a request decodes to the same bits alone and in any batch of <= 128 rows (larger batches take the pair GEMM: another summation order).
 #pragma once
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>

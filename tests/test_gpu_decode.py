@@ -84,6 +84,53 @@ def test_prefill_and_decode_match_the_no_cache_definition(fmx_mod, cfg, kw, opts
     assert np.array_equal(sc_all[i], sc_one[0])
 
 
+@pytest.mark.parametrize("B,opts", [
+    (40, {}),                                   # row_gemm_kernel<4> (33 .. 64 rows)
+    (100, {}),                                  # row_gemm_kernel<8> (65 .. 128 rows)
+    (150, {}),                                  # > 128 rows: the pair GEMM in partial-output mode (split K) + the same reductions
+    (24, dict(decode_rowgemm=0, decode_fork=0)),   # small batch on the pair-GEMM partial path, LoRA kernels on the serving stream
+])
+def test_decode_batch_sizes_and_paths_match_the_definition(fmx_mod, B, opts):
+    """Decode iterations at the batch sizes that select the other projection kernels (tests above stay <= 16 rows): a sample of
+    requests against the no-cache oracle after prefill and after two decode steps, and alone == in-batch bit for bit."""
+    from paper_2606_09643_b200.session import Session
+    wl = make_workload("cfg4", n_layers=1, batch=B, max_len=24, n_tasks=12)
+    s = Session(wl, max_req=B, max_tokens=max(wl.n_tokens, 64))
+    for k, v in opts.items():
+        s.fmx.set_option(k, v)
+    s.enable_decode(n_slots=B, max_req=B)
+    bb, get, tasks = G.bb_dict(wl), G.make_get(wl), G.task_dicts(wl)
+    slots = np.random.default_rng(B).permutation(B).astype(np.int32)
+    scores, nxt, _ = s.prefill(wl.packed_inputs(), wl.task_ids, wl.lengths, slots, with_heads=False)
+    seqs = [list(map(int, wl.request_input(i))) for i in range(B)]
+    sample = sorted(set([0, 1, B // 3, B // 2, B - 2, B - 1, int(np.argmax(wl.lengths)), int(np.argmin(wl.lengths))]))
+    for i in sample:
+        check_scores(scores[i], D.lm_scores(bb, get, tasks[int(wl.task_ids[i])], seqs[i]), f"B={B} prefill request {i}")
+    pending = [int(t) for t in nxt]
+    for step in range(2):
+        toks = torch.tensor(pending, dtype=torch.int32, device="cuda")
+        pos = np.array([len(q) for q in seqs], dtype=np.int32)
+        sc, nx = s.decode_step(toks.data_ptr(), wl.task_ids, slots, pos)
+        for i in range(B):
+            seqs[i].append(pending[i])
+        for i in sample:
+            ref = D.lm_scores(bb, get, tasks[int(wl.task_ids[i])], seqs[i])
+            check_scores(sc[i], ref, f"B={B} decode step {step} request {i}")
+            check_token(nx[i], ref, f"B={B} decode step {step} request {i}")
+        pending = [int(t) for t in nx]
+    # alone == in the batch (the projection kernel is chosen by the BATCH size, so this holds within a size class only:
+    # compare against a batch of the same class that contains the request)
+    toks = torch.tensor(pending, dtype=torch.int32, device="cuda")
+    pos = np.array([len(q) for q in seqs], dtype=np.int32)
+    sc_all, _ = s.decode_step(toks.data_ptr(), wl.task_ids, slots, pos)
+    keep = np.arange(B)[::-1].copy()[: max(B - 3, 1)]                  # another order, three requests fewer, same size class
+    lo = {40: 33, 100: 65, 150: 129, 24: 17}[B]
+    assert len(keep) >= lo
+    sc_sub, _ = s.decode_step(toks[torch.from_numpy(keep).cuda()].contiguous().data_ptr(), wl.task_ids[keep], slots[keep], pos[keep])
+    for j, i in enumerate(keep[:5]):
+        assert np.array_equal(sc_all[i], sc_sub[j]), f"B={B}: request {i} decodes differently in another batch"
+
+
 def test_decode_steps_replay_the_cached_graph_with_identical_results(fmx_mod):
     """On a non-default stream the decode iterations of one batch shape are captured once and replayed, positions and slots
     changing from step to step: the tokens and scores equal those of plain launches bit for bit."""
