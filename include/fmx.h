@@ -257,7 +257,7 @@ int fmx_prefill(fmx_ctx *ctx, fmx_backbone_t bb, const void *inputs, const int32
  *   positions  HOST int32 [n_req]
  * workspace: >= fmx_workspace_bytes(n_req, n_req tokens).
  * Reproducibility: a request's scores do not depend on which other requests share the iteration, bit for bit, among batches
- * of 1 .. 128 requests and among batches of 129 .. 256 (the two ranges run different projection kernels). */
+ * of 1 .. 128 requests, among batches of 129 .. 256 and among larger ones (the three ranges run different projection kernels). */
 int fmx_decode_step(fmx_ctx *ctx, fmx_backbone_t bb, const int32_t *tokens, const int32_t *task_ids, const int32_t *slots,
                     const int32_t *positions, int32_t n_req, float *scores, int32_t *next_tokens, void *kv_cache,
                     int32_t n_slots, void *workspace, size_t workspace_bytes, void *cuda_stream);

@@ -89,6 +89,7 @@ def test_prefill_and_decode_match_the_no_cache_definition(fmx_mod, cfg, kw, opts
     (100, {}),                                  # row_gemm_kernel<8> (65 .. 128 rows)
     (150, {}),                                  # > 128 rows: the pair GEMM in partial-output mode (split K) + the same reductions
     (24, dict(decode_rowgemm=0, decode_fork=0)),   # small batch on the pair-GEMM partial path, LoRA kernels on the serving stream
+    (300, {}),                                  # > 256 rows (two row tiles): the prefill kernels (segmented tensor-core LoRA, fused epilogues) + decode attention
 ])
 def test_decode_batch_sizes_and_paths_match_the_definition(fmx_mod, B, opts):
     """Decode iterations at the batch sizes that select the other projection kernels (tests above stay <= 16 rows): a sample of
@@ -124,7 +125,7 @@ def test_decode_batch_sizes_and_paths_match_the_definition(fmx_mod, B, opts):
     pos = np.array([len(q) for q in seqs], dtype=np.int32)
     sc_all, _ = s.decode_step(toks.data_ptr(), wl.task_ids, slots, pos)
     keep = np.arange(B)[::-1].copy()[: max(B - 3, 1)]                  # another order, three requests fewer, same size class
-    lo = {40: 33, 100: 65, 150: 129, 24: 17}[B]
+    lo = {40: 33, 100: 65, 150: 129, 24: 17, 300: 257}[B]
     assert len(keep) >= lo
     sc_sub, _ = s.decode_step(toks[torch.from_numpy(keep).cuda()].contiguous().data_ptr(), wl.task_ids[keep], slots[keep], pos[keep])
     for j, i in enumerate(keep[:5]):
