@@ -145,6 +145,8 @@ def build_workload(args):
     if args.workload == "cfg5":
         return make_workload("cfg5", n_tasks=args.tasks, dist=args.dist, adapters=not args.no_adapters, mlp_hidden=args.mlp_hidden, enc_channels=args.enc_channels,
                              rel_bias=args.rel_bias)
+    if args.workload == "decode":                       # (the reference arm on this workload times the cfg4 prefill oracle)
+        return make_workload("cfg4")
     return make_workload(args.workload, mlp_hidden=args.mlp_hidden, enc_channels=args.enc_channels, rel_bias=args.rel_bias)
 
 
