@@ -73,9 +73,10 @@ __device__ inline V block_exclusive_scan(V *a, int n, V *scratch) {
 __device__ inline long long block_exclusive_scan_ll(long long *a, int n, long long *scratch) { return block_exclusive_scan<long long>(a, n, scratch); }
 __device__ inline int block_exclusive_scan_i(int *a, int n, int *scratch) { return block_exclusive_scan<int>(a, n, scratch); }
 
-// Exclusive scan of f(0) .. f(n - 1) written to out[0 .. n) (global), f evaluated twice per element; returns the total.
-template <typename V, typename F>
-__device__ inline V block_exclusive_scan_fn(int n, F f, V *out, V *scratch) {
+// Exclusive scan of f(0) .. f(n - 1); emit(i, offset) receives every element's exclusive offset (f is evaluated twice per
+// element, emit once, by the thread that owns the element's run); returns the total.  Every thread of the block must call it.
+template <typename V, typename F, typename E>
+__device__ inline V block_exclusive_scan_emit(int n, F f, E emit, V *scratch) {
   const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, wid = tid >> 5;
   const int per = (n + nt - 1) / nt;
   const int lo = min(tid * per, n), hi = min(lo + per, n);
@@ -96,7 +97,33 @@ __device__ inline V block_exclusive_scan_fn(int n, F f, V *out, V *scratch) {
   }
   __syncthreads();
   V run = scratch[wid] + incl - s;
-  for (int i = lo; i < hi; ++i) { out[i] = run; run += f(i); }
+  for (int i = lo; i < hi; ++i) { emit(i, run); run += f(i); }
+  const V total = scratch[32];
+  __syncthreads();
+  return total;
+}
+// Exclusive scan over 4 consecutive values per thread (thread t owns elements 4 t .. 4 t + 3), in registers; returns the total.
+template <typename V>
+__device__ inline V block_exclusive_scan_reg4(V (&v)[4], V *scratch) {
+  const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, wid = tid >> 5;
+  const V s = (v[0] + v[1]) + (v[2] + v[3]);
+  V incl = s;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const V x = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += x; }
+  if (lane == 31) scratch[wid] = incl;
+  __syncthreads();
+  if (wid == 0) {
+    const V w = lane < (nt >> 5) ? scratch[lane] : V(0);
+    V wi = w;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const V x = __shfl_up_sync(0xffffffffu, wi, d); if (lane >= d) wi += x; }
+    scratch[lane] = wi - w;
+    if (lane == 31) scratch[32] = wi;
+  }
+  __syncthreads();
+  V run = scratch[wid] + incl - s;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) { const V x = v[k]; v[k] = run; run += x; }
   const V total = scratch[32];
   __syncthreads();
   return total;
@@ -104,9 +131,10 @@ __device__ inline V block_exclusive_scan_fn(int n, F f, V *out, V *scratch) {
 
 // One CTA.  Stable counting sort of request indices by task id, then the prefix tables and the
 // (row-tile, task) block table the segmented GEMMs walk.  Integer only; deterministic.
-// The ids and lengths are read from global memory once (ids to shared memory, lengths to registers); ranking and the scans of the
-// counts and the sorted lengths run in shared memory, the offset tables are scanned from their defining expressions and written
-// once - the kernel's time is the handful of dependent global round trips that remain, not arithmetic.
+// Global memory is read twice, each time with every load of the block in flight at once: the ids and lengths of the thread's four
+// consecutive requests, then the task tables at those ids.  Ranking, the scans of the counts and of the sorted lengths run in
+// shared memory, the input / output offsets are scanned in registers, the block table is filled inside its own scan; everything
+// else is a store.  (B <= 4096 = 4 x kSortThreads, T <= 1024.)
 __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortArgs a) {
   __shared__ int s_cnt[1024 + 1];          // per-task count, then task_req_off
   __shared__ int s_tok[1024 + 1];          // task_tok_off
@@ -120,12 +148,23 @@ __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortAr
   griddep_launch();
   griddep_wait();
 
-  int len_r[4];                            // lengths of the requests tid, tid + 1024, ... (B <= 4096)
+  const int i0 = 4 * tid;                  // this thread's requests: i0 .. i0 + 3
+  int id_r[4], len_r[4];
 #pragma unroll
   for (int k = 0; k < 4; ++k) {
-    const int i = tid + k * kSortThreads;
-    len_r[k] = i < B ? t.lengths[i] : 0;
-    if (i < B) s_task[i] = (unsigned short)t.task_ids[i];
+    const bool ok = i0 + k < B;
+    id_r[k] = ok ? t.task_ids[i0 + k] : 0;
+    len_r[k] = ok ? t.lengths[i0 + k] : 0;
+  }
+  long long vin[4], vout[4];               // packed-input elements / output values of the request (0 past the end)
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const bool ok = i0 + k < B;
+    const int ch = (ok && a.task_enc_ch) ? max(a.task_enc_ch[id_r[k]], 1) : 1;
+    const int ho = ok ? a.task_head_out[id_r[k]] : 0, hk = ok ? a.task_head_kind[id_r[k]] : 0;
+    vin[k] = ok ? (long long)len_r[k] * a.in_per_tok + a.in_per_req * ch : 0;
+    vout[k] = (long long)ho * (hk == 4 ? len_r[k] : 1);
+    if (ok) s_task[i0 + k] = (unsigned short)id_r[k];
   }
   for (int i = tid; i <= T; i += blockDim.x) s_cnt[i] = 0;
   __syncthreads();
@@ -145,7 +184,15 @@ __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortAr
       __syncwarp();
     }
   }
-  __syncthreads();
+  // (5) input / output offsets in ORIGINAL request order (registers; warp 0 joins after the ranking)
+  {
+    const long long tin = block_exclusive_scan_reg4<long long>(vin, s_scratch_ll);
+    const long long tout = block_exclusive_scan_reg4<long long>(vout, s_scratch_ll);
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      if (i0 + k < B) { t.in_off[i0 + k] = vin[k]; t.out_off[i0 + k] = vout[k]; }
+    if (tid == 0) { t.in_off[B] = tin; t.out_off[B] = tout; }
+  }
   // (2) task_req_off = exclusive scan of the counts
   if (tid == 0) s_cnt[T] = 0;
   __syncthreads();
@@ -154,13 +201,12 @@ __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortAr
   // (3) perm / inv_perm / sorted lengths
 #pragma unroll
   for (int k = 0; k < 4; ++k) {
-    const int i = tid + k * kSortThreads;
+    const int i = i0 + k;
     if (i >= B) continue;
-    const int tk = s_task[i];
-    const int pos = s_cnt[tk] + s_rank[i];
+    const int pos = s_cnt[id_r[k]] + s_rank[i];
     t.perm[pos] = i;
     t.inv_perm[i] = pos;
-    t.task_sorted[pos] = tk;
+    t.task_sorted[pos] = id_r[k];
     s_slen[pos] = len_r[k];
   }
   if (tid == 0) s_slen[B] = 0;
@@ -169,18 +215,8 @@ __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortAr
   block_exclusive_scan_i(s_slen, B + 1, s_scratch);
   for (int i = tid; i <= B; i += blockDim.x) t.cu_tok[i] = s_slen[i];
   for (int i = tid; i <= T; i += blockDim.x) { const int v = s_slen[s_cnt[i]]; s_tok[i] = v; t.task_tok_off[i] = v; }
-  // (5) input / output offsets in ORIGINAL request order
-  block_exclusive_scan_fn<long long>(B + 1, [&](int i) -> long long {
-    if (i >= B) return 0;
-    const int ch = a.task_enc_ch ? max(a.task_enc_ch[s_task[i]], 1) : 1;
-    return (long long)t.lengths[i] * a.in_per_tok + a.in_per_req * ch;
-  }, t.in_off, s_scratch_ll);
-  block_exclusive_scan_fn<long long>(B + 1, [&](int i) -> long long {
-    if (i >= B) return 0;
-    const int tk = s_task[i];
-    return (long long)a.task_head_out[tk] * (a.task_head_kind[tk] == 4 ? t.lengths[i] : 1);
-  }, t.out_off, s_scratch_ll);
-  // (6) block table: for each row tile, the non-empty task segments that intersect it.
+  __syncthreads();
+  // (6) block table: for each row tile, the non-empty task segments that intersect it; filled inside the scan of their counts.
   const int n_tok = s_tok[T];
   auto first_task_after = [&](int row) {     // smallest task with tok_off[task+1] > row
     int lo = 0, hi = T;                      // invariant: answer in [lo, hi)
@@ -188,16 +224,16 @@ __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortAr
     return lo;
   };
   auto tile_blocks = [&](int m) {
+    if (m >= a.n_tiles) return 0;
     const int r0 = m * a.tile_rows, r1 = min(r0 + a.tile_rows, n_tok);
     int cnt = 0;
     for (int k = first_task_after(r0); k < T && s_tok[k] < r1; ++k) cnt += (s_tok[k + 1] > s_tok[k]);
     return cnt;
   };
-  const int n_blk = block_exclusive_scan_fn<int>(a.n_tiles + 1, [&](int m) { return m < a.n_tiles ? tile_blocks(m) : 0; }, t.tile_blk_off, s_scratch);
-  if (tid == 0) *t.n_blk = n_blk;
-  for (int m = tid; m < a.n_tiles; m += blockDim.x) {
+  const int n_blk = block_exclusive_scan_emit<int>(a.n_tiles + 1, tile_blocks, [&](int m, int b) {
+    t.tile_blk_off[m] = b;
+    if (m >= a.n_tiles) return;
     const int r0 = m * a.tile_rows, r1 = min(r0 + a.tile_rows, n_tok);
-    int b = t.tile_blk_off[m];
     for (int k = first_task_after(r0); k < T && s_tok[k] < r1; ++k) {
       if (s_tok[k + 1] <= s_tok[k]) continue;
       t.blk_tile[b] = m;
@@ -206,7 +242,8 @@ __global__ void __launch_bounds__(kSortThreads, 1) task_sort_kernel(const SortAr
       t.blk_hi[b] = min(s_tok[k + 1], r1) - r0;
       ++b;
     }
-  }
+  }, s_scratch);
+  if (tid == 0) *t.n_blk = n_blk;
 }
 
 // row -> (sorted request index, position within the request)
