@@ -1635,8 +1635,8 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     const int groups = (B + 15) / 16, ogs = (max_out_flat + 31) / 32;
     int n_kc = 0;
     if (c->o.head_tiled == 2 && d.tokens_per_request > 0)
-      for (int k = 1; k <= 8; k *= 2)
-        if (Kf % (256ll * k) == 0) { n_kc = k; if ((long long)groups * ogs * k >= 4ll * c->sm_count) break; }   // >= 4 CTAs per SM (two rounds of the two resident ones): a CTA streams one task's weights per pass at single-SM bandwidth
+      for (int k = 1; k <= 16; k *= 2)
+        if (Kf % (256ll * k) == 0) { n_kc = k; if ((long long)groups * ogs * k >= 8ll * c->sm_count) break; }   // >= 8 CTAs per SM, i.e. four rounds of the two resident ones: a CTA streams one task's weights per pass at single-SM bandwidth (measured on cfg5: 1 / 2 / 4 / 8 per SM = 0.46 / 0.32 / 0.27 / 0.24 ms)
     while (n_kc > 0 && (size_t)groups * ogs * n_kc * 512 > w.head_part_floats) n_kc /= 2;     // fit the workspace's partial budget
     if (n_kc > 0) {
       LAUNCH(Lh, F_HEAD, (launch_k(head_flatten_mma_kernel, dim3(groups, ogs, n_kc), 256, 0, S, ha, B, n_kc, w.head_part)));
