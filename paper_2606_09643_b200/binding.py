@@ -54,7 +54,7 @@ class BfqParams(C.Structure):
     _fields_ = [("n_tasks", C.c_int32), ("b_max", C.c_int32), ("lat_ms", C.POINTER(C.c_double)), ("l_tok_ms", C.c_double)]
 
 
-OPTIONS = {"attention_impl": 0, "pdl": 2, "shrink_stages": 3, "half_tiles": 4, "attn_short": 5, "rope_fused": 6, "head_tiled": 7, "shrink_fused": 8, "graph": 9, "reverse": 10, "expand_wide": 11, "deep_pipe": 12, "decode_fork": 13, "decode_rowgemm": 14}
+OPTIONS = {"attention_impl": 0, "pdl": 2, "shrink_stages": 3, "half_tiles": 4, "attn_short": 5, "rope_fused": 6, "head_tiled": 7, "shrink_fused": 8, "graph": 9, "reverse": 10, "expand_wide": 11, "deep_pipe": 12, "decode_fork": 13, "decode_rowgemm": 14, "embed_small": 15}
 
 
 class FmxError(RuntimeError):

@@ -109,6 +109,7 @@ struct Opts {
   int attn_short = 2;     // 0: generic kernel, 1: pipelined mma.sync kernel, 2: tcgen05 head-pair kernel where it applies
   int graph = 1;
   int attn_impl = FMX_ATTN_AUTO;
+  int embed_small = 1;    // PATCH_LINEAR with patch_dim <= 8: CUDA-core embed kernel instead of the one-k-block GEMM
   int decode_rowgemm = 1; // decode iterations of <= 128 rows: projections on the lean mma.sync kernel (row_gemm.cuh) instead of the pair GEMM
   int decode_fork = 1;    // decode iterations: row-wise LoRA kernels on the auxiliary stream beside the projection GEMM
 };
@@ -1477,12 +1478,20 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
     pa.task_enc_W = (const bf16 *const *)c->d_task_enc_W; pa.task_enc_b = (const bf16 *const *)c->d_task_enc_b;
     pa.series_len = (d.tokens_per_request - (d.has_cls ? 1 : 0)) * d.patch_dim;
     pa.A = w.Hid;
-    LAUNCH(Lh, F_EMBED, (launch_k(pack_patches_kernel, Ni, 128, 0, S, pa)));
-    if ((e = encode_2d(c, &mPk, w.Hid, Ni, bb.Kp, bb.Kp, 128))) return e;
-    PairGemmParams p = base;
-    p.mode = GM_EMBED_F32; p.amap = mPk; p.K = bb.Kp; p.n_chunks = d.d_model / 128;
-    p.wmap[0] = bb.mEmbedW[wv(p)]; p.wmap_h[0] = bb.mEmbedW[1]; p.omap = oX; p.posb = bb.posb; p.ld_pos = d.d_model;
-    LAUNCH(Lh, F_EMBED, launch_pair_gemm(c, S, p));
+    pa.tpr = 128;
+    while (pa.tpr > 8 && pa.tpr / 2 >= bb.Kp) pa.tpr /= 2;          // 8 .. 128 threads per row: tiny patches share a block
+    LAUNCH(Lh, F_EMBED, (launch_k(pack_patches_kernel, (Ni + 128 / pa.tpr - 1) / (128 / pa.tpr), 128, 0, S, pa)));
+    if (bb.Kp == 8 && c->o.embed_small) {
+      // a one-k-block GEMM is all epilogue: tiny patches go through the CUDA-core kernel (kernels.cuh)
+      LAUNCH(Lh, F_EMBED, (launch_k(embed_small_patch_kernel, dim3((Ni + kEmbRows - 1) / kEmbRows, (d.d_model / 4 + 255) / 256), 256, 0, S,
+                                    (const bf16 *)w.Hid, (const bf16 *)bb.embed_Wpad, (const float *)bb.posb, (const int *)w.t.row_pos, Ni, d.d_model, w.X)));
+    } else {
+      if ((e = encode_2d(c, &mPk, w.Hid, Ni, bb.Kp, bb.Kp, 128))) return e;
+      PairGemmParams p = base;
+      p.mode = GM_EMBED_F32; p.amap = mPk; p.K = bb.Kp; p.n_chunks = d.d_model / 128;
+      p.wmap[0] = bb.mEmbedW[wv(p)]; p.wmap_h[0] = bb.mEmbedW[1]; p.omap = oX; p.posb = bb.posb; p.ld_pos = d.d_model;
+      LAUNCH(Lh, F_EMBED, launch_pair_gemm(c, S, p));
+    }
   } else {
     EmbedArgs ea{};
     ea.inputs = inputs; ea.perm = w.t.perm; ea.row_req = w.t.row_req; ea.row_pos = w.t.row_pos; ea.in_off = w.t.in_off;
@@ -2073,6 +2082,9 @@ int fmx_set_option(fmx_ctx *c, int32_t option, int32_t value) {
       return FMX_OK;
     case FMX_OPT_HALF_TILES:
       c->o.half_tiles = value ? 1 : 0;
+      return FMX_OK;
+    case FMX_OPT_EMBED_SMALL:
+      c->o.embed_small = value ? 1 : 0;
       return FMX_OK;
     case FMX_OPT_DECODE_ROWGEMM:
       c->o.decode_rowgemm = value ? 1 : 0;

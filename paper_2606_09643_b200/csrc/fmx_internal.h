@@ -67,6 +67,7 @@ enum {
                                     before the reduction; set 0 when the serving stream belongs to an SM partition */
   FMX_OPT_DECODE_ROWGEMM = 14,   /* 1 (default): decode iterations of <= 128 rows run their projections on the lean mma.sync
                                     kernel (row_gemm.cuh); 0 = the pair GEMM in partial-output mode */
+  FMX_OPT_EMBED_SMALL = 15,      /* 1 (default): patch embeddings with patch_dim <= 8 run on a CUDA-core kernel; 0 = the GEMM */
   FMX_OPT_PDL = 2                /* programmatic dependent launch of the forward's kernels:
                                     0 = off, 1 = always, 2 (default) = only for batches of <= 4096 token rows */
 };

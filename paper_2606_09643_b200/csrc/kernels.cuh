@@ -319,20 +319,22 @@ struct PackArgs {
   const __nv_bfloat16 *const *task_enc_W, *const *task_enc_b;
   int series_len;                  // n_patches * patch_dim (elements of one channel)
   __nv_bfloat16 *A;                // [N, Kp] task-sorted patch rows (CLS rows and the K pad are zero)
+  int tpr;                         // threads per row (a power of two <= blockDim.x): a block packs blockDim.x / tpr rows
 };
 
-// PATCH_LINEAR: gather (and patchify) into the A operand of the embed GEMM.  One block per row.
+// PATCH_LINEAR: gather (and patchify) into the A operand of the embed GEMM.  tpr threads per row.
 __global__ void pack_patches_kernel(const PackArgs a) {
   griddep_launch();
   griddep_wait();
-  const int r = blockIdx.x;
+  const int r = blockIdx.x * (blockDim.x / a.tpr) + threadIdx.x / a.tpr;
+  if (r >= a.N) return;
   const int pos = a.row_pos[r], i = a.perm[a.row_req[r]];
   const __nv_bfloat16 *src = a.inputs + a.in_off[i];
   __nv_bfloat16 *dst = a.A + (size_t)r * a.Kp;
   const int pi = pos - a.has_cls;
   const int P = a.patch_hw, g = a.img_c ? a.img_hw / P : 1;
   const int gy = pi / g, gx = pi - gy * g;
-  for (int e = threadIdx.x; e < a.Kp; e += blockDim.x) {
+  for (int e = threadIdx.x % a.tpr; e < a.Kp; e += a.tpr) {
     __nv_bfloat16 v = __float2bfloat16(0.0f);
     if (pi >= 0 && e < a.patch_dim) {
       if (a.img_c) {
@@ -367,6 +369,43 @@ __global__ void build_posb_kernel(float *posb, const __nv_bfloat16 *b, const __n
   else if (b) v = __bfloat162float(b[c]);
   if (pos) v += __bfloat162float(pos[idx]);
   posb[idx] = v;
+}
+
+// Patch embedding with a tiny patch (K_p = 8: the time-series backbones of cfg2 / cfg5): X[row, :] = A[row, :K_p] W_e^T + posb[pos(row)]
+// is a stream of 4 KB fp32 rows out for 16 bytes in - through the tensor-core GEMM it costs 512 epilogues of 256 KB for one
+// mostly-zero k-block each (measured 0.10 ms per step on cfg5); here a thread keeps the weights of its 4 columns in registers and
+// walks kEmbRows rows.  fp32 accumulation in k order.  grid (ceil(N / kEmbRows), d / 1024 rounded up), 256 threads.
+constexpr int kEmbRows = 16;
+__global__ void __launch_bounds__(256) embed_small_patch_kernel(const __nv_bfloat16 *__restrict__ A, const __nv_bfloat16 *__restrict__ Wpad,
+                                                                const float *__restrict__ posb, const int *__restrict__ row_pos, int N, int d,
+                                                                float *__restrict__ X) {
+  griddep_launch();
+  griddep_wait();
+  const int c = (blockIdx.y * 256 + threadIdx.x) * 4;
+  if (c >= d) return;
+  float w[4][8];
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const uint4 v = *reinterpret_cast<const uint4 *>(Wpad + (size_t)(c + j) * 8);
+    w[j][0] = bf16_lo(v.x); w[j][1] = bf16_hi(v.x); w[j][2] = bf16_lo(v.y); w[j][3] = bf16_hi(v.y);
+    w[j][4] = bf16_lo(v.z); w[j][5] = bf16_hi(v.z); w[j][6] = bf16_lo(v.w); w[j][7] = bf16_hi(v.w);
+  }
+  const int r0 = blockIdx.x * kEmbRows, r1 = min(N, r0 + kEmbRows);
+#pragma unroll 4
+  for (int r = r0; r < r1; ++r) {
+    const uint4 av = *reinterpret_cast<const uint4 *>(A + (size_t)r * 8);
+    const float x[8] = {bf16_lo(av.x), bf16_hi(av.x), bf16_lo(av.y), bf16_hi(av.y), bf16_lo(av.z), bf16_hi(av.z), bf16_lo(av.w), bf16_hi(av.w)};
+    const float4 pb = *reinterpret_cast<const float4 *>(posb + (size_t)row_pos[r] * d + c);
+    float o[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      float acc = 0.0f;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) acc = fmaf(x[k], w[j][k], acc);
+      o[j] = acc;
+    }
+    *reinterpret_cast<float4 *>(X + (size_t)r * d + c) = make_float4(o[0] + pb.x, o[1] + pb.y, o[2] + pb.z, o[3] + pb.w);
+  }
 }
 
 // W_e [d, patch_dim] -> [d, Kp] zero padded (row stride must be a multiple of 16 B for TMA)
