@@ -76,8 +76,7 @@ __device__ __forceinline__ void chunk_source(const GemmParams &p, int c, int &s,
 // GeLU(x) = x * Phi(x), Phi(x) = 0.5 erfc(-x / sqrt 2), with erfc(z) = 2^(-z Q(z)) for z >= 0, Q a quartic fitted (minimax
 // on |erf error|, fp32 evaluation) to -log2(erfc z) / z on [0, 4.2]: |error| <= 6.7e-7 in erf, |error| <= 1.4e-6 in GeLU over
 // [-12, 12], far below the bf16 rounding of the output; beyond the fit range the quartic keeps growing, so erfc -> 0.  The
-// 1/sqrt(2) is folded into the coefficients (in |x|).  Phi is formed without cancellation on either side: x < 0: 0.5 E;
-// x >= 0: 1 - 0.5 E.  One MUFU op (ex2) and 4 FMAs per element: the GeLU epilogue of the FFN-in GEMM was issue-bound with
+// 1/sqrt(2) is folded into the coefficients (in |x|).  One MUFU op (ex2) and 4 FMAs per element: the GeLU epilogue of the FFN-in GEMM was issue-bound with
 // erff (~30 instructions) and still the slower side with the Abramowitz-Stegun 7.1.26 form (rcp + ex2 + 10 FMA-pipe ops).
 __device__ __forceinline__ float gelu_erf_f(float x) {
   const float ax = fabsf(x);
@@ -87,8 +86,9 @@ __device__ __forceinline__ float gelu_erf_f(float x) {
   p = fmaf(p, ax, -1.15109488f);
   float e;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(p * ax));
-  const float h = 0.5f * e;
-  return x * (x < 0.0f ? h : 1.0f - h);
+  // x Phi(x) = x (1 - E / 2) for x >= 0 and x E / 2 for x < 0, i.e. max(x, 0) - |x| E / 2 on both sides: three operations instead of
+  // the five of scale / subtract / compare / select / multiply (the FFN-in epilogue of the GeLU backbones is issue-bound)
+  return fmaf(ax * e, -0.5f, fmaxf(x, 0.0f));
 }
 // silu(x) = x / (1 + e^-x) with ex2.approx and rcp.approx (2 MUFU ops, 3 FMA-pipe ops; an IEEE division is ~10 more).
 // Very negative finite x: e^-x overflows to +inf, rcp gives 0, the product is -0 (the limit); relative error ~2^-22, far below
