@@ -1372,11 +1372,13 @@ static int forward_impl(fmx_ctx *c, Backbone &bb, const void *inputs, const int3
 
   // Decode iterations (one row tile of <= 256 rows, a few rows per task).  The segmented tensor-core LoRA path would load a 256-row U
   // tile and a slab block per (tile, task) for a few rows of work, and a projection with few N tiles would be streamed by a handful
-  // of CTA pairs.  So in this mode (row_mode): (1) row_shrink_kernel + row_expand_kernel compute every row's LoRA delta on CUDA cores, (2) the GEMM runs
-  // without shrink / expand and stores raw fp32 partials, its K axis split over ~all CTA pairs when it has few tiles, (3)
-  // splitk_reduce_kernel adds the partials in split order, the delta and the bias and applies activation / SwiGLU / the residual
-  // update.  Every choice depends on the projection's shape only, never on the batch, so a request decodes to the same bits alone
-  // and in a batch.  (Prefill keeps the fused path: its outputs must not depend on the batch size.)
+  // of CTA pairs.  So in this mode (row_mode): (1) row_shrink_kernel + row_expand_kernel compute every row's LoRA delta on CUDA cores,
+  // on the auxiliary stream beside (2) the projection without shrink / expand, which stores raw fp32 partials of K slices:
+  // row_gemm_kernel for <= 128 rows, else the pair GEMM in partial-output mode with its K axis split over the CTA pairs; (3) a
+  // reduction adds the partials in split order, the delta and the bias and applies what follows (RoPE + cache append, SwiGLU /
+  // activation, residual update + the next norm).  Within each of the two size classes every choice depends on the projection's
+  // shape only, never on the batch, so a request decodes to the same bits alone and in a batch of its class.  (Prefill keeps the
+  // fused path: its outputs must not depend on the batch size.)
   const bool row_mode = kv && kv->decode && w.splitk && bb.row_bt && w.n_tiles == 1;
   // row mode fuses what follows a reduction into it: RoPE + the cache append after q / k / v, the next norm after a residual update
   const bool row_norm_fused = row_mode && d.d_model <= 4096;
