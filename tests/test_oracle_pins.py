@@ -371,3 +371,22 @@ def test_relative_position_buckets_by_hand():
     tab = np.arange(32 * 2, dtype=np.float64).reshape(32, 2)
     m = rel_bias_matrix(tab, 4, True, 32, 128)
     assert m.shape == (2, 4, 4) and m[1, 0, 0] == tab[0, 1] and m[0, 2, 0] == tab[2, 0] and m[0, 0, 3] == tab[19, 0]
+
+
+def test_relative_bias_workload_variant_reaches_the_oracle():
+    """The generator's rel_bias variant (reading 36): the table is part of the backbone's tensors, the oracle's forward
+    uses it (outputs change), and a zero table gives the plain backbone back exactly."""
+    from fmx_workloads import make_workload
+    from oracle import from_workload as G
+    wl = make_workload("cfg2", n_layers=1, batch=3, rel_bias=True)
+    assert wl.bb.rel_buckets == 32 and wl.bb.rel_max_distance == 128 and "rel_bias.W" in wl.backbone_tensor_names()
+    assert wl.tensor("rel_bias.W").shape == (32, wl.bb.n_q_heads)
+    with_bias = G.oracle_outputs(wl)
+    plain = G.oracle_outputs(make_workload("cfg2", n_layers=1, batch=3))
+    assert max(float(np.abs(a - b).max()) for a, b in zip(with_bias, plain)) > 1e-3
+    bb, get, tasks = G.bb_dict(wl), G.make_get(wl), G.task_dicts(wl)
+    zero = lambda name: np.zeros((32, wl.bb.n_q_heads)) if name == "rel_bias.W" else get(name)
+    x = O.tokens_from_input(bb, get, wl.request_input(0), tasks[int(wl.task_ids[0])])
+    a = O.layer_forward(bb, zero, tasks[int(wl.task_ids[0])], 0, x)
+    b = O.layer_forward({**bb, "rel_buckets": 0}, get, tasks[int(wl.task_ids[0])], 0, x)
+    assert np.array_equal(a, b)
