@@ -60,19 +60,28 @@ __global__ void __launch_bounds__(256) row_gemm_kernel(const RowGemmArgs a) {
   }
   const int nK = (a.K + kRgBK - 1) / kRgBK;
   const int kb0 = ks * a.chunks_per_split, kb1 = min(nK, kb0 + a.chunks_per_split);
+  // the thread's copies of a chunk are the same (row, 16-byte piece) pairs every time: their source pointers and shared-memory
+  // offsets are computed once, a chunk then costs one add and one cp.async per copy
+  constexpr int kCopies = ((kRowsX + kRgCols) * 8 + 255) / 256;
+  const __nv_bfloat16 *src[kCopies];
+  int sdst[kCopies], pc8[kCopies];                              // pc8 < 0: no copy / zero row
+#pragma unroll
+  for (int c = 0; c < kCopies; ++c) {
+    const int idx = threadIdx.x + c * 256, row = idx >> 3, pc = idx & 7;
+    sdst[c] = row * kRgLd + pc * 8;
+    pc8[c] = pc * 8;
+    if (idx >= (kRowsX + kRgCols) * 8) { pc8[c] = -1; src[c] = a.x; sdst[c] = 0; }
+    else if (row < kRowsX) { src[c] = a.x + (size_t)(row < a.M ? row : 0) * a.K + pc * 8; if (row >= a.M) pc8[c] = -2; }
+    else src[c] = Wp + (size_t)(row - kRowsX) * a.K + pc * 8;
+  }
   auto load_stage = [&](int kb, int stage) {
-    __nv_bfloat16 *sx = smem + (size_t)stage * kStageElems, *sw = sx + kRowsX * kRgLd;
+    __nv_bfloat16 *sbase = smem + (size_t)stage * kStageElems;
     const int k0 = kb * kRgBK;
-    for (int idx = threadIdx.x; idx < (kRowsX + kRgCols) * 8; idx += 256) {
-      const int row = idx >> 3, pc = idx & 7;
-      const bool kin = k0 + pc * 8 < a.K;                       // K is a multiple of 8
-      if (row < kRowsX) {
-        const bool ok = row < a.M && kin;
-        cp_async_16(sx + row * kRgLd + pc * 8, a.x + (size_t)(ok ? row : 0) * a.K + (ok ? k0 + pc * 8 : 0), ok ? 16 : 0);
-      } else {
-        const int n = row - kRowsX;
-        cp_async_16(sw + n * kRgLd + pc * 8, Wp + (size_t)n * a.K + (kin ? k0 + pc * 8 : 0), kin ? 16 : 0);
-      }
+#pragma unroll
+    for (int c = 0; c < kCopies; ++c) {
+      if (pc8[c] == -1) continue;
+      const bool ok = pc8[c] >= 0 && k0 + pc8[c] < a.K;         // (K is a multiple of 8; rows past M and the K tail are zero-filled)
+      cp_async_16(sbase + sdst[c], src[c] + (ok ? k0 : 0), ok ? 16 : 0);
     }
   };
   float acc[MT][2][4];
